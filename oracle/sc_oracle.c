@@ -1,0 +1,395 @@
+/*
+ * sc_oracle.c -- CPU ORACLE (TEST INFRASTRUCTURE, NOT THE PRODUCT).  See sc_oracle.h for scope and pins.
+ *
+ * Everything is evaluated directly at every FFT bin in plain FP64, in the order the paper / SURVEY.md 8(c)
+ * states it: no interpolation, no blocking, no fusion.  Build: gcc -O2 -ffp-contract=off -fopenmp.
+ *
+ * Citations: PAPER.md:<line> = /root/reference/PAPER.md; "O1..O7" and "Q1..Q17" = SURVEY.md section 8(c) readings
+ * (listed again in DESIGN.md), used where the paper names a model but prints no formula.
+ */
+#include "sc_oracle.h"
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define SCO_PI      3.141592653589793238462643383279502884
+#define SCO_EULER   0.577215664901532860606512090082402431
+#define SCO_MSUN_S  4.925491025543576e-06   /* G Msun / c^3 in seconds (O2) */
+
+/* ------------------------------------------------------------------------------------------------
+ * O2 -- phase.  PAPER.md:219 names "TaylorF2Ecc" [49] and prints no formula; the reading is the textbook
+ * non-spinning TaylorF2 stationary-phase phase to 3.5PN plus the leading-order e0^2 term:
+ *   v = (pi M f)^(1/3),  M = M_c eta^(-3/5)
+ *   Psi(f) = 2 pi f t_c - phi_c - pi/4 + 3/(128 eta) v^-5 sum_{k=0}^{7} psi_k v^k ,   phi_c = 0.
+ * ------------------------------------------------------------------------------------------------ */
+static int theta_valid(const double th[8]) {
+  for (int i = 0; i < 8; ++i) if (!isfinite(th[i])) return 0;
+  if (!(th[0] > 0.0)) return 0;
+  if (!(th[1] > 0.0 && th[1] <= 0.25)) return 0;
+  return 1;
+}
+
+/* psi_k(eta, v) for k = 0..7 (psi_5 and psi_6 carry ln v). */
+static void pn_coeffs(double eta, double v, double psi[8]) {
+  const double pi = SCO_PI, eta2 = eta * eta, eta3 = eta2 * eta;
+  psi[0] = 1.0;
+  psi[1] = 0.0;
+  psi[2] = 3715.0 / 756.0 + 55.0 * eta / 9.0;
+  psi[3] = -16.0 * pi;
+  psi[4] = 15293365.0 / 508032.0 + 27145.0 * eta / 504.0 + 3085.0 * eta2 / 72.0;
+  psi[5] = pi * (38645.0 / 756.0 - 65.0 * eta / 9.0) * (1.0 + 3.0 * log(v));
+  psi[6] = 11583231236531.0 / 4694215680.0 - 640.0 * pi * pi / 3.0 - 6848.0 * SCO_EULER / 21.0
+           - (6848.0 / 21.0) * log(4.0 * v)
+           + (-15737765635.0 / 3048192.0 + 2255.0 * pi * pi / 12.0) * eta
+           + 76055.0 * eta2 / 1728.0 - 127825.0 * eta3 / 1296.0;
+  psi[7] = pi * (77096675.0 / 254016.0 + 378515.0 * eta / 1512.0 - 74045.0 * eta2 / 756.0);
+}
+
+double sco_phase(const sco_config* c, const double th[8], double f) {
+  const double pi = SCO_PI;
+  const double Mc = th[0] * SCO_MSUN_S, eta = th[1], tc = th[2], e0 = th[7];
+  const double M = Mc * pow(eta, -0.6);
+  const double v = cbrt(pi * M * f);
+  double psi[8];
+  pn_coeffs(eta, v, psi);
+  double sum = 0.0;
+  for (int k = 0; k <= c->pn_order_x2 && k <= 7; ++k) sum += psi[k] * pow(v, (double)(k - 5));
+  double Psi = 2.0 * pi * f * tc - pi / 4.0 + 3.0 / (128.0 * eta) * sum;
+  if (c->ecc_leading) {
+    /* Q5: Delta Psi = -(3/(128 eta)) v^-5 (2355/1462) e0^2 (v_ref/v)^(19/3) */
+    const double vref = cbrt(pi * M * c->f_ref_ecc);
+    Psi += -3.0 / (128.0 * eta) * pow(v, -5.0) * (2355.0 / 1462.0) * e0 * e0 * pow(vref / v, 19.0 / 3.0);
+  }
+  return Psi;
+}
+
+/* O3 -- t(f) = (1/2pi) dPsi/df, term by term with dv/df = v/(3f):
+ *   d/df[psi_k v^(k-5)] = (k-5) psi_k v^(k-5)/(3f)           (k != 5, 6)
+ *   d/df[psi_5]         = P5 * 3 * (1/(3f)),   P5 = pi(38645/756 - 65 eta/9)
+ *   d/df[psi_6 v]       = (psi_6 - 6848/21) v/(3f)
+ * Newtonian limit: t_c - t(f) = (5/256) M_c^(-5/3) (pi f)^(-8/3). */
+double sco_tf(const sco_config* c, const double th[8], double f) {
+  const double pi = SCO_PI;
+  const double Mc = th[0] * SCO_MSUN_S, eta = th[1], tc = th[2], e0 = th[7];
+  const double M = Mc * pow(eta, -0.6);
+  const double v = cbrt(pi * M * f);
+  double psi[8];
+  pn_coeffs(eta, v, psi);
+  double sum = 0.0;
+  for (int k = 0; k <= c->pn_order_x2 && k <= 7; ++k) {
+    if (k == 5) sum += 3.0 * pi * (38645.0 / 756.0 - 65.0 * eta / 9.0);
+    else if (k == 6) sum += (psi[6] - 6848.0 / 21.0) * v;
+    else sum += (double)(k - 5) * psi[k] * pow(v, (double)(k - 5));
+  }
+  double dPsi = 2.0 * pi * tc + 3.0 / (128.0 * eta) * sum / (3.0 * f);
+  if (c->ecc_leading) {
+    /* the eccentric term scales as f^(-34/9) */
+    const double vref = cbrt(pi * M * c->f_ref_ecc);
+    const double dPsi_e = -3.0 / (128.0 * eta) * pow(v, -5.0) * (2355.0 / 1462.0) * e0 * e0 * pow(vref / v, 19.0 / 3.0);
+    dPsi += dPsi_e * (-34.0 / 9.0) / f;
+  }
+  return dPsi / (2.0 * pi);
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * O4 -- orbits and response.  PAPER.md:233-241 (Eq. 16) cites the BBHx implementation of [56] and prints
+ * no formula; the reading is the leading-order frequency-domain response with the orbit frozen at t_f.
+ * Equal-arm orbits to first order in e = L/(2 sqrt3 AU) (Q6); positions in light-seconds.
+ * ------------------------------------------------------------------------------------------------ */
+void sco_orbit(const sco_config* c, double t, double p[4][3]) {
+  const double pi = SCO_PI;
+  const double AU = c->au_s, L = c->arm_L_s;
+  const double e = L / (2.0 * sqrt(3.0) * AU);
+  const double alpha = 2.0 * pi * t / c->year_s + c->orbit_alpha0;
+  const double sa = sin(alpha), ca = cos(alpha);
+  p[0][0] = AU * ca; p[0][1] = AU * sa; p[0][2] = 0.0;
+  for (int n = 1; n <= 3; ++n) {
+    const double bn = 2.0 * pi * (double)(n - 1) / 3.0 + c->orbit_lambda0;
+    const double sb = sin(bn), cb = cos(bn);
+    p[n][0] = p[0][0] + AU * e * (sa * ca * sb - (1.0 + sa * sa) * cb);
+    p[n][1] = p[0][1] + AU * e * (sa * ca * cb - (1.0 + ca * ca) * sb);
+    p[n][2] = -sqrt(3.0) * AU * e * cos(alpha - bn);
+  }
+}
+
+static double dot3(const double a[3], const double b[3]) { return a[0] * b[0] + a[1] * b[1] + a[2] * b[2]; }
+
+/* sky basis (O4): n_hat source direction, k = -n_hat propagation, (u, v, k) right-handed (Q17). */
+static void sky_basis(const double th[8], double k[3], double u[3], double v[3]) {
+  const double lam = th[3], bet = th[4];
+  const double cl = cos(lam), sl = sin(lam), cb = cos(bet), sb = sin(bet);
+  k[0] = -cb * cl; k[1] = -cb * sl; k[2] = -sb;
+  u[0] = -sb * cl; u[1] = -sb * sl; u[2] = cb;
+  v[0] = -sl;      v[1] = cl;       v[2] = 0.0;
+}
+
+/* single link s->r given the orbit p[][] (at t_f) and the sky basis */
+static void link_core(const sco_config* c, const double th[8], double f, double p[4][3],
+                      const double k[3], const double u[3], const double v[3], int s, int r, double out[2]) {
+  const double pi = SCO_PI, L = c->arm_L_s;
+  const double iota = th[5], pol = th[6];
+  double n[3];
+  for (int i = 0; i < 3; ++i) n[i] = p[r][i] - p[s][i];
+  const double nn = sqrt(dot3(n, n));
+  for (int i = 0; i < 3; ++i) n[i] /= nn;
+  /* polarisation: e+ = u(x)u - v(x)v, ex = u(x)v + v(x)u; eps+ = cos2psi e+ + sin2psi ex, epsx = -sin2psi e+ + cos2psi ex */
+  const double nu = dot3(n, u), nv = dot3(n, v);
+  const double nep = nu * nu - nv * nv, nex = 2.0 * nu * nv;
+  const double c2 = cos(2.0 * pol), s2 = sin(2.0 * pol);
+  const double Fp = c2 * nep + s2 * nex, Fx = -s2 * nep + c2 * nex;
+  /* zeta_sr = (1+cos^2 iota)/2 (n.eps+.n) - i cos(iota) (n.epsx.n)   [h+ = (1+cos^2 i)/2 A e^-iPsi, hx = -i cos i A e^-iPsi] */
+  const double ci = cos(iota);
+  const double zr = 0.5 * (1.0 + ci * ci) * Fp, zi = -ci * Fx;
+  /* y_sr = -i pi f L sinc[pi f L (1 - k.n)] exp[-i pi f (L + k.(p_r + p_s))] zeta */
+  const double kn = dot3(k, n);
+  const double x = pi * f * L * (1.0 - kn);
+  const double sinc = (x == 0.0) ? 1.0 : sin(x) / x;
+  double prs[3];
+  for (int i = 0; i < 3; ++i) prs[i] = p[r][i] + p[s][i];
+  const double ph = -pi * f * (L + dot3(k, prs));
+  const double er = cos(ph), ei = sin(ph);
+  /* (-i a)(er + i ei)(zr + i zi), a = pi f L sinc */
+  const double a = pi * f * L * sinc;
+  const double wr = er * zr - ei * zi, wi = er * zi + ei * zr;   /* e * zeta */
+  out[0] = a * wi;      /* -i (wr + i wi) = wi - i wr */
+  out[1] = -a * wr;
+}
+
+void sco_link(const sco_config* c, const double th[8], double f, double t, int s, int r, double out[2]) {
+  double p[4][3], k[3], u[3], v[3];
+  sco_orbit(c, t, p);
+  sky_basis(th, k, u, v);
+  link_core(c, th, f, p, k, u, v, s, r, out);
+}
+
+void sco_tdi(const sco_config* c, const double th[8], double f, double t, double out[6][2]) {
+  const double pi = SCO_PI, L = c->arm_L_s;
+  /* y[s][r], 1-based */
+  double y[4][4][2], p[4][3], k[3], u[3], v[3];
+  sco_orbit(c, t, p);
+  sky_basis(th, k, u, v);
+  for (int s = 1; s <= 3; ++s)
+    for (int r = 1; r <= 3; ++r)
+      if (s != r) link_core(c, th, f, p, k, u, v, s, r, y[s][r]);
+  const double Dr = cos(2.0 * pi * f * L), Di = -sin(2.0 * pi * f * L);   /* D = e^{-2 pi i f L} */
+  const double D2r = Dr * Dr - Di * Di, D2i = 2.0 * Dr * Di;
+  const double gr = 1.0 - D2r, gi = -D2i;                                 /* 1 - D^2 */
+  /* TDI 1st generation (Q6): X = (1-D^2)[(y31 + D y13) - (y21 + D y12)], Y and Z by cyclic 1->2->3->1 */
+  double XYZ[3][2];
+  for (int m = 0; m < 3; ++m) {
+    const int a = 1 + m % 3, b = 1 + (m + 1) % 3, cc = 1 + (m + 2) % 3;   /* (a,b,c) = (1,2,3),(2,3,1),(3,1,2) */
+    /* [(y_ca + D y_ac) - (y_ba + D y_ab)] */
+    const double tr = (y[cc][a][0] + Dr * y[a][cc][0] - Di * y[a][cc][1]) - (y[b][a][0] + Dr * y[a][b][0] - Di * y[a][b][1]);
+    const double ti = (y[cc][a][1] + Dr * y[a][cc][1] + Di * y[a][cc][0]) - (y[b][a][1] + Dr * y[a][b][1] + Di * y[a][b][0]);
+    XYZ[m][0] = gr * tr - gi * ti;
+    XYZ[m][1] = gr * ti + gi * tr;
+  }
+  for (int q = 0; q < 2; ++q) {
+    const double X = XYZ[0][q], Y = XYZ[1][q], Z = XYZ[2][q];
+    out[0][q] = X; out[1][q] = Y; out[2][q] = Z;
+    out[3][q] = (Z - X) / sqrt(2.0);                 /* A */
+    out[4][q] = (X - 2.0 * Y + Z) / sqrt(6.0);       /* E */
+    out[5][q] = (X + Y + Z) / sqrt(3.0);             /* T */
+  }
+}
+
+/* O2+O3+O4: h_alpha(f_j) = T_alpha(theta, f_j; t_f) * f^(-7/6) * e^{-i Psi(f_j)}  (Eq. 16),
+ * zero outside the time window 0 <= t(f_j) <= T_obs when window_mode = 1 (Q4). */
+int64_t sco_template(const sco_config* c, const double th[8], int64_t j_begin, int64_t n, double* hA, double* hE) {
+  memset(hA, 0, (size_t)n * 2 * sizeof(double));
+  if (hE) memset(hE, 0, (size_t)n * 2 * sizeof(double));
+  if (!theta_valid(th)) return 0;
+  int64_t inwin = 0;
+  for (int64_t i = 0; i < n; ++i) {
+    const double f = (double)(c->j0 + j_begin + i) / c->T_obs_s;
+    const double t = sco_tf(c, th, f);
+    if (c->window_mode == 1 && !(t >= 0.0 && t <= c->T_obs_s)) continue;
+    ++inwin;
+    const double Psi = sco_phase(c, th, f);
+    const double amp = pow(f, -7.0 / 6.0);
+    double tdi[6][2];
+    sco_tdi(c, th, f, t, tdi);
+    const double er = amp * cos(Psi), ei = -amp * sin(Psi);      /* A e^{-i Psi} */
+    hA[2 * i]     = tdi[3][0] * er - tdi[3][1] * ei;
+    hA[2 * i + 1] = tdi[3][0] * ei + tdi[3][1] * er;
+    if (hE) {
+      hE[2 * i]     = tdi[4][0] * er - tdi[4][1] * ei;
+      hE[2 * i + 1] = tdi[4][0] * ei + tdi[4][1] * er;
+    }
+  }
+  return inwin;
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * O1 -- statistic core.  Eq. 7: [a|b]_n = sum_alpha 4 Re int_{f_n}^{f_n+1} a b^dagger / S df,
+ * evaluated as a Riemann sum over FFT bins (Q7: half-open segments, no end-point weights).
+ * Eq. 10: x_n = max_phi [d | h e^{i phi}]_n = 4 df |z_n| with ONE complex z_n summed over
+ * channels (Q1);  [h|h]_n = 4 df sigma_n;  Upsilon_N = sum_n x_n^2/[h|h]_n = 4 df sum_n |z_n|^2/sigma_n.
+ * Segments with sigma_n = 0 contribute 0 (Q8).
+ * ------------------------------------------------------------------------------------------------ */
+double sco_stat_from_arrays(const double* dA, const double* dE, const double* hA, const double* hE,
+                            const double* SA, const double* SE, double df,
+                            const int64_t* edges, int64_t n_seg, double* out_seg) {
+  double ups = 0.0;
+  for (int64_t k = 0; k < n_seg; ++k) {
+    double zr = 0.0, zi = 0.0, sig = 0.0;
+    for (int64_t j = edges[k]; j < edges[k + 1]; ++j) {
+      /* d conj(h) / S */
+      zr += (dA[2 * j] * hA[2 * j] + dA[2 * j + 1] * hA[2 * j + 1]) / SA[j];
+      zi += (dA[2 * j + 1] * hA[2 * j] - dA[2 * j] * hA[2 * j + 1]) / SA[j];
+      sig += (hA[2 * j] * hA[2 * j] + hA[2 * j + 1] * hA[2 * j + 1]) / SA[j];
+      if (dE && hE && SE) {
+        zr += (dE[2 * j] * hE[2 * j] + dE[2 * j + 1] * hE[2 * j + 1]) / SE[j];
+        zi += (dE[2 * j + 1] * hE[2 * j] - dE[2 * j] * hE[2 * j + 1]) / SE[j];
+        sig += (hE[2 * j] * hE[2 * j] + hE[2 * j + 1] * hE[2 * j + 1]) / SE[j];
+      }
+    }
+    if (out_seg) { out_seg[3 * k] = zr; out_seg[3 * k + 1] = zi; out_seg[3 * k + 2] = sig; }
+    if (sig > 0.0) {
+      const double x = 4.0 * df * sqrt(zr * zr + zi * zi);     /* x_n, Eq. 10 */
+      const double hh = 4.0 * df * sig;                        /* [h|h]_n */
+      ups += x * x / hh;
+    }
+  }
+  return ups;
+}
+
+/* Eq. 1: <a|b> = sum_alpha 4 Re sum_j a b^dagger / S df. */
+double sco_inner(const double* aA, const double* aE, const double* bA, const double* bE,
+                 const double* SA, const double* SE, double df, int64_t n) {
+  double acc = 0.0;
+  for (int64_t j = 0; j < n; ++j) {
+    acc += (aA[2 * j] * bA[2 * j] + aA[2 * j + 1] * bA[2 * j + 1]) / SA[j];
+    if (aE && bE && SE) acc += (aE[2 * j] * bE[2 * j] + aE[2 * j + 1] * bE[2 * j + 1]) / SE[j];
+  }
+  return 4.0 * df * acc;
+}
+
+int sco_num_threads(void) {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+
+void sco_eval_stat_levels(const sco_config* c, const double* dA, const double* dE, const double* SA, const double* SE,
+                          const double* params, int64_t P, const int64_t* edges_cat, const int64_t* n_segs,
+                          int64_t n_levels, double* out) {
+  const int64_t n = c->n_bins;
+  const double df = 1.0 / c->T_obs_s;
+  const int two = (c->n_channels >= 2);
+#pragma omp parallel
+  {
+    double* hA = (double*)malloc((size_t)n * 2 * sizeof(double));
+    double* hE = (double*)malloc((size_t)n * 2 * sizeof(double));
+#pragma omp for schedule(dynamic, 1)
+    for (int64_t p = 0; p < P; ++p) {
+      sco_template(c, params + 8 * p, 0, n, hA, two ? hE : NULL);
+      const int64_t* e = edges_cat;
+      for (int64_t l = 0; l < n_levels; ++l) {
+        out[l * P + p] = sco_stat_from_arrays(dA, two ? dE : NULL, hA, two ? hE : NULL, SA, two ? SE : NULL, df, e, n_segs[l], NULL);
+        e += n_segs[l] + 1;
+      }
+    }
+    free(hA); free(hE);
+  }
+}
+
+void sco_eval_stat(const sco_config* c, const double* dA, const double* dE, const double* SA, const double* SE,
+                   const double* params, int64_t P, const int64_t* edges, int64_t n_seg,
+                   double* out, double* out_seg, int64_t* n_inwin) {
+  const int64_t n = c->n_bins;
+  const double df = 1.0 / c->T_obs_s;
+  const int two = (c->n_channels >= 2);
+#pragma omp parallel
+  {
+    double* hA = (double*)malloc((size_t)n * 2 * sizeof(double));
+    double* hE = (double*)malloc((size_t)n * 2 * sizeof(double));
+#pragma omp for schedule(dynamic, 1)
+    for (int64_t p = 0; p < P; ++p) {
+      const int64_t w = sco_template(c, params + 8 * p, 0, n, hA, two ? hE : NULL);
+      if (n_inwin) n_inwin[p] = w;
+      out[p] = sco_stat_from_arrays(dA, two ? dE : NULL, hA, two ? hE : NULL, SA, two ? SE : NULL, df, edges, n_seg,
+                                    out_seg ? out_seg + (size_t)p * (size_t)n_seg * 3 : NULL);
+    }
+    free(hA); free(hE);
+  }
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * Q10 -- Philox4x32-10, restated from the published algorithm (Salmon et al., SC'11).
+ * ------------------------------------------------------------------------------------------------ */
+void sco_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
+  uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3], k0 = key[0], k1 = key[1];
+  for (int round = 0; round < 10; ++round) {
+    const uint64_t p0 = (uint64_t)0xD2511F53u * c0, p1 = (uint64_t)0xCD9E8D57u * c2;
+    const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0, n1 = (uint32_t)p1;
+    const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1, n3 = (uint32_t)p0;
+    c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+    k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+  }
+  out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+void sco_pso_uniforms(uint64_t seed, uint64_t particle, uint64_t iter, double rP[8], double rG[8]) {
+  const uint32_t key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)};
+  uint32_t w[16];
+  for (uint32_t b = 0; b < 4; ++b) {
+    const uint32_t ctr[4] = {(uint32_t)particle, (uint32_t)iter, b, 0u};
+    sco_philox4x32_10(ctr, key, w + 4 * b);
+  }
+  for (int m = 0; m < 8; ++m) {
+    rP[m] = ((double)w[m] + 0.5) * 0x1p-32;
+    rG[m] = ((double)w[8 + m] + 0.5) * 0x1p-32;
+  }
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * O7 -- one synchronous PSO step.  Eq. 14, Eq. 15, Eq. 13;
+ * bests use iteration i-1 quantities; reflecting boundary and sign(0) = +1 per Q9.
+ * Swarms are n_swarms equal contiguous blocks of particles.
+ * ------------------------------------------------------------------------------------------------ */
+void sco_pso_step(double* pos, double* vel, double* pbest_pos, double* pbest_val, const double* stat,
+                  double* gbest_pos, double* gbest_val, const double* lo, const double* hi, const double* eps_min,
+                  double omega, double phi_p, double phi_g, uint64_t seed, uint64_t iter,
+                  int64_t P, int32_t n_swarms) {
+  /* (1) personal bests: strict improvement */
+  for (int64_t p = 0; p < P; ++p)
+    if (stat[p] > pbest_val[p]) {
+      pbest_val[p] = stat[p];
+      for (int m = 0; m < 8; ++m) pbest_pos[8 * p + m] = pos[8 * p + m];
+    }
+  /* (2) swarm bests: arg max of the personal bests, lowest index on ties */
+  const int64_t per = P / n_swarms;
+  for (int32_t s = 0; s < n_swarms; ++s) {
+    int64_t best = (int64_t)s * per;
+    for (int64_t p = best + 1; p < (int64_t)(s + 1) * per; ++p)
+      if (pbest_val[p] > pbest_val[best]) best = p;
+    gbest_val[s] = pbest_val[best];
+    for (int m = 0; m < 8; ++m) gbest_pos[8 * s + m] = pbest_pos[8 * best + m];
+  }
+  /* (3)-(6) */
+  for (int64_t p = 0; p < P; ++p) {
+    const int32_t s = (int32_t)(p / per);
+    double rP[8], rG[8];
+    sco_pso_uniforms(seed, (uint64_t)p, iter, rP, rG);
+    for (int m = 0; m < 8; ++m) {
+      const double th = pos[8 * p + m];
+      const double u = omega * vel[8 * p + m] + phi_p * rP[m] * (pbest_pos[8 * p + m] - th)
+                       + phi_g * rG[m] * (gbest_pos[8 * s + m] - th);                         /* Eq. 14 */
+      const double au = fabs(u), eps = eps_min[m];
+      double v;
+      if (au > 0.0) v = (eps > au ? eps : au) * (u / au);                                     /* Eq. 15 */
+      else v = (eps > 0.0) ? eps : 0.0;                                                       /* Q9: sign(0) = +1 */
+      double x = th + v;                                                                      /* Eq. 13 */
+      if (x < lo[m]) { x = lo[m]; v = -v; }                                                   /* Q9: reflect */
+      else if (x > hi[m]) { x = hi[m]; v = -v; }
+      pos[8 * p + m] = x;
+      vel[8 * p + m] = v;
+    }
+  }
+}

@@ -1,0 +1,102 @@
+/*
+ * sc_oracle.h -- CPU ORACLE for the semi-coherent statistic (TEST INFRASTRUCTURE, NOT THE PRODUCT).
+ *
+ * Plain, slow, double-precision, direct evaluation of what the hot path of
+ * arxiv 2408.13170 (Bandopadhyay & Moore) computes.  Written from the paper text
+ * (/root/reference/PAPER.md, cited as PAPER.md:<line>) and from the readings of
+ * SURVEY.md section 8(c) (cited as O1..O7, Q1..Q17) where the paper prints no formula.
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+ * legs may use anything in this directory.  It shares no code with the CUDA path under
+ * paper_2408_13170_b200/ and neither includes the other.
+ *
+ * Parity pins (tests/test_oracle_*.py, all `-m "not gpu"`):
+ *   sco_stat_from_arrays : brute-force phase-grid maximisation of Eq. 7/10 on tiny grids; d=h identities;
+ *                          phase/rescale invariance; refinement monotonicity; Cauchy-Schwarz; impulse indexing;
+ *                          Monte-Carlo moments of Eq. 11-12.
+ *   sco_phase / sco_tf   : Newtonian closed form; Table I / III t_c values;
+ *                          finite-difference identity t(f) = Psi'(f)/2pi in long double; cycle count.
+ *                          PARITY WITH LALSimulation / TaylorF2Ecc [49] IS UNPINNED (not in the container).
+ *   sco_orbit/sco_template: arm lengths = L, centroid on the 1-AU circle; two-pulse single-link identity;
+ *                          long-wavelength Michelson limit; T-combination -> 0; beta = +-pi/2 kills the Doppler term.
+ *                          PARITY WITH BBHx [56] IS UNPINNED (not in the container).
+ *   sco_philox4x32_10    : known-answer vectors of the published algorithm (Salmon et al. 2011), moments.
+ *   sco_pso_step         : hand-computed one-particle examples of Eq. 14 -> 15 -> 13.
+ */
+#ifndef SC_ORACLE_H
+#define SC_ORACLE_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* Field-for-field the same information the product's config carries; declared independently. */
+typedef struct {
+  double  T_obs_s;        /* observation time; df = 1/T_obs                   */
+  int64_t j0;             /* f_j = (j0 + j)/T_obs_s                                          */
+  int64_t n_bins;
+  int32_t n_channels;     /* 2 = A,E  (Q16)                                                  */
+  int32_t window_mode;    /* 1 = h(f)=0 where t(f) outside [0,T_obs]  (Q4)                   */
+  int32_t pn_order_x2;    /* highest PN term kept in the phase sum, 7 = 3.5PN (O2)           */
+  int32_t ecc_leading;    /* 1 = leading-order e0^2 phase term (Q5)                          */
+  double  f_ref_ecc;      /* GW frequency at which e0 is defined                             */
+  double  arm_L_s, au_s, orbit_alpha0, orbit_lambda0, year_s;   /* orbit constants (Q6)      */
+} sco_config;
+
+/* theta = (M_c [Msun, detector frame], eta, t_c [s from data start], lambda, beta, iota, psi, e_0)  (D3, Q3) */
+
+/* O2: stationary-phase TaylorF2 phase Psi(f) [rad], h ~ A e^{-i Psi}. */
+double sco_phase(const sco_config* c, const double theta[8], double f);
+/* O3: t(f) = Psi'(f)/(2 pi) [s], analytic term-by-term derivative of O2. */
+double sco_tf(const sco_config* c, const double theta[8], double f);
+/* O4: spacecraft positions p[0]=centroid p0, p[1..3]=spacecraft 1..3, in light-seconds, at time t [s]. */
+void sco_orbit(const sco_config* c, double t, double p[4][3]);
+/* O4: single-link response y_sr(f) for link s->r (1-based), WITHOUT the factor A(f) e^{-i Psi(f)}:
+ * out = -i pi f L sinc[pi f L (1 - k.n_sr)] exp[-i pi f (L + k.(p_r+p_s))] zeta_sr ; orbit evaluated at time t. */
+void sco_link(const sco_config* c, const double theta[8], double f, double t, int s, int r, double out_ri[2]);
+/* O4: TDI transfer functions (X,Y,Z,A,E,T)(f) at orbit time t, without A(f) e^{-i Psi}; out_ri[6][2]. */
+void sco_tdi(const sco_config* c, const double theta[8], double f, double t, double out_ri[6][2]);
+/* O2+O3+O4 (+Q4 window): h_A, h_E on bins [j_begin, j_begin+n); interleaved re/im, n each.
+ * Returns the number of bins inside the time window. Invalid theta -> all zeros, returns 0. */
+int64_t sco_template(const sco_config* c, const double theta[8], int64_t j_begin, int64_t n,
+                     double* hA_ri, double* hE_ri);
+
+/* O1: Eq. 1/7/8/10 on arrays.  d,h interleaved re/im per channel (E pointers may be NULL for one channel),
+ * S one-sided PSD per bin, edges[n_seg+1] bin indices, df = 1/T_obs.
+ * out_seg (may be NULL) = [n_seg][3] = (Re z_k, Im z_k, sigma_k) with
+ *   z_k = sum_a sum_j d_a conj(h_a)/S_a ,  sigma_k = sum_a sum_j |h_a|^2/S_a ;
+ * returns Upsilon_N = 4 df sum_{k: sigma_k>0} |z_k|^2/sigma_k. */
+double sco_stat_from_arrays(const double* dA_ri, const double* dE_ri, const double* hA_ri, const double* hE_ri,
+                            const double* S_A, const double* S_E, double df,
+                            const int64_t* edges, int64_t n_seg, double* out_seg);
+/* Eq. 1 coherent inner product <a|b> over bins [0,n) (A3: rho^2 = <h|h>). */
+double sco_inner(const double* aA_ri, const double* aE_ri, const double* bA_ri, const double* bE_ri,
+                 const double* S_A, const double* S_E, double df, int64_t n);
+
+/* Whole-population statistic: for each particle, sco_template then sco_stat_from_arrays (OpenMP over particles).
+ * out[n_particles]; out_seg (may be NULL) [n_particles][n_seg][3]; n_inwin (may be NULL) [n_particles]. */
+void sco_eval_stat(const sco_config* c, const double* dA_ri, const double* dE_ri, const double* S_A, const double* S_E,
+                   const double* params, int64_t n_particles, const int64_t* edges, int64_t n_seg,
+                   double* out, double* out_seg, int64_t* n_inwin);
+/* Same templates, several edge lists at once (hierarchy levels): edges_cat = concatenated lists, n_segs[n_levels];
+ * out [n_levels][n_particles]. */
+void sco_eval_stat_levels(const sco_config* c, const double* dA_ri, const double* dE_ri, const double* S_A, const double* S_E,
+                          const double* params, int64_t n_particles, const int64_t* edges_cat, const int64_t* n_segs,
+                          int64_t n_levels, double* out);
+int sco_num_threads(void);
+
+/* Q10: Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11). */
+void sco_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
+/* Q10: the 16 uniforms of (seed, particle, iter): r_P[0..7], r_G[0..7], u = (word + 0.5) 2^-32. */
+void sco_pso_uniforms(uint64_t seed, uint64_t particle, uint64_t iter, double rP[8], double rG[8]);
+/* O7: one synchronous PSO step, Eq. 13-15 + best bookkeeping + reflecting boundary (Q9). */
+void sco_pso_step(double* pos, double* vel, double* pbest_pos, double* pbest_val, const double* stat,
+                  double* gbest_pos, double* gbest_val, const double* lo, const double* hi, const double* eps_min,
+                  double omega, double phi_p, double phi_g, uint64_t seed, uint64_t iter,
+                  int64_t n_particles, int32_t n_swarms);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,213 @@
+"""ctypes binding of the CPU ORACLE (oracle/sc_oracle.c).  TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import this.
+It shares no code with paper_2408_13170_b200/ and neither imports the other.
+Argument marshalling only: every number is computed by the C file beside it.
+"""
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "sc_oracle.c")
+_LIB = os.path.join(_HERE, "libsc_oracle.so")
+
+
+def build(force=False):
+    """Compile the oracle with gcc (plain FP64, no contraction, OpenMP over particles)."""
+    deps = [_SRC, os.path.join(_HERE, "sc_oracle.h")]
+    if (not force and os.path.exists(_LIB)
+            and all(os.path.getmtime(_LIB) >= os.path.getmtime(d) for d in deps)):
+        return _LIB
+    subprocess.check_call(["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared", "-Wall",
+                           "-o", _LIB, _SRC, "-lm"])
+    return _LIB
+
+
+class Config(C.Structure):
+    _fields_ = [("T_obs_s", C.c_double), ("j0", C.c_int64), ("n_bins", C.c_int64),
+                ("n_channels", C.c_int32), ("window_mode", C.c_int32), ("pn_order_x2", C.c_int32),
+                ("ecc_leading", C.c_int32), ("f_ref_ecc", C.c_double),
+                ("arm_L_s", C.c_double), ("au_s", C.c_double), ("orbit_alpha0", C.c_double),
+                ("orbit_lambda0", C.c_double), ("year_s", C.c_double)]
+
+
+def make_config(d):
+    """d: dict with the field names above (what sc_synth.grid_config returns)."""
+    c = Config()
+    for k, _ in Config._fields_:
+        setattr(c, k, d[k])
+    return c
+
+
+_lib = None
+_dp = C.POINTER(C.c_double)
+_ip = C.POINTER(C.c_int64)
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+        L = _lib
+        L.sco_phase.restype = C.c_double
+        L.sco_phase.argtypes = [C.POINTER(Config), _dp, C.c_double]
+        L.sco_tf.restype = C.c_double
+        L.sco_tf.argtypes = [C.POINTER(Config), _dp, C.c_double]
+        L.sco_orbit.argtypes = [C.POINTER(Config), C.c_double, _dp]
+        L.sco_link.argtypes = [C.POINTER(Config), _dp, C.c_double, C.c_double, C.c_int, C.c_int, _dp]
+        L.sco_tdi.argtypes = [C.POINTER(Config), _dp, C.c_double, C.c_double, _dp]
+        L.sco_template.restype = C.c_int64
+        L.sco_template.argtypes = [C.POINTER(Config), _dp, C.c_int64, C.c_int64, _dp, _dp]
+        L.sco_stat_from_arrays.restype = C.c_double
+        L.sco_stat_from_arrays.argtypes = [_dp, _dp, _dp, _dp, _dp, _dp, C.c_double, _ip, C.c_int64, _dp]
+        L.sco_inner.restype = C.c_double
+        L.sco_inner.argtypes = [_dp, _dp, _dp, _dp, _dp, _dp, C.c_double, C.c_int64]
+        L.sco_eval_stat.argtypes = [C.POINTER(Config), _dp, _dp, _dp, _dp, _dp, C.c_int64, _ip, C.c_int64,
+                                    _dp, _dp, _ip]
+        L.sco_eval_stat_levels.argtypes = [C.POINTER(Config), _dp, _dp, _dp, _dp, _dp, C.c_int64, _ip, _ip,
+                                           C.c_int64, _dp]
+        L.sco_num_threads.restype = C.c_int
+        L.sco_philox4x32_10.argtypes = [C.POINTER(C.c_uint32), C.POINTER(C.c_uint32), C.POINTER(C.c_uint32)]
+        L.sco_pso_uniforms.argtypes = [C.c_uint64, C.c_uint64, C.c_uint64, _dp, _dp]
+        L.sco_pso_step.argtypes = [_dp, _dp, _dp, _dp, _dp, _dp, _dp, _dp, _dp, _dp,
+                                   C.c_double, C.c_double, C.c_double, C.c_uint64, C.c_uint64, C.c_int64, C.c_int32]
+    return _lib
+
+
+def _d(a):
+    return None if a is None else a.ctypes.data_as(_dp)
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _ri(z):
+    """complex128 array -> the same memory viewed as interleaved re/im float64."""
+    if z is None:
+        return None
+    z = np.ascontiguousarray(z, dtype=np.complex128)
+    return z.view(np.float64)
+
+
+def phase(cfg, theta, f):
+    th = _f64(theta)
+    return lib().sco_phase(C.byref(cfg), _d(th), float(f))
+
+
+def tf(cfg, theta, f):
+    th = _f64(theta)
+    return lib().sco_tf(C.byref(cfg), _d(th), float(f))
+
+
+def orbit(cfg, t):
+    p = np.zeros((4, 3))
+    lib().sco_orbit(C.byref(cfg), float(t), _d(p))
+    return p
+
+
+def link(cfg, theta, f, t, s, r):
+    th = _f64(theta)
+    o = np.zeros(2)
+    lib().sco_link(C.byref(cfg), _d(th), float(f), float(t), int(s), int(r), _d(o))
+    return complex(o[0], o[1])
+
+
+def tdi(cfg, theta, f, t):
+    """dict X,Y,Z,A,E,T -> complex transfer function (without A(f) e^{-i Psi})."""
+    th = _f64(theta)
+    o = np.zeros((6, 2))
+    lib().sco_tdi(C.byref(cfg), _d(th), float(f), float(t), _d(o))
+    return {k: complex(o[i, 0], o[i, 1]) for i, k in enumerate("XYZAET")}
+
+
+def template(cfg, theta, j_begin=0, n=None):
+    """(h_A, h_E, n_in_window) on bins [j_begin, j_begin+n)."""
+    n = int(cfg.n_bins - j_begin if n is None else n)
+    th = _f64(theta)
+    hA = np.zeros(n, dtype=np.complex128)
+    hE = np.zeros(n, dtype=np.complex128)
+    w = lib().sco_template(C.byref(cfg), _d(th), int(j_begin), n, _d(hA.view(np.float64)), _d(hE.view(np.float64)))
+    return hA, hE, int(w)
+
+
+def stat_from_arrays(dA, dE, hA, hE, SA, SE, df, edges, want_seg=False):
+    edges = np.ascontiguousarray(edges, dtype=np.int64)
+    n_seg = len(edges) - 1
+    seg = np.zeros((n_seg, 3)) if want_seg else None
+    a = [_ri(dA), _ri(dE), _ri(hA), _ri(hE), None if SA is None else _f64(SA), None if SE is None else _f64(SE)]
+    u = lib().sco_stat_from_arrays(_d(a[0]), _d(a[1]), _d(a[2]), _d(a[3]), _d(a[4]), _d(a[5]), float(df),
+                                   edges.ctypes.data_as(_ip), n_seg, _d(seg))
+    return (u, seg) if want_seg else u
+
+
+def inner(aA, aE, bA, bE, SA, SE, df):
+    a = [_ri(aA), _ri(aE), _ri(bA), _ri(bE), _f64(SA), None if SE is None else _f64(SE)]
+    return lib().sco_inner(_d(a[0]), _d(a[1]), _d(a[2]), _d(a[3]), _d(a[4]), _d(a[5]), float(df), len(aA))
+
+
+def eval_stat(cfg, dA, dE, SA, SE, params, edges, want_seg=False, want_inwin=False):
+    params = _f64(params).reshape(-1, 8)
+    P = params.shape[0]
+    edges = np.ascontiguousarray(edges, dtype=np.int64)
+    n_seg = len(edges) - 1
+    out = np.zeros(P)
+    seg = np.zeros((P, n_seg, 3)) if want_seg else None
+    inw = np.zeros(P, dtype=np.int64) if want_inwin else None
+    a = [_ri(dA), _ri(dE), _f64(SA), _f64(SE)]
+    lib().sco_eval_stat(C.byref(cfg), _d(a[0]), _d(a[1]), _d(a[2]), _d(a[3]), _d(params), P,
+                        edges.ctypes.data_as(_ip), n_seg, _d(out), _d(seg),
+                        None if inw is None else inw.ctypes.data_as(_ip))
+    res = [out]
+    if want_seg:
+        res.append(seg)
+    if want_inwin:
+        res.append(inw)
+    return res[0] if len(res) == 1 else tuple(res)
+
+
+def eval_stat_levels(cfg, dA, dE, SA, SE, params, edges_list):
+    """Several edge lists (hierarchy levels) from one template per particle -> [n_levels][P]."""
+    params = _f64(params).reshape(-1, 8)
+    P = params.shape[0]
+    cat = np.ascontiguousarray(np.concatenate([np.asarray(e, dtype=np.int64) for e in edges_list]))
+    ns = np.array([len(e) - 1 for e in edges_list], dtype=np.int64)
+    out = np.zeros((len(edges_list), P))
+    a = [_ri(dA), _ri(dE), _f64(SA), _f64(SE)]
+    lib().sco_eval_stat_levels(C.byref(cfg), _d(a[0]), _d(a[1]), _d(a[2]), _d(a[3]), _d(params), P,
+                               cat.ctypes.data_as(_ip), ns.ctypes.data_as(_ip), len(edges_list), _d(out))
+    return out
+
+
+def num_threads():
+    return lib().sco_num_threads()
+
+
+def philox4x32_10(ctr, key):
+    c = (C.c_uint32 * 4)(*[int(x) for x in ctr])
+    k = (C.c_uint32 * 2)(*[int(x) for x in key])
+    o = (C.c_uint32 * 4)()
+    lib().sco_philox4x32_10(c, k, o)
+    return [int(x) for x in o]
+
+
+def pso_uniforms(seed, particle, it):
+    rP = np.zeros(8)
+    rG = np.zeros(8)
+    lib().sco_pso_uniforms(int(seed), int(particle), int(it), _d(rP), _d(rG))
+    return rP, rG
+
+
+def pso_step(pos, vel, pbest_pos, pbest_val, stat, gbest_pos, gbest_val, lo, hi, eps_min,
+             omega, phi_p, phi_g, seed, it, n_swarms):
+    """In-place on float64 C-contiguous arrays (pos, vel, pbest_pos [P,8]; pbest_val [P]; gbest_* [S,8],[S])."""
+    for a in (pos, vel, pbest_pos, pbest_val, gbest_pos, gbest_val):
+        assert a.dtype == np.float64 and a.flags.c_contiguous
+    P = pos.shape[0]
+    st, lo, hi, ep = _f64(stat), _f64(lo), _f64(hi), _f64(eps_min)
+    lib().sco_pso_step(_d(pos), _d(vel), _d(pbest_pos), _d(pbest_val), _d(st), _d(gbest_pos), _d(gbest_val),
+                       _d(lo), _d(hi), _d(ep), float(omega), float(phi_p), float(phi_g), int(seed), int(it),
+                       P, int(n_swarms))
