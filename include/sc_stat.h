@@ -1,0 +1,136 @@
+/*
+ * sc_stat.h -- C ABI of the B200-native semi-coherent statistic library (libscstat.so).
+ *
+ * Hot path of Bandopadhyay & Moore, "A GPU-accelerated semi-coherent hierarchical search for stellar-mass
+ * binary inspiral signals in LISA" (arXiv 2408.13170; text at /root/reference/PAPER.md, cited PAPER.md:<line>):
+ * batched evaluation of the semi-coherent detection statistic Upsilon_N (Eq. 10) for a whole
+ * particle-swarm population, plus the PSO update (Eq. 13-15).  Where the paper names a model
+ * but prints no formula (waveform, response), the readings O1..O7 / Q1..Q17 of SURVEY.md 8(c) are used; they are
+ * restated in DESIGN.md.
+ *
+ * Conventions
+ *  - Plain C, no exceptions, no torch types.  Every function returns an int status (0 = SC_OK, negative = error);
+ *    the message of the last error is available from sc_last_error().
+ *  - "device" = pointer to CUDA device memory of the current device; "host" = ordinary host memory.
+ *  - The caller owns every buffer it passes.  The handle owns its whitened copy of the data and its scratch
+ *    (grown lazily); nothing caller-visible is allocated by the library.
+ *  - All work is enqueued on the given cudaStream_t (passed as void*; NULL = default stream).  No host
+ *    synchronisation happens inside the *_stat / pso calls unless stated; one handle is used from one stream
+ *    at a time.
+ *  - CUDA errors are sticky in the handle: after SC_ERR_CUDA every call returns SC_ERR_CUDA.
+ *  - There is NO CPU fallback: without a CUDA device sc_init_data fails with SC_ERR_CUDA.
+ *
+ * Particle parameter row (D3, Q3), FP64, row-major [n_particles][8]:
+ *    theta = ( M_c [Msun, detector frame], eta, t_c [s from data start], lambda, beta, iota, psi, e_0 ).
+ * Per-particle invalid input (non-finite, eta outside (0, 0.25], M_c <= 0) gives Upsilon = 0, never NaN.
+ */
+#ifndef SC_STAT_H
+#define SC_STAT_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sc_handle sc_handle;    /* opaque, library-owned */
+
+/* POD, copied at init.  Frequency grid f_j = (j0 + j)/T_obs_s, j = 0..n_bins-1 (the FFT grid). */
+typedef struct {
+  double  T_obs_s;        /* observation time; df = 1/T_obs                                         */
+  int64_t j0;             /* first bin index                                                         */
+  int64_t n_bins;         /* 1 <= n_bins < 2^31                                                      */
+  int32_t n_channels;     /* 2 (A,E).  3 (T) is reserved and rejected                                */
+  int32_t window_mode;    /* 0 = none, 1 = template is zero where t(f) is outside [0, T_obs]  (Q4)   */
+  int32_t pn_order_x2;    /* highest phase term kept, 0..7; 7 = 3.5PN (O2)                           */
+  int32_t ecc_leading;    /* 1 = include the leading-order e0^2 phase term (Q5)                      */
+  double  f_ref_ecc;      /* GW frequency at which e0 is defined                                     */
+  double  arm_L_s, au_s, orbit_alpha0, orbit_lambda0, year_s;   /* orbit constants, seconds / rad (Q6) */
+} sc_config;
+
+enum {
+  SC_OK = 0,
+  SC_ERR_INVALID_ARG = -1,   /* null pointer, n <= 0, bad config, edges not non-decreasing or out of [0, n_bins] */
+  SC_ERR_NOT_INIT = -2,      /* null / freed handle                                                             */
+  SC_ERR_CUDA = -3,          /* a CUDA call or kernel failed (sticky)                                           */
+  SC_ERR_OOM = -4            /* device allocation failed                                                        */
+};
+
+/* Options for sc_set_option. */
+enum {
+  SC_OPT_PRECISION = 1,      /* 0 = auto (FP32 amplitude path when n_seg >= SC_OPT_F32_MIN_SEG, else all-FP64),
+                                1 = force FP32 amplitude path, 2 = force all-FP64.  Phase is FP64 always.       */
+  SC_OPT_F32_MIN_SEG = 2,    /* threshold of the auto rule (default 8)               */
+  SC_OPT_SCRATCH_BYTES = 3,  /* cap of the node-table scratch; larger populations are processed in batches      */
+  SC_OPT_TC_MAX_S = 4,       /* the caller's upper bound on t_c [s] over the particles (the search tile's t_c range,
+                                PAPER.md:253); sets the coarse node spacing to about one day of signal time at the
+                                low band edge.  Default 10 yr.                                  */
+  SC_OPT_STRIDE_LOG2 = 5     /* 0 = automatic (rule above), else log2 of the coarse node spacing in bins (2..12)   */
+};
+
+/* a0 -- data whitening, once per data stream (PSD known; Eq. 1 weights).
+ * dA_ri, dE_ri: DEVICE, interleaved (re, im) FP64, n_bins complex each.  S_A, S_E: DEVICE, one-sided PSD, n_bins.
+ * Stores W_a = d_a * 4df/S_a and G_a = 4df/S_a (rescaled to O(1)) in FP32 and FP64; the inputs are not kept.
+ * Bins with non-finite or non-positive S are given zero weight.  Synchronises the stream once (to size the scale).
+ * On success *out is a new handle (free with sc_free). */
+int sc_init_data(sc_handle** out, const sc_config* cfg,
+                 const double* dA_ri, const double* dE_ri, const double* S_A, const double* S_E,
+                 void* cuda_stream);
+/* Same with HOST buffers (copied to the device inside). */
+int sc_init_data_host(sc_handle** out, const sc_config* cfg,
+                      const double* dA_ri, const double* dE_ri, const double* S_A, const double* S_E,
+                      void* cuda_stream);
+
+/* a1..a6 -- Upsilon_N(d, theta_p) for every particle (Eq. 7, 8, 10; readings Q1, Q2, Q7, Q8):
+ *   z_k = sum_a sum_{j in [e_k, e_k+1)} d_a conj(h_a)/S_a,  sigma_k = sum_a sum_j |h_a|^2/S_a,
+ *   out[p] = 4 df sum_{k: sigma_k > 0} |z_k|^2 / sigma_k,
+ * with h_a(theta, f_j) = T_a(theta, f_j) A(f_j) e^{-i Psi(f_j)} (Eq. 16; O2-O4, window Q4).
+ * params: DEVICE [n_particles][8].  seg_edges: HOST or DEVICE, n_seg+1 non-decreasing bin indices in [0, n_bins]
+ * shared by all particles (Q2); edges may cover only part of the band and may contain empty segments.  A device
+ * pointer is copied back to the host first (one stream synchronisation); host pointers cost no synchronisation.
+ * out: DEVICE [n_particles]. */
+int sc_eval_stat(sc_handle* h, const double* params, int64_t n_particles,
+                 const int32_t* seg_edges, int32_t n_seg, double* out, void* cuda_stream);
+/* Same with HOST params / out (copies inside; synchronises the stream before returning). */
+int sc_eval_stat_host(sc_handle* h, const double* params, int64_t n_particles,
+                      const int32_t* seg_edges, int32_t n_seg, double* out, void* cuda_stream);
+
+/* Debug / parity: the per-segment sums themselves, out_seg DEVICE [n_particles][n_seg][3] = (Re z_k, Im z_k, sigma_k)
+ * in the units of the definition above (template amplitude A(f) = f^(-7/6), O2). */
+int sc_eval_segments(sc_handle* h, const double* params, int64_t n_particles,
+                     const int32_t* seg_edges, int32_t n_seg, double* out_seg, void* cuda_stream);
+
+/* The template itself on the dense grid through the same node tables and interpolants the statistic uses
+ * (for injections and element-wise parity).  params: DEVICE [n_templates][8];
+ * hA_ri, hE_ri: DEVICE [n_templates][n_bins] complex FP64 interleaved. */
+int sc_gen_template(sc_handle* h, const double* params, int64_t n_templates,
+                    double* hA_ri, double* hE_ri, void* cuda_stream);
+
+/* a7 -- one synchronous PSO iteration (Eq. 13-15; App. B; readings Q9, Q10):
+ *  (1) personal bests: stat[p] > pbest_val[p] (strict) -> pbest := (pos[p], stat[p]);
+ *  (2) per swarm (n_swarms equal contiguous blocks): gbest := arg max pbest_val, lowest index on ties;
+ *  (3) u = omega v + phi_p r_P (pbest - pos) + phi_g r_G (gbest - pos), r ~ U(0,1) from Philox4x32-10 keyed by
+ *      seed with counter (particle, iter, block, 0);  (4) v = max(eps, |u|) sign(u) (sign(0) = +1);
+ *  (5) pos += v;  (6) reflect at [lo, hi].
+ * All arrays DEVICE, FP64: pos, vel, pbest_pos [n_particles][8]; pbest_val, stat [n_particles];
+ * gbest_pos [n_swarms][8], gbest_val [n_swarms] (outputs); lo, hi, eps_min [8].
+ * n_particles must be a multiple of n_swarms. */
+int sc_pso_step(sc_handle* h, double* pos, double* vel, double* pbest_pos, double* pbest_val,
+                const double* stat, double* gbest_pos, double* gbest_val,
+                const double* lo, const double* hi, const double* eps_min,
+                double omega, double phi_p, double phi_g, uint64_t seed, uint64_t iter,
+                int64_t n_particles, int32_t n_swarms, void* cuda_stream);
+
+/* Counters of the last sc_eval_stat / sc_eval_segments call (synchronises the stream):
+ *  evaluated_bins = sum_p |{j in window_p} intersect [e_0, e_N)|  (the "evaluated (particle x bin)" of the metric),
+ *  kernel_launches = CUDA kernels launched by the library since the handle was created. */
+int sc_get_counters(sc_handle* h, int64_t* evaluated_bins, int64_t* kernel_launches, void* cuda_stream);
+
+int sc_set_option(sc_handle* h, int32_t option, int64_t value);
+int sc_free(sc_handle* h);
+const char* sc_last_error(const sc_handle* h);    /* h may be NULL: error of the last failed sc_init_data */
+const char* sc_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,16 @@
+"""B200-native semi-coherent statistic (hot path of arXiv 2408.13170): thin Python binding over libscstat.so.
+
+Every step of the path runs in the CUDA kernels of csrc/; this package only marshals arguments.
+There is no CPU fallback: importing works anywhere, but every call needs the built library and a CUDA device.
+"""
+from .binding import (SCError, ScConfig, Handle, load_library, library_path, sc_init_data, sc_init_data_host,
+                      sc_eval_stat, sc_eval_stat_host, sc_eval_segments, sc_gen_template, sc_pso_step,
+                      sc_get_counters, sc_set_option, sc_free, sc_last_error, sc_version,
+                      SC_OPT_PRECISION, SC_OPT_F32_MIN_SEG, SC_OPT_SCRATCH_BYTES, SC_OPT_TC_MAX_S,
+                      SC_OPT_STRIDE_LOG2, EXPORTED_SYMBOLS)
+
+__all__ = ["SCError", "ScConfig", "Handle", "load_library", "library_path", "sc_init_data", "sc_init_data_host",
+           "sc_eval_stat", "sc_eval_stat_host", "sc_eval_segments", "sc_gen_template", "sc_pso_step",
+           "sc_get_counters", "sc_set_option", "sc_free", "sc_last_error", "sc_version",
+           "SC_OPT_PRECISION", "SC_OPT_F32_MIN_SEG", "SC_OPT_SCRATCH_BYTES", "SC_OPT_TC_MAX_S", "SC_OPT_STRIDE_LOG2",
+           "EXPORTED_SYMBOLS"]

@@ -1,0 +1,328 @@
+"""ctypes binding of libscstat.so: the same names as include/sc_stat.h, argument marshalling only.
+
+Device arguments are torch CUDA tensors (float64 / int32, contiguous); PyTorch is used for device memory and
+streams, nothing else.  Calls go to the current torch CUDA stream unless `stream` is given.
+If the library is missing or cannot be loaded every call raises SCError -- there is no fallback path.
+"""
+import ctypes as C
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libscstat.so")
+
+SC_OK, SC_ERR_INVALID_ARG, SC_ERR_NOT_INIT, SC_ERR_CUDA, SC_ERR_OOM = 0, -1, -2, -3, -4
+SC_OPT_PRECISION, SC_OPT_F32_MIN_SEG, SC_OPT_SCRATCH_BYTES, SC_OPT_TC_MAX_S, SC_OPT_STRIDE_LOG2 = 1, 2, 3, 4, 5
+
+EXPORTED_SYMBOLS = ["sc_init_data", "sc_init_data_host", "sc_eval_stat", "sc_eval_stat_host", "sc_eval_segments",
+                    "sc_gen_template", "sc_pso_step", "sc_get_counters", "sc_set_option", "sc_free",
+                    "sc_last_error", "sc_version"]
+
+
+class SCError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"scstat error {code}: {msg}")
+        self.code = code
+
+
+class ScConfig(C.Structure):
+    """sc_config of include/sc_stat.h."""
+    _fields_ = [("T_obs_s", C.c_double), ("j0", C.c_int64), ("n_bins", C.c_int64),
+                ("n_channels", C.c_int32), ("window_mode", C.c_int32), ("pn_order_x2", C.c_int32),
+                ("ecc_leading", C.c_int32), ("f_ref_ecc", C.c_double),
+                ("arm_L_s", C.c_double), ("au_s", C.c_double), ("orbit_alpha0", C.c_double),
+                ("orbit_lambda0", C.c_double), ("year_s", C.c_double)]
+
+    @classmethod
+    def from_dict(cls, d):
+        c = cls()
+        for k, _ in cls._fields_:
+            setattr(c, k, d[k])
+        return c
+
+
+_lib = None
+_vp = C.c_void_p
+
+
+def library_path():
+    return _LIB_PATH
+
+
+def load_library():
+    """Load libscstat.so (built by paper_2408_13170_b200.build / __graft_entry__.build()).  Fails loudly."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise SCError(SC_ERR_NOT_INIT, f"{_LIB_PATH} not built: run `python -m paper_2408_13170_b200.build` "
+                                       "(needs nvcc); there is no CPU fallback")
+    try:
+        L = C.CDLL(_LIB_PATH)
+    except OSError as e:
+        raise SCError(SC_ERR_NOT_INIT, f"cannot load {_LIB_PATH}: {e}; there is no CPU fallback")
+    cfgp = C.POINTER(ScConfig)
+    L.sc_init_data.restype = C.c_int
+    L.sc_init_data.argtypes = [C.POINTER(_vp), cfgp, _vp, _vp, _vp, _vp, _vp]
+    L.sc_init_data_host.restype = C.c_int
+    L.sc_init_data_host.argtypes = [C.POINTER(_vp), cfgp, _vp, _vp, _vp, _vp, _vp]
+    for name in ("sc_eval_stat", "sc_eval_stat_host", "sc_eval_segments"):
+        f = getattr(L, name)
+        f.restype = C.c_int
+        f.argtypes = [_vp, _vp, C.c_int64, _vp, C.c_int32, _vp, _vp]
+    L.sc_gen_template.restype = C.c_int
+    L.sc_gen_template.argtypes = [_vp, _vp, C.c_int64, _vp, _vp, _vp]
+    L.sc_pso_step.restype = C.c_int
+    L.sc_pso_step.argtypes = [_vp] + [_vp] * 10 + [C.c_double] * 3 + [C.c_uint64, C.c_uint64, C.c_int64, C.c_int32, _vp]
+    L.sc_get_counters.restype = C.c_int
+    L.sc_get_counters.argtypes = [_vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64), _vp]
+    L.sc_set_option.restype = C.c_int
+    L.sc_set_option.argtypes = [_vp, C.c_int32, C.c_int64]
+    L.sc_free.restype = C.c_int
+    L.sc_free.argtypes = [_vp]
+    L.sc_last_error.restype = C.c_char_p
+    L.sc_last_error.argtypes = [_vp]
+    L.sc_version.restype = C.c_char_p
+    L.sc_version.argtypes = []
+    _lib = L
+    return L
+
+
+def _torch():
+    import torch
+    return torch
+
+
+def _stream(stream):
+    if stream is not None:
+        return _vp(int(stream))
+    return _vp(int(_torch().cuda.current_stream().cuda_stream))
+
+
+def _dev(t, dtype, name):
+    torch = _torch()
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == dtype and t.is_contiguous()):
+        raise SCError(SC_ERR_INVALID_ARG, f"{name}: need a contiguous CUDA tensor of dtype {dtype}")
+    return _vp(t.data_ptr())
+
+
+def _host_f64(a, name):
+    import numpy as np
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    return a, _vp(a.ctypes.data)
+
+
+def _edges_arg(seg_edges):
+    """HOST numpy int32 array (preferred) or DEVICE int32 tensor -> (keepalive, pointer, n_seg)."""
+    import numpy as np
+    torch = _torch()
+    if isinstance(seg_edges, torch.Tensor):
+        if seg_edges.is_cuda:
+            if seg_edges.dtype != torch.int32 or not seg_edges.is_contiguous():
+                raise SCError(SC_ERR_INVALID_ARG, "seg_edges: device tensor must be contiguous int32")
+            return seg_edges, _vp(seg_edges.data_ptr()), int(seg_edges.numel()) - 1
+        seg_edges = seg_edges.numpy()
+    e = np.ascontiguousarray(seg_edges)
+    if e.size and (e.min() < -2 ** 31 or e.max() >= 2 ** 31):
+        raise SCError(SC_ERR_INVALID_ARG, "seg_edges out of int32 range")
+    e = e.astype(np.int32)
+    return e, _vp(e.ctypes.data), int(e.size) - 1
+
+
+def _check(rc, h):
+    if rc != SC_OK:
+        msg = load_library().sc_last_error(h)
+        raise SCError(rc, msg.decode() if msg else "")
+
+
+# ---------------------------------------------------------------------------------------------- C-named functions
+def sc_version():
+    return load_library().sc_version().decode()
+
+
+def sc_last_error(h=None):
+    m = load_library().sc_last_error(h)
+    return m.decode() if m else ""
+
+
+def sc_init_data(cfg, dA_ri, dE_ri, S_A, S_E, stream=None):
+    """DEVICE float64 tensors: dA_ri, dE_ri [n_bins, 2] (re, im), S_A, S_E [n_bins].  Returns the opaque handle."""
+    torch = _torch()
+    L = load_library()
+    if not isinstance(cfg, ScConfig):
+        cfg = ScConfig.from_dict(cfg)
+    n = int(cfg.n_bins)
+    for t, m, nm in ((dA_ri, 2 * n, "dA_ri"), (dE_ri, 2 * n, "dE_ri"), (S_A, n, "S_A"), (S_E, n, "S_E")):
+        if isinstance(t, torch.Tensor) and t.numel() != m:
+            raise SCError(SC_ERR_INVALID_ARG, f"{nm}: expected {m} float64 values, got {t.numel()}")
+    h = _vp()
+    rc = L.sc_init_data(C.byref(h), C.byref(cfg), _dev(dA_ri, torch.float64, "dA_ri"), _dev(dE_ri, torch.float64, "dE_ri"),
+                        _dev(S_A, torch.float64, "S_A"), _dev(S_E, torch.float64, "S_E"), _stream(stream))
+    _check(rc, None)
+    return h
+
+
+def sc_init_data_host(cfg, dA, dE, S_A, S_E, stream=None):
+    """HOST numpy arrays: dA, dE complex128 [n_bins] (or float64 [n_bins, 2]); S_A, S_E float64 [n_bins]."""
+    import numpy as np
+    L = load_library()
+    if not isinstance(cfg, ScConfig):
+        cfg = ScConfig.from_dict(cfg)
+    n = int(cfg.n_bins)
+    arrs = []
+    for a, m, nm in ((dA, 2 * n, "dA"), (dE, 2 * n, "dE"), (S_A, n, "S_A"), (S_E, n, "S_E")):
+        a = np.ascontiguousarray(a)
+        if np.iscomplexobj(a):
+            a = np.ascontiguousarray(a, dtype=np.complex128).view(np.float64)
+        a = np.ascontiguousarray(a, dtype=np.float64)
+        if a.size != m:
+            raise SCError(SC_ERR_INVALID_ARG, f"{nm}: expected {m} float64 values, got {a.size}")
+        arrs.append(a)
+    h = _vp()
+    rc = L.sc_init_data_host(C.byref(h), C.byref(cfg), *[_vp(a.ctypes.data) for a in arrs], _stream(stream))
+    _check(rc, None)
+    return h
+
+
+def sc_eval_stat(h, params, n_particles, seg_edges, n_seg, out, stream=None):
+    torch = _torch()
+    keep, ep, ns = _edges_arg(seg_edges)
+    if ns != n_seg:
+        raise SCError(SC_ERR_INVALID_ARG, f"seg_edges has {ns + 1} entries, expected n_seg + 1 = {n_seg + 1}")
+    if params.numel() != 8 * n_particles or out.numel() != n_particles:
+        raise SCError(SC_ERR_INVALID_ARG, "params must be [n_particles, 8] and out [n_particles]")
+    rc = load_library().sc_eval_stat(h, _dev(params, torch.float64, "params"), n_particles, ep, n_seg,
+                                     _dev(out, torch.float64, "out"), _stream(stream))
+    _check(rc, h)
+    return out
+
+
+def sc_eval_stat_host(h, params, n_particles, seg_edges, n_seg, out, stream=None):
+    """HOST numpy params [n_particles, 8] / out [n_particles] (float64); copies run inside the C call."""
+    import numpy as np
+    keep, ep, ns = _edges_arg(seg_edges)
+    if ns != n_seg:
+        raise SCError(SC_ERR_INVALID_ARG, f"seg_edges has {ns + 1} entries, expected n_seg + 1 = {n_seg + 1}")
+    if not (isinstance(params, np.ndarray) and params.dtype == np.float64 and params.flags.c_contiguous
+            and params.size == 8 * n_particles):
+        raise SCError(SC_ERR_INVALID_ARG, "params: need C-contiguous float64 numpy [n_particles, 8]")
+    if not (isinstance(out, np.ndarray) and out.dtype == np.float64 and out.flags.c_contiguous and out.size == n_particles):
+        raise SCError(SC_ERR_INVALID_ARG, "out: need C-contiguous float64 numpy [n_particles]")
+    rc = load_library().sc_eval_stat_host(h, _vp(params.ctypes.data), n_particles, ep, n_seg, _vp(out.ctypes.data),
+                                          _stream(stream))
+    _check(rc, h)
+    return out
+
+
+def sc_eval_segments(h, params, n_particles, seg_edges, n_seg, out_seg, stream=None):
+    torch = _torch()
+    keep, ep, ns = _edges_arg(seg_edges)
+    if ns != n_seg:
+        raise SCError(SC_ERR_INVALID_ARG, f"seg_edges has {ns + 1} entries, expected n_seg + 1 = {n_seg + 1}")
+    if params.numel() != 8 * n_particles or out_seg.numel() != n_particles * n_seg * 3:
+        raise SCError(SC_ERR_INVALID_ARG, "params must be [n_particles, 8] and out_seg [n_particles, n_seg, 3]")
+    rc = load_library().sc_eval_segments(h, _dev(params, torch.float64, "params"), n_particles, ep, n_seg,
+                                         _dev(out_seg, torch.float64, "out_seg"), _stream(stream))
+    _check(rc, h)
+    return out_seg
+
+
+def sc_gen_template(h, params, n_templates, hA_ri, hE_ri, stream=None):
+    torch = _torch()
+    rc = load_library().sc_gen_template(h, _dev(params, torch.float64, "params"), n_templates,
+                                        _dev(hA_ri, torch.float64, "hA_ri"), _dev(hE_ri, torch.float64, "hE_ri"),
+                                        _stream(stream))
+    _check(rc, h)
+    return hA_ri, hE_ri
+
+
+def sc_pso_step(h, pos, vel, pbest_pos, pbest_val, stat, gbest_pos, gbest_val, lo, hi, eps_min,
+                omega, phi_p, phi_g, seed, iter, n_particles, n_swarms, stream=None):
+    torch = _torch()
+    names = ["pos", "vel", "pbest_pos", "pbest_val", "stat", "gbest_pos", "gbest_val", "lo", "hi", "eps_min"]
+    tens = [pos, vel, pbest_pos, pbest_val, stat, gbest_pos, gbest_val, lo, hi, eps_min]
+    sizes = [8 * n_particles] * 3 + [n_particles] * 2 + [8 * n_swarms, n_swarms, 8, 8, 8]
+    for t, nm, sz in zip(tens, names, sizes):
+        if isinstance(t, torch.Tensor) and t.numel() != sz:
+            raise SCError(SC_ERR_INVALID_ARG, f"{nm}: expected {sz} values, got {t.numel()}")
+    ptrs = [_dev(t, torch.float64, nm) for t, nm in zip(tens, names)]
+    rc = load_library().sc_pso_step(h, *ptrs, float(omega), float(phi_p), float(phi_g), int(seed) & (2 ** 64 - 1),
+                                    int(iter), int(n_particles), int(n_swarms), _stream(stream))
+    _check(rc, h)
+
+
+def sc_get_counters(h, stream=None):
+    """(evaluated_bins of the last eval, kernel launches since init); synchronises the stream."""
+    a, b = C.c_int64(0), C.c_int64(0)
+    rc = load_library().sc_get_counters(h, C.byref(a), C.byref(b), _stream(stream))
+    _check(rc, h)
+    return a.value, b.value
+
+
+def sc_set_option(h, option, value):
+    _check(load_library().sc_set_option(h, int(option), int(value)), h)
+
+
+def sc_free(h):
+    if h is not None and h.value:
+        load_library().sc_free(h)
+        h.value = None
+
+
+# ---------------------------------------------------------------------------------------------- convenience wrapper
+class Handle:
+    """Owns one sc_handle.  Methods forward to the C-named functions above."""
+
+    def __init__(self, cfg, dA, dE, S_A, S_E, host=False, stream=None):
+        self.cfg = cfg if isinstance(cfg, ScConfig) else ScConfig.from_dict(cfg)
+        self.h = (sc_init_data_host if host else sc_init_data)(self.cfg, dA, dE, S_A, S_E, stream)
+
+    def eval_stat(self, params, seg_edges, out=None, stream=None):
+        torch = _torch()
+        P = params.shape[0]
+        if out is None:
+            out = torch.empty(P, dtype=torch.float64, device=params.device)
+        return sc_eval_stat(self.h, params, P, seg_edges, len(seg_edges) - 1, out, stream)
+
+    def eval_stat_host(self, params, seg_edges, out=None, stream=None):
+        import numpy as np
+        P = params.shape[0]
+        if out is None:
+            out = np.empty(P, dtype=np.float64)
+        return sc_eval_stat_host(self.h, params, P, seg_edges, len(seg_edges) - 1, out, stream)
+
+    def eval_segments(self, params, seg_edges, stream=None):
+        torch = _torch()
+        P, N = params.shape[0], len(seg_edges) - 1
+        out = torch.empty((P, N, 3), dtype=torch.float64, device=params.device)
+        return sc_eval_segments(self.h, params, P, seg_edges, N, out, stream)
+
+    def gen_template(self, params, stream=None):
+        """-> (h_A, h_E) complex128 CUDA tensors [n_templates, n_bins]."""
+        torch = _torch()
+        params = params.reshape(-1, 8)
+        n = int(self.cfg.n_bins)
+        hA = torch.empty((params.shape[0], n, 2), dtype=torch.float64, device=params.device)
+        hE = torch.empty_like(hA)
+        sc_gen_template(self.h, params, params.shape[0], hA, hE, stream)
+        return torch.view_as_complex(hA), torch.view_as_complex(hE)
+
+    def pso_step(self, state, stat, lo, hi, eps_min, omega, phi_p, phi_g, seed, it, n_swarms, stream=None):
+        """state: dict of CUDA tensors pos, vel, pbest_pos, pbest_val, gbest_pos, gbest_val (updated in place)."""
+        sc_pso_step(self.h, state["pos"], state["vel"], state["pbest_pos"], state["pbest_val"], stat,
+                    state["gbest_pos"], state["gbest_val"], lo, hi, eps_min, omega, phi_p, phi_g, seed, it,
+                    state["pos"].shape[0], n_swarms, stream)
+
+    def counters(self, stream=None):
+        return sc_get_counters(self.h, stream)
+
+    def set_option(self, option, value):
+        sc_set_option(self.h, option, value)
+
+    def close(self):
+        sc_free(self.h)
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,1003 @@
+// sc_stat.cu -- kernels and C ABI of libscstat.so (sm_100a).  See include/sc_stat.h for the contract and
+// DESIGN.md for the design.  No CPU fallback, no torch, no third-party code.
+//
+// Pipeline of one sc_eval_stat call, per batch of particles:
+//   k_particle_consts  a1 + a3  per-particle constants, validity, time window [jlo, jhi) by bisection on t(f_j)
+//   k_nodes            a2       phase / amplitude at the coarse nodes (one node per `stride` bins)
+//   k_dense<R, SEG>    a4 + a5  THE HOT LOOP: lane = particle, warp walks the bins of its chunk in order;
+//                               whitened data broadcast from shared memory; FP64 phase by forward differences;
+//                               complete segments are finalised in registers, straddlers leave fragments
+//   k_stitch           a6       fixed-order stitch of the fragments -> Upsilon[p]
+#include "../../include/sc_stat.h"
+#include "sc_math.cuh"
+
+#include <algorithm>
+#include <climits>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+using namespace sc;
+
+namespace {
+
+constexpr int kBlock = 128;            // threads per CTA of the dense kernel = particles per CTA
+constexpr int kChunkF32 = 2048;        // bins per CTA, FP32 amplitude path (24 B/bin of shared memory)
+constexpr int kChunkF64 = 1024;        // bins per CTA, all-FP64 path (48 B/bin)
+constexpr int kFlushBins = 32;         // FP32 partial sums are folded into the FP64 accumulators this often
+constexpr int kFragFields = 7;         // partial Upsilon, head (zr, zi, sg), tail (zr, zi, sg)
+constexpr double kMagic = 6755399441055744.0;   // 1.5 * 2^52: (x + kMagic) - kMagic = rint(x), low word = int
+
+// chunk flags (host-built from the edges, shared by all particles)
+enum : uint8_t { CF_HEAD = 1, CF_HEAD_CLOSES = 2, CF_TAIL = 4 };
+
+// ------------------------------------------------------------------------------------------------ whitening (a0)
+__global__ void k_max_weight(const double* __restrict__ S_A, const double* __restrict__ S_E, int n, double four_df,
+                             unsigned long long* __restrict__ out_max_bits) {
+  double m = 0.0;
+  for (int j = blockIdx.x * blockDim.x + threadIdx.x; j < n; j += gridDim.x * blockDim.x) {
+    const double a = S_A[j], e = S_E[j];
+    if (isfinite(a) && a > 0.0) m = fmax(m, four_df / a);
+    if (isfinite(e) && e > 0.0) m = fmax(m, four_df / e);
+  }
+  for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+  if ((threadIdx.x & 31) == 0 && isfinite(m)) atomicMax(out_max_bits, (unsigned long long)__double_as_longlong(m));
+}
+
+// W_a = d_a * (4 df / S_a) / s0,  G_a = (4 df / S_a) / s0^2  with s0 a power of two (exact rescaling).
+__global__ void k_whiten(const double* __restrict__ dA, const double* __restrict__ dE,
+                         const double* __restrict__ S_A, const double* __restrict__ S_E, int n, double four_df,
+                         double inv_s0, float4* __restrict__ W32, float2* __restrict__ G32,
+                         double4* __restrict__ W64, double2* __restrict__ G64) {
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= n) return;
+  const double a = S_A[j], e = S_E[j];
+  const double ua = (isfinite(a) && a > 0.0) ? four_df / a : 0.0;
+  const double ue = (isfinite(e) && e > 0.0) ? four_df / e : 0.0;
+  double4 w;
+  w.x = dA[2 * j] * ua * inv_s0; w.y = dA[2 * j + 1] * ua * inv_s0;
+  w.z = dE[2 * j] * ue * inv_s0; w.w = dE[2 * j + 1] * ue * inv_s0;
+  if (!(isfinite(w.x) && isfinite(w.y))) { w.x = 0.0; w.y = 0.0; }
+  if (!(isfinite(w.z) && isfinite(w.w))) { w.z = 0.0; w.w = 0.0; }
+  double2 g;
+  g.x = ua * inv_s0 * inv_s0; g.y = ue * inv_s0 * inv_s0;
+  W64[j] = w; G64[j] = g;
+  W32[j] = make_float4((float)w.x, (float)w.y, (float)w.z, (float)w.w);
+  G32[j] = make_float2((float)g.x, (float)g.y);
+}
+
+// ------------------------------------------------------------------------------------------------ a1 + a3
+__global__ void k_particle_consts(DevCfg c, const double* __restrict__ params, int P, int P_pad,
+                                  double* __restrict__ pc, int* __restrict__ jlo_out, int* __restrict__ jhi_out,
+                                  int e_first, int e_last, unsigned long long* __restrict__ eval_bins) {
+  const int p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= P_pad) return;
+  int jlo = 0, jhi = 0;
+  Particle q = {};
+  if (p < P) {
+    double th[8];
+    bool ok = true;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) { th[i] = params[(size_t)p * 8 + i]; ok = ok && isfinite(th[i]); }
+    ok = ok && (th[0] > 0.0) && (th[1] > 0.0) && (th[1] <= 0.25);
+    if (ok) {
+      const double M = th[0] * kMsunSec * pow(th[1], -0.6);
+      q.piM = kPi * M; q.eta = th[1]; q.tc = th[2];
+      q.tau_hi = th[2] * c.inv_T;
+      q.tau_lo = fma(-q.tau_hi, c.T_obs, th[2]) * c.inv_T;
+      sincos(th[3], &q.sl, &q.cl);
+      sincos(th[4], &q.sb, &q.cb);
+      sincos(2.0 * th[6], &q.s2p, &q.c2p);
+      q.ci = cos(th[5]);
+      q.ecc = 0.0;
+      if (c.ecc_leading) q.ecc = (2355.0 / 1462.0) * th[7] * th[7] * pow(cbrt(q.piM * c.f_ref_ecc), 19.0 / 3.0);
+      if (c.window_mode == 1) {
+        // Q4: the template lives where 0 <= t(f_j) <= T_obs; t(f) is monotone, so bisect on the bin index
+        // with t(f_j) evaluated directly at the bin frequencies (same expression the definition uses).
+        int lo = 0, hi = c.n_bins;       // first j with t(f_j) >= 0
+        while (lo < hi) {
+          const int mid = (lo + hi) >> 1;
+          if (tf_direct(c, q, (double)(c.j0 + mid) / c.T_obs) >= 0.0) hi = mid; else lo = mid + 1;
+        }
+        jlo = lo;
+        lo = jlo; hi = c.n_bins;          // first j with t(f_j) > T_obs
+        while (lo < hi) {
+          const int mid = (lo + hi) >> 1;
+          if (tf_direct(c, q, (double)(c.j0 + mid) / c.T_obs) > c.T_obs) hi = mid; else lo = mid + 1;
+        }
+        jhi = lo;
+      } else {
+        jlo = 0; jhi = c.n_bins;
+      }
+    }
+    const int a = max(jlo, e_first), b = min(jhi, e_last);
+    if (b > a) atomicAdd(eval_bins, (unsigned long long)(b - a));
+  }
+  pc[PC_PIM * (size_t)P_pad + p] = q.piM;       pc[PC_ETA * (size_t)P_pad + p] = q.eta;
+  pc[PC_TC * (size_t)P_pad + p] = q.tc;         pc[PC_TAU_HI * (size_t)P_pad + p] = q.tau_hi;
+  pc[PC_TAU_LO * (size_t)P_pad + p] = q.tau_lo; pc[PC_CL * (size_t)P_pad + p] = q.cl;
+  pc[PC_SL * (size_t)P_pad + p] = q.sl;         pc[PC_CB * (size_t)P_pad + p] = q.cb;
+  pc[PC_SB * (size_t)P_pad + p] = q.sb;         pc[PC_C2P * (size_t)P_pad + p] = q.c2p;
+  pc[PC_S2P * (size_t)P_pad + p] = q.s2p;       pc[PC_CI * (size_t)P_pad + p] = q.ci;
+  pc[PC_ECC * (size_t)P_pad + p] = q.ecc;
+  jlo_out[p] = jlo; jhi_out[p] = jhi;
+}
+
+// ------------------------------------------------------------------------------------------------ a2
+// One thread per (node, particle), particle fastest -> coalesced [node][particle] tables.
+template <typename R>
+__global__ void k_nodes(DevCfg c, const double* __restrict__ pc, const int* __restrict__ jlo, const int* __restrict__ jhi,
+                        int P_pad, int* __restrict__ node_n, double* __restrict__ node_frac,
+                        R* __restrict__ node_amp /* [node][4][P_pad] */) {
+  const int p = blockIdx.x * blockDim.x + threadIdx.x;
+  const int i = blockIdx.y;                       // 0 .. n_nodes-1  <->  node index i - kNodeOff
+  if (p >= P_pad) return;
+  const long long pos = ((long long)i - kNodeOff) << c.log2_stride;   // bin position of the node
+  const int lo = jlo[p], hi = jhi[p];
+  NodeOut o = {};
+  // nodes farther than the stencils reach from the particle's window are never read
+  const long long reach = 4LL << c.log2_stride;
+  if (hi > lo && pos >= (long long)lo - reach && pos <= (long long)hi + reach && c.j0 + pos > 0) {
+    const Particle q = load_particle(pc, P_pad, p);
+    o = eval_node(c, q, c.j0 + pos);
+  }
+  const size_t at = (size_t)i * P_pad + p;
+  node_n[at] = o.n_turns;
+  node_frac[at] = o.frac;
+  R* a = node_amp + (size_t)i * 4 * P_pad + p;
+  a[0] = (R)o.Ar; a[(size_t)P_pad] = (R)o.Ai; a[2 * (size_t)P_pad] = (R)o.Er; a[3 * (size_t)P_pad] = (R)o.Ei;
+}
+
+// ------------------------------------------------------------------------------------------------ a4 + a5
+// sin, cos of 2 pi x for |x| <= 1/8 turn (Taylor in x^2, coefficients (2 pi)^k / k!).
+__device__ __forceinline__ void sincos_2pi_small(float x, float& s, float& c) {
+  const float x2 = x * x;
+  float ps = fmaf(x2, 42.0586939448976531f, -76.7058597530613858f);  // (2pi)^9/9!, -(2pi)^7/7!
+  ps = fmaf(ps, x2, 81.6052492760750542f);                            // (2pi)^5/5!
+  ps = fmaf(ps, x2, -41.3417022403997602f);                           // -(2pi)^3/3!
+  ps = fmaf(ps, x2, 6.28318530717958648f);
+  s = ps * x;
+  float pc = fmaf(x2, -26.4262567833743975f, 60.2446413718766604f);  // -(2pi)^10/10!, (2pi)^8/8!
+  pc = fmaf(pc, x2, -85.4568172066937277f);                           // -(2pi)^6/6!
+  pc = fmaf(pc, x2, 64.9393940226682915f);                            // (2pi)^4/4!
+  pc = fmaf(pc, x2, -19.7392088021787172f);                           // -(2pi)^2/2!
+  c = fmaf(pc, x2, 1.0f);
+}
+__device__ __forceinline__ void sincos_2pi_small(double x, double& s, double& c) {
+  const double x2 = x * x;
+  double ps = fma(x2, -0.71812230177850051223, 3.8199525848482821277);     // -(2pi)^15/15!, (2pi)^13/13!
+  ps = fma(ps, x2, -15.094642576822990392);                                 // -(2pi)^11/11!
+  ps = fma(ps, x2, 42.058693944897653145);
+  ps = fma(ps, x2, -76.705859753061385842);
+  ps = fma(ps, x2, 81.605249276075054203);
+  ps = fma(ps, x2, -41.341702240399760234);
+  ps = fma(ps, x2, 6.2831853071795864769);
+  s = ps * x;
+  double pc = fma(x2, 0.28200596845579121507, -1.7143907110886720654);     // (2pi)^16/16!, -(2pi)^14/14!
+  pc = fma(pc, x2, 7.9035363713184688042);                                  // (2pi)^12/12!
+  pc = fma(pc, x2, -26.426256783374397453);
+  pc = fma(pc, x2, 60.244641371876660363);
+  pc = fma(pc, x2, -85.456817206693727736);
+  pc = fma(pc, x2, 64.939394022668291491);
+  pc = fma(pc, x2, -19.739208802178717238);
+  c = fma(pc, x2, 1.0);
+}
+
+template <typename R> struct DataT;
+template <> struct DataT<float> { using W = float4; using G = float2; static constexpr int chunk = kChunkF32; };
+template <> struct DataT<double> { using W = double4; using G = double2; static constexpr int chunk = kChunkF64; };
+
+struct DenseArgs {
+  const int* edges;            // [n_seg + 1]
+  int n_seg;
+  int chunk_first;             // first chunk launched (global chunk index)
+  const int* chunk_k0;         // [n_chunks_launched] last k with e_k <= chunk start (-1 .. n_seg)
+  const int* node_n;           // [n_nodes][P_pad]
+  const double* node_frac;
+  const void* node_amp;        // R [n_nodes][4][P_pad]
+  const int* jlo; const int* jhi;
+  int P_pad;
+  double* frag;                // [n_chunks_launched][kFragFields][P_pad]
+  double* out_seg;             // SEG mode: [P][n_seg][3] (already offset to this batch), else nullptr
+  int P;                       // particles in this batch
+  double seg_scale_z, seg_scale_s;
+};
+
+template <typename R, bool SEG>
+__global__ void __launch_bounds__(kBlock) k_dense(DevCfg c, DenseArgs a, const typename DataT<R>::W* __restrict__ Wg,
+                                                  const typename DataT<R>::G* __restrict__ Gg) {
+  using WT = typename DataT<R>::W;
+  using GT = typename DataT<R>::G;
+  constexpr int CH = DataT<R>::chunk;
+  __shared__ WT sW[CH];
+  __shared__ GT sG[CH];
+
+  const int chunk_l = blockIdx.x;                              // launched-chunk index
+  const int cs = (a.chunk_first + chunk_l) * CH;
+  const int ce = min(cs + CH, c.n_bins);
+  const int p = blockIdx.y * kBlock + threadIdx.x;             // particle within the batch (P_pad is a multiple of kBlock)
+
+  for (int t = threadIdx.x; t < ce - cs; t += kBlock) { sW[t] = Wg[cs + t]; sG[t] = Gg[cs + t]; }
+  __syncthreads();
+
+  const int jlo = a.jlo[p], jhi = a.jhi[p];
+  const int S = c.stride, Sf = S >> 2;
+  const R hS = R(1.0) / R(Sf);
+  const R* __restrict__ namp = reinterpret_cast<const R*>(a.node_amp);
+
+  int k = a.chunk_k0[chunk_l];
+  int next_edge = (k + 1 <= a.n_seg) ? a.edges[k + 1] : INT_MAX;
+  bool open_at_edge = (k >= 0 && k < a.n_seg) ? (a.edges[k] == cs) : true;
+  double Zr = 0.0, Zi = 0.0, Sg = 0.0, ups = 0.0;
+  double* frag = a.frag + (size_t)chunk_l * kFragFields * a.P_pad + p;
+
+  auto close_piece = [&](bool at_edge_end) {
+    // at_edge_end: the piece ends at e_{k+1}.  open_at_edge: it began at e_k.
+    if (open_at_edge && at_edge_end) {
+      if (SEG) {
+        if (p < a.P) {
+          double* o = a.out_seg + ((size_t)p * a.n_seg + k) * 3;
+          o[0] = Zr * a.seg_scale_z; o[1] = Zi * a.seg_scale_z; o[2] = Sg * a.seg_scale_s;
+        }
+      } else if (Sg > 0.0) {
+        ups += (Zr * Zr + Zi * Zi) / Sg;
+      }
+    } else if (!open_at_edge) {          // began in an earlier chunk: head fragment (closed or running through)
+      frag[(size_t)1 * a.P_pad] = Zr; frag[(size_t)2 * a.P_pad] = Zi; frag[(size_t)3 * a.P_pad] = Sg;
+    } else {                             // began here, continues into the next chunk: tail fragment
+      frag[(size_t)4 * a.P_pad] = Zr; frag[(size_t)5 * a.P_pad] = Zi; frag[(size_t)6 * a.P_pad] = Sg;
+    }
+    Zr = 0.0; Zi = 0.0; Sg = 0.0;
+  };
+
+  int fd_pos = -1;                   // bin the forward-difference state is positioned at (-1: none)
+  double phi = 0.0, d1 = 0.0, d2 = 0.0, d3 = 0.0, d4 = 0.0, d5 = 0.0;
+  int quad = 0;
+  for (int ib = cs; ib < ce; ib += Sf) {
+    const int ie = min(ib + Sf, ce);
+    const bool lane_in = (ib >= jlo) && (ie <= jhi);
+    const bool lane_out = (ie <= jlo) || (ib >= jhi);
+    const bool all_in = __all_sync(0xffffffffu, lane_in);
+    const bool all_out = __all_sync(0xffffffffu, lane_out);
+
+    R cf[4][4];        // cubic coefficients of (Ar, Ai, Er, Ei) in t = (u - u_sub)/fine_stride
+    if (!all_out) {
+      const int ic = ib >> c.log2_stride;                      // coarse interval
+      const int i0 = ic + kNodeOff;                            // table row of its left node
+      const int q = (ib >> (c.log2_stride - 2)) & 3;           // fine sub-interval within the coarse one
+      if (fd_pos != ib || q == 0) {
+        // (re)build the phase forward differences at u0 = ib - ic*stride from the 6-node quintic
+        const size_t base = (size_t)i0 * a.P_pad + p;
+        const int n0 = a.node_n[base];
+        const double r0 = a.node_frac[base];
+        double Y[6];
+#pragma unroll
+        for (int m = -2; m <= 3; ++m) {
+          const size_t at = (size_t)(i0 + m) * a.P_pad + p;
+          Y[m + 2] = (double)(a.node_n[at] - n0) + (a.node_frac[at] - r0);
+        }
+        double b[6], d[6];
+        quintic_coeffs(Y, 1.0 / (double)S, b);
+        const int u0 = ib - (ic << c.log2_stride);
+        if (u0) taylor_shift(b, (double)u0);
+        forward_diffs(b, d);
+        phi = r0 + b[0]; d1 = d[1]; d2 = d[2]; d3 = d[3]; d4 = d[4]; d5 = d[5];
+        quad = 0;
+        fd_pos = ib;
+      }
+#pragma unroll
+      for (int r = 0; r < 4; ++r) {
+        const R* col = namp + ((size_t)i0 * 4 + r) * a.P_pad + p;
+        const ptrdiff_t st = (ptrdiff_t)4 * a.P_pad;
+        R nd[6];
+#pragma unroll
+        for (int m = -2; m <= 3; ++m) nd[m + 2] = col[m * st];
+        fine_cubic<R>(nd, q, cf[r][0], cf[r][1], cf[r][2], cf[r][3]);
+      }
+    }
+    R s = R(0.0);
+
+    // one bin: phase step + reduction (FP64), sincos, amplitude cubic, multiply-accumulate
+    auto bin = [&](int j, bool masked, R& zr, R& zi, R& sg) {
+      // reduce phi to |x| <= 1/8 turn, carrying the quadrant
+      const double t = fma(phi, 4.0, kMagic);
+      quad += __double2loint(t);
+      const double kf = t - kMagic;
+      phi = fma(kf, -0.25, phi);
+      R sn, cn;
+      sincos_2pi_small((R)phi, sn, cn);
+      // rotate by quad * 90 degrees
+      const bool swp = quad & 1;
+      R cr = swp ? sn : cn, sr = swp ? cn : sn;
+      cr = ((quad + 1) & 2) ? -cr : cr;
+      sr = (quad & 2) ? -sr : sr;
+      // advance the forward differences to the next bin
+      phi += d1; d1 += d2; d2 += d3; d3 += d4; d4 += d5;
+      // amplitudes
+      const R Ar = fma(fma(fma(cf[0][3], s, cf[0][2]), s, cf[0][1]), s, cf[0][0]);
+      const R Ai = fma(fma(fma(cf[1][3], s, cf[1][2]), s, cf[1][1]), s, cf[1][0]);
+      const R Er = fma(fma(fma(cf[2][3], s, cf[2][2]), s, cf[2][1]), s, cf[2][0]);
+      const R Ei = fma(fma(fma(cf[3][3], s, cf[3][2]), s, cf[3][1]), s, cf[3][0]);
+      s += hS;
+      const WT w = sW[j - cs];
+      const GT g = sG[j - cs];
+      // q = W_A conj(c_A) + W_E conj(c_E)
+      R qr = fma(w.x, Ar, fma(w.y, Ai, fma(w.z, Er, w.w * Ei)));
+      R qi = fma(w.y, Ar, fma(-w.x, Ai, fma(w.w, Er, -(w.z * Ei))));
+      R ss = fma(g.x, fma(Ar, Ar, Ai * Ai), g.y * fma(Er, Er, Ei * Ei));
+      if (masked) {
+        const bool in = (j >= jlo) && (j < jhi);
+        qr = in ? qr : R(0.0); qi = in ? qi : R(0.0); ss = in ? ss : R(0.0);
+      }
+      // z += q e^{+2 pi i Phi}
+      zr = fma(qr, cr, fma(-qi, sr, zr));
+      zi = fma(qr, sr, fma(qi, cr, zi));
+      sg += ss;
+    };
+
+    int j = ib;
+    while (j < ie) {
+      const int b = min(next_edge, ie);
+      const bool live = (k >= 0) && (k < a.n_seg);
+      if (b > j) {
+        if (all_out) {
+          // nothing to add; the forward-difference state is rebuilt at the next interval
+        } else if (!live) {
+          for (int jj = j; jj < b; ++jj) { phi += d1; d1 += d2; d2 += d3; d3 += d4; d4 += d5; s += hS; }
+          fd_pos = b;
+        } else {
+          for (int jj = j; jj < b;) {
+            const int e2 = min(jj + kFlushBins, b);
+            R zr = R(0.0), zi = R(0.0), sg = R(0.0);
+            if (all_in) { for (; jj < e2; ++jj) bin(jj, false, zr, zi, sg); }
+            else        { for (; jj < e2; ++jj) bin(jj, true, zr, zi, sg); }
+            Zr += (double)zr; Zi += (double)zi; Sg += (double)sg;
+          }
+          fd_pos = b;
+        }
+        j = b;
+      }
+      if (j == next_edge) {
+        if (live) close_piece(true);
+        ++k;
+        next_edge = (k + 1 <= a.n_seg) ? a.edges[k + 1] : INT_MAX;
+        open_at_edge = true;
+      }
+    }
+  }
+  // the piece still open at the chunk end
+  if (k >= 0 && k < a.n_seg) close_piece(false);
+  if (!SEG) frag[0] = ups;
+}
+
+// ------------------------------------------------------------------------------------------------ a6
+__global__ void k_stitch(const double* __restrict__ frag, const uint8_t* __restrict__ flags, int n_chunks, int P_pad,
+                         int P, double* __restrict__ out) {
+  const int p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= P) return;
+  double ups = 0.0, zr = 0.0, zi = 0.0, sg = 0.0;
+  for (int cI = 0; cI < n_chunks; ++cI) {
+    const double* f = frag + (size_t)cI * kFragFields * P_pad + p;
+    const uint8_t fl = flags[cI];
+    if (fl & CF_HEAD) {
+      zr += f[(size_t)1 * P_pad]; zi += f[(size_t)2 * P_pad]; sg += f[(size_t)3 * P_pad];
+      if (fl & CF_HEAD_CLOSES) {
+        if (sg > 0.0) ups += (zr * zr + zi * zi) / sg;
+        zr = 0.0; zi = 0.0; sg = 0.0;
+      }
+    }
+    ups += f[0];
+    if (fl & CF_TAIL) { zr = f[(size_t)4 * P_pad]; zi = f[(size_t)5 * P_pad]; sg = f[(size_t)6 * P_pad]; }
+  }
+  out[p] = ups;
+}
+
+__global__ void k_stitch_seg(const double* __restrict__ frag, const uint8_t* __restrict__ flags,
+                             const int* __restrict__ chunk_k0, int n_chunks, int P_pad, int P, int n_seg,
+                             double sz, double ss, double* __restrict__ out_seg) {
+  const int p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= P) return;
+  double zr = 0.0, zi = 0.0, sg = 0.0;
+  for (int cI = 0; cI < n_chunks; ++cI) {
+    const double* f = frag + (size_t)cI * kFragFields * P_pad + p;
+    const uint8_t fl = flags[cI];
+    if (fl & CF_HEAD) {
+      zr += f[(size_t)1 * P_pad]; zi += f[(size_t)2 * P_pad]; sg += f[(size_t)3 * P_pad];
+      if (fl & CF_HEAD_CLOSES) {
+        double* o = out_seg + ((size_t)p * n_seg + chunk_k0[cI]) * 3;
+        o[0] = zr * sz; o[1] = zi * sz; o[2] = sg * ss;
+        zr = 0.0; zi = 0.0; sg = 0.0;
+      }
+    }
+    if (fl & CF_TAIL) { zr = f[(size_t)4 * P_pad]; zi = f[(size_t)5 * P_pad]; sg = f[(size_t)6 * P_pad]; }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------ template generation
+// h_alpha(f_j) through the same node tables and interpolants (polynomials evaluated directly instead of by
+// forward differences).  One thread per (bin, template).
+__global__ void k_template(DevCfg c, const int* __restrict__ node_n, const double* __restrict__ node_frac,
+                           const double* __restrict__ node_amp, const int* __restrict__ jlo, const int* __restrict__ jhi,
+                           int P_pad, int P, double amp_scale, double* __restrict__ hA, double* __restrict__ hE) {
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  const int p = blockIdx.y;
+  if (j >= c.n_bins || p >= P) return;
+  double2 oA = make_double2(0.0, 0.0), oE = oA;
+  if (j >= jlo[p] && j < jhi[p]) {
+    const int i0 = (j >> c.log2_stride) + kNodeOff;
+    const double u = (double)(j - ((j >> c.log2_stride) << c.log2_stride));
+    const size_t base = (size_t)i0 * P_pad + p;
+    const int n0 = node_n[base];
+    const double r0 = node_frac[base];
+    double Y[6], b[6];
+    for (int m = -2; m <= 3; ++m) {
+      const size_t at = (size_t)(i0 + m) * P_pad + p;
+      Y[m + 2] = (double)(node_n[at] - n0) + (node_frac[at] - r0);
+    }
+    quintic_coeffs(Y, 1.0 / (double)c.stride, b);
+    double phi = r0 + u * (b[1] + u * (b[2] + u * (b[3] + u * (b[4] + u * b[5]))));
+    phi -= rint(phi);
+    double sn, cn;
+    sincospi(2.0 * phi, &sn, &cn);
+    const int Sf = c.stride >> 2;
+    const int q = (int)u / Sf;
+    const double s = (u - (double)(q * Sf)) / (double)Sf;
+    double v[4];
+    for (int r = 0; r < 4; ++r) {
+      const double* col = node_amp + ((size_t)i0 * 4 + r) * P_pad + p;
+      const ptrdiff_t st = (ptrdiff_t)4 * P_pad;
+      double nd[6];
+      for (int m = -2; m <= 3; ++m) nd[m + 2] = col[m * st];
+      double a0, a1, a2, a3;
+      fine_cubic<double>(nd, q, a0, a1, a2, a3);
+      v[r] = (a0 + s * (a1 + s * (a2 + s * a3))) * amp_scale;
+    }
+    // h = amp * e^{-2 pi i Phi}
+    oA = make_double2(v[0] * cn + v[1] * sn, v[1] * cn - v[0] * sn);
+    oE = make_double2(v[2] * cn + v[3] * sn, v[3] * cn - v[2] * sn);
+  }
+  reinterpret_cast<double2*>(hA)[(size_t)p * c.n_bins + j] = oA;
+  reinterpret_cast<double2*>(hE)[(size_t)p * c.n_bins + j] = oE;
+}
+
+// ------------------------------------------------------------------------------------------------ a7 PSO
+// (1)+(2): one CTA per swarm.
+__global__ void k_pso_best(const double* __restrict__ pos, double* __restrict__ pbest_pos, double* __restrict__ pbest_val,
+                           const double* __restrict__ stat, double* __restrict__ gbest_pos, double* __restrict__ gbest_val,
+                           int per_swarm) {
+  const int s = blockIdx.x;
+  const long long p0 = (long long)s * per_swarm;
+  double best = -INFINITY;
+  long long besti = LLONG_MAX;
+  bool any = false;
+  for (int t = threadIdx.x; t < per_swarm; t += blockDim.x) {
+    const long long p = p0 + t;
+    double pv = pbest_val[p];
+    const double st = stat[p];
+    if (st > pv) {
+      pv = st;
+      pbest_val[p] = st;
+#pragma unroll
+      for (int m = 0; m < 8; ++m) pbest_pos[p * 8 + m] = pos[p * 8 + m];
+    }
+    // arg max with lowest index on ties; NaN never wins; the first element seeds the comparison like a serial scan
+    if (!any || pv > best) { best = pv; besti = p; any = true; }
+  }
+  __shared__ double sv[32];
+  __shared__ long long si[32];
+  __shared__ int sa[32];
+  // serial-scan semantics: candidate (v, i) beats (w, j) if v > w, or (v == w or both not comparable) and i < j.
+  auto better = [](double v, long long i, bool av, double w, long long j, bool aw) {
+    if (!aw) return av;
+    if (!av) return false;
+    if (v > w) return true;
+    if (w > v) return false;
+    return i < j;
+  };
+  for (int o = 16; o > 0; o >>= 1) {
+    const double ov = __shfl_xor_sync(0xffffffffu, best, o);
+    const long long oi = __shfl_xor_sync(0xffffffffu, besti, o);
+    const int oa = __shfl_xor_sync(0xffffffffu, (int)any, o);
+    if (better(ov, oi, oa, best, besti, any)) { best = ov; besti = oi; any = oa; }
+  }
+  const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+  if (l == 0) { sv[w] = best; si[w] = besti; sa[w] = any; }
+  __syncthreads();
+  if (w == 0) {
+    const int nw = (blockDim.x + 31) >> 5;
+    best = (l < nw) ? sv[l] : -INFINITY; besti = (l < nw) ? si[l] : LLONG_MAX; any = (l < nw) ? sa[l] : false;
+    for (int o = 16; o > 0; o >>= 1) {
+      const double ov = __shfl_xor_sync(0xffffffffu, best, o);
+      const long long oi = __shfl_xor_sync(0xffffffffu, besti, o);
+      const int oa = __shfl_xor_sync(0xffffffffu, (int)any, o);
+      if (better(ov, oi, oa, best, besti, any)) { best = ov; besti = oi; any = oa; }
+    }
+    if (l == 0) { si[0] = besti; }
+  }
+  __syncthreads();
+  const long long bi = si[0];
+  if (threadIdx.x < 8) gbest_pos[s * 8 + threadIdx.x] = pbest_pos[bi * 8 + threadIdx.x];
+  if (threadIdx.x == 8) gbest_val[s] = pbest_val[bi];
+}
+
+// (3)-(6): one thread per particle.
+__global__ void k_pso_move(double* __restrict__ pos, double* __restrict__ vel, const double* __restrict__ pbest_pos,
+                           const double* __restrict__ gbest_pos, const double* __restrict__ lo, const double* __restrict__ hi,
+                           const double* __restrict__ eps_min, double omega, double phi_p, double phi_g,
+                           uint64_t seed, uint64_t iter, long long P, int per_swarm) {
+  const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= P) return;
+  const int s = (int)(p / per_swarm);
+  uint32_t w[16];
+#pragma unroll
+  for (uint32_t b = 0; b < 4; ++b)
+    philox4x32_10((uint32_t)p, (uint32_t)iter, b, 0u, (uint32_t)seed, (uint32_t)(seed >> 32), w + 4 * b);
+#pragma unroll
+  for (int m = 0; m < 8; ++m) {
+    const double rP = ((double)w[m] + 0.5) * 0x1p-32, rG = ((double)w[8 + m] + 0.5) * 0x1p-32;
+    const double th = pos[p * 8 + m];
+    // Eq. 14, same association as written: (Omega v + Phi_P r_P (Psi - theta)) + Phi_G r_G (Xi - theta), no contraction
+    const double t1 = __dmul_rn(omega, vel[p * 8 + m]);
+    const double t2 = __dmul_rn(__dmul_rn(phi_p, rP), __dsub_rn(pbest_pos[p * 8 + m], th));
+    const double t3 = __dmul_rn(__dmul_rn(phi_g, rG), __dsub_rn(gbest_pos[s * 8 + m], th));
+    const double u = __dadd_rn(__dadd_rn(t1, t2), t3);
+    const double au = fabs(u), eps = eps_min[m];
+    double v;
+    if (au > 0.0) v = (eps > au ? eps : au) * (u / au);      // Eq. 15
+    else v = (eps > 0.0) ? eps : 0.0;                        // Q9: sign(0) = +1
+    double x = th + v;                                       // Eq. 13
+    if (x < lo[m]) { x = lo[m]; v = -v; }                    // Q9: reflect
+    else if (x > hi[m]) { x = hi[m]; v = -v; }
+    pos[p * 8 + m] = x;
+    vel[p * 8 + m] = v;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------ host side
+thread_local std::string g_init_error;
+
+}  // namespace
+
+struct sc_handle {
+  sc_config cfg;
+  DevCfg dc;
+  int device = 0;
+  double s0 = 1.0;                 // weight scale (power of two)
+  float4* W32 = nullptr; float2* G32 = nullptr; double4* W64 = nullptr; double2* G64 = nullptr;
+  // options
+  int precision = 0; int f32_min_seg = 8; size_t scratch_cap = (size_t)8 << 30;
+  double tc_max_s = 10.0 * 31557600.0; int forced_stride_log2 = 0;
+  // scratch
+  void* scratch = nullptr; size_t scratch_bytes = 0;
+  int* d_edges = nullptr; int* d_chunk_k0 = nullptr; uint8_t* d_flags = nullptr; size_t edge_cap = 0, k0_cap = 0, flags_cap = 0;
+  unsigned long long* d_counter = nullptr;
+  double* d_params_stage = nullptr; double* d_out_stage = nullptr; size_t stage_cap = 0;
+  // cached edge analysis
+  std::vector<int> edges; int cached_chunk = 0; int chunk_first = 0, n_chunks = 0;
+  std::vector<int> chunk_k0; std::vector<uint8_t> flags;
+  long long launches = 0;
+  bool cuda_failed = false;
+  std::string err;
+};
+
+namespace {
+
+int fail(sc_handle* h, int code, const char* fmt, ...);
+int pick_stride_log2(const sc_config& cfg, double tc_max_s, int forced);
+
+void set_stride(sc_handle* h) {
+  DevCfg& d = h->dc;
+  d.log2_stride = pick_stride_log2(h->cfg, h->tc_max_s, h->forced_stride_log2);
+  d.stride = 1 << d.log2_stride;
+  const int n_int = (d.n_bins + d.stride - 1) / d.stride;
+  d.n_nodes = n_int + kNodeOff + 4;
+}
+
+int fail(sc_handle* h, int code, const char* fmt, ...) {
+  char buf[512];
+  va_list ap; va_start(ap, fmt); vsnprintf(buf, sizeof buf, fmt, ap); va_end(ap);
+  if (h) { h->err = buf; if (code == SC_ERR_CUDA) h->cuda_failed = true; }
+  else g_init_error = buf;
+  return code;
+}
+
+#define SC_CUDA(h, call)                                                                         \
+  do { cudaError_t e_ = (call);                                                                  \
+       if (e_ != cudaSuccess) return fail((h), e_ == cudaErrorMemoryAllocation ? SC_ERR_OOM : SC_ERR_CUDA, \
+                                          "%s failed: %s", #call, cudaGetErrorString(e_)); } while (0)
+
+int check_launch(sc_handle* h, const char* what) {
+  h->launches++;
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(h, SC_ERR_CUDA, "launch of %s failed: %s", what, cudaGetErrorString(e));
+  return SC_OK;
+}
+
+// Coarse node spacing: the slowly varying amplitudes change on the orbital time scale,
+// so the spacing is set in TIME: about one day at the slowest-chirping corner of the problem.  Time per bin is
+// |dt/df| df = (8/3) tau / (f T_obs) with tau <= tc_max (Newtonian), largest at the low band edge.
+int pick_stride_log2(const sc_config& cfg, double tc_max_s, int forced) {
+  if (forced > 0) return std::min(std::max(forced, 2), 12);
+  const double f_lo = (double)std::max<int64_t>(cfg.j0, 1) / cfg.T_obs_s;
+  const double s_per_bin = (8.0 / 3.0) * tc_max_s / (f_lo * cfg.T_obs_s);
+  int lg = 5;
+  while (lg < 10 && (double)(2 << lg) * s_per_bin <= 86400.0) ++lg;
+  return lg;
+}
+
+
+
+int grow(sc_handle* h, void** ptr, size_t* cap, size_t need) {
+  if (*cap >= need) return SC_OK;
+  if (*ptr) { cudaFree(*ptr); *ptr = nullptr; *cap = 0; }
+  SC_CUDA(h, cudaMalloc(ptr, need));
+  *cap = need;
+  return SC_OK;
+}
+
+// Host analysis of the edge list for a given chunk length: which chunks are launched, the segment each one
+// starts in, and which fragments each chunk leaves (shared by all particles, Q2).
+void analyse_edges(sc_handle* h, int CH) {
+  const std::vector<int>& e = h->edges;
+  const int n_seg = (int)e.size() - 1;
+  h->cached_chunk = CH;
+  h->chunk_k0.clear(); h->flags.clear();
+  h->chunk_first = 0; h->n_chunks = 0;
+  if (e[n_seg] <= e[0]) return;
+  h->chunk_first = e[0] / CH;
+  const int chunk_last = (e[n_seg] - 1) / CH;
+  h->n_chunks = chunk_last - h->chunk_first + 1;
+  for (int cI = 0; cI < h->n_chunks; ++cI) {
+    const int cs = (h->chunk_first + cI) * CH;
+    const int ce = std::min(cs + CH, (int)h->cfg.n_bins);
+    const int k0 = (int)(std::upper_bound(e.begin(), e.end(), cs) - e.begin()) - 1;   // last k with e_k <= cs
+    uint8_t fl = 0;
+    if (k0 >= 0 && k0 < n_seg && e[k0] < cs) {
+      fl |= CF_HEAD;
+      if (e[k0 + 1] <= ce) fl |= CF_HEAD_CLOSES;
+    }
+    // the piece open at the chunk end belongs to segment kt = last k with e_k < ce; it is a tail if it began here
+    const int kt = (int)(std::lower_bound(e.begin(), e.end(), ce) - e.begin()) - 1;
+    if (kt >= 0 && kt < n_seg && e[kt + 1] > ce && e[kt] >= cs) fl |= CF_TAIL;
+    h->chunk_k0.push_back(k0);
+    h->flags.push_back(fl);
+  }
+}
+
+template <typename R>
+int run_batches(sc_handle* h, const double* params, int64_t P, double* out, double* out_seg, cudaStream_t st,
+                bool seg_mode) {
+  constexpr int CH = DataT<R>::chunk;
+  const int n_seg = (int)h->edges.size() - 1;
+  const DevCfg& dc = h->dc;
+  const int n_nodes = dc.n_nodes;
+  const int n_chunks = h->n_chunks;
+  // per-particle scratch bytes
+  const size_t per_p = (size_t)kPcFields * 8 + 8 /* jlo, jhi */ + (size_t)n_nodes * (4 + 8 + 4 * sizeof(R))
+                       + (size_t)std::max(n_chunks, 1) * kFragFields * 8;
+  int64_t Pb_max = (int64_t)(h->scratch_cap / per_p) / kBlock * kBlock;
+  if (Pb_max < kBlock) Pb_max = kBlock;
+  const int64_t P_round = (P + kBlock - 1) / kBlock * kBlock;
+  const int P_pad = (int)std::min<int64_t>(Pb_max, P_round);
+  int rc = grow(h, &h->scratch, &h->scratch_bytes, per_p * (size_t)P_pad + 1024);
+  if (rc) return rc;
+  // carve
+  char* base = (char*)h->scratch;
+  auto take = [&](size_t bytes) { char* r = base; base += (bytes + 255) / 256 * 256; return r; };
+  double* pc = (double*)take((size_t)kPcFields * 8 * P_pad);
+  int* jlo = (int*)take((size_t)4 * P_pad);
+  int* jhi = (int*)take((size_t)4 * P_pad);
+  int* node_n = (int*)take((size_t)n_nodes * 4 * P_pad);
+  double* node_frac = (double*)take((size_t)n_nodes * 8 * P_pad);
+  R* node_amp = (R*)take((size_t)n_nodes * 4 * sizeof(R) * P_pad);
+  double* frag = (double*)take((size_t)std::max(n_chunks, 1) * kFragFields * 8 * P_pad);
+  (void)base;
+
+  const int e_first = h->edges.front(), e_last = h->edges.back();
+  const double four_df = 4.0 / h->cfg.T_obs_s;
+  const double h0 = pow(dc.f_amp_ref, -7.0 / 6.0);
+  const double sz = h->s0 * h0 / four_df, ss = h->s0 * h->s0 * h0 * h0 / four_df;
+
+  for (int64_t pb = 0; pb < P; pb += P_pad) {
+    const int Pn = (int)std::min<int64_t>(P_pad, P - pb);
+    k_particle_consts<<<(P_pad + 127) / 128, 128, 0, st>>>(dc, params + pb * 8, Pn, P_pad, pc, jlo, jhi, e_first, e_last,
+                                                          h->d_counter);
+    if ((rc = check_launch(h, "k_particle_consts"))) return rc;
+    if (n_chunks == 0) {
+      if (!seg_mode) SC_CUDA(h, cudaMemsetAsync(out + pb, 0, (size_t)Pn * 8, st));
+      continue;
+    }
+    k_nodes<R><<<dim3((P_pad + 127) / 128, n_nodes), 128, 0, st>>>(dc, pc, jlo, jhi, P_pad, node_n, node_frac, node_amp);
+    if ((rc = check_launch(h, "k_nodes"))) return rc;
+    DenseArgs a;
+    a.edges = h->d_edges; a.n_seg = n_seg; a.chunk_first = h->chunk_first; a.chunk_k0 = h->d_chunk_k0;
+    a.node_n = node_n; a.node_frac = node_frac; a.node_amp = node_amp; a.jlo = jlo; a.jhi = jhi; a.P_pad = P_pad;
+    a.frag = frag; a.out_seg = seg_mode ? out_seg + (size_t)pb * n_seg * 3 : nullptr; a.P = Pn;
+    a.seg_scale_z = sz; a.seg_scale_s = ss;
+    const dim3 grid(n_chunks, P_pad / kBlock);
+    if (seg_mode) k_dense<R, true><<<grid, kBlock, 0, st>>>(dc, a, (const typename DataT<R>::W*)(sizeof(R) == 4 ? (void*)h->W32 : (void*)h->W64),
+                                                            (const typename DataT<R>::G*)(sizeof(R) == 4 ? (void*)h->G32 : (void*)h->G64));
+    else k_dense<R, false><<<grid, kBlock, 0, st>>>(dc, a, (const typename DataT<R>::W*)(sizeof(R) == 4 ? (void*)h->W32 : (void*)h->W64),
+                                                    (const typename DataT<R>::G*)(sizeof(R) == 4 ? (void*)h->G32 : (void*)h->G64));
+    if ((rc = check_launch(h, "k_dense"))) return rc;
+    if (seg_mode) k_stitch_seg<<<(Pn + 127) / 128, 128, 0, st>>>(frag, h->d_flags, h->d_chunk_k0, n_chunks, P_pad, Pn, n_seg, sz, ss,
+                                                                out_seg + (size_t)pb * n_seg * 3);
+    else k_stitch<<<(Pn + 127) / 128, 128, 0, st>>>(frag, h->d_flags, n_chunks, P_pad, Pn, out + pb);
+    if ((rc = check_launch(h, "k_stitch"))) return rc;
+  }
+  return SC_OK;
+}
+
+int prepare_edges(sc_handle* h, const int32_t* seg_edges, int32_t n_seg, int CH, cudaStream_t st) {
+  if (!seg_edges || n_seg <= 0) return fail(h, SC_ERR_INVALID_ARG, "seg_edges is null or n_seg <= 0");
+  std::vector<int> e((size_t)n_seg + 1);
+  cudaPointerAttributes at;
+  cudaError_t pe = cudaPointerGetAttributes(&at, seg_edges);
+  if (pe != cudaSuccess) { cudaGetLastError(); at.type = cudaMemoryTypeUnregistered; }
+  if (at.type == cudaMemoryTypeDevice) {
+    SC_CUDA(h, cudaMemcpyAsync(e.data(), seg_edges, e.size() * 4, cudaMemcpyDeviceToHost, st));
+    SC_CUDA(h, cudaStreamSynchronize(st));
+  } else {
+    memcpy(e.data(), seg_edges, e.size() * 4);
+  }
+  if (e[0] < 0 || e[n_seg] > h->cfg.n_bins) return fail(h, SC_ERR_INVALID_ARG, "seg_edges outside [0, n_bins]");
+  for (int k = 0; k < n_seg; ++k)
+    if (e[k + 1] < e[k]) return fail(h, SC_ERR_INVALID_ARG, "seg_edges not non-decreasing at k=%d", k);
+  if (e == h->edges && CH == h->cached_chunk) return SC_OK;
+  h->edges.swap(e);
+  analyse_edges(h, CH);
+  int rc;
+  if ((rc = grow(h, (void**)&h->d_edges, &h->edge_cap, h->edges.size() * 4))) return rc;
+  if ((rc = grow(h, (void**)&h->d_chunk_k0, &h->k0_cap, (size_t)std::max(h->n_chunks, 1) * 4))) return rc;
+  if ((rc = grow(h, (void**)&h->d_flags, &h->flags_cap, (size_t)std::max(h->n_chunks, 1)))) return rc;
+  SC_CUDA(h, cudaMemcpyAsync(h->d_edges, h->edges.data(), h->edges.size() * 4, cudaMemcpyHostToDevice, st));
+  if (h->n_chunks > 0) {
+    SC_CUDA(h, cudaMemcpyAsync(h->d_chunk_k0, h->chunk_k0.data(), (size_t)h->n_chunks * 4, cudaMemcpyHostToDevice, st));
+    SC_CUDA(h, cudaMemcpyAsync(h->d_flags, h->flags.data(), (size_t)h->n_chunks, cudaMemcpyHostToDevice, st));
+  }
+  return SC_OK;
+}
+
+int eval_common(sc_handle* h, const double* params, int64_t P, const int32_t* seg_edges, int32_t n_seg,
+                double* out, double* out_seg, void* stream, bool seg_mode) {
+  if (!h) return SC_ERR_NOT_INIT;
+  if (h->cuda_failed) return SC_ERR_CUDA;
+  if (!params || P <= 0 || (!seg_mode && !out) || (seg_mode && !out_seg))
+    return fail(h, SC_ERR_INVALID_ARG, "null pointer or n_particles <= 0");
+  cudaStream_t st = (cudaStream_t)stream;
+  const bool f64 = (h->precision == 2) || (h->precision == 0 && n_seg < h->f32_min_seg);
+  int rc = prepare_edges(h, seg_edges, n_seg, f64 ? kChunkF64 : kChunkF32, st);
+  if (rc) return rc;
+  SC_CUDA(h, cudaMemsetAsync(h->d_counter, 0, 8, st));
+  if (seg_mode) SC_CUDA(h, cudaMemsetAsync(out_seg, 0, (size_t)P * n_seg * 3 * 8, st));
+  return f64 ? run_batches<double>(h, params, P, out, out_seg, st, seg_mode)
+             : run_batches<float>(h, params, P, out, out_seg, st, seg_mode);
+}
+
+int init_common(sc_handle** out, const sc_config* cfg, const double* dA, const double* dE, const double* S_A,
+                const double* S_E, void* stream, bool host_inputs) {
+  if (!out) return fail(nullptr, SC_ERR_INVALID_ARG, "out is null");
+  *out = nullptr;
+  if (!cfg || !dA || !dE || !S_A || !S_E) return fail(nullptr, SC_ERR_INVALID_ARG, "null pointer");
+  if (!(cfg->T_obs_s > 0.0) || cfg->n_bins < 1 || cfg->n_bins >= (int64_t)1 << 31 || cfg->j0 < 0)
+    return fail(nullptr, SC_ERR_INVALID_ARG, "bad grid (T_obs_s, j0, n_bins)");
+  if (cfg->n_channels != 2) return fail(nullptr, SC_ERR_INVALID_ARG, "n_channels must be 2 (A,E); T is reserved");
+  if (cfg->pn_order_x2 < 0 || cfg->pn_order_x2 > 7) return fail(nullptr, SC_ERR_INVALID_ARG, "pn_order_x2 must be 0..7");
+  if (cfg->window_mode != 0 && cfg->window_mode != 1) return fail(nullptr, SC_ERR_INVALID_ARG, "window_mode must be 0 or 1");
+  if (!(cfg->arm_L_s > 0.0) || !(cfg->au_s > 0.0) || !(cfg->year_s > 0.0))
+    return fail(nullptr, SC_ERR_INVALID_ARG, "orbit constants must be positive");
+  int ndev = 0;
+  cudaError_t e = cudaGetDeviceCount(&ndev);
+  if (e != cudaSuccess || ndev == 0) {
+    cudaGetLastError();
+    return fail(nullptr, SC_ERR_CUDA, "no CUDA device (%s); this library has no CPU fallback",
+                e == cudaSuccess ? "device count 0" : cudaGetErrorString(e));
+  }
+  sc_handle* h = new sc_handle();
+  h->cfg = *cfg;
+  cudaStream_t st = (cudaStream_t)stream;
+  const int n = (int)cfg->n_bins;
+  DevCfg& d = h->dc;
+  d.T_obs = cfg->T_obs_s; d.inv_T = 1.0 / cfg->T_obs_s; d.j0 = cfg->j0; d.n_bins = n;
+  d.window_mode = cfg->window_mode; d.pn_order_x2 = cfg->pn_order_x2; d.ecc_leading = cfg->ecc_leading;
+  d.f_ref_ecc = cfg->f_ref_ecc; d.L = cfg->arm_L_s; d.AU = cfg->au_s; d.alpha0 = cfg->orbit_alpha0; d.year = cfg->year_s;
+  for (int m = 0; m < 3; ++m) {
+    const double b = 2.0 * kPi * m / 3.0 + cfg->orbit_lambda0;
+    d.sbn[m] = sin(b); d.cbn[m] = cos(b);
+  }
+  d.f_amp_ref = (double)std::max<int64_t>(cfg->j0, 1) / cfg->T_obs_s;
+  set_stride(h);
+  auto bail = [&](int code) { sc_free(h); return code; };
+#define SC_INIT(call)                                                                              \
+  do { cudaError_t e_ = (call);                                                                    \
+       if (e_ != cudaSuccess) { fail(nullptr, e_ == cudaErrorMemoryAllocation ? SC_ERR_OOM : SC_ERR_CUDA, \
+                                     "%s failed: %s", #call, cudaGetErrorString(e_));              \
+                                return bail(e_ == cudaErrorMemoryAllocation ? SC_ERR_OOM : SC_ERR_CUDA); } } while (0)
+  SC_INIT(cudaGetDevice(&h->device));
+  SC_INIT(cudaMalloc(&h->W32, (size_t)n * sizeof(float4)));
+  SC_INIT(cudaMalloc(&h->G32, (size_t)n * sizeof(float2)));
+  SC_INIT(cudaMalloc(&h->W64, (size_t)n * sizeof(double4)));
+  SC_INIT(cudaMalloc(&h->G64, (size_t)n * sizeof(double2)));
+  SC_INIT(cudaMalloc(&h->d_counter, 16));
+  SC_INIT(cudaMemsetAsync(h->d_counter, 0, 16, st));
+  double* stage = nullptr;
+  const double *pA = dA, *pE = dE, *pSA = S_A, *pSE = S_E;
+  if (host_inputs) {
+    SC_INIT(cudaMalloc(&stage, (size_t)n * 6 * 8));
+    SC_INIT(cudaMemcpyAsync(stage, dA, (size_t)n * 16, cudaMemcpyHostToDevice, st));
+    SC_INIT(cudaMemcpyAsync(stage + 2 * (size_t)n, dE, (size_t)n * 16, cudaMemcpyHostToDevice, st));
+    SC_INIT(cudaMemcpyAsync(stage + 4 * (size_t)n, S_A, (size_t)n * 8, cudaMemcpyHostToDevice, st));
+    SC_INIT(cudaMemcpyAsync(stage + 5 * (size_t)n, S_E, (size_t)n * 8, cudaMemcpyHostToDevice, st));
+    pA = stage; pE = stage + 2 * (size_t)n; pSA = stage + 4 * (size_t)n; pSE = stage + 5 * (size_t)n;
+  }
+  const double four_df = 4.0 / cfg->T_obs_s;
+  k_max_weight<<<std::min((n + 255) / 256, 1184), 256, 0, st>>>(pSA, pSE, n, four_df, h->d_counter + 1);
+  h->launches++;
+  unsigned long long bits = 0;
+  SC_INIT(cudaMemcpyAsync(&bits, h->d_counter + 1, 8, cudaMemcpyDeviceToHost, st));
+  SC_INIT(cudaStreamSynchronize(st));
+  double umax;
+  memcpy(&umax, &bits, 8);
+  int ex = 0;
+  if (umax > 0.0 && std::isfinite(umax)) { frexp(umax, &ex); }       // umax = m 2^ex, m in [0.5, 1)
+  h->s0 = ldexp(1.0, (ex + 1) / 2);                                   // s0^2 >= umax, power of two
+  k_whiten<<<(n + 255) / 256, 256, 0, st>>>(pA, pE, pSA, pSE, n, four_df, 1.0 / h->s0, h->W32, h->G32, h->W64, h->G64);
+  h->launches++;
+  SC_INIT(cudaGetLastError());
+  if (stage) { SC_INIT(cudaStreamSynchronize(st)); cudaFree(stage); }
+#undef SC_INIT
+  *out = h;
+  return SC_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int sc_init_data(sc_handle** out, const sc_config* cfg, const double* dA, const double* dE, const double* S_A,
+                 const double* S_E, void* stream) {
+  return init_common(out, cfg, dA, dE, S_A, S_E, stream, false);
+}
+
+int sc_init_data_host(sc_handle** out, const sc_config* cfg, const double* dA, const double* dE, const double* S_A,
+                      const double* S_E, void* stream) {
+  return init_common(out, cfg, dA, dE, S_A, S_E, stream, true);
+}
+
+int sc_eval_stat(sc_handle* h, const double* params, int64_t P, const int32_t* seg_edges, int32_t n_seg, double* out,
+                 void* stream) {
+  return eval_common(h, params, P, seg_edges, n_seg, out, nullptr, stream, false);
+}
+
+int sc_eval_segments(sc_handle* h, const double* params, int64_t P, const int32_t* seg_edges, int32_t n_seg,
+                     double* out_seg, void* stream) {
+  return eval_common(h, params, P, seg_edges, n_seg, nullptr, out_seg, stream, true);
+}
+
+int sc_eval_stat_host(sc_handle* h, const double* params, int64_t P, const int32_t* seg_edges, int32_t n_seg,
+                      double* out, void* stream) {
+  if (!h) return SC_ERR_NOT_INIT;
+  if (h->cuda_failed) return SC_ERR_CUDA;
+  if (!params || !out || P <= 0) return fail(h, SC_ERR_INVALID_ARG, "null pointer or n_particles <= 0");
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t need = (size_t)P * 9 * 8;
+  if (h->stage_cap < need) {
+    if (h->d_params_stage) cudaFree(h->d_params_stage);
+    h->d_params_stage = nullptr; h->stage_cap = 0;
+    SC_CUDA(h, cudaMalloc(&h->d_params_stage, need));
+    h->stage_cap = need;
+  }
+  h->d_out_stage = h->d_params_stage + (size_t)P * 8;
+  SC_CUDA(h, cudaMemcpyAsync(h->d_params_stage, params, (size_t)P * 64, cudaMemcpyHostToDevice, st));
+  int rc = eval_common(h, h->d_params_stage, P, seg_edges, n_seg, h->d_out_stage, nullptr, stream, false);
+  if (rc) return rc;
+  SC_CUDA(h, cudaMemcpyAsync(out, h->d_out_stage, (size_t)P * 8, cudaMemcpyDeviceToHost, st));
+  SC_CUDA(h, cudaStreamSynchronize(st));
+  return SC_OK;
+}
+
+int sc_gen_template(sc_handle* h, const double* params, int64_t P, double* hA, double* hE, void* stream) {
+  if (!h) return SC_ERR_NOT_INIT;
+  if (h->cuda_failed) return SC_ERR_CUDA;
+  if (!params || !hA || !hE || P <= 0) return fail(h, SC_ERR_INVALID_ARG, "null pointer or n_templates <= 0");
+  cudaStream_t st = (cudaStream_t)stream;
+  const DevCfg& dc = h->dc;
+  const int n_nodes = dc.n_nodes;
+  const int P_pad = kBlock;       // templates are generated kBlock at a time
+  const size_t per_p = (size_t)kPcFields * 8 + 8 + (size_t)n_nodes * (4 + 8 + 32);
+  int rc = grow(h, &h->scratch, &h->scratch_bytes, per_p * (size_t)P_pad + 8192);
+  if (rc) return rc;
+  char* base = (char*)h->scratch;
+  auto take = [&](size_t bytes) { char* r = base; base += (bytes + 255) / 256 * 256; return r; };
+  double* pc = (double*)take((size_t)kPcFields * 8 * P_pad);
+  int* jlo = (int*)take((size_t)4 * P_pad);
+  int* jhi = (int*)take((size_t)4 * P_pad);
+  int* node_n = (int*)take((size_t)n_nodes * 4 * P_pad);
+  double* node_frac = (double*)take((size_t)n_nodes * 8 * P_pad);
+  double* node_amp = (double*)take((size_t)n_nodes * 32 * P_pad);
+  const double h0 = pow(dc.f_amp_ref, -7.0 / 6.0);
+  for (int64_t pb = 0; pb < P; pb += P_pad) {
+    const int Pn = (int)std::min<int64_t>(P_pad, P - pb);
+    k_particle_consts<<<1, kBlock, 0, st>>>(dc, params + pb * 8, Pn, P_pad, pc, jlo, jhi, 0, 0, h->d_counter);
+    if ((rc = check_launch(h, "k_particle_consts"))) return rc;
+    k_nodes<double><<<dim3(1, n_nodes), kBlock, 0, st>>>(dc, pc, jlo, jhi, P_pad, node_n, node_frac, node_amp);
+    if ((rc = check_launch(h, "k_nodes"))) return rc;
+    k_template<<<dim3((dc.n_bins + 255) / 256, Pn), 256, 0, st>>>(dc, node_n, node_frac, node_amp, jlo, jhi, P_pad, Pn, h0,
+                                                                 hA + (size_t)pb * dc.n_bins * 2, hE + (size_t)pb * dc.n_bins * 2);
+    if ((rc = check_launch(h, "k_template"))) return rc;
+  }
+  return SC_OK;
+}
+
+int sc_pso_step(sc_handle* h, double* pos, double* vel, double* pbest_pos, double* pbest_val, const double* stat,
+                double* gbest_pos, double* gbest_val, const double* lo, const double* hi, const double* eps_min,
+                double omega, double phi_p, double phi_g, uint64_t seed, uint64_t iter, int64_t P, int32_t n_swarms,
+                void* stream) {
+  if (!h) return SC_ERR_NOT_INIT;
+  if (h->cuda_failed) return SC_ERR_CUDA;
+  if (!pos || !vel || !pbest_pos || !pbest_val || !stat || !gbest_pos || !gbest_val || !lo || !hi || !eps_min)
+    return fail(h, SC_ERR_INVALID_ARG, "null pointer");
+  if (P <= 0 || n_swarms <= 0 || P % n_swarms != 0 || P / n_swarms > INT32_MAX)
+    return fail(h, SC_ERR_INVALID_ARG, "n_particles must be a positive multiple of n_swarms");
+  cudaStream_t st = (cudaStream_t)stream;
+  const int per = (int)(P / n_swarms);
+  int rc;
+  k_pso_best<<<n_swarms, 1024, 0, st>>>(pos, pbest_pos, pbest_val, stat, gbest_pos, gbest_val, per);
+  if ((rc = check_launch(h, "k_pso_best"))) return rc;
+  k_pso_move<<<(unsigned)((P + 127) / 128), 128, 0, st>>>(pos, vel, pbest_pos, gbest_pos, lo, hi, eps_min, omega, phi_p, phi_g,
+                                                          seed, iter, P, per);
+  return check_launch(h, "k_pso_move");
+}
+
+int sc_get_counters(sc_handle* h, int64_t* evaluated_bins, int64_t* kernel_launches, void* stream) {
+  if (!h) return SC_ERR_NOT_INIT;
+  if (h->cuda_failed) return SC_ERR_CUDA;
+  unsigned long long v = 0;
+  SC_CUDA(h, cudaMemcpyAsync(&v, h->d_counter, 8, cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+  SC_CUDA(h, cudaStreamSynchronize((cudaStream_t)stream));
+  if (evaluated_bins) *evaluated_bins = (int64_t)v;
+  if (kernel_launches) *kernel_launches = h->launches;
+  return SC_OK;
+}
+
+int sc_set_option(sc_handle* h, int32_t option, int64_t value) {
+  if (!h) return SC_ERR_NOT_INIT;
+  switch (option) {
+    case SC_OPT_PRECISION:
+      if (value < 0 || value > 2) return fail(h, SC_ERR_INVALID_ARG, "precision must be 0, 1 or 2");
+      h->precision = (int)value; return SC_OK;
+    case SC_OPT_F32_MIN_SEG:
+      if (value < 1) return fail(h, SC_ERR_INVALID_ARG, "f32_min_seg must be >= 1");
+      h->f32_min_seg = (int)std::min<int64_t>(value, INT32_MAX); return SC_OK;
+    case SC_OPT_SCRATCH_BYTES:
+      if (value < (1 << 20)) return fail(h, SC_ERR_INVALID_ARG, "scratch cap must be >= 1 MiB");
+      h->scratch_cap = (size_t)value; return SC_OK;
+    case SC_OPT_TC_MAX_S:
+      if (value < 1) return fail(h, SC_ERR_INVALID_ARG, "tc_max_s must be >= 1");
+      h->tc_max_s = (double)value; set_stride(h); return SC_OK;
+    case SC_OPT_STRIDE_LOG2:
+      if (value != 0 && (value < 2 || value > 12)) return fail(h, SC_ERR_INVALID_ARG, "stride_log2 must be 0 (auto) or 2..12");
+      h->forced_stride_log2 = (int)value; set_stride(h); return SC_OK;
+    default:
+      return fail(h, SC_ERR_INVALID_ARG, "unknown option %d", (int)option);
+  }
+}
+
+int sc_free(sc_handle* h) {
+  if (!h) return SC_ERR_NOT_INIT;
+  cudaFree(h->W32); cudaFree(h->G32); cudaFree(h->W64); cudaFree(h->G64);
+  cudaFree(h->scratch); cudaFree(h->d_edges); cudaFree(h->d_chunk_k0); cudaFree(h->d_flags);
+  cudaFree(h->d_counter); cudaFree(h->d_params_stage);
+  cudaGetLastError();
+  delete h;
+  return SC_OK;
+}
+
+const char* sc_last_error(const sc_handle* h) { return h ? h->err.c_str() : g_init_error.c_str(); }
+
+const char* sc_version(void) { return "scstat 0.1 (sm_100a)"; }
+
+}  // extern "C"
