@@ -1,0 +1,338 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the semi-coherent statistic hot path on B200 (BASELINE.json metric).
+
+One "step" = one swarm iteration of the whole hot path: sc_eval_stat for the whole
+population (node evaluation, dense waveform x response x segment reduction, stitch) followed by sc_pso_step,
+device-resident, no host round trip.  Workload at N = 1: BASELINE.json configs[2] ("c3": T = 4 yr, band
+0.017-0.030 Hz, 1 640 996 bins, 10^4 particles, N_seg = 5000, PSO 0.7/1.5/1.5) -- the configuration the metric's
+target is quoted on.  For N > 1 every rank searches its own independent tile (own noise realisation and population,
+replicated nothing, no data-path collective): weak scaling.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 3]
+
+Prints ONE JSON line (rank 0).  `--impl reference` times the CPU oracle (oracle/, as it stands) on a bounded sample.
+Inputs are synthetic (sc_synth); injections in the GPU arm come from the library's own
+sc_gen_template, never from the oracle.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+import sc_synth as sy  # noqa: E402
+
+METRIC = "particle_x_freq_bin_evals_per_s"
+UNIT = "particle-bin/s"
+C_DP = 24          # FP64 instructions per (particle, bin) of the fixed op model, SURVEY.md 8(d)
+NOMINAL_DFMA = 148 * 64 * 1.965e9   # 148 SMs x 64 FP64 lanes x max SM clock (B200_PROFILING.md unit counts / clocks)
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--particles", type=int, default=None, help="override the population size (debug)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def workload_name(cid, spec, cfg, P, N):
+    return (f"c{cid}: T={spec['T_obs_yr']}yr band {spec['band'][0]}-{spec['band'][1]}Hz n_bins={cfg['n_bins']} "
+            f"P={P} N_seg={N}")
+
+
+def pso_params(spec, N):
+    if "pso" in spec:
+        return spec["pso"]
+    key = min(sy.TABLE_IV, key=lambda k: abs(np.log(k) - np.log(max(N, 1))))
+    return sy.TABLE_IV[key]
+
+
+# ---------------------------------------------------------------------------------------------- reference arm
+def oracle_sample_run(inp, N, n_particles, steps, warmup):
+    """Times the CPU oracle, as it stands, on the first n_particles of the population: statistic + PSO step."""
+    from oracle import sc_oracle as orc
+    cfg = orc.make_config(inp["cfg"])
+    e = inp["edges"][N]
+    pos = inp["particles"][:n_particles].copy()
+    vel = inp["velocities"][:n_particles].copy()
+    pbp, pbv = pos.copy(), np.full(n_particles, -np.inf)
+    gp, gv = np.zeros((1, 8)), np.zeros(1)
+    hp = pso_params(inp["spec"], N)
+    dA, dE = inp["noise_A"], inp["noise_E"]          # noise-only stream: the oracle's cost does not depend on the data
+    times = []
+    for it in range(warmup + steps):
+        t0 = time.perf_counter()
+        st = orc.eval_stat(cfg, dA, dE, inp["S_A"], inp["S_E"], pos, e)
+        orc.pso_step(pos, vel, pbp, pbv, st, gp, gv, inp["lo"], inp["hi"], np.array(hp["eps"], dtype=np.float64),
+                     hp["omega"], hp["phi_p"], hp["phi_g"], inp["pso_seed"], it, 1)
+        if it >= warmup:
+            times.append(time.perf_counter() - t0)
+    return float(np.mean(times)), orc.num_threads()
+
+
+def run_reference(args, rank, world):
+    if rank != 0:
+        return
+    cid = args.config
+    spec = sy.CONFIGS[cid]
+    inp = sy.config_inputs(cid, P=64)
+    N = spec["n_segs"][0]
+    from oracle import sc_oracle as orc
+    cores = orc.num_threads()
+    n_p = max(1, min(64, cores))
+    steps, warmup = max(1, min(args.steps, 5)), min(args.warmup, 1)
+    sec, cores = oracle_sample_run(inp, N, n_p, steps, warmup)
+    nb = inp["cfg"]["n_bins"]
+    val = n_p * nb / sec
+    sample = f"{n_p} particles x all {nb} bins per step ({steps} timed steps, {warmup} warm-up), noise-only stream"
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+            "warmup": warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(cid, spec, inp["cfg"], n_p, N)},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ---------------------------------------------------------------------------------------------- GPU arm
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--id={index}", f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.f,
+                                      stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.f.read().splitlines():
+            c = [x.strip() for x in ln.split(",")]
+            if len(c) < 8:
+                continue
+            try:
+                sm.append(float(c[0])); mx.append(float(c[1]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, c[4:8]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        self.f.close()
+        os.unlink(self.f.name)
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(np.max(mx)), reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+def run_ours(args, rank, local_rank, world):
+    import torch
+    import torch.distributed as dist
+    import paper_2408_13170_b200 as sc
+
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    cid = args.config
+    spec = sy.CONFIGS[cid]
+    inp = sy.config_inputs(cid, P=args.particles, replica=rank)
+    cfg = inp["cfg"]
+    N = spec["n_segs"][0]
+    e = inp["edges"][N].astype(np.int32)
+    nb = cfg["n_bins"]
+    P = inp["particles"].shape[0]
+    n_swarms = spec["n_swarms"]
+    hp = pso_params(spec, N)
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    S_A, S_E = t(inp["S_A"]), t(inp["S_E"])
+    nA, nE = t(inp["noise_A"]), t(inp["noise_E"])
+
+    # data = noise + kappa * h(theta_inj), the injection generated by the library itself (sc_gen_template)
+    H0 = sc.Handle(cfg, torch.view_as_real(nA).contiguous(), torch.view_as_real(nE).contiguous(), S_A, S_E)
+    dA, dE = nA.clone(), nE.clone()
+    for inj in inp["injections"]:
+        hA, hE = H0.gen_template(t(inj["theta"][None, :]))
+        rho2 = 4.0 * inp["df"] * ((hA[0].abs() ** 2 / S_A).sum() + (hE[0].abs() ** 2 / S_E).sum())
+        kappa = inj["rho"] / torch.sqrt(rho2)
+        dA += kappa * hA[0]
+        dE += kappa * hE[0]
+    H0.close()
+    H = sc.Handle(cfg, torch.view_as_real(dA).contiguous(), torch.view_as_real(dE).contiguous(), S_A, S_E)
+    # the caller knows its tile: t_c upper bound of the prior box sets the coarse node spacing (SC_OPT_TC_MAX_S)
+    H.set_option(sc.SC_OPT_TC_MAX_S, int(np.ceil(inp["hi"][2])))
+    H.set_option(sc.SC_OPT_PROFILE, 1)
+
+    lo, hi, eps = t(inp["lo"]), t(inp["hi"]), t(np.array(hp["eps"], dtype=np.float64))
+    state = dict(pos=t(inp["particles"]), vel=t(inp["velocities"]), pbest_pos=t(inp["particles"]),
+                 pbest_val=torch.full((P,), -np.inf, dtype=torch.float64, device=dev),
+                 gbest_pos=torch.zeros((n_swarms, 8), dtype=torch.float64, device=dev),
+                 gbest_val=torch.zeros(n_swarms, dtype=torch.float64, device=dev))
+    stat = torch.empty(P, dtype=torch.float64, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > 126 MB L2
+
+    def step(it):
+        H.eval_stat(state["pos"], e, out=stat)
+        H.pso_step(state, stat, lo, hi, eps, hp["omega"], hp["phi_p"], hp["phi_g"], inp["pso_seed"], it, n_swarms)
+
+    for it in range(args.warmup):
+        step(it)
+    torch.cuda.synchronize()
+    H.timing()                               # reset the per-class accumulators
+    _, launches0 = H.counters()
+    sampler = ClockSampler(torch.cuda.current_device() if "CUDA_VISIBLE_DEVICES" not in os.environ
+                           else int(os.environ["CUDA_VISIBLE_DEVICES"].split(",")[local_rank]))
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    eval_bins = 0
+    barrier()
+    t_wall0 = time.perf_counter()
+    for i, (a, b) in enumerate(evs):
+        flush.fill_(i & 0xFF)                # L2 flush between timed iterations (outside the events)
+        a.record()
+        step(args.warmup + i)
+        b.record()
+    barrier()
+    t_wall = time.perf_counter() - t_wall0
+    clocks = sampler.stop()
+    ms_steps = [a.elapsed_time(b) for a, b in evs]
+    ms_total = float(np.sum(ms_steps))
+    timing = H.timing()
+    eval_bins, launches1 = H.counters()      # evaluated bins of the LAST eval (the swarm moves; representative)
+    gpu_launches = launches1 - launches0
+
+    # ---- e2e: the same step through the HOST-buffer entry point, copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        k2 = max(1, min(args.steps, 5))
+        pos_h = torch.empty((P, 8), dtype=torch.float64).pin_memory()
+        stat_h = torch.empty(P, dtype=torch.float64).pin_memory()
+        pos_h.copy_(state["pos"])
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        a.record()
+        for i in range(k2):
+            H.eval_stat_host(pos_h.numpy(), e, out=stat_h.numpy())               # H2D params, D2H Upsilon (inside the C call)
+            stat.copy_(stat_h, non_blocking=True)                                 # H2D Upsilon for the device-side PSO
+            H.pso_step(state, stat, lo, hi, eps, hp["omega"], hp["phi_p"], hp["phi_g"], inp["pso_seed"],
+                       args.warmup + args.steps + i, n_swarms)
+            pos_h.copy_(state["pos"], non_blocking=True)                          # D2H new positions
+            torch.cuda.synchronize()
+        b.record()
+        barrier()
+        ms_e2e = a.elapsed_time(b) / k2
+        e2e = dict(ms=ms_e2e, h2d=P * 64 + P * 8, d2h=P * 8 + P * 64)
+        H.timing()
+
+    # ---- reduce over ranks: max time, summed work
+    ms_max, units = ms_total, float(P) * nb * args.steps
+    e2e_ms_max = e2e["ms"] if e2e else 0.0
+    if world > 1:
+        v = torch.tensor([ms_total, e2e_ms_max], dtype=torch.float64, device=dev)
+        dist.all_reduce(v, op=dist.ReduceOp.MAX)
+        ms_max, e2e_ms_max = v[0].item(), v[1].item()
+        u = torch.tensor([units], dtype=torch.float64, device=dev)
+        dist.all_reduce(u, op=dist.ReduceOp.SUM)
+        units = u.item()
+
+    if rank == 0:
+        value = units / (ms_max * 1e-3)
+        ms_per_step = ms_max / args.steps
+        dense_ms, dense_n = timing["dense"]
+        dense_avg = dense_ms / max(dense_n, 1)
+        try:
+            dfma = sc.sc_measure_fp64_peak()
+        except sc.SCError:
+            dfma = None
+        # roofline of the dominant kernel (k_dense), fixed FP64 op model of SURVEY.md 8(d): 24 FP64 instr = 48 flop per
+        # EVALUATED (particle, bin); peak = measured DFMA rate x 2 flop
+        ach = 2.0 * C_DP * eval_bins / (dense_avg * 1e-3) / 1e12 if dense_avg > 0 else None
+        peak = 2.0 * (dfma or NOMINAL_DFMA) / 1e12
+        roof = {"bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
+                "frac": (ach / peak) if ach else None, "traffic": None,
+                "kernel": "k_dense<float,false>", "kernel_ms_per_launch": dense_avg,
+                "model": f"{C_DP} FP64 instr (= {2 * C_DP} flop) per evaluated particle-bin, SURVEY.md 8(d)",
+                "peak_source": ("measured in this run by sc_measure_fp64_peak (DFMA/s x 2)" if dfma else
+                                "nominal 148 SM x 64 lanes x 1.965 GHz x 2"),
+                "peak_nominal_max_clock": 2.0 * NOMINAL_DFMA / 1e12,
+                "evaluated_particle_bins_per_launch": eval_bins,
+                "evaluated_pb_per_s": eval_bins / (dense_avg * 1e-3) if dense_avg > 0 else None,
+                "frac_vs_nominal_max_clock": (ach / (2.0 * NOMINAL_DFMA / 1e12)) if ach else None}
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f64 phase + f32 amplitude/accumulate-flush-to-f64", "data": "synthetic",
+                "config": {"workload": workload_name(cid, spec, cfg, P, N), "l2": "flushed between timed steps "
+                           "(256 MiB write); per-step node tables (GBs) exceed L2 anyway",
+                           "pso": {k: hp[k] for k in ("omega", "phi_p", "phi_g")}, "n_swarms": n_swarms,
+                           "parallelism": f"independent tiles x{world}" if world > 1 else "1 GPU"},
+                "swarm_iters_per_s": world * 1e3 / ms_per_step,
+                "kernel_ms_per_step": {k: v[0] / args.steps for k, v in timing.items() if v[1]},
+                "wall_s_timed_region": t_wall,
+                "clocks": {"sm_mhz": clocks["sm_mhz"], "sm_max_mhz": clocks["sm_max_mhz"], "reasons": clocks["reasons"],
+                           "samples": clocks["samples"]},
+                "roofline": roof, "gpu_launches": int(gpu_launches)}
+        if e2e:
+            line["e2e"] = {"value": world * float(P) * nb / (e2e_ms_max * 1e-3), "unit": UNIT,
+                           "h2d_bytes_per_step": e2e["h2d"], "d2h_bytes_per_step": e2e["d2h"],
+                           "ms_per_step": e2e_ms_max}
+        if not args.no_cpu_baseline and world == 1:
+            from oracle import sc_oracle as orc
+            cores = orc.num_threads()
+            n_p = max(8, min(64, cores))
+            sec, cores = oracle_sample_run(sy.config_inputs(cid, P=n_p), N, n_p, 1, 0)
+            line["cpu_baseline"] = {"value": n_p * nb / sec, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                    "sample": f"{n_p} particles x all {nb} bins, 1 step (statistic + PSO), {sec:.1f} s wall"}
+        print(json.dumps(line), flush=True)
+    H.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+    else:
+        run_ours(args, rank, local_rank, world)
+
+
+if __name__ == "__main__":
+    main()

@@ -64,8 +64,13 @@ enum {
   SC_OPT_TC_MAX_S = 4,       /* the caller's upper bound on t_c [s] over the particles (the search tile's t_c range,
                                 PAPER.md:253); sets the coarse node spacing to about one day of signal time at the
                                 low band edge.  Default 10 yr.                                  */
-  SC_OPT_STRIDE_LOG2 = 5     /* 0 = automatic (rule above), else log2 of the coarse node spacing in bins (2..12)   */
+  SC_OPT_STRIDE_LOG2 = 5,    /* 0 = automatic (rule above), else log2 of the coarse node spacing in bins (2..12)   */
+  SC_OPT_PROFILE = 6         /* 1 = record a CUDA event pair around every kernel launch (read by sc_get_timing)     */
 };
+
+/* Kernel classes of sc_get_timing. */
+enum { SC_TIME_NODES = 0, SC_TIME_DENSE = 1, SC_TIME_STITCH = 2, SC_TIME_PSO = 3, SC_TIME_OTHER = 4,
+       SC_N_TIMING_CLASSES = 5 };
 
 /* a0 -- data whitening, once per data stream (PSD known; Eq. 1 weights).
  * dA_ri, dE_ri: DEVICE, interleaved (re, im) FP64, n_bins complex each.  S_A, S_E: DEVICE, one-sided PSD, n_bins.
@@ -124,6 +129,15 @@ int sc_pso_step(sc_handle* h, double* pos, double* vel, double* pbest_pos, doubl
  *  evaluated_bins = sum_p |{j in window_p} intersect [e_0, e_N)|  (the "evaluated (particle x bin)" of the metric),
  *  kernel_launches = CUDA kernels launched by the library since the handle was created. */
 int sc_get_counters(sc_handle* h, int64_t* evaluated_bins, int64_t* kernel_launches, void* cuda_stream);
+
+/* With SC_OPT_PROFILE = 1: device time [ms] and launch count per kernel class since the previous call, measured with
+ * CUDA events on the launching stream (ms_per_class, launches_per_class: HOST arrays of SC_N_TIMING_CLASSES; either
+ * may be NULL).  Synchronises the stream and resets the accumulators. */
+int sc_get_timing(sc_handle* h, double* ms_per_class, int64_t* launches_per_class, void* cuda_stream);
+
+/* Roofline denominator: sustained FP64 FMA rate of the current device, in DFMA/s, from a
+ * dependent-chain-free microbenchmark (8 chains per thread, all SMs).  Needs no handle.  Synchronises. */
+int sc_measure_fp64_peak(double* dfma_per_s, void* cuda_stream);
 
 int sc_set_option(sc_handle* h, int32_t option, int64_t value);
 int sc_free(sc_handle* h);

@@ -11,10 +11,12 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libscstat.so")
 
 SC_OK, SC_ERR_INVALID_ARG, SC_ERR_NOT_INIT, SC_ERR_CUDA, SC_ERR_OOM = 0, -1, -2, -3, -4
-SC_OPT_PRECISION, SC_OPT_F32_MIN_SEG, SC_OPT_SCRATCH_BYTES, SC_OPT_TC_MAX_S, SC_OPT_STRIDE_LOG2 = 1, 2, 3, 4, 5
+SC_OPT_PRECISION, SC_OPT_F32_MIN_SEG, SC_OPT_SCRATCH_BYTES, SC_OPT_TC_MAX_S, SC_OPT_STRIDE_LOG2, SC_OPT_PROFILE = 1, 2, 3, 4, 5, 6
+SC_TIMING_CLASSES = ["nodes", "dense", "stitch", "pso", "other"]
 
 EXPORTED_SYMBOLS = ["sc_init_data", "sc_init_data_host", "sc_eval_stat", "sc_eval_stat_host", "sc_eval_segments",
-                    "sc_gen_template", "sc_pso_step", "sc_get_counters", "sc_set_option", "sc_free",
+                    "sc_gen_template", "sc_pso_step", "sc_get_counters", "sc_get_timing", "sc_measure_fp64_peak",
+                    "sc_set_option", "sc_free",
                     "sc_last_error", "sc_version"]
 
 
@@ -75,6 +77,10 @@ def load_library():
     L.sc_pso_step.argtypes = [_vp] + [_vp] * 10 + [C.c_double] * 3 + [C.c_uint64, C.c_uint64, C.c_int64, C.c_int32, _vp]
     L.sc_get_counters.restype = C.c_int
     L.sc_get_counters.argtypes = [_vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64), _vp]
+    L.sc_get_timing.restype = C.c_int
+    L.sc_get_timing.argtypes = [_vp, C.POINTER(C.c_double), C.POINTER(C.c_int64), _vp]
+    L.sc_measure_fp64_peak.restype = C.c_int
+    L.sc_measure_fp64_peak.argtypes = [C.POINTER(C.c_double), _vp]
     L.sc_set_option.restype = C.c_int
     L.sc_set_option.argtypes = [_vp, C.c_int32, C.c_int64]
     L.sc_free.restype = C.c_int
@@ -258,6 +264,20 @@ def sc_get_counters(h, stream=None):
     return a.value, b.value
 
 
+def sc_get_timing(h, stream=None):
+    """{class: (ms, launches)} since the previous call (needs SC_OPT_PROFILE = 1); synchronises the stream."""
+    ms = (C.c_double * len(SC_TIMING_CLASSES))()
+    n = (C.c_int64 * len(SC_TIMING_CLASSES))()
+    _check(load_library().sc_get_timing(h, ms, n, _stream(stream)), h)
+    return {k: (ms[i], n[i]) for i, k in enumerate(SC_TIMING_CLASSES)}
+
+
+def sc_measure_fp64_peak(stream=None):
+    v = C.c_double(0.0)
+    _check(load_library().sc_measure_fp64_peak(C.byref(v), _stream(stream)), None)
+    return v.value
+
+
 def sc_set_option(h, option, value):
     _check(load_library().sc_set_option(h, int(option), int(value)), h)
 
@@ -314,6 +334,9 @@ class Handle:
 
     def counters(self, stream=None):
         return sc_get_counters(self.h, stream)
+
+    def timing(self, stream=None):
+        return sc_get_timing(self.h, stream)
 
     def set_option(self, option, value):
         sc_set_option(self.h, option, value)

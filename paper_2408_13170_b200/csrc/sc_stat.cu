@@ -556,6 +556,17 @@ __global__ void k_pso_move(double* __restrict__ pos, double* __restrict__ vel, c
   }
 }
 
+// ------------------------------------------------------------------------------------------------ peaks
+// FP64 FMA throughput probe for the roofline denominator: 8 independent DFMA chains per thread.
+__global__ void k_dfma_peak(double* __restrict__ out, int iters, double a, double b) {
+  double x0 = threadIdx.x, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
+  for (int i = 0; i < iters; ++i) {
+    x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
+    x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
+  }
+  out[blockIdx.x * blockDim.x + threadIdx.x] = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
+}
+
 // ------------------------------------------------------------------------------------------------ host side
 thread_local std::string g_init_error;
 
@@ -579,6 +590,11 @@ struct sc_handle {
   std::vector<int> edges; int cached_chunk = 0; int chunk_first = 0, n_chunks = 0;
   std::vector<int> chunk_k0; std::vector<uint8_t> flags;
   long long launches = 0;
+  // optional per-kernel-class device timing (SC_OPT_PROFILE): event pairs recorded around each launch
+  bool profile = false;
+  struct Ev { cudaEvent_t a, b; int cls; };
+  std::vector<Ev> evs; size_t ev_used = 0;
+  double cls_ms[SC_N_TIMING_CLASSES] = {0, 0, 0, 0, 0}; long long cls_n[SC_N_TIMING_CLASSES] = {0, 0, 0, 0, 0};
   bool cuda_failed = false;
   std::string err;
 };
@@ -608,6 +624,23 @@ int fail(sc_handle* h, int code, const char* fmt, ...) {
   do { cudaError_t e_ = (call);                                                                  \
        if (e_ != cudaSuccess) return fail((h), e_ == cudaErrorMemoryAllocation ? SC_ERR_OOM : SC_ERR_CUDA, \
                                           "%s failed: %s", #call, cudaGetErrorString(e_)); } while (0)
+
+// RAII: records an event pair around one kernel launch when profiling is on.
+struct Timed {
+  sc_handle* h; cudaStream_t st; int idx = -1;
+  Timed(sc_handle* h_, cudaStream_t st_, int cls) : h(h_), st(st_) {
+    if (!h->profile) return;
+    if (h->ev_used == h->evs.size()) {
+      sc_handle::Ev e; e.cls = cls;
+      if (cudaEventCreate(&e.a) != cudaSuccess || cudaEventCreate(&e.b) != cudaSuccess) { cudaGetLastError(); return; }
+      h->evs.push_back(e);
+    }
+    idx = (int)h->ev_used++;
+    h->evs[idx].cls = cls;
+    cudaEventRecord(h->evs[idx].a, st);
+  }
+  ~Timed() { if (idx >= 0) cudaEventRecord(h->evs[idx].b, st); }
+};
 
 int check_launch(sc_handle* h, const char* what) {
   h->launches++;
@@ -703,14 +736,20 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
 
   for (int64_t pb = 0; pb < P; pb += P_pad) {
     const int Pn = (int)std::min<int64_t>(P_pad, P - pb);
-    k_particle_consts<<<(P_pad + 127) / 128, 128, 0, st>>>(dc, params + pb * 8, Pn, P_pad, pc, jlo, jhi, e_first, e_last,
-                                                          h->d_counter);
+    {
+      Timed tm(h, st, SC_TIME_NODES);
+      k_particle_consts<<<(P_pad + 127) / 128, 128, 0, st>>>(dc, params + pb * 8, Pn, P_pad, pc, jlo, jhi, e_first, e_last,
+                                                            h->d_counter);
+    }
     if ((rc = check_launch(h, "k_particle_consts"))) return rc;
     if (n_chunks == 0) {
       if (!seg_mode) SC_CUDA(h, cudaMemsetAsync(out + pb, 0, (size_t)Pn * 8, st));
       continue;
     }
-    k_nodes<R><<<dim3((P_pad + 127) / 128, n_nodes), 128, 0, st>>>(dc, pc, jlo, jhi, P_pad, node_n, node_frac, node_amp);
+    {
+      Timed tm(h, st, SC_TIME_NODES);
+      k_nodes<R><<<dim3((P_pad + 127) / 128, n_nodes), 128, 0, st>>>(dc, pc, jlo, jhi, P_pad, node_n, node_frac, node_amp);
+    }
     if ((rc = check_launch(h, "k_nodes"))) return rc;
     DenseArgs a;
     a.edges = h->d_edges; a.n_seg = n_seg; a.chunk_first = h->chunk_first; a.chunk_k0 = h->d_chunk_k0;
@@ -718,11 +757,15 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
     a.frag = frag; a.out_seg = seg_mode ? out_seg + (size_t)pb * n_seg * 3 : nullptr; a.P = Pn;
     a.seg_scale_z = sz; a.seg_scale_s = ss;
     const dim3 grid(n_chunks, P_pad / kBlock);
+    {
+    Timed tm(h, st, SC_TIME_DENSE);
     if (seg_mode) k_dense<R, true><<<grid, kBlock, 0, st>>>(dc, a, (const typename DataT<R>::W*)(sizeof(R) == 4 ? (void*)h->W32 : (void*)h->W64),
                                                             (const typename DataT<R>::G*)(sizeof(R) == 4 ? (void*)h->G32 : (void*)h->G64));
     else k_dense<R, false><<<grid, kBlock, 0, st>>>(dc, a, (const typename DataT<R>::W*)(sizeof(R) == 4 ? (void*)h->W32 : (void*)h->W64),
                                                     (const typename DataT<R>::G*)(sizeof(R) == 4 ? (void*)h->G32 : (void*)h->G64));
+    }
     if ((rc = check_launch(h, "k_dense"))) return rc;
+    Timed tm2(h, st, SC_TIME_STITCH);
     if (seg_mode) k_stitch_seg<<<(Pn + 127) / 128, 128, 0, st>>>(frag, h->d_flags, h->d_chunk_k0, n_chunks, P_pad, Pn, n_seg, sz, ss,
                                                                 out_seg + (size_t)pb * n_seg * 3);
     else k_stitch<<<(Pn + 127) / 128, 128, 0, st>>>(frag, h->d_flags, n_chunks, P_pad, Pn, out + pb);
@@ -945,6 +988,7 @@ int sc_pso_step(sc_handle* h, double* pos, double* vel, double* pbest_pos, doubl
   cudaStream_t st = (cudaStream_t)stream;
   const int per = (int)(P / n_swarms);
   int rc;
+  Timed tm(h, st, SC_TIME_PSO);
   k_pso_best<<<n_swarms, 1024, 0, st>>>(pos, pbest_pos, pbest_val, stat, gbest_pos, gbest_val, per);
   if ((rc = check_launch(h, "k_pso_best"))) return rc;
   k_pso_move<<<(unsigned)((P + 127) / 128), 128, 0, st>>>(pos, vel, pbest_pos, gbest_pos, lo, hi, eps_min, omega, phi_p, phi_g,
@@ -963,6 +1007,54 @@ int sc_get_counters(sc_handle* h, int64_t* evaluated_bins, int64_t* kernel_launc
   return SC_OK;
 }
 
+int sc_get_timing(sc_handle* h, double* ms_per_class, int64_t* launches_per_class, void* stream) {
+  if (!h) return SC_ERR_NOT_INIT;
+  if (h->cuda_failed) return SC_ERR_CUDA;
+  SC_CUDA(h, cudaStreamSynchronize((cudaStream_t)stream));
+  for (size_t i = 0; i < h->ev_used; ++i) {
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, h->evs[i].a, h->evs[i].b) == cudaSuccess) {
+      h->cls_ms[h->evs[i].cls] += ms; h->cls_n[h->evs[i].cls]++;
+    } else cudaGetLastError();
+  }
+  h->ev_used = 0;
+  for (int c = 0; c < SC_N_TIMING_CLASSES; ++c) {
+    if (ms_per_class) ms_per_class[c] = h->cls_ms[c];
+    if (launches_per_class) launches_per_class[c] = h->cls_n[c];
+    h->cls_ms[c] = 0.0; h->cls_n[c] = 0;
+  }
+  return SC_OK;
+}
+
+int sc_measure_fp64_peak(double* dfma_per_s, void* stream) {
+  if (!dfma_per_s) return SC_ERR_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  int dev = 0, sms = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+    cudaGetLastError();
+    return fail(nullptr, SC_ERR_CUDA, "no CUDA device; this library has no CPU fallback");
+  }
+  const int blocks = sms * 8, threads = 256, iters = 1 << 15;
+  double* buf = nullptr;
+  if (cudaMalloc(&buf, (size_t)blocks * threads * 8) != cudaSuccess) { cudaGetLastError(); return fail(nullptr, SC_ERR_OOM, "cudaMalloc failed"); }
+  cudaEvent_t a, b;
+  cudaEventCreate(&a); cudaEventCreate(&b);
+  float best = 1e30f;
+  for (int rep = 0; rep < 4; ++rep) {
+    cudaEventRecord(a, st);
+    k_dfma_peak<<<blocks, threads, 0, st>>>(buf, iters, 0.999999, 1e-9);
+    cudaEventRecord(b, st);
+    cudaEventSynchronize(b);
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, a, b);
+    if (rep > 0 && ms < best) best = ms;
+  }
+  cudaEventDestroy(a); cudaEventDestroy(b); cudaFree(buf);
+  if (cudaGetLastError() != cudaSuccess) return fail(nullptr, SC_ERR_CUDA, "k_dfma_peak failed");
+  *dfma_per_s = (double)blocks * threads * 8.0 * iters / (best * 1e-3);
+  return SC_OK;
+}
+
 int sc_set_option(sc_handle* h, int32_t option, int64_t value) {
   if (!h) return SC_ERR_NOT_INIT;
   switch (option) {
@@ -975,6 +1067,8 @@ int sc_set_option(sc_handle* h, int32_t option, int64_t value) {
     case SC_OPT_SCRATCH_BYTES:
       if (value < (1 << 20)) return fail(h, SC_ERR_INVALID_ARG, "scratch cap must be >= 1 MiB");
       h->scratch_cap = (size_t)value; return SC_OK;
+    case SC_OPT_PROFILE:
+      h->profile = (value != 0); return SC_OK;
     case SC_OPT_TC_MAX_S:
       if (value < 1) return fail(h, SC_ERR_INVALID_ARG, "tc_max_s must be >= 1");
       h->tc_max_s = (double)value; set_stride(h); return SC_OK;
@@ -991,6 +1085,7 @@ int sc_free(sc_handle* h) {
   cudaFree(h->W32); cudaFree(h->G32); cudaFree(h->W64); cudaFree(h->G64);
   cudaFree(h->scratch); cudaFree(h->d_edges); cudaFree(h->d_chunk_k0); cudaFree(h->d_flags);
   cudaFree(h->d_counter); cudaFree(h->d_params_stage);
+  for (auto& e : h->evs) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
   cudaGetLastError();
   delete h;
   return SC_OK;

@@ -145,17 +145,18 @@ CONFIGS = {
 }
 
 
-def config_inputs(config_id, P=None):
+def config_inputs(config_id, P=None, replica=0):
     """Everything about config c<id> that does not need a template: grid, PSD, noise, injection parameters
-    (un-scaled), prior box, particles, velocities, edge lists.  The caller adds kappa*h(theta_inj) to 'noise'."""
+    (un-scaled), prior box, particles, velocities, edge lists.  The caller adds kappa*h(theta_inj) to 'noise'.
+    replica > 0 draws an independent noise realisation and population (other GPUs / repeated noise seeds, config 4)."""
     spec = CONFIGS[config_id]
     f_lo, f_hi = spec["band"]
     cfg = grid_config(spec["T_obs_yr"], f_lo, f_hi)
     f = freqs(cfg)
     S = psd_AE(f)
     df = 1.0 / cfg["T_obs_s"]
-    nA = draw_noise(seed_for("noise", config_id, 0), S, df)
-    nE = draw_noise(seed_for("noise", config_id, 1), S, df)
+    nA = draw_noise(seed_for("noise", config_id, 2 * replica), S, df)
+    nE = draw_noise(seed_for("noise", config_id, 2 * replica + 1), S, df)
     rng = np.random.default_rng(seed_for("injection", config_id))
     injections = []
     for s in spec["inj"]:
@@ -171,7 +172,7 @@ def config_inputs(config_id, P=None):
     n = spec["P"] if P is None else P
     return dict(id=config_id, spec=spec, cfg=cfg, f=f, S_A=S, S_E=S.copy(), df=df, noise_A=nA, noise_E=nE,
                 injections=injections, lo=lo, hi=hi,
-                particles=draw_particles(seed_for("particles", config_id), spec["P"], lo, hi)[:n].copy(),
-                velocities=draw_velocities(seed_for("velocities", config_id), spec["P"], lo, hi)[:n].copy(),
+                particles=draw_particles(seed_for("particles", config_id, replica), spec["P"], lo, hi)[:n].copy(),
+                velocities=draw_velocities(seed_for("velocities", config_id, replica), spec["P"], lo, hi)[:n].copy(),
                 edges={N: edges(cfg["n_bins"], N) for N in spec["n_segs"]},
-                pso_seed=seed_for("pso", config_id))
+                pso_seed=seed_for("pso", config_id, replica))

@@ -1,0 +1,372 @@
+"""GPU-vs-oracle parity through the C ABI (all `-m gpu`).
+
+Bar (BASELINE.json north_star): |Upsilon_gpu - Upsilon_oracle| <= 1e-6 * Upsilon_oracle for EVERY particle, on every
+config; bit-exact segment-boundary indexing.  Data streams are assembled from sc_synth noise plus the ORACLE's
+templates (tests/helpers.py); nothing the oracle sees comes from the CUDA path.
+Full-size cases run the GPU in bench.py's launch configuration (whole population) and compare a seeded sample of
+particles the oracle can afford, plus properties that hold at any size.
+"""
+import numpy as np
+import pytest
+
+import sc_synth as sy
+from helpers import gpu_handle, make_data, rel_err
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-6          # relative, per particle (north_star)
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return torch
+
+
+@pytest.fixture(scope="module")
+def sc():
+    import paper_2408_13170_b200 as sc
+    sc.load_library()          # fails loudly if the extension is missing
+    return sc
+
+
+def _dev(torch, a):
+    return torch.from_numpy(np.ascontiguousarray(a)).to("cuda:0")
+
+
+def _sample_idx(P, n, seed):
+    return np.sort(np.random.default_rng(seed).choice(P, size=min(n, P), replace=False))
+
+
+# ---------------------------------------------------------------------------------------------- config 1 (full)
+@pytest.fixture(scope="module")
+def c1(oracle, torch_cuda, sc):
+    inp = sy.config_inputs(1)
+    cfg, dA, dE = make_data(oracle, inp)
+    H = gpu_handle(inp, dA, dE)
+    yield dict(inp=inp, cfg=cfg, dA=dA, dE=dE, H=H)
+    H.close()
+
+
+@pytest.mark.parametrize("prec", [1, 2], ids=["fp32amp", "allfp64"])
+def test_c1_full_population(c1, oracle, torch_cuda, sc, prec):
+    inp, H = c1["inp"], c1["H"]
+    e = inp["edges"][1000]
+    ref, refseg = oracle.eval_stat(c1["cfg"], c1["dA"], c1["dE"], inp["S_A"], inp["S_E"], inp["particles"], e, want_seg=True)
+    H.set_option(sc.SC_OPT_PRECISION, prec)
+    par = _dev(torch_cuda, inp["particles"])
+    got = H.eval_stat(par, e).cpu().numpy()
+    assert rel_err(got, ref).max() <= TOL
+    seg = H.eval_segments(par, e).cpu().numpy()
+    scale = np.abs(refseg).max(axis=1, keepdims=True)            # per particle, per component
+    tol_seg = 2e-6 if prec == 1 else 1e-7
+    assert (np.abs(seg - refseg) / scale).max() <= tol_seg
+    # the statistic recomputed from the GPU's own segments agrees with the GPU's statistic (stitch = definition)
+    z2 = seg[:, :, 0] ** 2 + seg[:, :, 1] ** 2
+    with np.errstate(invalid="ignore", divide="ignore"):
+        u = 4 * inp["df"] * np.where(seg[:, :, 2] > 0, z2 / seg[:, :, 2], 0.0).sum(axis=1)
+    assert rel_err(u, got).max() <= 1e-12
+    H.set_option(sc.SC_OPT_PRECISION, 0)
+
+
+def test_c1_template_elementwise(c1, oracle, torch_cuda):
+    """sc_gen_template (same node tables / interpolants as the statistic) against the oracle's direct evaluation."""
+    inp, H = c1["inp"], c1["H"]
+    thetas = np.vstack([inp["injections"][0]["theta"][None, :], inp["particles"][:3]])
+    gA, gE = H.gen_template(_dev(torch_cuda, thetas))
+    gA, gE = gA.cpu().numpy(), gE.cpu().numpy()
+    for i, th in enumerate(thetas):
+        hA, hE, w = oracle.template(c1["cfg"], th)
+        assert np.array_equal(np.abs(gA[i]) > 0, np.abs(hA) > 0)          # identical time window, bin for bin
+        assert int((np.abs(gA[i]) > 0).sum()) == w
+        assert np.abs(gA[i] - hA).max() <= 1e-7 * np.abs(hA).max()
+        assert np.abs(gE[i] - hE).max() <= 1e-7 * np.abs(hE).max()
+
+
+def test_c1_hierarchy_levels_and_single_segment(c1, oracle, torch_cuda, sc):
+    inp, H = c1["inp"], c1["H"]
+    nb = inp["cfg"]["n_bins"]
+    par = _dev(torch_cuda, inp["particles"])
+    levels = [1, 3, 10, 100, 1000, 7919, nb]                 # N = n_bins: one bin per segment
+    elist = [sy.edges(nb, N) for N in levels]
+    ref = oracle.eval_stat_levels(c1["cfg"], c1["dA"], c1["dE"], inp["S_A"], inp["S_E"], inp["particles"], elist)
+    prev = None
+    for N, e, r in zip(levels, elist, ref):
+        got = H.eval_stat(par, e).cpu().numpy()               # auto precision: all-FP64 below 8 segments
+        assert rel_err(got, r).max() <= TOL, N
+        if prev is not None and N % prev[0] == 0:
+            assert np.all(got >= prev[1] * (1 - 1e-9))        # nested refinement never decreases Upsilon
+        prev = (N, got)
+
+
+def test_c1_partial_and_empty_edges(c1, oracle, torch_cuda):
+    inp, H = c1["inp"], c1["H"]
+    nb = inp["cfg"]["n_bins"]
+    par = _dev(torch_cuda, inp["particles"][:9])               # ragged population
+    for e in (np.array([5000, 5000, 5001, 9000, 9000, 20000, 20000], dtype=np.int64),      # empties, 1-bin, partial cover
+              np.array([0, 1, 2, 3, nb], dtype=np.int64),
+              np.array([2047, 2048, 2049, 4096, 6144, 6145], dtype=np.int64),              # edges on / next to chunk borders
+              np.array([nb - 1, nb], dtype=np.int64),
+              np.array([17, 17], dtype=np.int64)):                                          # nothing covered
+        ref, refseg = oracle.eval_stat(c1["cfg"], c1["dA"], c1["dE"], inp["S_A"], inp["S_E"], inp["particles"][:9], e, want_seg=True)
+        got = H.eval_stat(par, e).cpu().numpy()
+        assert np.all(np.abs(got - ref) <= TOL * np.abs(ref)), e
+        seg = H.eval_segments(par, e).cpu().numpy()
+        scale = max(np.abs(refseg).max(), 1e-300)
+        assert np.abs(seg - refseg).max() <= 2e-6 * scale
+        assert np.array_equal(seg[:, np.diff(e) == 0, :], np.zeros_like(seg[:, np.diff(e) == 0, :]))
+
+
+def test_invalid_particles_give_zero(c1, torch_cuda):
+    inp, H = c1["inp"], c1["H"]
+    p = inp["particles"][:6].copy()
+    p[0, 1] = 0.26; p[1, 0] = -1.0; p[2, 2] = np.nan; p[3, 5] = np.inf; p[4, 1] = 0.0
+    got = H.eval_stat(_dev(torch_cuda, p), inp["edges"][1000]).cpu().numpy()
+    assert np.array_equal(got[:5], np.zeros(5)) and got[5] > 0 and np.all(np.isfinite(got))
+
+
+def test_determinism_batching_and_host_entry(c1, torch_cuda, sc):
+    inp, H = c1["inp"], c1["H"]
+    e = inp["edges"][1000]
+    par = _dev(torch_cuda, inp["particles"])
+    a = H.eval_stat(par, e).cpu().numpy()
+    b = H.eval_stat(par, e).cpu().numpy()
+    assert np.array_equal(a, b)                                 # no atomics in the bin loop: bitwise reproducible
+    H.set_option(sc.SC_OPT_SCRATCH_BYTES, 1 << 20)              # force several particle batches
+    c = H.eval_stat(par, e).cpu().numpy()
+    H.set_option(sc.SC_OPT_SCRATCH_BYTES, 8 << 30)
+    assert np.array_equal(a, c)
+    d = H.eval_stat_host(inp["particles"], e)                   # host-buffer entry point
+    assert np.array_equal(a, d)
+    e_dev = torch_cuda.from_numpy(e.astype(np.int32)).to("cuda:0")
+    f = H.eval_stat(par, e_dev).cpu().numpy()                   # device-resident edges
+    assert np.array_equal(a, f)
+    for P in (1, 5, 33, 64):
+        g = H.eval_stat(par[:P].contiguous(), e).cpu().numpy()
+        assert np.array_equal(g, a[:P])
+
+
+def test_error_codes(c1, torch_cuda, sc):
+    inp, H = c1["inp"], c1["H"]
+    par = _dev(torch_cuda, inp["particles"][:4])
+    nb = inp["cfg"]["n_bins"]
+    for bad in (np.array([0, 10, 5, nb]), np.array([-1, 10, nb]), np.array([0, nb + 1])):
+        with pytest.raises(sc.SCError) as ei:
+            H.eval_stat(par, bad)
+        assert ei.value.code == -1
+    with pytest.raises(sc.SCError):
+        sc.Handle(dict(inp["cfg"], n_channels=3), par, par, par, par)
+    # the handle still works after argument errors
+    assert H.eval_stat(par, inp["edges"][1000]).shape[0] == 4
+
+
+# ---------------------------------------------------------------------------------------------- bit-exact indexing
+def test_segment_indexing_bit_exact(oracle, torch_cuda, sc):
+    """One-bin impulse data: exactly one segment may be non-zero, the k with e_k <= j < e_{k+1} (Q2, Q7)."""
+    cfgd = sy.grid_config(0.5, 0.018, 0.020, window_mode=0)
+    nb = cfgd["n_bins"]
+    S = sy.psd_AE(sy.freqs(cfgd))
+    th = sy.config_inputs(1, P=1)["particles"]
+    rng = np.random.default_rng(12)
+    edge_sets = [sy.edges(nb, 1000), sy.edges(nb, 7),
+                 np.array([0, 0, 1, 1, 2, 2047, 2048, 2048, 2049, 4095, 4097, 30000, nb], dtype=np.int64),
+                 np.array([100, 2048, 4096, 31000], dtype=np.int64)]
+    bins = sorted(set([0, 1, 2, 2046, 2047, 2048, 2049, 4095, 4096, 4097, 99, 100, 30999, 31000, nb - 1]
+                      + list(rng.integers(0, nb, 10))))
+    for j in bins:
+        dA = np.zeros(nb, dtype=complex)
+        dA[j] = (1.0 - 2.0j) * np.sqrt(S[j])
+        H = gpu_handle(dict(cfg=cfgd, S_A=S, S_E=S), dA, dA * 0)
+        for e in edge_sets:
+            seg = H.eval_segments(_dev(torch_cuda, th), e).cpu().numpy()[0]
+            nz = np.nonzero(seg[:, 0] ** 2 + seg[:, 1] ** 2)[0]
+            k = np.searchsorted(e, j, side="right") - 1
+            inside = 0 <= k < len(e) - 1 and e[k] <= j < e[k + 1]
+            assert list(nz) == ([k] if inside else []), (j, e[:6])
+        H.close()
+
+
+# ---------------------------------------------------------------------------------------------- configs 2..5
+def _full_launch_case(oracle, torch, sc, cid, n_sample, seed, tc_hint=True):
+    inp = sy.config_inputs(cid)
+    cfg, dA, dE = make_data(oracle, inp)
+    H = gpu_handle(inp, dA, dE)
+    if tc_hint:
+        H.set_option(sc.SC_OPT_TC_MAX_S, int(np.ceil(inp["hi"][2])))      # what bench.py sets: the tile's t_c bound
+    P = inp["particles"].shape[0]
+    idx = _sample_idx(P, n_sample, seed)
+    levels = inp["spec"]["n_segs"]
+    ref = oracle.eval_stat_levels(cfg, dA, dE, inp["S_A"], inp["S_E"], inp["particles"][idx], [inp["edges"][N] for N in levels])
+    par = _dev(torch, inp["particles"])
+    got = {}
+    for N in levels:
+        got[N] = H.eval_stat(par, inp["edges"][N]).cpu().numpy()            # whole population, bench launch config
+    dd = oracle.inner(dA, dE, dA, dE, inp["S_A"], inp["S_E"], inp["df"])
+    inp["evaluated_fraction"] = H.counters()[0] / (P * inp["cfg"]["n_bins"])      # share of bins inside the time windows
+    H.close()
+    return inp, levels, idx, ref, got, dd
+
+
+def _check_case(inp, levels, idx, ref, got, dd):
+    for l, N in enumerate(levels):
+        err = rel_err(got[N][idx], ref[l])
+        assert err.max() <= TOL, (N, err.max())
+        assert np.all(np.isfinite(got[N])) and np.all(got[N] >= 0) and np.all(got[N] <= dd * (1 + 1e-9))   # Cauchy-Schwarz
+    for a, b in zip(levels, levels[1:]):                       # levels are listed fine -> coarse and nest
+        if a % b == 0:
+            assert np.all(got[a] >= got[b] * (1 - 1e-7))
+
+
+def test_c2_levels(oracle, torch_cuda, sc):
+    _check_case(*_full_launch_case(oracle, torch_cuda, sc, 2, 32, 2))
+
+
+def test_c3_bench_configuration(oracle, torch_cuda, sc):
+    inp, levels, idx, ref, got, dd = _full_launch_case(oracle, torch_cuda, sc, 3, 16, 3)
+    _check_case(inp, levels, idx, ref, got, dd)
+    # Eq. 11: away from the source Upsilon_N ~ N(2N', 4N') with N' the segments the time window leaves
+    # non-empty (Q8): the population median sits at 2 N'
+    N = levels[0] * inp["evaluated_fraction"]
+    assert abs(np.median(got[levels[0]]) - 2 * N) < 5 * 2 * np.sqrt(N)
+
+
+def test_c4_noise_only_levels(oracle, torch_cuda, sc):
+    inp, levels, idx, ref, got, dd = _full_launch_case(oracle, torch_cuda, sc, 4, 12, 4)
+    _check_case(inp, levels, idx, ref, got, dd)
+    for N in levels:            # pure noise: mean 2N', sd 2 sqrt N' (Eq. 11), N' = segments inside the time window (Q8)
+        Np = N * inp["evaluated_fraction"]
+        assert abs(got[N].mean() - 2 * Np) < 2 + 6 * 2 * np.sqrt(Np) / np.sqrt(len(got[N]))
+        assert got[N].std() == pytest.approx(2 * np.sqrt(Np), rel=0.35)
+
+
+def test_c5_full_hierarchy_with_coherent_level(oracle, torch_cuda, sc):
+    inp, levels, idx, ref, got, dd = _full_launch_case(oracle, torch_cuda, sc, 5, 10, 5)
+    assert levels[-1] == 1
+    _check_case(inp, levels, idx, ref, got, dd)
+
+
+def test_default_stride_without_tile_hint(oracle, torch_cuda, sc):
+    """Without SC_OPT_TC_MAX_S the conservative default (t_c <= 10 yr) must meet the same bar."""
+    inp, levels, idx, ref, got, dd = _full_launch_case(oracle, torch_cuda, sc, 2, 8, 7, tc_hint=False)
+    _check_case(inp, levels, idx, ref, got, dd)
+
+
+# ---------------------------------------------------------------------------------------------- model variants
+@pytest.mark.parametrize("window_mode,ecc", [(0, 0), (1, 1), (0, 1)])
+def test_window_off_and_eccentric_term(oracle, torch_cuda, sc, window_mode, ecc):
+    base = sy.config_inputs(1, P=24)
+    cfgd = dict(base["cfg"], window_mode=window_mode, ecc_leading=ecc, f_ref_ecc=0.018)
+    inp = dict(base, cfg=cfgd)
+    parts = base["particles"].copy()
+    if ecc:
+        parts[:, 7] = np.random.default_rng(5).uniform(0.005, 0.1, len(parts))      # Table I prior
+        inp["injections"] = [dict(theta=np.concatenate([base["injections"][0]["theta"][:7], [0.05]]), rho=20.0)]
+    cfg, dA, dE = make_data(oracle, inp)
+    H = gpu_handle(inp, dA, dE)
+    for N in (1, 100, 1000):
+        e = sy.edges(cfgd["n_bins"], N)
+        ref = oracle.eval_stat(cfg, dA, dE, inp["S_A"], inp["S_E"], parts, e)
+        got = H.eval_stat(_dev(torch_cuda, parts), e).cpu().numpy()
+        assert rel_err(got, ref).max() <= TOL, (N, window_mode, ecc)
+    H.close()
+
+
+@pytest.mark.parametrize("pn", [0, 4])
+def test_lower_pn_orders(oracle, torch_cuda, sc, pn):
+    base = sy.config_inputs(1, P=8)
+    inp = dict(base, cfg=dict(base["cfg"], pn_order_x2=pn, window_mode=0))
+    cfg, dA, dE = make_data(oracle, inp)
+    H = gpu_handle(inp, dA, dE)
+    e = sy.edges(inp["cfg"]["n_bins"], 100)
+    ref = oracle.eval_stat(cfg, dA, dE, inp["S_A"], inp["S_E"], base["particles"], e)
+    got = H.eval_stat(_dev(torch_cuda, base["particles"]), e).cpu().numpy()
+    assert rel_err(got, ref).max() <= TOL
+    H.close()
+
+
+# ---------------------------------------------------------------------------------------------- north_star identities on the GPU
+def test_noise_free_exact_match_gives_rho_squared(oracle, torch_cuda, sc):
+    """d = kappa h(theta_inj), no noise: Upsilon_N(theta_inj) = rho^2 for N = 1 and every refinement."""
+    inp = sy.config_inputs(1, P=1)
+    cfg = oracle.make_config(inp["cfg"])
+    th = inp["injections"][0]["theta"]
+    hA, hE, _ = oracle.template(cfg, th)
+    rho = 20.0
+    kappa = rho / np.sqrt(oracle.inner(hA, hE, hA, hE, inp["S_A"], inp["S_E"], inp["df"]))
+    H = gpu_handle(inp, kappa * hA, kappa * hE)
+    for N in (1, 10, 1000):
+        got = H.eval_stat(_dev(torch_cuda, th[None, :]), sy.edges(cfg.n_bins, N)).cpu().numpy()[0]
+        assert got == pytest.approx(rho ** 2, rel=TOL)
+    H.close()
+
+
+# ---------------------------------------------------------------------------------------------- PSO
+def _pso_state(torch, pos, vel, S):
+    P = pos.shape[0]
+    return dict(pos=_dev(torch, pos), vel=_dev(torch, vel), pbest_pos=_dev(torch, pos + 0.0),
+                pbest_val=torch.full((P,), -np.inf, dtype=torch.float64, device="cuda:0"),
+                gbest_pos=torch.zeros((S, 8), dtype=torch.float64, device="cuda:0"),
+                gbest_val=torch.zeros(S, dtype=torch.float64, device="cuda:0"))
+
+
+@pytest.mark.parametrize("P,S", [(64, 1), (4000, 4), (40000, 4), (10007, 1)])
+def test_pso_step_parity(c1, oracle, torch_cuda, P, S):
+    H = c1["H"]
+    rng = np.random.default_rng(P)
+    lo, hi = c1["inp"]["lo"], c1["inp"]["hi"].copy()
+    hi[7] = 0.1
+    pos = lo + (hi - lo) * rng.random((P, 8))
+    vel = (hi - lo) * rng.uniform(-0.4, 0.4, (P, 8))           # large velocities: the boundary rule fires often
+    eps = np.array([0.1, 0.05, 0.0, 0.1, 0.1, 0.2, 0.1, 0.1]) * 0.1
+    st = _pso_state(torch_cuda, pos, vel, S)
+    o = dict(pos=pos.copy(), vel=vel.copy(), pbp=pos.copy(), pbv=np.full(P, -np.inf), gp=np.zeros((S, 8)), gv=np.zeros(S))
+    for it in range(3):
+        stat = np.round(rng.normal(100, 10, P), 0)              # rounded: many exact ties
+        H.pso_step(st, _dev(torch_cuda, stat), _dev(torch_cuda, lo), _dev(torch_cuda, hi), _dev(torch_cuda, eps),
+                   0.5, 0.2, 0.3, 12345678901234567, it, S)
+        oracle.pso_step(o["pos"], o["vel"], o["pbp"], o["pbv"], stat, o["gp"], o["gv"], lo, hi, eps, 0.5, 0.2, 0.3,
+                        12345678901234567, it, S)
+        assert np.array_equal(st["pbest_val"].cpu().numpy(), o["pbv"])
+        assert np.array_equal(st["pbest_pos"].cpu().numpy(), o["pbp"])
+        assert np.array_equal(st["gbest_val"].cpu().numpy(), o["gv"])
+        assert np.array_equal(st["gbest_pos"].cpu().numpy(), o["gp"])          # arg max incl. lowest-index tie rule
+        # Eq. 13-15: identical uniforms (bit-equal Philox) and the same association -> <= 1e-13 relative
+        span = hi - lo + 1e-300
+        assert (np.abs(st["pos"].cpu().numpy() - o["pos"]) / span).max() <= 1e-13
+        assert (np.abs(st["vel"].cpu().numpy() - o["vel"]) / span).max() <= 1e-13
+
+
+def test_pso_uniforms_bit_equal(c1, oracle, torch_cuda):
+    """omega = phi_p = 0, phi_g = 1, pos = 0, gbest = 1 in every dimension: the new position IS r_G (Q10)."""
+    H = c1["H"]
+    P = 257
+    z = np.zeros((P, 8))
+    st = _pso_state(torch_cuda, z, z, 1)
+    st["pbest_pos"] = _dev(torch_cuda, np.ones((P, 8)))
+    st["pbest_val"] = _dev(torch_cuda, np.full(P, 5.0))
+    lo, hi = np.full(8, -10.0), np.full(8, 10.0)
+    H.pso_step(st, _dev(torch_cuda, np.zeros(P)), _dev(torch_cuda, lo), _dev(torch_cuda, hi), _dev(torch_cuda, np.zeros(8)),
+               0.0, 0.0, 1.0, 987654321, 77, 1)
+    got = st["pos"].cpu().numpy()
+    for p in (0, 1, 100, 256):
+        _, rG = oracle.pso_uniforms(987654321, p, 77)
+        assert np.array_equal(got[p], rG)
+
+
+def test_device_resident_search_improves_best(c1, torch_cuda, sc):
+    """A short device-resident loop (eval + PSO, no host round trip) on config 1: the swarm best never decreases and
+    ends above the initial best (trajectory parity with the oracle is not required: arg-max flips amplify 1e-6)."""
+    inp, H = c1["inp"], c1["H"]
+    e = inp["edges"][1000]
+    st = _pso_state(torch_cuda, inp["particles"], inp["velocities"], 1)
+    lo, hi, eps = (_dev(torch_cuda, a) for a in (inp["lo"], inp["hi"], np.zeros(8)))
+    stat = torch_cuda.empty(64, dtype=torch_cuda.float64, device="cuda:0")
+    best = []
+    for it in range(12):
+        H.eval_stat(st["pos"], e, out=stat)
+        H.pso_step(st, stat, lo, hi, eps, 0.7, 1.5, 1.5, inp["pso_seed"], it, 1)
+        best.append(st["gbest_val"].item())
+    assert all(b >= a for a, b in zip(best, best[1:])) and best[-1] >= best[0]
+    pos = st["pos"].cpu().numpy()
+    assert np.all(pos >= inp["lo"]) and np.all(pos <= inp["hi"])
