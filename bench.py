@@ -45,6 +45,8 @@ def parse():
     ap.add_argument("--particles", type=int, default=None, help="override the population size (debug)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--opt", action="append", default=[], metavar="ID=VALUE",
+                    help="extra sc_set_option(ID, VALUE) calls on the handle (experiments)")
     return ap.parse_args()
 
 
@@ -197,6 +199,9 @@ def run_ours(args, rank, local_rank, world):
     # the caller knows its tile: t_c upper bound of the prior box sets the coarse node spacing (SC_OPT_TC_MAX_S)
     H.set_option(sc.SC_OPT_TC_MAX_S, int(np.ceil(inp["hi"][2])))
     H.set_option(sc.SC_OPT_PROFILE, 1)
+    for kv in args.opt:
+        k_, v_ = kv.split("=")
+        H.set_option(int(k_), int(v_))
 
     lo, hi, eps = t(inp["lo"]), t(inp["hi"]), t(np.array(hp["eps"], dtype=np.float64))
     state = dict(pos=t(inp["particles"]), vel=t(inp["velocities"]), pbest_pos=t(inp["particles"]),

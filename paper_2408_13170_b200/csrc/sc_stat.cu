@@ -132,8 +132,8 @@ template <typename R>
 __global__ void k_nodes(DevCfg c, const double* __restrict__ pc, const int* __restrict__ jlo, const int* __restrict__ jhi,
                         int P_pad, int* __restrict__ node_n, double* __restrict__ node_frac,
                         R* __restrict__ node_amp /* [node][4][P_pad] */) {
-  const int p = blockIdx.x * blockDim.x + threadIdx.x;
-  const int i = blockIdx.y;                       // 0 .. n_nodes-1  <->  node index i - kNodeOff
+  const int p = blockIdx.y * blockDim.x + threadIdx.x;
+  const int i = blockIdx.x;                       // 0 .. n_nodes-1  <->  node index i - kNodeOff
   if (p >= P_pad) return;
   const long long pos = ((long long)i - kNodeOff) << c.log2_stride;   // bin position of the node
   const int lo = jlo[p], hi = jhi[p];
@@ -206,7 +206,7 @@ struct DenseArgs {
   double seg_scale_z, seg_scale_s;
 };
 
-template <typename R, bool SEG>
+template <typename R, bool SEG, int SC>
 __global__ void __launch_bounds__(kBlock) k_dense(DevCfg c, DenseArgs a, const typename DataT<R>::W* __restrict__ Wg,
                                                   const typename DataT<R>::G* __restrict__ Gg) {
   using WT = typename DataT<R>::W;
@@ -302,18 +302,27 @@ __global__ void __launch_bounds__(kBlock) k_dense(DevCfg c, DenseArgs a, const t
 
     // one bin: phase step + reduction (FP64), sincos, amplitude cubic, multiply-accumulate
     auto bin = [&](int j, bool masked, R& zr, R& zi, R& sg) {
-      // reduce phi to |x| <= 1/8 turn, carrying the quadrant
-      const double t = fma(phi, 4.0, kMagic);
-      quad += __double2loint(t);
-      const double kf = t - kMagic;
-      phi = fma(kf, -0.25, phi);
-      R sn, cn;
-      sincos_2pi_small((R)phi, sn, cn);
-      // rotate by quad * 90 degrees
-      const bool swp = quad & 1;
-      R cr = swp ? sn : cn, sr = swp ? cn : sn;
-      cr = ((quad + 1) & 2) ? -cr : cr;
-      sr = (quad & 2) ? -sr : sr;
+      R cr, sr;
+      if (SC == 2 && sizeof(R) == 4) {
+        // The phase is never reduced in FP64: adding 1.5 * 2^20 leaves rint(phi * 2^32) mod 2^32 in the low word,
+        // i.e. the fraction of a turn in [-1/2, 1/2) as an int32; hardware sin/cos (MUFU) of that angle.
+        const int n = __double2loint(phi + 1572864.0);
+        const float xr = (float)n * 1.4629180792671596e-09f;          // 2 pi / 2^32
+        cr = (R)__cosf(xr); sr = (R)__sinf(xr);
+      } else {
+        // reduce phi to |x| <= 1/8 turn, carrying the quadrant
+        const double t = fma(phi, 4.0, kMagic);
+        quad += __double2loint(t);
+        const double kf = t - kMagic;
+        phi = fma(kf, -0.25, phi);
+        R sn, cn;
+        sincos_2pi_small((R)phi, sn, cn);
+        // rotate by quad * 90 degrees
+        const bool swp = quad & 1;
+        cr = swp ? sn : cn; sr = swp ? cn : sn;
+        cr = ((quad + 1) & 2) ? -cr : cr;
+        sr = (quad & 2) ? -sr : sr;
+      }
       // advance the forward differences to the next bin
       phi += d1; d1 += d2; d2 += d3; d3 += d4; d4 += d5;
       // amplitudes
@@ -375,7 +384,7 @@ __global__ void __launch_bounds__(kBlock) k_dense(DevCfg c, DenseArgs a, const t
 
 // ------------------------------------------------------------------------------------------------ a6
 __global__ void k_stitch(const double* __restrict__ frag, const uint8_t* __restrict__ flags, int n_chunks, int P_pad,
-                         int P, double* __restrict__ out) {
+                         int P, double scale, double* __restrict__ out) {
   const int p = blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= P) return;
   double ups = 0.0, zr = 0.0, zi = 0.0, sg = 0.0;
@@ -392,7 +401,7 @@ __global__ void k_stitch(const double* __restrict__ frag, const uint8_t* __restr
     ups += f[0];
     if (fl & CF_TAIL) { zr = f[(size_t)4 * P_pad]; zi = f[(size_t)5 * P_pad]; sg = f[(size_t)6 * P_pad]; }
   }
-  out[p] = ups;
+  out[p] = ups * scale;
 }
 
 __global__ void k_stitch_seg(const double* __restrict__ frag, const uint8_t* __restrict__ flags,
@@ -556,6 +565,28 @@ __global__ void k_pso_move(double* __restrict__ pos, double* __restrict__ vel, c
   }
 }
 
+// ------------------------------------------------------------------------------------------------ MUFU gain
+// The hardware sin/cos (MUFU) used by the fast FP32 path has a small systematic gain: <cos^2 + sin^2> over uniformly
+// distributed angles is not exactly 1.  It is measured once per handle with the very instruction sequence of the
+// dense kernel (2^20 equispaced angles, fixed-order reduction => deterministic) and divided out of Upsilon.
+__global__ void k_mufu_gain(double* __restrict__ out) {
+  __shared__ double sh[1024];
+  double acc = 0.0;
+  for (int i = 0; i < 1024; ++i) {
+    const int n = (int)(((unsigned)(i * 1024 + threadIdx.x) << 12) + 2048u);
+    const float xr = (float)n * 1.4629180792671596e-09f;
+    const float cr = __cosf(xr), sr = __sinf(xr);
+    acc += (double)cr * (double)cr + (double)sr * (double)sr;
+  }
+  sh[threadIdx.x] = acc;
+  __syncthreads();
+  for (int o = 512; o > 0; o >>= 1) {
+    if (threadIdx.x < o) sh[threadIdx.x] += sh[threadIdx.x + o];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) out[0] = sh[0] / 1048576.0;
+}
+
 // ------------------------------------------------------------------------------------------------ peaks
 // FP64 FMA throughput probe for the roofline denominator: 8 independent DFMA chains per thread.
 __global__ void k_dfma_peak(double* __restrict__ out, int iters, double a, double b) {
@@ -580,7 +611,8 @@ struct sc_handle {
   float4* W32 = nullptr; float2* G32 = nullptr; double4* W64 = nullptr; double2* G64 = nullptr;
   // options
   int precision = 0; int f32_min_seg = 8; size_t scratch_cap = (size_t)8 << 30;
-  double tc_max_s = 10.0 * 31557600.0; int forced_stride_log2 = 0;
+  double tc_max_s = 10.0 * 31557600.0; int forced_stride_log2 = 0; int sincos_mode = 0; int mufu_min_seg = 64;
+  double mufu_gain2 = 1.0;        // <cos^2 + sin^2> of the hardware sin/cos, measured at init
   // scratch
   void* scratch = nullptr; size_t scratch_bytes = 0;
   int* d_edges = nullptr; int* d_chunk_k0 = nullptr; uint8_t* d_flags = nullptr; size_t edge_cap = 0, k0_cap = 0, flags_cap = 0;
@@ -731,6 +763,8 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
 
   const int e_first = h->edges.front(), e_last = h->edges.back();
   const double four_df = 4.0 / h->cfg.T_obs_s;
+  // sin/cos flavour of the FP32 path: hardware MUFU (gain-calibrated) from mufu_min_seg segments up, else polynomial
+  const int sincos = (h->sincos_mode == 0) ? (n_seg >= h->mufu_min_seg ? 2 : 0) : (h->sincos_mode == 2 ? 2 : 0);
   const double h0 = pow(dc.f_amp_ref, -7.0 / 6.0);
   const double sz = h->s0 * h0 / four_df, ss = h->s0 * h->s0 * h0 * h0 / four_df;
 
@@ -748,7 +782,7 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
     }
     {
       Timed tm(h, st, SC_TIME_NODES);
-      k_nodes<R><<<dim3((P_pad + 127) / 128, n_nodes), 128, 0, st>>>(dc, pc, jlo, jhi, P_pad, node_n, node_frac, node_amp);
+      k_nodes<R><<<dim3(n_nodes, (P_pad + 127) / 128), 128, 0, st>>>(dc, pc, jlo, jhi, P_pad, node_n, node_frac, node_amp);
     }
     if ((rc = check_launch(h, "k_nodes"))) return rc;
     DenseArgs a;
@@ -758,17 +792,21 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
     a.seg_scale_z = sz; a.seg_scale_s = ss;
     const dim3 grid(n_chunks, P_pad / kBlock);
     {
-    Timed tm(h, st, SC_TIME_DENSE);
-    if (seg_mode) k_dense<R, true><<<grid, kBlock, 0, st>>>(dc, a, (const typename DataT<R>::W*)(sizeof(R) == 4 ? (void*)h->W32 : (void*)h->W64),
-                                                            (const typename DataT<R>::G*)(sizeof(R) == 4 ? (void*)h->G32 : (void*)h->G64));
-    else k_dense<R, false><<<grid, kBlock, 0, st>>>(dc, a, (const typename DataT<R>::W*)(sizeof(R) == 4 ? (void*)h->W32 : (void*)h->W64),
-                                                    (const typename DataT<R>::G*)(sizeof(R) == 4 ? (void*)h->G32 : (void*)h->G64));
+      Timed tm(h, st, SC_TIME_DENSE);
+      using WT = typename DataT<R>::W;
+      using GT = typename DataT<R>::G;
+      const WT* Wp = (const WT*)(sizeof(R) == 4 ? (void*)h->W32 : (void*)h->W64);
+      const GT* Gp = (const GT*)(sizeof(R) == 4 ? (void*)h->G32 : (void*)h->G64);
+      if (seg_mode) k_dense<R, true, 0><<<grid, kBlock, 0, st>>>(dc, a, Wp, Gp);
+      else if (sizeof(R) == 4 && sincos == 2) k_dense<R, false, 2><<<grid, kBlock, 0, st>>>(dc, a, Wp, Gp);
+      else k_dense<R, false, 0><<<grid, kBlock, 0, st>>>(dc, a, Wp, Gp);
     }
     if ((rc = check_launch(h, "k_dense"))) return rc;
     Timed tm2(h, st, SC_TIME_STITCH);
     if (seg_mode) k_stitch_seg<<<(Pn + 127) / 128, 128, 0, st>>>(frag, h->d_flags, h->d_chunk_k0, n_chunks, P_pad, Pn, n_seg, sz, ss,
                                                                 out_seg + (size_t)pb * n_seg * 3);
-    else k_stitch<<<(Pn + 127) / 128, 128, 0, st>>>(frag, h->d_flags, n_chunks, P_pad, Pn, out + pb);
+    else k_stitch<<<(Pn + 127) / 128, 128, 0, st>>>(frag, h->d_flags, n_chunks, P_pad, Pn,
+                                                    (sizeof(R) == 4 && sincos == 2) ? 1.0 / h->mufu_gain2 : 1.0, out + pb);
     if ((rc = check_launch(h, "k_stitch"))) return rc;
   }
   return SC_OK;
@@ -890,6 +928,14 @@ int init_common(sc_handle** out, const sc_config* cfg, const double* dA, const d
   k_whiten<<<(n + 255) / 256, 256, 0, st>>>(pA, pE, pSA, pSE, n, four_df, 1.0 / h->s0, h->W32, h->G32, h->W64, h->G64);
   h->launches++;
   SC_INIT(cudaGetLastError());
+  k_mufu_gain<<<1, 1024, 0, st>>>((double*)(h->d_counter + 1));
+  h->launches++;
+  SC_INIT(cudaMemcpyAsync(&h->mufu_gain2, h->d_counter + 1, 8, cudaMemcpyDeviceToHost, st));
+  SC_INIT(cudaStreamSynchronize(st));
+  if (!(h->mufu_gain2 > 0.999 && h->mufu_gain2 < 1.001)) {
+    fail(nullptr, SC_ERR_CUDA, "hardware sin/cos gain calibration out of range (%g)", h->mufu_gain2);
+    return bail(SC_ERR_CUDA);
+  }
   if (stage) { SC_INIT(cudaStreamSynchronize(st)); cudaFree(stage); }
 #undef SC_INIT
   *out = h;
@@ -966,7 +1012,7 @@ int sc_gen_template(sc_handle* h, const double* params, int64_t P, double* hA, d
     const int Pn = (int)std::min<int64_t>(P_pad, P - pb);
     k_particle_consts<<<1, kBlock, 0, st>>>(dc, params + pb * 8, Pn, P_pad, pc, jlo, jhi, 0, 0, h->d_counter);
     if ((rc = check_launch(h, "k_particle_consts"))) return rc;
-    k_nodes<double><<<dim3(1, n_nodes), kBlock, 0, st>>>(dc, pc, jlo, jhi, P_pad, node_n, node_frac, node_amp);
+    k_nodes<double><<<dim3(n_nodes, 1), kBlock, 0, st>>>(dc, pc, jlo, jhi, P_pad, node_n, node_frac, node_amp);
     if ((rc = check_launch(h, "k_nodes"))) return rc;
     k_template<<<dim3((dc.n_bins + 255) / 256, Pn), 256, 0, st>>>(dc, node_n, node_frac, node_amp, jlo, jhi, P_pad, Pn, h0,
                                                                  hA + (size_t)pb * dc.n_bins * 2, hE + (size_t)pb * dc.n_bins * 2);
@@ -1069,6 +1115,12 @@ int sc_set_option(sc_handle* h, int32_t option, int64_t value) {
       h->scratch_cap = (size_t)value; return SC_OK;
     case SC_OPT_PROFILE:
       h->profile = (value != 0); return SC_OK;
+    case SC_OPT_MUFU_MIN_SEG:
+      if (value < 1) return fail(h, SC_ERR_INVALID_ARG, "mufu_min_seg must be >= 1");
+      h->mufu_min_seg = (int)std::min<int64_t>(value, INT32_MAX); return SC_OK;
+    case SC_OPT_SINCOS:
+      if (value < 0 || value > 2) return fail(h, SC_ERR_INVALID_ARG, "sincos must be 0, 1 or 2");
+      h->sincos_mode = (int)value; return SC_OK;
     case SC_OPT_TC_MAX_S:
       if (value < 1) return fail(h, SC_ERR_INVALID_ARG, "tc_max_s must be >= 1");
       h->tc_max_s = (double)value; set_stride(h); return SC_OK;
