@@ -64,7 +64,7 @@ enum {
   SC_OPT_TC_MAX_S = 4,       /* the caller's upper bound on t_c [s] over the particles (the search tile's t_c range,
                                 PAPER.md:253); sets the coarse node spacing to about one day of signal time at the
                                 low band edge.  Default 10 yr.                                  */
-  SC_OPT_STRIDE_LOG2 = 5,    /* 0 = automatic (rule above), else log2 of the coarse node spacing in bins (2..12)   */
+  SC_OPT_STRIDE_LOG2 = 5,    /* 0 = automatic (rule above), else log2 of the coarse node spacing in bins (3..12)   */
   SC_OPT_PROFILE = 6,        /* 1 = record a CUDA event pair around every kernel launch (read by sc_get_timing)     */
   SC_OPT_SINCOS = 7,         /* FP32 amplitude path: sin/cos of the phase.  0 = automatic: hardware MUFU sin/cos
                                 (gain-calibrated at init) when n_seg >= SC_OPT_MUFU_MIN_SEG, else FP32 polynomial;

@@ -48,25 +48,37 @@ __global__ void k_max_weight(const double* __restrict__ S_A, const double* __res
 }
 
 // W_a = d_a * (4 df / S_a) / s0,  G_a = (4 df / S_a) / s0^2  with s0 a power of two (exact rescaling).
-__global__ void k_whiten(const double* __restrict__ dA, const double* __restrict__ dE,
-                         const double* __restrict__ S_A, const double* __restrict__ S_E, int n, double four_df,
-                         double inv_s0, float4* __restrict__ W32, float2* __restrict__ G32,
-                         double4* __restrict__ W64, double2* __restrict__ G64) {
-  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+// FP64 copies per bin (all-FP64 path) and the FP32 copy in the bin-pair layout of k_dense2: for pair m = bins
+// (2m, 2m+1) three 16-byte records (wAr, wAi), (wEr, wEi), (gA, gE), each field as (even bin, odd bin); bins past
+// n_bins (padding up to a whole chunk) are zero.
+__device__ __forceinline__ void whiten_bin(const double* __restrict__ dA, const double* __restrict__ dE,
+                                           const double* __restrict__ S_A, const double* __restrict__ S_E, int j, int n,
+                                           double four_df, double inv_s0, double4& w, double2& g) {
+  w = make_double4(0.0, 0.0, 0.0, 0.0); g = make_double2(0.0, 0.0);
   if (j >= n) return;
   const double a = S_A[j], e = S_E[j];
   const double ua = (isfinite(a) && a > 0.0) ? four_df / a : 0.0;
   const double ue = (isfinite(e) && e > 0.0) ? four_df / e : 0.0;
-  double4 w;
   w.x = dA[2 * j] * ua * inv_s0; w.y = dA[2 * j + 1] * ua * inv_s0;
   w.z = dE[2 * j] * ue * inv_s0; w.w = dE[2 * j + 1] * ue * inv_s0;
   if (!(isfinite(w.x) && isfinite(w.y))) { w.x = 0.0; w.y = 0.0; }
   if (!(isfinite(w.z) && isfinite(w.w))) { w.z = 0.0; w.w = 0.0; }
-  double2 g;
   g.x = ua * inv_s0 * inv_s0; g.y = ue * inv_s0 * inv_s0;
-  W64[j] = w; G64[j] = g;
-  W32[j] = make_float4((float)w.x, (float)w.y, (float)w.z, (float)w.w);
-  G32[j] = make_float2((float)g.x, (float)g.y);
+}
+__global__ void k_whiten(const double* __restrict__ dA, const double* __restrict__ dE,
+                         const double* __restrict__ S_A, const double* __restrict__ S_E, int n, int n_pairs_pad,
+                         double four_df, double inv_s0, float4* __restrict__ D32,
+                         double4* __restrict__ W64, double2* __restrict__ G64) {
+  const int m = blockIdx.x * blockDim.x + threadIdx.x;
+  if (m >= n_pairs_pad) return;
+  double4 w0, w1; double2 g0, g1;
+  whiten_bin(dA, dE, S_A, S_E, 2 * m, n, four_df, inv_s0, w0, g0);
+  whiten_bin(dA, dE, S_A, S_E, 2 * m + 1, n, four_df, inv_s0, w1, g1);
+  if (2 * m < n) { W64[2 * m] = w0; G64[2 * m] = g0; }
+  if (2 * m + 1 < n) { W64[2 * m + 1] = w1; G64[2 * m + 1] = g1; }
+  D32[3 * (size_t)m + 0] = make_float4((float)w0.x, (float)w1.x, (float)w0.y, (float)w1.y);
+  D32[3 * (size_t)m + 1] = make_float4((float)w0.z, (float)w1.z, (float)w0.w, (float)w1.w);
+  D32[3 * (size_t)m + 2] = make_float4((float)g0.x, (float)g1.x, (float)g0.y, (float)g1.y);
 }
 
 // ------------------------------------------------------------------------------------------------ a1 + a3
@@ -206,9 +218,13 @@ struct DenseArgs {
   double seg_scale_z, seg_scale_s;
 };
 
-template <typename R, bool SEG, int SC>
-__global__ void __launch_bounds__(kBlock) k_dense(DevCfg c, DenseArgs a, const typename DataT<R>::W* __restrict__ Wg,
-                                                  const typename DataT<R>::G* __restrict__ Gg) {
+// All-FP64 flavour (few segments, N_seg < 8 by default): one bin per step, quintic phase by 5 forward differences,
+// FP64 polynomial sin/cos, FP64 amplitudes and accumulation.
+template <bool SEG>
+__global__ void __launch_bounds__(kBlock) k_dense(DevCfg c, DenseArgs a, const double4* __restrict__ Wg,
+                                                  const double2* __restrict__ Gg) {
+  using R = double;
+  constexpr int SC = 0;
   using WT = typename DataT<R>::W;
   using GT = typename DataT<R>::G;
   constexpr int CH = DataT<R>::chunk;
@@ -376,6 +392,264 @@ __global__ void __launch_bounds__(kBlock) k_dense(DevCfg c, DenseArgs a, const t
         open_at_edge = true;
       }
     }
+  }
+  // the piece still open at the chunk end
+  if (k >= 0 && k < a.n_seg) close_piece(false);
+  if (!SEG) frag[0] = ups;
+}
+
+
+// ------------------------------------------------------------------------------------------------ a4 + a5, FP32x2
+// The FP32-amplitude flavour of the hot loop, written for the packed FP32 pipe of sm_100a (FFMA2 / FMUL2 / FADD2:
+// one issue slot carries two FP32 operations).  Each lane (= particle) walks its chunk two bins at a time: the low
+// half of every packed register belongs to the even bin 2m, the high half to the odd bin 2m+1, so the whole
+// per-bin arithmetic (amplitude cubics, the complex multiply-accumulate with the data, |h|^2) is element-wise and
+// needs no swizzle.  Segment edges on odd bins split a pair between two segments (the pair is evaluated once).
+// Phase: per fine sub-interval the 6-node quintic is economised (Chebyshev) to a cubic and advanced by forward
+// differences, 3 FP64 adds per bin; the fraction of a turn is read from the low word of phi + 1.5 * 2^20.
+typedef unsigned long long u64;
+__device__ __forceinline__ u64 f2pack(float lo, float hi) { u64 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ void f2unpack(u64 v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ u64 f2fma(u64 a, u64 b, u64 c) { u64 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
+__device__ __forceinline__ u64 f2mul(u64 a, u64 b) { u64 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ u64 f2add(u64 a, u64 b) { u64 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ u64 f2neg(u64 a) { float lo, hi; f2unpack(a, lo, hi); return f2pack(-lo, -hi); }   // folded into FFMA2 by ptxas
+__device__ __forceinline__ u64 f2bcast(float v) { return f2pack(v, v); }
+
+__device__ __forceinline__ u64 f2sub(u64 a, u64 b) { u64 r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+
+// Cubic coefficients on fine sub-interval q for two amplitude components at once (the halves of the packed registers):
+// kFineM applied to node[m] - node[2], so that the rounding of the matrix entries acts on small differences only.
+__device__ __forceinline__ void fine_cubic2(const u64 nd[6], int q, u64 out[4]) {
+  u64 dl[6];
+#pragma unroll
+  for (int m = 0; m < 6; ++m) dl[m] = f2sub(nd[m], nd[2]);
+#pragma unroll
+  for (int kk = 0; kk < 4; ++kk) {
+    u64 acc = (kk == 0) ? nd[2] : 0ull;
+#pragma unroll
+    for (int m = 0; m < 6; ++m)
+      if (m != 2) acc = f2fma(f2bcast(kFineM[q][kk][m]), dl[m], acc);
+    out[kk] = acc;
+  }
+}
+
+constexpr int kPairRec = 3;            // ulonglong2 records per bin pair: (wAr, wAi), (wEr, wEi), (gA, gE), each (even, odd)
+
+// FP32 sin/cos of a phase given as a signed 32-bit fraction of a turn: polynomial flavour (SC = 0).
+__device__ __forceinline__ void sincos_frac32(int n, float& sr, float& cr) {
+  const int q = (n + (1 << 29)) >> 30;                       // nearest quarter turn
+  const float x = (float)(n - (q << 30)) * 2.3283064365386963e-10f;   // |x| <= 1/8 turn
+  float sn, cn;
+  sincos_2pi_small(x, sn, cn);
+  const bool swp = q & 1;
+  cr = swp ? sn : cn; sr = swp ? cn : sn;
+  cr = ((q + 1) & 2) ? -cr : cr;
+  sr = (q & 2) ? -sr : sr;
+}
+
+template <bool SEG, int SC>
+__global__ void __launch_bounds__(kBlock) k_dense2(DevCfg c, DenseArgs a, const ulonglong2* __restrict__ Dg) {
+  constexpr int CH = kChunkF32;
+  __shared__ ulonglong2 sD[CH / 2 * kPairRec];                 // 48 KB
+
+  const int chunk_l = blockIdx.x;
+  const int cs = (a.chunk_first + chunk_l) * CH;
+  const int ce = min(cs + CH, c.n_bins);
+  const int ce2 = (ce + 1) & ~1;                               // pair-aligned end (data beyond n_bins is zero)
+  const int p = blockIdx.y * kBlock + threadIdx.x;
+
+  {
+    const ulonglong2* src = Dg + (size_t)(cs >> 1) * kPairRec;
+#pragma unroll 4
+    for (int t = threadIdx.x; t < CH / 2 * kPairRec; t += kBlock) sD[t] = src[t];
+  }
+  __syncthreads();
+
+  const int jlo = a.jlo[p], jhi = a.jhi[p];
+  const int S = c.stride, Sf = S >> 2;
+  const float hS = 1.0f / (float)Sf;
+  const u64 h2 = f2bcast(2.0f * hS);
+  const u64 K2 = f2bcast(1.4629180792671596e-09f);            // 2 pi / 2^32
+  const float* __restrict__ namp = reinterpret_cast<const float*>(a.node_amp);
+
+  int k = a.chunk_k0[chunk_l];
+  int next_edge = (k + 1 <= a.n_seg) ? a.edges[k + 1] : INT_MAX;
+  bool open_at_edge = (k >= 0 && k < a.n_seg) ? (a.edges[k] == cs) : true;
+  double Zr = 0.0, Zi = 0.0, Sg = 0.0, ups = 0.0;
+  double* frag = a.frag + (size_t)chunk_l * kFragFields * a.P_pad + p;
+
+  auto close_piece = [&](bool at_edge_end) {
+    if (open_at_edge && at_edge_end) {
+      if (SEG) {
+        if (p < a.P) {
+          double* o = a.out_seg + ((size_t)p * a.n_seg + k) * 3;
+          o[0] = Zr * a.seg_scale_z; o[1] = Zi * a.seg_scale_z; o[2] = Sg * a.seg_scale_s;
+        }
+      } else if (Sg > 0.0) {
+        ups += (Zr * Zr + Zi * Zi) / Sg;
+      }
+    } else if (!open_at_edge) {
+      frag[(size_t)1 * a.P_pad] = Zr; frag[(size_t)2 * a.P_pad] = Zi; frag[(size_t)3 * a.P_pad] = Sg;
+    } else {
+      frag[(size_t)4 * a.P_pad] = Zr; frag[(size_t)5 * a.P_pad] = Zi; frag[(size_t)6 * a.P_pad] = Sg;
+    }
+    Zr = 0.0; Zi = 0.0; Sg = 0.0;
+  };
+  auto next_segment = [&]() {
+    ++k;
+    next_edge = (k + 1 <= a.n_seg) ? a.edges[k + 1] : INT_MAX;
+    open_at_edge = true;
+  };
+
+  double phi = 0.0, d1 = 0.0, d2 = 0.0, d3 = 0.0;
+  for (int ib = cs; ib < ce2; ib += Sf) {
+    const int ie = min(ib + Sf, ce2);
+    const bool lane_in = (ib >= jlo) && (ie <= jhi);
+    const bool lane_out = (ie <= jlo) || (ib >= jhi);
+    const bool all_in = __all_sync(0xffffffffu, lane_in);
+    const bool all_out = __all_sync(0xffffffffu, lane_out);
+
+    float cf[4][4];    // cubic coefficients of (Ar, Ai, Er, Ei) in s = (j - ib)/Sf (FFMA2 broadcasts a scalar operand)
+    if (!all_out) {
+      const int ic = ib >> c.log2_stride;
+      const int i0 = ic + kNodeOff;
+      const int q = (ib >> (c.log2_stride - 2)) & 3;
+      {
+        // phase: quintic through 6 nodes -> Taylor shift to the centre of the fine sub-interval -> Chebyshev
+        // economisation to a cubic on [-H, H] -> shift to the start -> forward differences for unit steps
+        const size_t base = (size_t)i0 * a.P_pad + p;
+        const int n0 = a.node_n[base];
+        const double r0 = a.node_frac[base];
+        double Y[6];
+#pragma unroll
+        for (int m = -2; m <= 3; ++m) {
+          const size_t at = (size_t)(i0 + m) * a.P_pad + p;
+          Y[m + 2] = (double)(a.node_n[at] - n0) + (a.node_frac[at] - r0);
+        }
+        double b[6];
+        quintic_coeffs(Y, 1.0 / (double)S, b);
+        const double H = 0.5 * (double)Sf;
+        taylor_shift(b, (double)(ib - (ic << c.log2_stride)) + H);
+        const double H2 = H * H, H4 = H2 * H2;
+        b[0] = fma(-0.125 * H4, b[4], b[0]);
+        b[2] = fma(H2, b[4], b[2]);
+        b[1] = fma(-0.3125 * H4, b[5], b[1]);
+        b[3] = fma(1.25 * H2, b[5], b[3]);
+#pragma unroll
+        for (int i = 0; i < 3; ++i)
+#pragma unroll
+          for (int j = 2; j >= i; --j) b[j] = fma(-H, b[j + 1], b[j]);
+        phi = r0 + b[0];
+        d1 = b[1] + b[2] + b[3];
+        d2 = 2.0 * b[2] + 6.0 * b[3];
+        d3 = 6.0 * b[3];
+      }
+#pragma unroll
+      for (int r = 0; r < 4; r += 2) {                          // (Ar, Ai) then (Er, Ei) as packed halves
+        const float* col = namp + ((size_t)i0 * 4 + r) * a.P_pad + p;
+        const ptrdiff_t st = (ptrdiff_t)4 * a.P_pad;
+        u64 nd[6], o[4];
+#pragma unroll
+        for (int m = -2; m <= 3; ++m) nd[m + 2] = f2pack(col[m * st], col[m * st + a.P_pad]);
+        fine_cubic2(nd, q, o);
+#pragma unroll
+        for (int kk = 0; kk < 4; ++kk) f2unpack(o[kk], cf[r][kk], cf[r + 1][kk]);
+      }
+    }
+
+    u64 s2 = 0;        // (s_j, s_{j+1}) of the next pair
+    const ulonglong2* rec = sD;   // its data record
+    // one bin pair (j, j+1): FP64 phase steps, sin/cos, amplitude cubics, multiply-accumulate into packed sums
+    auto pair = [&](int j, bool masked, u64& zr2, u64& zi2, u64& sg2) {
+      const int n0 = __double2loint(phi + 1572864.0);
+      phi += d1; d1 += d2; d2 += d3;
+      const int n1 = __double2loint(phi + 1572864.0);
+      phi += d1; d1 += d2; d2 += d3;
+      float c0, c1, s0, s1;
+      if (SC == 2) {
+        float x0, x1;
+        f2unpack(f2mul(f2pack((float)n0, (float)n1), K2), x0, x1);
+        c0 = __cosf(x0); s0 = __sinf(x0); c1 = __cosf(x1); s1 = __sinf(x1);
+      } else {
+        sincos_frac32(n0, s0, c0);
+        sincos_frac32(n1, s1, c1);
+      }
+      u64 cr2 = f2pack(c0, c1), sr2 = f2pack(s0, s1);
+      const u64 Ar = f2fma(f2fma(f2fma(f2bcast(cf[0][3]), s2, f2bcast(cf[0][2])), s2, f2bcast(cf[0][1])), s2, f2bcast(cf[0][0]));
+      const u64 Ai = f2fma(f2fma(f2fma(f2bcast(cf[1][3]), s2, f2bcast(cf[1][2])), s2, f2bcast(cf[1][1])), s2, f2bcast(cf[1][0]));
+      const u64 Er = f2fma(f2fma(f2fma(f2bcast(cf[2][3]), s2, f2bcast(cf[2][2])), s2, f2bcast(cf[2][1])), s2, f2bcast(cf[2][0]));
+      const u64 Ei = f2fma(f2fma(f2fma(f2bcast(cf[3][3]), s2, f2bcast(cf[3][2])), s2, f2bcast(cf[3][1])), s2, f2bcast(cf[3][0]));
+      s2 = f2add(s2, h2);
+      const ulonglong2 wA = rec[0], wE = rec[1];
+      ulonglong2 g = rec[2];
+      rec += kPairRec;
+      if (masked) {
+        const u64 m2 = f2pack((j >= jlo && j < jhi) ? 1.0f : 0.0f, (j + 1 >= jlo && j + 1 < jhi) ? 1.0f : 0.0f);
+        cr2 = f2mul(cr2, m2); sr2 = f2mul(sr2, m2); g.x = f2mul(g.x, m2); g.y = f2mul(g.y, m2);
+      }
+      // q = W_A conj(c_A) + W_E conj(c_E)
+      const u64 qr = f2fma(wA.x, Ar, f2fma(wA.y, Ai, f2fma(wE.x, Er, f2mul(wE.y, Ei))));
+      const u64 qi = f2fma(wA.y, Ar, f2fma(f2neg(wA.x), Ai, f2fma(wE.y, Er, f2neg(f2mul(wE.x, Ei)))));
+      sg2 = f2fma(g.x, f2fma(Ar, Ar, f2mul(Ai, Ai)), f2fma(g.y, f2fma(Er, Er, f2mul(Ei, Ei)), sg2));
+      // z += q e^{+2 pi i Phi}
+      zr2 = f2fma(qr, cr2, f2fma(f2neg(qi), sr2, zr2));
+      zi2 = f2fma(qr, sr2, f2fma(qi, cr2, zi2));
+    };
+    auto fold = [&](u64 zr2, u64 zi2, u64 sg2, bool lo, bool hi) {
+      float l, h;
+      f2unpack(zr2, l, h); Zr += (double)((lo ? l : 0.0f) + (hi ? h : 0.0f));
+      f2unpack(zi2, l, h); Zi += (double)((lo ? l : 0.0f) + (hi ? h : 0.0f));
+      f2unpack(sg2, l, h); Sg += (double)((lo ? l : 0.0f) + (hi ? h : 0.0f));
+    };
+
+    int j = ib;
+    while (j < ie) {
+      while (next_edge == j) {                                 // edges on the pair start (incl. empty segments)
+        if (k >= 0 && k < a.n_seg) close_piece(true);
+        next_segment();
+      }
+      bool live = (k >= 0) && (k < a.n_seg);
+      if (next_edge == j + 1) {
+        // an edge between the two bins of this pair: evaluate it once, low half -> segment k, high half -> the next
+        u64 zr2 = 0, zi2 = 0, sg2 = 0;
+        if (!all_out) {
+          s2 = f2pack((float)(j - ib) * hS, (float)(j + 1 - ib) * hS);
+          rec = sD + ((j - cs) >> 1) * kPairRec;
+          pair(j, true, zr2, zi2, sg2);
+        }
+        if (live) fold(zr2, zi2, sg2, true, false);
+        while (next_edge == j + 1) {
+          if (k >= 0 && k < a.n_seg) close_piece(true);
+          next_segment();
+        }
+        if ((k >= 0) && (k < a.n_seg)) fold(zr2, zi2, sg2, false, true);
+        j += 2;
+        continue;
+      }
+      const int b = min(ie, next_edge & ~1);                   // next_edge >= j + 2 here
+      if (all_out) {
+        // nothing to add; the phase is rebuilt at the next sub-interval
+      } else if (!live) {
+        for (int jj = j; jj < b; ++jj) { phi += d1; d1 += d2; d2 += d3; }
+      } else {
+        s2 = f2pack((float)(j - ib) * hS, (float)(j + 1 - ib) * hS);
+        rec = sD + ((j - cs) >> 1) * kPairRec;
+        for (int jj = j; jj < b;) {
+          const int e2 = min(jj + kFlushBins, b);
+          u64 zr2 = 0, zi2 = 0, sg2 = 0;
+          if (all_in) { for (; jj < e2; jj += 2) pair(jj, false, zr2, zi2, sg2); }
+          else        { for (; jj < e2; jj += 2) pair(jj, true, zr2, zi2, sg2); }
+          fold(zr2, zi2, sg2, true, true);
+        }
+      }
+      j = b;
+    }
+  }
+  // a segment that ends exactly on the chunk end closes here (the host's CF_HEAD_CLOSES rule says the same)
+  if (next_edge == ce2) {
+    if (k >= 0 && k < a.n_seg) close_piece(true);
+    next_segment();
   }
   // the piece still open at the chunk end
   if (k >= 0 && k < a.n_seg) close_piece(false);
@@ -608,10 +882,11 @@ struct sc_handle {
   DevCfg dc;
   int device = 0;
   double s0 = 1.0;                 // weight scale (power of two)
-  float4* W32 = nullptr; float2* G32 = nullptr; double4* W64 = nullptr; double2* G64 = nullptr;
+  float4* D32 = nullptr; double4* W64 = nullptr; double2* G64 = nullptr;   // D32: bin-pair layout of k_dense2
   // options
   int precision = 0; int f32_min_seg = 8; size_t scratch_cap = (size_t)8 << 30;
   double tc_max_s = 10.0 * 31557600.0; int forced_stride_log2 = 0; int sincos_mode = 0; int mufu_min_seg = 64;
+  int lg_f32 = 5, lg_f64 = 5;      // log2 of the coarse node spacing per precision mode (set_stride)
   double mufu_gain2 = 1.0;        // <cos^2 + sin^2> of the hardware sin/cos, measured at init
   // scratch
   void* scratch = nullptr; size_t scratch_bytes = 0;
@@ -634,14 +909,23 @@ struct sc_handle {
 namespace {
 
 int fail(sc_handle* h, int code, const char* fmt, ...);
-int pick_stride_log2(const sc_config& cfg, double tc_max_s, int forced);
+int pick_stride_log2(const sc_config& cfg, double tc_max_s, int forced, double max_days);
 
-void set_stride(sc_handle* h) {
-  DevCfg& d = h->dc;
-  d.log2_stride = pick_stride_log2(h->cfg, h->tc_max_s, h->forced_stride_log2);
-  d.stride = 1 << d.log2_stride;
+// Node spacing per precision mode: the all-FP64 path (N_seg < 8, where 1e-8 rad matters)
+// keeps the nodes <= 2 days of signal time apart, the FP32-amplitude path (error floor ~1e-8 relative) <= 4 days.
+constexpr double kNodeDaysF64 = 2.0, kNodeDaysF32 = 4.0;
+
+void apply_stride(DevCfg& d, int lg) {
+  d.log2_stride = lg;
+  d.stride = 1 << lg;
   const int n_int = (d.n_bins + d.stride - 1) / d.stride;
   d.n_nodes = n_int + kNodeOff + 4;
+}
+
+void set_stride(sc_handle* h) {
+  h->lg_f64 = pick_stride_log2(h->cfg, h->tc_max_s, h->forced_stride_log2, kNodeDaysF64);
+  h->lg_f32 = pick_stride_log2(h->cfg, h->tc_max_s, h->forced_stride_log2, kNodeDaysF32);
+  apply_stride(h->dc, h->lg_f64);
 }
 
 int fail(sc_handle* h, int code, const char* fmt, ...) {
@@ -682,18 +966,16 @@ int check_launch(sc_handle* h, const char* what) {
 }
 
 // Coarse node spacing: the slowly varying amplitudes change on the orbital time scale,
-// so the spacing is set in TIME: about one day at the slowest-chirping corner of the problem.  Time per bin is
+// so the spacing is set in TIME: at most max_days at the slowest-chirping corner of the problem.  Time per bin is
 // |dt/df| df = (8/3) tau / (f T_obs) with tau <= tc_max (Newtonian), largest at the low band edge.
-int pick_stride_log2(const sc_config& cfg, double tc_max_s, int forced) {
-  if (forced > 0) return std::min(std::max(forced, 2), 12);
+int pick_stride_log2(const sc_config& cfg, double tc_max_s, int forced, double max_days) {
+  if (forced > 0) return std::min(std::max(forced, 3), 12);
   const double f_lo = (double)std::max<int64_t>(cfg.j0, 1) / cfg.T_obs_s;
   const double s_per_bin = (8.0 / 3.0) * tc_max_s / (f_lo * cfg.T_obs_s);
   int lg = 5;
-  while (lg < 10 && (double)(2 << lg) * s_per_bin <= 86400.0) ++lg;
+  while (lg < 11 && (double)(2 << lg) * s_per_bin <= max_days * 86400.0) ++lg;
   return lg;
 }
-
-
 
 int grow(sc_handle* h, void** ptr, size_t* cap, size_t need) {
   if (*cap >= need) return SC_OK;
@@ -735,9 +1017,9 @@ void analyse_edges(sc_handle* h, int CH) {
 template <typename R>
 int run_batches(sc_handle* h, const double* params, int64_t P, double* out, double* out_seg, cudaStream_t st,
                 bool seg_mode) {
-  constexpr int CH = DataT<R>::chunk;
   const int n_seg = (int)h->edges.size() - 1;
-  const DevCfg& dc = h->dc;
+  DevCfg dc = h->dc;
+  apply_stride(dc, sizeof(R) == 4 ? h->lg_f32 : h->lg_f64);
   const int n_nodes = dc.n_nodes;
   const int n_chunks = h->n_chunks;
   // per-particle scratch bytes
@@ -793,13 +1075,15 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
     const dim3 grid(n_chunks, P_pad / kBlock);
     {
       Timed tm(h, st, SC_TIME_DENSE);
-      using WT = typename DataT<R>::W;
-      using GT = typename DataT<R>::G;
-      const WT* Wp = (const WT*)(sizeof(R) == 4 ? (void*)h->W32 : (void*)h->W64);
-      const GT* Gp = (const GT*)(sizeof(R) == 4 ? (void*)h->G32 : (void*)h->G64);
-      if (seg_mode) k_dense<R, true, 0><<<grid, kBlock, 0, st>>>(dc, a, Wp, Gp);
-      else if (sizeof(R) == 4 && sincos == 2) k_dense<R, false, 2><<<grid, kBlock, 0, st>>>(dc, a, Wp, Gp);
-      else k_dense<R, false, 0><<<grid, kBlock, 0, st>>>(dc, a, Wp, Gp);
+      if (sizeof(R) == 4) {
+        const ulonglong2* Dp = reinterpret_cast<const ulonglong2*>(h->D32);
+        if (seg_mode) k_dense2<true, 0><<<grid, kBlock, 0, st>>>(dc, a, Dp);
+        else if (sincos == 2) k_dense2<false, 2><<<grid, kBlock, 0, st>>>(dc, a, Dp);
+        else k_dense2<false, 0><<<grid, kBlock, 0, st>>>(dc, a, Dp);
+      } else {
+        if (seg_mode) k_dense<true><<<grid, kBlock, 0, st>>>(dc, a, h->W64, h->G64);
+        else k_dense<false><<<grid, kBlock, 0, st>>>(dc, a, h->W64, h->G64);
+      }
     }
     if ((rc = check_launch(h, "k_dense"))) return rc;
     Timed tm2(h, st, SC_TIME_STITCH);
@@ -898,8 +1182,8 @@ int init_common(sc_handle** out, const sc_config* cfg, const double* dA, const d
                                      "%s failed: %s", #call, cudaGetErrorString(e_));              \
                                 return bail(e_ == cudaErrorMemoryAllocation ? SC_ERR_OOM : SC_ERR_CUDA); } } while (0)
   SC_INIT(cudaGetDevice(&h->device));
-  SC_INIT(cudaMalloc(&h->W32, (size_t)n * sizeof(float4)));
-  SC_INIT(cudaMalloc(&h->G32, (size_t)n * sizeof(float2)));
+  const int n_pairs_pad = (n + kChunkF32 - 1) / kChunkF32 * (kChunkF32 / 2);
+  SC_INIT(cudaMalloc(&h->D32, (size_t)n_pairs_pad * kPairRec * sizeof(float4)));
   SC_INIT(cudaMalloc(&h->W64, (size_t)n * sizeof(double4)));
   SC_INIT(cudaMalloc(&h->G64, (size_t)n * sizeof(double2)));
   SC_INIT(cudaMalloc(&h->d_counter, 16));
@@ -925,7 +1209,7 @@ int init_common(sc_handle** out, const sc_config* cfg, const double* dA, const d
   int ex = 0;
   if (umax > 0.0 && std::isfinite(umax)) { frexp(umax, &ex); }       // umax = m 2^ex, m in [0.5, 1)
   h->s0 = ldexp(1.0, (ex + 1) / 2);                                   // s0^2 >= umax, power of two
-  k_whiten<<<(n + 255) / 256, 256, 0, st>>>(pA, pE, pSA, pSE, n, four_df, 1.0 / h->s0, h->W32, h->G32, h->W64, h->G64);
+  k_whiten<<<(n_pairs_pad + 255) / 256, 256, 0, st>>>(pA, pE, pSA, pSE, n, n_pairs_pad, four_df, 1.0 / h->s0, h->D32, h->W64, h->G64);
   h->launches++;
   SC_INIT(cudaGetLastError());
   k_mufu_gain<<<1, 1024, 0, st>>>((double*)(h->d_counter + 1));
@@ -1125,7 +1409,7 @@ int sc_set_option(sc_handle* h, int32_t option, int64_t value) {
       if (value < 1) return fail(h, SC_ERR_INVALID_ARG, "tc_max_s must be >= 1");
       h->tc_max_s = (double)value; set_stride(h); return SC_OK;
     case SC_OPT_STRIDE_LOG2:
-      if (value != 0 && (value < 2 || value > 12)) return fail(h, SC_ERR_INVALID_ARG, "stride_log2 must be 0 (auto) or 2..12");
+      if (value != 0 && (value < 3 || value > 12)) return fail(h, SC_ERR_INVALID_ARG, "stride_log2 must be 0 (auto) or 3..12");
       h->forced_stride_log2 = (int)value; set_stride(h); return SC_OK;
     default:
       return fail(h, SC_ERR_INVALID_ARG, "unknown option %d", (int)option);
@@ -1134,7 +1418,7 @@ int sc_set_option(sc_handle* h, int32_t option, int64_t value) {
 
 int sc_free(sc_handle* h) {
   if (!h) return SC_ERR_NOT_INIT;
-  cudaFree(h->W32); cudaFree(h->G32); cudaFree(h->W64); cudaFree(h->G64);
+  cudaFree(h->D32); cudaFree(h->W64); cudaFree(h->G64);
   cudaFree(h->scratch); cudaFree(h->d_edges); cudaFree(h->d_chunk_k0); cudaFree(h->d_flags);
   cudaFree(h->d_counter); cudaFree(h->d_params_stage);
   for (auto& e : h->evs) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
