@@ -18,6 +18,7 @@
 #include <cstdio>
 #include <cstring>
 #include <string>
+#include <type_traits>
 #include <vector>
 
 using namespace sc;
@@ -199,7 +200,6 @@ __device__ __forceinline__ void sincos_2pi_small(double x, double& s, double& c)
 }
 
 template <typename R> struct DataT;
-template <> struct DataT<float> { using W = float4; using G = float2; static constexpr int chunk = kChunkF32; };
 template <> struct DataT<double> { using W = double4; using G = double2; static constexpr int chunk = kChunkF64; };
 
 struct DenseArgs {
@@ -216,6 +216,9 @@ struct DenseArgs {
   double* out_seg;             // SEG mode: [P][n_seg][3] (already offset to this batch), else nullptr
   int P;                       // particles in this batch
   double seg_scale_z, seg_scale_s;
+  // k_dense2 only: pieces = fine sub-intervals cut at the segment edges, with the moments of the sigma weights
+  const int* piece_first;      // [n_sub_launched + 1] first piece of each launched fine sub-interval
+  const ulonglong2* moments;   // [n_pieces][4] = 8 packed (A, E) pairs: sum_j g_a(j) s_j^m, m = 0..6, pad
 };
 
 // All-FP64 flavour (few segments, N_seg < 8 by default): one bin per step, quintic phase by 5 forward differences,
@@ -434,7 +437,34 @@ __device__ __forceinline__ void fine_cubic2(const u64 nd[6], int q, u64 out[4]) 
   }
 }
 
-constexpr int kPairRec = 3;            // ulonglong2 records per bin pair: (wAr, wAi), (wEr, wEi), (gA, gE), each (even, odd)
+#ifndef SC_DENSE2_MINB
+#define SC_DENSE2_MINB 4     /* CTAs per SM the register allocation aims at (128 registers/thread) */
+#endif
+constexpr int kPairRec = 3;
+
+// Moments of the sigma weights over one piece (a fine sub-interval cut at the segment edges; shared by all particles):
+//   M_a,m = sum_{j in piece} G_a(j) s_j^m,  s_j = (j - sub-interval start)/Sf,  m = 0..6,  a = A, E.
+// On a fine sub-interval the amplitudes are cubics in s, so |c_a(s)|^2 is a polynomial of degree 6 and
+// sigma_piece = sum_m (e_A,m M_A,m + e_E,m M_E,m) -- the per-bin evaluation of |h|^2 leaves the hot loop.
+__global__ void k_moments(const double2* __restrict__ G64, const int* __restrict__ piece_lo, const int* __restrict__ piece_hi,
+                          int n_pieces, int n_bins, int log2_fine, float2* __restrict__ out /* [n_pieces][8] */) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n_pieces) return;
+  const int lo = piece_lo[i], hi = min(piece_hi[i], n_bins);
+  const int ib = (lo >> log2_fine) << log2_fine;
+  const double hS = 1.0 / (double)(1 << log2_fine);
+  double mA[7] = {0, 0, 0, 0, 0, 0, 0}, mE[7] = {0, 0, 0, 0, 0, 0, 0};
+  for (int j = lo; j < hi; ++j) {
+    const double2 g = G64[j];
+    const double sj = (double)(j - ib) * hS;
+    double pw = 1.0;
+#pragma unroll
+    for (int m = 0; m < 7; ++m) { mA[m] = fma(g.x, pw, mA[m]); mE[m] = fma(g.y, pw, mE[m]); pw *= sj; }
+  }
+#pragma unroll
+  for (int m = 0; m < 7; ++m) out[(size_t)i * 8 + m] = make_float2((float)mA[m], (float)mE[m]);
+  out[(size_t)i * 8 + 7] = make_float2(0.f, 0.f);
+}            // ulonglong2 records per bin pair: (wAr, wAi), (wEr, wEi), (gA, gE), each (even, odd)
 
 // FP32 sin/cos of a phase given as a signed 32-bit fraction of a turn: polynomial flavour (SC = 0).
 __device__ __forceinline__ void sincos_frac32(int n, float& sr, float& cr) {
@@ -449,7 +479,7 @@ __device__ __forceinline__ void sincos_frac32(int n, float& sr, float& cr) {
 }
 
 template <bool SEG, int SC>
-__global__ void __launch_bounds__(kBlock) k_dense2(DevCfg c, DenseArgs a, const ulonglong2* __restrict__ Dg) {
+__global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2(DevCfg c, DenseArgs a, const ulonglong2* __restrict__ Dg) {
   constexpr int CH = kChunkF32;
   __shared__ ulonglong2 sD[CH / 2 * kPairRec];                 // 48 KB
 
@@ -560,8 +590,11 @@ __global__ void __launch_bounds__(kBlock) k_dense2(DevCfg c, DenseArgs a, const 
 
     u64 s2 = 0;        // (s_j, s_{j+1}) of the next pair
     const ulonglong2* rec = sD;   // its data record
-    // one bin pair (j, j+1): FP64 phase steps, sin/cos, amplitude cubics, multiply-accumulate into packed sums
-    auto pair = [&](int j, bool masked, u64& zr2, u64& zi2, u64& sg2) {
+    // one bin pair (j, j+1): FP64 phase steps, sin/cos, amplitude cubics, multiply-accumulate into packed sums.
+    // MASKED: apply the particle's time window per bin.  WITH_SG: accumulate |h|^2 per bin (otherwise sigma comes
+    // from the piece moments).
+    auto pair = [&](int j, auto masked_c, auto with_sg_c, u64& zr2, u64& zi2, u64& sg2) {
+      constexpr bool MASKED = decltype(masked_c)::value, WITH_SG = decltype(with_sg_c)::value;
       const int n0 = __double2loint(phi + 1572864.0);
       phi += d1; d1 += d2; d2 += d3;
       const int n1 = __double2loint(phi + 1572864.0);
@@ -582,75 +615,100 @@ __global__ void __launch_bounds__(kBlock) k_dense2(DevCfg c, DenseArgs a, const 
       const u64 Ei = f2fma(f2fma(f2fma(f2bcast(cf[3][3]), s2, f2bcast(cf[3][2])), s2, f2bcast(cf[3][1])), s2, f2bcast(cf[3][0]));
       s2 = f2add(s2, h2);
       const ulonglong2 wA = rec[0], wE = rec[1];
-      ulonglong2 g = rec[2];
-      rec += kPairRec;
-      if (masked) {
-        const u64 m2 = f2pack((j >= jlo && j < jhi) ? 1.0f : 0.0f, (j + 1 >= jlo && j + 1 < jhi) ? 1.0f : 0.0f);
-        cr2 = f2mul(cr2, m2); sr2 = f2mul(sr2, m2); g.x = f2mul(g.x, m2); g.y = f2mul(g.y, m2);
+      u64 m2 = 0;
+      if (MASKED) {
+        m2 = f2pack((j >= jlo && j < jhi) ? 1.0f : 0.0f, (j + 1 >= jlo && j + 1 < jhi) ? 1.0f : 0.0f);
+        cr2 = f2mul(cr2, m2); sr2 = f2mul(sr2, m2);
       }
       // q = W_A conj(c_A) + W_E conj(c_E)
       const u64 qr = f2fma(wA.x, Ar, f2fma(wA.y, Ai, f2fma(wE.x, Er, f2mul(wE.y, Ei))));
       const u64 qi = f2fma(wA.y, Ar, f2fma(f2neg(wA.x), Ai, f2fma(wE.y, Er, f2neg(f2mul(wE.x, Ei)))));
-      sg2 = f2fma(g.x, f2fma(Ar, Ar, f2mul(Ai, Ai)), f2fma(g.y, f2fma(Er, Er, f2mul(Ei, Ei)), sg2));
+      if (WITH_SG) {
+        ulonglong2 g = rec[2];
+        if (MASKED) { g.x = f2mul(g.x, m2); g.y = f2mul(g.y, m2); }
+        sg2 = f2fma(g.x, f2fma(Ar, Ar, f2mul(Ai, Ai)), f2fma(g.y, f2fma(Er, Er, f2mul(Ei, Ei)), sg2));
+      }
+      rec += kPairRec;
       // z += q e^{+2 pi i Phi}
       zr2 = f2fma(qr, cr2, f2fma(f2neg(qi), sr2, zr2));
       zi2 = f2fma(qr, sr2, f2fma(qi, cr2, zi2));
     };
-    auto fold = [&](u64 zr2, u64 zi2, u64 sg2, bool lo, bool hi) {
+    // sigma of one piece from its moments: |c_a(s)|^2 = sum_m e_a,m s^m with the cubic coefficients of this
+    // sub-interval; both channels at once (A in the low half, E in the high half)
+    auto sigma_piece = [&](int piece) {
+      const ulonglong2* mp = a.moments + (size_t)piece * 4;
+      const ulonglong2 m01 = mp[0], m23 = mp[1], m45 = mp[2], m6 = mp[3];
+      u64 R[4], I[4];
+#pragma unroll
+      for (int i = 0; i < 4; ++i) { R[i] = f2pack(cf[0][i], cf[2][i]); I[i] = f2pack(cf[1][i], cf[3][i]); }
+      const u64 two = f2bcast(2.0f);
+      const u64 R0x2 = f2mul(R[0], two), I0x2 = f2mul(I[0], two), R1x2 = f2mul(R[1], two), I1x2 = f2mul(I[1], two);
+      const u64 R2x2 = f2mul(R[2], two), I2x2 = f2mul(I[2], two);
+      const u64 e0 = f2fma(R[0], R[0], f2mul(I[0], I[0]));
+      const u64 e1 = f2fma(R0x2, R[1], f2mul(I0x2, I[1]));
+      const u64 e2 = f2fma(R0x2, R[2], f2fma(I0x2, I[2], f2fma(R[1], R[1], f2mul(I[1], I[1]))));
+      const u64 e3 = f2fma(R0x2, R[3], f2fma(I0x2, I[3], f2fma(R1x2, R[2], f2mul(I1x2, I[2]))));
+      const u64 e4 = f2fma(R1x2, R[3], f2fma(I1x2, I[3], f2fma(R[2], R[2], f2mul(I[2], I[2]))));
+      const u64 e5 = f2fma(R2x2, R[3], f2mul(I2x2, I[3]));
+      const u64 e6 = f2fma(R[3], R[3], f2mul(I[3], I[3]));
+      u64 acc = f2mul(e0, m01.x);
+      acc = f2fma(e1, m01.y, acc); acc = f2fma(e2, m23.x, acc); acc = f2fma(e3, m23.y, acc);
+      acc = f2fma(e4, m45.x, acc); acc = f2fma(e5, m45.y, acc); acc = f2fma(e6, m6.x, acc);
       float l, h;
-      f2unpack(zr2, l, h); Zr += (double)((lo ? l : 0.0f) + (hi ? h : 0.0f));
-      f2unpack(zi2, l, h); Zi += (double)((lo ? l : 0.0f) + (hi ? h : 0.0f));
-      f2unpack(sg2, l, h); Sg += (double)((lo ? l : 0.0f) + (hi ? h : 0.0f));
+      f2unpack(acc, l, h);
+      Sg += (double)l + (double)h;
     };
+    using T_ = std::true_type; using F_ = std::false_type;
 
-    int j = ib;
-    while (j < ie) {
-      while (next_edge == j) {                                 // edges on the pair start (incl. empty segments)
+    // Walk the pieces of this sub-interval (it is cut at every distinct edge inside it).  Pairs are evaluated once:
+    // when a piece ends on an odd bin the straddling pair forms a flush group of its own, its low half goes to the
+    // piece that ends and its high half is carried into the next piece.
+    const bool use_mom = all_in;      // all lanes inside their windows: sigma from the piece moments, unmasked pairs
+    int piece = use_mom ? a.piece_first[(ib >> (c.log2_stride - 2)) - ((a.chunk_first * CH) >> (c.log2_stride - 2))] : 0;
+    float car_zr = 0.f, car_zi = 0.f, car_sg = 0.f;
+    bool carry = false;
+    int pl = ib;
+    while (pl < ie) {
+      const int ph = min(next_edge, ie);                       // next_edge > pl: edges <= pl are consumed
+      const bool live = (k >= 0) && (k < a.n_seg);
+      int jj = pl;
+      if (carry) {
+        if (live) { Zr += (double)car_zr; Zi += (double)car_zi; Sg += (double)car_sg; }
+        carry = false;
+        jj = pl + 1;
+      }
+      const int jfull = ph & ~1;                               // full pairs end here; a straddling pair follows if ph is odd
+      if (!all_out) {
+        if (!live && jj < jfull) {
+          for (int t = jj; t < jfull; ++t) { phi += d1; d1 += d2; d2 += d3; }
+          jj = jfull;
+        }
+        s2 = f2pack((float)(jj - ib) * hS, (float)(jj + 1 - ib) * hS);
+        rec = sD + ((jj - cs) >> 1) * kPairRec;
+        while (jj < ph) {
+          const bool split = (jj == jfull);                    // the pair (ph - 1, ph)
+          const int e2 = split ? jj + 2 : min(jj + kFlushBins, jfull);
+          u64 zr2 = 0, zi2 = 0, sg2 = 0;
+          if (use_mom) { for (; jj < e2; jj += 2) pair(jj, F_{}, F_{}, zr2, zi2, sg2); }
+          else         { for (; jj < e2; jj += 2) pair(jj, T_{}, T_{}, zr2, zi2, sg2); }
+          float zrl, zrh, zil, zih, sgl, sgh;
+          f2unpack(zr2, zrl, zrh); f2unpack(zi2, zil, zih); f2unpack(sg2, sgl, sgh);
+          if (split) { car_zr = zrh; car_zi = zih; car_sg = sgh; carry = true; zrh = 0.f; zih = 0.f; sgh = 0.f; }
+          if (live) { Zr += (double)(zrl + zrh); Zi += (double)(zil + zih); Sg += (double)(sgl + sgh); }
+        }
+      } else if (ph & 1) {
+        car_zr = 0.f; car_zi = 0.f; car_sg = 0.f; carry = true;   // keep the bookkeeping of the walk uniform
+      }
+      if (use_mom && live) sigma_piece(piece);
+      ++piece;
+      while (next_edge == ph) {                                // segments that end here (incl. empty ones)
         if (k >= 0 && k < a.n_seg) close_piece(true);
         next_segment();
       }
-      bool live = (k >= 0) && (k < a.n_seg);
-      if (next_edge == j + 1) {
-        // an edge between the two bins of this pair: evaluate it once, low half -> segment k, high half -> the next
-        u64 zr2 = 0, zi2 = 0, sg2 = 0;
-        if (!all_out) {
-          s2 = f2pack((float)(j - ib) * hS, (float)(j + 1 - ib) * hS);
-          rec = sD + ((j - cs) >> 1) * kPairRec;
-          pair(j, true, zr2, zi2, sg2);
-        }
-        if (live) fold(zr2, zi2, sg2, true, false);
-        while (next_edge == j + 1) {
-          if (k >= 0 && k < a.n_seg) close_piece(true);
-          next_segment();
-        }
-        if ((k >= 0) && (k < a.n_seg)) fold(zr2, zi2, sg2, false, true);
-        j += 2;
-        continue;
-      }
-      const int b = min(ie, next_edge & ~1);                   // next_edge >= j + 2 here
-      if (all_out) {
-        // nothing to add; the phase is rebuilt at the next sub-interval
-      } else if (!live) {
-        for (int jj = j; jj < b; ++jj) { phi += d1; d1 += d2; d2 += d3; }
-      } else {
-        s2 = f2pack((float)(j - ib) * hS, (float)(j + 1 - ib) * hS);
-        rec = sD + ((j - cs) >> 1) * kPairRec;
-        for (int jj = j; jj < b;) {
-          const int e2 = min(jj + kFlushBins, b);
-          u64 zr2 = 0, zi2 = 0, sg2 = 0;
-          if (all_in) { for (; jj < e2; jj += 2) pair(jj, false, zr2, zi2, sg2); }
-          else        { for (; jj < e2; jj += 2) pair(jj, true, zr2, zi2, sg2); }
-          fold(zr2, zi2, sg2, true, true);
-        }
-      }
-      j = b;
+      pl = ph;
     }
   }
-  // a segment that ends exactly on the chunk end closes here (the host's CF_HEAD_CLOSES rule says the same)
-  if (next_edge == ce2) {
-    if (k >= 0 && k < a.n_seg) close_piece(true);
-    next_segment();
-  }
+  // (a segment that ends exactly on the chunk end was closed by the walk: the host's CF_HEAD_CLOSES rule says the same)
   // the piece still open at the chunk end
   if (k >= 0 && k < a.n_seg) close_piece(false);
   if (!SEG) frag[0] = ups;
@@ -896,6 +954,10 @@ struct sc_handle {
   // cached edge analysis
   std::vector<int> edges; int cached_chunk = 0; int chunk_first = 0, n_chunks = 0;
   std::vector<int> chunk_k0; std::vector<uint8_t> flags;
+  // pieces (fine sub-intervals cut at the edges) and their sigma moments, for k_dense2; cached with the edges
+  int cached_lg = 0; int n_pieces = 0;
+  int* d_piece_first = nullptr; int* d_piece_lo = nullptr; int* d_piece_hi = nullptr; float2* d_moments = nullptr;
+  size_t pf_cap = 0, plo_cap = 0, phi_cap = 0, mom_cap = 0;
   long long launches = 0;
   // optional per-kernel-class device timing (SC_OPT_PROFILE): event pairs recorded around each launch
   bool profile = false;
@@ -1072,6 +1134,7 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
     a.node_n = node_n; a.node_frac = node_frac; a.node_amp = node_amp; a.jlo = jlo; a.jhi = jhi; a.P_pad = P_pad;
     a.frag = frag; a.out_seg = seg_mode ? out_seg + (size_t)pb * n_seg * 3 : nullptr; a.P = Pn;
     a.seg_scale_z = sz; a.seg_scale_s = ss;
+    a.piece_first = h->d_piece_first; a.moments = reinterpret_cast<const ulonglong2*>(h->d_moments);
     const dim3 grid(n_chunks, P_pad / kBlock);
     {
       Timed tm(h, st, SC_TIME_DENSE);
@@ -1096,7 +1159,53 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
   return SC_OK;
 }
 
-int prepare_edges(sc_handle* h, const int32_t* seg_edges, int32_t n_seg, int CH, cudaStream_t st) {
+// Pieces of the launched range for fine sub-intervals of 2^lg_fine bins: every sub-interval is cut at the distinct
+// edges strictly inside it (the same walk k_dense2 does); their sigma moments are computed on the device.
+int build_pieces(sc_handle* h, int CH, int lg_fine, cudaStream_t st) {
+  const std::vector<int>& e = h->edges;
+  const int Sf = 1 << lg_fine;
+  const int nb2 = ((int)h->cfg.n_bins + 1) & ~1;
+  const long long isub0 = (long long)h->chunk_first * CH / Sf;
+  const int n_sub = (int)((long long)h->n_chunks * CH / Sf);
+  std::vector<int> first((size_t)n_sub + 1), lo, hi;
+  size_t idx = 0;
+  for (int t = 0; t < n_sub; ++t) {
+    first[t] = (int)lo.size();
+    const long long ib = (isub0 + t) * Sf;
+    if (ib >= nb2) continue;
+    const int iek = (int)std::min<long long>(ib + Sf, nb2);
+    int cur = (int)ib;
+    while (idx < e.size() && e[idx] <= ib) ++idx;
+    while (idx < e.size() && e[idx] < iek) {
+      if (e[idx] > cur) { lo.push_back(cur); hi.push_back(e[idx]); cur = e[idx]; }
+      ++idx;
+    }
+    lo.push_back(cur); hi.push_back(iek);
+  }
+  first[n_sub] = (int)lo.size();
+  h->n_pieces = (int)lo.size();
+  int rc;
+  if ((rc = grow(h, (void**)&h->d_piece_first, &h->pf_cap, first.size() * 4))) return rc;
+  if ((rc = grow(h, (void**)&h->d_piece_lo, &h->plo_cap, std::max<size_t>(lo.size(), 1) * 4))) return rc;
+  if ((rc = grow(h, (void**)&h->d_piece_hi, &h->phi_cap, std::max<size_t>(hi.size(), 1) * 4))) return rc;
+  if ((rc = grow(h, (void**)&h->d_moments, &h->mom_cap, std::max<size_t>(lo.size(), 1) * 8 * sizeof(float2)))) return rc;
+  SC_CUDA(h, cudaMemcpyAsync(h->d_piece_first, first.data(), first.size() * 4, cudaMemcpyHostToDevice, st));
+  if (h->n_pieces > 0) {
+    SC_CUDA(h, cudaMemcpyAsync(h->d_piece_lo, lo.data(), lo.size() * 4, cudaMemcpyHostToDevice, st));
+    SC_CUDA(h, cudaMemcpyAsync(h->d_piece_hi, hi.data(), hi.size() * 4, cudaMemcpyHostToDevice, st));
+    SC_CUDA(h, cudaStreamSynchronize(st));       // the host vectors go out of scope
+    Timed tm(h, st, SC_TIME_OTHER);
+    k_moments<<<(h->n_pieces + 127) / 128, 128, 0, st>>>(h->G64, h->d_piece_lo, h->d_piece_hi, h->n_pieces, (int)h->cfg.n_bins,
+                                                        lg_fine, h->d_moments);
+    if ((rc = check_launch(h, "k_moments"))) return rc;
+  } else {
+    SC_CUDA(h, cudaStreamSynchronize(st));
+  }
+  return SC_OK;
+}
+
+// lg_fine > 0: also build the piece tables of k_dense2 for fine sub-intervals of 2^lg_fine bins.
+int prepare_edges(sc_handle* h, const int32_t* seg_edges, int32_t n_seg, int CH, int lg_fine, cudaStream_t st) {
   if (!seg_edges || n_seg <= 0) return fail(h, SC_ERR_INVALID_ARG, "seg_edges is null or n_seg <= 0");
   std::vector<int> e((size_t)n_seg + 1);
   cudaPointerAttributes at;
@@ -1111,10 +1220,12 @@ int prepare_edges(sc_handle* h, const int32_t* seg_edges, int32_t n_seg, int CH,
   if (e[0] < 0 || e[n_seg] > h->cfg.n_bins) return fail(h, SC_ERR_INVALID_ARG, "seg_edges outside [0, n_bins]");
   for (int k = 0; k < n_seg; ++k)
     if (e[k + 1] < e[k]) return fail(h, SC_ERR_INVALID_ARG, "seg_edges not non-decreasing at k=%d", k);
-  if (e == h->edges && CH == h->cached_chunk) return SC_OK;
+  if (e == h->edges && CH == h->cached_chunk && lg_fine == h->cached_lg) return SC_OK;
   h->edges.swap(e);
   analyse_edges(h, CH);
+  h->cached_lg = lg_fine;
   int rc;
+  if (lg_fine > 0 && (rc = build_pieces(h, CH, lg_fine, st))) { h->cached_chunk = 0; return rc; }
   if ((rc = grow(h, (void**)&h->d_edges, &h->edge_cap, h->edges.size() * 4))) return rc;
   if ((rc = grow(h, (void**)&h->d_chunk_k0, &h->k0_cap, (size_t)std::max(h->n_chunks, 1) * 4))) return rc;
   if ((rc = grow(h, (void**)&h->d_flags, &h->flags_cap, (size_t)std::max(h->n_chunks, 1)))) return rc;
@@ -1134,7 +1245,7 @@ int eval_common(sc_handle* h, const double* params, int64_t P, const int32_t* se
     return fail(h, SC_ERR_INVALID_ARG, "null pointer or n_particles <= 0");
   cudaStream_t st = (cudaStream_t)stream;
   const bool f64 = (h->precision == 2) || (h->precision == 0 && n_seg < h->f32_min_seg);
-  int rc = prepare_edges(h, seg_edges, n_seg, f64 ? kChunkF64 : kChunkF32, st);
+  int rc = prepare_edges(h, seg_edges, n_seg, f64 ? kChunkF64 : kChunkF32, f64 ? 0 : h->lg_f32 - 2, st);
   if (rc) return rc;
   SC_CUDA(h, cudaMemsetAsync(h->d_counter, 0, 8, st));
   if (seg_mode) SC_CUDA(h, cudaMemsetAsync(out_seg, 0, (size_t)P * n_seg * 3 * 8, st));
@@ -1421,6 +1532,7 @@ int sc_free(sc_handle* h) {
   cudaFree(h->D32); cudaFree(h->W64); cudaFree(h->G64);
   cudaFree(h->scratch); cudaFree(h->d_edges); cudaFree(h->d_chunk_k0); cudaFree(h->d_flags);
   cudaFree(h->d_counter); cudaFree(h->d_params_stage);
+  cudaFree(h->d_piece_first); cudaFree(h->d_piece_lo); cudaFree(h->d_piece_hi); cudaFree(h->d_moments);
   for (auto& e : h->evs) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
   cudaGetLastError();
   delete h;
