@@ -33,6 +33,27 @@ METRIC = "particle_x_freq_bin_evals_per_s"
 UNIT = "particle-bin/s"
 C_DP = 24          # FP64 instructions per (particle, bin) of the fixed op model, SURVEY.md 8(d)
 NOMINAL_DFMA = 148 * 64 * 1.965e9   # 148 SMs x 64 FP64 lanes x max SM clock (B200_PROFILING.md unit counts / clocks)
+# The kernel's own mix: FP32-pipe lane slots per evaluated (particle, bin) in the k_dense2 loop,
+# 26 packed FFMA2/FMUL2/FADD2 (2 slots each) + 3 scalar per bin PAIR; peak = 148 SMs x 128 FP32 lanes x max SM clock.
+FP32_SLOTS_PER_BIN = (26 * 2 + 3) / 2.0
+NOMINAL_FP32_SLOTS = 148 * 128 * 1.965e9
+DENSE_PROFILE = os.path.join(ROOT, "profiles", "r01_k_dense2_full.md")
+
+
+def dram_traffic_from_profile():
+    """dram__bytes_read.sum + dram__bytes_write.sum of one k_dense2 launch, from the committed ncu --set full summary."""
+    import re
+    try:
+        txt = open(DENSE_PROFILE).read()
+    except OSError:
+        return None
+    tot, mult = 0.0, {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+    for name in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+        m = re.search(r"\|\s*" + re.escape(name) + r"\s*\|\s*(\w+)\s*\|\s*([0-9.eE+-]+)\s*\|", txt)
+        if not m or m.group(1) not in mult:
+            return None
+        tot += float(m.group(2)) * mult[m.group(1)]
+    return tot
 
 
 def parse():
@@ -288,21 +309,27 @@ def run_ours(args, rank, local_rank, world):
         # EVALUATED (particle, bin); peak = measured DFMA rate x 2 flop
         ach = 2.0 * C_DP * eval_bins / (dense_avg * 1e-3) / 1e12 if dense_avg > 0 else None
         peak = 2.0 * (dfma or NOMINAL_DFMA) / 1e12
+        pbs = eval_bins / (dense_avg * 1e-3) if dense_avg > 0 else None
         roof = {"bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
-                "frac": (ach / peak) if ach else None, "traffic": None,
-                "kernel": "k_dense<float,false>", "kernel_ms_per_launch": dense_avg,
+                "frac": (ach / peak) if ach else None, "traffic": dram_traffic_from_profile(),
+                "traffic_source": "profiles/r01_k_dense2_full.md (ncu --set full, one launch, same command)",
+                "kernel": "k_dense2<false,2>", "kernel_ms_per_launch": dense_avg,
+                "own_mix": {"what": "FP32 pipe of the kernel as built (packed FFMA2 loop): lane slots per evaluated "
+                                    "particle-bin x evaluated particle-bins/s / (148 SM x 128 lanes x 1.965 GHz)",
+                            "fp32_slots_per_bin": FP32_SLOTS_PER_BIN,
+                            "frac": (pbs * FP32_SLOTS_PER_BIN / NOMINAL_FP32_SLOTS) if pbs else None},
                 "model": f"{C_DP} FP64 instr (= {2 * C_DP} flop) per evaluated particle-bin, SURVEY.md 8(d)",
                 "peak_source": ("measured in this run by sc_measure_fp64_peak (DFMA/s x 2)" if dfma else
                                 "nominal 148 SM x 64 lanes x 1.965 GHz x 2"),
                 "peak_nominal_max_clock": 2.0 * NOMINAL_DFMA / 1e12,
                 "evaluated_particle_bins_per_launch": eval_bins,
-                "evaluated_pb_per_s": eval_bins / (dense_avg * 1e-3) if dense_avg > 0 else None,
+                "evaluated_pb_per_s": pbs,
                 "frac_vs_nominal_max_clock": (ach / (2.0 * NOMINAL_DFMA / 1e12)) if ach else None}
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f64 phase + f32 amplitude/accumulate-flush-to-f64", "data": "synthetic",
                 "config": {"workload": workload_name(cid, spec, cfg, P, N), "l2": "flushed between timed steps "
-                           "(256 MiB write); per-step node tables (GBs) exceed L2 anyway",
+                           "(256 MiB write); per-step node tables + fragments (~1 GB) exceed L2 anyway",
                            "pso": {k: hp[k] for k in ("omega", "phi_p", "phi_g")}, "n_swarms": n_swarms,
                            "parallelism": f"independent tiles x{world}" if world > 1 else "1 GPU"},
                 "swarm_iters_per_s": world * 1e3 / ms_per_step,
@@ -318,10 +345,11 @@ def run_ours(args, rank, local_rank, world):
         if not args.no_cpu_baseline and world == 1:
             from oracle import sc_oracle as orc
             cores = orc.num_threads()
-            n_p = max(8, min(64, cores))
-            sec, cores = oracle_sample_run(sy.config_inputs(cid, P=n_p), N, n_p, 1, 0)
+            n_p, k_cpu = 4 * max(8, min(32, cores)), 2          # ~10-20 s of CPU work on the box's cores
+            sec, cores = oracle_sample_run(sy.config_inputs(cid, P=n_p), N, n_p, k_cpu, 0)
             line["cpu_baseline"] = {"value": n_p * nb / sec, "unit": UNIT, "cores": cores, "kind": "oracle",
-                                    "sample": f"{n_p} particles x all {nb} bins, 1 step (statistic + PSO), {sec:.1f} s wall"}
+                                    "sample": f"{n_p} particles x all {nb} bins per step, {k_cpu} steps (statistic + PSO), "
+                                              f"{sec * k_cpu:.1f} s wall"}
         print(json.dumps(line), flush=True)
     H.close()
     if world > 1:
