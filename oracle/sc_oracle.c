@@ -268,6 +268,90 @@ double sco_inner(const double* aA, const double* aE, const double* bA, const dou
   return 4.0 * df * acc;
 }
 
+/* ------------------------------------------------------------------------------------------------
+ * Eq. 8: O_hat_N(d,h) = sum_n max_phi [d|h e^{i phi}]_n = sum_n x_n = 4 df sum_n |z_n|;
+ * Eq. 3: <h|h> = sum_n [h|h]_n = 4 df sum_n sigma_n;  Eq. 10: Upsilon_N.
+ * seg = [n_seg][3] = (Re z_n, Im z_n, sigma_n) as sco_stat_from_arrays writes it.  out3 = (Upsilon_N, O_hat_N, <h|h>).
+ * Segments with sigma_n = 0 have z_n = 0 as well and contribute nothing to any of the three (Q8).
+ * ------------------------------------------------------------------------------------------------ */
+void sco_components_from_seg(const double* seg, int64_t n_seg, double df, double out3[3]) {
+  double ups = 0.0, ohat = 0.0, hh = 0.0;
+  for (int64_t n = 0; n < n_seg; ++n) {
+    const double zr = seg[3 * n], zi = seg[3 * n + 1], sig = seg[3 * n + 2];
+    if (sig > 0.0) {
+      const double x = 4.0 * df * sqrt(zr * zr + zi * zi);
+      const double h_n = 4.0 * df * sig;
+      ups += x * x / h_n;
+      ohat += x;
+      hh += h_n;
+    }
+  }
+  out3[0] = ups; out3[1] = ohat; out3[2] = hh;
+}
+
+/* Eq. 9: log L_hat_N = -1/2 <d|d> - 1/2 <h|h> + O_hat_N(d,h) for the template amp * h, with
+ * hh = <h|h> and ohat = O_hat_N(d,h) of the unit-amplitude template (both are homogeneous in the amplitude). */
+double sco_loglike(double dd, double hh, double ohat, double amp) {
+  return -0.5 * dd - 0.5 * amp * amp * hh + amp * ohat;
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * "the segment boundaries are chosen such that each of the N segments contains an equal amount of
+ * squared SNR ... f_n is reevaluated for every new value of theta".  On the FFT grid (reading Q18):
+ *   s_j = sum_alpha |h_alpha(f_j)|^2 / S_alpha(f_j)     (the integrand of <h|h>, Eq. 1/3)
+ *   C_j = sum_{j' < j} s_j'  (C_0 = 0, C_n_bins = C, summed in bin order),
+ *   e_0 = 0,  e_N = n_bins,  e_n = min{ j : C_j >= C n / N }  for 0 < n < N.
+ * If C = 0 (empty template) every interior edge is 0.
+ * ------------------------------------------------------------------------------------------------ */
+void sco_equal_snr_edges(const double* hA, const double* hE, const double* SA, const double* SE,
+                         int64_t n_bins, int64_t n_seg, int64_t* edges) {
+  double total = 0.0;
+  for (int64_t j = 0; j < n_bins; ++j) {
+    total += (hA[2 * j] * hA[2 * j] + hA[2 * j + 1] * hA[2 * j + 1]) / SA[j];
+    if (hE && SE) total += (hE[2 * j] * hE[2 * j] + hE[2 * j + 1] * hE[2 * j + 1]) / SE[j];
+  }
+  edges[0] = 0; edges[n_seg] = n_bins;
+  double cum = 0.0;            /* C_j */
+  int64_t j = 0;
+  for (int64_t n = 1; n < n_seg; ++n) {
+    const double target = total * (double)n / (double)n_seg;
+    while (j < n_bins && !(cum >= target)) {
+      cum += (hA[2 * j] * hA[2 * j] + hA[2 * j + 1] * hA[2 * j + 1]) / SA[j];
+      if (hE && SE) cum += (hE[2 * j] * hE[2 * j] + hE[2 * j + 1] * hE[2 * j + 1]) / SE[j];
+      ++j;
+    }
+    edges[n] = (total > 0.0) ? j : 0;
+  }
+}
+
+/* Upsilon_N with per-particle equal-SNR^2 edges.  in_edges (may be NULL): [P][n_seg+1] edges to use
+ * instead of computing them (the parity tests pass the edges the device chose: where floating point decides an
+ * integer the decision is taken once).  out_edges (may be NULL): [P][n_seg+1] the edges used. */
+void sco_eval_stat_adaptive(const sco_config* c, const double* dA, const double* dE, const double* SA, const double* SE,
+                            const double* params, int64_t P, int64_t n_seg, const int64_t* in_edges,
+                            double* out, int64_t* out_edges, double* out_comp3) {
+  const int64_t n = c->n_bins;
+  const double df = 1.0 / c->T_obs_s;
+  const int two = (c->n_channels >= 2);
+#pragma omp parallel
+  {
+    double* hA = (double*)malloc((size_t)n * 2 * sizeof(double));
+    double* hE = (double*)malloc((size_t)n * 2 * sizeof(double));
+    int64_t* e = (int64_t*)malloc((size_t)(n_seg + 1) * sizeof(int64_t));
+    double* seg = (double*)malloc((size_t)n_seg * 3 * sizeof(double));
+#pragma omp for schedule(dynamic, 1)
+    for (int64_t p = 0; p < P; ++p) {
+      sco_template(c, params + 8 * p, 0, n, hA, two ? hE : NULL);
+      if (in_edges) memcpy(e, in_edges + p * (n_seg + 1), (size_t)(n_seg + 1) * sizeof(int64_t));
+      else sco_equal_snr_edges(hA, two ? hE : NULL, SA, two ? SE : NULL, n, n_seg, e);
+      out[p] = sco_stat_from_arrays(dA, two ? dE : NULL, hA, two ? hE : NULL, SA, two ? SE : NULL, df, e, n_seg, seg);
+      if (out_edges) memcpy(out_edges + p * (n_seg + 1), e, (size_t)(n_seg + 1) * sizeof(int64_t));
+      if (out_comp3) sco_components_from_seg(seg, n_seg, df, out_comp3 + 3 * p);
+    }
+    free(hA); free(hE); free(e); free(seg);
+  }
+}
+
 int sco_num_threads(void) {
 #ifdef _OPENMP
   return omp_get_max_threads();

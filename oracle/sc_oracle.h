@@ -20,6 +20,11 @@
  *   sco_orbit/sco_template: arm lengths = L, centroid on the 1-AU circle; two-pulse single-link identity;
  *                          long-wavelength Michelson limit; T-combination -> 0; beta = +-pi/2 kills the Doppler term.
  *                          PARITY WITH BBHx [56] IS UNPINNED (not in the container).
+ *   sco_components_from_seg / sco_loglike : noise-free d = A0 h gives log L_hat(A0) = 0; N = 1: max over a phase grid;
+ *                          max over the amplitude gives -1/2<d|d> + 1/2 X^2/H, = Upsilon_1/2 - <d|d>/2 at N = 1.
+ *   sco_equal_snr_edges  : flat s_j -> e_n = ceil(n n_bins/N); power-law s_j against the closed-form quantiles;
+ *                          every segment holds C/N to within one bin's s_j; App. A: linear chirp +
+ *                          white PSD -> equal-duration segments.
  *   sco_philox4x32_10    : known-answer vectors of the published algorithm (Salmon et al. 2011), moments.
  *   sco_pso_step         : hand-computed one-particle examples of Eq. 14 -> 15 -> 13.
  */
@@ -84,6 +89,18 @@ void sco_eval_stat(const sco_config* c, const double* dA_ri, const double* dE_ri
 void sco_eval_stat_levels(const sco_config* c, const double* dA_ri, const double* dE_ri, const double* S_A, const double* S_E,
                           const double* params, int64_t n_particles, const int64_t* edges_cat, const int64_t* n_segs,
                           int64_t n_levels, double* out);
+/* Eq. 8, 3, 10 from the per-segment sums: out3 = (Upsilon_N, O_hat_N = sum_n x_n, <h|h> = sum_n [h|h]_n). */
+void sco_components_from_seg(const double* seg, int64_t n_seg, double df, double out3[3]);
+/* Eq. 9: log L_hat_N = -1/2 <d|d> - 1/2 amp^2 <h|h> + amp O_hat_N (hh, ohat of the unit-amplitude template). */
+double sco_loglike(double dd, double hh, double ohat, double amp);
+/* PAPER.md:120 (reading Q18): equal squared-SNR segment edges of one template on the FFT grid:
+ * e_0 = 0, e_N = n_bins, e_n = min{ j : sum_{j'<j} s_j' >= (n/N) sum_j s_j },  s_j = sum_a |h_a|^2/S_a. */
+void sco_equal_snr_edges(const double* hA_ri, const double* hE_ri, const double* S_A, const double* S_E,
+                         int64_t n_bins, int64_t n_seg, int64_t* edges);
+/* Upsilon_N with per-particle equal-SNR^2 edges; in_edges / out_edges [P][n_seg+1] and out_comp3 [P][3] may be NULL. */
+void sco_eval_stat_adaptive(const sco_config* c, const double* dA_ri, const double* dE_ri, const double* S_A,
+                            const double* S_E, const double* params, int64_t n_particles, int64_t n_seg,
+                            const int64_t* in_edges, double* out, int64_t* out_edges, double* out_comp3);
 int sco_num_threads(void);
 
 /* Q10: Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11). */

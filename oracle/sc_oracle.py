@@ -69,6 +69,12 @@ def lib():
                                     _dp, _dp, _ip]
         L.sco_eval_stat_levels.argtypes = [C.POINTER(Config), _dp, _dp, _dp, _dp, _dp, C.c_int64, _ip, _ip,
                                            C.c_int64, _dp]
+        L.sco_components_from_seg.argtypes = [_dp, C.c_int64, C.c_double, _dp]
+        L.sco_loglike.restype = C.c_double
+        L.sco_loglike.argtypes = [C.c_double, C.c_double, C.c_double, C.c_double]
+        L.sco_equal_snr_edges.argtypes = [_dp, _dp, _dp, _dp, C.c_int64, C.c_int64, _ip]
+        L.sco_eval_stat_adaptive.argtypes = [C.POINTER(Config), _dp, _dp, _dp, _dp, _dp, C.c_int64, C.c_int64, _ip,
+                                             _dp, _ip, _dp]
         L.sco_num_threads.restype = C.c_int
         L.sco_philox4x32_10.argtypes = [C.POINTER(C.c_uint32), C.POINTER(C.c_uint32), C.POINTER(C.c_uint32)]
         L.sco_pso_uniforms.argtypes = [C.c_uint64, C.c_uint64, C.c_uint64, _dp, _dp]
@@ -180,6 +186,46 @@ def eval_stat_levels(cfg, dA, dE, SA, SE, params, edges_list):
     lib().sco_eval_stat_levels(C.byref(cfg), _d(a[0]), _d(a[1]), _d(a[2]), _d(a[3]), _d(params), P,
                                cat.ctypes.data_as(_ip), ns.ctypes.data_as(_ip), len(edges_list), _d(out))
     return out
+
+
+def components_from_seg(seg, df):
+    """(Upsilon_N, O_hat_N, <h|h>) from [n_seg][3] per-segment sums (Eq. 10, 8, 3)."""
+    seg = _f64(seg).reshape(-1, 3)
+    out = np.zeros(3)
+    lib().sco_components_from_seg(_d(seg), seg.shape[0], float(df), _d(out))
+    return out
+
+
+def loglike(dd, hh, ohat, amp):
+    return lib().sco_loglike(float(dd), float(hh), float(ohat), float(amp))
+
+
+def equal_snr_edges(hA, hE, SA, SE, n_seg):
+    n = len(hA)
+    e = np.zeros(n_seg + 1, dtype=np.int64)
+    a = [_ri(hA), None if hE is None else _ri(hE), _f64(SA), None if SE is None else _f64(SE)]
+    lib().sco_equal_snr_edges(_d(a[0]), _d(a[1]), _d(a[2]), _d(a[3]), n, n_seg, e.ctypes.data_as(_ip))
+    return e
+
+
+def eval_stat_adaptive(cfg, dA, dE, SA, SE, params, n_seg, in_edges=None, want_edges=False, want_comp=False):
+    """Upsilon_N with per-particle equal-SNR^2 edges; in_edges [P][n_seg+1] overrides the choice."""
+    params = _f64(params).reshape(-1, 8)
+    P = params.shape[0]
+    out = np.zeros(P)
+    ie = None if in_edges is None else np.ascontiguousarray(in_edges, dtype=np.int64).reshape(P, n_seg + 1)
+    oe = np.zeros((P, n_seg + 1), dtype=np.int64) if want_edges else None
+    oc = np.zeros((P, 3)) if want_comp else None
+    a = [_ri(dA), _ri(dE), _f64(SA), _f64(SE)]
+    lib().sco_eval_stat_adaptive(C.byref(cfg), _d(a[0]), _d(a[1]), _d(a[2]), _d(a[3]), _d(params), P, n_seg,
+                                 None if ie is None else ie.ctypes.data_as(_ip), _d(out),
+                                 None if oe is None else oe.ctypes.data_as(_ip), _d(oc))
+    res = [out]
+    if want_edges:
+        res.append(oe)
+    if want_comp:
+        res.append(oc)
+    return res[0] if len(res) == 1 else tuple(res)
 
 
 def num_threads():

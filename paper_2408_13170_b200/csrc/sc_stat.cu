@@ -29,7 +29,7 @@ constexpr int kBlock = 128;            // threads per CTA of the dense kernel = 
 constexpr int kChunkF32 = 2048;        // bins per CTA, FP32 amplitude path (24 B/bin of shared memory)
 constexpr int kChunkF64 = 1024;        // bins per CTA, all-FP64 path (48 B/bin)
 constexpr int kFlushBins = 32;         // FP32 partial sums are folded into the FP64 accumulators this often
-constexpr int kFragFields = 7;         // partial Upsilon, head (zr, zi, sg), tail (zr, zi, sg)
+constexpr int kFragFields = 9;         // partial Upsilon, head (zr, zi, sg), tail (zr, zi, sg), partial sum|z|, partial sum sigma
 constexpr double kMagic = 6755399441055744.0;   // 1.5 * 2^52: (x + kMagic) - kMagic = rint(x), low word = int
 
 // chunk flags (host-built from the edges, shared by all particles)
@@ -216,6 +216,7 @@ struct DenseArgs {
   double* out_seg;             // SEG mode: [P][n_seg][3] (already offset to this batch), else nullptr
   int P;                       // particles in this batch
   double seg_scale_z, seg_scale_s;
+  int comp;                    // also accumulate sum_k |z_k| and sum_k sigma_k (Eq. 8, 9 components)
   // k_dense2 only: pieces = fine sub-intervals cut at the segment edges, with the moments of the sigma weights
   const int* piece_first;      // [n_sub_launched + 1] first piece of each launched fine sub-interval
   const ulonglong2* moments;   // [n_pieces][4] = 8 packed (A, E) pairs: sum_j g_a(j) s_j^m, m = 0..6, pad
@@ -250,7 +251,7 @@ __global__ void __launch_bounds__(kBlock) k_dense(DevCfg c, DenseArgs a, const d
   int k = a.chunk_k0[chunk_l];
   int next_edge = (k + 1 <= a.n_seg) ? a.edges[k + 1] : INT_MAX;
   bool open_at_edge = (k >= 0 && k < a.n_seg) ? (a.edges[k] == cs) : true;
-  double Zr = 0.0, Zi = 0.0, Sg = 0.0, ups = 0.0;
+  double Zr = 0.0, Zi = 0.0, Sg = 0.0, ups = 0.0, xs = 0.0, hs = 0.0;
   double* frag = a.frag + (size_t)chunk_l * kFragFields * a.P_pad + p;
 
   auto close_piece = [&](bool at_edge_end) {
@@ -262,7 +263,9 @@ __global__ void __launch_bounds__(kBlock) k_dense(DevCfg c, DenseArgs a, const d
           o[0] = Zr * a.seg_scale_z; o[1] = Zi * a.seg_scale_z; o[2] = Sg * a.seg_scale_s;
         }
       } else if (Sg > 0.0) {
-        ups += (Zr * Zr + Zi * Zi) / Sg;
+        const double z2 = Zr * Zr + Zi * Zi;
+        ups += z2 / Sg;
+        if (a.comp) { xs += sqrt(z2); hs += Sg; }
       }
     } else if (!open_at_edge) {          // began in an earlier chunk: head fragment (closed or running through)
       frag[(size_t)1 * a.P_pad] = Zr; frag[(size_t)2 * a.P_pad] = Zi; frag[(size_t)3 * a.P_pad] = Sg;
@@ -398,7 +401,10 @@ __global__ void __launch_bounds__(kBlock) k_dense(DevCfg c, DenseArgs a, const d
   }
   // the piece still open at the chunk end
   if (k >= 0 && k < a.n_seg) close_piece(false);
-  if (!SEG) frag[0] = ups;
+  if (!SEG) {
+    frag[0] = ups;
+    if (a.comp) { frag[(size_t)7 * a.P_pad] = xs; frag[(size_t)8 * a.P_pad] = hs; }
+  }
 }
 
 
@@ -506,7 +512,7 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2(DevCfg c, Den
   int k = a.chunk_k0[chunk_l];
   int next_edge = (k + 1 <= a.n_seg) ? a.edges[k + 1] : INT_MAX;
   bool open_at_edge = (k >= 0 && k < a.n_seg) ? (a.edges[k] == cs) : true;
-  double Zr = 0.0, Zi = 0.0, Sg = 0.0, ups = 0.0;
+  double Zr = 0.0, Zi = 0.0, Sg = 0.0, ups = 0.0, xs = 0.0, hs = 0.0;
   double* frag = a.frag + (size_t)chunk_l * kFragFields * a.P_pad + p;
 
   auto close_piece = [&](bool at_edge_end) {
@@ -517,7 +523,9 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2(DevCfg c, Den
           o[0] = Zr * a.seg_scale_z; o[1] = Zi * a.seg_scale_z; o[2] = Sg * a.seg_scale_s;
         }
       } else if (Sg > 0.0) {
-        ups += (Zr * Zr + Zi * Zi) / Sg;
+        const double z2 = Zr * Zr + Zi * Zi;
+        ups += z2 / Sg;
+        if (a.comp) { xs += sqrt(z2); hs += Sg; }
       }
     } else if (!open_at_edge) {
       frag[(size_t)1 * a.P_pad] = Zr; frag[(size_t)2 * a.P_pad] = Zi; frag[(size_t)3 * a.P_pad] = Sg;
@@ -711,29 +719,40 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2(DevCfg c, Den
   // (a segment that ends exactly on the chunk end was closed by the walk: the host's CF_HEAD_CLOSES rule says the same)
   // the piece still open at the chunk end
   if (k >= 0 && k < a.n_seg) close_piece(false);
-  if (!SEG) frag[0] = ups;
+  if (!SEG) {
+    frag[0] = ups;
+    if (a.comp) { frag[(size_t)7 * a.P_pad] = xs; frag[(size_t)8 * a.P_pad] = hs; }
+  }
 }
 
 // ------------------------------------------------------------------------------------------------ a6
+// out[p] = Upsilon.  comp3 != nullptr: also comp3[p] = (Upsilon, X = sum_k |z_k| x_scale, H = sum_k sigma_k h_scale).
 __global__ void k_stitch(const double* __restrict__ frag, const uint8_t* __restrict__ flags, int n_chunks, int P_pad,
-                         int P, double scale, double* __restrict__ out) {
+                         int P, double scale, double* __restrict__ out, double* __restrict__ comp3, double x_scale,
+                         double h_scale) {
   const int p = blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= P) return;
-  double ups = 0.0, zr = 0.0, zi = 0.0, sg = 0.0;
+  double ups = 0.0, zr = 0.0, zi = 0.0, sg = 0.0, xs = 0.0, hs = 0.0;
   for (int cI = 0; cI < n_chunks; ++cI) {
     const double* f = frag + (size_t)cI * kFragFields * P_pad + p;
     const uint8_t fl = flags[cI];
     if (fl & CF_HEAD) {
       zr += f[(size_t)1 * P_pad]; zi += f[(size_t)2 * P_pad]; sg += f[(size_t)3 * P_pad];
       if (fl & CF_HEAD_CLOSES) {
-        if (sg > 0.0) ups += (zr * zr + zi * zi) / sg;
+        if (sg > 0.0) {
+          const double z2 = zr * zr + zi * zi;
+          ups += z2 / sg;
+          if (comp3) { xs += sqrt(z2); hs += sg; }
+        }
         zr = 0.0; zi = 0.0; sg = 0.0;
       }
     }
     ups += f[0];
+    if (comp3) { xs += f[(size_t)7 * P_pad]; hs += f[(size_t)8 * P_pad]; }
     if (fl & CF_TAIL) { zr = f[(size_t)4 * P_pad]; zi = f[(size_t)5 * P_pad]; sg = f[(size_t)6 * P_pad]; }
   }
-  out[p] = ups * scale;
+  if (out) out[p] = ups * scale;
+  if (comp3) { comp3[3 * (size_t)p] = ups * scale; comp3[3 * (size_t)p + 1] = xs * x_scale; comp3[3 * (size_t)p + 2] = hs * h_scale; }
 }
 
 __global__ void k_stitch_seg(const double* __restrict__ frag, const uint8_t* __restrict__ flags,
