@@ -108,6 +108,22 @@ int sc_eval_stat_host(sc_handle* h, const double* params, int64_t n_particles,
 int sc_eval_segments(sc_handle* h, const double* params, int64_t n_particles,
                      const int32_t* seg_edges, int32_t n_seg, double* out_seg, void* cuda_stream);
 
+/* Eq. 8, 3, 10 from the same per-segment sums: out3 DEVICE [n_particles][3] =
+ *   ( Upsilon_N,  O_hat_N = sum_k x_k = 4 df sum_k |z_k|,  <h|h> = sum_k [h|h]_k = 4 df sum_k sigma_k ),
+ * the last two for the unit-amplitude template A(f) = f^(-7/6) (O2); a template of amplitude A has A O_hat, A^2 <h|h>.
+ * Arguments otherwise as sc_eval_stat. */
+int sc_eval_components(sc_handle* h, const double* params, int64_t n_particles,
+                       const int32_t* seg_edges, int32_t n_seg, double* out3, void* cuda_stream);
+
+/* Eq. 9: the semi-coherent log-likelihood log L_hat_N = -1/2 <d|d> - 1/2 A_p^2 <h|h> + A_p O_hat_N
+ * of the template A_p f^(-7/6) T_a e^{-i Psi} (A_p carries 1/D_L and the chirp-mass prefactor).
+ * amp: DEVICE [n_particles]; out: DEVICE [n_particles]. */
+int sc_eval_loglike(sc_handle* h, const double* params, const double* amp, int64_t n_particles,
+                    const int32_t* seg_edges, int32_t n_seg, double* out, void* cuda_stream);
+
+/* <d|d> of the data stream the handle was built from (Eq. 1; computed once in sc_init_data).  dd: HOST. */
+int sc_data_norm(sc_handle* h, double* dd);
+
 /* The template itself on the dense grid through the same node tables and interpolants the statistic uses
  * (for injections and element-wise parity).  params: DEVICE [n_templates][8];
  * hA_ri, hE_ri: DEVICE [n_templates][n_bins] complex FP64 interleaved. */

@@ -15,7 +15,7 @@ SC_OPT_PRECISION, SC_OPT_F32_MIN_SEG, SC_OPT_SCRATCH_BYTES, SC_OPT_TC_MAX_S, SC_
 SC_TIMING_CLASSES = ["nodes", "dense", "stitch", "pso", "other"]
 
 EXPORTED_SYMBOLS = ["sc_init_data", "sc_init_data_host", "sc_eval_stat", "sc_eval_stat_host", "sc_eval_segments",
-                    "sc_gen_template", "sc_pso_step", "sc_get_counters", "sc_get_timing", "sc_measure_fp64_peak",
+                    "sc_eval_components", "sc_eval_loglike", "sc_data_norm", "sc_gen_template", "sc_pso_step", "sc_get_counters", "sc_get_timing", "sc_measure_fp64_peak",
                     "sc_set_option", "sc_free",
                     "sc_last_error", "sc_version"]
 
@@ -67,10 +67,14 @@ def load_library():
     L.sc_init_data.argtypes = [C.POINTER(_vp), cfgp, _vp, _vp, _vp, _vp, _vp]
     L.sc_init_data_host.restype = C.c_int
     L.sc_init_data_host.argtypes = [C.POINTER(_vp), cfgp, _vp, _vp, _vp, _vp, _vp]
-    for name in ("sc_eval_stat", "sc_eval_stat_host", "sc_eval_segments"):
+    for name in ("sc_eval_stat", "sc_eval_stat_host", "sc_eval_segments", "sc_eval_components"):
         f = getattr(L, name)
         f.restype = C.c_int
         f.argtypes = [_vp, _vp, C.c_int64, _vp, C.c_int32, _vp, _vp]
+    L.sc_eval_loglike.restype = C.c_int
+    L.sc_eval_loglike.argtypes = [_vp, _vp, _vp, C.c_int64, _vp, C.c_int32, _vp, _vp]
+    L.sc_data_norm.restype = C.c_int
+    L.sc_data_norm.argtypes = [_vp, C.POINTER(C.c_double)]
     L.sc_gen_template.restype = C.c_int
     L.sc_gen_template.argtypes = [_vp, _vp, C.c_int64, _vp, _vp, _vp]
     L.sc_pso_step.restype = C.c_int
@@ -232,6 +236,38 @@ def sc_eval_segments(h, params, n_particles, seg_edges, n_seg, out_seg, stream=N
     return out_seg
 
 
+def sc_eval_components(h, params, n_particles, seg_edges, n_seg, out3, stream=None):
+    torch = _torch()
+    keep, ep, ns = _edges_arg(seg_edges)
+    if ns != n_seg:
+        raise SCError(SC_ERR_INVALID_ARG, f"seg_edges has {ns + 1} entries, expected n_seg + 1 = {n_seg + 1}")
+    if params.numel() != 8 * n_particles or out3.numel() != n_particles * 3:
+        raise SCError(SC_ERR_INVALID_ARG, "params must be [n_particles, 8] and out3 [n_particles, 3]")
+    rc = load_library().sc_eval_components(h, _dev(params, torch.float64, "params"), n_particles, ep, n_seg,
+                                           _dev(out3, torch.float64, "out3"), _stream(stream))
+    _check(rc, h)
+    return out3
+
+
+def sc_eval_loglike(h, params, amp, n_particles, seg_edges, n_seg, out, stream=None):
+    torch = _torch()
+    keep, ep, ns = _edges_arg(seg_edges)
+    if ns != n_seg:
+        raise SCError(SC_ERR_INVALID_ARG, f"seg_edges has {ns + 1} entries, expected n_seg + 1 = {n_seg + 1}")
+    if params.numel() != 8 * n_particles or amp.numel() != n_particles or out.numel() != n_particles:
+        raise SCError(SC_ERR_INVALID_ARG, "params must be [n_particles, 8], amp and out [n_particles]")
+    rc = load_library().sc_eval_loglike(h, _dev(params, torch.float64, "params"), _dev(amp, torch.float64, "amp"),
+                                        n_particles, ep, n_seg, _dev(out, torch.float64, "out"), _stream(stream))
+    _check(rc, h)
+    return out
+
+
+def sc_data_norm(h):
+    v = C.c_double(0.0)
+    _check(load_library().sc_data_norm(h, C.byref(v)), h)
+    return v.value
+
+
 def sc_gen_template(h, params, n_templates, hA_ri, hE_ri, stream=None):
     torch = _torch()
     rc = load_library().sc_gen_template(h, _dev(params, torch.float64, "params"), n_templates,
@@ -315,6 +351,23 @@ class Handle:
         P, N = params.shape[0], len(seg_edges) - 1
         out = torch.empty((P, N, 3), dtype=torch.float64, device=params.device)
         return sc_eval_segments(self.h, params, P, seg_edges, N, out, stream)
+
+    def eval_components(self, params, seg_edges, stream=None):
+        """-> CUDA tensor [P, 3] = (Upsilon_N, O_hat_N, <h|h>)  (Eq. 10, 8, 3)."""
+        torch = _torch()
+        P = params.shape[0]
+        out = torch.empty((P, 3), dtype=torch.float64, device=params.device)
+        return sc_eval_components(self.h, params, P, seg_edges, len(seg_edges) - 1, out, stream)
+
+    def eval_loglike(self, params, amp, seg_edges, stream=None):
+        """-> CUDA tensor [P] = log L_hat_N (Eq. 9) for template amplitudes amp [P]."""
+        torch = _torch()
+        P = params.shape[0]
+        out = torch.empty(P, dtype=torch.float64, device=params.device)
+        return sc_eval_loglike(self.h, params, amp, P, seg_edges, len(seg_edges) - 1, out, stream)
+
+    def data_norm(self):
+        return sc_data_norm(self.h)
 
     def gen_template(self, params, stream=None):
         """-> (h_A, h_E) complex128 CUDA tensors [n_templates, n_bins]."""

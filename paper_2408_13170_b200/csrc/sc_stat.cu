@@ -82,6 +82,35 @@ __global__ void k_whiten(const double* __restrict__ dA, const double* __restrict
   D32[3 * (size_t)m + 2] = make_float4((float)g0.x, (float)g1.x, (float)g0.y, (float)g1.y);
 }
 
+// <d|d> = 4 df sum_a sum_j |d_a|^2 / S_a = sum |W|^2 / G over the bins with non-zero weight (Eq. 1 with a = b = d;
+// the constant of Eq. 9).  Fixed grid and a fixed-order tree: deterministic.  part: [gridDim.x] partial sums.
+__global__ void k_data_norm(const double4* __restrict__ W64, const double2* __restrict__ G64, int n, double* __restrict__ part) {
+  __shared__ double sh[256];
+  double acc = 0.0;
+  for (int j = blockIdx.x * blockDim.x + threadIdx.x; j < n; j += gridDim.x * blockDim.x) {
+    const double4 w = W64[j]; const double2 g = G64[j];
+    if (g.x > 0.0) acc += (w.x * w.x + w.y * w.y) / g.x;
+    if (g.y > 0.0) acc += (w.z * w.z + w.w * w.w) / g.y;
+  }
+  sh[threadIdx.x] = acc;
+  __syncthreads();
+  for (int o = 128; o > 0; o >>= 1) {
+    if (threadIdx.x < o) sh[threadIdx.x] += sh[threadIdx.x + o];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) part[blockIdx.x] = sh[0];
+}
+
+// Eq. 9: log L_hat_N = -1/2 <d|d> - 1/2 A^2 <h|h> + A O_hat_N for a template of amplitude A times the
+// unit-amplitude template the components refer to.
+__global__ void k_loglike(const double* __restrict__ comp3, const double* __restrict__ amp, double dd, int P,
+                          double* __restrict__ out) {
+  const int p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= P) return;
+  const double A = amp[p];
+  out[p] = -0.5 * dd - 0.5 * A * A * comp3[3 * (size_t)p + 2] + A * comp3[3 * (size_t)p + 1];
+}
+
 // ------------------------------------------------------------------------------------------------ a1 + a3
 __global__ void k_particle_consts(DevCfg c, const double* __restrict__ params, int P, int P_pad,
                                   double* __restrict__ pc, int* __restrict__ jlo_out, int* __restrict__ jhi_out,
@@ -965,6 +994,8 @@ struct sc_handle {
   double tc_max_s = 10.0 * 31557600.0; int forced_stride_log2 = 0; int sincos_mode = 0; int mufu_min_seg = 64;
   int lg_f32 = 5, lg_f64 = 5;      // log2 of the coarse node spacing per precision mode (set_stride)
   double mufu_gain2 = 1.0;        // <cos^2 + sin^2> of the hardware sin/cos, measured at init
+  double dd = 0.0;                // <d|d> (Eq. 1), computed at init
+  double* d_comp = nullptr; size_t comp_cap = 0;   // components scratch of sc_eval_loglike
   // scratch
   void* scratch = nullptr; size_t scratch_bytes = 0;
   int* d_edges = nullptr; int* d_chunk_k0 = nullptr; uint8_t* d_flags = nullptr; size_t edge_cap = 0, k0_cap = 0, flags_cap = 0;
@@ -1096,8 +1127,8 @@ void analyse_edges(sc_handle* h, int CH) {
 }
 
 template <typename R>
-int run_batches(sc_handle* h, const double* params, int64_t P, double* out, double* out_seg, cudaStream_t st,
-                bool seg_mode) {
+int run_batches(sc_handle* h, const double* params, int64_t P, double* out, double* out_seg, double* out_comp,
+                cudaStream_t st, bool seg_mode) {
   const int n_seg = (int)h->edges.size() - 1;
   DevCfg dc = h->dc;
   apply_stride(dc, sizeof(R) == 4 ? h->lg_f32 : h->lg_f64);
@@ -1140,7 +1171,8 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
     }
     if ((rc = check_launch(h, "k_particle_consts"))) return rc;
     if (n_chunks == 0) {
-      if (!seg_mode) SC_CUDA(h, cudaMemsetAsync(out + pb, 0, (size_t)Pn * 8, st));
+      if (!seg_mode && out) SC_CUDA(h, cudaMemsetAsync(out + pb, 0, (size_t)Pn * 8, st));
+      if (out_comp) SC_CUDA(h, cudaMemsetAsync(out_comp + pb * 3, 0, (size_t)Pn * 24, st));
       continue;
     }
     {
@@ -1152,7 +1184,7 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
     a.edges = h->d_edges; a.n_seg = n_seg; a.chunk_first = h->chunk_first; a.chunk_k0 = h->d_chunk_k0;
     a.node_n = node_n; a.node_frac = node_frac; a.node_amp = node_amp; a.jlo = jlo; a.jhi = jhi; a.P_pad = P_pad;
     a.frag = frag; a.out_seg = seg_mode ? out_seg + (size_t)pb * n_seg * 3 : nullptr; a.P = Pn;
-    a.seg_scale_z = sz; a.seg_scale_s = ss;
+    a.seg_scale_z = sz; a.seg_scale_s = ss; a.comp = out_comp ? 1 : 0;
     a.piece_first = h->d_piece_first; a.moments = reinterpret_cast<const ulonglong2*>(h->d_moments);
     const dim3 grid(n_chunks, P_pad / kBlock);
     {
@@ -1171,8 +1203,14 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
     Timed tm2(h, st, SC_TIME_STITCH);
     if (seg_mode) k_stitch_seg<<<(Pn + 127) / 128, 128, 0, st>>>(frag, h->d_flags, h->d_chunk_k0, n_chunks, P_pad, Pn, n_seg, sz, ss,
                                                                 out_seg + (size_t)pb * n_seg * 3);
-    else k_stitch<<<(Pn + 127) / 128, 128, 0, st>>>(frag, h->d_flags, n_chunks, P_pad, Pn,
-                                                    (sizeof(R) == 4 && sincos == 2) ? 1.0 / h->mufu_gain2 : 1.0, out + pb);
+    else {
+      // the hardware sin/cos gain g (g^2 = mufu_gain2) multiplies every |z_k|: Upsilon by g^2, O_hat by g, <h|h> not at all.
+      // Units (whitened -> definition): Upsilon is scale free, x_k = 4 df |z_k| = |Z_k| s0 h0, [h|h]_k = Sg_k s0^2 h0^2.
+      const double g2 = (sizeof(R) == 4 && sincos == 2) ? h->mufu_gain2 : 1.0;
+      k_stitch<<<(Pn + 127) / 128, 128, 0, st>>>(frag, h->d_flags, n_chunks, P_pad, Pn, 1.0 / g2, out ? out + pb : nullptr,
+                                                 out_comp ? out_comp + pb * 3 : nullptr, h->s0 * h0 / sqrt(g2),
+                                                 h->s0 * h->s0 * h0 * h0);
+    }
     if ((rc = check_launch(h, "k_stitch"))) return rc;
   }
   return SC_OK;
@@ -1257,10 +1295,10 @@ int prepare_edges(sc_handle* h, const int32_t* seg_edges, int32_t n_seg, int CH,
 }
 
 int eval_common(sc_handle* h, const double* params, int64_t P, const int32_t* seg_edges, int32_t n_seg,
-                double* out, double* out_seg, void* stream, bool seg_mode) {
+                double* out, double* out_seg, void* stream, bool seg_mode, double* out_comp = nullptr) {
   if (!h) return SC_ERR_NOT_INIT;
   if (h->cuda_failed) return SC_ERR_CUDA;
-  if (!params || P <= 0 || (!seg_mode && !out) || (seg_mode && !out_seg))
+  if (!params || P <= 0 || (!seg_mode && !out && !out_comp) || (seg_mode && !out_seg))
     return fail(h, SC_ERR_INVALID_ARG, "null pointer or n_particles <= 0");
   cudaStream_t st = (cudaStream_t)stream;
   const bool f64 = (h->precision == 2) || (h->precision == 0 && n_seg < h->f32_min_seg);
@@ -1268,8 +1306,8 @@ int eval_common(sc_handle* h, const double* params, int64_t P, const int32_t* se
   if (rc) return rc;
   SC_CUDA(h, cudaMemsetAsync(h->d_counter, 0, 8, st));
   if (seg_mode) SC_CUDA(h, cudaMemsetAsync(out_seg, 0, (size_t)P * n_seg * 3 * 8, st));
-  return f64 ? run_batches<double>(h, params, P, out, out_seg, st, seg_mode)
-             : run_batches<float>(h, params, P, out, out_seg, st, seg_mode);
+  return f64 ? run_batches<double>(h, params, P, out, out_seg, out_comp, st, seg_mode)
+             : run_batches<float>(h, params, P, out, out_seg, out_comp, st, seg_mode);
 }
 
 int init_common(sc_handle** out, const sc_config* cfg, const double* dA, const double* dE, const double* S_A,
@@ -1350,6 +1388,19 @@ int init_common(sc_handle** out, const sc_config* cfg, const double* dA, const d
     fail(nullptr, SC_ERR_CUDA, "hardware sin/cos gain calibration out of range (%g)", h->mufu_gain2);
     return bail(SC_ERR_CUDA);
   }
+  {
+    double* part = nullptr;
+    SC_INIT(cudaMalloc(&part, 256 * 8));
+    k_data_norm<<<256, 256, 0, st>>>(h->W64, h->G64, n, part);
+    h->launches++;
+    double hp[256];
+    SC_INIT(cudaMemcpyAsync(hp, part, sizeof hp, cudaMemcpyDeviceToHost, st));
+    SC_INIT(cudaStreamSynchronize(st));
+    cudaFree(part);
+    double acc = 0.0;
+    for (int i = 0; i < 256; ++i) acc += hp[i];
+    h->dd = acc;      // |W|^2/G = |d|^2 4df/S: the scale s0 cancels
+  }
   if (stage) { SC_INIT(cudaStreamSynchronize(st)); cudaFree(stage); }
 #undef SC_INIT
   *out = h;
@@ -1378,6 +1429,31 @@ int sc_eval_stat(sc_handle* h, const double* params, int64_t P, const int32_t* s
 int sc_eval_segments(sc_handle* h, const double* params, int64_t P, const int32_t* seg_edges, int32_t n_seg,
                      double* out_seg, void* stream) {
   return eval_common(h, params, P, seg_edges, n_seg, nullptr, out_seg, stream, true);
+}
+
+int sc_eval_components(sc_handle* h, const double* params, int64_t P, const int32_t* seg_edges, int32_t n_seg,
+                       double* out3, void* stream) {
+  if (!out3) return h ? fail(h, SC_ERR_INVALID_ARG, "out3 is null") : SC_ERR_NOT_INIT;
+  return eval_common(h, params, P, seg_edges, n_seg, nullptr, nullptr, stream, false, out3);
+}
+
+int sc_eval_loglike(sc_handle* h, const double* params, const double* amp, int64_t P, const int32_t* seg_edges,
+                    int32_t n_seg, double* out, void* stream) {
+  if (!h) return SC_ERR_NOT_INIT;
+  if (h->cuda_failed) return SC_ERR_CUDA;
+  if (!params || !amp || !out || P <= 0) return fail(h, SC_ERR_INVALID_ARG, "null pointer or n_particles <= 0");
+  int rc = grow(h, (void**)&h->d_comp, &h->comp_cap, (size_t)P * 24);
+  if (rc) return rc;
+  if ((rc = eval_common(h, params, P, seg_edges, n_seg, nullptr, nullptr, stream, false, h->d_comp))) return rc;
+  k_loglike<<<(unsigned)((P + 127) / 128), 128, 0, (cudaStream_t)stream>>>(h->d_comp, amp, h->dd, (int)P, out);
+  return check_launch(h, "k_loglike");
+}
+
+int sc_data_norm(sc_handle* h, double* dd) {
+  if (!h) return SC_ERR_NOT_INIT;
+  if (!dd) return fail(h, SC_ERR_INVALID_ARG, "dd is null");
+  *dd = h->dd;
+  return SC_OK;
 }
 
 int sc_eval_stat_host(sc_handle* h, const double* params, int64_t P, const int32_t* seg_edges, int32_t n_seg,
@@ -1550,7 +1626,7 @@ int sc_free(sc_handle* h) {
   if (!h) return SC_ERR_NOT_INIT;
   cudaFree(h->D32); cudaFree(h->W64); cudaFree(h->G64);
   cudaFree(h->scratch); cudaFree(h->d_edges); cudaFree(h->d_chunk_k0); cudaFree(h->d_flags);
-  cudaFree(h->d_counter); cudaFree(h->d_params_stage);
+  cudaFree(h->d_counter); cudaFree(h->d_params_stage); cudaFree(h->d_comp);
   cudaFree(h->d_piece_first); cudaFree(h->d_piece_lo); cudaFree(h->d_piece_hi); cudaFree(h->d_moments);
   for (auto& e : h->evs) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
   cudaGetLastError();

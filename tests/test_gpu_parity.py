@@ -119,6 +119,32 @@ def test_c1_partial_and_empty_edges(c1, oracle, torch_cuda):
         assert np.array_equal(seg[:, np.diff(e) == 0, :], np.zeros_like(seg[:, np.diff(e) == 0, :]))
 
 
+@pytest.mark.parametrize("N,prec", [(1, 0), (50, 0), (1000, 0), (1000, 2), (100, 1)])
+def test_c1_components_and_loglike(c1, oracle, torch_cuda, sc, N, prec):
+    """Eq. 8 (O_hat_N), Eq. 3 (<h|h>) and Eq. 9 (log L_hat_N) from the same per-segment sums, against the oracle's
+    sco_components_from_seg / sco_loglike applied to the ORACLE's segments."""
+    inp, H = c1["inp"], c1["H"]
+    e = sy.edges(inp["cfg"]["n_bins"], N)
+    ref, refseg = oracle.eval_stat(c1["cfg"], c1["dA"], c1["dE"], inp["S_A"], inp["S_E"], inp["particles"], e, want_seg=True)
+    comp_ref = np.array([oracle.components_from_seg(s, inp["df"]) for s in refseg])
+    dd = oracle.inner(c1["dA"], c1["dE"], c1["dA"], c1["dE"], inp["S_A"], inp["S_E"], inp["df"])
+    assert H.data_norm() == pytest.approx(dd, rel=1e-12)
+    H.set_option(sc.SC_OPT_PRECISION, prec)
+    par = _dev(torch_cuda, inp["particles"])
+    comp = H.eval_components(par, e).cpu().numpy()
+    assert rel_err(comp[:, 0], ref).max() <= TOL
+    assert np.array_equal(comp[:, 0], H.eval_stat(par, e).cpu().numpy())      # same kernels, same order
+    assert rel_err(comp[:, 1], comp_ref[:, 1]).max() <= TOL
+    assert rel_err(comp[:, 2], comp_ref[:, 2]).max() <= TOL
+    # amplitude that maximises Eq. 9: A = O_hat/<h|h>; also an arbitrary one
+    for amp in (comp_ref[:, 1] / comp_ref[:, 2], np.full(len(ref), 3.0e-3 * np.median(comp_ref[:, 1] / comp_ref[:, 2]))):
+        want = np.array([oracle.loglike(dd, c[2], c[1], a) for c, a in zip(comp_ref, amp)])
+        got = H.eval_loglike(par, _dev(torch_cuda, amp), e).cpu().numpy()
+        # log L_hat = -dd/2 + (small): the bar is relative to the data-independent part that the template controls
+        assert (np.abs(got - want) / np.maximum(np.abs(want + 0.5 * dd), 1e-300)).max() <= 2 * TOL
+    H.set_option(sc.SC_OPT_PRECISION, 0)
+
+
 def test_invalid_particles_give_zero(c1, torch_cuda):
     inp, H = c1["inp"], c1["H"]
     p = inp["particles"][:6].copy()
