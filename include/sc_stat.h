@@ -108,6 +108,18 @@ int sc_eval_stat_host(sc_handle* h, const double* params, int64_t n_particles,
 int sc_eval_segments(sc_handle* h, const double* params, int64_t n_particles,
                      const int32_t* seg_edges, int32_t n_seg, double* out_seg, void* cuda_stream);
 
+/* Upsilon_N with the paper's own segments (App. A): boundaries f_n(theta) chosen for
+ * EVERY particle such that each segment holds an equal share of the template's squared SNR.  On the FFT grid (reading
+ * Q18): s_j = sum_a |h_a(f_j)|^2 / S_a(f_j), C = sum_j s_j, e_0 = 0, e_N = n_bins and
+ *   e_n = min{ j : sum_{j' < j} s_j' >= C n / N },  n = 1 .. N-1;
+ * then out[p] as in sc_eval_stat on those edges.  The cumulative sums are formed in the kernel's arithmetic (FP32
+ * amplitudes, FP64 running sum), so an edge can sit one bin away from where an FP64 evaluation puts it.
+ * out: DEVICE [n_particles] or NULL; out_edges: DEVICE int32 [n_particles][n_seg + 1] or NULL (the edges used; all
+ * zero but the last for a particle whose template is empty); out3: DEVICE [n_particles][3] or NULL (as
+ * sc_eval_components).  n_seg = 1 is sc_eval_stat on (0, n_bins); 2 <= n_seg runs the FP32-amplitude path. */
+int sc_eval_stat_adaptive(sc_handle* h, const double* params, int64_t n_particles, int32_t n_seg,
+                          double* out, int32_t* out_edges, double* out3, void* cuda_stream);
+
 /* Eq. 8, 3, 10 from the same per-segment sums: out3 DEVICE [n_particles][3] =
  *   ( Upsilon_N,  O_hat_N = sum_k x_k = 4 df sum_k |z_k|,  <h|h> = sum_k [h|h]_k = 4 df sum_k sigma_k ),
  * the last two for the unit-amplitude template A(f) = f^(-7/6) (O2); a template of amplitude A has A O_hat, A^2 <h|h>.

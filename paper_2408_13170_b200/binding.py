@@ -15,7 +15,7 @@ SC_OPT_PRECISION, SC_OPT_F32_MIN_SEG, SC_OPT_SCRATCH_BYTES, SC_OPT_TC_MAX_S, SC_
 SC_TIMING_CLASSES = ["nodes", "dense", "stitch", "pso", "other"]
 
 EXPORTED_SYMBOLS = ["sc_init_data", "sc_init_data_host", "sc_eval_stat", "sc_eval_stat_host", "sc_eval_segments",
-                    "sc_eval_components", "sc_eval_loglike", "sc_data_norm", "sc_gen_template", "sc_pso_step", "sc_get_counters", "sc_get_timing", "sc_measure_fp64_peak",
+                    "sc_eval_stat_adaptive", "sc_eval_components", "sc_eval_loglike", "sc_data_norm", "sc_gen_template", "sc_pso_step", "sc_get_counters", "sc_get_timing", "sc_measure_fp64_peak",
                     "sc_set_option", "sc_free",
                     "sc_last_error", "sc_version"]
 
@@ -71,6 +71,8 @@ def load_library():
         f = getattr(L, name)
         f.restype = C.c_int
         f.argtypes = [_vp, _vp, C.c_int64, _vp, C.c_int32, _vp, _vp]
+    L.sc_eval_stat_adaptive.restype = C.c_int
+    L.sc_eval_stat_adaptive.argtypes = [_vp, _vp, C.c_int64, C.c_int32, _vp, _vp, _vp, _vp]
     L.sc_eval_loglike.restype = C.c_int
     L.sc_eval_loglike.argtypes = [_vp, _vp, _vp, C.c_int64, _vp, C.c_int32, _vp, _vp]
     L.sc_data_norm.restype = C.c_int
@@ -236,6 +238,24 @@ def sc_eval_segments(h, params, n_particles, seg_edges, n_seg, out_seg, stream=N
     return out_seg
 
 
+def sc_eval_stat_adaptive(h, params, n_particles, n_seg, out=None, out_edges=None, out3=None, stream=None):
+    """Per-particle equal-SNR^2 segments.  out [P] f64, out_edges [P, n_seg+1] int32, out3 [P, 3] f64:
+    CUDA tensors or None (at least one of out / out3)."""
+    torch = _torch()
+    if params.numel() != 8 * n_particles:
+        raise SCError(SC_ERR_INVALID_ARG, "params must be [n_particles, 8]")
+    for t, sz, nm in ((out, n_particles, "out"), (out_edges, n_particles * (n_seg + 1), "out_edges"), (out3, 3 * n_particles, "out3")):
+        if t is not None and t.numel() != sz:
+            raise SCError(SC_ERR_INVALID_ARG, f"{nm}: expected {sz} values, got {t.numel()}")
+    rc = load_library().sc_eval_stat_adaptive(
+        h, _dev(params, torch.float64, "params"), n_particles, n_seg,
+        None if out is None else _dev(out, torch.float64, "out"),
+        None if out_edges is None else _dev(out_edges, torch.int32, "out_edges"),
+        None if out3 is None else _dev(out3, torch.float64, "out3"), _stream(stream))
+    _check(rc, h)
+    return out, out_edges, out3
+
+
 def sc_eval_components(h, params, n_particles, seg_edges, n_seg, out3, stream=None):
     torch = _torch()
     keep, ep, ns = _edges_arg(seg_edges)
@@ -351,6 +371,17 @@ class Handle:
         P, N = params.shape[0], len(seg_edges) - 1
         out = torch.empty((P, N, 3), dtype=torch.float64, device=params.device)
         return sc_eval_segments(self.h, params, P, seg_edges, N, out, stream)
+
+    def eval_stat_adaptive(self, params, n_seg, want_edges=False, want_comp=False, stream=None):
+        """Upsilon_N on per-particle equal-SNR^2 segments -> out [P] (, edges [P, n_seg+1] int32) (, comp [P, 3])."""
+        torch = _torch()
+        P = params.shape[0]
+        out = torch.empty(P, dtype=torch.float64, device=params.device)
+        ed = torch.empty((P, n_seg + 1), dtype=torch.int32, device=params.device) if want_edges else None
+        c3 = torch.empty((P, 3), dtype=torch.float64, device=params.device) if want_comp else None
+        sc_eval_stat_adaptive(self.h, params, P, n_seg, out, ed, c3, stream)
+        res = [out] + ([ed] if want_edges else []) + ([c3] if want_comp else [])
+        return res[0] if len(res) == 1 else tuple(res)
 
     def eval_components(self, params, seg_edges, stream=None):
         """-> CUDA tensor [P, 3] = (Upsilon_N, O_hat_N, <h|h>)  (Eq. 10, 8, 3)."""

@@ -485,7 +485,10 @@ __global__ void k_moments(const double2* __restrict__ G64, const int* __restrict
                           int n_pieces, int n_bins, int log2_fine, float2* __restrict__ out /* [n_pieces][8] */) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n_pieces) return;
-  const int lo = piece_lo[i], hi = min(piece_hi[i], n_bins);
+  // piece_lo == nullptr: uniform pieces of 2^(int)(size_t)piece_hi bins (the groups / sub-intervals of the adaptive path)
+  const int lg_u = (int)(size_t)piece_hi;
+  const int lo = piece_lo ? piece_lo[i] : (i << lg_u);
+  const int hi = min(piece_lo ? piece_hi[i] : ((i + 1) << lg_u), n_bins);
   const int ib = (lo >> log2_fine) << log2_fine;
   const double hS = 1.0 / (double)(1 << log2_fine);
   double mA[7] = {0, 0, 0, 0, 0, 0, 0}, mE[7] = {0, 0, 0, 0, 0, 0, 0};
@@ -513,6 +516,131 @@ __device__ __forceinline__ void sincos_frac32(int n, float& sr, float& cr) {
   sr = (q & 2) ? -sr : sr;
 }
 
+// ---- pieces of the packed hot loop shared by k_dense2 (shared edges) and k_dense2_ad (per-particle edges) ----
+struct PhaseFD { double phi, d1, d2, d3; };   // phase in turns at the next bin and its forward differences (unit steps)
+
+// Phase on fine sub-interval [ib, ib + Sf): quintic through 6 nodes -> Taylor shift to the centre of the sub-interval ->
+// Chebyshev economisation to a cubic on [-H, H] -> shift to the start -> forward differences for unit steps.
+__device__ __forceinline__ void sub_phase(const DevCfg& c, const DenseArgs& a, int p, int ib, PhaseFD& ph) {
+  const int ic = ib >> c.log2_stride;
+  const int i0 = ic + kNodeOff;
+  const int S = c.stride, Sf = S >> 2;
+  const size_t base = (size_t)i0 * a.P_pad + p;
+  const int n0 = a.node_n[base];
+  const double r0 = a.node_frac[base];
+  double Y[6];
+#pragma unroll
+  for (int m = -2; m <= 3; ++m) {
+    const size_t at = (size_t)(i0 + m) * a.P_pad + p;
+    Y[m + 2] = (double)(a.node_n[at] - n0) + (a.node_frac[at] - r0);
+  }
+  double b[6];
+  quintic_coeffs(Y, 1.0 / (double)S, b);
+  const double H = 0.5 * (double)Sf;
+  taylor_shift(b, (double)(ib - (ic << c.log2_stride)) + H);
+  const double H2 = H * H, H4 = H2 * H2;
+  b[0] = fma(-0.125 * H4, b[4], b[0]);
+  b[2] = fma(H2, b[4], b[2]);
+  b[1] = fma(-0.3125 * H4, b[5], b[1]);
+  b[3] = fma(1.25 * H2, b[5], b[3]);
+#pragma unroll
+  for (int i = 0; i < 3; ++i)
+#pragma unroll
+    for (int j = 2; j >= i; --j) b[j] = fma(-H, b[j + 1], b[j]);
+  ph.phi = r0 + b[0];
+  ph.d1 = b[1] + b[2] + b[3];
+  ph.d2 = 2.0 * b[2] + 6.0 * b[3];
+  ph.d3 = 6.0 * b[3];
+}
+
+// Cubic coefficients of (Ar, Ai, Er, Ei) on that sub-interval in s = (j - ib)/Sf.
+__device__ __forceinline__ void sub_amps(const DevCfg& c, const DenseArgs& a, int p, int ib, float (&cf)[4][4]) {
+  const int i0 = (ib >> c.log2_stride) + kNodeOff;
+  const int q = (ib >> (c.log2_stride - 2)) & 3;
+  const float* __restrict__ namp = reinterpret_cast<const float*>(a.node_amp);
+#pragma unroll
+  for (int r = 0; r < 4; r += 2) {                          // (Ar, Ai) then (Er, Ei) as packed halves
+    const float* col = namp + ((size_t)i0 * 4 + r) * a.P_pad + p;
+    const ptrdiff_t st = (ptrdiff_t)4 * a.P_pad;
+    u64 nd[6], o[4];
+#pragma unroll
+    for (int m = -2; m <= 3; ++m) nd[m + 2] = f2pack(col[m * st], col[m * st + a.P_pad]);
+    fine_cubic2(nd, q, o);
+#pragma unroll
+    for (int kk = 0; kk < 4; ++kk) f2unpack(o[kk], cf[r][kk], cf[r + 1][kk]);
+  }
+}
+
+// One bin pair (j, j+1): FP64 phase steps, sin/cos, amplitude cubics, multiply-accumulate into packed sums (low half =
+// even bin, high half = odd bin).  MASKED: apply the particle's time window per bin.  WITH_SG: accumulate |h|^2 per
+// bin (otherwise sigma comes from the moments).  s2 = (s_j, s_{j+1}), rec = the pair's data record; both advance.
+template <bool MASKED, bool WITH_SG, int SC>
+__device__ __forceinline__ void pair_eval(PhaseFD& ph, const float (&cf)[4][4], u64& s2, const ulonglong2*& rec, int j,
+                                          int jlo, int jhi, u64 h2, u64 K2, u64& zr2, u64& zi2, u64& sg2) {
+  const int n0 = __double2loint(ph.phi + 1572864.0);
+  ph.phi += ph.d1; ph.d1 += ph.d2; ph.d2 += ph.d3;
+  const int n1 = __double2loint(ph.phi + 1572864.0);
+  ph.phi += ph.d1; ph.d1 += ph.d2; ph.d2 += ph.d3;
+  float c0, c1, s0, s1;
+  if (SC == 2) {
+    float x0, x1;
+    f2unpack(f2mul(f2pack((float)n0, (float)n1), K2), x0, x1);
+    c0 = __cosf(x0); s0 = __sinf(x0); c1 = __cosf(x1); s1 = __sinf(x1);
+  } else {
+    sincos_frac32(n0, s0, c0);
+    sincos_frac32(n1, s1, c1);
+  }
+  u64 cr2 = f2pack(c0, c1), sr2 = f2pack(s0, s1);
+  const u64 Ar = f2fma(f2fma(f2fma(f2bcast(cf[0][3]), s2, f2bcast(cf[0][2])), s2, f2bcast(cf[0][1])), s2, f2bcast(cf[0][0]));
+  const u64 Ai = f2fma(f2fma(f2fma(f2bcast(cf[1][3]), s2, f2bcast(cf[1][2])), s2, f2bcast(cf[1][1])), s2, f2bcast(cf[1][0]));
+  const u64 Er = f2fma(f2fma(f2fma(f2bcast(cf[2][3]), s2, f2bcast(cf[2][2])), s2, f2bcast(cf[2][1])), s2, f2bcast(cf[2][0]));
+  const u64 Ei = f2fma(f2fma(f2fma(f2bcast(cf[3][3]), s2, f2bcast(cf[3][2])), s2, f2bcast(cf[3][1])), s2, f2bcast(cf[3][0]));
+  s2 = f2add(s2, h2);
+  const ulonglong2 wA = rec[0], wE = rec[1];
+  u64 m2 = 0;
+  if (MASKED) {
+    m2 = f2pack((j >= jlo && j < jhi) ? 1.0f : 0.0f, (j + 1 >= jlo && j + 1 < jhi) ? 1.0f : 0.0f);
+    cr2 = f2mul(cr2, m2); sr2 = f2mul(sr2, m2);
+  }
+  // q = W_A conj(c_A) + W_E conj(c_E)
+  const u64 qr = f2fma(wA.x, Ar, f2fma(wA.y, Ai, f2fma(wE.x, Er, f2mul(wE.y, Ei))));
+  const u64 qi = f2fma(wA.y, Ar, f2fma(f2neg(wA.x), Ai, f2fma(wE.y, Er, f2neg(f2mul(wE.x, Ei)))));
+  if (WITH_SG) {
+    ulonglong2 g = rec[2];
+    if (MASKED) { g.x = f2mul(g.x, m2); g.y = f2mul(g.y, m2); }
+    sg2 = f2fma(g.x, f2fma(Ar, Ar, f2mul(Ai, Ai)), f2fma(g.y, f2fma(Er, Er, f2mul(Ei, Ei)), sg2));
+  }
+  rec += kPairRec;
+  // z += q e^{+2 pi i Phi}
+  zr2 = f2fma(qr, cr2, f2fma(f2neg(qi), sr2, zr2));
+  zi2 = f2fma(qr, sr2, f2fma(qi, cr2, zi2));
+}
+
+// sigma of a run of bins from the moments of its weights: |c_a(s)|^2 = sum_m e_a,m s^m with the cubic coefficients of
+// the sub-interval; both channels at once (A in the low half, E in the high half).  mp: 4 records = 8 (A, E) pairs.
+__device__ __forceinline__ double sigma_moments(const float (&cf)[4][4], const ulonglong2* __restrict__ mp) {
+  const ulonglong2 m01 = mp[0], m23 = mp[1], m45 = mp[2], m6 = mp[3];
+  u64 R[4], I[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) { R[i] = f2pack(cf[0][i], cf[2][i]); I[i] = f2pack(cf[1][i], cf[3][i]); }
+  const u64 two = f2bcast(2.0f);
+  const u64 R0x2 = f2mul(R[0], two), I0x2 = f2mul(I[0], two), R1x2 = f2mul(R[1], two), I1x2 = f2mul(I[1], two);
+  const u64 R2x2 = f2mul(R[2], two), I2x2 = f2mul(I[2], two);
+  const u64 e0 = f2fma(R[0], R[0], f2mul(I[0], I[0]));
+  const u64 e1 = f2fma(R0x2, R[1], f2mul(I0x2, I[1]));
+  const u64 e2 = f2fma(R0x2, R[2], f2fma(I0x2, I[2], f2fma(R[1], R[1], f2mul(I[1], I[1]))));
+  const u64 e3 = f2fma(R0x2, R[3], f2fma(I0x2, I[3], f2fma(R1x2, R[2], f2mul(I1x2, I[2]))));
+  const u64 e4 = f2fma(R1x2, R[3], f2fma(I1x2, I[3], f2fma(R[2], R[2], f2mul(I[2], I[2]))));
+  const u64 e5 = f2fma(R2x2, R[3], f2mul(I2x2, I[3]));
+  const u64 e6 = f2fma(R[3], R[3], f2mul(I[3], I[3]));
+  u64 acc = f2mul(e0, m01.x);
+  acc = f2fma(e1, m01.y, acc); acc = f2fma(e2, m23.x, acc); acc = f2fma(e3, m23.y, acc);
+  acc = f2fma(e4, m45.x, acc); acc = f2fma(e5, m45.y, acc); acc = f2fma(e6, m6.x, acc);
+  float l, h;
+  f2unpack(acc, l, h);
+  return (double)l + (double)h;
+}
+
 template <bool SEG, int SC>
 __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2(DevCfg c, DenseArgs a, const ulonglong2* __restrict__ Dg) {
   constexpr int CH = kChunkF32;
@@ -536,7 +664,6 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2(DevCfg c, Den
   const float hS = 1.0f / (float)Sf;
   const u64 h2 = f2bcast(2.0f * hS);
   const u64 K2 = f2bcast(1.4629180792671596e-09f);            // 2 pi / 2^32
-  const float* __restrict__ namp = reinterpret_cast<const float*>(a.node_amp);
 
   int k = a.chunk_k0[chunk_l];
   int next_edge = (k + 1 <= a.n_seg) ? a.edges[k + 1] : INT_MAX;
@@ -569,7 +696,7 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2(DevCfg c, Den
     open_at_edge = true;
   };
 
-  double phi = 0.0, d1 = 0.0, d2 = 0.0, d3 = 0.0;
+  PhaseFD fd = {0.0, 0.0, 0.0, 0.0};
   for (int ib = cs; ib < ce2; ib += Sf) {
     const int ie = min(ib + Sf, ce2);
     const bool lane_in = (ib >= jlo) && (ie <= jhi);
@@ -579,122 +706,16 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2(DevCfg c, Den
 
     float cf[4][4];    // cubic coefficients of (Ar, Ai, Er, Ei) in s = (j - ib)/Sf (FFMA2 broadcasts a scalar operand)
     if (!all_out) {
-      const int ic = ib >> c.log2_stride;
-      const int i0 = ic + kNodeOff;
-      const int q = (ib >> (c.log2_stride - 2)) & 3;
-      {
-        // phase: quintic through 6 nodes -> Taylor shift to the centre of the fine sub-interval -> Chebyshev
-        // economisation to a cubic on [-H, H] -> shift to the start -> forward differences for unit steps
-        const size_t base = (size_t)i0 * a.P_pad + p;
-        const int n0 = a.node_n[base];
-        const double r0 = a.node_frac[base];
-        double Y[6];
-#pragma unroll
-        for (int m = -2; m <= 3; ++m) {
-          const size_t at = (size_t)(i0 + m) * a.P_pad + p;
-          Y[m + 2] = (double)(a.node_n[at] - n0) + (a.node_frac[at] - r0);
-        }
-        double b[6];
-        quintic_coeffs(Y, 1.0 / (double)S, b);
-        const double H = 0.5 * (double)Sf;
-        taylor_shift(b, (double)(ib - (ic << c.log2_stride)) + H);
-        const double H2 = H * H, H4 = H2 * H2;
-        b[0] = fma(-0.125 * H4, b[4], b[0]);
-        b[2] = fma(H2, b[4], b[2]);
-        b[1] = fma(-0.3125 * H4, b[5], b[1]);
-        b[3] = fma(1.25 * H2, b[5], b[3]);
-#pragma unroll
-        for (int i = 0; i < 3; ++i)
-#pragma unroll
-          for (int j = 2; j >= i; --j) b[j] = fma(-H, b[j + 1], b[j]);
-        phi = r0 + b[0];
-        d1 = b[1] + b[2] + b[3];
-        d2 = 2.0 * b[2] + 6.0 * b[3];
-        d3 = 6.0 * b[3];
-      }
-#pragma unroll
-      for (int r = 0; r < 4; r += 2) {                          // (Ar, Ai) then (Er, Ei) as packed halves
-        const float* col = namp + ((size_t)i0 * 4 + r) * a.P_pad + p;
-        const ptrdiff_t st = (ptrdiff_t)4 * a.P_pad;
-        u64 nd[6], o[4];
-#pragma unroll
-        for (int m = -2; m <= 3; ++m) nd[m + 2] = f2pack(col[m * st], col[m * st + a.P_pad]);
-        fine_cubic2(nd, q, o);
-#pragma unroll
-        for (int kk = 0; kk < 4; ++kk) f2unpack(o[kk], cf[r][kk], cf[r + 1][kk]);
-      }
+      sub_phase(c, a, p, ib, fd);
+      sub_amps(c, a, p, ib, cf);
     }
 
     u64 s2 = 0;        // (s_j, s_{j+1}) of the next pair
     const ulonglong2* rec = sD;   // its data record
-    // one bin pair (j, j+1): FP64 phase steps, sin/cos, amplitude cubics, multiply-accumulate into packed sums.
-    // MASKED: apply the particle's time window per bin.  WITH_SG: accumulate |h|^2 per bin (otherwise sigma comes
-    // from the piece moments).
     auto pair = [&](int j, auto masked_c, auto with_sg_c, u64& zr2, u64& zi2, u64& sg2) {
-      constexpr bool MASKED = decltype(masked_c)::value, WITH_SG = decltype(with_sg_c)::value;
-      const int n0 = __double2loint(phi + 1572864.0);
-      phi += d1; d1 += d2; d2 += d3;
-      const int n1 = __double2loint(phi + 1572864.0);
-      phi += d1; d1 += d2; d2 += d3;
-      float c0, c1, s0, s1;
-      if (SC == 2) {
-        float x0, x1;
-        f2unpack(f2mul(f2pack((float)n0, (float)n1), K2), x0, x1);
-        c0 = __cosf(x0); s0 = __sinf(x0); c1 = __cosf(x1); s1 = __sinf(x1);
-      } else {
-        sincos_frac32(n0, s0, c0);
-        sincos_frac32(n1, s1, c1);
-      }
-      u64 cr2 = f2pack(c0, c1), sr2 = f2pack(s0, s1);
-      const u64 Ar = f2fma(f2fma(f2fma(f2bcast(cf[0][3]), s2, f2bcast(cf[0][2])), s2, f2bcast(cf[0][1])), s2, f2bcast(cf[0][0]));
-      const u64 Ai = f2fma(f2fma(f2fma(f2bcast(cf[1][3]), s2, f2bcast(cf[1][2])), s2, f2bcast(cf[1][1])), s2, f2bcast(cf[1][0]));
-      const u64 Er = f2fma(f2fma(f2fma(f2bcast(cf[2][3]), s2, f2bcast(cf[2][2])), s2, f2bcast(cf[2][1])), s2, f2bcast(cf[2][0]));
-      const u64 Ei = f2fma(f2fma(f2fma(f2bcast(cf[3][3]), s2, f2bcast(cf[3][2])), s2, f2bcast(cf[3][1])), s2, f2bcast(cf[3][0]));
-      s2 = f2add(s2, h2);
-      const ulonglong2 wA = rec[0], wE = rec[1];
-      u64 m2 = 0;
-      if (MASKED) {
-        m2 = f2pack((j >= jlo && j < jhi) ? 1.0f : 0.0f, (j + 1 >= jlo && j + 1 < jhi) ? 1.0f : 0.0f);
-        cr2 = f2mul(cr2, m2); sr2 = f2mul(sr2, m2);
-      }
-      // q = W_A conj(c_A) + W_E conj(c_E)
-      const u64 qr = f2fma(wA.x, Ar, f2fma(wA.y, Ai, f2fma(wE.x, Er, f2mul(wE.y, Ei))));
-      const u64 qi = f2fma(wA.y, Ar, f2fma(f2neg(wA.x), Ai, f2fma(wE.y, Er, f2neg(f2mul(wE.x, Ei)))));
-      if (WITH_SG) {
-        ulonglong2 g = rec[2];
-        if (MASKED) { g.x = f2mul(g.x, m2); g.y = f2mul(g.y, m2); }
-        sg2 = f2fma(g.x, f2fma(Ar, Ar, f2mul(Ai, Ai)), f2fma(g.y, f2fma(Er, Er, f2mul(Ei, Ei)), sg2));
-      }
-      rec += kPairRec;
-      // z += q e^{+2 pi i Phi}
-      zr2 = f2fma(qr, cr2, f2fma(f2neg(qi), sr2, zr2));
-      zi2 = f2fma(qr, sr2, f2fma(qi, cr2, zi2));
+      pair_eval<decltype(masked_c)::value, decltype(with_sg_c)::value, SC>(fd, cf, s2, rec, j, jlo, jhi, h2, K2, zr2, zi2, sg2);
     };
-    // sigma of one piece from its moments: |c_a(s)|^2 = sum_m e_a,m s^m with the cubic coefficients of this
-    // sub-interval; both channels at once (A in the low half, E in the high half)
-    auto sigma_piece = [&](int piece) {
-      const ulonglong2* mp = a.moments + (size_t)piece * 4;
-      const ulonglong2 m01 = mp[0], m23 = mp[1], m45 = mp[2], m6 = mp[3];
-      u64 R[4], I[4];
-#pragma unroll
-      for (int i = 0; i < 4; ++i) { R[i] = f2pack(cf[0][i], cf[2][i]); I[i] = f2pack(cf[1][i], cf[3][i]); }
-      const u64 two = f2bcast(2.0f);
-      const u64 R0x2 = f2mul(R[0], two), I0x2 = f2mul(I[0], two), R1x2 = f2mul(R[1], two), I1x2 = f2mul(I[1], two);
-      const u64 R2x2 = f2mul(R[2], two), I2x2 = f2mul(I[2], two);
-      const u64 e0 = f2fma(R[0], R[0], f2mul(I[0], I[0]));
-      const u64 e1 = f2fma(R0x2, R[1], f2mul(I0x2, I[1]));
-      const u64 e2 = f2fma(R0x2, R[2], f2fma(I0x2, I[2], f2fma(R[1], R[1], f2mul(I[1], I[1]))));
-      const u64 e3 = f2fma(R0x2, R[3], f2fma(I0x2, I[3], f2fma(R1x2, R[2], f2mul(I1x2, I[2]))));
-      const u64 e4 = f2fma(R1x2, R[3], f2fma(I1x2, I[3], f2fma(R[2], R[2], f2mul(I[2], I[2]))));
-      const u64 e5 = f2fma(R2x2, R[3], f2mul(I2x2, I[3]));
-      const u64 e6 = f2fma(R[3], R[3], f2mul(I[3], I[3]));
-      u64 acc = f2mul(e0, m01.x);
-      acc = f2fma(e1, m01.y, acc); acc = f2fma(e2, m23.x, acc); acc = f2fma(e3, m23.y, acc);
-      acc = f2fma(e4, m45.x, acc); acc = f2fma(e5, m45.y, acc); acc = f2fma(e6, m6.x, acc);
-      float l, h;
-      f2unpack(acc, l, h);
-      Sg += (double)l + (double)h;
-    };
+    auto sigma_piece = [&](int piece) { Sg += sigma_moments(cf, a.moments + (size_t)piece * 4); };
     using T_ = std::true_type; using F_ = std::false_type;
 
     // Walk the pieces of this sub-interval (it is cut at every distinct edge inside it).  Pairs are evaluated once:
@@ -717,7 +738,7 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2(DevCfg c, Den
       const int jfull = ph & ~1;                               // full pairs end here; a straddling pair follows if ph is odd
       if (!all_out) {
         if (!live && jj < jfull) {
-          for (int t = jj; t < jfull; ++t) { phi += d1; d1 += d2; d2 += d3; }
+          for (int t = jj; t < jfull; ++t) { fd.phi += fd.d1; fd.d1 += fd.d2; fd.d2 += fd.d3; }
           jj = jfull;
         }
         s2 = f2pack((float)(jj - ib) * hS, (float)(jj + 1 - ib) * hS);
@@ -752,6 +773,227 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2(DevCfg c, Den
     frag[0] = ups;
     if (a.comp) { frag[(size_t)7 * a.P_pad] = xs; frag[(size_t)8 * a.P_pad] = hs; }
   }
+}
+
+// ------------------------------------------------------------------------------------------------ per-particle segments
+// Equal squared-SNR segments re-evaluated for every particle (App. A):
+//   s_j = sum_a |h_a(f_j)|^2 / S_a(f_j),  C = sum_j s_j,  e_0 = 0, e_N = n_bins,
+//   e_n = min{ j : sum_{j' < j} s_j' >= C n / N }   (n = 1 .. N-1),
+// then Upsilon_N on those edges.  Three steps, all with lane = particle:
+//   k_sigma_chunks   sigma of every (chunk, particle) from the moments of the weights (no per-bin work inside the window)
+//   k_scan_chunks    prefix sum over chunks -> cumulative sigma at every chunk start, and C
+//   k_dense2_ad      the hot loop of k_dense2 with a running cumulative sigma per lane: groups of <= 32 bins in which
+//                    no lane of the warp reaches its next target (decided from the group's moments) take the unmasked
+//                    packed path; the others are walked bin by bin and the segments are closed where the running sum
+//                    crosses the target.  The number of edges closed inside a chunk is fixed by the scanned sums
+//                    (k0 = K(cbase[chunk]), k1 = K(cbase[chunk + 1])), so neighbouring chunks always agree.
+constexpr int kFragAd = 10;    // partial Upsilon, head (zr, zi, sg), tail (zr, zi, sg), head-closes flag, partial sum|z|, sum sigma
+
+struct AdaptArgs {
+  int n_seg, n_chunks;
+  const double* cbase;         // [n_chunks + 1][P_pad]: cumulative sigma at the chunk starts; row n_chunks = C
+  const ulonglong2* gmom;      // [n_groups][4] moments of the weights over groups of 2^lg_group bins
+  const ulonglong2* smom;      // [n_sub][4]    ... over the fine sub-intervals
+  int lg_group;
+  int* out_edges;              // [P][n_seg + 1] of this batch, or nullptr
+  double* chunk_sigma;         // = cbase (written by k_sigma_chunks before the scan)
+};
+
+__device__ __forceinline__ double seg_target(double C, int n, int N) { return C * (double)n / (double)N; }
+// K(c) = max{ n in [0, N-1] : C n / N <= c }: the segment that contains the first bin whose cumulative sum is c.
+__device__ __forceinline__ int seg_index(double cum, double C, int N) {
+  if (!(C > 0.0)) return 0;
+  int n = (int)(cum / C * (double)N);
+  n = min(max(n, 0), N - 1);
+  while (n + 1 <= N - 1 && seg_target(C, n + 1, N) <= cum) ++n;
+  while (n > 0 && seg_target(C, n, N) > cum) --n;
+  return n;
+}
+
+__global__ void __launch_bounds__(kBlock) k_sigma_chunks(DevCfg c, DenseArgs a, AdaptArgs ad, const float4* __restrict__ D32) {
+  constexpr int CH = kChunkF32;
+  const int chunk = blockIdx.x;
+  const int cs = chunk * CH;
+  const int ce = min(cs + CH, c.n_bins);
+  const int ce2 = (ce + 1) & ~1;
+  const int p = blockIdx.y * kBlock + threadIdx.x;
+  const int jlo = a.jlo[p], jhi = a.jhi[p];
+  const int Sf = c.stride >> 2;
+  const float hS = 1.0f / (float)Sf;
+  double tot = 0.0;
+  for (int ib = cs; ib < ce2; ib += Sf) {
+    const int ie = min(ib + Sf, ce2);
+    const bool lane_in = (ib >= jlo) && (ie <= jhi);
+    const bool lane_out = (ie <= jlo) || (ib >= jhi);
+    const bool all_in = __all_sync(0xffffffffu, lane_in);
+    const bool all_out = __all_sync(0xffffffffu, lane_out);
+    if (all_out) continue;
+    float cf[4][4];
+    sub_amps(c, a, p, ib, cf);
+    if (all_in) {
+      tot += sigma_moments(cf, ad.smom + (size_t)(ib >> (c.log2_stride - 2)) * 4);
+    } else {
+      // a window border of some lane falls in this sub-interval: bin by bin, masked (two sub-intervals per particle)
+      for (int j = ib; j < ie; ++j) {
+        const float sj = (float)(j - ib) * hS;
+        const float Ar = fmaf(fmaf(fmaf(cf[0][3], sj, cf[0][2]), sj, cf[0][1]), sj, cf[0][0]);
+        const float Ai = fmaf(fmaf(fmaf(cf[1][3], sj, cf[1][2]), sj, cf[1][1]), sj, cf[1][0]);
+        const float Er = fmaf(fmaf(fmaf(cf[2][3], sj, cf[2][2]), sj, cf[2][1]), sj, cf[2][0]);
+        const float Ei = fmaf(fmaf(fmaf(cf[3][3], sj, cf[3][2]), sj, cf[3][1]), sj, cf[3][0]);
+        const float4 g = D32[(size_t)(j >> 1) * kPairRec + 2];            // (gA even, gA odd, gE even, gE odd)
+        const float gA = (j & 1) ? g.y : g.x, gE = (j & 1) ? g.w : g.z;
+        const float sg = fmaf(gA, fmaf(Ar, Ar, Ai * Ai), gE * fmaf(Er, Er, Ei * Ei));
+        if (j >= jlo && j < jhi) tot += (double)sg;
+      }
+    }
+  }
+  ad.chunk_sigma[(size_t)(chunk + 1) * a.P_pad + p] = tot;
+}
+
+__global__ void k_scan_chunks(double* __restrict__ cbase, int n_chunks, int P_pad) {
+  const int p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= P_pad) return;
+  double acc = 0.0;
+  cbase[p] = 0.0;
+  for (int i = 1; i <= n_chunks; ++i) {
+    acc += cbase[(size_t)i * P_pad + p];
+    cbase[(size_t)i * P_pad + p] = acc;
+  }
+}
+
+template <int SC>
+__global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2_ad(DevCfg c, DenseArgs a, AdaptArgs ad,
+                                                                      const ulonglong2* __restrict__ Dg) {
+  constexpr int CH = kChunkF32;
+  __shared__ ulonglong2 sD[CH / 2 * kPairRec];
+  const int chunk = blockIdx.x;
+  const int cs = chunk * CH;
+  const int ce = min(cs + CH, c.n_bins);
+  const int ce2 = (ce + 1) & ~1;
+  const int p = blockIdx.y * kBlock + threadIdx.x;
+  {
+    const ulonglong2* src = Dg + (size_t)(cs >> 1) * kPairRec;
+#pragma unroll 4
+    for (int t = threadIdx.x; t < CH / 2 * kPairRec; t += kBlock) sD[t] = src[t];
+  }
+  __syncthreads();
+
+  const int jlo = a.jlo[p], jhi = a.jhi[p];
+  const int Sf = c.stride >> 2;
+  const float hS = 1.0f / (float)Sf;
+  const u64 h2 = f2bcast(2.0f * hS);
+  const u64 K2 = f2bcast(1.4629180792671596e-09f);
+  const int N = ad.n_seg;
+  const int Gs = 1 << ad.lg_group;
+
+  const double C = ad.cbase[(size_t)ad.n_chunks * a.P_pad + p];
+  const double cb0 = ad.cbase[(size_t)chunk * a.P_pad + p];
+  const double cb1 = ad.cbase[(size_t)(chunk + 1) * a.P_pad + p];
+  int k = seg_index(cb0, C, N);                 // segment open at the chunk start
+  const int k1 = seg_index(cb1, C, N);          // edges k+1 .. k1 are closed inside this chunk, no more, no fewer
+  double t_next = (k < k1) ? seg_target(C, k + 1, N) - cb0 : INFINITY;
+  double crel = 0.0, c_open = 0.0;              // cumulative sigma relative to the chunk start; its value where the open piece began
+  double Zr = 0.0, Zi = 0.0, ups = 0.0, xs = 0.0, hs = 0.0;
+  bool closed_any = false;
+  double* frag = a.frag + (size_t)chunk * kFragAd * a.P_pad + p;
+
+  auto close_at = [&](int j) {                  // edge k+1 lies at bin j
+    const double Sg = crel - c_open;
+    if (!closed_any) {                          // the piece that was open at the chunk start: head fragment
+      frag[(size_t)1 * a.P_pad] = Zr; frag[(size_t)2 * a.P_pad] = Zi; frag[(size_t)3 * a.P_pad] = Sg;
+      closed_any = true;
+    } else if (Sg > 0.0) {
+      const double z2 = Zr * Zr + Zi * Zi;
+      ups += z2 / Sg;
+      if (a.comp) { xs += sqrt(z2); hs += Sg; }
+    }
+    Zr = 0.0; Zi = 0.0; c_open = crel;
+    ++k;
+    if (ad.out_edges && p < a.P) ad.out_edges[(size_t)p * (N + 1) + k] = j;
+    t_next = (k < k1) ? seg_target(C, k + 1, N) - cb0 : INFINITY;
+  };
+
+  PhaseFD ph = {0.0, 0.0, 0.0, 0.0};
+  for (int ib = cs; ib < ce2; ib += Sf) {
+    const int ie = min(ib + Sf, ce2);
+    const bool lane_in = (ib >= jlo) && (ie <= jhi);
+    const bool lane_out = (ie <= jlo) || (ib >= jhi);
+    const bool all_in = __all_sync(0xffffffffu, lane_in);
+    const bool all_out = __all_sync(0xffffffffu, lane_out);
+    if (all_out) continue;
+    float cf[4][4];
+    sub_phase(c, a, p, ib, ph);
+    sub_amps(c, a, p, ib, cf);
+    u64 s2 = f2pack(0.0f, hS);
+    const ulonglong2* rec = sD + ((ib - cs) >> 1) * kPairRec;
+    for (int gs = ib; gs < ie; gs += Gs) {
+      const int ge = min(gs + Gs, ie);
+      const double sg_m = sigma_moments(cf, ad.gmom + (size_t)(gs >> ad.lg_group) * 4);
+      // would the running sum reach this lane's next target inside the group?  (margin: the per-bin and the moment sums
+      // differ by FP32 rounding; a group flagged needlessly only takes the slower path)
+      const bool cross = (k < k1) && (crel + sg_m * 1.0001 >= t_next);
+      const bool slow = !all_in || __any_sync(0xffffffffu, cross);
+      if (!slow) {
+        u64 zr2 = 0, zi2 = 0, sg2 = 0;
+        for (int jj = gs; jj < ge; jj += 2) pair_eval<false, false, SC>(ph, cf, s2, rec, jj, jlo, jhi, h2, K2, zr2, zi2, sg2);
+        float zrl, zrh, zil, zih;
+        f2unpack(zr2, zrl, zrh); f2unpack(zi2, zil, zih);
+        Zr += (double)(zrl + zrh); Zi += (double)(zil + zih);
+        crel += sg_m;
+      } else {
+        for (int jj = gs; jj < ge; jj += 2) {
+          u64 zr2 = 0, zi2 = 0, sg2 = 0;
+          pair_eval<true, true, SC>(ph, cf, s2, rec, jj, jlo, jhi, h2, K2, zr2, zi2, sg2);
+          float zrl, zrh, zil, zih, sgl, sgh;
+          f2unpack(zr2, zrl, zrh); f2unpack(zi2, zil, zih); f2unpack(sg2, sgl, sgh);
+          while (k < k1 && crel >= t_next) close_at(jj);          // e_n = first bin whose cumulative sum reached the target
+          Zr += (double)zrl; Zi += (double)zil; crel += (double)sgl;
+          while (k < k1 && crel >= t_next) close_at(jj + 1);
+          Zr += (double)zrh; Zi += (double)zih; crel += (double)sgh;
+        }
+      }
+    }
+  }
+  while (k < k1) close_at(ce);                  // targets the scanned sums place in this chunk (rounding): at its end
+  const double Sg = crel - c_open;
+  if (!closed_any) {
+    frag[(size_t)1 * a.P_pad] = Zr; frag[(size_t)2 * a.P_pad] = Zi; frag[(size_t)3 * a.P_pad] = Sg;
+    frag[(size_t)4 * a.P_pad] = 0.0; frag[(size_t)5 * a.P_pad] = 0.0; frag[(size_t)6 * a.P_pad] = 0.0;
+  } else {
+    frag[(size_t)4 * a.P_pad] = Zr; frag[(size_t)5 * a.P_pad] = Zi; frag[(size_t)6 * a.P_pad] = Sg;
+  }
+  frag[(size_t)7 * a.P_pad] = closed_any ? 1.0 : 0.0;
+  frag[0] = ups;
+  if (a.comp) { frag[(size_t)8 * a.P_pad] = xs; frag[(size_t)9 * a.P_pad] = hs; }
+}
+
+__global__ void k_stitch_ad(const double* __restrict__ frag, int n_chunks, int P_pad, int P, double scale,
+                            double* __restrict__ out, double* __restrict__ comp3, double x_scale, double h_scale,
+                            int* __restrict__ out_edges, int n_seg, int n_bins) {
+  const int p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= P) return;
+  double ups = 0.0, zr = 0.0, zi = 0.0, sg = 0.0, xs = 0.0, hs = 0.0;
+  auto finish = [&]() {
+    if (sg > 0.0) {
+      const double z2 = zr * zr + zi * zi;
+      ups += z2 / sg;
+      if (comp3) { xs += sqrt(z2); hs += sg; }
+    }
+  };
+  for (int cI = 0; cI < n_chunks; ++cI) {
+    const double* f = frag + (size_t)cI * kFragAd * P_pad + p;
+    zr += f[(size_t)1 * P_pad]; zi += f[(size_t)2 * P_pad]; sg += f[(size_t)3 * P_pad];
+    if (f[(size_t)7 * P_pad] != 0.0) {
+      finish();
+      zr = f[(size_t)4 * P_pad]; zi = f[(size_t)5 * P_pad]; sg = f[(size_t)6 * P_pad];
+    }
+    ups += f[0];
+    if (comp3) { xs += f[(size_t)8 * P_pad]; hs += f[(size_t)9 * P_pad]; }
+  }
+  finish();                                     // the last segment closes at e_N = n_bins
+  if (out) out[p] = ups * scale;
+  if (comp3) { comp3[3 * (size_t)p] = ups * scale; comp3[3 * (size_t)p + 1] = xs * x_scale; comp3[3 * (size_t)p + 2] = hs * h_scale; }
+  if (out_edges) { out_edges[(size_t)p * (n_seg + 1)] = 0; out_edges[(size_t)p * (n_seg + 1) + n_seg] = n_bins; }
 }
 
 // ------------------------------------------------------------------------------------------------ a6
@@ -996,6 +1238,8 @@ struct sc_handle {
   double mufu_gain2 = 1.0;        // <cos^2 + sin^2> of the hardware sin/cos, measured at init
   double dd = 0.0;                // <d|d> (Eq. 1), computed at init
   double* d_comp = nullptr; size_t comp_cap = 0;   // components scratch of sc_eval_loglike
+  // adaptive (per-particle) segments: moments of the weights over groups and fine sub-intervals, cached per node spacing
+  int ad_lg = 0; float2* d_gmom = nullptr; float2* d_smom = nullptr; size_t gmom_cap = 0, smom_cap = 0;
   // scratch
   void* scratch = nullptr; size_t scratch_bytes = 0;
   int* d_edges = nullptr; int* d_chunk_k0 = nullptr; uint8_t* d_flags = nullptr; size_t edge_cap = 0, k0_cap = 0, flags_cap = 0;
@@ -1310,6 +1554,103 @@ int eval_common(sc_handle* h, const double* params, int64_t P, const int32_t* se
              : run_batches<float>(h, params, P, out, out_seg, out_comp, st, seg_mode);
 }
 
+// Per-particle equal-SNR^2 segments: see the kernels above.  FP32-amplitude path.
+int run_adaptive(sc_handle* h, const double* params, int64_t P, int n_seg, double* out, int32_t* out_edges, double* out_comp,
+                 cudaStream_t st) {
+  DevCfg dc = h->dc;
+  apply_stride(dc, h->lg_f32);
+  const int CH = kChunkF32;
+  const int n_nodes = dc.n_nodes;
+  const int n_chunks = (dc.n_bins + CH - 1) / CH;
+  const int lg_fine = dc.log2_stride - 2, lg_group = std::min(5, lg_fine);
+  int rc;
+  // moments tables (shared by all particles; depend on the data and the node spacing only)
+  const int n_groups = (int)(((long long)n_chunks * CH) >> lg_group), n_sub = (int)(((long long)n_chunks * CH) >> lg_fine);
+  if (h->ad_lg != dc.log2_stride) {
+    if ((rc = grow(h, (void**)&h->d_gmom, &h->gmom_cap, (size_t)n_groups * 8 * sizeof(float2)))) return rc;
+    if ((rc = grow(h, (void**)&h->d_smom, &h->smom_cap, (size_t)n_sub * 8 * sizeof(float2)))) return rc;
+    Timed tm(h, st, SC_TIME_OTHER);
+    k_moments<<<(n_groups + 127) / 128, 128, 0, st>>>(h->G64, nullptr, (const int*)(size_t)lg_group, n_groups, dc.n_bins, lg_fine, h->d_gmom);
+    if ((rc = check_launch(h, "k_moments"))) return rc;
+    k_moments<<<(n_sub + 127) / 128, 128, 0, st>>>(h->G64, nullptr, (const int*)(size_t)lg_fine, n_sub, dc.n_bins, lg_fine, h->d_smom);
+    if ((rc = check_launch(h, "k_moments"))) return rc;
+    h->ad_lg = dc.log2_stride;
+  }
+  const size_t per_p = (size_t)kPcFields * 8 + 8 + (size_t)n_nodes * (4 + 8 + 4 * sizeof(float))
+                       + (size_t)(n_chunks + 1) * 8 + (size_t)n_chunks * kFragAd * 8;
+  int64_t Pb_max = (int64_t)(h->scratch_cap / per_p) / kBlock * kBlock;
+  if (Pb_max < kBlock) Pb_max = kBlock;
+  const int64_t P_round = (P + kBlock - 1) / kBlock * kBlock;
+  const int P_pad = (int)std::min<int64_t>(Pb_max, P_round);
+  if ((rc = grow(h, &h->scratch, &h->scratch_bytes, per_p * (size_t)P_pad + 2048))) return rc;
+  char* base = (char*)h->scratch;
+  auto take = [&](size_t bytes) { char* r = base; base += (bytes + 255) / 256 * 256; return r; };
+  double* pc = (double*)take((size_t)kPcFields * 8 * P_pad);
+  int* jlo = (int*)take((size_t)4 * P_pad);
+  int* jhi = (int*)take((size_t)4 * P_pad);
+  int* node_n = (int*)take((size_t)n_nodes * 4 * P_pad);
+  double* node_frac = (double*)take((size_t)n_nodes * 8 * P_pad);
+  float* node_amp = (float*)take((size_t)n_nodes * 4 * sizeof(float) * P_pad);
+  double* cbase = (double*)take((size_t)(n_chunks + 1) * 8 * P_pad);
+  double* frag = (double*)take((size_t)n_chunks * kFragAd * 8 * P_pad);
+  (void)base;
+
+  const double four_df = 4.0 / h->cfg.T_obs_s;
+  const int sincos = (h->sincos_mode == 0) ? (n_seg >= h->mufu_min_seg ? 2 : 0) : (h->sincos_mode == 2 ? 2 : 0);
+  const double h0 = pow(dc.f_amp_ref, -7.0 / 6.0);
+  (void)four_df;
+  if (out_edges) SC_CUDA(h, cudaMemsetAsync(out_edges, 0, (size_t)P * (n_seg + 1) * 4, st));
+
+  for (int64_t pb = 0; pb < P; pb += P_pad) {
+    const int Pn = (int)std::min<int64_t>(P_pad, P - pb);
+    {
+      Timed tm(h, st, SC_TIME_NODES);
+      k_particle_consts<<<(P_pad + 127) / 128, 128, 0, st>>>(dc, params + pb * 8, Pn, P_pad, pc, jlo, jhi, 0, dc.n_bins, h->d_counter);
+    }
+    if ((rc = check_launch(h, "k_particle_consts"))) return rc;
+    {
+      Timed tm(h, st, SC_TIME_NODES);
+      k_nodes<float><<<dim3(n_nodes, (P_pad + 127) / 128), 128, 0, st>>>(dc, pc, jlo, jhi, P_pad, node_n, node_frac, node_amp);
+    }
+    if ((rc = check_launch(h, "k_nodes"))) return rc;
+    DenseArgs a = {};
+    a.node_n = node_n; a.node_frac = node_frac; a.node_amp = node_amp; a.jlo = jlo; a.jhi = jhi; a.P_pad = P_pad;
+    a.frag = frag; a.P = Pn; a.comp = out_comp ? 1 : 0; a.n_seg = n_seg;
+    AdaptArgs ad = {};
+    ad.n_seg = n_seg; ad.n_chunks = n_chunks; ad.cbase = cbase; ad.chunk_sigma = cbase;
+    ad.gmom = reinterpret_cast<const ulonglong2*>(h->d_gmom); ad.smom = reinterpret_cast<const ulonglong2*>(h->d_smom);
+    ad.lg_group = lg_group;
+    ad.out_edges = out_edges ? out_edges + (size_t)pb * (n_seg + 1) : nullptr;
+    const dim3 grid(n_chunks, P_pad / kBlock);
+    {
+      Timed tm(h, st, SC_TIME_OTHER);
+      k_sigma_chunks<<<grid, kBlock, 0, st>>>(dc, a, ad, h->D32);
+      if ((rc = check_launch(h, "k_sigma_chunks"))) return rc;
+      k_scan_chunks<<<(P_pad + 127) / 128, 128, 0, st>>>(cbase, n_chunks, P_pad);
+      if ((rc = check_launch(h, "k_scan_chunks"))) return rc;
+    }
+    {
+      Timed tm(h, st, SC_TIME_DENSE);
+      const ulonglong2* Dp = reinterpret_cast<const ulonglong2*>(h->D32);
+      if (sincos == 2) k_dense2_ad<2><<<grid, kBlock, 0, st>>>(dc, a, ad, Dp);
+      else k_dense2_ad<0><<<grid, kBlock, 0, st>>>(dc, a, ad, Dp);
+    }
+    if ((rc = check_launch(h, "k_dense2_ad"))) return rc;
+    Timed tm2(h, st, SC_TIME_STITCH);
+    const double g2 = (sincos == 2) ? h->mufu_gain2 : 1.0;
+    k_stitch_ad<<<(Pn + 127) / 128, 128, 0, st>>>(frag, n_chunks, P_pad, Pn, 1.0 / g2, out ? out + pb : nullptr,
+                                                  out_comp ? out_comp + pb * 3 : nullptr, h->s0 * h0 / sqrt(g2),
+                                                  h->s0 * h->s0 * h0 * h0, ad.out_edges, n_seg, dc.n_bins);
+    if ((rc = check_launch(h, "k_stitch_ad"))) return rc;
+  }
+  return SC_OK;
+}
+
+__global__ void k_fill_edges01(int* __restrict__ out_edges, int P, int n_bins) {
+  const int p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p < P) { out_edges[2 * (size_t)p] = 0; out_edges[2 * (size_t)p + 1] = n_bins; }
+}
+
 int init_common(sc_handle** out, const sc_config* cfg, const double* dA, const double* dE, const double* S_A,
                 const double* S_E, void* stream, bool host_inputs) {
   if (!out) return fail(nullptr, SC_ERR_INVALID_ARG, "out is null");
@@ -1454,6 +1795,27 @@ int sc_data_norm(sc_handle* h, double* dd) {
   if (!dd) return fail(h, SC_ERR_INVALID_ARG, "dd is null");
   *dd = h->dd;
   return SC_OK;
+}
+
+int sc_eval_stat_adaptive(sc_handle* h, const double* params, int64_t P, int32_t n_seg, double* out, int32_t* out_edges,
+                          double* out3, void* stream) {
+  if (!h) return SC_ERR_NOT_INIT;
+  if (h->cuda_failed) return SC_ERR_CUDA;
+  if (!params || P <= 0 || n_seg <= 0 || (!out && !out3)) return fail(h, SC_ERR_INVALID_ARG, "null pointer, n_particles <= 0 or n_seg <= 0");
+  if (n_seg > h->cfg.n_bins) return fail(h, SC_ERR_INVALID_ARG, "n_seg exceeds n_bins");
+  cudaStream_t st = (cudaStream_t)stream;
+  if (n_seg == 1) {                              // one segment: the edges are (0, n_bins) for every particle
+    const int32_t e[2] = {0, (int32_t)h->cfg.n_bins};
+    int rc = eval_common(h, params, P, e, 1, out, nullptr, stream, false, out3);
+    if (rc) return rc;
+    if (out_edges) {
+      k_fill_edges01<<<(unsigned)((P + 127) / 128), 128, 0, st>>>(out_edges, (int)P, (int)h->cfg.n_bins);
+      return check_launch(h, "k_fill_edges01");
+    }
+    return SC_OK;
+  }
+  SC_CUDA(h, cudaMemsetAsync(h->d_counter, 0, 8, st));
+  return run_adaptive(h, params, P, n_seg, out, out_edges, out3, st);
 }
 
 int sc_eval_stat_host(sc_handle* h, const double* params, int64_t P, const int32_t* seg_edges, int32_t n_seg,
@@ -1626,7 +1988,7 @@ int sc_free(sc_handle* h) {
   if (!h) return SC_ERR_NOT_INIT;
   cudaFree(h->D32); cudaFree(h->W64); cudaFree(h->G64);
   cudaFree(h->scratch); cudaFree(h->d_edges); cudaFree(h->d_chunk_k0); cudaFree(h->d_flags);
-  cudaFree(h->d_counter); cudaFree(h->d_params_stage); cudaFree(h->d_comp);
+  cudaFree(h->d_counter); cudaFree(h->d_params_stage); cudaFree(h->d_comp); cudaFree(h->d_gmom); cudaFree(h->d_smom);
   cudaFree(h->d_piece_first); cudaFree(h->d_piece_lo); cudaFree(h->d_piece_hi); cudaFree(h->d_moments);
   for (auto& e : h->evs) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
   cudaGetLastError();
