@@ -475,6 +475,7 @@ __device__ __forceinline__ void fine_cubic2(const u64 nd[6], int q, u64 out[4]) 
 #ifndef SC_DENSE2_MINB
 #define SC_DENSE2_MINB 4     /* CTAs per SM the register allocation aims at (128 registers/thread) */
 #endif
+
 constexpr int kPairRec = 3;
 
 // Moments of the sigma weights over one piece (a fine sub-interval cut at the segment edges; shared by all particles):
@@ -518,6 +519,22 @@ __device__ __forceinline__ void sincos_frac32(int n, float& sr, float& cr) {
 
 // ---- pieces of the packed hot loop shared by k_dense2 (shared edges) and k_dense2_ad (per-particle edges) ----
 struct PhaseFD { double phi, d1, d2, d3; };   // phase in turns at the next bin and its forward differences (unit steps)
+__device__ __forceinline__ void phase_next_pair(PhaseFD& ph, int& n0, int& n1) {
+  n0 = __double2loint(ph.phi + 1572864.0);
+  ph.phi += ph.d1; ph.d1 += ph.d2; ph.d2 += ph.d3;
+  n1 = __double2loint(ph.phi + 1572864.0);
+  ph.phi += ph.d1; ph.d1 += ph.d2; ph.d2 += ph.d3;
+}
+__device__ __forceinline__ void phase_skip_pair(PhaseFD& ph) {
+  ph.phi += ph.d1; ph.d1 += ph.d2; ph.d2 += ph.d3;
+  ph.phi += ph.d1; ph.d1 += ph.d2; ph.d2 += ph.d3;
+}
+__device__ __forceinline__ void phase_set(PhaseFD& ph, double p0, const double b[6]) {
+  ph.phi = p0;
+  ph.d1 = b[1] + b[2] + b[3];
+  ph.d2 = 2.0 * b[2] + 6.0 * b[3];
+  ph.d3 = 6.0 * b[3];
+}
 
 // Phase on fine sub-interval [ib, ib + Sf): quintic through 6 nodes -> Taylor shift to the centre of the sub-interval ->
 // Chebyshev economisation to a cubic on [-H, H] -> shift to the start -> forward differences for unit steps.
@@ -547,10 +564,7 @@ __device__ __forceinline__ void sub_phase(const DevCfg& c, const DenseArgs& a, i
   for (int i = 0; i < 3; ++i)
 #pragma unroll
     for (int j = 2; j >= i; --j) b[j] = fma(-H, b[j + 1], b[j]);
-  ph.phi = r0 + b[0];
-  ph.d1 = b[1] + b[2] + b[3];
-  ph.d2 = 2.0 * b[2] + 6.0 * b[3];
-  ph.d3 = 6.0 * b[3];
+  phase_set(ph, r0 + b[0], b);
 }
 
 // Cubic coefficients of (Ar, Ai, Er, Ei) on that sub-interval in s = (j - ib)/Sf.
@@ -577,10 +591,8 @@ __device__ __forceinline__ void sub_amps(const DevCfg& c, const DenseArgs& a, in
 template <bool MASKED, bool WITH_SG, int SC>
 __device__ __forceinline__ void pair_eval(PhaseFD& ph, const float (&cf)[4][4], u64& s2, const ulonglong2*& rec, int j,
                                           int jlo, int jhi, u64 h2, u64 K2, u64& zr2, u64& zi2, u64& sg2) {
-  const int n0 = __double2loint(ph.phi + 1572864.0);
-  ph.phi += ph.d1; ph.d1 += ph.d2; ph.d2 += ph.d3;
-  const int n1 = __double2loint(ph.phi + 1572864.0);
-  ph.phi += ph.d1; ph.d1 += ph.d2; ph.d2 += ph.d3;
+  int n0, n1;
+  phase_next_pair(ph, n0, n1);
   float c0, c1, s0, s1;
   if (SC == 2) {
     float x0, x1;
@@ -641,6 +653,56 @@ __device__ __forceinline__ double sigma_moments(const float (&cf)[4][4], const u
   return (double)l + (double)h;
 }
 
+// sin, cos of the phase at the next two bins as packed halves; advances the phase by two bins.
+template <int SC>
+__device__ __forceinline__ void sincos_pair(PhaseFD& ph, u64 K2, u64& cr2, u64& sr2) {
+  int n0, n1;
+  phase_next_pair(ph, n0, n1);
+  float c0, c1, s0, s1;
+  if (SC == 2) {
+    float x0, x1;
+    f2unpack(f2mul(f2pack((float)n0, (float)n1), K2), x0, x1);
+    c0 = __cosf(x0); s0 = __sinf(x0); c1 = __cosf(x1); s1 = __sinf(x1);
+  } else {
+    sincos_frac32(n0, s0, c0);
+    sincos_frac32(n1, s1, c1);
+  }
+  cr2 = f2pack(c0, c1); sr2 = f2pack(s0, s1);
+}
+// amplitude cubics at (s_j, s_{j+1}), q = W_A conj(c_A) + W_E conj(c_E), z += q e^{+2 pi i Phi}
+__device__ __forceinline__ void mac_pair(const float (&cf)[4][4], u64& s2, const ulonglong2 wA, const ulonglong2 wE, u64 h2,
+                                         u64 cr2, u64 sr2, u64& zr2, u64& zi2) {
+  const u64 Ar = f2fma(f2fma(f2fma(f2bcast(cf[0][3]), s2, f2bcast(cf[0][2])), s2, f2bcast(cf[0][1])), s2, f2bcast(cf[0][0]));
+  const u64 Ai = f2fma(f2fma(f2fma(f2bcast(cf[1][3]), s2, f2bcast(cf[1][2])), s2, f2bcast(cf[1][1])), s2, f2bcast(cf[1][0]));
+  const u64 Er = f2fma(f2fma(f2fma(f2bcast(cf[2][3]), s2, f2bcast(cf[2][2])), s2, f2bcast(cf[2][1])), s2, f2bcast(cf[2][0]));
+  const u64 Ei = f2fma(f2fma(f2fma(f2bcast(cf[3][3]), s2, f2bcast(cf[3][2])), s2, f2bcast(cf[3][1])), s2, f2bcast(cf[3][0]));
+  s2 = f2add(s2, h2);
+  const u64 qr = f2fma(wA.x, Ar, f2fma(wA.y, Ai, f2fma(wE.x, Er, f2mul(wE.y, Ei))));
+  const u64 qi = f2fma(wA.y, Ar, f2fma(f2neg(wA.x), Ai, f2fma(wE.y, Er, f2neg(f2mul(wE.x, Ei)))));
+  zr2 = f2fma(qr, cr2, f2fma(f2neg(qi), sr2, zr2));
+  zi2 = f2fma(qr, sr2, f2fma(qi, cr2, zi2));
+}
+// n >= 1 consecutive unmasked pairs, software-pipelined by hand: the sin/cos (FP64 step, conversion, MUFU) and the
+// shared-memory loads of pair i+1 are issued before the multiply-accumulate of pair i.
+template <int SC>
+__device__ __forceinline__ void pairs_fast(PhaseFD& ph, const float (&cf)[4][4], u64& s2, const ulonglong2*& rec, int n,
+                                           u64 h2, u64 K2, u64& zr2, u64& zi2) {
+  u64 cr, sr;
+  sincos_pair<SC>(ph, K2, cr, sr);
+  ulonglong2 wA = rec[0], wE = rec[1];
+#pragma unroll 1
+  for (int i = 1; i < n; ++i) {
+    u64 crn, srn;
+    sincos_pair<SC>(ph, K2, crn, srn);
+    rec += kPairRec;
+    const ulonglong2 wAn = rec[0], wEn = rec[1];
+    mac_pair(cf, s2, wA, wE, h2, cr, sr, zr2, zi2);
+    cr = crn; sr = srn; wA = wAn; wE = wEn;
+  }
+  rec += kPairRec;
+  mac_pair(cf, s2, wA, wE, h2, cr, sr, zr2, zi2);
+}
+
 template <bool SEG, int SC>
 __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2(DevCfg c, DenseArgs a, const ulonglong2* __restrict__ Dg) {
   constexpr int CH = kChunkF32;
@@ -696,7 +758,7 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2(DevCfg c, Den
     open_at_edge = true;
   };
 
-  PhaseFD fd = {0.0, 0.0, 0.0, 0.0};
+  PhaseFD fd = {};
   for (int ib = cs; ib < ce2; ib += Sf) {
     const int ie = min(ib + Sf, ce2);
     const bool lane_in = (ib >= jlo) && (ie <= jhi);
@@ -738,7 +800,7 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2(DevCfg c, Den
       const int jfull = ph & ~1;                               // full pairs end here; a straddling pair follows if ph is odd
       if (!all_out) {
         if (!live && jj < jfull) {
-          for (int t = jj; t < jfull; ++t) { fd.phi += fd.d1; fd.d1 += fd.d2; fd.d2 += fd.d3; }
+          for (int t = jj; t < jfull; t += 2) phase_skip_pair(fd);
           jj = jfull;
         }
         s2 = f2pack((float)(jj - ib) * hS, (float)(jj + 1 - ib) * hS);
@@ -747,7 +809,7 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2(DevCfg c, Den
           const bool split = (jj == jfull);                    // the pair (ph - 1, ph)
           const int e2 = split ? jj + 2 : min(jj + kFlushBins, jfull);
           u64 zr2 = 0, zi2 = 0, sg2 = 0;
-          if (use_mom) { for (; jj < e2; jj += 2) pair(jj, F_{}, F_{}, zr2, zi2, sg2); }
+          if (use_mom) { pairs_fast<SC>(fd, cf, s2, rec, (e2 - jj) >> 1, h2, K2, zr2, zi2); jj = e2; }
           else         { for (; jj < e2; jj += 2) pair(jj, T_{}, T_{}, zr2, zi2, sg2); }
           float zrl, zrh, zil, zih, sgl, sgh;
           f2unpack(zr2, zrl, zrh); f2unpack(zi2, zil, zih); f2unpack(sg2, sgl, sgh);
@@ -913,7 +975,7 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2_ad(DevCfg c, 
     t_next = (k < k1) ? seg_target(C, k + 1, N) - cb0 : INFINITY;
   };
 
-  PhaseFD ph = {0.0, 0.0, 0.0, 0.0};
+  PhaseFD ph = {};
   for (int ib = cs; ib < ce2; ib += Sf) {
     const int ie = min(ib + Sf, ce2);
     const bool lane_in = (ib >= jlo) && (ie <= jhi);
@@ -934,8 +996,8 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2_ad(DevCfg c, 
       const bool cross = (k < k1) && (crel + sg_m * 1.0001 >= t_next);
       const bool slow = !all_in || __any_sync(0xffffffffu, cross);
       if (!slow) {
-        u64 zr2 = 0, zi2 = 0, sg2 = 0;
-        for (int jj = gs; jj < ge; jj += 2) pair_eval<false, false, SC>(ph, cf, s2, rec, jj, jlo, jhi, h2, K2, zr2, zi2, sg2);
+        u64 zr2 = 0, zi2 = 0;
+        pairs_fast<SC>(ph, cf, s2, rec, (ge - gs) >> 1, h2, K2, zr2, zi2);
         float zrl, zrh, zil, zih;
         f2unpack(zr2, zrl, zrh); f2unpack(zi2, zil, zih);
         Zr += (double)(zrl + zrh); Zi += (double)(zil + zih);
