@@ -477,3 +477,96 @@ void sco_pso_step(double* pos, double* vel, double* pbest_pos, double* pbest_val
     }
   }
 }
+
+
+/* ------------------------------------------------------------------------------------------------
+ * Multi-swarm bookkeeping of the hierarchical search (readings Q19-Q21 of DESIGN.md).
+ * ------------------------------------------------------------------------------------------------ */
+
+/* O7 with swarm membership given by a label per particle (after k-means regrouping the members of a swarm are no
+ * longer contiguous).  A swarm without members gets gbest_val = -inf and keeps its gbest_pos. */
+void sco_pso_step_labeled(double* pos, double* vel, double* pbest_pos, double* pbest_val, const double* stat,
+                          double* gbest_pos, double* gbest_val, const int32_t* label, const double* lo, const double* hi,
+                          const double* eps_min, double omega, double phi_p, double phi_g, uint64_t seed, uint64_t iter,
+                          int64_t P, int32_t n_swarms) {
+  for (int64_t p = 0; p < P; ++p)
+    if (stat[p] > pbest_val[p]) {
+      pbest_val[p] = stat[p];
+      for (int m = 0; m < 8; ++m) pbest_pos[8 * p + m] = pos[8 * p + m];
+    }
+  for (int32_t s = 0; s < n_swarms; ++s) {
+    int64_t best = -1;
+    for (int64_t p = 0; p < P; ++p)
+      if (label[p] == s && (best < 0 || pbest_val[p] > pbest_val[best])) best = p;
+    if (best < 0) { gbest_val[s] = -INFINITY; continue; }
+    gbest_val[s] = pbest_val[best];
+    for (int m = 0; m < 8; ++m) gbest_pos[8 * s + m] = pbest_pos[8 * best + m];
+  }
+  for (int64_t p = 0; p < P; ++p) {
+    const int32_t s = label[p];
+    double rP[8], rG[8];
+    sco_pso_uniforms(seed, (uint64_t)p, iter, rP, rG);
+    for (int m = 0; m < 8; ++m) {
+      const double th = pos[8 * p + m];
+      const double u = omega * vel[8 * p + m] + phi_p * rP[m] * (pbest_pos[8 * p + m] - th)
+                       + phi_g * rG[m] * (gbest_pos[8 * s + m] - th);                         /* Eq. 14 */
+      const double au = fabs(u), eps = eps_min[m];
+      double v;
+      if (au > 0.0) v = (eps > au ? eps : au) * (u / au);                                     /* Eq. 15 */
+      else v = (eps > 0.0) ? eps : 0.0;
+      double x = th + v;                                                                      /* Eq. 13 */
+      if (x < lo[m]) { x = lo[m]; v = -v; }
+      else if (x > hi[m]) { x = hi[m]; v = -v; }
+      pos[8 * p + m] = x;
+      vel[8 * p + m] = v;
+    }
+  }
+}
+
+/* k-means (Lloyd's algorithm) on the particle positions, in coordinates scaled by the prior box:
+ * y_m = (theta_m - lo_m)/(hi_m - lo_m) for the dimensions with hi_m > lo_m, others ignored (Q19).
+ * cent [K][8] in: initial centroids (theta units), out: final.  Each iteration: (a) label[p] = arg min_k |y_p - y_k|^2,
+ * lowest k on ties; (b) centroid_k = mean of its members (sums in particle order), a cluster without members keeps its
+ * centroid.  Stops when no label changes or after max_iter iterations; returns the number of iterations run.
+ * count [K] (may be NULL) = members per cluster. */
+int32_t sco_kmeans(const double* pos, int64_t P, const double* lo, const double* hi, double* cent, int32_t K,
+                   int32_t max_iter, int32_t* label, int64_t* count) {
+  double w[8];
+  for (int m = 0; m < 8; ++m) w[m] = (hi[m] > lo[m]) ? 1.0 / (hi[m] - lo[m]) : 0.0;
+  for (int64_t p = 0; p < P; ++p) label[p] = -1;
+  int32_t it = 0;
+  double* sum = (double*)malloc((size_t)K * 8 * sizeof(double));
+  int64_t* cnt = (int64_t*)malloc((size_t)K * sizeof(int64_t));
+  while (it < max_iter) {
+    ++it;
+    int64_t changed = 0;
+    for (int64_t p = 0; p < P; ++p) {
+      int32_t bk = 0; double bd = INFINITY;
+      for (int32_t k = 0; k < K; ++k) {
+        double d = 0.0;
+        for (int m = 0; m < 8; ++m) { const double t = (pos[8 * p + m] - cent[8 * k + m]) * w[m]; d += t * t; }
+        if (d < bd) { bd = d; bk = k; }
+      }
+      if (label[p] != bk) { label[p] = bk; ++changed; }
+    }
+    for (int32_t k = 0; k < K; ++k) { cnt[k] = 0; for (int m = 0; m < 8; ++m) sum[8 * k + m] = 0.0; }
+    for (int64_t p = 0; p < P; ++p) {
+      const int32_t k = label[p];
+      ++cnt[k];
+      for (int m = 0; m < 8; ++m) sum[8 * k + m] += pos[8 * p + m];
+    }
+    for (int32_t k = 0; k < K; ++k)
+      if (cnt[k] > 0) for (int m = 0; m < 8; ++m) cent[8 * k + m] = sum[8 * k + m] / (double)cnt[k];
+    if (changed == 0) break;
+  }
+  if (count) for (int32_t k = 0; k < K; ++k) count[k] = cnt[k];
+  free(sum); free(cnt);
+  return it;
+}
+
+/* App. B: a swarm has converged when the best value in its history has not improved by more than delta
+ * over the last `window` iterations.  hist [n_iter] = best-so-far after each iteration of the rung. */
+int32_t sco_converged(const double* hist, int64_t n_iter, int32_t window, double delta) {
+  if (n_iter <= window) return 0;
+  return (hist[n_iter - 1] - hist[n_iter - 1 - window] <= delta) ? 1 : 0;
+}

@@ -27,6 +27,12 @@
  *                          white PSD -> equal-duration segments.
  *   sco_philox4x32_10    : known-answer vectors of the published algorithm (Salmon et al. 2011), moments.
  *   sco_pso_step         : hand-computed one-particle examples of Eq. 14 -> 15 -> 13.
+ *   sco_pso_step_labeled : equals sco_pso_step when the labels are the contiguous blocks; invariant under a permutation
+ *                          of the particles that carries the labels along (uniforms are keyed by the particle index).
+ *   sco_kmeans           : well-separated blobs recover the generating partition; fixed point (nearest-centroid labels,
+ *                          centroids = member means); within-cluster sum of squares never increases; a hand-computed
+ *                          1-D example; scikit-learn's Lloyd KMeans from the same initial centroids gives the same labels.
+ *   sco_converged        : the rule of PAPER.md:508 on hand-written histories.
  */
 #ifndef SC_ORACLE_H
 #define SC_ORACLE_H
@@ -112,6 +118,17 @@ void sco_pso_step(double* pos, double* vel, double* pbest_pos, double* pbest_val
                   double* gbest_pos, double* gbest_val, const double* lo, const double* hi, const double* eps_min,
                   double omega, double phi_p, double phi_g, uint64_t seed, uint64_t iter,
                   int64_t n_particles, int32_t n_swarms);
+
+/* O7 with a swarm label per particle (members need not be contiguous; PAPER.md:199 regrouping). */
+void sco_pso_step_labeled(double* pos, double* vel, double* pbest_pos, double* pbest_val, const double* stat,
+                          double* gbest_pos, double* gbest_val, const int32_t* label, const double* lo, const double* hi,
+                          const double* eps_min, double omega, double phi_p, double phi_g, uint64_t seed, uint64_t iter,
+                          int64_t n_particles, int32_t n_swarms);
+/* Lloyd's k-means on the particle positions in prior-box units (Q19); returns the iterations run. */
+int32_t sco_kmeans(const double* pos, int64_t n_particles, const double* lo, const double* hi, double* cent, int32_t K,
+                   int32_t max_iter, int32_t* label, int64_t* count);
+/* convergence rule "best does not improve by more than delta in `window` iterations". */
+int32_t sco_converged(const double* hist, int64_t n_iter, int32_t window, double delta);
 
 #ifdef __cplusplus
 }

@@ -80,6 +80,13 @@ def lib():
         L.sco_pso_uniforms.argtypes = [C.c_uint64, C.c_uint64, C.c_uint64, _dp, _dp]
         L.sco_pso_step.argtypes = [_dp, _dp, _dp, _dp, _dp, _dp, _dp, _dp, _dp, _dp,
                                    C.c_double, C.c_double, C.c_double, C.c_uint64, C.c_uint64, C.c_int64, C.c_int32]
+        _i32p = C.POINTER(C.c_int32)
+        L.sco_pso_step_labeled.argtypes = [_dp, _dp, _dp, _dp, _dp, _dp, _dp, _i32p, _dp, _dp, _dp,
+                                           C.c_double, C.c_double, C.c_double, C.c_uint64, C.c_uint64, C.c_int64, C.c_int32]
+        L.sco_kmeans.restype = C.c_int32
+        L.sco_kmeans.argtypes = [_dp, C.c_int64, _dp, _dp, _dp, C.c_int32, C.c_int32, _i32p, _ip]
+        L.sco_converged.restype = C.c_int32
+        L.sco_converged.argtypes = [_dp, C.c_int64, C.c_int32, C.c_double]
     return _lib
 
 
@@ -257,3 +264,34 @@ def pso_step(pos, vel, pbest_pos, pbest_val, stat, gbest_pos, gbest_val, lo, hi,
     lib().sco_pso_step(_d(pos), _d(vel), _d(pbest_pos), _d(pbest_val), _d(st), _d(gbest_pos), _d(gbest_val),
                        _d(lo), _d(hi), _d(ep), float(omega), float(phi_p), float(phi_g), int(seed), int(it),
                        P, int(n_swarms))
+
+
+def pso_step_labeled(pos, vel, pbest_pos, pbest_val, stat, gbest_pos, gbest_val, label, lo, hi, eps_min,
+                     omega, phi_p, phi_g, seed, it):
+    """As pso_step with an int32 swarm label per particle (in place)."""
+    for a in (pos, vel, pbest_pos, pbest_val, gbest_pos, gbest_val):
+        assert a.dtype == np.float64 and a.flags.c_contiguous
+    lab = np.ascontiguousarray(label, dtype=np.int32)
+    P, S = pos.shape[0], gbest_val.shape[0]
+    st, lo, hi, ep = _f64(stat), _f64(lo), _f64(hi), _f64(eps_min)
+    lib().sco_pso_step_labeled(_d(pos), _d(vel), _d(pbest_pos), _d(pbest_val), _d(st), _d(gbest_pos), _d(gbest_val),
+                               lab.ctypes.data_as(C.POINTER(C.c_int32)), _d(lo), _d(hi), _d(ep), float(omega),
+                               float(phi_p), float(phi_g), int(seed), int(it), P, S)
+
+
+def kmeans(pos, lo, hi, cent, max_iter=100):
+    """Lloyd's k-means in prior-box units -> (labels int32 [P], centroids [K,8], counts int64 [K], iterations)."""
+    pos = _f64(pos).reshape(-1, 8)
+    cent = np.array(cent, dtype=np.float64, order="C").reshape(-1, 8).copy()
+    lo, hi = _f64(lo), _f64(hi)
+    P, K = pos.shape[0], cent.shape[0]
+    lab = np.zeros(P, dtype=np.int32)
+    cnt = np.zeros(K, dtype=np.int64)
+    it = lib().sco_kmeans(_d(pos), P, _d(lo), _d(hi), _d(cent), K, int(max_iter),
+                          lab.ctypes.data_as(C.POINTER(C.c_int32)), cnt.ctypes.data_as(_ip))
+    return lab, cent, cnt, int(it)
+
+
+def converged(hist, window, delta):
+    h = _f64(hist)
+    return bool(lib().sco_converged(_d(h), len(h), int(window), float(delta)))
