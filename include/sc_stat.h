@@ -157,6 +157,54 @@ int sc_pso_step(sc_handle* h, double* pos, double* vel, double* pbest_pos, doubl
                 double omega, double phi_p, double phi_g, uint64_t seed, uint64_t iter,
                 int64_t n_particles, int32_t n_swarms, void* cuda_stream);
 
+/* a7 with swarm membership given by a label per particle (after the k-means regrouping of PAPER.md:199 the members of
+ * a swarm are not contiguous).  label: DEVICE int32 [n_particles], values in [0, n_swarms).  A swarm without members
+ * gets gbest_val = -inf and keeps its gbest_pos.  Otherwise exactly sc_pso_step. */
+int sc_pso_step_labeled(sc_handle* h, double* pos, double* vel, double* pbest_pos, double* pbest_val,
+                        const double* stat, double* gbest_pos, double* gbest_val, const int32_t* label,
+                        const double* lo, const double* hi, const double* eps_min,
+                        double omega, double phi_p, double phi_g, uint64_t seed, uint64_t iter,
+                        int64_t n_particles, int32_t n_swarms, void* cuda_stream);
+
+/* Multi-swarm regrouping: Lloyd's k-means on all particle positions in prior-box units,
+ * y_m = (theta_m - lo_m)/(hi_m - lo_m) over the dimensions with hi_m > lo_m (reading Q19).  Per iteration:
+ * label[p] = arg min_k |y_p - y_k|^2 (lowest k on ties); centroid_k = mean of its members (a cluster without members keeps
+ * its centroid).  Stops when no label changes or after max_iter iterations (one stream synchronisation per iteration).
+ * pos: DEVICE [n_particles][8]; lo, hi: DEVICE [8]; cent: DEVICE [K][8], in = initial centroids, out = final; K <= 128;
+ * label: DEVICE int32 [n_particles] (out); count: DEVICE int64 [K] or NULL (out); n_iter: HOST or NULL (out). */
+int sc_kmeans(sc_handle* h, const double* pos, int64_t n_particles, const double* lo, const double* hi,
+              double* cent, int32_t K, int32_t max_iter, int32_t* label, int64_t* count, int32_t* n_iter,
+              void* cuda_stream);
+
+/* The search of one tile (Fig. 2; Sec. III A-B; App. B). */
+#define SC_MAX_RUNGS 8
+typedef struct {
+  int32_t n_rungs;                      /* ladder length, <= SC_MAX_RUNGS                                             */
+  int32_t n_seg[SC_MAX_RUNGS];          /* the ladder, e.g. {100, 50, 10, 1}                            */
+  double  omega[SC_MAX_RUNGS], phi_p[SC_MAX_RUNGS], phi_g[SC_MAX_RUNGS];   /* Table IV per rung     */
+  double  eps_min[SC_MAX_RUNGS][8];     /* minimum velocities per rung, in the order of the parameter row              */
+  int32_t adaptive_edges;               /* 1 = per-particle equal-SNR^2 segments, 0 = equal-width edges */
+  int32_t conv_window;                  /* 50                                                          */
+  double  conv_delta;                   /* 2.0                                                          */
+  int32_t max_iters_per_rung;           /* hard cap (the paper states none)                                            */
+  int32_t kmeans_max_iters;             /* Lloyd iterations cap; 0 = no regrouping between rungs                       */
+  double  threshold;                    /* 100: swarms whose final best reaches it are flagged (Fig. 2)  */
+  uint64_t seed;                        /* PSO uniforms: Philox key; the iteration counter runs on across rungs        */
+} sc_search_config;
+/* For every rung N: { Upsilon_N(pos) for all particles; sc_pso_step_labeled } until every non-empty swarm satisfies
+ * "best has not improved by more than conv_delta over conv_window iterations" (or max_iters_per_rung); personal bests
+ * start afresh on every rung (the objective changes, reading Q21); between rungs sc_kmeans regroups all particles from
+ * the swarm bests as initial centroids (the particle count is conserved; the number of swarm slots is fixed, reading Q20).
+ * pos, vel: DEVICE [n_particles][8], in = initial state, out = final.  label: DEVICE int32 [n_particles], in = initial
+ * swarm of each particle, out = final.  lo, hi: DEVICE [8].  Outputs (HOST; all but best_* may be NULL):
+ * best_pos [n_swarms][8], best_val [n_swarms] = swarm bests on the last rung; n_members [n_swarms]; passed [n_swarms] =
+ * best_val >= threshold; iters_per_rung [n_rungs]; hist [n_rungs][n_swarms][max_iters_per_rung] = best after every
+ * iteration (0 beyond the iterations run).  Synchronises the stream every iteration (S doubles read back). */
+int sc_search_run(sc_handle* h, const sc_search_config* cfg, double* pos, double* vel, int32_t* label,
+                  int64_t n_particles, int32_t n_swarms, const double* lo, const double* hi,
+                  double* best_pos, double* best_val, int64_t* n_members, int32_t* passed, int32_t* iters_per_rung,
+                  double* hist, void* cuda_stream);
+
 /* Counters of the last sc_eval_stat / sc_eval_segments call (synchronises the stream):
  *  evaluated_bins = sum_p |{j in window_p} intersect [e_0, e_N)|  (the "evaluated (particle x bin)" of the metric),
  *  kernel_launches = CUDA kernels launched by the library since the handle was created. */

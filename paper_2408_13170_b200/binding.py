@@ -15,7 +15,7 @@ SC_OPT_PRECISION, SC_OPT_F32_MIN_SEG, SC_OPT_SCRATCH_BYTES, SC_OPT_TC_MAX_S, SC_
 SC_TIMING_CLASSES = ["nodes", "dense", "stitch", "pso", "other"]
 
 EXPORTED_SYMBOLS = ["sc_init_data", "sc_init_data_host", "sc_eval_stat", "sc_eval_stat_host", "sc_eval_segments",
-                    "sc_eval_stat_adaptive", "sc_eval_components", "sc_eval_loglike", "sc_data_norm", "sc_gen_template", "sc_pso_step", "sc_get_counters", "sc_get_timing", "sc_measure_fp64_peak",
+                    "sc_eval_stat_adaptive", "sc_eval_components", "sc_eval_loglike", "sc_data_norm", "sc_gen_template", "sc_pso_step", "sc_pso_step_labeled", "sc_kmeans", "sc_search_run", "sc_get_counters", "sc_get_timing", "sc_measure_fp64_peak",
                     "sc_set_option", "sc_free",
                     "sc_last_error", "sc_version"]
 
@@ -39,6 +39,35 @@ class ScConfig(C.Structure):
         c = cls()
         for k, _ in cls._fields_:
             setattr(c, k, d[k])
+        return c
+
+
+SC_MAX_RUNGS = 8
+
+
+class ScSearchConfig(C.Structure):
+    """sc_search_config of include/sc_stat.h."""
+    _fields_ = [("n_rungs", C.c_int32), ("n_seg", C.c_int32 * SC_MAX_RUNGS),
+                ("omega", C.c_double * SC_MAX_RUNGS), ("phi_p", C.c_double * SC_MAX_RUNGS), ("phi_g", C.c_double * SC_MAX_RUNGS),
+                ("eps_min", (C.c_double * 8) * SC_MAX_RUNGS),
+                ("adaptive_edges", C.c_int32), ("conv_window", C.c_int32), ("conv_delta", C.c_double),
+                ("max_iters_per_rung", C.c_int32), ("kmeans_max_iters", C.c_int32), ("threshold", C.c_double),
+                ("seed", C.c_uint64)]
+
+    @classmethod
+    def make(cls, ladder, hyper, adaptive_edges=True, conv_window=50, conv_delta=2.0, max_iters_per_rung=1000,
+             kmeans_max_iters=100, threshold=100.0, seed=0):
+        """ladder: segment counts per rung; hyper: per rung a dict with omega, phi_p, phi_g, eps (8 values)."""
+        c = cls()
+        c.n_rungs = len(ladder)
+        for r, (N, hp) in enumerate(zip(ladder, hyper)):
+            c.n_seg[r] = int(N)
+            c.omega[r], c.phi_p[r], c.phi_g[r] = float(hp["omega"]), float(hp["phi_p"]), float(hp["phi_g"])
+            for m in range(8):
+                c.eps_min[r][m] = float(hp["eps"][m])
+        c.adaptive_edges, c.conv_window, c.conv_delta = int(bool(adaptive_edges)), int(conv_window), float(conv_delta)
+        c.max_iters_per_rung, c.kmeans_max_iters = int(max_iters_per_rung), int(kmeans_max_iters)
+        c.threshold, c.seed = float(threshold), int(seed) & (2 ** 64 - 1)
         return c
 
 
@@ -81,6 +110,13 @@ def load_library():
     L.sc_gen_template.argtypes = [_vp, _vp, C.c_int64, _vp, _vp, _vp]
     L.sc_pso_step.restype = C.c_int
     L.sc_pso_step.argtypes = [_vp] + [_vp] * 10 + [C.c_double] * 3 + [C.c_uint64, C.c_uint64, C.c_int64, C.c_int32, _vp]
+    L.sc_pso_step_labeled.restype = C.c_int
+    L.sc_pso_step_labeled.argtypes = [_vp] + [_vp] * 11 + [C.c_double] * 3 + [C.c_uint64, C.c_uint64, C.c_int64, C.c_int32, _vp]
+    L.sc_kmeans.restype = C.c_int
+    L.sc_kmeans.argtypes = [_vp, _vp, C.c_int64, _vp, _vp, _vp, C.c_int32, C.c_int32, _vp, _vp, C.POINTER(C.c_int32), _vp]
+    L.sc_search_run.restype = C.c_int
+    L.sc_search_run.argtypes = [_vp, C.POINTER(ScSearchConfig), _vp, _vp, _vp, C.c_int64, C.c_int32, _vp, _vp,
+                                _vp, _vp, _vp, _vp, _vp, _vp, _vp]
     L.sc_get_counters.restype = C.c_int
     L.sc_get_counters.argtypes = [_vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64), _vp]
     L.sc_get_timing.restype = C.c_int
@@ -312,6 +348,57 @@ def sc_pso_step(h, pos, vel, pbest_pos, pbest_val, stat, gbest_pos, gbest_val, l
     _check(rc, h)
 
 
+def sc_pso_step_labeled(h, pos, vel, pbest_pos, pbest_val, stat, gbest_pos, gbest_val, label, lo, hi, eps_min,
+                        omega, phi_p, phi_g, seed, iter, n_particles, n_swarms, stream=None):
+    torch = _torch()
+    names = ["pos", "vel", "pbest_pos", "pbest_val", "stat", "gbest_pos", "gbest_val", "lo", "hi", "eps_min"]
+    tens = [pos, vel, pbest_pos, pbest_val, stat, gbest_pos, gbest_val, lo, hi, eps_min]
+    sizes = [8 * n_particles] * 3 + [n_particles] * 2 + [8 * n_swarms, n_swarms, 8, 8, 8]
+    for t, nm, sz in zip(tens, names, sizes):
+        if isinstance(t, torch.Tensor) and t.numel() != sz:
+            raise SCError(SC_ERR_INVALID_ARG, f"{nm}: expected {sz} values, got {t.numel()}")
+    if label.numel() != n_particles:
+        raise SCError(SC_ERR_INVALID_ARG, "label: expected n_particles int32 values")
+    ptrs = [_dev(t, torch.float64, nm) for t, nm in zip(tens, names)]
+    ptrs.insert(7, _dev(label, torch.int32, "label"))
+    rc = load_library().sc_pso_step_labeled(h, *ptrs, float(omega), float(phi_p), float(phi_g), int(seed) & (2 ** 64 - 1),
+                                            int(iter), int(n_particles), int(n_swarms), _stream(stream))
+    _check(rc, h)
+
+
+def sc_kmeans(h, pos, n_particles, lo, hi, cent, K, max_iter, label, count=None, stream=None):
+    """-> iterations run.  All tensors CUDA: pos [P,8], lo/hi [8], cent [K,8] (in/out) f64; label [P] int32; count [K] int64."""
+    torch = _torch()
+    if pos.numel() != 8 * n_particles or cent.numel() != 8 * K or label.numel() != n_particles:
+        raise SCError(SC_ERR_INVALID_ARG, "pos [P,8], cent [K,8], label [P] expected")
+    n_it = C.c_int32(0)
+    rc = load_library().sc_kmeans(h, _dev(pos, torch.float64, "pos"), n_particles, _dev(lo, torch.float64, "lo"),
+                                  _dev(hi, torch.float64, "hi"), _dev(cent, torch.float64, "cent"), K, max_iter,
+                                  _dev(label, torch.int32, "label"),
+                                  None if count is None else _dev(count, torch.int64, "count"), C.byref(n_it), _stream(stream))
+    _check(rc, h)
+    return n_it.value
+
+
+def sc_search_run(h, cfg, pos, vel, label, n_particles, n_swarms, lo, hi, stream=None):
+    """Runs the ladder on the device; pos, vel, label are updated in place.  Returns a dict of HOST numpy results."""
+    import numpy as np
+    torch = _torch()
+    if pos.numel() != 8 * n_particles or vel.numel() != 8 * n_particles or label.numel() != n_particles:
+        raise SCError(SC_ERR_INVALID_ARG, "pos, vel [P,8] and label [P] expected")
+    S, R, M = int(n_swarms), int(cfg.n_rungs), int(cfg.max_iters_per_rung)
+    best_pos, best_val = np.zeros((S, 8)), np.zeros(S)
+    n_members, passed = np.zeros(S, dtype=np.int64), np.zeros(S, dtype=np.int32)
+    iters, hist = np.zeros(max(R, 1), dtype=np.int32), np.zeros((max(R, 1), S, max(M, 1)))
+    p = lambda a: _vp(a.ctypes.data)
+    rc = load_library().sc_search_run(h, C.byref(cfg), _dev(pos, torch.float64, "pos"), _dev(vel, torch.float64, "vel"),
+                                      _dev(label, torch.int32, "label"), n_particles, S, _dev(lo, torch.float64, "lo"),
+                                      _dev(hi, torch.float64, "hi"), p(best_pos), p(best_val), p(n_members), p(passed),
+                                      p(iters), p(hist), _stream(stream))
+    _check(rc, h)
+    return dict(best_pos=best_pos, best_val=best_val, n_members=n_members, passed=passed, iters_per_rung=iters, hist=hist)
+
+
 def sc_get_counters(h, stream=None):
     """(evaluated_bins of the last eval, kernel launches since init); synchronises the stream."""
     a, b = C.c_int64(0), C.c_int64(0)
@@ -415,6 +502,23 @@ class Handle:
         sc_pso_step(self.h, state["pos"], state["vel"], state["pbest_pos"], state["pbest_val"], stat,
                     state["gbest_pos"], state["gbest_val"], lo, hi, eps_min, omega, phi_p, phi_g, seed, it,
                     state["pos"].shape[0], n_swarms, stream)
+
+    def pso_step_labeled(self, state, stat, label, lo, hi, eps_min, omega, phi_p, phi_g, seed, it, stream=None):
+        sc_pso_step_labeled(self.h, state["pos"], state["vel"], state["pbest_pos"], state["pbest_val"], stat,
+                            state["gbest_pos"], state["gbest_val"], label, lo, hi, eps_min, omega, phi_p, phi_g, seed, it,
+                            state["pos"].shape[0], state["gbest_val"].shape[0], stream)
+
+    def kmeans(self, pos, lo, hi, cent, max_iter=100, stream=None):
+        """-> (label int32 [P], count int64 [K], iterations); cent [K,8] is updated in place."""
+        torch = _torch()
+        P, K = pos.shape[0], cent.shape[0]
+        label = torch.empty(P, dtype=torch.int32, device=pos.device)
+        count = torch.empty(K, dtype=torch.int64, device=pos.device)
+        it = sc_kmeans(self.h, pos, P, lo, hi, cent, K, max_iter, label, count, stream)
+        return label, count, it
+
+    def search_run(self, cfg, pos, vel, label, n_swarms, lo, hi, stream=None):
+        return sc_search_run(self.h, cfg, pos, vel, label, pos.shape[0], n_swarms, lo, hi, stream)
 
     def counters(self, stream=None):
         return sc_get_counters(self.h, stream)

@@ -111,6 +111,11 @@ __global__ void k_loglike(const double* __restrict__ comp3, const double* __rest
   out[p] = -0.5 * dd - 0.5 * A * A * comp3[3 * (size_t)p + 2] + A * comp3[3 * (size_t)p + 1];
 }
 
+__global__ void k_fill(double* __restrict__ x, long long n, double v) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) x[i] = v;
+}
+
 // ------------------------------------------------------------------------------------------------ a1 + a3
 __global__ void k_particle_consts(DevCfg c, const double* __restrict__ params, int P, int P_pad,
                                   double* __restrict__ pc, int* __restrict__ jlo_out, int* __restrict__ jhi_out,
@@ -1157,17 +1162,20 @@ __global__ void k_template(DevCfg c, const int* __restrict__ node_n, const doubl
 }
 
 // ------------------------------------------------------------------------------------------------ a7 PSO
-// (1)+(2): one CTA per swarm.
+// (1)+(2): one CTA per swarm.  label == nullptr: swarm s = particles [s per_swarm, (s+1) per_swarm); else swarm s = the
+// particles with label[p] == s (n_scan = n_particles; a swarm without members gets gbest_val = -inf, gbest_pos untouched).
 __global__ void k_pso_best(const double* __restrict__ pos, double* __restrict__ pbest_pos, double* __restrict__ pbest_val,
                            const double* __restrict__ stat, double* __restrict__ gbest_pos, double* __restrict__ gbest_val,
-                           int per_swarm) {
+                           int per_swarm, const int* __restrict__ label, long long n_scan) {
   const int s = blockIdx.x;
-  const long long p0 = (long long)s * per_swarm;
+  const long long p0 = label ? 0 : (long long)s * per_swarm;
+  const long long n_t = label ? n_scan : per_swarm;
   double best = -INFINITY;
   long long besti = LLONG_MAX;
   bool any = false;
-  for (int t = threadIdx.x; t < per_swarm; t += blockDim.x) {
+  for (long long t = threadIdx.x; t < n_t; t += blockDim.x) {
     const long long p = p0 + t;
+    if (label && label[p] != s) continue;
     double pv = pbest_val[p];
     const double st = stat[p];
     if (st > pv) {
@@ -1208,10 +1216,14 @@ __global__ void k_pso_best(const double* __restrict__ pos, double* __restrict__ 
       const int oa = __shfl_xor_sync(0xffffffffu, (int)any, o);
       if (better(ov, oi, oa, best, besti, any)) { best = ov; besti = oi; any = oa; }
     }
-    if (l == 0) { si[0] = besti; }
+    if (l == 0) { si[0] = besti; sa[0] = any; }
   }
   __syncthreads();
   const long long bi = si[0];
+  if (!sa[0]) {                                  // no members (labelled swarms only)
+    if (threadIdx.x == 8) gbest_val[s] = -INFINITY;
+    return;
+  }
   if (threadIdx.x < 8) gbest_pos[s * 8 + threadIdx.x] = pbest_pos[bi * 8 + threadIdx.x];
   if (threadIdx.x == 8) gbest_val[s] = pbest_val[bi];
 }
@@ -1220,10 +1232,10 @@ __global__ void k_pso_best(const double* __restrict__ pos, double* __restrict__ 
 __global__ void k_pso_move(double* __restrict__ pos, double* __restrict__ vel, const double* __restrict__ pbest_pos,
                            const double* __restrict__ gbest_pos, const double* __restrict__ lo, const double* __restrict__ hi,
                            const double* __restrict__ eps_min, double omega, double phi_p, double phi_g,
-                           uint64_t seed, uint64_t iter, long long P, int per_swarm) {
+                           uint64_t seed, uint64_t iter, long long P, int per_swarm, const int* __restrict__ label) {
   const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= P) return;
-  const int s = (int)(p / per_swarm);
+  const int s = label ? label[p] : (int)(p / per_swarm);
   uint32_t w[16];
 #pragma unroll
   for (uint32_t b = 0; b < 4; ++b)
@@ -1247,6 +1259,41 @@ __global__ void k_pso_move(double* __restrict__ pos, double* __restrict__ vel, c
     pos[p * 8 + m] = x;
     vel[p * 8 + m] = v;
   }
+}
+
+// ------------------------------------------------------------------------------------------------ k-means regrouping
+// Lloyd's algorithm on the particle positions in prior-box units (reading Q19).  Same arithmetic order
+// as the definition: squared distance accumulated over the dimensions in order without contraction, lowest k on ties;
+// centroid sums in particle order (one thread per (cluster, dimension) walks all particles: K * 8 threads, a few MB of
+// L2-resident reads -- k-means runs once per rung of the ladder).
+__global__ void k_km_assign(const double* __restrict__ pos, long long P, const double* __restrict__ lo,
+                            const double* __restrict__ hi, const double* __restrict__ cent, int K, int* __restrict__ label,
+                            int* __restrict__ changed) {
+  extern __shared__ double sc_[];
+  const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= P) return;
+  double w[8], x[8];
+#pragma unroll
+  for (int m = 0; m < 8; ++m) { w[m] = (hi[m] > lo[m]) ? 1.0 / (hi[m] - lo[m]) : 0.0; x[m] = pos[p * 8 + m]; }
+  int bk = 0;
+  double bd = INFINITY;
+  for (int k = 0; k < K; ++k) {
+    double d = 0.0;
+#pragma unroll
+    for (int m = 0; m < 8; ++m) { const double t = __dmul_rn(__dsub_rn(x[m], cent[k * 8 + m]), w[m]); d = __dadd_rn(d, __dmul_rn(t, t)); }
+    if (d < bd) { bd = d; bk = k; }
+  }
+  if (label[p] != bk) { label[p] = bk; atomicAdd(changed, 1); }
+}
+__global__ void k_km_update(const double* __restrict__ pos, long long P, const int* __restrict__ label,
+                            double* __restrict__ cent, long long* __restrict__ count) {
+  const int k = blockIdx.x, m = threadIdx.x;
+  double sum = 0.0;
+  long long n = 0;
+  for (long long p = 0; p < P; ++p)
+    if (label[p] == k) { sum = __dadd_rn(sum, pos[p * 8 + m]); ++n; }
+  if (n > 0) cent[k * 8 + m] = sum / (double)n;
+  if (m == 0) count[k] = n;
 }
 
 // ------------------------------------------------------------------------------------------------ MUFU gain
@@ -1300,6 +1347,7 @@ struct sc_handle {
   double mufu_gain2 = 1.0;        // <cos^2 + sin^2> of the hardware sin/cos, measured at init
   double dd = 0.0;                // <d|d> (Eq. 1), computed at init
   double* d_comp = nullptr; size_t comp_cap = 0;   // components scratch of sc_eval_loglike
+  void* d_km = nullptr; size_t km_cap = 0;         // k-means: changed counter + member counts
   // adaptive (per-particle) segments: moments of the weights over groups and fine sub-intervals, cached per node spacing
   int ad_lg = 0; float2* d_gmom = nullptr; float2* d_smom = nullptr; size_t gmom_cap = 0, smom_cap = 0;
   // scratch
@@ -1880,6 +1928,107 @@ int sc_eval_stat_adaptive(sc_handle* h, const double* params, int64_t P, int32_t
   return run_adaptive(h, params, P, n_seg, out, out_edges, out3, st);
 }
 
+// ------------------------------------------------------------------------------------------------ hierarchical search
+// Fig. 2 / Sec. III of the paper (App. B): for every rung N of the ladder
+// { evaluate Upsilon_N for all particles -> PSO step (Eq. 13-15) per swarm } until every swarm has converged, then
+// k-means regrouping of all particles and the next rung; after the last rung swarms whose best reaches the threshold are
+// flagged.  The population never leaves the device; the host reads back one double per swarm and iteration (the bests,
+// for the convergence rule).
+int sc_search_run(sc_handle* h, const sc_search_config* sc, double* pos, double* vel, int32_t* label, int64_t P,
+                  int32_t n_swarms, const double* lo, const double* hi, double* best_pos, double* best_val,
+                  int64_t* n_members, int32_t* passed, int32_t* iters_per_rung, double* hist, void* stream) {
+  if (!h) return SC_ERR_NOT_INIT;
+  if (h->cuda_failed) return SC_ERR_CUDA;
+  if (!sc || !pos || !vel || !label || !lo || !hi || !best_pos || !best_val)
+    return fail(h, SC_ERR_INVALID_ARG, "null pointer");
+  if (P <= 0 || n_swarms <= 0 || n_swarms > 128) return fail(h, SC_ERR_INVALID_ARG, "need n_particles > 0 and 1 <= n_swarms <= 128");
+  if (sc->n_rungs < 1 || sc->n_rungs > SC_MAX_RUNGS) return fail(h, SC_ERR_INVALID_ARG, "n_rungs must be 1..%d", SC_MAX_RUNGS);
+  if (sc->conv_window < 1 || sc->max_iters_per_rung < 1 || sc->kmeans_max_iters < 0)
+    return fail(h, SC_ERR_INVALID_ARG, "conv_window, max_iters_per_rung must be >= 1 and kmeans_max_iters >= 0");
+  for (int r = 0; r < sc->n_rungs; ++r)
+    if (sc->n_seg[r] < 1 || sc->n_seg[r] > h->cfg.n_bins) return fail(h, SC_ERR_INVALID_ARG, "n_seg[%d] out of range", r);
+  cudaStream_t st = (cudaStream_t)stream;
+  const int S = n_swarms;
+  const int64_t nb = h->cfg.n_bins;
+  // device state owned by this call
+  double* buf = nullptr;
+  const size_t n_d = (size_t)P * 8 + (size_t)P * 2 + (size_t)S * 8 * 2 + (size_t)S + 8;
+  SC_CUDA(h, cudaMalloc(&buf, n_d * 8 + (size_t)S * 8));
+  double* pbest_pos = buf; double* pbest_val = pbest_pos + (size_t)P * 8; double* stat = pbest_val + P;
+  double* gbest_pos = stat + P; double* cent = gbest_pos + (size_t)S * 8; double* gbest_val = cent + (size_t)S * 8;
+  double* eps_d = gbest_val + S;
+  long long* cnt_d = (long long*)(eps_d + 8);
+  std::vector<double> gv((size_t)S), hst;
+  std::vector<int64_t> cnt((size_t)S, 0);
+  std::vector<int32_t> e;
+  int rc = SC_OK;
+  uint64_t iter_global = 0;
+  auto cleanup = [&](int code) { cudaFree(buf); return code; };
+#define SC_S(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cleanup(fail(h, SC_ERR_CUDA, "%s failed: %s", #call, cudaGetErrorString(e_))); } while (0)
+  SC_S(cudaMemsetAsync(gbest_pos, 0, (size_t)S * 8 * 8, st));
+
+  for (int r = 0; r < sc->n_rungs; ++r) {
+    const int N = sc->n_seg[r];
+    // the objective changes with N: personal bests start afresh on every rung (Q21)
+    k_fill<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(pbest_val, (long long)P, -INFINITY);
+    if ((rc = check_launch(h, "k_fill"))) return cleanup(rc);
+    SC_S(cudaMemcpyAsync(pbest_pos, pos, (size_t)P * 64, cudaMemcpyDeviceToDevice, st));
+    SC_S(cudaMemcpyAsync(eps_d, sc->eps_min[r], 64, cudaMemcpyHostToDevice, st));
+    if (!sc->adaptive_edges || N == 1) {
+      e.resize((size_t)N + 1);
+      for (int k = 0; k <= N; ++k) e[k] = (int32_t)(((long long)k * nb) / N);       // equal-width shared edges (Q2)
+    }
+    hst.assign((size_t)S * sc->max_iters_per_rung, 0.0);
+    int it = 0;
+    for (; it < sc->max_iters_per_rung; ++it) {
+      if (sc->adaptive_edges && N > 1) rc = sc_eval_stat_adaptive(h, pos, P, N, stat, nullptr, nullptr, stream);
+      else rc = eval_common(h, pos, P, e.data(), N, stat, nullptr, stream, false);
+      if (rc) return cleanup(rc);
+      rc = sc_pso_step_labeled(h, pos, vel, pbest_pos, pbest_val, stat, gbest_pos, gbest_val, label, lo, hi, eps_d,
+                               sc->omega[r], sc->phi_p[r], sc->phi_g[r], sc->seed, iter_global++, P, S, stream);
+      if (rc) return cleanup(rc);
+      SC_S(cudaMemcpyAsync(gv.data(), gbest_val, (size_t)S * 8, cudaMemcpyDeviceToHost, st));
+      SC_S(cudaStreamSynchronize(st));
+      bool all_conv = true;
+      for (int s = 0; s < S; ++s) {
+        hst[(size_t)s * sc->max_iters_per_rung + it] = gv[s];
+        if (gv[s] == -INFINITY) continue;                                   // empty swarm
+        // converged when the best has not improved by more than conv_delta over conv_window iterations
+        const bool conv = (it >= sc->conv_window) &&
+                          (gv[s] - hst[(size_t)s * sc->max_iters_per_rung + it - sc->conv_window] <= sc->conv_delta);
+        all_conv = all_conv && conv;
+      }
+      if (all_conv) { ++it; break; }
+    }
+    if (iters_per_rung) iters_per_rung[r] = it;
+    if (hist)
+      for (int s = 0; s < S; ++s)
+        memcpy(hist + ((size_t)r * S + s) * sc->max_iters_per_rung, hst.data() + (size_t)s * sc->max_iters_per_rung,
+               (size_t)sc->max_iters_per_rung * 8);
+    if (r + 1 < sc->n_rungs && sc->kmeans_max_iters > 0) {
+      // regroup all particles: k-means from the current swarm bests (Q19)
+      SC_S(cudaMemcpyAsync(cent, gbest_pos, (size_t)S * 64, cudaMemcpyDeviceToDevice, st));
+      int32_t n_it = 0;
+      if ((rc = sc_kmeans(h, pos, P, lo, hi, cent, S, sc->kmeans_max_iters, label, (int64_t*)cnt_d, &n_it, stream))) return cleanup(rc);
+    }
+  }
+  // results: the bests of the last rung
+  SC_S(cudaMemcpyAsync(best_val, gbest_val, (size_t)S * 8, cudaMemcpyDeviceToHost, st));
+  SC_S(cudaMemcpyAsync(best_pos, gbest_pos, (size_t)S * 64, cudaMemcpyDeviceToHost, st));
+  {
+    std::vector<int32_t> lab((size_t)P);
+    SC_S(cudaMemcpyAsync(lab.data(), label, (size_t)P * 4, cudaMemcpyDeviceToHost, st));
+    SC_S(cudaStreamSynchronize(st));
+    for (int64_t p = 0; p < P; ++p) if (lab[p] >= 0 && lab[p] < S) ++cnt[lab[p]];
+  }
+  for (int s = 0; s < S; ++s) {
+    if (n_members) n_members[s] = cnt[s];
+    if (passed) passed[s] = (cnt[s] > 0 && best_val[s] >= sc->threshold) ? 1 : 0;
+  }
+#undef SC_S
+  return cleanup(SC_OK);
+}
+
 int sc_eval_stat_host(sc_handle* h, const double* params, int64_t P, const int32_t* seg_edges, int32_t n_seg,
                       double* out, void* stream) {
   if (!h) return SC_ERR_NOT_INIT;
@@ -1949,11 +2098,63 @@ int sc_pso_step(sc_handle* h, double* pos, double* vel, double* pbest_pos, doubl
   const int per = (int)(P / n_swarms);
   int rc;
   Timed tm(h, st, SC_TIME_PSO);
-  k_pso_best<<<n_swarms, 1024, 0, st>>>(pos, pbest_pos, pbest_val, stat, gbest_pos, gbest_val, per);
+  k_pso_best<<<n_swarms, 1024, 0, st>>>(pos, pbest_pos, pbest_val, stat, gbest_pos, gbest_val, per, nullptr, 0);
   if ((rc = check_launch(h, "k_pso_best"))) return rc;
   k_pso_move<<<(unsigned)((P + 127) / 128), 128, 0, st>>>(pos, vel, pbest_pos, gbest_pos, lo, hi, eps_min, omega, phi_p, phi_g,
-                                                          seed, iter, P, per);
+                                                          seed, iter, P, per, nullptr);
   return check_launch(h, "k_pso_move");
+}
+
+int sc_pso_step_labeled(sc_handle* h, double* pos, double* vel, double* pbest_pos, double* pbest_val, const double* stat,
+                        double* gbest_pos, double* gbest_val, const int32_t* label, const double* lo, const double* hi,
+                        const double* eps_min, double omega, double phi_p, double phi_g, uint64_t seed, uint64_t iter,
+                        int64_t P, int32_t n_swarms, void* stream) {
+  if (!h) return SC_ERR_NOT_INIT;
+  if (h->cuda_failed) return SC_ERR_CUDA;
+  if (!pos || !vel || !pbest_pos || !pbest_val || !stat || !gbest_pos || !gbest_val || !label || !lo || !hi || !eps_min)
+    return fail(h, SC_ERR_INVALID_ARG, "null pointer");
+  if (P <= 0 || n_swarms <= 0) return fail(h, SC_ERR_INVALID_ARG, "n_particles and n_swarms must be positive");
+  cudaStream_t st = (cudaStream_t)stream;
+  int rc;
+  Timed tm(h, st, SC_TIME_PSO);
+  k_pso_best<<<n_swarms, 1024, 0, st>>>(pos, pbest_pos, pbest_val, stat, gbest_pos, gbest_val, 0, label, (long long)P);
+  if ((rc = check_launch(h, "k_pso_best"))) return rc;
+  k_pso_move<<<(unsigned)((P + 127) / 128), 128, 0, st>>>(pos, vel, pbest_pos, gbest_pos, lo, hi, eps_min, omega, phi_p, phi_g,
+                                                          seed, iter, P, 1, label);
+  return check_launch(h, "k_pso_move");
+}
+
+int sc_kmeans(sc_handle* h, const double* pos, int64_t P, const double* lo, const double* hi, double* cent, int32_t K,
+              int32_t max_iter, int32_t* label, int64_t* count, int32_t* n_iter, void* stream) {
+  if (!h) return SC_ERR_NOT_INIT;
+  if (h->cuda_failed) return SC_ERR_CUDA;
+  if (!pos || !lo || !hi || !cent || !label) return fail(h, SC_ERR_INVALID_ARG, "null pointer");
+  if (P <= 0 || K <= 0 || K > 128 || max_iter <= 0) return fail(h, SC_ERR_INVALID_ARG, "need n_particles > 0, 1 <= K <= 128, max_iter > 0");
+  cudaStream_t st = (cudaStream_t)stream;
+  int rc;
+  if ((rc = grow(h, (void**)&h->d_km, &h->km_cap, 16 + (size_t)K * 8))) return rc;
+  int* d_changed = (int*)h->d_km;
+  long long* d_cnt = (long long*)((char*)h->d_km + 16);
+  SC_CUDA(h, cudaMemsetAsync(label, 0xFF, (size_t)P * 4, st));       // -1: every particle counts as changed in iteration 1
+  int it = 0;
+  while (it < max_iter) {
+    ++it;
+    SC_CUDA(h, cudaMemsetAsync(d_changed, 0, 4, st));
+    {
+      Timed tm(h, st, SC_TIME_PSO);
+      k_km_assign<<<(unsigned)((P + 127) / 128), 128, 0, st>>>(pos, (long long)P, lo, hi, cent, K, label, d_changed);
+      if ((rc = check_launch(h, "k_km_assign"))) return rc;
+      k_km_update<<<K, 8, 0, st>>>(pos, (long long)P, label, cent, d_cnt);
+      if ((rc = check_launch(h, "k_km_update"))) return rc;
+    }
+    int changed = 0;
+    SC_CUDA(h, cudaMemcpyAsync(&changed, d_changed, 4, cudaMemcpyDeviceToHost, st));
+    SC_CUDA(h, cudaStreamSynchronize(st));
+    if (changed == 0) break;
+  }
+  if (count) SC_CUDA(h, cudaMemcpyAsync(count, d_cnt, (size_t)K * 8, cudaMemcpyDeviceToDevice, st));
+  if (n_iter) *n_iter = it;
+  return SC_OK;
 }
 
 int sc_get_counters(sc_handle* h, int64_t* evaluated_bins, int64_t* kernel_launches, void* stream) {
@@ -2050,7 +2251,7 @@ int sc_free(sc_handle* h) {
   if (!h) return SC_ERR_NOT_INIT;
   cudaFree(h->D32); cudaFree(h->W64); cudaFree(h->G64);
   cudaFree(h->scratch); cudaFree(h->d_edges); cudaFree(h->d_chunk_k0); cudaFree(h->d_flags);
-  cudaFree(h->d_counter); cudaFree(h->d_params_stage); cudaFree(h->d_comp); cudaFree(h->d_gmom); cudaFree(h->d_smom);
+  cudaFree(h->d_counter); cudaFree(h->d_params_stage); cudaFree(h->d_comp); cudaFree(h->d_km); cudaFree(h->d_gmom); cudaFree(h->d_smom);
   cudaFree(h->d_piece_first); cudaFree(h->d_piece_lo); cudaFree(h->d_piece_hi); cudaFree(h->d_moments);
   for (auto& e : h->evs) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
   cudaGetLastError();
