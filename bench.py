@@ -37,7 +37,7 @@ NOMINAL_DFMA = 148 * 64 * 1.965e9   # 148 SMs x 64 FP64 lanes x max SM clock (B2
 # 26 packed FFMA2/FMUL2/FADD2 (2 slots each) + 3 scalar per bin PAIR; peak = 148 SMs x 128 FP32 lanes x max SM clock.
 FP32_SLOTS_PER_BIN = (26 * 2 + 3) / 2.0
 NOMINAL_FP32_SLOTS = 148 * 128 * 1.965e9
-DENSE_PROFILE = os.path.join(ROOT, "profiles", "r01_k_dense2_full.md")
+DENSE_PROFILE = os.path.join(ROOT, "profiles", "r01c_k_dense2_full.md")
 
 
 def dram_traffic_from_profile():
@@ -64,6 +64,10 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--particles", type=int, default=None, help="override the population size (debug)")
+    ap.add_argument("--adaptive-nseg", type=int, default=0, metavar="N",
+                    help="time the step with per-particle equal-SNR^2 segments (sc_eval_stat_adaptive, PAPER.md:120) and N "
+                         "segments instead of the config's shared edges")
+    ap.add_argument("--no-extras", action="store_true", help="skip the extra (untimed-region) measurements")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--opt", action="append", default=[], metavar="ID=VALUE",
@@ -232,8 +236,15 @@ def run_ours(args, rank, local_rank, world):
     stat = torch.empty(P, dtype=torch.float64, device=dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > 126 MB L2
 
+    ad_N = args.adaptive_nseg
+    if ad_N:
+        N = ad_N
+
     def step(it):
-        H.eval_stat(state["pos"], e, out=stat)
+        if ad_N:
+            sc.sc_eval_stat_adaptive(H.h, state["pos"], P, ad_N, stat)
+        else:
+            H.eval_stat(state["pos"], e, out=stat)
         H.pso_step(state, stat, lo, hi, eps, hp["omega"], hp["phi_p"], hp["phi_g"], inp["pso_seed"], it, n_swarms)
 
     for it in range(args.warmup):
@@ -261,9 +272,26 @@ def run_ours(args, rank, local_rank, world):
     eval_bins, launches1 = H.counters()      # evaluated bins of the LAST eval (the swarm moves; representative)
     gpu_launches = launches1 - launches0
 
+    # ---- extras (outside the timed region): the paper's own segment definition at the first rung of its ladder
+    extras = {}
+    if not args.no_extras and not ad_N and rank == 0:
+        H.timing()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        for i in range(4):
+            if i == 1:
+                torch.cuda.synchronize(); H.timing(); a.record()
+            sc.sc_eval_stat_adaptive(H.h, state["pos"], P, 100, stat)
+        b.record()
+        torch.cuda.synchronize()
+        tma = H.timing()
+        extras["adaptive_segments_N100"] = {
+            "what": "sc_eval_stat_adaptive (per-particle equal-SNR^2 segments, PAPER.md:120), N = 100, same population",
+            "ms_per_eval": a.elapsed_time(b) / 3, "particle_bin_per_s": float(P) * nb / (a.elapsed_time(b) / 3 * 1e-3),
+            "kernel_ms_per_eval": {k: v[0] / 3 for k, v in tma.items() if v[1]}}
+
     # ---- e2e: the same step through the HOST-buffer entry point, copies inside the timed region
     e2e = None
-    if not args.no_e2e:
+    if not args.no_e2e and not ad_N:
         k2 = max(1, min(args.steps, 5))
         pos_h = torch.empty((P, 8), dtype=torch.float64).pin_memory()
         stat_h = torch.empty(P, dtype=torch.float64).pin_memory()
@@ -312,8 +340,8 @@ def run_ours(args, rank, local_rank, world):
         pbs = eval_bins / (dense_avg * 1e-3) if dense_avg > 0 else None
         roof = {"bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
                 "frac": (ach / peak) if ach else None, "traffic": dram_traffic_from_profile(),
-                "traffic_source": "profiles/r01_k_dense2_full.md (ncu --set full, one launch, same command)",
-                "kernel": "k_dense2<false,2>", "kernel_ms_per_launch": dense_avg,
+                "traffic_source": "profiles/r01c_k_dense2_full.md (ncu --set full, one launch, same command)",
+                "kernel": "k_dense2_ad<2>" if ad_N else "k_dense2<false,2>", "kernel_ms_per_launch": dense_avg,
                 "own_mix": {"what": "FP32 pipe of the kernel as built (packed FFMA2 loop): lane slots per evaluated "
                                     "particle-bin x evaluated particle-bins/s / (148 SM x 128 lanes x 1.965 GHz)",
                             "fp32_slots_per_bin": FP32_SLOTS_PER_BIN,
@@ -338,6 +366,10 @@ def run_ours(args, rank, local_rank, world):
                 "clocks": {"sm_mhz": clocks["sm_mhz"], "sm_max_mhz": clocks["sm_max_mhz"], "reasons": clocks["reasons"],
                            "samples": clocks["samples"]},
                 "roofline": roof, "gpu_launches": int(gpu_launches)}
+        if ad_N:
+            line["config"]["segments"] = f"per-particle equal-SNR^2 (PAPER.md:120), N = {ad_N}"
+        if extras:
+            line["extras"] = extras
         if e2e:
             line["e2e"] = {"value": world * float(P) * nb / (e2e_ms_max * 1e-3), "unit": UNIT,
                            "h2d_bytes_per_step": e2e["h2d"], "d2h_bytes_per_step": e2e["d2h"],
