@@ -289,6 +289,42 @@ def run_ours(args, rank, local_rank, world):
             "ms_per_eval": a.elapsed_time(b) / 3, "particle_bin_per_s": float(P) * nb / (a.elapsed_time(b) / 3 * 1e-3),
             "kernel_ms_per_eval": {k: v[0] / 3 for k, v in tma.items() if v[1]}}
 
+    # ---- extras: the second workload (Fig. 3): many data streams x one template, HBM-bound
+    if not args.no_extras and not ad_N and rank == 0:
+        D = 256
+        try:
+            Ws = torch.randn((D, nb, 4), dtype=torch.float32, device=dev)       # whitened noise-only streams, 16 B per bin
+            th = state["gbest_pos"][0].contiguous()
+            e100 = sy.edges(nb, 100).astype(np.int32)
+            outs = torch.empty(D, dtype=torch.float64, device=dev)
+            H.eval_stat_streams(th, Ws, e100, out=outs)
+            torch.cuda.synchronize(); H.timing()
+            reps = 5
+            for _ in range(reps):
+                flush.fill_(1)
+                H.eval_stat_streams(th, Ws, e100, out=outs)
+            torch.cuda.synchronize()
+            tms = H.timing()
+            z_ms = tms["dense"][0] / reps
+            peaks = {}
+            try:
+                peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+            except (OSError, ValueError):
+                pass
+            peak = float(peaks.get("hbm_gbs", 6650.0))
+            gbs = D * nb * 16.0 / (z_ms * 1e-3) / 1e9
+            extras["streams_x_one_template"] = {
+                "what": f"sc_eval_stat_streams: {D} FP32 streams x {nb} bins (c3 grid), N = 100, one template",
+                "kernel": "k_streams_z<float4,float>", "kernel_ms_per_launch": z_ms,
+                "ms_per_eval_all_kernels": sum(v[0] for v in tms.values()) / reps,
+                "stream_bin_per_s": D * nb / (z_ms * 1e-3),
+                "roofline": {"bound": "hbm", "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak,
+                             "traffic": None, "algorithmic_bytes_per_stream_bin": 16,
+                             "peak_source": "MEASURED_PEAKS.json hbm_gbs (of measured)" if peaks else "fallback 6650 GB/s (of fallback)"}}
+            del Ws
+        except (RuntimeError, sc.SCError) as ex:                                # e.g. not enough memory for the streams
+            extras["streams_x_one_template"] = {"skipped": str(ex)[:200]}
+
     # ---- e2e: the same step through the HOST-buffer entry point, copies inside the timed region
     e2e = None
     if not args.no_e2e and not ad_N:

@@ -205,6 +205,20 @@ int sc_search_run(sc_handle* h, const sc_search_config* cfg, double* pos, double
                   double* best_pos, double* best_val, int64_t* n_members, int32_t* passed, int32_t* iters_per_rung,
                   double* hist, void* cuda_stream);
 
+/* Second workload (the 5000 noise realisations of Fig. 3): MANY data streams that
+ * share the handle's PSD against ONE template.  The handle's own data stream is not used.
+ * sc_whiten_streams: dA_ri, dE_ri DEVICE FP64 [n_streams][n_bins][2] -> W DEVICE [n_streams][n_bins][4]
+ *   = (A re, A im, E re, E im) of d 4df/S (rescaled to O(1) like the handle's own copy), FP32 (out_f64 = 0) or FP64.
+ * sc_eval_stat_streams: out[d] = Upsilon_N(d_d, theta) (Eq. 10) for d = 0 .. n_streams-1 (<= 65535); theta: DEVICE [8];
+ *   W as written by sc_whiten_streams (w_is_f64 says which flavour); seg_edges as in sc_eval_stat; out: DEVICE
+ *   [n_streams].  The template and sigma_k are evaluated once in FP64; the per-stream sums run in the precision of W
+ *   (FP32 streams: use for n_seg >= 8, like the FP32-amplitude path; FP64 streams for fewer segments).
+ *   This path is HBM-bound: 16 (FP32) or 32 (FP64) bytes per stream and bin. */
+int sc_whiten_streams(sc_handle* h, const double* dA_ri, const double* dE_ri, int64_t n_streams, int32_t out_f64,
+                      void* W, void* cuda_stream);
+int sc_eval_stat_streams(sc_handle* h, const double* theta, const void* W, int32_t w_is_f64, int64_t n_streams,
+                         const int32_t* seg_edges, int32_t n_seg, double* out, void* cuda_stream);
+
 /* Counters of the last sc_eval_stat / sc_eval_segments call (synchronises the stream):
  *  evaluated_bins = sum_p |{j in window_p} intersect [e_0, e_N)|  (the "evaluated (particle x bin)" of the metric),
  *  kernel_launches = CUDA kernels launched by the library since the handle was created. */

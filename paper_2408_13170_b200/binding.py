@@ -15,7 +15,7 @@ SC_OPT_PRECISION, SC_OPT_F32_MIN_SEG, SC_OPT_SCRATCH_BYTES, SC_OPT_TC_MAX_S, SC_
 SC_TIMING_CLASSES = ["nodes", "dense", "stitch", "pso", "other"]
 
 EXPORTED_SYMBOLS = ["sc_init_data", "sc_init_data_host", "sc_eval_stat", "sc_eval_stat_host", "sc_eval_segments",
-                    "sc_eval_stat_adaptive", "sc_eval_components", "sc_eval_loglike", "sc_data_norm", "sc_gen_template", "sc_pso_step", "sc_pso_step_labeled", "sc_kmeans", "sc_search_run", "sc_get_counters", "sc_get_timing", "sc_measure_fp64_peak",
+                    "sc_eval_stat_adaptive", "sc_eval_components", "sc_eval_loglike", "sc_data_norm", "sc_gen_template", "sc_pso_step", "sc_pso_step_labeled", "sc_kmeans", "sc_search_run", "sc_whiten_streams", "sc_eval_stat_streams", "sc_get_counters", "sc_get_timing", "sc_measure_fp64_peak",
                     "sc_set_option", "sc_free",
                     "sc_last_error", "sc_version"]
 
@@ -117,6 +117,10 @@ def load_library():
     L.sc_search_run.restype = C.c_int
     L.sc_search_run.argtypes = [_vp, C.POINTER(ScSearchConfig), _vp, _vp, _vp, C.c_int64, C.c_int32, _vp, _vp,
                                 _vp, _vp, _vp, _vp, _vp, _vp, _vp]
+    L.sc_whiten_streams.restype = C.c_int
+    L.sc_whiten_streams.argtypes = [_vp, _vp, _vp, C.c_int64, C.c_int32, _vp, _vp]
+    L.sc_eval_stat_streams.restype = C.c_int
+    L.sc_eval_stat_streams.argtypes = [_vp, _vp, _vp, C.c_int32, C.c_int64, _vp, C.c_int32, _vp, _vp]
     L.sc_get_counters.restype = C.c_int
     L.sc_get_counters.argtypes = [_vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64), _vp]
     L.sc_get_timing.restype = C.c_int
@@ -399,6 +403,33 @@ def sc_search_run(h, cfg, pos, vel, label, n_particles, n_swarms, lo, hi, stream
     return dict(best_pos=best_pos, best_val=best_val, n_members=n_members, passed=passed, iters_per_rung=iters, hist=hist)
 
 
+def sc_whiten_streams(h, dA_ri, dE_ri, n_streams, W, stream=None):
+    """dA_ri, dE_ri: CUDA f64 [n_streams, n_bins, 2]; W: CUDA [n_streams, n_bins, 4] float32 or float64 (out)."""
+    torch = _torch()
+    if W.dtype not in (torch.float32, torch.float64):
+        raise SCError(SC_ERR_INVALID_ARG, "W must be float32 or float64")
+    if dA_ri.numel() != dE_ri.numel() or W.numel() != 2 * dA_ri.numel() or dA_ri.numel() % (2 * n_streams):
+        raise SCError(SC_ERR_INVALID_ARG, "expected dA_ri, dE_ri [n_streams, n_bins, 2] and W [n_streams, n_bins, 4]")
+    rc = load_library().sc_whiten_streams(h, _dev(dA_ri, torch.float64, "dA_ri"), _dev(dE_ri, torch.float64, "dE_ri"),
+                                          n_streams, int(W.dtype == torch.float64), _dev(W, W.dtype, "W"), _stream(stream))
+    _check(rc, h)
+    return W
+
+
+def sc_eval_stat_streams(h, theta, W, n_streams, seg_edges, n_seg, out, stream=None):
+    torch = _torch()
+    keep, ep, ns = _edges_arg(seg_edges)
+    if ns != n_seg:
+        raise SCError(SC_ERR_INVALID_ARG, f"seg_edges has {ns + 1} entries, expected n_seg + 1 = {n_seg + 1}")
+    if theta.numel() != 8 or out.numel() != n_streams or W.dtype not in (torch.float32, torch.float64) or W.numel() % (4 * n_streams):
+        raise SCError(SC_ERR_INVALID_ARG, "theta [8], W [n_streams, n_bins, 4] (float32/float64), out [n_streams] expected")
+    rc = load_library().sc_eval_stat_streams(h, _dev(theta, torch.float64, "theta"), _dev(W, W.dtype, "W"),
+                                             int(W.dtype == torch.float64), n_streams, ep, n_seg,
+                                             _dev(out, torch.float64, "out"), _stream(stream))
+    _check(rc, h)
+    return out
+
+
 def sc_get_counters(h, stream=None):
     """(evaluated_bins of the last eval, kernel launches since init); synchronises the stream."""
     a, b = C.c_int64(0), C.c_int64(0)
@@ -519,6 +550,21 @@ class Handle:
 
     def search_run(self, cfg, pos, vel, label, n_swarms, lo, hi, stream=None):
         return sc_search_run(self.h, cfg, pos, vel, label, pos.shape[0], n_swarms, lo, hi, stream)
+
+    def whiten_streams(self, dA, dE, f64=False, stream=None):
+        """dA, dE: CUDA complex128 [n_streams, n_bins] -> whitened W [n_streams, n_bins, 4] (float32 or float64)."""
+        torch = _torch()
+        D, n = dA.shape
+        W = torch.empty((D, n, 4), dtype=torch.float64 if f64 else torch.float32, device=dA.device)
+        return sc_whiten_streams(self.h, torch.view_as_real(dA).contiguous(), torch.view_as_real(dE).contiguous(), D, W, stream)
+
+    def eval_stat_streams(self, theta, W, seg_edges, out=None, stream=None):
+        """Upsilon_N of ONE template (theta [8]) against every stream of W -> [n_streams]."""
+        torch = _torch()
+        D = W.shape[0]
+        if out is None:
+            out = torch.empty(D, dtype=torch.float64, device=W.device)
+        return sc_eval_stat_streams(self.h, theta, W, D, seg_edges, len(seg_edges) - 1, out, stream)
 
     def counters(self, stream=None):
         return sc_get_counters(self.h, stream)

@@ -1296,6 +1296,106 @@ __global__ void k_km_update(const double* __restrict__ pos, long long P, const i
   if (m == 0) count[k] = n;
 }
 
+// ------------------------------------------------------------------------------------------------ many data streams x one template
+// Second workload (the 5000 noise realisations of Fig. 3): Upsilon_N of ONE template
+// against many data streams that share the PSD.  The template and its sigma_k are computed once; per stream and bin
+// the work is one 16-byte (FP32) or 32-byte (FP64) load and 8 multiply-adds, so this path is HBM-bound.
+//   W_d(j)  = d_d(j) 4df/S(j) / s0  (whitened streams, [stream][bin][(A re, A im, E re, E im)])
+//   z_k[d]  = sum_{j in segment k} W_d(j) . conj(h(j)),   sigma_k = sum_j (|h_A|^2 G_A + |h_E|^2 G_E),  Upsilon[d] = sum_k |z_k[d]|^2 / sigma_k
+// Segments are cut into pieces of <= kStreamPiece bins; one warp per (piece, stream), lanes stride over the bins
+// (coalesced), shuffle reduction, partial z in [piece][stream] order; k_streams_finish walks the pieces in order.
+constexpr int kStreamPiece = 1024;
+
+__global__ void k_whiten_streams_f32(const double* __restrict__ dA, const double* __restrict__ dE, const double2* __restrict__ G64,
+                                     double s0, long long n_bins, long long n_streams, float4* __restrict__ W) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n_bins * n_streams) return;
+  const double2 g = G64[i % n_bins];
+  W[i] = make_float4((float)(dA[2 * i] * g.x * s0), (float)(dA[2 * i + 1] * g.x * s0),
+                     (float)(dE[2 * i] * g.y * s0), (float)(dE[2 * i + 1] * g.y * s0));
+}
+__global__ void k_whiten_streams_f64(const double* __restrict__ dA, const double* __restrict__ dE, const double2* __restrict__ G64,
+                                     double s0, long long n_bins, long long n_streams, double4* __restrict__ W) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n_bins * n_streams) return;
+  const double2 g = G64[i % n_bins];
+  W[i] = make_double4(dA[2 * i] * g.x * s0, dA[2 * i + 1] * g.x * s0, dE[2 * i] * g.y * s0, dE[2 * i + 1] * g.y * s0);
+}
+// template of the streams path: (h_A re, im, h_E re, im) in FP64 and FP32, from the k_template output
+__global__ void k_streams_template(const double* __restrict__ hA, const double* __restrict__ hE, int n_bins,
+                                   double4* __restrict__ T64, float4* __restrict__ T32) {
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= n_bins) return;
+  const double4 t = make_double4(hA[2 * j], hA[2 * j + 1], hE[2 * j], hE[2 * j + 1]);
+  T64[j] = t;
+  T32[j] = make_float4((float)t.x, (float)t.y, (float)t.z, (float)t.w);
+}
+// sigma of every piece (template only): one warp per piece, fixed-order reduction
+__global__ void k_streams_sigma(const double4* __restrict__ T64, const double2* __restrict__ G64, const int* __restrict__ piece_lo,
+                                const int* __restrict__ piece_hi, int n_pieces, double* __restrict__ piece_sigma) {
+  const int piece = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  if (piece >= n_pieces) return;
+  const int lane = threadIdx.x & 31;
+  double acc = 0.0;
+  for (int j = piece_lo[piece] + lane; j < piece_hi[piece]; j += 32) {
+    const double4 t = T64[j]; const double2 g = G64[j];
+    acc += (t.x * t.x + t.y * t.y) * g.x + (t.z * t.z + t.w * t.w) * g.y;
+  }
+  for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+  if (lane == 0) piece_sigma[piece] = acc;
+}
+// streaming (evict-first) loads: every stream byte is read exactly once
+__device__ __forceinline__ float4 ld_stream(const float4* p) { return __ldcs(p); }
+__device__ __forceinline__ double4 ld_stream(const double4* p) {
+  const double2 a = __ldcs(reinterpret_cast<const double2*>(p)), b = __ldcs(reinterpret_cast<const double2*>(p) + 1);
+  return make_double4(a.x, a.y, b.x, b.y);
+}
+template <typename W4, typename R>
+__global__ void __launch_bounds__(256) k_streams_z(const W4* __restrict__ W, const W4* __restrict__ T, const int* __restrict__ piece_lo,
+                                                   const int* __restrict__ piece_hi, int n_pieces, long long n_bins, int n_streams,
+                                                   double2* __restrict__ zpart /* [n_pieces][n_streams] */) {
+  const int piece = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  if (piece >= n_pieces) return;
+  const int d = blockIdx.y;
+  const int lane = threadIdx.x & 31;
+  const W4* __restrict__ Wd = W + (size_t)d * n_bins;
+  const int lo = piece_lo[piece], hi = piece_hi[piece];
+  R zr0 = 0, zi0 = 0, zr1 = 0, zi1 = 0;
+  int j = lo + lane;
+  for (; j + 32 < hi; j += 64) {                      // two independent loads in flight per lane
+    const W4 w0 = ld_stream(Wd + j), w1 = ld_stream(Wd + j + 32);
+    const W4 t0 = T[j], t1 = T[j + 32];
+    zr0 += w0.x * t0.x + w0.y * t0.y + w0.z * t0.z + w0.w * t0.w;     // Re (w conj t)
+    zi0 += w0.y * t0.x - w0.x * t0.y + w0.w * t0.z - w0.z * t0.w;     // Im (w conj t)
+    zr1 += w1.x * t1.x + w1.y * t1.y + w1.z * t1.z + w1.w * t1.w;
+    zi1 += w1.y * t1.x - w1.x * t1.y + w1.w * t1.z - w1.z * t1.w;
+  }
+  if (j < hi) {
+    const W4 w0 = ld_stream(Wd + j); const W4 t0 = T[j];
+    zr0 += w0.x * t0.x + w0.y * t0.y + w0.z * t0.z + w0.w * t0.w;
+    zi0 += w0.y * t0.x - w0.x * t0.y + w0.w * t0.z - w0.z * t0.w;
+  }
+  double zr = (double)zr0 + (double)zr1, zi = (double)zi0 + (double)zi1;
+  for (int o = 16; o > 0; o >>= 1) { zr += __shfl_xor_sync(0xffffffffu, zr, o); zi += __shfl_xor_sync(0xffffffffu, zi, o); }
+  if (lane == 0) zpart[(size_t)piece * n_streams + d] = make_double2(zr, zi);
+}
+__global__ void k_streams_finish(const double2* __restrict__ zpart, const double* __restrict__ piece_sigma,
+                                 const int* __restrict__ piece_last /* 1 = last piece of its segment */, int n_pieces,
+                                 int n_streams, double* __restrict__ out) {
+  const int d = blockIdx.x * blockDim.x + threadIdx.x;
+  if (d >= n_streams) return;
+  double ups = 0.0, zr = 0.0, zi = 0.0, sg = 0.0;
+  for (int i = 0; i < n_pieces; ++i) {
+    const double2 z = zpart[(size_t)i * n_streams + d];
+    zr += z.x; zi += z.y; sg += piece_sigma[i];
+    if (piece_last[i]) {
+      if (sg > 0.0) ups += (zr * zr + zi * zi) / sg;
+      zr = 0.0; zi = 0.0; sg = 0.0;
+    }
+  }
+  out[d] = ups;
+}
+
 // ------------------------------------------------------------------------------------------------ MUFU gain
 // The hardware sin/cos (MUFU) used by the fast FP32 path has a small systematic gain: <cos^2 + sin^2> over uniformly
 // distributed angles is not exactly 1.  It is measured once per handle with the very instruction sequence of the
@@ -1348,6 +1448,10 @@ struct sc_handle {
   double dd = 0.0;                // <d|d> (Eq. 1), computed at init
   double* d_comp = nullptr; size_t comp_cap = 0;   // components scratch of sc_eval_loglike
   void* d_km = nullptr; size_t km_cap = 0;         // k-means: changed counter + member counts
+  // streams workload: template (FP64 + FP32), pieces of the edge list, per-piece sigma and z partials
+  double4* d_T64 = nullptr; float4* d_T32 = nullptr; size_t t64_cap = 0, t32_cap = 0;
+  int* d_sp = nullptr; size_t sp_cap = 0; double* d_spsig = nullptr; size_t spsig_cap = 0;
+  double2* d_zpart = nullptr; size_t zpart_cap = 0; double* d_hh = nullptr; size_t hh_cap = 0;
   // adaptive (per-particle) segments: moments of the weights over groups and fine sub-intervals, cached per node spacing
   int ad_lg = 0; float2* d_gmom = nullptr; float2* d_smom = nullptr; size_t gmom_cap = 0, smom_cap = 0;
   // scratch
@@ -2029,6 +2133,79 @@ int sc_search_run(sc_handle* h, const sc_search_config* sc, double* pos, double*
   return cleanup(SC_OK);
 }
 
+int sc_whiten_streams(sc_handle* h, const double* dA_ri, const double* dE_ri, int64_t n_streams, int32_t out_f64, void* W,
+                      void* stream) {
+  if (!h) return SC_ERR_NOT_INIT;
+  if (h->cuda_failed) return SC_ERR_CUDA;
+  if (!dA_ri || !dE_ri || !W || n_streams <= 0) return fail(h, SC_ERR_INVALID_ARG, "null pointer or n_streams <= 0");
+  cudaStream_t st = (cudaStream_t)stream;
+  const long long nb = h->cfg.n_bins, tot = nb * n_streams;
+  const unsigned grid = (unsigned)((tot + 255) / 256);
+  if (out_f64) k_whiten_streams_f64<<<grid, 256, 0, st>>>(dA_ri, dE_ri, h->G64, h->s0, nb, n_streams, (double4*)W);
+  else k_whiten_streams_f32<<<grid, 256, 0, st>>>(dA_ri, dE_ri, h->G64, h->s0, nb, n_streams, (float4*)W);
+  return check_launch(h, "k_whiten_streams");
+}
+
+int sc_eval_stat_streams(sc_handle* h, const double* theta, const void* W, int32_t w_is_f64, int64_t n_streams,
+                         const int32_t* seg_edges, int32_t n_seg, double* out, void* stream) {
+  if (!h) return SC_ERR_NOT_INIT;
+  if (h->cuda_failed) return SC_ERR_CUDA;
+  if (!theta || !W || !out || n_streams <= 0 || n_streams > 65535) return fail(h, SC_ERR_INVALID_ARG, "null pointer or n_streams outside 1..65535");
+  if (!seg_edges || n_seg <= 0) return fail(h, SC_ERR_INVALID_ARG, "seg_edges is null or n_seg <= 0");
+  cudaStream_t st = (cudaStream_t)stream;
+  const int nb = (int)h->cfg.n_bins;
+  std::vector<int> e((size_t)n_seg + 1);
+  cudaPointerAttributes at;
+  if (cudaPointerGetAttributes(&at, seg_edges) != cudaSuccess) { cudaGetLastError(); at.type = cudaMemoryTypeUnregistered; }
+  if (at.type == cudaMemoryTypeDevice) {
+    SC_CUDA(h, cudaMemcpyAsync(e.data(), seg_edges, e.size() * 4, cudaMemcpyDeviceToHost, st));
+    SC_CUDA(h, cudaStreamSynchronize(st));
+  } else memcpy(e.data(), seg_edges, e.size() * 4);
+  if (e[0] < 0 || e[n_seg] > nb) return fail(h, SC_ERR_INVALID_ARG, "seg_edges outside [0, n_bins]");
+  for (int k = 0; k < n_seg; ++k)
+    if (e[k + 1] < e[k]) return fail(h, SC_ERR_INVALID_ARG, "seg_edges not non-decreasing at k=%d", k);
+  // pieces of the non-empty segments
+  std::vector<int> plo, phi, plast;
+  for (int k = 0; k < n_seg; ++k)
+    for (int a = e[k]; a < e[k + 1]; a += kStreamPiece) {
+      plo.push_back(a); phi.push_back(std::min(a + kStreamPiece, e[k + 1])); plast.push_back(a + kStreamPiece >= e[k + 1] ? 1 : 0);
+    }
+  const int n_pieces = (int)plo.size();
+  if (n_pieces == 0) { SC_CUDA(h, cudaMemsetAsync(out, 0, (size_t)n_streams * 8, st)); return SC_OK; }
+  int rc;
+  if ((rc = grow(h, (void**)&h->d_sp, &h->sp_cap, (size_t)n_pieces * 12))) return rc;
+  if ((rc = grow(h, (void**)&h->d_spsig, &h->spsig_cap, (size_t)n_pieces * 8))) return rc;
+  if ((rc = grow(h, (void**)&h->d_zpart, &h->zpart_cap, (size_t)n_pieces * n_streams * 16))) return rc;
+  if ((rc = grow(h, (void**)&h->d_T64, &h->t64_cap, (size_t)nb * 32))) return rc;
+  if ((rc = grow(h, (void**)&h->d_T32, &h->t32_cap, (size_t)nb * 16))) return rc;
+  if ((rc = grow(h, (void**)&h->d_hh, &h->hh_cap, (size_t)nb * 32))) return rc;
+  int* d_lo = h->d_sp; int* d_hi = d_lo + n_pieces; int* d_last = d_hi + n_pieces;
+  SC_CUDA(h, cudaMemcpyAsync(d_lo, plo.data(), (size_t)n_pieces * 4, cudaMemcpyHostToDevice, st));
+  SC_CUDA(h, cudaMemcpyAsync(d_hi, phi.data(), (size_t)n_pieces * 4, cudaMemcpyHostToDevice, st));
+  SC_CUDA(h, cudaMemcpyAsync(d_last, plast.data(), (size_t)n_pieces * 4, cudaMemcpyHostToDevice, st));
+  SC_CUDA(h, cudaStreamSynchronize(st));             // the host vectors go out of scope
+  // the template, once (same node tables and interpolants as everything else)
+  double* hA = h->d_hh; double* hE = hA + (size_t)nb * 2;
+  if ((rc = sc_gen_template(h, theta, 1, hA, hE, stream))) return rc;
+  {
+    Timed tm(h, st, SC_TIME_OTHER);
+    k_streams_template<<<(nb + 255) / 256, 256, 0, st>>>(hA, hE, nb, h->d_T64, h->d_T32);
+    if ((rc = check_launch(h, "k_streams_template"))) return rc;
+    k_streams_sigma<<<(n_pieces + 7) / 8, 256, 0, st>>>(h->d_T64, h->G64, d_lo, d_hi, n_pieces, h->d_spsig);
+    if ((rc = check_launch(h, "k_streams_sigma"))) return rc;
+  }
+  {
+    Timed tm(h, st, SC_TIME_DENSE);
+    const dim3 grid((n_pieces + 7) / 8, (unsigned)n_streams);
+    if (w_is_f64) k_streams_z<double4, double><<<grid, 256, 0, st>>>((const double4*)W, h->d_T64, d_lo, d_hi, n_pieces, nb, (int)n_streams, h->d_zpart);
+    else k_streams_z<float4, float><<<grid, 256, 0, st>>>((const float4*)W, h->d_T32, d_lo, d_hi, n_pieces, nb, (int)n_streams, h->d_zpart);
+    if ((rc = check_launch(h, "k_streams_z"))) return rc;
+  }
+  Timed tm2(h, st, SC_TIME_STITCH);
+  k_streams_finish<<<(unsigned)((n_streams + 127) / 128), 128, 0, st>>>(h->d_zpart, h->d_spsig, d_last, n_pieces, (int)n_streams, out);
+  return check_launch(h, "k_streams_finish");
+}
+
 int sc_eval_stat_host(sc_handle* h, const double* params, int64_t P, const int32_t* seg_edges, int32_t n_seg,
                       double* out, void* stream) {
   if (!h) return SC_ERR_NOT_INIT;
@@ -2251,7 +2428,8 @@ int sc_free(sc_handle* h) {
   if (!h) return SC_ERR_NOT_INIT;
   cudaFree(h->D32); cudaFree(h->W64); cudaFree(h->G64);
   cudaFree(h->scratch); cudaFree(h->d_edges); cudaFree(h->d_chunk_k0); cudaFree(h->d_flags);
-  cudaFree(h->d_counter); cudaFree(h->d_params_stage); cudaFree(h->d_comp); cudaFree(h->d_km); cudaFree(h->d_gmom); cudaFree(h->d_smom);
+  cudaFree(h->d_counter); cudaFree(h->d_params_stage); cudaFree(h->d_comp); cudaFree(h->d_km); cudaFree(h->d_T64); cudaFree(h->d_T32); cudaFree(h->d_sp);
+  cudaFree(h->d_spsig); cudaFree(h->d_zpart); cudaFree(h->d_hh); cudaFree(h->d_gmom); cudaFree(h->d_smom);
   cudaFree(h->d_piece_first); cudaFree(h->d_piece_lo); cudaFree(h->d_piece_hi); cudaFree(h->d_moments);
   for (auto& e : h->evs) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
   cudaGetLastError();
