@@ -413,7 +413,7 @@ def run_ours(args, rank, local_rank, world):
         if not args.no_cpu_baseline and world == 1:
             from oracle import sc_oracle as orc
             cores = orc.num_threads()
-            n_p, k_cpu = 4 * max(8, min(32, cores)), 2          # ~10-20 s of CPU work on the box's cores
+            n_p, k_cpu = 4 * max(8, min(32, cores)), 3          # ~10-20 s of CPU work on the box's cores
             sec, cores = oracle_sample_run(sy.config_inputs(cid, P=n_p), N, n_p, k_cpu, 0)
             line["cpu_baseline"] = {"value": n_p * nb / sec, "unit": UNIT, "cores": cores, "kind": "oracle",
                                     "sample": f"{n_p} particles x all {nb} bins per step, {k_cpu} steps (statistic + PSO), "

@@ -172,7 +172,7 @@ def config_inputs(config_id, P=None, replica=0):
     n = spec["P"] if P is None else P
     return dict(id=config_id, spec=spec, cfg=cfg, f=f, S_A=S, S_E=S.copy(), df=df, noise_A=nA, noise_E=nE,
                 injections=injections, lo=lo, hi=hi,
-                particles=draw_particles(seed_for("particles", config_id, replica), spec["P"], lo, hi)[:n].copy(),
-                velocities=draw_velocities(seed_for("velocities", config_id, replica), spec["P"], lo, hi)[:n].copy(),
+                particles=draw_particles(seed_for("particles", config_id, replica), max(spec["P"], n), lo, hi)[:n].copy(),
+                velocities=draw_velocities(seed_for("velocities", config_id, replica), max(spec["P"], n), lo, hi)[:n].copy(),
                 edges={N: edges(cfg["n_bins"], N) for N in spec["n_segs"]},
                 pso_seed=seed_for("pso", config_id, replica))
