@@ -198,9 +198,17 @@ void sco_tdi(const sco_config* c, const double th[8], double f, double t, double
 
 /* O2+O3+O4: h_alpha(f_j) = T_alpha(theta, f_j; t_f) * f^(-7/6) * e^{-i Psi(f_j)}  (Eq. 16),
  * zero outside the time window 0 <= t(f_j) <= T_obs when window_mode = 1 (Q4). */
+int64_t sco_template3(const sco_config* c, const double th[8], int64_t j_begin, int64_t n, double* hA, double* hE,
+                      double* hT);
 int64_t sco_template(const sco_config* c, const double th[8], int64_t j_begin, int64_t n, double* hA, double* hE) {
+  return sco_template3(c, th, j_begin, n, hA, hE, NULL);
+}
+/* The same with the third TDI channel T = (X + Y + Z)/sqrt(3) (the paper uses A, E and T; Q16). */
+int64_t sco_template3(const sco_config* c, const double th[8], int64_t j_begin, int64_t n, double* hA, double* hE,
+                      double* hT) {
   memset(hA, 0, (size_t)n * 2 * sizeof(double));
   if (hE) memset(hE, 0, (size_t)n * 2 * sizeof(double));
+  if (hT) memset(hT, 0, (size_t)n * 2 * sizeof(double));
   if (!theta_valid(th)) return 0;
   int64_t inwin = 0;
   for (int64_t i = 0; i < n; ++i) {
@@ -218,6 +226,10 @@ int64_t sco_template(const sco_config* c, const double th[8], int64_t j_begin, i
     if (hE) {
       hE[2 * i]     = tdi[4][0] * er - tdi[4][1] * ei;
       hE[2 * i + 1] = tdi[4][0] * ei + tdi[4][1] * er;
+    }
+    if (hT) {
+      hT[2 * i]     = tdi[5][0] * er - tdi[5][1] * ei;
+      hT[2 * i + 1] = tdi[5][0] * ei + tdi[5][1] * er;
     }
   }
   return inwin;
@@ -569,4 +581,59 @@ int32_t sco_kmeans(const double* pos, int64_t P, const double* lo, const double*
 int32_t sco_converged(const double* hist, int64_t n_iter, int32_t window, double delta) {
   if (n_iter <= window) return 0;
   return (hist[n_iter - 1] - hist[n_iter - 1 - window] <= delta) ? 1 : 0;
+}
+
+
+/* ------------------------------------------------------------------------------------------------
+ * Three TDI channels A, E, T (Eq. 1 and 7 sum over alpha in {A, E, T}).  Same definitions as above
+ * with one more term in every channel sum.
+ * ------------------------------------------------------------------------------------------------ */
+double sco_stat_from_arrays3(const double* dA, const double* dE, const double* dT, const double* hA, const double* hE,
+                             const double* hT, const double* SA, const double* SE, const double* ST, double df,
+                             const int64_t* edges, int64_t n_seg, double* out_seg) {
+  const double* d[3] = {dA, dE, dT};
+  const double* h[3] = {hA, hE, hT};
+  const double* S[3] = {SA, SE, ST};
+  double ups = 0.0;
+  for (int64_t k = 0; k < n_seg; ++k) {
+    double zr = 0.0, zi = 0.0, sig = 0.0;
+    for (int64_t j = edges[k]; j < edges[k + 1]; ++j)
+      for (int a = 0; a < 3; ++a) {
+        zr += (d[a][2 * j] * h[a][2 * j] + d[a][2 * j + 1] * h[a][2 * j + 1]) / S[a][j];
+        zi += (d[a][2 * j + 1] * h[a][2 * j] - d[a][2 * j] * h[a][2 * j + 1]) / S[a][j];
+        sig += (h[a][2 * j] * h[a][2 * j] + h[a][2 * j + 1] * h[a][2 * j + 1]) / S[a][j];
+      }
+    if (out_seg) { out_seg[3 * k] = zr; out_seg[3 * k + 1] = zi; out_seg[3 * k + 2] = sig; }
+    if (sig > 0.0) {
+      const double x = 4.0 * df * sqrt(zr * zr + zi * zi);
+      const double hh = 4.0 * df * sig;
+      ups += x * x / hh;
+    }
+  }
+  return ups;
+}
+
+double sco_inner3(const double* aA, const double* aE, const double* aT, const double* bA, const double* bE, const double* bT,
+                  const double* SA, const double* SE, const double* ST, double df, int64_t n) {
+  return sco_inner(aA, aE, bA, bE, SA, SE, df, n) + sco_inner(aT, NULL, bT, NULL, ST, NULL, df, n);
+}
+
+void sco_eval_stat3(const sco_config* c, const double* dA, const double* dE, const double* dT, const double* SA,
+                    const double* SE, const double* ST, const double* params, int64_t P, const int64_t* edges,
+                    int64_t n_seg, double* out, double* out_seg) {
+  const int64_t n = c->n_bins;
+  const double df = 1.0 / c->T_obs_s;
+#pragma omp parallel
+  {
+    double* hA = (double*)malloc((size_t)n * 2 * sizeof(double));
+    double* hE = (double*)malloc((size_t)n * 2 * sizeof(double));
+    double* hT = (double*)malloc((size_t)n * 2 * sizeof(double));
+#pragma omp for schedule(dynamic, 1)
+    for (int64_t p = 0; p < P; ++p) {
+      sco_template3(c, params + 8 * p, 0, n, hA, hE, hT);
+      out[p] = sco_stat_from_arrays3(dA, dE, dT, hA, hE, hT, SA, SE, ST, df, edges, n_seg,
+                                     out_seg ? out_seg + (size_t)p * (size_t)n_seg * 3 : NULL);
+    }
+    free(hA); free(hE); free(hT);
+  }
 }

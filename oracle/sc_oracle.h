@@ -33,6 +33,9 @@
  *                          centroids = member means); within-cluster sum of squares never increases; a hand-computed
  *                          1-D example; scikit-learn's Lloyd KMeans from the same initial centroids gives the same labels.
  *   sco_converged        : the rule of PAPER.md:508 on hand-written histories.
+ *   sco_*3 (A, E, T)     : reduce to the two-channel functions when the T data and template vanish; T template = the
+ *                          (X+Y+Z)/sqrt(3) of sco_tdi (pinned above: T -> 0 in the long-wavelength limit); d = h gives rho^2
+ *                          = <h|h>_A + <h|h>_E + <h|h>_T for any edges; brute-force phase grid on tiny grids.
  */
 #ifndef SC_ORACLE_H
 #define SC_ORACLE_H
@@ -118,6 +121,18 @@ void sco_pso_step(double* pos, double* vel, double* pbest_pos, double* pbest_val
                   double* gbest_pos, double* gbest_val, const double* lo, const double* hi, const double* eps_min,
                   double omega, double phi_p, double phi_g, uint64_t seed, uint64_t iter,
                   int64_t n_particles, int32_t n_swarms);
+
+/* Three channels A, E, T: the same definitions with one more term in every channel sum. */
+int64_t sco_template3(const sco_config* c, const double theta[8], int64_t j_begin, int64_t n,
+                      double* hA_ri, double* hE_ri, double* hT_ri);
+double sco_stat_from_arrays3(const double* dA_ri, const double* dE_ri, const double* dT_ri, const double* hA_ri,
+                             const double* hE_ri, const double* hT_ri, const double* S_A, const double* S_E,
+                             const double* S_T, double df, const int64_t* edges, int64_t n_seg, double* out_seg);
+double sco_inner3(const double* aA, const double* aE, const double* aT, const double* bA, const double* bE, const double* bT,
+                  const double* S_A, const double* S_E, const double* S_T, double df, int64_t n);
+void sco_eval_stat3(const sco_config* c, const double* dA_ri, const double* dE_ri, const double* dT_ri, const double* S_A,
+                    const double* S_E, const double* S_T, const double* params, int64_t n_particles,
+                    const int64_t* edges, int64_t n_seg, double* out, double* out_seg);
 
 /* O7 with a swarm label per particle (members need not be contiguous; PAPER.md:199 regrouping). */
 void sco_pso_step_labeled(double* pos, double* vel, double* pbest_pos, double* pbest_val, const double* stat,

@@ -85,6 +85,13 @@ def lib():
                                            C.c_double, C.c_double, C.c_double, C.c_uint64, C.c_uint64, C.c_int64, C.c_int32]
         L.sco_kmeans.restype = C.c_int32
         L.sco_kmeans.argtypes = [_dp, C.c_int64, _dp, _dp, _dp, C.c_int32, C.c_int32, _i32p, _ip]
+        L.sco_template3.restype = C.c_int64
+        L.sco_template3.argtypes = [C.POINTER(Config), _dp, C.c_int64, C.c_int64, _dp, _dp, _dp]
+        L.sco_stat_from_arrays3.restype = C.c_double
+        L.sco_stat_from_arrays3.argtypes = [_dp] * 9 + [C.c_double, _ip, C.c_int64, _dp]
+        L.sco_inner3.restype = C.c_double
+        L.sco_inner3.argtypes = [_dp] * 9 + [C.c_double, C.c_int64]
+        L.sco_eval_stat3.argtypes = [C.POINTER(Config)] + [_dp] * 7 + [C.c_int64, _ip, C.c_int64, _dp, _dp]
         L.sco_converged.restype = C.c_int32
         L.sco_converged.argtypes = [_dp, C.c_int64, C.c_int32, C.c_double]
     return _lib
@@ -295,3 +302,40 @@ def kmeans(pos, lo, hi, cent, max_iter=100):
 def converged(hist, window, delta):
     h = _f64(hist)
     return bool(lib().sco_converged(_d(h), len(h), int(window), float(delta)))
+
+
+# ---------------------------------------------------------------------------------------------- three channels A, E, T
+def template3(cfg, theta, j_begin=0, n=None):
+    """(h_A, h_E, h_T, n_in_window)."""
+    n = int(cfg.n_bins - j_begin if n is None else n)
+    th = _f64(theta)
+    h = [np.zeros(n, dtype=np.complex128) for _ in range(3)]
+    w = lib().sco_template3(C.byref(cfg), _d(th), int(j_begin), n, *[_d(x.view(np.float64)) for x in h])
+    return h[0], h[1], h[2], int(w)
+
+
+def stat_from_arrays3(d3, h3, S3, df, edges, want_seg=False):
+    """d3, h3: (A, E, T) complex arrays; S3: (S_A, S_E, S_T)."""
+    edges = np.ascontiguousarray(edges, dtype=np.int64)
+    n_seg = len(edges) - 1
+    seg = np.zeros((n_seg, 3)) if want_seg else None
+    a = [_ri(x) for x in d3] + [_ri(x) for x in h3] + [_f64(x) for x in S3]
+    u = lib().sco_stat_from_arrays3(*[_d(x) for x in a], float(df), edges.ctypes.data_as(_ip), n_seg, _d(seg))
+    return (u, seg) if want_seg else u
+
+
+def inner3(a3, b3, S3, df):
+    a = [_ri(x) for x in a3] + [_ri(x) for x in b3] + [_f64(x) for x in S3]
+    return lib().sco_inner3(*[_d(x) for x in a], float(df), len(a3[0]))
+
+
+def eval_stat3(cfg, d3, S3, params, edges, want_seg=False):
+    params = _f64(params).reshape(-1, 8)
+    P = params.shape[0]
+    edges = np.ascontiguousarray(edges, dtype=np.int64)
+    n_seg = len(edges) - 1
+    out = np.zeros(P)
+    seg = np.zeros((P, n_seg, 3)) if want_seg else None
+    a = [_ri(x) for x in d3] + [_f64(x) for x in S3]
+    lib().sco_eval_stat3(C.byref(cfg), *[_d(x) for x in a], _d(params), P, edges.ctypes.data_as(_ip), n_seg, _d(out), _d(seg))
+    return (out, seg) if want_seg else out

@@ -63,6 +63,23 @@ def psd_AE(f):
     return 8.0 * np.sin(x) ** 2 * (2.0 * S_acc * (3.0 + 2.0 * np.cos(x) + np.cos(2.0 * x)) + S_oms * (2.0 + np.cos(x)))
 
 
+def psd_T(f):
+    """The third TDI-1 channel T = (X + Y + Z)/sqrt(3), same link-noise model: S_T = S_X + 2 S_XY."""
+    f = np.asarray(f, dtype=np.float64)
+    x = 2.0 * np.pi * f * ARM_L_S
+    S_oms = (15e-12) ** 2 * (1.0 + (2e-3 / f) ** 4) * (2.0 * np.pi * f / C_M_S) ** 2
+    S_acc = (3e-15) ** 2 * (1.0 + (0.4e-3 / f) ** 2) * (1.0 + (f / 8e-3) ** 4) / (2.0 * np.pi * f * C_M_S) ** 2
+    return 16.0 * np.sin(x) ** 2 * ((1.0 - np.cos(x)) * S_oms + 2.0 * (1.0 - np.cos(x)) ** 2 * S_acc)
+
+
+def link_noise_sources(f):
+    """(S_oms, S_acc) per link / test mass in fractional-frequency units: the two inputs of psd_AE and psd_T."""
+    f = np.asarray(f, dtype=np.float64)
+    S_oms = (15e-12) ** 2 * (1.0 + (2e-3 / f) ** 4) * (2.0 * np.pi * f / C_M_S) ** 2
+    S_acc = (3e-15) ** 2 * (1.0 + (0.4e-3 / f) ** 2) * (1.0 + (f / 8e-3) ** 4) / (2.0 * np.pi * f * C_M_S) ** 2
+    return S_oms, S_acc
+
+
 def draw_noise(seed, S, df):
     """O6: Re n, Im n ~ N(0, S/(4 df)) independent per bin (so <n|h> ~ N(0, <h|h>))."""
     rng = np.random.default_rng(seed)
