@@ -39,7 +39,7 @@ typedef struct {
   double  T_obs_s;        /* observation time; df = 1/T_obs                                         */
   int64_t j0;             /* first bin index                                                         */
   int64_t n_bins;         /* 1 <= n_bins < 2^31                                                      */
-  int32_t n_channels;     /* 2 (A,E).  3 (T) is reserved and rejected                                */
+  int32_t n_channels;     /* 2 (A,E) for sc_init_data; 3 (A,E,T) for sc_init_data3                   */
   int32_t window_mode;    /* 0 = none, 1 = template is zero where t(f) is outside [0, T_obs]  (Q4)   */
   int32_t pn_order_x2;    /* highest phase term kept, 0..7; 7 = 3.5PN (O2)                           */
   int32_t ecc_leading;    /* 1 = include the leading-order e0^2 phase term (Q5)                      */
@@ -88,6 +88,19 @@ int sc_init_data(sc_handle** out, const sc_config* cfg,
 int sc_init_data_host(sc_handle** out, const sc_config* cfg,
                       const double* dA_ri, const double* dE_ri, const double* S_A, const double* S_E,
                       void* cuda_stream);
+
+/* Three TDI channels A, E, T (Eq. 1 and Eq. 7 sum over alpha in {A, E, T}; T = (X + Y + Z)/sqrt(3),
+ * reading Q16).  cfg->n_channels must be 3; all arrays DEVICE as in sc_init_data.  On such a handle sc_eval_stat[_host],
+ * sc_eval_segments, sc_eval_components, sc_eval_loglike, sc_data_norm and sc_search_run (equal-width edges) include the
+ * T channel: its per-segment sums come from a second pass through the same kernels and are added to those of A and E
+ * before |z_k|^2 / sigma_k is formed (one common phase per segment, Q1).  sc_eval_stat_adaptive (n_seg > 1) and the
+ * streams workload return SC_ERR_INVALID_ARG on three-channel handles. */
+int sc_init_data3(sc_handle** out, const sc_config* cfg,
+                  const double* dA_ri, const double* dE_ri, const double* dT_ri,
+                  const double* S_A, const double* S_E, const double* S_T, void* cuda_stream);
+/* sc_gen_template with the T channel: hT_ri DEVICE [n_templates][n_bins] complex FP64 interleaved. */
+int sc_gen_template3(sc_handle* h, const double* params, int64_t n_templates,
+                     double* hA_ri, double* hE_ri, double* hT_ri, void* cuda_stream);
 
 /* a1..a6 -- Upsilon_N(d, theta_p) for every particle (Eq. 7, 8, 10; readings Q1, Q2, Q7, Q8):
  *   z_k = sum_a sum_{j in [e_k, e_k+1)} d_a conj(h_a)/S_a,  sigma_k = sum_a sum_j |h_a|^2/S_a,

@@ -14,7 +14,7 @@ SC_OK, SC_ERR_INVALID_ARG, SC_ERR_NOT_INIT, SC_ERR_CUDA, SC_ERR_OOM = 0, -1, -2,
 SC_OPT_PRECISION, SC_OPT_F32_MIN_SEG, SC_OPT_SCRATCH_BYTES, SC_OPT_TC_MAX_S, SC_OPT_STRIDE_LOG2, SC_OPT_PROFILE, SC_OPT_SINCOS, SC_OPT_MUFU_MIN_SEG = 1, 2, 3, 4, 5, 6, 7, 8
 SC_TIMING_CLASSES = ["nodes", "dense", "stitch", "pso", "other"]
 
-EXPORTED_SYMBOLS = ["sc_init_data", "sc_init_data_host", "sc_eval_stat", "sc_eval_stat_host", "sc_eval_segments",
+EXPORTED_SYMBOLS = ["sc_init_data", "sc_init_data_host", "sc_init_data3", "sc_gen_template3", "sc_eval_stat", "sc_eval_stat_host", "sc_eval_segments",
                     "sc_eval_stat_adaptive", "sc_eval_components", "sc_eval_loglike", "sc_data_norm", "sc_gen_template", "sc_pso_step", "sc_pso_step_labeled", "sc_kmeans", "sc_search_run", "sc_whiten_streams", "sc_eval_stat_streams", "sc_get_counters", "sc_get_timing", "sc_measure_fp64_peak",
                     "sc_set_option", "sc_free",
                     "sc_last_error", "sc_version"]
@@ -94,6 +94,10 @@ def load_library():
     cfgp = C.POINTER(ScConfig)
     L.sc_init_data.restype = C.c_int
     L.sc_init_data.argtypes = [C.POINTER(_vp), cfgp, _vp, _vp, _vp, _vp, _vp]
+    L.sc_init_data3.restype = C.c_int
+    L.sc_init_data3.argtypes = [C.POINTER(_vp), cfgp, _vp, _vp, _vp, _vp, _vp, _vp, _vp]
+    L.sc_gen_template3.restype = C.c_int
+    L.sc_gen_template3.argtypes = [_vp, _vp, C.c_int64, _vp, _vp, _vp, _vp]
     L.sc_init_data_host.restype = C.c_int
     L.sc_init_data_host.argtypes = [C.POINTER(_vp), cfgp, _vp, _vp, _vp, _vp, _vp]
     for name in ("sc_eval_stat", "sc_eval_stat_host", "sc_eval_segments", "sc_eval_components"):
@@ -211,6 +215,33 @@ def sc_init_data(cfg, dA_ri, dE_ri, S_A, S_E, stream=None):
                         _dev(S_A, torch.float64, "S_A"), _dev(S_E, torch.float64, "S_E"), _stream(stream))
     _check(rc, None)
     return h
+
+
+def sc_init_data3(cfg, dA_ri, dE_ri, dT_ri, S_A, S_E, S_T, stream=None):
+    """Three channels (A, E, T): DEVICE float64 tensors as in sc_init_data; cfg.n_channels must be 3."""
+    torch = _torch()
+    L = load_library()
+    if not isinstance(cfg, ScConfig):
+        cfg = ScConfig.from_dict(cfg)
+    n = int(cfg.n_bins)
+    names = ("dA_ri", "dE_ri", "dT_ri", "S_A", "S_E", "S_T")
+    for t, m, nm in zip((dA_ri, dE_ri, dT_ri, S_A, S_E, S_T), (2 * n,) * 3 + (n,) * 3, names):
+        if isinstance(t, torch.Tensor) and t.numel() != m:
+            raise SCError(SC_ERR_INVALID_ARG, f"{nm}: expected {m} float64 values, got {t.numel()}")
+    h = _vp()
+    rc = L.sc_init_data3(C.byref(h), C.byref(cfg), *[_dev(t, torch.float64, nm) for t, nm in
+                                                     zip((dA_ri, dE_ri, dT_ri, S_A, S_E, S_T), names)], _stream(stream))
+    _check(rc, None)
+    return h
+
+
+def sc_gen_template3(h, params, n_templates, hA_ri, hE_ri, hT_ri, stream=None):
+    torch = _torch()
+    rc = load_library().sc_gen_template3(h, _dev(params, torch.float64, "params"), n_templates,
+                                         _dev(hA_ri, torch.float64, "hA_ri"), _dev(hE_ri, torch.float64, "hE_ri"),
+                                         _dev(hT_ri, torch.float64, "hT_ri"), _stream(stream))
+    _check(rc, h)
+    return hA_ri, hE_ri, hT_ri
 
 
 def sc_init_data_host(cfg, dA, dE, S_A, S_E, stream=None):
@@ -466,9 +497,12 @@ def sc_free(h):
 class Handle:
     """Owns one sc_handle.  Methods forward to the C-named functions above."""
 
-    def __init__(self, cfg, dA, dE, S_A, S_E, host=False, stream=None):
+    def __init__(self, cfg, dA, dE, S_A, S_E, host=False, stream=None, dT=None, S_T=None):
         self.cfg = cfg if isinstance(cfg, ScConfig) else ScConfig.from_dict(cfg)
-        self.h = (sc_init_data_host if host else sc_init_data)(self.cfg, dA, dE, S_A, S_E, stream)
+        if dT is not None:                      # three channels (A, E, T)
+            self.h = sc_init_data3(self.cfg, dA, dE, dT, S_A, S_E, S_T, stream)
+        else:
+            self.h = (sc_init_data_host if host else sc_init_data)(self.cfg, dA, dE, S_A, S_E, stream)
 
     def eval_stat(self, params, seg_edges, out=None, stream=None):
         torch = _torch()
@@ -527,6 +561,15 @@ class Handle:
         hE = torch.empty_like(hA)
         sc_gen_template(self.h, params, params.shape[0], hA, hE, stream)
         return torch.view_as_complex(hA), torch.view_as_complex(hE)
+
+    def gen_template3(self, params, stream=None):
+        """-> (h_A, h_E, h_T) complex128 CUDA tensors [n_templates, n_bins] (three-channel handles)."""
+        torch = _torch()
+        params = params.reshape(-1, 8)
+        n = int(self.cfg.n_bins)
+        h3 = [torch.empty((params.shape[0], n, 2), dtype=torch.float64, device=params.device) for _ in range(3)]
+        sc_gen_template3(self.h, params, params.shape[0], *h3, stream)
+        return tuple(torch.view_as_complex(x) for x in h3)
 
     def pso_step(self, state, stat, lo, hi, eps_min, omega, phi_p, phi_g, seed, it, n_swarms, stream=None):
         """state: dict of CUDA tensors pos, vel, pbest_pos, pbest_val, gbest_pos, gbest_val (updated in place)."""

@@ -28,6 +28,7 @@ struct DevCfg {
   double f_amp_ref;             // amplitude normalisation: A(f) = (f / f_amp_ref)^(-7/6)
   int log2_stride, stride;      // coarse node spacing in bins (power of two, >= 4)
   int n_nodes;                  // nodes i = -kNodeOff .. n_intervals + 3
+  int chan_set;                 // 0: the node amplitudes are (A, E); 1: (T, 0) -- the T pass of a three-channel handle
 };
 // Each coarse interval is cut into 4 fine sub-intervals (stride/4 bins) on which the amplitudes are local cubics.
 constexpr int kNodeOff = 2;     // the quintic phase stencil reaches 2 nodes to the left, 3 to the right
@@ -192,6 +193,13 @@ __device__ NodeOut eval_node(const DevCfg& c, const Particle& q, long long jglob
   const double fr = f / c.f_amp_ref;
   const double amp = 1.0 / (fr * cbrt(sqrt(fr)));                   // (f/f_ref)^(-7/6)
   const double s2 = 0.7071067811865476 * amp, s6 = 0.4082482904638631 * amp;
+  if (c.chan_set == 1) {                                             // T = (X + Y + Z)/sqrt(3) in the first slot
+    const double s3 = 0.5773502691896258 * amp;
+    o.Ar = (XYZ[0][0] + XYZ[1][0] + XYZ[2][0]) * s3;
+    o.Ai = (XYZ[0][1] + XYZ[1][1] + XYZ[2][1]) * s3;
+    o.Er = 0.0; o.Ei = 0.0;
+    return o;
+  }
   o.Ar = (XYZ[2][0] - XYZ[0][0]) * s2;
   o.Ai = (XYZ[2][1] - XYZ[0][1]) * s2;
   o.Er = (XYZ[0][0] - 2.0 * XYZ[1][0] + XYZ[2][0]) * s6;

@@ -1467,6 +1467,9 @@ struct sc_handle {
   int* d_piece_first = nullptr; int* d_piece_lo = nullptr; int* d_piece_hi = nullptr; float2* d_moments = nullptr;
   size_t pf_cap = 0, plo_cap = 0, phi_cap = 0, mom_cap = 0;
   long long launches = 0;
+  // three-channel handles (A, E, T): the T channel lives in a second handle whose first slot carries T (chan_set = 1)
+  // and whose second slot is empty; the per-segment sums of both are added before |z|^2/sigma is formed
+  sc_handle* sub = nullptr; double* d_seg3 = nullptr; size_t seg3_cap = 0;
   // optional per-kernel-class device timing (SC_OPT_PROFILE): event pairs recorded around each launch
   bool profile = false;
   struct Ev { cudaEvent_t a, b; int cls; };
@@ -1768,6 +1771,60 @@ int eval_common(sc_handle* h, const double* params, int64_t P, const int32_t* se
              : run_batches<float>(h, params, P, out, out_seg, out_comp, st, seg_mode);
 }
 
+// ------------------------------------------------------------------------------------------------ three channels (A, E, T)
+// out = 4 df sum_k |zAE_k + zT_k|^2 / (sigAE_k + sigT_k) from the per-segment sums of the two passes (definition units),
+// optionally the combined segments and the Eq. 8 / Eq. 3 components.
+__global__ void k_combine3(const double* __restrict__ segA, const double* __restrict__ segT, int P, int n_seg, double four_df,
+                           double* __restrict__ out, double* __restrict__ out_seg, double* __restrict__ comp3) {
+  const int p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= P) return;
+  double ups = 0.0, xs = 0.0, hs = 0.0;
+  for (int k = 0; k < n_seg; ++k) {
+    const size_t at = ((size_t)p * n_seg + k) * 3;
+    const double zr = segA[at] + segT[at], zi = segA[at + 1] + segT[at + 1], sg = segA[at + 2] + segT[at + 2];
+    if (out_seg) { out_seg[at] = zr; out_seg[at + 1] = zi; out_seg[at + 2] = sg; }
+    if (sg > 0.0) {
+      const double z2 = zr * zr + zi * zi;
+      ups += z2 / sg; xs += sqrt(z2); hs += sg;
+    }
+  }
+  if (out) out[p] = four_df * ups;
+  if (comp3) { comp3[3 * (size_t)p] = four_df * ups; comp3[3 * (size_t)p + 1] = four_df * xs; comp3[3 * (size_t)p + 2] = four_df * hs; }
+}
+
+// Statistic / segments / components of a handle with or without the T channel.
+int eval_any(sc_handle* h, const double* params, int64_t P, const int32_t* seg_edges, int32_t n_seg,
+             double* out, double* out_seg, void* stream, bool seg_mode, double* out_comp = nullptr) {
+  if (!h) return SC_ERR_NOT_INIT;
+  if (!h->sub) return eval_common(h, params, P, seg_edges, n_seg, out, out_seg, stream, seg_mode, out_comp);
+  if (h->cuda_failed) return SC_ERR_CUDA;
+  if (!params || P <= 0 || (!seg_mode && !out && !out_comp) || (seg_mode && !out_seg) || !seg_edges || n_seg <= 0)
+    return fail(h, SC_ERR_INVALID_ARG, "null pointer, n_particles <= 0 or n_seg <= 0");
+  cudaStream_t st = (cudaStream_t)stream;
+  // batches of particles such that the two segment tables fit in 2 GiB
+  const size_t per_p = (size_t)n_seg * 24;
+  int64_t Pb = (int64_t)std::max<size_t>(1, ((size_t)1 << 30) / per_p);
+  Pb = std::min<int64_t>(Pb, P);
+  int rc = grow(h, (void**)&h->d_seg3, &h->seg3_cap, 2 * per_p * (size_t)Pb);
+  if (rc) return rc;
+  double* segA = h->d_seg3; double* segT = segA + (size_t)Pb * n_seg * 3;
+  const double four_df = 4.0 / h->cfg.T_obs_s;
+  for (int64_t pb = 0; pb < P; pb += Pb) {
+    const int64_t Pn = std::min<int64_t>(Pb, P - pb);
+    if ((rc = eval_common(h, params + pb * 8, Pn, seg_edges, n_seg, nullptr, segA, stream, true))) return rc;
+    if ((rc = eval_common(h->sub, params + pb * 8, Pn, seg_edges, n_seg, nullptr, segT, stream, true))) {
+      fail(h, rc, "T pass: %s", h->sub->err.c_str());
+      return rc;
+    }
+    Timed tm(h, st, SC_TIME_STITCH);
+    k_combine3<<<(unsigned)((Pn + 127) / 128), 128, 0, st>>>(segA, segT, (int)Pn, n_seg, four_df, out ? out + pb : nullptr,
+                                                            seg_mode ? out_seg + (size_t)pb * n_seg * 3 : nullptr,
+                                                            out_comp ? out_comp + pb * 3 : nullptr);
+    if ((rc = check_launch(h, "k_combine3"))) return rc;
+  }
+  return SC_OK;
+}
+
 // Per-particle equal-SNR^2 segments: see the kernels above.  FP32-amplitude path.
 int run_adaptive(sc_handle* h, const double* params, int64_t P, int n_seg, double* out, int32_t* out_edges, double* out_comp,
                  cudaStream_t st) {
@@ -1866,13 +1923,13 @@ __global__ void k_fill_edges01(int* __restrict__ out_edges, int P, int n_bins) {
 }
 
 int init_common(sc_handle** out, const sc_config* cfg, const double* dA, const double* dE, const double* S_A,
-                const double* S_E, void* stream, bool host_inputs) {
+                const double* S_E, void* stream, bool host_inputs, int chan_set = 0) {
   if (!out) return fail(nullptr, SC_ERR_INVALID_ARG, "out is null");
   *out = nullptr;
   if (!cfg || !dA || !dE || !S_A || !S_E) return fail(nullptr, SC_ERR_INVALID_ARG, "null pointer");
   if (!(cfg->T_obs_s > 0.0) || cfg->n_bins < 1 || cfg->n_bins >= (int64_t)1 << 31 || cfg->j0 < 0)
     return fail(nullptr, SC_ERR_INVALID_ARG, "bad grid (T_obs_s, j0, n_bins)");
-  if (cfg->n_channels != 2) return fail(nullptr, SC_ERR_INVALID_ARG, "n_channels must be 2 (A,E); T is reserved");
+  if (cfg->n_channels != 2) return fail(nullptr, SC_ERR_INVALID_ARG, "n_channels must be 2 (A,E) here; three channels: sc_init_data3");
   if (cfg->pn_order_x2 < 0 || cfg->pn_order_x2 > 7) return fail(nullptr, SC_ERR_INVALID_ARG, "pn_order_x2 must be 0..7");
   if (cfg->window_mode != 0 && cfg->window_mode != 1) return fail(nullptr, SC_ERR_INVALID_ARG, "window_mode must be 0 or 1");
   if (!(cfg->arm_L_s > 0.0) || !(cfg->au_s > 0.0) || !(cfg->year_s > 0.0))
@@ -1897,6 +1954,7 @@ int init_common(sc_handle** out, const sc_config* cfg, const double* dA, const d
     d.sbn[m] = sin(b); d.cbn[m] = cos(b);
   }
   d.f_amp_ref = (double)std::max<int64_t>(cfg->j0, 1) / cfg->T_obs_s;
+  d.chan_set = chan_set;
   set_stride(h);
   auto bail = [&](int code) { sc_free(h); return code; };
 #define SC_INIT(call)                                                                              \
@@ -1976,20 +2034,61 @@ int sc_init_data_host(sc_handle** out, const sc_config* cfg, const double* dA, c
   return init_common(out, cfg, dA, dE, S_A, S_E, stream, true);
 }
 
+int sc_init_data3(sc_handle** out, const sc_config* cfg, const double* dA, const double* dE, const double* dT,
+                  const double* S_A, const double* S_E, const double* S_T, void* stream) {
+  if (!out) return fail(nullptr, SC_ERR_INVALID_ARG, "out is null");
+  *out = nullptr;
+  if (!cfg || !dT || !S_T) return fail(nullptr, SC_ERR_INVALID_ARG, "null pointer");
+  if (cfg->n_channels != 3) return fail(nullptr, SC_ERR_INVALID_ARG, "sc_init_data3 needs n_channels = 3");
+  sc_config c2 = *cfg;
+  c2.n_channels = 2;
+  sc_handle* h = nullptr;
+  int rc = init_common(&h, &c2, dA, dE, S_A, S_E, stream, false, 0);
+  if (rc) return rc;
+  // T pass: (T, nothing) with the PSD S_T in both slots (the second slot carries zero data and a zero template)
+  double* zeros = nullptr;
+  if (cudaMalloc(&zeros, (size_t)cfg->n_bins * 16) != cudaSuccess) { cudaGetLastError(); sc_free(h); return fail(nullptr, SC_ERR_OOM, "cudaMalloc failed"); }
+  cudaMemsetAsync(zeros, 0, (size_t)cfg->n_bins * 16, (cudaStream_t)stream);
+  rc = init_common(&h->sub, &c2, dT, zeros, S_T, S_T, stream, false, 1);
+  cudaStreamSynchronize((cudaStream_t)stream);
+  cudaFree(zeros);
+  if (rc) { sc_free(h); return rc; }
+  h->cfg.n_channels = 3;
+  *out = h;
+  return SC_OK;
+}
+
+int sc_gen_template3(sc_handle* h, const double* params, int64_t P, double* hA, double* hE, double* hT, void* stream) {
+  if (!h) return SC_ERR_NOT_INIT;
+  if (!h->sub) return fail(h, SC_ERR_INVALID_ARG, "not a three-channel handle");
+  if (!hT) return fail(h, SC_ERR_INVALID_ARG, "hT is null");
+  int rc = sc_gen_template(h, params, P, hA, hE, stream);
+  if (rc) return rc;
+  // the T pass writes T into its first slot; its second (empty) slot goes to scratch
+  cudaStream_t st = (cudaStream_t)stream;
+  double* dump = nullptr;
+  SC_CUDA(h, cudaMalloc(&dump, (size_t)P * h->cfg.n_bins * 16));
+  rc = sc_gen_template(h->sub, params, P, hT, dump, stream);
+  cudaStreamSynchronize(st);
+  cudaFree(dump);
+  if (rc) fail(h, rc, "T pass: %s", h->sub->err.c_str());
+  return rc;
+}
+
 int sc_eval_stat(sc_handle* h, const double* params, int64_t P, const int32_t* seg_edges, int32_t n_seg, double* out,
                  void* stream) {
-  return eval_common(h, params, P, seg_edges, n_seg, out, nullptr, stream, false);
+  return eval_any(h, params, P, seg_edges, n_seg, out, nullptr, stream, false);
 }
 
 int sc_eval_segments(sc_handle* h, const double* params, int64_t P, const int32_t* seg_edges, int32_t n_seg,
                      double* out_seg, void* stream) {
-  return eval_common(h, params, P, seg_edges, n_seg, nullptr, out_seg, stream, true);
+  return eval_any(h, params, P, seg_edges, n_seg, nullptr, out_seg, stream, true);
 }
 
 int sc_eval_components(sc_handle* h, const double* params, int64_t P, const int32_t* seg_edges, int32_t n_seg,
                        double* out3, void* stream) {
   if (!out3) return h ? fail(h, SC_ERR_INVALID_ARG, "out3 is null") : SC_ERR_NOT_INIT;
-  return eval_common(h, params, P, seg_edges, n_seg, nullptr, nullptr, stream, false, out3);
+  return eval_any(h, params, P, seg_edges, n_seg, nullptr, nullptr, stream, false, out3);
 }
 
 int sc_eval_loglike(sc_handle* h, const double* params, const double* amp, int64_t P, const int32_t* seg_edges,
@@ -1999,7 +2098,7 @@ int sc_eval_loglike(sc_handle* h, const double* params, const double* amp, int64
   if (!params || !amp || !out || P <= 0) return fail(h, SC_ERR_INVALID_ARG, "null pointer or n_particles <= 0");
   int rc = grow(h, (void**)&h->d_comp, &h->comp_cap, (size_t)P * 24);
   if (rc) return rc;
-  if ((rc = eval_common(h, params, P, seg_edges, n_seg, nullptr, nullptr, stream, false, h->d_comp))) return rc;
+  if ((rc = eval_any(h, params, P, seg_edges, n_seg, nullptr, nullptr, stream, false, h->d_comp))) return rc;
   k_loglike<<<(unsigned)((P + 127) / 128), 128, 0, (cudaStream_t)stream>>>(h->d_comp, amp, h->dd, (int)P, out);
   return check_launch(h, "k_loglike");
 }
@@ -2007,7 +2106,7 @@ int sc_eval_loglike(sc_handle* h, const double* params, const double* amp, int64
 int sc_data_norm(sc_handle* h, double* dd) {
   if (!h) return SC_ERR_NOT_INIT;
   if (!dd) return fail(h, SC_ERR_INVALID_ARG, "dd is null");
-  *dd = h->dd;
+  *dd = h->dd + (h->sub ? h->sub->dd : 0.0);
   return SC_OK;
 }
 
@@ -2018,9 +2117,10 @@ int sc_eval_stat_adaptive(sc_handle* h, const double* params, int64_t P, int32_t
   if (!params || P <= 0 || n_seg <= 0 || (!out && !out3)) return fail(h, SC_ERR_INVALID_ARG, "null pointer, n_particles <= 0 or n_seg <= 0");
   if (n_seg > h->cfg.n_bins) return fail(h, SC_ERR_INVALID_ARG, "n_seg exceeds n_bins");
   cudaStream_t st = (cudaStream_t)stream;
+  if (h->sub && n_seg > 1) return fail(h, SC_ERR_INVALID_ARG, "per-particle segments are not available on three-channel handles");
   if (n_seg == 1) {                              // one segment: the edges are (0, n_bins) for every particle
     const int32_t e[2] = {0, (int32_t)h->cfg.n_bins};
-    int rc = eval_common(h, params, P, e, 1, out, nullptr, stream, false, out3);
+    int rc = eval_any(h, params, P, e, 1, out, nullptr, stream, false, out3);
     if (rc) return rc;
     if (out_edges) {
       k_fill_edges01<<<(unsigned)((P + 127) / 128), 128, 0, st>>>(out_edges, (int)P, (int)h->cfg.n_bins);
@@ -2051,6 +2151,7 @@ int sc_search_run(sc_handle* h, const sc_search_config* sc, double* pos, double*
     return fail(h, SC_ERR_INVALID_ARG, "conv_window, max_iters_per_rung must be >= 1 and kmeans_max_iters >= 0");
   for (int r = 0; r < sc->n_rungs; ++r)
     if (sc->n_seg[r] < 1 || sc->n_seg[r] > h->cfg.n_bins) return fail(h, SC_ERR_INVALID_ARG, "n_seg[%d] out of range", r);
+  if (h->sub && sc->adaptive_edges) return fail(h, SC_ERR_INVALID_ARG, "per-particle segments are not available on three-channel handles");
   cudaStream_t st = (cudaStream_t)stream;
   const int S = n_swarms;
   const int64_t nb = h->cfg.n_bins;
@@ -2086,7 +2187,7 @@ int sc_search_run(sc_handle* h, const sc_search_config* sc, double* pos, double*
     int it = 0;
     for (; it < sc->max_iters_per_rung; ++it) {
       if (sc->adaptive_edges && N > 1) rc = sc_eval_stat_adaptive(h, pos, P, N, stat, nullptr, nullptr, stream);
-      else rc = eval_common(h, pos, P, e.data(), N, stat, nullptr, stream, false);
+      else rc = eval_any(h, pos, P, e.data(), N, stat, nullptr, stream, false);
       if (rc) return cleanup(rc);
       rc = sc_pso_step_labeled(h, pos, vel, pbest_pos, pbest_val, stat, gbest_pos, gbest_val, label, lo, hi, eps_d,
                                sc->omega[r], sc->phi_p[r], sc->phi_g[r], sc->seed, iter_global++, P, S, stream);
@@ -2152,6 +2253,7 @@ int sc_eval_stat_streams(sc_handle* h, const double* theta, const void* W, int32
   if (h->cuda_failed) return SC_ERR_CUDA;
   if (!theta || !W || !out || n_streams <= 0 || n_streams > 65535) return fail(h, SC_ERR_INVALID_ARG, "null pointer or n_streams outside 1..65535");
   if (!seg_edges || n_seg <= 0) return fail(h, SC_ERR_INVALID_ARG, "seg_edges is null or n_seg <= 0");
+  if (h->sub) return fail(h, SC_ERR_INVALID_ARG, "the streams workload is not available on three-channel handles");
   cudaStream_t st = (cudaStream_t)stream;
   const int nb = (int)h->cfg.n_bins;
   std::vector<int> e((size_t)n_seg + 1);
@@ -2221,7 +2323,7 @@ int sc_eval_stat_host(sc_handle* h, const double* params, int64_t P, const int32
   }
   h->d_out_stage = h->d_params_stage + (size_t)P * 8;
   SC_CUDA(h, cudaMemcpyAsync(h->d_params_stage, params, (size_t)P * 64, cudaMemcpyHostToDevice, st));
-  int rc = eval_common(h, h->d_params_stage, P, seg_edges, n_seg, h->d_out_stage, nullptr, stream, false);
+  int rc = eval_any(h, h->d_params_stage, P, seg_edges, n_seg, h->d_out_stage, nullptr, stream, false);
   if (rc) return rc;
   SC_CUDA(h, cudaMemcpyAsync(out, h->d_out_stage, (size_t)P * 8, cudaMemcpyDeviceToHost, st));
   SC_CUDA(h, cudaStreamSynchronize(st));
@@ -2395,6 +2497,7 @@ int sc_measure_fp64_peak(double* dfma_per_s, void* stream) {
 
 int sc_set_option(sc_handle* h, int32_t option, int64_t value) {
   if (!h) return SC_ERR_NOT_INIT;
+  if (h->sub && option != SC_OPT_PROFILE) { const int rc = sc_set_option(h->sub, option, value); if (rc) return fail(h, rc, "%s", h->sub->err.c_str()); }
   switch (option) {
     case SC_OPT_PRECISION:
       if (value < 0 || value > 2) return fail(h, SC_ERR_INVALID_ARG, "precision must be 0, 1 or 2");
@@ -2426,6 +2529,8 @@ int sc_set_option(sc_handle* h, int32_t option, int64_t value) {
 
 int sc_free(sc_handle* h) {
   if (!h) return SC_ERR_NOT_INIT;
+  if (h->sub) sc_free(h->sub);
+  cudaFree(h->d_seg3);
   cudaFree(h->D32); cudaFree(h->W64); cudaFree(h->G64);
   cudaFree(h->scratch); cudaFree(h->d_edges); cudaFree(h->d_chunk_k0); cudaFree(h->d_flags);
   cudaFree(h->d_counter); cudaFree(h->d_params_stage); cudaFree(h->d_comp); cudaFree(h->d_km); cudaFree(h->d_T64); cudaFree(h->d_T32); cudaFree(h->d_sp);
