@@ -69,12 +69,19 @@ enum {
   SC_OPT_SINCOS = 7,         /* FP32 amplitude path: sin/cos of the phase.  0 = automatic: hardware MUFU sin/cos
                                 (gain-calibrated at init) when n_seg >= SC_OPT_MUFU_MIN_SEG, else FP32 polynomial;
                                 1 = polynomial always; 2 = MUFU always.  See DESIGN.md "Precision".                  */
-  SC_OPT_MUFU_MIN_SEG = 8    /* threshold of that rule (default 64)                                                  */
+  SC_OPT_MUFU_MIN_SEG = 8,   /* threshold of that rule (default 32)                                                  */
+  SC_OPT_ESCALATE = 9,       /* 1 (default): in the automatic precision mode sc_eval_stat / sc_eval_stat_host / the search
+                                driver re-evaluate, by the all-FP64 path, every particle whose FP32-path statistic came
+                                out as 0 < Upsilon < tau (the FP32 path's relative error grows like 1/sqrt(Upsilon));
+                                selection, compaction and scatter happen on the device, no host synchronisation.
+                                0 = off.  Not applied by sc_eval_segments / _components / _loglike / _adaptive.        */
+  SC_OPT_ESC_TAU_POLY_X1000 = 10,  /* tau x 1000 for the polynomial sin/cos flavour (default 6000)                    */
+  SC_OPT_ESC_TAU_MUFU_X1000 = 11   /* tau x 1000 for the hardware sin/cos flavour (default 16000)                     */
 };
 
 /* Kernel classes of sc_get_timing. */
 enum { SC_TIME_NODES = 0, SC_TIME_DENSE = 1, SC_TIME_STITCH = 2, SC_TIME_PSO = 3, SC_TIME_OTHER = 4,
-       SC_N_TIMING_CLASSES = 5 };
+       SC_TIME_ESC = 5 /* every kernel of the escalation pass (SC_OPT_ESCALATE) */, SC_N_TIMING_CLASSES = 6 };
 
 /* a0 -- data whitening, once per data stream (PSD known; Eq. 1 weights).
  * dA_ri, dE_ri: DEVICE, interleaved (re, im) FP64, n_bins complex each.  S_A, S_E: DEVICE, one-sided PSD, n_bins.

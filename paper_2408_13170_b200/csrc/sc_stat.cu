@@ -119,8 +119,14 @@ __global__ void k_fill(double* __restrict__ x, long long n, double v) {
 // ------------------------------------------------------------------------------------------------ a1 + a3
 __global__ void k_particle_consts(DevCfg c, const double* __restrict__ params, int P, int P_pad,
                                   double* __restrict__ pc, int* __restrict__ jlo_out, int* __restrict__ jhi_out,
-                                  int e_first, int e_last, unsigned long long* __restrict__ eval_bins) {
-  const int p = blockIdx.x * blockDim.x + threadIdx.x;
+                                  int e_first, int e_last, unsigned long long* __restrict__ eval_bins,
+                                  const int* __restrict__ esc_count = nullptr, int esc_pb = 0) {
+  // escalation pass: the number of particles is known on the device only; the launched blocks stride over the
+  // 128-particle blocks below it (the grid is sized from a host-side hint, correctness does not depend on it)
+  if (esc_count) P = min(P, *esc_count - esc_pb);
+  for (int pblk = blockIdx.x; ; pblk += gridDim.x) {
+  if (esc_count && pblk * (int)blockDim.x >= P) return;
+  const int p = pblk * blockDim.x + threadIdx.x;
   if (p >= P_pad) return;
   int jlo = 0, jhi = 0;
   Particle q = {};
@@ -161,7 +167,7 @@ __global__ void k_particle_consts(DevCfg c, const double* __restrict__ params, i
       }
     }
     const int a = max(jlo, e_first), b = min(jhi, e_last);
-    if (b > a) atomicAdd(eval_bins, (unsigned long long)(b - a));
+    if (b > a && eval_bins) atomicAdd(eval_bins, (unsigned long long)(b - a));
   }
   pc[PC_PIM * (size_t)P_pad + p] = q.piM;       pc[PC_ETA * (size_t)P_pad + p] = q.eta;
   pc[PC_TC * (size_t)P_pad + p] = q.tc;         pc[PC_TAU_HI * (size_t)P_pad + p] = q.tau_hi;
@@ -171,16 +177,22 @@ __global__ void k_particle_consts(DevCfg c, const double* __restrict__ params, i
   pc[PC_S2P * (size_t)P_pad + p] = q.s2p;       pc[PC_CI * (size_t)P_pad + p] = q.ci;
   pc[PC_ECC * (size_t)P_pad + p] = q.ecc;
   jlo_out[p] = jlo; jhi_out[p] = jhi;
+  if (!esc_count) return;
+  }
 }
 
 // ------------------------------------------------------------------------------------------------ a2
 // One thread per (node, particle), particle fastest -> coalesced [node][particle] tables.
-template <typename R>
+template <typename R, bool ESC = false>
 __global__ void k_nodes(DevCfg c, const double* __restrict__ pc, const int* __restrict__ jlo, const int* __restrict__ jhi,
                         int P_pad, int* __restrict__ node_n, double* __restrict__ node_frac,
-                        R* __restrict__ node_amp /* [node][4][P_pad] */) {
-  const int p = blockIdx.y * blockDim.x + threadIdx.x;
+                        R* __restrict__ node_amp /* [node][4][P_pad] */, const int* __restrict__ esc_count = nullptr,
+                        int esc_pb = 0) {
   const int i = blockIdx.x;                       // 0 .. n_nodes-1  <->  node index i - kNodeOff
+  const int esc_lim = ESC ? min(*esc_count - esc_pb, P_pad) : 0;
+  for (int pblk = blockIdx.y; ; pblk += gridDim.y) {   // one pass, except in the escalation pass (see k_particle_consts)
+  if (ESC && pblk * (int)blockDim.x >= esc_lim) return;
+  const int p = pblk * blockDim.x + threadIdx.x;
   if (p >= P_pad) return;
   const long long pos = ((long long)i - kNodeOff) << c.log2_stride;   // bin position of the node
   const int lo = jlo[p], hi = jhi[p];
@@ -196,6 +208,8 @@ __global__ void k_nodes(DevCfg c, const double* __restrict__ pc, const int* __re
   node_frac[at] = o.frac;
   R* a = node_amp + (size_t)i * 4 * P_pad + p;
   a[0] = (R)o.Ar; a[(size_t)P_pad] = (R)o.Ai; a[2 * (size_t)P_pad] = (R)o.Er; a[3 * (size_t)P_pad] = (R)o.Ei;
+  if (!ESC) return;
+  }
 }
 
 // ------------------------------------------------------------------------------------------------ a4 + a5
@@ -254,11 +268,13 @@ struct DenseArgs {
   // k_dense2 only: pieces = fine sub-intervals cut at the segment edges, with the moments of the sigma weights
   const int* piece_first;      // [n_sub_launched + 1] first piece of each launched fine sub-interval
   const ulonglong2* moments;   // [n_pieces][4] = 8 packed (A, E) pairs: sum_j g_a(j) s_j^m, m = 0..6, pad
+  // escalation pass (k_dense only): device-side particle count and this batch's offset; nullptr otherwise
+  const int* esc_count; int esc_pb;
 };
 
 // All-FP64 flavour (few segments, N_seg < 8 by default): one bin per step, quintic phase by 5 forward differences,
 // FP64 polynomial sin/cos, FP64 amplitudes and accumulation.
-template <bool SEG>
+template <bool SEG, bool ESC = false>
 __global__ void __launch_bounds__(kBlock) k_dense(DevCfg c, DenseArgs a, const double4* __restrict__ Wg,
                                                   const double2* __restrict__ Gg) {
   using R = double;
@@ -272,10 +288,16 @@ __global__ void __launch_bounds__(kBlock) k_dense(DevCfg c, DenseArgs a, const d
   const int chunk_l = blockIdx.x;                              // launched-chunk index
   const int cs = (a.chunk_first + chunk_l) * CH;
   const int ce = min(cs + CH, c.n_bins);
-  const int p = blockIdx.y * kBlock + threadIdx.x;             // particle within the batch (P_pad is a multiple of kBlock)
+  const int esc_lim = ESC ? min(*a.esc_count - a.esc_pb, a.P_pad) : 0;
+  if (ESC && (int)(blockIdx.y * kBlock) >= esc_lim) return;
 
   for (int t = threadIdx.x; t < ce - cs; t += kBlock) { sW[t] = Wg[cs + t]; sG[t] = Gg[cs + t]; }
   __syncthreads();
+
+  // one pass over the block's 128 particles; in the escalation pass the blocks stride over the selected particles
+  for (int pblk = blockIdx.y; ; pblk += gridDim.y) {
+  if (ESC && pblk * kBlock >= esc_lim) return;
+  const int p = pblk * kBlock + threadIdx.x;                   // particle within the batch (P_pad is a multiple of kBlock)
 
   const int jlo = a.jlo[p], jhi = a.jhi[p];
   const int S = c.stride, Sf = S >> 2;
@@ -438,6 +460,8 @@ __global__ void __launch_bounds__(kBlock) k_dense(DevCfg c, DenseArgs a, const d
   if (!SEG) {
     frag[0] = ups;
     if (a.comp) { frag[(size_t)7 * a.P_pad] = xs; frag[(size_t)8 * a.P_pad] = hs; }
+  }
+  if (!ESC) return;
   }
 }
 
@@ -1067,30 +1091,46 @@ __global__ void k_stitch_ad(const double* __restrict__ frag, int n_chunks, int P
 // out[p] = Upsilon.  comp3 != nullptr: also comp3[p] = (Upsilon, X = sum_k |z_k| x_scale, H = sum_k sigma_k h_scale).
 __global__ void k_stitch(const double* __restrict__ frag, const uint8_t* __restrict__ flags, int n_chunks, int P_pad,
                          int P, double scale, double* __restrict__ out, double* __restrict__ comp3, double x_scale,
-                         double h_scale) {
-  const int p = blockIdx.x * blockDim.x + threadIdx.x;
-  if (p >= P) return;
+                         double h_scale, const int* __restrict__ esc_count = nullptr, int esc_pb = 0) {
+  if (esc_count) P = min(P, *esc_count - esc_pb);
+  for (int p = blockIdx.x * blockDim.x + threadIdx.x; p < P; p += gridDim.x * blockDim.x) {
   double ups = 0.0, zr = 0.0, zi = 0.0, sg = 0.0, xs = 0.0, hs = 0.0;
-  for (int cI = 0; cI < n_chunks; ++cI) {
-    const double* f = frag + (size_t)cI * kFragFields * P_pad + p;
-    const uint8_t fl = flags[cI];
-    if (fl & CF_HEAD) {
-      zr += f[(size_t)1 * P_pad]; zi += f[(size_t)2 * P_pad]; sg += f[(size_t)3 * P_pad];
-      if (fl & CF_HEAD_CLOSES) {
-        if (sg > 0.0) {
-          const double z2 = zr * zr + zi * zi;
-          ups += z2 / sg;
-          if (comp3) { xs += sqrt(z2); hs += sg; }
-        }
-        zr = 0.0; zi = 0.0; sg = 0.0;
-      }
+  // The walk is serial per particle (fixed order = bitwise reproducible); the loads are not: the fragments of kU chunks
+  // are fetched unconditionally (fields a chunk did not write are never used) before they are folded in.
+  constexpr int kU = 8;
+  for (int c0 = 0; c0 < n_chunks; c0 += kU) {
+    double v[kU][7], w7[kU], w8[kU];
+#pragma unroll
+    for (int u = 0; u < kU; ++u) {
+      const int cI = min(c0 + u, n_chunks - 1);
+      const double* f = frag + (size_t)cI * kFragFields * P_pad + p;
+#pragma unroll
+      for (int m = 0; m < 7; ++m) v[u][m] = f[(size_t)m * P_pad];
+      w7[u] = comp3 ? f[(size_t)7 * P_pad] : 0.0; w8[u] = comp3 ? f[(size_t)8 * P_pad] : 0.0;
     }
-    ups += f[0];
-    if (comp3) { xs += f[(size_t)7 * P_pad]; hs += f[(size_t)8 * P_pad]; }
-    if (fl & CF_TAIL) { zr = f[(size_t)4 * P_pad]; zi = f[(size_t)5 * P_pad]; sg = f[(size_t)6 * P_pad]; }
+#pragma unroll
+    for (int u = 0; u < kU; ++u) {
+      if (c0 + u >= n_chunks) break;
+      const uint8_t fl = flags[c0 + u];
+      if (fl & CF_HEAD) {
+        zr += v[u][1]; zi += v[u][2]; sg += v[u][3];
+        if (fl & CF_HEAD_CLOSES) {
+          if (sg > 0.0) {
+            const double z2 = zr * zr + zi * zi;
+            ups += z2 / sg;
+            if (comp3) { xs += sqrt(z2); hs += sg; }
+          }
+          zr = 0.0; zi = 0.0; sg = 0.0;
+        }
+      }
+      ups += v[u][0];
+      if (comp3) { xs += w7[u]; hs += w8[u]; }
+      if (fl & CF_TAIL) { zr = v[u][4]; zi = v[u][5]; sg = v[u][6]; }
+    }
   }
   if (out) out[p] = ups * scale;
   if (comp3) { comp3[3 * (size_t)p] = ups * scale; comp3[3 * (size_t)p + 1] = xs * x_scale; comp3[3 * (size_t)p + 2] = hs * h_scale; }
+  }
 }
 
 __global__ void k_stitch_seg(const double* __restrict__ frag, const uint8_t* __restrict__ flags,
@@ -1400,6 +1440,42 @@ __global__ void k_streams_finish(const double2* __restrict__ zpart, const double
 // The hardware sin/cos (MUFU) used by the fast FP32 path has a small systematic gain: <cos^2 + sin^2> over uniformly
 // distributed angles is not exactly 1.  It is measured once per handle with the very instruction sequence of the
 // dense kernel (2^20 equispaced angles, fixed-order reduction => deterministic) and divided out of Upsilon.
+// ------------------------------------------------------------------------------------------------ escalation
+// Particles whose FP32-path statistic is below tau (0 < Upsilon < tau): ascending index list, count and gathered
+// parameter rows.  One CTA of 1024 threads scans the population in order (deterministic).
+__global__ void __launch_bounds__(1024) k_esc_select(const double* __restrict__ ups, const double* __restrict__ params, int P,
+                                                     double tau, int* __restrict__ idx, int* __restrict__ count,
+                                                     double* __restrict__ params_c) {
+  __shared__ int wsum[32];
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  int base = 0;
+  for (int t0 = 0; t0 < P; t0 += 1024) {
+    const int p = t0 + threadIdx.x;
+    const double u = (p < P) ? ups[p] : 0.0;
+    const bool f = (u > 0.0) && (u < tau);
+    const unsigned b = __ballot_sync(0xffffffffu, f);
+    if (lane == 0) wsum[w] = __popc(b);
+    __syncthreads();
+    int off = 0, tot = 0;
+#pragma unroll
+    for (int i = 0; i < 32; ++i) { const int v = wsum[i]; off += (i < w) ? v : 0; tot += v; }
+    if (f) {
+      const int at = base + off + __popc(b & ((1u << lane) - 1u));
+      idx[at] = p;
+#pragma unroll
+      for (int i = 0; i < 8; ++i) params_c[(size_t)at * 8 + i] = params[(size_t)p * 8 + i];
+    }
+    base += tot;
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) *count = base;
+}
+__global__ void k_esc_scatter(const int* __restrict__ idx, const int* __restrict__ count, const double* __restrict__ ups_c,
+                              double* __restrict__ ups) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < *count) ups[idx[i]] = ups_c[i];
+}
+
 __global__ void k_mufu_gain(double* __restrict__ out) {
   __shared__ double sh[1024];
   double acc = 0.0;
@@ -1434,7 +1510,20 @@ thread_local std::string g_init_error;
 
 }  // namespace
 
-struct sc_handle {
+// The analysis of one edge list for one chunk length (host vectors + their device copies).  A handle keeps two: the one in
+// use and an alternate (the all-FP64 chunking of the same edges, used by the escalation pass), swapped by swap_edge_cache.
+struct EdgeCache {
+  int* d_edges = nullptr; int* d_chunk_k0 = nullptr; uint8_t* d_flags = nullptr; size_t edge_cap = 0, k0_cap = 0, flags_cap = 0;
+  // cached edge analysis
+  std::vector<int> edges; int cached_chunk = 0; int chunk_first = 0, n_chunks = 0;
+  std::vector<int> chunk_k0; std::vector<uint8_t> flags;
+  // pieces (fine sub-intervals cut at the edges) and their sigma moments, for k_dense2; cached with the edges
+  int cached_lg = 0; int n_pieces = 0;
+  int* d_piece_first = nullptr; int* d_piece_lo = nullptr; int* d_piece_hi = nullptr; float2* d_moments = nullptr;
+  size_t pf_cap = 0, plo_cap = 0, phi_cap = 0, mom_cap = 0;
+};
+
+struct sc_handle : EdgeCache {
   sc_config cfg;
   DevCfg dc;
   int device = 0;
@@ -1442,7 +1531,7 @@ struct sc_handle {
   float4* D32 = nullptr; double4* W64 = nullptr; double2* G64 = nullptr;   // D32: bin-pair layout of k_dense2
   // options
   int precision = 0; int f32_min_seg = 8; size_t scratch_cap = (size_t)8 << 30;
-  double tc_max_s = 10.0 * 31557600.0; int forced_stride_log2 = 0; int sincos_mode = 0; int mufu_min_seg = 64;
+  double tc_max_s = 10.0 * 31557600.0; int forced_stride_log2 = 0; int sincos_mode = 0; int mufu_min_seg = 32;
   int lg_f32 = 5, lg_f64 = 5;      // log2 of the coarse node spacing per precision mode (set_stride)
   double mufu_gain2 = 1.0;        // <cos^2 + sin^2> of the hardware sin/cos, measured at init
   double dd = 0.0;                // <d|d> (Eq. 1), computed at init
@@ -1456,17 +1545,15 @@ struct sc_handle {
   int ad_lg = 0; float2* d_gmom = nullptr; float2* d_smom = nullptr; size_t gmom_cap = 0, smom_cap = 0;
   // scratch
   void* scratch = nullptr; size_t scratch_bytes = 0;
-  int* d_edges = nullptr; int* d_chunk_k0 = nullptr; uint8_t* d_flags = nullptr; size_t edge_cap = 0, k0_cap = 0, flags_cap = 0;
   unsigned long long* d_counter = nullptr;
   double* d_params_stage = nullptr; double* d_out_stage = nullptr; size_t stage_cap = 0;
-  // cached edge analysis
-  std::vector<int> edges; int cached_chunk = 0; int chunk_first = 0, n_chunks = 0;
-  std::vector<int> chunk_k0; std::vector<uint8_t> flags;
-  // pieces (fine sub-intervals cut at the edges) and their sigma moments, for k_dense2; cached with the edges
-  int cached_lg = 0; int n_pieces = 0;
-  int* d_piece_first = nullptr; int* d_piece_lo = nullptr; int* d_piece_hi = nullptr; float2* d_moments = nullptr;
-  size_t pf_cap = 0, plo_cap = 0, phi_cap = 0, mom_cap = 0;
   long long launches = 0;
+  EdgeCache alt;                   // see EdgeCache
+  // escalation: particles whose FP32-path Upsilon is below the mode's threshold are re-evaluated
+  // by the all-FP64 path; compacted index list, count, gathered parameters and their results
+  int escalate = 1; double esc_tau_poly = 6.0, esc_tau_mufu = 16.0;
+  int* d_esc_idx = nullptr; int* d_esc_count = nullptr; double* d_esc_params = nullptr; double* d_esc_out = nullptr;
+  size_t esc_idx_cap = 0, esc_cnt_cap = 0, esc_par_cap = 0, esc_out_cap = 0; int* h_esc_hint = nullptr;
   // three-channel handles (A, E, T): the T channel lives in a second handle whose first slot carries T (chan_set = 1)
   // and whose second slot is empty; the per-segment sums of both are added before |z|^2/sigma is formed
   sc_handle* sub = nullptr; double* d_seg3 = nullptr; size_t seg3_cap = 0;
@@ -1474,7 +1561,7 @@ struct sc_handle {
   bool profile = false;
   struct Ev { cudaEvent_t a, b; int cls; };
   std::vector<Ev> evs; size_t ev_used = 0;
-  double cls_ms[SC_N_TIMING_CLASSES] = {0, 0, 0, 0, 0}; long long cls_n[SC_N_TIMING_CLASSES] = {0, 0, 0, 0, 0};
+  double cls_ms[SC_N_TIMING_CLASSES] = {}; long long cls_n[SC_N_TIMING_CLASSES] = {};
   bool cuda_failed = false;
   std::string err;
 };
@@ -1589,7 +1676,11 @@ void analyse_edges(sc_handle* h, int CH) {
 
 template <typename R>
 int run_batches(sc_handle* h, const double* params, int64_t P, double* out, double* out_seg, double* out_comp,
-                cudaStream_t st, bool seg_mode) {
+                cudaStream_t st, bool seg_mode, const int* esc_count = nullptr, int esc_blocks = 0) {
+  // esc_count != nullptr: the escalation pass -- P is an upper bound, the number of particles sits on the device;
+  // its launches are timed as SC_TIME_ESC and do not count evaluated bins twice
+  const int cls_nodes = esc_count ? SC_TIME_ESC : SC_TIME_NODES, cls_dense = esc_count ? SC_TIME_ESC : SC_TIME_DENSE,
+            cls_stitch = esc_count ? SC_TIME_ESC : SC_TIME_STITCH;
   const int n_seg = (int)h->edges.size() - 1;
   DevCfg dc = h->dc;
   apply_stride(dc, sizeof(R) == 4 ? h->lg_f32 : h->lg_f64);
@@ -1623,12 +1714,14 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
   const double h0 = pow(dc.f_amp_ref, -7.0 / 6.0);
   const double sz = h->s0 * h0 / four_df, ss = h->s0 * h->s0 * h0 * h0 / four_df;
 
+  // particle blocks launched per kernel: all of them, or (escalation pass) the caller's estimate -- the kernels stride
+  const int pblocks = esc_count ? std::max(1, std::min(esc_blocks, P_pad / kBlock)) : P_pad / kBlock;
   for (int64_t pb = 0; pb < P; pb += P_pad) {
     const int Pn = (int)std::min<int64_t>(P_pad, P - pb);
     {
-      Timed tm(h, st, SC_TIME_NODES);
-      k_particle_consts<<<(P_pad + 127) / 128, 128, 0, st>>>(dc, params + pb * 8, Pn, P_pad, pc, jlo, jhi, e_first, e_last,
-                                                            h->d_counter);
+      Timed tm(h, st, cls_nodes);
+      k_particle_consts<<<pblocks, 128, 0, st>>>(dc, params + pb * 8, Pn, P_pad, pc, jlo, jhi, e_first, e_last,
+                                                            esc_count ? nullptr : h->d_counter, esc_count, (int)pb);
     }
     if ((rc = check_launch(h, "k_particle_consts"))) return rc;
     if (n_chunks == 0) {
@@ -1637,19 +1730,21 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
       continue;
     }
     {
-      Timed tm(h, st, SC_TIME_NODES);
-      k_nodes<R><<<dim3(n_nodes, (P_pad + 127) / 128), 128, 0, st>>>(dc, pc, jlo, jhi, P_pad, node_n, node_frac, node_amp);
+      Timed tm(h, st, cls_nodes);
+      if (esc_count) k_nodes<R, true><<<dim3(n_nodes, pblocks), 128, 0, st>>>(dc, pc, jlo, jhi, P_pad, node_n, node_frac, node_amp, esc_count, (int)pb);
+      else k_nodes<R, false><<<dim3(n_nodes, pblocks), 128, 0, st>>>(dc, pc, jlo, jhi, P_pad, node_n, node_frac, node_amp);
     }
     if ((rc = check_launch(h, "k_nodes"))) return rc;
-    DenseArgs a;
+    DenseArgs a = {};
+    a.esc_count = esc_count; a.esc_pb = (int)pb;
     a.edges = h->d_edges; a.n_seg = n_seg; a.chunk_first = h->chunk_first; a.chunk_k0 = h->d_chunk_k0;
     a.node_n = node_n; a.node_frac = node_frac; a.node_amp = node_amp; a.jlo = jlo; a.jhi = jhi; a.P_pad = P_pad;
     a.frag = frag; a.out_seg = seg_mode ? out_seg + (size_t)pb * n_seg * 3 : nullptr; a.P = Pn;
     a.seg_scale_z = sz; a.seg_scale_s = ss; a.comp = out_comp ? 1 : 0;
     a.piece_first = h->d_piece_first; a.moments = reinterpret_cast<const ulonglong2*>(h->d_moments);
-    const dim3 grid(n_chunks, P_pad / kBlock);
+    const dim3 grid(n_chunks, pblocks);
     {
-      Timed tm(h, st, SC_TIME_DENSE);
+      Timed tm(h, st, cls_dense);
       if (sizeof(R) == 4) {
         const ulonglong2* Dp = reinterpret_cast<const ulonglong2*>(h->D32);
         if (seg_mode) k_dense2<true, 0><<<grid, kBlock, 0, st>>>(dc, a, Dp);
@@ -1657,20 +1752,21 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
         else k_dense2<false, 0><<<grid, kBlock, 0, st>>>(dc, a, Dp);
       } else {
         if (seg_mode) k_dense<true><<<grid, kBlock, 0, st>>>(dc, a, h->W64, h->G64);
+        else if (esc_count) k_dense<false, true><<<grid, kBlock, 0, st>>>(dc, a, h->W64, h->G64);
         else k_dense<false><<<grid, kBlock, 0, st>>>(dc, a, h->W64, h->G64);
       }
     }
     if ((rc = check_launch(h, "k_dense"))) return rc;
-    Timed tm2(h, st, SC_TIME_STITCH);
+    Timed tm2(h, st, cls_stitch);
     if (seg_mode) k_stitch_seg<<<(Pn + 127) / 128, 128, 0, st>>>(frag, h->d_flags, h->d_chunk_k0, n_chunks, P_pad, Pn, n_seg, sz, ss,
                                                                 out_seg + (size_t)pb * n_seg * 3);
     else {
       // the hardware sin/cos gain g (g^2 = mufu_gain2) multiplies every |z_k|: Upsilon by g^2, O_hat by g, <h|h> not at all.
       // Units (whitened -> definition): Upsilon is scale free, x_k = 4 df |z_k| = |Z_k| s0 h0, [h|h]_k = Sg_k s0^2 h0^2.
       const double g2 = (sizeof(R) == 4 && sincos == 2) ? h->mufu_gain2 : 1.0;
-      k_stitch<<<(Pn + 127) / 128, 128, 0, st>>>(frag, h->d_flags, n_chunks, P_pad, Pn, 1.0 / g2, out ? out + pb : nullptr,
+      k_stitch<<<esc_count ? pblocks : (Pn + 127) / 128, 128, 0, st>>>(frag, h->d_flags, n_chunks, P_pad, Pn, 1.0 / g2, out ? out + pb : nullptr,
                                                  out_comp ? out_comp + pb * 3 : nullptr, h->s0 * h0 / sqrt(g2),
-                                                 h->s0 * h->s0 * h0 * h0);
+                                                 h->s0 * h->s0 * h0 * h0, esc_count, (int)pb);
     }
     if ((rc = check_launch(h, "k_stitch"))) return rc;
   }
@@ -1767,8 +1863,43 @@ int eval_common(sc_handle* h, const double* params, int64_t P, const int32_t* se
   if (rc) return rc;
   SC_CUDA(h, cudaMemsetAsync(h->d_counter, 0, 8, st));
   if (seg_mode) SC_CUDA(h, cudaMemsetAsync(out_seg, 0, (size_t)P * n_seg * 3 * 8, st));
-  return f64 ? run_batches<double>(h, params, P, out, out_seg, out_comp, st, seg_mode)
-             : run_batches<float>(h, params, P, out, out_seg, out_comp, st, seg_mode);
+  if (f64) return run_batches<double>(h, params, P, out, out_seg, out_comp, st, seg_mode);
+  if ((rc = run_batches<float>(h, params, P, out, out_seg, out_comp, st, seg_mode))) return rc;
+  // Escalation: the FP32 path's error is ~ c / sqrt(Upsilon) relative (c <= 1.0e-6 polynomial,
+  // 1.6e-6 hardware sin/cos, measured against the oracle), so a particle whose statistic comes out below tau is evaluated
+  // again by the all-FP64 path.  Device-side selection, no host synchronisation: the FP64 kernels are launched for the
+  // worst case and their 128-particle blocks beyond the selected count return at once.
+  if (h->escalate && h->precision == 0 && !seg_mode && out && !out_comp && h->n_chunks > 0) {
+    if (P > INT32_MAX / 16) return SC_OK;
+    const bool mufu = (h->sincos_mode == 0) ? (n_seg >= h->mufu_min_seg) : (h->sincos_mode == 2);
+    const size_t P_round = (size_t)((P + kBlock - 1) / kBlock * kBlock);
+    if ((rc = grow(h, (void**)&h->d_esc_idx, &h->esc_idx_cap, (size_t)P * 4))) return rc;
+    if ((rc = grow(h, (void**)&h->d_esc_count, &h->esc_cnt_cap, 256))) return rc;
+    if ((rc = grow(h, (void**)&h->d_esc_params, &h->esc_par_cap, P_round * 64))) return rc;
+    if ((rc = grow(h, (void**)&h->d_esc_out, &h->esc_out_cap, P_round * 8))) return rc;
+    {
+      Timed tm(h, st, SC_TIME_ESC);
+      k_esc_select<<<1, 1024, 0, st>>>(out, params, (int)P, mufu ? h->esc_tau_mufu : h->esc_tau_poly, h->d_esc_idx,
+                                       h->d_esc_count, h->d_esc_params);
+    }
+    if ((rc = check_launch(h, "k_esc_select"))) return rc;
+    // grid-size hint: the count of the latest selection whose copy has landed (possibly an earlier call's); the kernels
+    // stride over the selected particles, so a stale or low hint costs parallelism, never correctness
+    if (!h->h_esc_hint) { SC_CUDA(h, cudaMallocHost((void**)&h->h_esc_hint, 4)); *h->h_esc_hint = (int)std::min<int64_t>(P, 1024); }
+    const int hint = *(volatile int*)h->h_esc_hint;
+    SC_CUDA(h, cudaMemcpyAsync(h->h_esc_hint, h->d_esc_count, 4, cudaMemcpyDeviceToHost, st));
+    const int esc_blocks = (int)std::min<int64_t>((2LL * hint + kBlock - 1) / kBlock + 1, (int64_t)P_round / kBlock);
+    const std::vector<int> e_host = h->edges;                  // host copy: the alternate cache analyses the same list
+    std::swap(static_cast<EdgeCache&>(*h), h->alt);
+    rc = prepare_edges(h, e_host.data(), n_seg, kChunkF64, 0, st);
+    if (!rc) rc = run_batches<double>(h, h->d_esc_params, P, h->d_esc_out, nullptr, nullptr, st, false, h->d_esc_count, esc_blocks);
+    std::swap(static_cast<EdgeCache&>(*h), h->alt);
+    if (rc) return rc;
+    Timed tm(h, st, SC_TIME_ESC);
+    k_esc_scatter<<<(unsigned)((P + 127) / 128), 128, 0, st>>>(h->d_esc_idx, h->d_esc_count, h->d_esc_out, out);
+    if ((rc = check_launch(h, "k_esc_scatter"))) return rc;
+  }
+  return SC_OK;
 }
 
 // ------------------------------------------------------------------------------------------------ three channels (A, E, T)
@@ -2513,6 +2644,13 @@ int sc_set_option(sc_handle* h, int32_t option, int64_t value) {
     case SC_OPT_MUFU_MIN_SEG:
       if (value < 1) return fail(h, SC_ERR_INVALID_ARG, "mufu_min_seg must be >= 1");
       h->mufu_min_seg = (int)std::min<int64_t>(value, INT32_MAX); return SC_OK;
+    case SC_OPT_ESCALATE:
+      if (value < 0 || value > 1) return fail(h, SC_ERR_INVALID_ARG, "escalate must be 0 or 1");
+      h->escalate = (int)value; return SC_OK;
+    case SC_OPT_ESC_TAU_POLY_X1000:
+    case SC_OPT_ESC_TAU_MUFU_X1000:
+      if (value < 0) return fail(h, SC_ERR_INVALID_ARG, "escalation threshold must be >= 0");
+      (option == SC_OPT_ESC_TAU_POLY_X1000 ? h->esc_tau_poly : h->esc_tau_mufu) = (double)value * 1e-3; return SC_OK;
     case SC_OPT_SINCOS:
       if (value < 0 || value > 2) return fail(h, SC_ERR_INVALID_ARG, "sincos must be 0, 1 or 2");
       h->sincos_mode = (int)value; return SC_OK;
@@ -2536,6 +2674,10 @@ int sc_free(sc_handle* h) {
   cudaFree(h->d_counter); cudaFree(h->d_params_stage); cudaFree(h->d_comp); cudaFree(h->d_km); cudaFree(h->d_T64); cudaFree(h->d_T32); cudaFree(h->d_sp);
   cudaFree(h->d_spsig); cudaFree(h->d_zpart); cudaFree(h->d_hh); cudaFree(h->d_gmom); cudaFree(h->d_smom);
   cudaFree(h->d_piece_first); cudaFree(h->d_piece_lo); cudaFree(h->d_piece_hi); cudaFree(h->d_moments);
+  cudaFree(h->alt.d_edges); cudaFree(h->alt.d_chunk_k0); cudaFree(h->alt.d_flags);
+  cudaFree(h->alt.d_piece_first); cudaFree(h->alt.d_piece_lo); cudaFree(h->alt.d_piece_hi); cudaFree(h->alt.d_moments);
+  cudaFreeHost(h->h_esc_hint);
+  cudaFree(h->d_esc_idx); cudaFree(h->d_esc_count); cudaFree(h->d_esc_params); cudaFree(h->d_esc_out);
   for (auto& e : h->evs) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
   cudaGetLastError();
   delete h;

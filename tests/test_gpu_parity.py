@@ -101,6 +101,36 @@ def test_c1_hierarchy_levels_and_single_segment(c1, oracle, torch_cuda, sc):
         prev = (N, got)
 
 
+@pytest.mark.parametrize("N", [8, 10, 16, 32, 50])
+def test_escalation_of_ill_conditioned_particles(oracle, torch_cuda, sc, N):
+    """Automatic precision: the FP32 path's relative error grows like c / sqrt(Upsilon), so every
+    particle with 0 < Upsilon < tau is re-evaluated by the all-FP64 path on the device.  c2's population at the paper's
+    coarse rungs (N = 50, 10) has such particles: the bar must hold for all of them, an escalated particle
+    must carry exactly the all-FP64 value, every other one exactly the FP32 path's."""
+    inp = sy.config_inputs(2, P=384)
+    cfg, dA, dE = make_data(oracle, inp)
+    H = gpu_handle(inp, dA, dE)
+    e = sy.edges(inp["cfg"]["n_bins"], N)
+    par = _dev(torch_cuda, inp["particles"])
+    ref = oracle.eval_stat(cfg, dA, dE, inp["S_A"], inp["S_E"], inp["particles"], e)
+    auto = H.eval_stat(par, e).cpu().numpy()
+    auto2 = H.eval_stat(par, e).cpu().numpy()                 # second call: grid hint now known, same result
+    H.set_option(sc.SC_OPT_ESCALATE, 0)
+    plain = H.eval_stat(par, e).cpu().numpy()
+    H.set_option(sc.SC_OPT_PRECISION, 2)
+    f64 = H.eval_stat(par, e).cpu().numpy()
+    H.close()
+    tau = 16.0 if N >= 32 else 6.0
+    esc = (plain > 0) & (plain < tau)
+    assert np.array_equal(auto, auto2)
+    assert np.array_equal(auto[esc], f64[esc]) and np.array_equal(auto[~esc], plain[~esc])
+    ok = ref > 0
+    assert rel_err(auto[ok], ref[ok]).max() <= TOL
+    assert rel_err(auto[ok], ref[ok]).max() <= 6e-7           # design margin: c_max / sqrt(tau) <= 4.1e-7
+    if N <= 16:
+        assert esc.sum() > 0                                  # the case is exercised
+
+
 def test_c1_partial_and_empty_edges(c1, oracle, torch_cuda):
     inp, H = c1["inp"], c1["H"]
     nb = inp["cfg"]["n_bins"]
