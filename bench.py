@@ -67,6 +67,10 @@ def parse():
     ap.add_argument("--adaptive-nseg", type=int, default=0, metavar="N",
                     help="time the step with per-particle equal-SNR^2 segments (sc_eval_stat_adaptive, PAPER.md:120) and N "
                          "segments instead of the config's shared edges")
+    ap.add_argument("--search", type=float, default=0.0, metavar="RHO",
+                    help="extras: also run ONE complete hierarchical search (Fig. 2; sc_search_run) at the paper's scale on "
+                         "this config's tile -- 6 swarms x 10^4 particles (PAPER.md:167, 506), ladder N = 100/50/10/1, Table "
+                         "IV hyper-parameters, per-particle segments -- with the injection rescaled to SNR RHO; takes minutes")
     ap.add_argument("--no-extras", action="store_true", help="skip the extra (untimed-region) measurements")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -179,6 +183,46 @@ class ClockSampler:
         if sm:
             out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(np.max(mx)), reasons=sorted(reasons), samples=len(sm))
         return out
+
+
+def run_search(sc, torch, dev, inp, cid, rho, S_A, S_E, nA, nE, n_swarms=6, per_swarm=10000, max_iters=1000):
+    """One complete search of one tile (Fig. 2): init from the prior, ladder N = 100/50/10/1
+    with Table IV hyper-parameters, convergence rule of App. B, k-means regrouping between rungs, threshold Upsilon_1 >= 100."""
+    big = sy.config_inputs(cid, P=n_swarms * per_swarm)
+    cfg, nb = inp["cfg"], inp["cfg"]["n_bins"]
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    H0 = sc.Handle(cfg, torch.view_as_real(nA).contiguous(), torch.view_as_real(nE).contiguous(), S_A, S_E)
+    th = inp["injections"][0]["theta"]
+    hA, hE = H0.gen_template(t(th[None, :]))
+    rho2 = 4.0 * inp["df"] * ((hA[0].abs() ** 2 / S_A).sum() + (hE[0].abs() ** 2 / S_E).sum())
+    kappa = rho / torch.sqrt(rho2)
+    dA, dE = nA + kappa * hA[0], nE + kappa * hE[0]
+    H0.close()
+    H = sc.Handle(cfg, torch.view_as_real(dA).contiguous(), torch.view_as_real(dE).contiguous(), S_A, S_E)
+    H.set_option(sc.SC_OPT_TC_MAX_S, int(np.ceil(big["hi"][2])))
+    ladder = [100, 50, 10, 1]
+    hyper = [dict(sy.TABLE_IV[min(sy.TABLE_IV, key=lambda k: abs(np.log(k) - np.log(N)))]) for N in ladder]
+    scfg = sc.ScSearchConfig.make(ladder, hyper, adaptive_edges=True, max_iters_per_rung=max_iters, seed=2408, threshold=100.0)
+    pos, vel = t(big["particles"]), t(big["velocities"])
+    label = torch.from_numpy(np.repeat(np.arange(n_swarms, dtype=np.int32), per_swarm)).to(dev)
+    ups1_inj = H.eval_stat(t(th[None, :]), sy.edges(nb, 1).astype(np.int32)).item()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    res = H.search_run(scfg, pos, vel, label, n_swarms, t(big["lo"]), t(big["hi"]))
+    torch.cuda.synchronize()
+    wall = time.perf_counter() - t0
+    H.close()
+    b = int(np.argmax(res["best_val"]))
+    iters = [int(x) for x in res["iters_per_rung"]]
+    return {"what": f"sc_search_run on the c{cid} tile: {n_swarms} swarms x {per_swarm} particles, ladder {ladder}, per-particle "
+                    f"equal-SNR^2 segments, Table IV hyper-parameters, injection at SNR {rho}",
+            "wall_s": wall, "iters_per_rung": iters, "particle_bin_evals": float(sum(iters)) * n_swarms * per_swarm * nb,
+            "best_upsilon_1": float(res["best_val"][b]), "upsilon_1_at_injection": ups1_inj,
+            "swarms_above_threshold": int(np.sum(res["passed"])),
+            "best_minus_injected": {"Mc_msun": float(res["best_pos"][b, 0] - th[0]), "eta": float(res["best_pos"][b, 1] - th[1]),
+                                    "tc_s": float(res["best_pos"][b, 2] - th[2])},
+            "paper_context": "PAPER.md:365-367: ~1-2 days per search on 1 A100 + 10 CPU processes (other hardware, the authors' "
+                             "waveform/response code): context, not a like-for-like baseline"}
 
 
 def run_ours(args, rank, local_rank, world):
@@ -324,6 +368,10 @@ def run_ours(args, rank, local_rank, world):
             del Ws
         except (RuntimeError, sc.SCError) as ex:                                # e.g. not enough memory for the streams
             extras["streams_x_one_template"] = {"skipped": str(ex)[:200]}
+
+    # ---- extras (opt-in): one complete hierarchical search at the paper's scale (context for PAPER.md:365-367)
+    if args.search > 0 and rank == 0 and inp["injections"]:
+        extras["hierarchical_search"] = run_search(sc, torch, dev, inp, cid, args.search, S_A, S_E, nA, nE)
 
     # ---- e2e: the same step through the HOST-buffer entry point, copies inside the timed region
     e2e = None
