@@ -71,6 +71,8 @@ def parse():
                     help="extras: also run ONE complete hierarchical search (Fig. 2; sc_search_run) at the paper's scale on "
                          "this config's tile -- 6 swarms x 10^4 particles (PAPER.md:167, 506), ladder N = 100/50/10/1, Table "
                          "IV hyper-parameters, per-particle segments -- with the injection rescaled to SNR RHO; takes minutes")
+    ap.add_argument("--search-ranking", action="store_true",
+                    help="with --search: sc_search_config.ranking_precision = 1 (all rungs on the FP32 path, bests re-evaluated in FP64)")
     ap.add_argument("--no-extras", action="store_true", help="skip the extra (untimed-region) measurements")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -185,7 +187,7 @@ class ClockSampler:
         return out
 
 
-def run_search(sc, torch, dev, inp, cid, rho, S_A, S_E, nA, nE, n_swarms=6, per_swarm=10000, max_iters=1000):
+def run_search(sc, torch, dev, inp, cid, rho, S_A, S_E, nA, nE, n_swarms=6, per_swarm=10000, max_iters=1000, ranking=0):
     """One complete search of one tile (Fig. 2): init from the prior, ladder N = 100/50/10/1
     with Table IV hyper-parameters, convergence rule of App. B, k-means regrouping between rungs, threshold Upsilon_1 >= 100."""
     big = sy.config_inputs(cid, P=n_swarms * per_swarm)
@@ -202,7 +204,8 @@ def run_search(sc, torch, dev, inp, cid, rho, S_A, S_E, nA, nE, n_swarms=6, per_
     H.set_option(sc.SC_OPT_TC_MAX_S, int(np.ceil(big["hi"][2])))
     ladder = [100, 50, 10, 1]
     hyper = [dict(sy.TABLE_IV[min(sy.TABLE_IV, key=lambda k: abs(np.log(k) - np.log(N)))]) for N in ladder]
-    scfg = sc.ScSearchConfig.make(ladder, hyper, adaptive_edges=True, max_iters_per_rung=max_iters, seed=2408, threshold=100.0)
+    scfg = sc.ScSearchConfig.make(ladder, hyper, adaptive_edges=True, max_iters_per_rung=max_iters, seed=2408, threshold=100.0,
+                                    ranking_precision=ranking)
     pos, vel = t(big["particles"]), t(big["velocities"])
     label = torch.from_numpy(np.repeat(np.arange(n_swarms, dtype=np.int32), per_swarm)).to(dev)
     ups1_inj = H.eval_stat(t(th[None, :]), sy.edges(nb, 1).astype(np.int32)).item()
@@ -215,7 +218,7 @@ def run_search(sc, torch, dev, inp, cid, rho, S_A, S_E, nA, nE, n_swarms=6, per_
     b = int(np.argmax(res["best_val"]))
     iters = [int(x) for x in res["iters_per_rung"]]
     return {"what": f"sc_search_run on the c{cid} tile: {n_swarms} swarms x {per_swarm} particles, ladder {ladder}, per-particle "
-                    f"equal-SNR^2 segments, Table IV hyper-parameters, injection at SNR {rho}",
+                    f"equal-SNR^2 segments, Table IV hyper-parameters, injection at SNR {rho}, ranking_precision = {ranking}",
             "wall_s": wall, "iters_per_rung": iters, "particle_bin_evals": float(sum(iters)) * n_swarms * per_swarm * nb,
             "best_upsilon_1": float(res["best_val"][b]), "upsilon_1_at_injection": ups1_inj,
             "swarms_above_threshold": int(np.sum(res["passed"])),
@@ -371,7 +374,7 @@ def run_ours(args, rank, local_rank, world):
 
     # ---- extras (opt-in): one complete hierarchical search at the paper's scale (context for PAPER.md:365-367)
     if args.search > 0 and rank == 0 and inp["injections"]:
-        extras["hierarchical_search"] = run_search(sc, torch, dev, inp, cid, args.search, S_A, S_E, nA, nE)
+        extras["hierarchical_search"] = run_search(sc, torch, dev, inp, cid, args.search, S_A, S_E, nA, nE, ranking=int(args.search_ranking))
 
     # ---- e2e: the same step through the HOST-buffer entry point, copies inside the timed region
     e2e = None

@@ -210,6 +210,12 @@ typedef struct {
   int32_t kmeans_max_iters;             /* Lloyd iterations cap; 0 = no regrouping between rungs                       */
   double  threshold;                    /* 100: swarms whose final best reaches it are flagged (Fig. 2)  */
   uint64_t seed;                        /* PSO uniforms: Philox key; the iteration counter runs on across rungs        */
+  int32_t ranking_precision;            /* 0: every evaluation as sc_eval_stat (1e-6 per particle: all-FP64 below 8 segments,
+                                           escalation).  1: the swarm only has to be RANKED -- all rungs run the FP32-amplitude
+                                           path without escalation (relative error <= 1.6e-6/sqrt(Upsilon): < 2e-7 for anything
+                                           near the Upsilon_1 >= 100 threshold), about 3x faster on the N < 8 rungs; the
+                                           reported best_val are re-evaluated by the all-FP64 path at the end.            */
+  int32_t reserved_;                    /* 0 */
 } sc_search_config;
 /* For every rung N: { Upsilon_N(pos) for all particles; sc_pso_step_labeled } until every non-empty swarm satisfies
  * "best has not improved by more than conv_delta over conv_window iterations" (or max_iters_per_rung); personal bests

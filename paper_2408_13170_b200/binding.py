@@ -53,11 +53,11 @@ class ScSearchConfig(C.Structure):
                 ("eps_min", (C.c_double * 8) * SC_MAX_RUNGS),
                 ("adaptive_edges", C.c_int32), ("conv_window", C.c_int32), ("conv_delta", C.c_double),
                 ("max_iters_per_rung", C.c_int32), ("kmeans_max_iters", C.c_int32), ("threshold", C.c_double),
-                ("seed", C.c_uint64)]
+                ("seed", C.c_uint64), ("ranking_precision", C.c_int32), ("reserved_", C.c_int32)]
 
     @classmethod
     def make(cls, ladder, hyper, adaptive_edges=True, conv_window=50, conv_delta=2.0, max_iters_per_rung=1000,
-             kmeans_max_iters=100, threshold=100.0, seed=0):
+             kmeans_max_iters=100, threshold=100.0, seed=0, ranking_precision=0):
         """ladder: segment counts per rung; hyper: per rung a dict with omega, phi_p, phi_g, eps (8 values)."""
         c = cls()
         c.n_rungs = len(ladder)
@@ -69,6 +69,7 @@ class ScSearchConfig(C.Structure):
         c.adaptive_edges, c.conv_window, c.conv_delta = int(bool(adaptive_edges)), int(conv_window), float(conv_delta)
         c.max_iters_per_rung, c.kmeans_max_iters = int(max_iters_per_rung), int(kmeans_max_iters)
         c.threshold, c.seed = float(threshold), int(seed) & (2 ** 64 - 1)
+        c.ranking_precision, c.reserved_ = int(ranking_precision), 0
         return c
 
 

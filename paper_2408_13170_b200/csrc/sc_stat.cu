@@ -1476,6 +1476,12 @@ __global__ void k_esc_scatter(const int* __restrict__ idx, const int* __restrict
   if (i < *count) ups[idx[i]] = ups_c[i];
 }
 
+// gbest_val[s] = re-evaluated value, except for empty swarms (-inf stays)
+__global__ void k_keep_empty(double* __restrict__ gbest_val, const double* __restrict__ re, int S) {
+  const int s = threadIdx.x;
+  if (s < S && gbest_val[s] != -INFINITY) gbest_val[s] = re[s];
+}
+
 __global__ void k_mufu_gain(double* __restrict__ out) {
   __shared__ double sh[1024];
   double acc = 0.0;
@@ -2299,7 +2305,10 @@ int sc_search_run(sc_handle* h, const sc_search_config* sc, double* pos, double*
   std::vector<int32_t> e;
   int rc = SC_OK;
   uint64_t iter_global = 0;
-  auto cleanup = [&](int code) { cudaFree(buf); return code; };
+  // ranking precision (sc_search_config): force the FP32-amplitude path without escalation for the whole search
+  const int saved_precision = h->precision, saved_escalate = h->escalate;
+  if (sc->ranking_precision) { h->precision = 1; h->escalate = 0; }
+  auto cleanup = [&](int code) { h->precision = saved_precision; h->escalate = saved_escalate; cudaFree(buf); return code; };
 #define SC_S(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cleanup(fail(h, SC_ERR_CUDA, "%s failed: %s", #call, cudaGetErrorString(e_))); } while (0)
   SC_S(cudaMemsetAsync(gbest_pos, 0, (size_t)S * 8 * 8, st));
 
@@ -2347,6 +2356,16 @@ int sc_search_run(sc_handle* h, const sc_search_config* sc, double* pos, double*
       int32_t n_it = 0;
       if ((rc = sc_kmeans(h, pos, P, lo, hi, cent, S, sc->kmeans_max_iters, label, (int64_t*)cnt_d, &n_it, stream))) return cleanup(rc);
     }
+  }
+  if (sc->ranking_precision) {
+    // the reported bests are re-evaluated at full accuracy (all-FP64 path) at the swarm-best positions
+    const int N = sc->n_seg[sc->n_rungs - 1];
+    h->precision = 2;
+    if (sc->adaptive_edges && N > 1) rc = sc_eval_stat_adaptive(h, gbest_pos, S, N, stat, nullptr, nullptr, stream);
+    else rc = eval_any(h, gbest_pos, S, e.data(), N, stat, nullptr, stream, false);
+    if (rc) return cleanup(rc);
+    k_keep_empty<<<1, 128, 0, st>>>(gbest_val, stat, S);
+    if ((rc = check_launch(h, "k_keep_empty"))) return cleanup(rc);
   }
   // results: the bests of the last rung
   SC_S(cudaMemcpyAsync(best_val, gbest_val, (size_t)S * 8, cudaMemcpyDeviceToHost, st));

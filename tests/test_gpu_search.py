@@ -107,8 +107,8 @@ def _search_cfg(sc, ladder, adaptive, eps_scale=None, **kw):
     return sc.ScSearchConfig.make(ladder, hyper, adaptive_edges=adaptive, **kw)
 
 
-@pytest.mark.parametrize("adaptive", [True, False])
-def test_search_run_recovers_injection_c1(env, oracle, adaptive):
+@pytest.mark.parametrize("adaptive,ranking", [(True, 0), (False, 0), (True, 1)], ids=["adaptive", "shared", "adaptive-ranking"])
+def test_search_run_recovers_injection_c1(env, oracle, adaptive, ranking):
     """Config 1 (SNR 20 injection, 0.5 yr): a 3-swarm search down the paper's ladder.  The best Upsilon_1 must reach
     the injected rho^2 region, the convergence rule replayed by the oracle must reproduce the iteration counts, and
     the particle count is conserved through the regrouping."""
@@ -130,7 +130,9 @@ def test_search_run_recovers_injection_c1(env, oracle, adaptive):
     ladder = [100, 50, 10, 1]
     # Table IV's minimum velocities are sized for the paper's 3 Msun tile; scale them with the box
     eps_scale = np.where(hi - lo > 0, (hi2 - lo2) / np.where(hi - lo > 0, hi - lo, 1.0), 1.0)
-    cfg = _search_cfg(sc, ladder, adaptive, eps_scale=eps_scale, max_iters_per_rung=150, seed=2408, threshold=100.0)
+    # ranking = 1: all rungs on the FP32 path (the swarm is only ranked), reported bests re-evaluated in all-FP64
+    cfg = _search_cfg(sc, ladder, adaptive, eps_scale=eps_scale, max_iters_per_rung=150, seed=2408, threshold=100.0,
+                      ranking_precision=ranking)
     d_pos, d_vel, d_lab = _dev(torch, pos), _dev(torch, vel), _dev(torch, label)
     res = H.search_run(cfg, d_pos, d_vel, d_lab, S, _dev(torch, lo2), _dev(torch, hi2))
     # particle count conserved, labels valid
