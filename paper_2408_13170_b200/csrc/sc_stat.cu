@@ -1071,15 +1071,28 @@ __global__ void k_stitch_ad(const double* __restrict__ frag, int n_chunks, int P
       if (comp3) { xs += sqrt(z2); hs += sg; }
     }
   };
-  for (int cI = 0; cI < n_chunks; ++cI) {
-    const double* f = frag + (size_t)cI * kFragAd * P_pad + p;
-    zr += f[(size_t)1 * P_pad]; zi += f[(size_t)2 * P_pad]; sg += f[(size_t)3 * P_pad];
-    if (f[(size_t)7 * P_pad] != 0.0) {
-      finish();
-      zr = f[(size_t)4 * P_pad]; zi = f[(size_t)5 * P_pad]; sg = f[(size_t)6 * P_pad];
+  // serial fold in chunk order (bitwise reproducible), loads of kU chunks in flight (as in k_stitch)
+  constexpr int kU = 8;
+  for (int c0 = 0; c0 < n_chunks; c0 += kU) {
+    double v[kU][8], w8[kU], w9[kU];
+#pragma unroll
+    for (int u = 0; u < kU; ++u) {
+      const double* f = frag + (size_t)min(c0 + u, n_chunks - 1) * kFragAd * P_pad + p;
+#pragma unroll
+      for (int m = 0; m < 8; ++m) v[u][m] = f[(size_t)m * P_pad];
+      w8[u] = comp3 ? f[(size_t)8 * P_pad] : 0.0; w9[u] = comp3 ? f[(size_t)9 * P_pad] : 0.0;
     }
-    ups += f[0];
-    if (comp3) { xs += f[(size_t)8 * P_pad]; hs += f[(size_t)9 * P_pad]; }
+#pragma unroll
+    for (int u = 0; u < kU; ++u) {
+      if (c0 + u >= n_chunks) break;
+      zr += v[u][1]; zi += v[u][2]; sg += v[u][3];
+      if (v[u][7] != 0.0) {
+        finish();
+        zr = v[u][4]; zi = v[u][5]; sg = v[u][6];
+      }
+      ups += v[u][0];
+      if (comp3) { xs += w8[u]; hs += w9[u]; }
+    }
   }
   finish();                                     // the last segment closes at e_N = n_bins
   if (out) out[p] = ups * scale;
