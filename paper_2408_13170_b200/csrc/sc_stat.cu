@@ -549,9 +549,9 @@ __device__ __forceinline__ void sincos_frac32(int n, float& sr, float& cr) {
 // ---- pieces of the packed hot loop shared by k_dense2 (shared edges) and k_dense2_ad (per-particle edges) ----
 struct PhaseFD { double phi, d1, d2, d3; };   // phase in turns at the next bin and its forward differences (unit steps)
 __device__ __forceinline__ void phase_next_pair(PhaseFD& ph, int& n0, int& n1) {
-  n0 = __double2loint(ph.phi + 1572864.0);
+  n0 = __double2loint(ph.phi);
   ph.phi += ph.d1; ph.d1 += ph.d2; ph.d2 += ph.d3;
-  n1 = __double2loint(ph.phi + 1572864.0);
+  n1 = __double2loint(ph.phi);
   ph.phi += ph.d1; ph.d1 += ph.d2; ph.d2 += ph.d3;
 }
 __device__ __forceinline__ void phase_skip_pair(PhaseFD& ph) {
@@ -559,7 +559,10 @@ __device__ __forceinline__ void phase_skip_pair(PhaseFD& ph) {
   ph.phi += ph.d1; ph.d1 += ph.d2; ph.d2 += ph.d3;
 }
 __device__ __forceinline__ void phase_set(PhaseFD& ph, double p0, const double b[6]) {
-  ph.phi = p0;
+  // phi carries the bias 1.5 * 2^20: in that binade the unit in the last place is 2^-32 turn, so the low word of phi IS the
+  // fraction of a turn as an int32 -- no separate biasing add per bin.  Every step then rounds to 2^-32 turn (1.5e-9 rad): a
+  // random walk of < 1e-8 rad over a fine sub-interval (<= 512 steps), far below the FP32 amplitudes' 1e-7 per bin.
+  ph.phi = p0 + 1572864.0;
   ph.d1 = b[1] + b[2] + b[3];
   ph.d2 = 2.0 * b[2] + 6.0 * b[3];
   ph.d3 = 6.0 * b[3];
