@@ -71,6 +71,9 @@ def parse():
                     help="extras: also run ONE complete hierarchical search (Fig. 2; sc_search_run) at the paper's scale on "
                          "this config's tile -- 6 swarms x 10^4 particles (PAPER.md:167, 506), ladder N = 100/50/10/1, Table "
                          "IV hyper-parameters, per-particle segments -- with the injection rescaled to SNR RHO; takes minutes")
+    ap.add_argument("--fap", type=int, default=0, metavar="SEEDS",
+                    help="extras: run the c4 workload (BASELINE configs[3]: noise only, 10^4 particles x 200 PSO iterations at "
+                         "N = 50000/5000/500) over SEEDS noise realisations and report the maximum statistic per seed and level")
     ap.add_argument("--search-ranking", action="store_true",
                     help="with --search: sc_search_config.ranking_precision = 1 (all rungs on the FP32 path, bests re-evaluated in FP64)")
     ap.add_argument("--no-extras", action="store_true", help="skip the extra (untimed-region) measurements")
@@ -187,28 +190,38 @@ class ClockSampler:
         return out
 
 
-def run_search(sc, torch, dev, inp, cid, rho, S_A, S_E, nA, nE, n_swarms=6, per_swarm=10000, max_iters=1000, ranking=0):
-    """One complete search of one tile (Fig. 2): init from the prior, ladder N = 100/50/10/1
-    with Table IV hyper-parameters, convergence rule of App. B, k-means regrouping between rungs, threshold Upsilon_1 >= 100."""
+def run_search(sc, torch, dev, inp, cid, rho, S_A, S_E, nA, nE, max_iters=1000, ranking=0):
+    """One complete search of one tile (Fig. 2): init from the prior, the ladder with Table IV
+    hyper-parameters, convergence rule of App. B, k-means regrouping between rungs, threshold Upsilon_1 >= 100.
+    c5 (BASELINE configs[4]): its own 4 swarms x 10^4 particles, ladder 50000/5000/500/50/1 on shared equal-width edges, both
+    injections at their configured SNRs.  Any other config: the paper's set-up -- 6 swarms x 10^4 particles (PAPER.md:167,
+    506), ladder 100/50/10/1 with per-particle equal-SNR^2 segments, the injection rescaled to SNR rho."""
+    spec = sy.CONFIGS[cid]
+    if cid == 5:
+        n_swarms, per_swarm, ladder, adaptive = spec["n_swarms"], spec["P"] // spec["n_swarms"], list(spec["n_segs"]), False
+    else:
+        n_swarms, per_swarm, ladder, adaptive = 6, 10000, [100, 50, 10, 1], True
     big = sy.config_inputs(cid, P=n_swarms * per_swarm)
     cfg, nb = inp["cfg"], inp["cfg"]["n_bins"]
     t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
     H0 = sc.Handle(cfg, torch.view_as_real(nA).contiguous(), torch.view_as_real(nE).contiguous(), S_A, S_E)
-    th = inp["injections"][0]["theta"]
-    hA, hE = H0.gen_template(t(th[None, :]))
-    rho2 = 4.0 * inp["df"] * ((hA[0].abs() ** 2 / S_A).sum() + (hE[0].abs() ** 2 / S_E).sum())
-    kappa = rho / torch.sqrt(rho2)
-    dA, dE = nA + kappa * hA[0], nE + kappa * hE[0]
+    dA, dE, snrs = nA.clone(), nE.clone(), []
+    for inj in inp["injections"]:
+        hA, hE = H0.gen_template(t(inj["theta"][None, :]))
+        rho2 = 4.0 * inp["df"] * ((hA[0].abs() ** 2 / S_A).sum() + (hE[0].abs() ** 2 / S_E).sum())
+        snrs.append(float(inj["rho"] if cid == 5 else rho))
+        dA += snrs[-1] / torch.sqrt(rho2) * hA[0]
+        dE += snrs[-1] / torch.sqrt(rho2) * hE[0]
     H0.close()
     H = sc.Handle(cfg, torch.view_as_real(dA).contiguous(), torch.view_as_real(dE).contiguous(), S_A, S_E)
     H.set_option(sc.SC_OPT_TC_MAX_S, int(np.ceil(big["hi"][2])))
-    ladder = [100, 50, 10, 1]
     hyper = [dict(sy.TABLE_IV[min(sy.TABLE_IV, key=lambda k: abs(np.log(k) - np.log(N)))]) for N in ladder]
-    scfg = sc.ScSearchConfig.make(ladder, hyper, adaptive_edges=True, max_iters_per_rung=max_iters, seed=2408, threshold=100.0,
-                                    ranking_precision=ranking)
+    scfg = sc.ScSearchConfig.make(ladder, hyper, adaptive_edges=adaptive, max_iters_per_rung=max_iters, seed=2408, threshold=100.0,
+                                  ranking_precision=ranking)
     pos, vel = t(big["particles"]), t(big["velocities"])
     label = torch.from_numpy(np.repeat(np.arange(n_swarms, dtype=np.int32), per_swarm)).to(dev)
-    ups1_inj = H.eval_stat(t(th[None, :]), sy.edges(nb, 1).astype(np.int32)).item()
+    ths = np.stack([inj["theta"] for inj in inp["injections"]])
+    ups1_inj = H.eval_stat(t(ths), sy.edges(nb, ladder[-1]).astype(np.int32)).cpu().numpy()
     torch.cuda.synchronize()
     t0 = time.perf_counter()
     res = H.search_run(scfg, pos, vel, label, n_swarms, t(big["lo"]), t(big["hi"]))
@@ -216,16 +229,60 @@ def run_search(sc, torch, dev, inp, cid, rho, S_A, S_E, nA, nE, n_swarms=6, per_
     wall = time.perf_counter() - t0
     H.close()
     b = int(np.argmax(res["best_val"]))
+    near = int(np.argmin(np.abs(ths[:, 0] - res["best_pos"][b, 0])))          # the injection the best swarm sits on
     iters = [int(x) for x in res["iters_per_rung"]]
-    return {"what": f"sc_search_run on the c{cid} tile: {n_swarms} swarms x {per_swarm} particles, ladder {ladder}, per-particle "
-                    f"equal-SNR^2 segments, Table IV hyper-parameters, injection at SNR {rho}, ranking_precision = {ranking}",
+    return {"what": f"sc_search_run on the c{cid} tile: {n_swarms} swarms x {per_swarm} particles, ladder {ladder}, "
+                    + ("per-particle equal-SNR^2 segments" if adaptive else "shared equal-width segments")
+                    + f", Table IV hyper-parameters, injection SNRs {snrs}, ranking_precision = {ranking}",
             "wall_s": wall, "iters_per_rung": iters, "particle_bin_evals": float(sum(iters)) * n_swarms * per_swarm * nb,
-            "best_upsilon_1": float(res["best_val"][b]), "upsilon_1_at_injection": ups1_inj,
+            "best_val_per_swarm": [float(v) if np.isfinite(v) else None for v in res["best_val"]],
+            "best_upsilon": float(res["best_val"][b]), "upsilon_at_injections": [float(v) for v in ups1_inj],
             "swarms_above_threshold": int(np.sum(res["passed"])),
-            "best_minus_injected": {"Mc_msun": float(res["best_pos"][b, 0] - th[0]), "eta": float(res["best_pos"][b, 1] - th[1]),
-                                    "tc_s": float(res["best_pos"][b, 2] - th[2])},
+            "best_minus_injected": {"Mc_msun": float(res["best_pos"][b, 0] - ths[near, 0]),
+                                    "eta": float(res["best_pos"][b, 1] - ths[near, 1]),
+                                    "tc_s": float(res["best_pos"][b, 2] - ths[near, 2])},
             "paper_context": "PAPER.md:365-367: ~1-2 days per search on 1 A100 + 10 CPU processes (other hardware, the authors' "
                              "waveform/response code): context, not a like-for-like baseline"}
+
+
+def run_fap(sc, torch, dev, cid, n_seeds):
+    """The workload of BASELINE configs[3] (c4): noise-only data, 10^4 particles x 200 PSO iterations at every level, repeated
+    over noise seeds -> the background of the maximum statistic (the shape of PAPER.md:323, 333-349 at reduced size)."""
+    spec = sy.CONFIGS[cid]
+    hp, iters, out = spec["pso"], spec["pso"]["iters"], {N: [] for N in spec["n_segs"]}
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    ms, n_eval, frac = 0.0, 0, None
+    for r in range(n_seeds):
+        inp = sy.config_inputs(cid, replica=r)
+        P, nb = inp["particles"].shape[0], inp["cfg"]["n_bins"]
+        H = sc.Handle(inp["cfg"], torch.view_as_real(t(inp["noise_A"])).contiguous(),
+                      torch.view_as_real(t(inp["noise_E"])).contiguous(), t(inp["S_A"]), t(inp["S_E"]))
+        H.set_option(sc.SC_OPT_TC_MAX_S, int(np.ceil(inp["hi"][2])))
+        lo, hi, eps = t(inp["lo"]), t(inp["hi"]), t(np.array(hp["eps"], dtype=np.float64))
+        stat = torch.empty(P, dtype=torch.float64, device=dev)
+        for N in spec["n_segs"]:
+            e = inp["edges"][N].astype(np.int32)
+            st = dict(pos=t(inp["particles"]), vel=t(inp["velocities"]), pbest_pos=t(inp["particles"]),
+                      pbest_val=torch.full((P,), -np.inf, dtype=torch.float64, device=dev),
+                      gbest_pos=torch.zeros((1, 8), dtype=torch.float64, device=dev),
+                      gbest_val=torch.zeros(1, dtype=torch.float64, device=dev))
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            for it in range(iters):
+                H.eval_stat(st["pos"], e, out=stat)
+                H.pso_step(st, stat, lo, hi, eps, hp["omega"], hp["phi_p"], hp["phi_g"], inp["pso_seed"], it, 1)
+            b.record()
+            torch.cuda.synchronize()
+            ms += a.elapsed_time(b); n_eval += iters
+            out[N].append(float(st["gbest_val"].item()))
+            if frac is None:
+                frac = H.counters()[0] / (float(P) * nb)
+        H.close()
+    return {"what": f"c{cid}: noise only, {spec['P']} particles x {iters} PSO iterations per level, {n_seeds} noise seeds; "
+                    "max statistic found per seed and level",
+            "max_upsilon_per_seed": {str(N): v for N, v in out.items()},
+            "noise_mean_2N_eff": {str(N): 2.0 * N * frac for N in out}, "noise_sd_2sqrtN_eff": {str(N): 2.0 * (N * frac) ** 0.5 for N in out},
+            "ms_per_iteration": ms / max(n_eval, 1), "iterations": n_eval}
 
 
 def run_ours(args, rank, local_rank, world):
@@ -361,7 +418,7 @@ def run_ours(args, rank, local_rank, world):
             peak = float(peaks.get("hbm_gbs", 6650.0))
             gbs = D * nb * 16.0 / (z_ms * 1e-3) / 1e9
             extras["streams_x_one_template"] = {
-                "what": f"sc_eval_stat_streams: {D} FP32 streams x {nb} bins (c3 grid), N = 100, one template",
+                "what": f"sc_eval_stat_streams: {D} FP32 streams x {nb} bins (c{cid} grid), N = 100, one template",
                 "kernel": "k_streams_z<float4,float>", "kernel_ms_per_launch": z_ms,
                 "ms_per_eval_all_kernels": sum(v[0] for v in tms.values()) / reps,
                 "stream_bin_per_s": D * nb / (z_ms * 1e-3),
@@ -375,6 +432,8 @@ def run_ours(args, rank, local_rank, world):
     # ---- extras (opt-in): one complete hierarchical search at the paper's scale (context for PAPER.md:365-367)
     if args.search > 0 and rank == 0 and inp["injections"]:
         extras["hierarchical_search"] = run_search(sc, torch, dev, inp, cid, args.search, S_A, S_E, nA, nE, ranking=int(args.search_ranking))
+    if args.fap > 0 and rank == 0:
+        extras["false_alarm_background"] = run_fap(sc, torch, dev, 4, args.fap)
 
     # ---- e2e: the same step through the HOST-buffer entry point, copies inside the timed region
     e2e = None
