@@ -76,7 +76,11 @@ enum {
                                 selection, compaction and scatter happen on the device, no host synchronisation.
                                 0 = off.  Not applied by sc_eval_segments / _components / _loglike / _adaptive.        */
   SC_OPT_ESC_TAU_POLY_X1000 = 10,  /* tau x 1000 for the polynomial sin/cos flavour (default 6000)                    */
-  SC_OPT_ESC_TAU_MUFU_X1000 = 11   /* tau x 1000 for the hardware sin/cos flavour (default 16000)                     */
+  SC_OPT_ESC_TAU_MUFU_X1000 = 11,  /* tau x 1000 for the hardware sin/cos flavour (default 16000)                     */
+  SC_OPT_WINDOW_SORT = 12    /* 1 (default): each particle batch is processed in the order of the time-window starts (stable
+                                radix sort on the device), so that the 32 particles of a warp share their windows; results
+                                are bitwise reproducible for a given population and option set, but a particle's rounding
+                                (FP32 path: ~1e-8 relative) depends on which particles share its warp.  0 = input order.  */
 };
 
 /* Kernel classes of sc_get_timing. */

@@ -11,6 +11,8 @@
 #include "../../include/sc_stat.h"
 #include "sc_math.cuh"
 
+#include <cub/device/device_radix_sort.cuh>
+
 #include <algorithm>
 #include <climits>
 #include <cmath>
@@ -182,33 +184,47 @@ __global__ void k_particle_consts(DevCfg c, const double* __restrict__ params, i
 }
 
 // ------------------------------------------------------------------------------------------------ a2
-// One thread per (node, particle), particle fastest -> coalesced [node][particle] tables.
+// One thread per (node, particle), particle fastest -> coalesced [node][particle] tables; a CTA takes 128 particles and
+// a group of kNodesPerCta consecutive nodes (one CTA per node is launch-bound when most of the table is out of reach).
+constexpr int kNodesPerCta = 16;
 template <typename R, bool ESC = false>
 __global__ void k_nodes(DevCfg c, const double* __restrict__ pc, const int* __restrict__ jlo, const int* __restrict__ jhi,
                         int P_pad, int* __restrict__ node_n, double* __restrict__ node_frac,
                         R* __restrict__ node_amp /* [node][4][P_pad] */, const int* __restrict__ esc_count = nullptr,
-                        int esc_pb = 0) {
-  const int i = blockIdx.x;                       // 0 .. n_nodes-1  <->  node index i - kNodeOff
+                        int esc_pb = 0, int skip_unreached = 0) {
+  const int i_first = blockIdx.x * kNodesPerCta;            // nodes i_first .. i_last-1  <->  node index i - kNodeOff
+  const int i_last = min(i_first + kNodesPerCta, c.n_nodes);
   const int esc_lim = ESC ? min(*esc_count - esc_pb, P_pad) : 0;
   for (int pblk = blockIdx.y; ; pblk += gridDim.y) {   // one pass, except in the escalation pass (see k_particle_consts)
-  if (ESC && pblk * (int)blockDim.x >= esc_lim) return;
-  const int p = pblk * blockDim.x + threadIdx.x;
-  if (p >= P_pad) return;
-  const long long pos = ((long long)i - kNodeOff) << c.log2_stride;   // bin position of the node
-  const int lo = jlo[p], hi = jhi[p];
-  NodeOut o = {};
-  // nodes farther than the stencils reach from the particle's window are never read
-  const long long reach = 4LL << c.log2_stride;
-  if (hi > lo && pos >= (long long)lo - reach && pos <= (long long)hi + reach && c.j0 + pos > 0) {
-    const Particle q = load_particle(pc, P_pad, p);
-    o = eval_node(c, q, c.j0 + pos);
-  }
-  const size_t at = (size_t)i * P_pad + p;
-  node_n[at] = o.n_turns;
-  node_frac[at] = o.frac;
-  R* a = node_amp + (size_t)i * 4 * P_pad + p;
-  a[0] = (R)o.Ar; a[(size_t)P_pad] = (R)o.Ai; a[2 * (size_t)P_pad] = (R)o.Er; a[3 * (size_t)P_pad] = (R)o.Ei;
-  if (!ESC) return;
+    if (ESC && pblk * (int)blockDim.x >= esc_lim) return;
+    const int p = pblk * blockDim.x + threadIdx.x;
+    if (p >= P_pad) return;
+    const int lo = jlo[p], hi = jhi[p];
+    // nodes farther than the stencils reach from the particle's window are never read
+    const long long reach = 4LL << c.log2_stride;
+    const long long r_lo = (long long)lo - reach, r_hi = (long long)hi + reach;
+    // skip_unreached (k_dense / k_dense2 as consumers): a warp reads a node only where one of its particles' windows is
+    // within reach of it, and then for all its lanes -- so a block none of whose particles reaches the node need not write
+    // it at all (with the batch sorted by window start that is most of the table when the windows are short)
+    const long long g_lo = ((long long)i_first - kNodeOff) << c.log2_stride, g_hi = ((long long)i_last - 1 - kNodeOff) << c.log2_stride;
+    const bool group_reached = hi > lo && g_hi >= r_lo && g_lo <= r_hi;
+    if (!(skip_unreached && !__syncthreads_or(group_reached))) {
+      Particle q = {};
+      if (group_reached) q = load_particle(pc, P_pad, p);
+      for (int i = i_first; i < i_last; ++i) {
+        const long long pos = ((long long)i - kNodeOff) << c.log2_stride;   // bin position of the node
+        const bool reached = hi > lo && pos >= r_lo && pos <= r_hi && c.j0 + pos > 0;
+        if (skip_unreached && !__syncthreads_or(reached)) continue;
+        NodeOut o = {};
+        if (reached) o = eval_node(c, q, c.j0 + pos);
+        const size_t at = (size_t)i * P_pad + p;
+        node_n[at] = o.n_turns;
+        node_frac[at] = o.frac;
+        R* a = node_amp + (size_t)i * 4 * P_pad + p;
+        a[0] = (R)o.Ar; a[(size_t)P_pad] = (R)o.Ai; a[2 * (size_t)P_pad] = (R)o.Er; a[3 * (size_t)P_pad] = (R)o.Ei;
+      }
+    }
+    if (!ESC) return;
   }
 }
 
@@ -290,6 +306,15 @@ __global__ void __launch_bounds__(kBlock) k_dense(DevCfg c, DenseArgs a, const d
   const int ce = min(cs + CH, c.n_bins);
   const int esc_lim = ESC ? min(*a.esc_count - a.esc_pb, a.P_pad) : 0;
   if (ESC && (int)(blockIdx.y * kBlock) >= esc_lim) return;
+  if (!ESC) {                                                  // as in k_dense2: nothing of this block lives in this chunk
+    const int p0 = blockIdx.y * kBlock + threadIdx.x;
+    if (!__syncthreads_or((a.jhi[p0] > cs) && (a.jlo[p0] < ce))) {
+      double* fz = a.frag + (size_t)chunk_l * kFragFields * a.P_pad + p0;
+#pragma unroll
+      for (int m = 0; m < kFragFields; ++m) fz[(size_t)m * a.P_pad] = 0.0;
+      return;
+    }
+  }
 
   for (int t = threadIdx.x; t < ce - cs; t += kBlock) { sW[t] = Wg[cs + t]; sG[t] = Gg[cs + t]; }
   __syncthreads();
@@ -746,6 +771,15 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2(DevCfg c, Den
   const int ce2 = (ce + 1) & ~1;                               // pair-aligned end (data beyond n_bins is zero)
   const int p = blockIdx.y * kBlock + threadIdx.x;
 
+  // no particle of this block has its time window in this chunk (common once the batch is sorted by window start):
+  // leave empty fragments and skip the staging of the data
+  if (!__syncthreads_or((a.jhi[p] > cs) && (a.jlo[p] < ce))) {
+    double* fz = a.frag + (size_t)chunk_l * kFragFields * a.P_pad + p;
+#pragma unroll
+    for (int m = 0; m < kFragFields; ++m) fz[(size_t)m * a.P_pad] = 0.0;
+    return;
+  }
+
   {
     const ulonglong2* src = Dg + (size_t)(cs >> 1) * kPairRec;
 #pragma unroll 4
@@ -1107,9 +1141,13 @@ __global__ void k_stitch_ad(const double* __restrict__ frag, int n_chunks, int P
 // out[p] = Upsilon.  comp3 != nullptr: also comp3[p] = (Upsilon, X = sum_k |z_k| x_scale, H = sum_k sigma_k h_scale).
 __global__ void k_stitch(const double* __restrict__ frag, const uint8_t* __restrict__ flags, int n_chunks, int P_pad,
                          int P, double scale, double* __restrict__ out, double* __restrict__ comp3, double x_scale,
-                         double h_scale, const int* __restrict__ esc_count = nullptr, int esc_pb = 0) {
+                         double h_scale, const int* __restrict__ esc_count = nullptr, int esc_pb = 0,
+                         const int* __restrict__ pmap = nullptr) {
   if (esc_count) P = min(P, *esc_count - esc_pb);
-  for (int p = blockIdx.x * blockDim.x + threadIdx.x; p < P; p += gridDim.x * blockDim.x) {
+  // pmap != nullptr: slot p of the tables holds particle pmap[p] of the batch (window sort); all P_pad slots are visited
+  for (int p = blockIdx.x * blockDim.x + threadIdx.x; p < (pmap ? P_pad : P); p += gridDim.x * blockDim.x) {
+  const int q = pmap ? pmap[p] : p;
+  if (q >= P) continue;
   double ups = 0.0, zr = 0.0, zi = 0.0, sg = 0.0, xs = 0.0, hs = 0.0;
   // The walk is serial per particle (fixed order = bitwise reproducible); the loads are not: the fragments of kU chunks
   // are fetched unconditionally (fields a chunk did not write are never used) before they are folded in.
@@ -1144,8 +1182,8 @@ __global__ void k_stitch(const double* __restrict__ frag, const uint8_t* __restr
       if (fl & CF_TAIL) { zr = v[u][4]; zi = v[u][5]; sg = v[u][6]; }
     }
   }
-  if (out) out[p] = ups * scale;
-  if (comp3) { comp3[3 * (size_t)p] = ups * scale; comp3[3 * (size_t)p + 1] = xs * x_scale; comp3[3 * (size_t)p + 2] = hs * h_scale; }
+  if (out) out[q] = ups * scale;
+  if (comp3) { comp3[3 * (size_t)q] = ups * scale; comp3[3 * (size_t)q + 1] = xs * x_scale; comp3[3 * (size_t)q + 2] = hs * h_scale; }
   }
 }
 
@@ -1456,6 +1494,26 @@ __global__ void k_streams_finish(const double2* __restrict__ zpart, const double
 // The hardware sin/cos (MUFU) used by the fast FP32 path has a small systematic gain: <cos^2 + sin^2> over uniformly
 // distributed angles is not exactly 1.  It is measured once per handle with the very instruction sequence of the
 // dense kernel (2^20 equispaced angles, fixed-order reduction => deterministic) and divided out of Upsilon.
+// ------------------------------------------------------------------------------------------------ window sort
+// Lanes of a warp are particles; a warp works on a fine sub-interval as soon as ONE of its particles' time windows
+// (Q4) overlaps it.  Where the windows cover only part of the band (c5: ~25 %) particles in input order waste most of the
+// lanes, so each batch is processed in the order of the window starts j_lo (stable radix sort of (j_lo, index)):
+// k_gather_sorted re-orders the per-particle constants and windows, k_stitch scatters through the same map.
+__global__ void k_iota(int* __restrict__ v, int n) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) v[i] = i;
+}
+__global__ void k_gather_sorted(const int* __restrict__ map, int P_pad, const double* __restrict__ pc_u,
+                                const int* __restrict__ jlo_u, const int* __restrict__ jhi_u, double* __restrict__ pc,
+                                int* __restrict__ jlo, int* __restrict__ jhi) {
+  const int p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= P_pad) return;
+  const int q = map[p];
+#pragma unroll
+  for (int f = 0; f < kPcFields; ++f) pc[(size_t)f * P_pad + p] = pc_u[(size_t)f * P_pad + q];
+  jlo[p] = jlo_u[q]; jhi[p] = jhi_u[q];
+}
+
 // ------------------------------------------------------------------------------------------------ escalation
 // Particles whose FP32-path statistic is below tau (0 < Upsilon < tau): ascending index list, count and gathered
 // parameter rows.  One CTA of 1024 threads scans the population in order (deterministic).
@@ -1576,6 +1634,7 @@ struct sc_handle : EdgeCache {
   int escalate = 1; double esc_tau_poly = 6.0, esc_tau_mufu = 16.0;
   int* d_esc_idx = nullptr; int* d_esc_count = nullptr; double* d_esc_params = nullptr; double* d_esc_out = nullptr;
   size_t esc_idx_cap = 0, esc_cnt_cap = 0, esc_par_cap = 0, esc_out_cap = 0; int* h_esc_hint = nullptr;
+  int window_sort = 1; void* d_sort_tmp = nullptr; size_t sort_cap = 0;   // cub radix-sort workspace of the window sort
   // three-channel handles (A, E, T): the T channel lives in a second handle whose first slot carries T (chan_set = 1)
   // and whose second slot is empty; the per-segment sums of both are added before |z|^2/sigma is formed
   sc_handle* sub = nullptr; double* d_seg3 = nullptr; size_t seg3_cap = 0;
@@ -1709,8 +1768,8 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
   const int n_nodes = dc.n_nodes;
   const int n_chunks = h->n_chunks;
   // per-particle scratch bytes
-  const size_t per_p = (size_t)kPcFields * 8 + 8 /* jlo, jhi */ + (size_t)n_nodes * (4 + 8 + 4 * sizeof(R))
-                       + (size_t)std::max(n_chunks, 1) * kFragFields * 8;
+  const size_t per_p = 2 * ((size_t)kPcFields * 8 + 8) /* constants, jlo, jhi: unsorted + sorted */ + 16 /* sort keys, map */
+                       + (size_t)n_nodes * (4 + 8 + 4 * sizeof(R)) + (size_t)std::max(n_chunks, 1) * kFragFields * 8;
   int64_t Pb_max = (int64_t)(h->scratch_cap / per_p) / kBlock * kBlock;
   if (Pb_max < kBlock) Pb_max = kBlock;
   const int64_t P_round = (P + kBlock - 1) / kBlock * kBlock;
@@ -1727,7 +1786,24 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
   double* node_frac = (double*)take((size_t)n_nodes * 8 * P_pad);
   R* node_amp = (R*)take((size_t)n_nodes * 4 * sizeof(R) * P_pad);
   double* frag = (double*)take((size_t)std::max(n_chunks, 1) * kFragFields * 8 * P_pad);
+  // window sort (see k_gather_sorted): not in the segment-table mode (rows are addressed by particle) nor in the
+  // escalation pass (few particles, count on the device)
+  const bool sorted = h->window_sort && !seg_mode && !esc_count && P_pad > kBlock;
+  double* pc_u = (double*)take((size_t)kPcFields * 8 * P_pad);
+  int* jlo_u = (int*)take((size_t)4 * P_pad);
+  int* jhi_u = (int*)take((size_t)4 * P_pad);
+  int* key_s = (int*)take((size_t)4 * P_pad);
+  int* iota = (int*)take((size_t)4 * P_pad);
+  int* pmap = (int*)take((size_t)4 * P_pad);
   (void)base;
+  size_t sort_bytes = 0;
+  if (sorted) {
+    if (cub::DeviceRadixSort::SortPairs(nullptr, sort_bytes, jlo_u, key_s, iota, pmap, P_pad, 0, 32, st) != cudaSuccess)
+      return fail(h, SC_ERR_CUDA, "cub::DeviceRadixSort size query failed");
+    if ((rc = grow(h, &h->d_sort_tmp, &h->sort_cap, sort_bytes + 256))) return rc;
+    k_iota<<<(P_pad + 255) / 256, 256, 0, st>>>(iota, P_pad);
+    if ((rc = check_launch(h, "k_iota"))) return rc;
+  }
 
   const int e_first = h->edges.front(), e_last = h->edges.back();
   const double four_df = 4.0 / h->cfg.T_obs_s;
@@ -1742,10 +1818,19 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
     const int Pn = (int)std::min<int64_t>(P_pad, P - pb);
     {
       Timed tm(h, st, cls_nodes);
-      k_particle_consts<<<pblocks, 128, 0, st>>>(dc, params + pb * 8, Pn, P_pad, pc, jlo, jhi, e_first, e_last,
-                                                            esc_count ? nullptr : h->d_counter, esc_count, (int)pb);
+      k_particle_consts<<<pblocks, 128, 0, st>>>(dc, params + pb * 8, Pn, P_pad, sorted ? pc_u : pc, sorted ? jlo_u : jlo,
+                                                 sorted ? jhi_u : jhi, e_first, e_last,
+                                                 esc_count ? nullptr : h->d_counter, esc_count, (int)pb);
     }
     if ((rc = check_launch(h, "k_particle_consts"))) return rc;
+    if (sorted && n_chunks > 0) {
+      Timed tm(h, st, cls_nodes);
+      if (cub::DeviceRadixSort::SortPairs(h->d_sort_tmp, sort_bytes, jlo_u, key_s, iota, pmap, P_pad, 0, 32, st) != cudaSuccess)
+        return fail(h, SC_ERR_CUDA, "cub::DeviceRadixSort::SortPairs failed");
+      h->launches += 3;
+      k_gather_sorted<<<(P_pad + 127) / 128, 128, 0, st>>>(pmap, P_pad, pc_u, jlo_u, jhi_u, pc, jlo, jhi);
+      if ((rc = check_launch(h, "k_gather_sorted"))) return rc;
+    }
     if (n_chunks == 0) {
       if (!seg_mode && out) SC_CUDA(h, cudaMemsetAsync(out + pb, 0, (size_t)Pn * 8, st));
       if (out_comp) SC_CUDA(h, cudaMemsetAsync(out_comp + pb * 3, 0, (size_t)Pn * 24, st));
@@ -1753,8 +1838,8 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
     }
     {
       Timed tm(h, st, cls_nodes);
-      if (esc_count) k_nodes<R, true><<<dim3(n_nodes, pblocks), 128, 0, st>>>(dc, pc, jlo, jhi, P_pad, node_n, node_frac, node_amp, esc_count, (int)pb);
-      else k_nodes<R, false><<<dim3(n_nodes, pblocks), 128, 0, st>>>(dc, pc, jlo, jhi, P_pad, node_n, node_frac, node_amp);
+      if (esc_count) k_nodes<R, true><<<dim3((n_nodes + kNodesPerCta - 1) / kNodesPerCta, pblocks), 128, 0, st>>>(dc, pc, jlo, jhi, P_pad, node_n, node_frac, node_amp, esc_count, (int)pb);
+      else k_nodes<R, false><<<dim3((n_nodes + kNodesPerCta - 1) / kNodesPerCta, pblocks), 128, 0, st>>>(dc, pc, jlo, jhi, P_pad, node_n, node_frac, node_amp, nullptr, 0, 1);
     }
     if ((rc = check_launch(h, "k_nodes"))) return rc;
     DenseArgs a = {};
@@ -1786,9 +1871,9 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
       // the hardware sin/cos gain g (g^2 = mufu_gain2) multiplies every |z_k|: Upsilon by g^2, O_hat by g, <h|h> not at all.
       // Units (whitened -> definition): Upsilon is scale free, x_k = 4 df |z_k| = |Z_k| s0 h0, [h|h]_k = Sg_k s0^2 h0^2.
       const double g2 = (sizeof(R) == 4 && sincos == 2) ? h->mufu_gain2 : 1.0;
-      k_stitch<<<esc_count ? pblocks : (Pn + 127) / 128, 128, 0, st>>>(frag, h->d_flags, n_chunks, P_pad, Pn, 1.0 / g2, out ? out + pb : nullptr,
+      k_stitch<<<esc_count ? pblocks : ((sorted ? P_pad : Pn) + 127) / 128, 128, 0, st>>>(frag, h->d_flags, n_chunks, P_pad, Pn, 1.0 / g2, out ? out + pb : nullptr,
                                                  out_comp ? out_comp + pb * 3 : nullptr, h->s0 * h0 / sqrt(g2),
-                                                 h->s0 * h->s0 * h0 * h0, esc_count, (int)pb);
+                                                 h->s0 * h->s0 * h0 * h0, esc_count, (int)pb, sorted ? pmap : nullptr);
     }
     if ((rc = check_launch(h, "k_stitch"))) return rc;
   }
@@ -2034,7 +2119,7 @@ int run_adaptive(sc_handle* h, const double* params, int64_t P, int n_seg, doubl
     if ((rc = check_launch(h, "k_particle_consts"))) return rc;
     {
       Timed tm(h, st, SC_TIME_NODES);
-      k_nodes<float><<<dim3(n_nodes, (P_pad + 127) / 128), 128, 0, st>>>(dc, pc, jlo, jhi, P_pad, node_n, node_frac, node_amp);
+      k_nodes<float><<<dim3((n_nodes + kNodesPerCta - 1) / kNodesPerCta, (P_pad + 127) / 128), 128, 0, st>>>(dc, pc, jlo, jhi, P_pad, node_n, node_frac, node_amp);
     }
     if ((rc = check_launch(h, "k_nodes"))) return rc;
     DenseArgs a = {};
@@ -2520,7 +2605,7 @@ int sc_gen_template(sc_handle* h, const double* params, int64_t P, double* hA, d
     const int Pn = (int)std::min<int64_t>(P_pad, P - pb);
     k_particle_consts<<<1, kBlock, 0, st>>>(dc, params + pb * 8, Pn, P_pad, pc, jlo, jhi, 0, 0, h->d_counter);
     if ((rc = check_launch(h, "k_particle_consts"))) return rc;
-    k_nodes<double><<<dim3(n_nodes, 1), kBlock, 0, st>>>(dc, pc, jlo, jhi, P_pad, node_n, node_frac, node_amp);
+    k_nodes<double><<<dim3((n_nodes + kNodesPerCta - 1) / kNodesPerCta, 1), kBlock, 0, st>>>(dc, pc, jlo, jhi, P_pad, node_n, node_frac, node_amp);
     if ((rc = check_launch(h, "k_nodes"))) return rc;
     k_template<<<dim3((dc.n_bins + 255) / 256, Pn), 256, 0, st>>>(dc, node_n, node_frac, node_amp, jlo, jhi, P_pad, Pn, h0,
                                                                  hA + (size_t)pb * dc.n_bins * 2, hE + (size_t)pb * dc.n_bins * 2);
@@ -2679,6 +2764,9 @@ int sc_set_option(sc_handle* h, int32_t option, int64_t value) {
     case SC_OPT_MUFU_MIN_SEG:
       if (value < 1) return fail(h, SC_ERR_INVALID_ARG, "mufu_min_seg must be >= 1");
       h->mufu_min_seg = (int)std::min<int64_t>(value, INT32_MAX); return SC_OK;
+    case SC_OPT_WINDOW_SORT:
+      if (value < 0 || value > 1) return fail(h, SC_ERR_INVALID_ARG, "window_sort must be 0 or 1");
+      h->window_sort = (int)value; return SC_OK;
     case SC_OPT_ESCALATE:
       if (value < 0 || value > 1) return fail(h, SC_ERR_INVALID_ARG, "escalate must be 0 or 1");
       h->escalate = (int)value; return SC_OK;
@@ -2711,7 +2799,7 @@ int sc_free(sc_handle* h) {
   cudaFree(h->d_piece_first); cudaFree(h->d_piece_lo); cudaFree(h->d_piece_hi); cudaFree(h->d_moments);
   cudaFree(h->alt.d_edges); cudaFree(h->alt.d_chunk_k0); cudaFree(h->alt.d_flags);
   cudaFree(h->alt.d_piece_first); cudaFree(h->alt.d_piece_lo); cudaFree(h->alt.d_piece_hi); cudaFree(h->alt.d_moments);
-  cudaFreeHost(h->h_esc_hint);
+  cudaFreeHost(h->h_esc_hint); cudaFree(h->d_sort_tmp);
   cudaFree(h->d_esc_idx); cudaFree(h->d_esc_count); cudaFree(h->d_esc_params); cudaFree(h->d_esc_out);
   for (auto& e : h->evs) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
   cudaGetLastError();

@@ -131,6 +131,37 @@ def test_escalation_of_ill_conditioned_particles(oracle, torch_cuda, sc, N):
         assert esc.sum() > 0                                  # the case is exercised
 
 
+def test_window_sort_is_a_pure_reordering(oracle, torch_cuda, sc):
+    """SC_OPT_WINDOW_SORT: batches are processed in the order of the window starts.  Against the oracle nothing changes;
+    against the input order only the rounding of the FP32 path does (the sigma of a sub-interval comes from the weight
+    moments when all 32 particles of the warp are inside their windows, from the per-bin sum otherwise); the all-FP64
+    path has one formula and is bit-identical either way.  Re-running and re-batching in input order is bitwise stable."""
+    inp = sy.config_inputs(2, P=640)
+    cfg, dA, dE = make_data(oracle, inp)
+    H = gpu_handle(inp, dA, dE)
+    par = _dev(torch_cuda, inp["particles"])
+    idx = _sample_idx(640, 48, 11)
+    for N in (100, 1):
+        e = sy.edges(inp["cfg"]["n_bins"], N)
+        ref = oracle.eval_stat(cfg, dA, dE, inp["S_A"], inp["S_E"], inp["particles"][idx], e)
+        H.set_option(sc.SC_OPT_WINDOW_SORT, 1)
+        a = H.eval_stat(par, e).cpu().numpy()
+        assert np.array_equal(a, H.eval_stat(par, e).cpu().numpy())
+        H.set_option(sc.SC_OPT_WINDOW_SORT, 0)
+        b = H.eval_stat(par, e).cpu().numpy()
+        H.set_option(sc.SC_OPT_SCRATCH_BYTES, 8 << 20)           # several batches, input order: same warps, same bits
+        c = H.eval_stat(par, e).cpu().numpy()
+        H.set_option(sc.SC_OPT_SCRATCH_BYTES, 8 << 30)
+        assert np.array_equal(b, c)
+        ok = ref > 0
+        assert rel_err(a[idx][ok], ref[ok]).max() <= TOL and rel_err(b[idx][ok], ref[ok]).max() <= TOL
+        if N == 1:
+            assert np.array_equal(a, b)
+        else:
+            assert rel_err(a[b > 0], b[b > 0]).max() <= 2e-7
+    H.close()
+
+
 def test_c1_partial_and_empty_edges(c1, oracle, torch_cuda):
     inp, H = c1["inp"], c1["H"]
     nb = inp["cfg"]["n_bins"]
