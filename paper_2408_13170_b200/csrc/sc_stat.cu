@@ -1142,7 +1142,9 @@ __global__ void k_stitch_ad(const double* __restrict__ frag, int n_chunks, int P
 __global__ void k_stitch(const double* __restrict__ frag, const uint8_t* __restrict__ flags, int n_chunks, int P_pad,
                          int P, double scale, double* __restrict__ out, double* __restrict__ comp3, double x_scale,
                          double h_scale, const int* __restrict__ esc_count = nullptr, int esc_pb = 0,
-                         const int* __restrict__ pmap = nullptr) {
+                         const int* __restrict__ pmap = nullptr, const int* __restrict__ jlo = nullptr,
+                         const int* __restrict__ jhi = nullptr, int chunk_first = 0, int chunk_len = 1,
+                         const int* __restrict__ next_close = nullptr) {
   if (esc_count) P = min(P, *esc_count - esc_pb);
   // pmap != nullptr: slot p of the tables holds particle pmap[p] of the batch (window sort); all P_pad slots are visited
   for (int p = blockIdx.x * blockDim.x + threadIdx.x; p < (pmap ? P_pad : P); p += gridDim.x * blockDim.x) {
@@ -1151,12 +1153,23 @@ __global__ void k_stitch(const double* __restrict__ frag, const uint8_t* __restr
   double ups = 0.0, zr = 0.0, zi = 0.0, sg = 0.0, xs = 0.0, hs = 0.0;
   // The walk is serial per particle (fixed order = bitwise reproducible); the loads are not: the fragments of kU chunks
   // are fetched unconditionally (fields a chunk did not write are never used) before they are folded in.
+  // Chunks that lie wholly outside the particle's time window hold empty fragments: only [c_lo, c_hi] is read; what
+  // the skipped chunks could still do is close the piece left open at c_hi (flags are shared by all particles).
+  int c_lo = 0, c_hi = n_chunks - 1;
+  if (jlo) {
+    const int lo = jlo[p], hi = jhi[p];
+    if (hi <= lo) { c_lo = 0; c_hi = -1; }
+    else {
+      c_lo = max(lo / chunk_len - chunk_first, 0);
+      c_hi = min((hi - 1) / chunk_len - chunk_first, n_chunks - 1);
+    }
+  }
   constexpr int kU = 8;
-  for (int c0 = 0; c0 < n_chunks; c0 += kU) {
+  for (int c0 = c_lo; c0 <= c_hi; c0 += kU) {
     double v[kU][7], w7[kU], w8[kU];
 #pragma unroll
     for (int u = 0; u < kU; ++u) {
-      const int cI = min(c0 + u, n_chunks - 1);
+      const int cI = min(c0 + u, c_hi);
       const double* f = frag + (size_t)cI * kFragFields * P_pad + p;
 #pragma unroll
       for (int m = 0; m < 7; ++m) v[u][m] = f[(size_t)m * P_pad];
@@ -1164,7 +1177,7 @@ __global__ void k_stitch(const double* __restrict__ frag, const uint8_t* __restr
     }
 #pragma unroll
     for (int u = 0; u < kU; ++u) {
-      if (c0 + u >= n_chunks) break;
+      if (c0 + u > c_hi) break;
       const uint8_t fl = flags[c0 + u];
       if (fl & CF_HEAD) {
         zr += v[u][1]; zi += v[u][2]; sg += v[u][3];
@@ -1181,6 +1194,12 @@ __global__ void k_stitch(const double* __restrict__ frag, const uint8_t* __restr
       if (comp3) { xs += w7[u]; hs += w8[u]; }
       if (fl & CF_TAIL) { zr = v[u][4]; zi = v[u][5]; sg = v[u][6]; }
     }
+  }
+  // the piece left open at c_hi runs on through empty chunks until one closes it (next_close, shared by all particles)
+  if (sg > 0.0 && next_close && c_hi >= 0 && c_hi < n_chunks - 1 && next_close[c_hi] >= 0) {
+    const double z2 = zr * zr + zi * zi;
+    ups += z2 / sg;
+    if (comp3) { xs += sqrt(z2); hs += sg; }
   }
   if (out) out[q] = ups * scale;
   if (comp3) { comp3[3 * (size_t)q] = ups * scale; comp3[3 * (size_t)q + 1] = xs * x_scale; comp3[3 * (size_t)q + 2] = hs * h_scale; }
@@ -1597,6 +1616,8 @@ struct EdgeCache {
   // cached edge analysis
   std::vector<int> edges; int cached_chunk = 0; int chunk_first = 0, n_chunks = 0;
   std::vector<int> chunk_k0; std::vector<uint8_t> flags;
+  // next_close[c]: the chunk in which a piece left open at the end of chunk c is closed (-1: it is not) -- for k_stitch
+  std::vector<int> next_close; int* d_next_close = nullptr; size_t nc_cap = 0;
   // pieces (fine sub-intervals cut at the edges) and their sigma moments, for k_dense2; cached with the edges
   int cached_lg = 0; int n_pieces = 0;
   int* d_piece_first = nullptr; int* d_piece_lo = nullptr; int* d_piece_hi = nullptr; float2* d_moments = nullptr;
@@ -1753,6 +1774,11 @@ void analyse_edges(sc_handle* h, int CH) {
     h->chunk_k0.push_back(k0);
     h->flags.push_back(fl);
   }
+  h->next_close.assign((size_t)h->n_chunks, -1);
+  for (int cI = h->n_chunks - 2; cI >= 0; --cI) {
+    const uint8_t fl = h->flags[(size_t)cI + 1];
+    if (fl & CF_HEAD) h->next_close[cI] = (fl & CF_HEAD_CLOSES) ? cI + 1 : h->next_close[(size_t)cI + 1];
+  }
 }
 
 template <typename R>
@@ -1873,7 +1899,8 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
       const double g2 = (sizeof(R) == 4 && sincos == 2) ? h->mufu_gain2 : 1.0;
       k_stitch<<<esc_count ? pblocks : ((sorted ? P_pad : Pn) + 127) / 128, 128, 0, st>>>(frag, h->d_flags, n_chunks, P_pad, Pn, 1.0 / g2, out ? out + pb : nullptr,
                                                  out_comp ? out_comp + pb * 3 : nullptr, h->s0 * h0 / sqrt(g2),
-                                                 h->s0 * h->s0 * h0 * h0, esc_count, (int)pb, sorted ? pmap : nullptr);
+                                                 h->s0 * h->s0 * h0 * h0, esc_count, (int)pb, sorted ? pmap : nullptr,
+                                                 jlo, jhi, h->chunk_first, sizeof(R) == 4 ? kChunkF32 : kChunkF64, h->d_next_close);
     }
     if ((rc = check_launch(h, "k_stitch"))) return rc;
   }
@@ -1950,10 +1977,12 @@ int prepare_edges(sc_handle* h, const int32_t* seg_edges, int32_t n_seg, int CH,
   if ((rc = grow(h, (void**)&h->d_edges, &h->edge_cap, h->edges.size() * 4))) return rc;
   if ((rc = grow(h, (void**)&h->d_chunk_k0, &h->k0_cap, (size_t)std::max(h->n_chunks, 1) * 4))) return rc;
   if ((rc = grow(h, (void**)&h->d_flags, &h->flags_cap, (size_t)std::max(h->n_chunks, 1)))) return rc;
+  if ((rc = grow(h, (void**)&h->d_next_close, &h->nc_cap, (size_t)std::max(h->n_chunks, 1) * 4))) return rc;
   SC_CUDA(h, cudaMemcpyAsync(h->d_edges, h->edges.data(), h->edges.size() * 4, cudaMemcpyHostToDevice, st));
   if (h->n_chunks > 0) {
     SC_CUDA(h, cudaMemcpyAsync(h->d_chunk_k0, h->chunk_k0.data(), (size_t)h->n_chunks * 4, cudaMemcpyHostToDevice, st));
     SC_CUDA(h, cudaMemcpyAsync(h->d_flags, h->flags.data(), (size_t)h->n_chunks, cudaMemcpyHostToDevice, st));
+    SC_CUDA(h, cudaMemcpyAsync(h->d_next_close, h->next_close.data(), (size_t)h->n_chunks * 4, cudaMemcpyHostToDevice, st));
   }
   return SC_OK;
 }
@@ -2797,7 +2826,7 @@ int sc_free(sc_handle* h) {
   cudaFree(h->d_counter); cudaFree(h->d_params_stage); cudaFree(h->d_comp); cudaFree(h->d_km); cudaFree(h->d_T64); cudaFree(h->d_T32); cudaFree(h->d_sp);
   cudaFree(h->d_spsig); cudaFree(h->d_zpart); cudaFree(h->d_hh); cudaFree(h->d_gmom); cudaFree(h->d_smom);
   cudaFree(h->d_piece_first); cudaFree(h->d_piece_lo); cudaFree(h->d_piece_hi); cudaFree(h->d_moments);
-  cudaFree(h->alt.d_edges); cudaFree(h->alt.d_chunk_k0); cudaFree(h->alt.d_flags);
+  cudaFree(h->alt.d_edges); cudaFree(h->alt.d_chunk_k0); cudaFree(h->alt.d_flags); cudaFree(h->alt.d_next_close); cudaFree(h->d_next_close);
   cudaFree(h->alt.d_piece_first); cudaFree(h->alt.d_piece_lo); cudaFree(h->alt.d_piece_hi); cudaFree(h->alt.d_moments);
   cudaFreeHost(h->h_esc_hint); cudaFree(h->d_sort_tmp);
   cudaFree(h->d_esc_idx); cudaFree(h->d_esc_count); cudaFree(h->d_esc_params); cudaFree(h->d_esc_out);
