@@ -4,7 +4,8 @@ import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(HERE, "csrc", "sc_stat.cu")
-DEPS = [SRC, os.path.join(HERE, "csrc", "sc_math.cuh"), os.path.join(HERE, "..", "include", "sc_stat.h")]
+DEPS = ([SRC, os.path.join(HERE, "..", "include", "sc_stat.h")]
+        + [os.path.join(HERE, "csrc", f) for f in sorted(os.listdir(os.path.join(HERE, "csrc"))) if f.endswith(".cuh")])
 LIB = os.path.join(HERE, "libscstat.so")
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

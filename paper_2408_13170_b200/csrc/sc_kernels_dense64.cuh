@@ -1,0 +1,270 @@
+// sc_kernels_dense64.cuh -- a4 + a5, all-FP64 flavour of the hot loop (few segments) and the shared DenseArgs.
+// Part of libscstat.so (one translation unit: sc_stat.cu includes the kernel files in pipeline order).
+#pragma once
+#include "sc_common.cuh"
+
+namespace {
+
+// ------------------------------------------------------------------------------------------------ a4 + a5
+// sin, cos of 2 pi x for |x| <= 1/8 turn (Taylor in x^2, coefficients (2 pi)^k / k!).
+__device__ __forceinline__ void sincos_2pi_small(float x, float& s, float& c) {
+  const float x2 = x * x;
+  float ps = fmaf(x2, 42.0586939448976531f, -76.7058597530613858f);  // (2pi)^9/9!, -(2pi)^7/7!
+  ps = fmaf(ps, x2, 81.6052492760750542f);                            // (2pi)^5/5!
+  ps = fmaf(ps, x2, -41.3417022403997602f);                           // -(2pi)^3/3!
+  ps = fmaf(ps, x2, 6.28318530717958648f);
+  s = ps * x;
+  float pc = fmaf(x2, -26.4262567833743975f, 60.2446413718766604f);  // -(2pi)^10/10!, (2pi)^8/8!
+  pc = fmaf(pc, x2, -85.4568172066937277f);                           // -(2pi)^6/6!
+  pc = fmaf(pc, x2, 64.9393940226682915f);                            // (2pi)^4/4!
+  pc = fmaf(pc, x2, -19.7392088021787172f);                           // -(2pi)^2/2!
+  c = fmaf(pc, x2, 1.0f);
+}
+__device__ __forceinline__ void sincos_2pi_small(double x, double& s, double& c) {
+  const double x2 = x * x;
+  double ps = fma(x2, -0.71812230177850051223, 3.8199525848482821277);     // -(2pi)^15/15!, (2pi)^13/13!
+  ps = fma(ps, x2, -15.094642576822990392);                                 // -(2pi)^11/11!
+  ps = fma(ps, x2, 42.058693944897653145);
+  ps = fma(ps, x2, -76.705859753061385842);
+  ps = fma(ps, x2, 81.605249276075054203);
+  ps = fma(ps, x2, -41.341702240399760234);
+  ps = fma(ps, x2, 6.2831853071795864769);
+  s = ps * x;
+  double pc = fma(x2, 0.28200596845579121507, -1.7143907110886720654);     // (2pi)^16/16!, -(2pi)^14/14!
+  pc = fma(pc, x2, 7.9035363713184688042);                                  // (2pi)^12/12!
+  pc = fma(pc, x2, -26.426256783374397453);
+  pc = fma(pc, x2, 60.244641371876660363);
+  pc = fma(pc, x2, -85.456817206693727736);
+  pc = fma(pc, x2, 64.939394022668291491);
+  pc = fma(pc, x2, -19.739208802178717238);
+  c = fma(pc, x2, 1.0);
+}
+
+template <typename R> struct DataT;
+template <> struct DataT<double> { using W = double4; using G = double2; static constexpr int chunk = kChunkF64; };
+
+struct DenseArgs {
+  const int* edges;            // [n_seg + 1]
+  int n_seg;
+  int chunk_first;             // first chunk launched (global chunk index)
+  const int* chunk_k0;         // [n_chunks_launched] last k with e_k <= chunk start (-1 .. n_seg)
+  const int* node_n;           // [n_nodes][P_pad]
+  const double* node_frac;
+  const void* node_amp;        // R [n_nodes][4][P_pad]
+  const int* jlo; const int* jhi;
+  int P_pad;
+  double* frag;                // [n_chunks_launched][kFragFields][P_pad]
+  double* out_seg;             // SEG mode: [P][n_seg][3] (already offset to this batch), else nullptr
+  int P;                       // particles in this batch
+  double seg_scale_z, seg_scale_s;
+  int comp;                    // also accumulate sum_k |z_k| and sum_k sigma_k (Eq. 8, 9 components)
+  // k_dense2 only: pieces = fine sub-intervals cut at the segment edges, with the moments of the sigma weights
+  const int* piece_first;      // [n_sub_launched + 1] first piece of each launched fine sub-interval
+  const ulonglong2* moments;   // [n_pieces][4] = 8 packed (A, E) pairs: sum_j g_a(j) s_j^m, m = 0..6, pad
+  // escalation pass (k_dense only): device-side particle count and this batch's offset; nullptr otherwise
+  const int* esc_count; int esc_pb;
+};
+
+// All-FP64 flavour (few segments, N_seg < 8 by default): one bin per step, quintic phase by 5 forward differences,
+// FP64 polynomial sin/cos, FP64 amplitudes and accumulation.
+template <bool SEG, bool ESC = false>
+__global__ void __launch_bounds__(kBlock) k_dense(DevCfg c, DenseArgs a, const double4* __restrict__ Wg,
+                                                  const double2* __restrict__ Gg) {
+  using R = double;
+  constexpr int SC = 0;
+  using WT = typename DataT<R>::W;
+  using GT = typename DataT<R>::G;
+  constexpr int CH = DataT<R>::chunk;
+  __shared__ WT sW[CH];
+  __shared__ GT sG[CH];
+
+  const int chunk_l = blockIdx.x;                              // launched-chunk index
+  const int cs = (a.chunk_first + chunk_l) * CH;
+  const int ce = min(cs + CH, c.n_bins);
+  const int esc_lim = ESC ? min(*a.esc_count - a.esc_pb, a.P_pad) : 0;
+  if (ESC && (int)(blockIdx.y * kBlock) >= esc_lim) return;
+  if (!ESC) {                                                  // as in k_dense2: nothing of this block lives in this chunk
+    const int p0 = blockIdx.y * kBlock + threadIdx.x;
+    if (!__syncthreads_or((a.jhi[p0] > cs) && (a.jlo[p0] < ce))) {
+      double* fz = a.frag + (size_t)chunk_l * kFragFields * a.P_pad + p0;
+#pragma unroll
+      for (int m = 0; m < kFragFields; ++m) fz[(size_t)m * a.P_pad] = 0.0;
+      return;
+    }
+  }
+
+  for (int t = threadIdx.x; t < ce - cs; t += kBlock) { sW[t] = Wg[cs + t]; sG[t] = Gg[cs + t]; }
+  __syncthreads();
+
+  // one pass over the block's 128 particles; in the escalation pass the blocks stride over the selected particles
+  for (int pblk = blockIdx.y; ; pblk += gridDim.y) {
+  if (ESC && pblk * kBlock >= esc_lim) return;
+  const int p = pblk * kBlock + threadIdx.x;                   // particle within the batch (P_pad is a multiple of kBlock)
+
+  const int jlo = a.jlo[p], jhi = a.jhi[p];
+  const int S = c.stride, Sf = S >> 2;
+  const R hS = R(1.0) / R(Sf);
+  const R* __restrict__ namp = reinterpret_cast<const R*>(a.node_amp);
+
+  int k = a.chunk_k0[chunk_l];
+  int next_edge = (k + 1 <= a.n_seg) ? a.edges[k + 1] : INT_MAX;
+  bool open_at_edge = (k >= 0 && k < a.n_seg) ? (a.edges[k] == cs) : true;
+  double Zr = 0.0, Zi = 0.0, Sg = 0.0, ups = 0.0, xs = 0.0, hs = 0.0;
+  double* frag = a.frag + (size_t)chunk_l * kFragFields * a.P_pad + p;
+
+  auto close_piece = [&](bool at_edge_end) {
+    // at_edge_end: the piece ends at e_{k+1}.  open_at_edge: it began at e_k.
+    if (open_at_edge && at_edge_end) {
+      if (SEG) {
+        if (p < a.P) {
+          double* o = a.out_seg + ((size_t)p * a.n_seg + k) * 3;
+          o[0] = Zr * a.seg_scale_z; o[1] = Zi * a.seg_scale_z; o[2] = Sg * a.seg_scale_s;
+        }
+      } else if (Sg > 0.0) {
+        const double z2 = Zr * Zr + Zi * Zi;
+        ups += z2 / Sg;
+        if (a.comp) { xs += sqrt(z2); hs += Sg; }
+      }
+    } else if (!open_at_edge) {          // began in an earlier chunk: head fragment (closed or running through)
+      frag[(size_t)1 * a.P_pad] = Zr; frag[(size_t)2 * a.P_pad] = Zi; frag[(size_t)3 * a.P_pad] = Sg;
+    } else {                             // began here, continues into the next chunk: tail fragment
+      frag[(size_t)4 * a.P_pad] = Zr; frag[(size_t)5 * a.P_pad] = Zi; frag[(size_t)6 * a.P_pad] = Sg;
+    }
+    Zr = 0.0; Zi = 0.0; Sg = 0.0;
+  };
+
+  int fd_pos = -1;                   // bin the forward-difference state is positioned at (-1: none)
+  double phi = 0.0, d1 = 0.0, d2 = 0.0, d3 = 0.0, d4 = 0.0, d5 = 0.0;
+  int quad = 0;
+  for (int ib = cs; ib < ce; ib += Sf) {
+    const int ie = min(ib + Sf, ce);
+    const bool lane_in = (ib >= jlo) && (ie <= jhi);
+    const bool lane_out = (ie <= jlo) || (ib >= jhi);
+    const bool all_in = __all_sync(0xffffffffu, lane_in);
+    const bool all_out = __all_sync(0xffffffffu, lane_out);
+
+    R cf[4][4];        // cubic coefficients of (Ar, Ai, Er, Ei) in t = (u - u_sub)/fine_stride
+    if (!all_out) {
+      const int ic = ib >> c.log2_stride;                      // coarse interval
+      const int i0 = ic + kNodeOff;                            // table row of its left node
+      const int q = (ib >> (c.log2_stride - 2)) & 3;           // fine sub-interval within the coarse one
+      if (fd_pos != ib || q == 0) {
+        // (re)build the phase forward differences at u0 = ib - ic*stride from the 6-node quintic
+        const size_t base = (size_t)i0 * a.P_pad + p;
+        const int n0 = a.node_n[base];
+        const double r0 = a.node_frac[base];
+        double Y[6];
+#pragma unroll
+        for (int m = -2; m <= 3; ++m) {
+          const size_t at = (size_t)(i0 + m) * a.P_pad + p;
+          Y[m + 2] = (double)(a.node_n[at] - n0) + (a.node_frac[at] - r0);
+        }
+        double b[6], d[6];
+        quintic_coeffs(Y, 1.0 / (double)S, b);
+        const int u0 = ib - (ic << c.log2_stride);
+        if (u0) taylor_shift(b, (double)u0);
+        forward_diffs(b, d);
+        phi = r0 + b[0]; d1 = d[1]; d2 = d[2]; d3 = d[3]; d4 = d[4]; d5 = d[5];
+        quad = 0;
+        fd_pos = ib;
+      }
+#pragma unroll
+      for (int r = 0; r < 4; ++r) {
+        const R* col = namp + ((size_t)i0 * 4 + r) * a.P_pad + p;
+        const ptrdiff_t st = (ptrdiff_t)4 * a.P_pad;
+        R nd[6];
+#pragma unroll
+        for (int m = -2; m <= 3; ++m) nd[m + 2] = col[m * st];
+        fine_cubic<R>(nd, q, cf[r][0], cf[r][1], cf[r][2], cf[r][3]);
+      }
+    }
+    R s = R(0.0);
+
+    // one bin: phase step + reduction (FP64), sincos, amplitude cubic, multiply-accumulate
+    auto bin = [&](int j, bool masked, R& zr, R& zi, R& sg) {
+      R cr, sr;
+      if (SC == 2 && sizeof(R) == 4) {
+        // The phase is never reduced in FP64: adding 1.5 * 2^20 leaves rint(phi * 2^32) mod 2^32 in the low word,
+        // i.e. the fraction of a turn in [-1/2, 1/2) as an int32; hardware sin/cos (MUFU) of that angle.
+        const int n = __double2loint(phi + 1572864.0);
+        const float xr = (float)n * 1.4629180792671596e-09f;          // 2 pi / 2^32
+        cr = (R)__cosf(xr); sr = (R)__sinf(xr);
+      } else {
+        // reduce phi to |x| <= 1/8 turn, carrying the quadrant
+        const double t = fma(phi, 4.0, kMagic);
+        quad += __double2loint(t);
+        const double kf = t - kMagic;
+        phi = fma(kf, -0.25, phi);
+        R sn, cn;
+        sincos_2pi_small((R)phi, sn, cn);
+        // rotate by quad * 90 degrees
+        const bool swp = quad & 1;
+        cr = swp ? sn : cn; sr = swp ? cn : sn;
+        cr = ((quad + 1) & 2) ? -cr : cr;
+        sr = (quad & 2) ? -sr : sr;
+      }
+      // advance the forward differences to the next bin
+      phi += d1; d1 += d2; d2 += d3; d3 += d4; d4 += d5;
+      // amplitudes
+      const R Ar = fma(fma(fma(cf[0][3], s, cf[0][2]), s, cf[0][1]), s, cf[0][0]);
+      const R Ai = fma(fma(fma(cf[1][3], s, cf[1][2]), s, cf[1][1]), s, cf[1][0]);
+      const R Er = fma(fma(fma(cf[2][3], s, cf[2][2]), s, cf[2][1]), s, cf[2][0]);
+      const R Ei = fma(fma(fma(cf[3][3], s, cf[3][2]), s, cf[3][1]), s, cf[3][0]);
+      s += hS;
+      const WT w = sW[j - cs];
+      const GT g = sG[j - cs];
+      // q = W_A conj(c_A) + W_E conj(c_E)
+      R qr = fma(w.x, Ar, fma(w.y, Ai, fma(w.z, Er, w.w * Ei)));
+      R qi = fma(w.y, Ar, fma(-w.x, Ai, fma(w.w, Er, -(w.z * Ei))));
+      R ss = fma(g.x, fma(Ar, Ar, Ai * Ai), g.y * fma(Er, Er, Ei * Ei));
+      if (masked) {
+        const bool in = (j >= jlo) && (j < jhi);
+        qr = in ? qr : R(0.0); qi = in ? qi : R(0.0); ss = in ? ss : R(0.0);
+      }
+      // z += q e^{+2 pi i Phi}
+      zr = fma(qr, cr, fma(-qi, sr, zr));
+      zi = fma(qr, sr, fma(qi, cr, zi));
+      sg += ss;
+    };
+
+    int j = ib;
+    while (j < ie) {
+      const int b = min(next_edge, ie);
+      const bool live = (k >= 0) && (k < a.n_seg);
+      if (b > j) {
+        if (all_out) {
+          // nothing to add; the forward-difference state is rebuilt at the next interval
+        } else if (!live) {
+          for (int jj = j; jj < b; ++jj) { phi += d1; d1 += d2; d2 += d3; d3 += d4; d4 += d5; s += hS; }
+          fd_pos = b;
+        } else {
+          for (int jj = j; jj < b;) {
+            const int e2 = min(jj + kFlushBins, b);
+            R zr = R(0.0), zi = R(0.0), sg = R(0.0);
+            if (all_in) { for (; jj < e2; ++jj) bin(jj, false, zr, zi, sg); }
+            else        { for (; jj < e2; ++jj) bin(jj, true, zr, zi, sg); }
+            Zr += (double)zr; Zi += (double)zi; Sg += (double)sg;
+          }
+          fd_pos = b;
+        }
+        j = b;
+      }
+      if (j == next_edge) {
+        if (live) close_piece(true);
+        ++k;
+        next_edge = (k + 1 <= a.n_seg) ? a.edges[k + 1] : INT_MAX;
+        open_at_edge = true;
+      }
+    }
+  }
+  // the piece still open at the chunk end
+  if (k >= 0 && k < a.n_seg) close_piece(false);
+  if (!SEG) {
+    frag[0] = ups;
+    if (a.comp) { frag[(size_t)7 * a.P_pad] = xs; frag[(size_t)8 * a.P_pad] = hs; }
+  }
+  if (!ESC) return;
+  }
+}
+
+}  // namespace
