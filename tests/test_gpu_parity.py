@@ -162,6 +162,36 @@ def test_window_sort_is_a_pure_reordering(oracle, torch_cuda, sc):
     H.close()
 
 
+def test_short_windows_skip_logic_c5(oracle, torch_cuda, sc):
+    """c5: every particle's time window covers a few per cent of the band, at its own place.  With the window sort most
+    (chunk, 128-particle block) CTAs and most (node, block) entries are skipped and k_stitch reads only the chunks of the
+    window; in input order nearly nothing is.  Both orders must give the same statistic for EVERY particle (bit for bit
+    on the all-FP64 path, to FP32 rounding otherwise), the components included, and the oracle's on a sample."""
+    inp = sy.config_inputs(5, P=1536)
+    cfg, dA, dE = make_data(oracle, inp)
+    H = gpu_handle(inp, dA, dE)
+    H.set_option(sc.SC_OPT_TC_MAX_S, int(np.ceil(inp["hi"][2])))
+    par = _dev(torch_cuda, inp["particles"])
+    idx = _sample_idx(1536, 6, 55)
+    for N in (500, 1):
+        e = sy.edges(inp["cfg"]["n_bins"], N)
+        ref = oracle.eval_stat(cfg, dA, dE, inp["S_A"], inp["S_E"], inp["particles"][idx], e)
+        res = {}
+        for srt in (1, 0):
+            H.set_option(sc.SC_OPT_WINDOW_SORT, srt)
+            res[srt] = (H.eval_stat(par, e).cpu().numpy(), H.eval_components(par, e).cpu().numpy())
+        a, b = res[1][0], res[0][0]
+        assert (a > 0).sum() > 1400
+        if N == 1:
+            assert np.array_equal(a, b) and np.array_equal(res[1][1], res[0][1])
+        else:
+            assert rel_err(a[b > 0], b[b > 0]).max() <= 2e-7
+            assert rel_err(res[1][1][:, 1:][b > 0], res[0][1][:, 1:][b > 0]).max() <= 2e-7
+        ok = ref > 0
+        assert rel_err(a[idx][ok], ref[ok]).max() <= TOL
+    H.close()
+
+
 def test_c1_partial_and_empty_edges(c1, oracle, torch_cuda):
     inp, H = c1["inp"], c1["H"]
     nb = inp["cfg"]["n_bins"]
