@@ -22,16 +22,15 @@ __device__ __forceinline__ void sincos_2pi_small(float x, float& s, float& c) {
 }
 __device__ __forceinline__ void sincos_2pi_small(double x, double& s, double& c) {
   const double x2 = x * x;
-  double ps = fma(x2, -0.71812230177850051223, 3.8199525848482821277);     // -(2pi)^15/15!, (2pi)^13/13!
-  ps = fma(ps, x2, -15.094642576822990392);                                 // -(2pi)^11/11!
+  // |x| <= 1/8 turn: the first omitted terms are (pi/4)^15/15! = 2e-14 (sin) and (pi/4)^16/16! = 1e-15 (cos)
+  double ps = fma(x2, 3.8199525848482821277, -15.094642576822990392);      // (2pi)^13/13!, -(2pi)^11/11!
   ps = fma(ps, x2, 42.058693944897653145);
   ps = fma(ps, x2, -76.705859753061385842);
   ps = fma(ps, x2, 81.605249276075054203);
   ps = fma(ps, x2, -41.341702240399760234);
   ps = fma(ps, x2, 6.2831853071795864769);
   s = ps * x;
-  double pc = fma(x2, 0.28200596845579121507, -1.7143907110886720654);     // (2pi)^16/16!, -(2pi)^14/14!
-  pc = fma(pc, x2, 7.9035363713184688042);                                  // (2pi)^12/12!
+  double pc = fma(x2, -1.7143907110886720654, 7.9035363713184688042);      // -(2pi)^14/14!, (2pi)^12/12!
   pc = fma(pc, x2, -26.426256783374397453);
   pc = fma(pc, x2, 60.244641371876660363);
   pc = fma(pc, x2, -85.456817206693727736);
