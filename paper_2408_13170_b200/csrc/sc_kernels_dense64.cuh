@@ -20,22 +20,22 @@ __device__ __forceinline__ void sincos_2pi_small(float x, float& s, float& c) {
   pc = fmaf(pc, x2, -19.7392088021787172f);                           // -(2pi)^2/2!
   c = fmaf(pc, x2, 1.0f);
 }
+// Taylor coefficients (2 pi)^k / k! in the constant bank: a DFMA takes them as c[bank][offset] operands (64-bit literals
+// would be rebuilt in uniform registers, two UMOV each, on every bin of the issue-bound all-FP64 loop).
+__constant__ double kSinC[7] = {3.8199525848482821277, -15.094642576822990392, 42.058693944897653145, -76.705859753061385842,
+                                81.605249276075054203, -41.341702240399760234, 6.2831853071795864769};   // x^13 .. x^1
+__constant__ double kCosC[7] = {-1.7143907110886720654, 7.9035363713184688042, -26.426256783374397453, 60.244641371876660363,
+                                -85.456817206693727736, 64.939394022668291491, -19.739208802178717238};  // x^14 .. x^2
 __device__ __forceinline__ void sincos_2pi_small(double x, double& s, double& c) {
   const double x2 = x * x;
   // |x| <= 1/8 turn: the first omitted terms are (pi/4)^15/15! = 2e-14 (sin) and (pi/4)^16/16! = 1e-15 (cos)
-  double ps = fma(x2, 3.8199525848482821277, -15.094642576822990392);      // (2pi)^13/13!, -(2pi)^11/11!
-  ps = fma(ps, x2, 42.058693944897653145);
-  ps = fma(ps, x2, -76.705859753061385842);
-  ps = fma(ps, x2, 81.605249276075054203);
-  ps = fma(ps, x2, -41.341702240399760234);
-  ps = fma(ps, x2, 6.2831853071795864769);
+  double ps = fma(x2, kSinC[0], kSinC[1]);
+#pragma unroll
+  for (int i = 2; i < 7; ++i) ps = fma(ps, x2, kSinC[i]);
   s = ps * x;
-  double pc = fma(x2, -1.7143907110886720654, 7.9035363713184688042);      // -(2pi)^14/14!, (2pi)^12/12!
-  pc = fma(pc, x2, -26.426256783374397453);
-  pc = fma(pc, x2, 60.244641371876660363);
-  pc = fma(pc, x2, -85.456817206693727736);
-  pc = fma(pc, x2, 64.939394022668291491);
-  pc = fma(pc, x2, -19.739208802178717238);
+  double pc = fma(x2, kCosC[0], kCosC[1]);
+#pragma unroll
+  for (int i = 2; i < 7; ++i) pc = fma(pc, x2, kCosC[i]);
   c = fma(pc, x2, 1.0);
 }
 
