@@ -51,7 +51,8 @@ constexpr int kPairRec = 3;
 // On a fine sub-interval the amplitudes are cubics in s, so |c_a(s)|^2 is a polynomial of degree 6 and
 // sigma_piece = sum_m (e_A,m M_A,m + e_E,m M_E,m) -- the per-bin evaluation of |h|^2 leaves the hot loop.
 __global__ void k_moments(const double2* __restrict__ G64, const int* __restrict__ piece_lo, const int* __restrict__ piece_hi,
-                          int n_pieces, int n_bins, int log2_fine, float2* __restrict__ out /* [n_pieces][8] */) {
+                          int n_pieces, int n_bins, int log2_fine, float2* __restrict__ out /* [n_pieces][8] */,
+                          double2* __restrict__ out64 = nullptr /* [n_pieces][7], all-FP64 path */) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n_pieces) return;
   // piece_lo == nullptr: uniform pieces of 2^(int)(size_t)piece_hi bins (the groups / sub-intervals of the adaptive path)
@@ -71,6 +72,10 @@ __global__ void k_moments(const double2* __restrict__ G64, const int* __restrict
 #pragma unroll
   for (int m = 0; m < 7; ++m) out[(size_t)i * 8 + m] = make_float2((float)mA[m], (float)mE[m]);
   out[(size_t)i * 8 + 7] = make_float2(0.f, 0.f);
+  if (out64) {
+#pragma unroll
+    for (int m = 0; m < 7; ++m) out64[(size_t)i * 7 + m] = make_double2(mA[m], mE[m]);
+  }
 }            // ulonglong2 records per bin pair: (wAr, wAi), (wEr, wEi), (gA, gE), each (even, odd)
 
 // FP32 sin/cos of a phase given as a signed 32-bit fraction of a turn: polynomial flavour (SC = 0).

@@ -60,9 +60,34 @@ struct DenseArgs {
   // k_dense2 only: pieces = fine sub-intervals cut at the segment edges, with the moments of the sigma weights
   const int* piece_first;      // [n_sub_launched + 1] first piece of each launched fine sub-interval
   const ulonglong2* moments;   // [n_pieces][4] = 8 packed (A, E) pairs: sum_j g_a(j) s_j^m, m = 0..6, pad
+  // k_dense only: FP64 moments of the sigma weights per piece, [n_pieces][7] (A, E) pairs, or nullptr (per-bin sigma)
+  const double2* moments64;
   // escalation pass (k_dense only): device-side particle count and this batch's offset; nullptr otherwise
   const int* esc_count; int esc_pb;
 };
+
+// sigma of one piece from the FP64 moments of its weights: on a fine sub-interval the amplitudes are cubics in s, so
+// |c_a(s)|^2 = sum_m e_a,m s^m (m = 0..6) and sigma_piece = sum_m (e_A,m M_A,m + e_E,m M_E,m) -- 7 FP64 operations per bin
+// leave the loop for ~45 per piece.
+__device__ __forceinline__ double sigma_moments64(const double (&cf)[4][4], const double2* __restrict__ M) {
+  double sig = 0.0;
+#pragma unroll
+  for (int ch = 0; ch < 2; ++ch) {
+    const double* R = cf[2 * ch];
+    const double* I = cf[2 * ch + 1];
+    double e[7];
+    e[0] = fma(R[0], R[0], I[0] * I[0]);
+    e[1] = 2.0 * fma(R[0], R[1], I[0] * I[1]);
+    e[2] = fma(2.0, fma(R[0], R[2], I[0] * I[2]), fma(R[1], R[1], I[1] * I[1]));
+    e[3] = 2.0 * (fma(R[0], R[3], I[0] * I[3]) + fma(R[1], R[2], I[1] * I[2]));
+    e[4] = fma(2.0, fma(R[1], R[3], I[1] * I[3]), fma(R[2], R[2], I[2] * I[2]));
+    e[5] = 2.0 * fma(R[2], R[3], I[2] * I[3]);
+    e[6] = fma(R[3], R[3], I[3] * I[3]);
+#pragma unroll
+    for (int m = 0; m < 7; ++m) sig = fma(e[m], ch == 0 ? M[m].x : M[m].y, sig);
+  }
+  return sig;
+}
 
 // All-FP64 flavour (few segments, N_seg < 8 by default): one bin per step, quintic phase by 5 forward differences,
 // FP64 polynomial sin/cos, FP64 amplitudes and accumulation.
@@ -180,7 +205,7 @@ __global__ void __launch_bounds__(kBlock) k_dense(DevCfg c, DenseArgs a, const d
     R s = R(0.0);
 
     // one bin: phase step + reduction (FP64), sincos, amplitude cubic, multiply-accumulate
-    auto bin = [&](int j, bool masked, R& zr, R& zi, R& sg) {
+    auto bin = [&](int j, bool masked, bool with_sg, R& zr, R& zi, R& sg) {
       R cr, sr;
       if (SC == 2 && sizeof(R) == 4) {
         // The phase is never reduced in FP64: adding 1.5 * 2^20 leaves rint(phi * 2^32) mod 2^32 in the low word,
@@ -211,11 +236,14 @@ __global__ void __launch_bounds__(kBlock) k_dense(DevCfg c, DenseArgs a, const d
       const R Ei = fma(fma(fma(cf[3][3], s, cf[3][2]), s, cf[3][1]), s, cf[3][0]);
       s += hS;
       const WT w = sW[j - cs];
-      const GT g = sG[j - cs];
       // q = W_A conj(c_A) + W_E conj(c_E)
       R qr = fma(w.x, Ar, fma(w.y, Ai, fma(w.z, Er, w.w * Ei)));
       R qi = fma(w.y, Ar, fma(-w.x, Ai, fma(w.w, Er, -(w.z * Ei))));
-      R ss = fma(g.x, fma(Ar, Ar, Ai * Ai), g.y * fma(Er, Er, Ei * Ei));
+      R ss = R(0.0);
+      if (with_sg) {
+        const GT g = sG[j - cs];
+        ss = fma(g.x, fma(Ar, Ar, Ai * Ai), g.y * fma(Er, Er, Ei * Ei));
+      }
       if (masked) {
         const bool in = (j >= jlo) && (j < jhi);
         qr = in ? qr : R(0.0); qi = in ? qi : R(0.0); ss = in ? ss : R(0.0);
@@ -226,6 +254,9 @@ __global__ void __launch_bounds__(kBlock) k_dense(DevCfg c, DenseArgs a, const d
       sg += ss;
     };
 
+    // all lanes inside their windows and moments available: sigma per piece from the moments, not per bin
+    const bool use_mom = all_in && (a.moments64 != nullptr);
+    int piece = use_mom ? a.piece_first[(ib >> (c.log2_stride - 2)) - ((a.chunk_first * CH) >> (c.log2_stride - 2))] : 0;
     int j = ib;
     while (j < ie) {
       const int b = min(next_edge, ie);
@@ -240,12 +271,15 @@ __global__ void __launch_bounds__(kBlock) k_dense(DevCfg c, DenseArgs a, const d
           for (int jj = j; jj < b;) {
             const int e2 = min(jj + kFlushBins, b);
             R zr = R(0.0), zi = R(0.0), sg = R(0.0);
-            if (all_in) { for (; jj < e2; ++jj) bin(jj, false, zr, zi, sg); }
-            else        { for (; jj < e2; ++jj) bin(jj, true, zr, zi, sg); }
+            if (use_mom)     { for (; jj < e2; ++jj) bin(jj, false, false, zr, zi, sg); }
+            else if (all_in) { for (; jj < e2; ++jj) bin(jj, false, true, zr, zi, sg); }
+            else             { for (; jj < e2; ++jj) bin(jj, true, true, zr, zi, sg); }
             Zr += (double)zr; Zi += (double)zi; Sg += (double)sg;
           }
+          if (use_mom) Sg += sigma_moments64(cf, a.moments64 + (size_t)piece * 7);
           fd_pos = b;
         }
+        ++piece;
         j = b;
       }
       if (j == next_edge) {

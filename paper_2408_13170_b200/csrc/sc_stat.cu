@@ -56,6 +56,7 @@ struct EdgeCache {
   int cached_lg = 0; int n_pieces = 0;
   int* d_piece_first = nullptr; int* d_piece_lo = nullptr; int* d_piece_hi = nullptr; float2* d_moments = nullptr;
   size_t pf_cap = 0, plo_cap = 0, phi_cap = 0, mom_cap = 0;
+  double2* d_moments64 = nullptr; size_t mom64_cap = 0;   // FP64 moments per piece (all-FP64 chunking only)
 };
 
 struct sc_handle : EdgeCache {
@@ -309,6 +310,7 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
     a.frag = frag; a.out_seg = seg_mode ? out_seg + (size_t)pb * n_seg * 3 : nullptr; a.P = Pn;
     a.seg_scale_z = sz; a.seg_scale_s = ss; a.comp = out_comp ? 1 : 0;
     a.piece_first = h->d_piece_first; a.moments = reinterpret_cast<const ulonglong2*>(h->d_moments);
+    a.moments64 = (sizeof(R) == 8 && h->cached_lg > 0) ? h->d_moments64 : nullptr;
     const dim3 grid(n_chunks, pblocks);
     {
       Timed tm(h, st, cls_dense);
@@ -371,6 +373,8 @@ int build_pieces(sc_handle* h, int CH, int lg_fine, cudaStream_t st) {
   if ((rc = grow(h, (void**)&h->d_piece_lo, &h->plo_cap, std::max<size_t>(lo.size(), 1) * 4))) return rc;
   if ((rc = grow(h, (void**)&h->d_piece_hi, &h->phi_cap, std::max<size_t>(hi.size(), 1) * 4))) return rc;
   if ((rc = grow(h, (void**)&h->d_moments, &h->mom_cap, std::max<size_t>(lo.size(), 1) * 8 * sizeof(float2)))) return rc;
+  const bool f64 = (CH == kChunkF64);            // the all-FP64 kernel reads the moments in FP64
+  if (f64 && (rc = grow(h, (void**)&h->d_moments64, &h->mom64_cap, std::max<size_t>(lo.size(), 1) * 7 * sizeof(double2)))) return rc;
   SC_CUDA(h, cudaMemcpyAsync(h->d_piece_first, first.data(), first.size() * 4, cudaMemcpyHostToDevice, st));
   if (h->n_pieces > 0) {
     SC_CUDA(h, cudaMemcpyAsync(h->d_piece_lo, lo.data(), lo.size() * 4, cudaMemcpyHostToDevice, st));
@@ -378,7 +382,7 @@ int build_pieces(sc_handle* h, int CH, int lg_fine, cudaStream_t st) {
     SC_CUDA(h, cudaStreamSynchronize(st));       // the host vectors go out of scope
     Timed tm(h, st, SC_TIME_OTHER);
     k_moments<<<(h->n_pieces + 127) / 128, 128, 0, st>>>(h->G64, h->d_piece_lo, h->d_piece_hi, h->n_pieces, (int)h->cfg.n_bins,
-                                                        lg_fine, h->d_moments);
+                                                        lg_fine, h->d_moments, f64 ? h->d_moments64 : nullptr);
     if ((rc = check_launch(h, "k_moments"))) return rc;
   } else {
     SC_CUDA(h, cudaStreamSynchronize(st));
@@ -429,7 +433,9 @@ int eval_common(sc_handle* h, const double* params, int64_t P, const int32_t* se
     return fail(h, SC_ERR_INVALID_ARG, "null pointer or n_particles <= 0");
   cudaStream_t st = (cudaStream_t)stream;
   const bool f64 = (h->precision == 2) || (h->precision == 0 && n_seg < h->f32_min_seg);
-  int rc = prepare_edges(h, seg_edges, n_seg, f64 ? kChunkF64 : kChunkF32, f64 ? 0 : h->lg_f32 - 2, st);
+  // all-FP64 path: sigma from FP64 piece moments when a fine sub-interval is long enough to pay for them (>= 32 bins)
+  const int lg_fine64 = (h->lg_f64 - 2 >= 5) ? h->lg_f64 - 2 : 0;
+  int rc = prepare_edges(h, seg_edges, n_seg, f64 ? kChunkF64 : kChunkF32, f64 ? lg_fine64 : h->lg_f32 - 2, st);
   if (rc) return rc;
   SC_CUDA(h, cudaMemsetAsync(h->d_counter, 0, 8, st));
   if (seg_mode) SC_CUDA(h, cudaMemsetAsync(out_seg, 0, (size_t)P * n_seg * 3 * 8, st));
@@ -461,7 +467,7 @@ int eval_common(sc_handle* h, const double* params, int64_t P, const int32_t* se
     const int esc_blocks = (int)std::min<int64_t>((2LL * hint + kBlock - 1) / kBlock + 1, (int64_t)P_round / kBlock);
     const std::vector<int> e_host = h->edges;                  // host copy: the alternate cache analyses the same list
     std::swap(static_cast<EdgeCache&>(*h), h->alt);
-    rc = prepare_edges(h, e_host.data(), n_seg, kChunkF64, 0, st);
+    rc = prepare_edges(h, e_host.data(), n_seg, kChunkF64, lg_fine64, st);
     if (!rc) rc = run_batches<double>(h, h->d_esc_params, P, h->d_esc_out, nullptr, nullptr, st, false, h->d_esc_count, esc_blocks);
     std::swap(static_cast<EdgeCache&>(*h), h->alt);
     if (rc) return rc;
@@ -1261,6 +1267,7 @@ int sc_free(sc_handle* h) {
   cudaFree(h->d_spsig); cudaFree(h->d_zpart); cudaFree(h->d_hh); cudaFree(h->d_gmom); cudaFree(h->d_smom);
   cudaFree(h->d_piece_first); cudaFree(h->d_piece_lo); cudaFree(h->d_piece_hi); cudaFree(h->d_moments);
   cudaFree(h->alt.d_edges); cudaFree(h->alt.d_chunk_k0); cudaFree(h->alt.d_flags); cudaFree(h->alt.d_next_close); cudaFree(h->d_next_close);
+  cudaFree(h->d_moments64); cudaFree(h->alt.d_moments64);
   cudaFree(h->alt.d_piece_first); cudaFree(h->alt.d_piece_lo); cudaFree(h->alt.d_piece_hi); cudaFree(h->alt.d_moments);
   cudaFreeHost(h->h_esc_hint); cudaFree(h->d_sort_tmp);
   cudaFree(h->d_esc_idx); cudaFree(h->d_esc_count); cudaFree(h->d_esc_params); cudaFree(h->d_esc_out);
