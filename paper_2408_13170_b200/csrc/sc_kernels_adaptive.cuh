@@ -27,6 +27,7 @@ struct AdaptArgs {
   int lg_group;
   int* out_edges;              // [P][n_seg + 1] of this batch, or nullptr
   double* chunk_sigma;         // = cbase (written by k_sigma_chunks before the scan)
+  const int* pmap;             // window sort: table slot -> particle of the batch (rows of out_edges), or nullptr
 };
 
 __device__ __forceinline__ double seg_target(double C, int n, int N) { return C * (double)n / (double)N; }
@@ -48,6 +49,10 @@ __global__ void __launch_bounds__(kBlock) k_sigma_chunks(DevCfg c, DenseArgs a, 
   const int ce2 = (ce + 1) & ~1;
   const int p = blockIdx.y * kBlock + threadIdx.x;
   const int jlo = a.jlo[p], jhi = a.jhi[p];
+  if (!__syncthreads_or((jhi > cs) && (jlo < ce))) {          // no particle of this block lives in this chunk
+    ad.chunk_sigma[(size_t)(chunk + 1) * a.P_pad + p] = 0.0;
+    return;
+  }
   const int Sf = c.stride >> 2;
   const float hS = 1.0f / (float)Sf;
   double tot = 0.0;
@@ -85,9 +90,17 @@ __global__ void k_scan_chunks(double* __restrict__ cbase, int n_chunks, int P_pa
   if (p >= P_pad) return;
   double acc = 0.0;
   cbase[p] = 0.0;
-  for (int i = 1; i <= n_chunks; ++i) {
-    acc += cbase[(size_t)i * P_pad + p];
-    cbase[(size_t)i * P_pad + p] = acc;
+  constexpr int kU = 8;                          // loads of kU chunks in flight; the sum itself stays in chunk order
+  for (int i0 = 1; i0 <= n_chunks; i0 += kU) {
+    double v[kU];
+#pragma unroll
+    for (int u = 0; u < kU; ++u) v[u] = cbase[(size_t)min(i0 + u, n_chunks) * P_pad + p];
+#pragma unroll
+    for (int u = 0; u < kU; ++u) {
+      if (i0 + u > n_chunks) break;
+      acc += v[u];
+      cbase[(size_t)(i0 + u) * P_pad + p] = acc;
+    }
   }
 }
 
@@ -101,6 +114,15 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2_ad(DevCfg c, 
   const int ce = min(cs + CH, c.n_bins);
   const int ce2 = (ce + 1) & ~1;
   const int p = blockIdx.y * kBlock + threadIdx.x;
+  const int jlo = a.jlo[p], jhi = a.jhi[p];
+  // no particle of this block lives in this chunk: its cumulative sigma does not move here, so no edge falls into the
+  // chunk (k == k1 below) -- the fragments of "nothing happened", without staging the data
+  if (!__syncthreads_or((jhi > cs) && (jlo < ce))) {
+    double* fz = a.frag + (size_t)chunk * kFragAd * a.P_pad + p;
+#pragma unroll
+    for (int m = 0; m < kFragAd; ++m) fz[(size_t)m * a.P_pad] = 0.0;
+    return;
+  }
   {
     const ulonglong2* src = Dg + (size_t)(cs >> 1) * kPairRec;
 #pragma unroll 4
@@ -108,7 +130,6 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2_ad(DevCfg c, 
   }
   __syncthreads();
 
-  const int jlo = a.jlo[p], jhi = a.jhi[p];
   const int Sf = c.stride >> 2;
   const float hS = 1.0f / (float)Sf;
   const u64 h2 = f2bcast(2.0f * hS);
@@ -126,6 +147,7 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2_ad(DevCfg c, 
   double Zr = 0.0, Zi = 0.0, ups = 0.0, xs = 0.0, hs = 0.0;
   bool closed_any = false;
   double* frag = a.frag + (size_t)chunk * kFragAd * a.P_pad + p;
+  const int pq = ad.pmap ? ad.pmap[p] : p;      // particle of the batch in this table slot
 
   auto close_at = [&](int j) {                  // edge k+1 lies at bin j
     const double Sg = crel - c_open;
@@ -139,7 +161,7 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2_ad(DevCfg c, 
     }
     Zr = 0.0; Zi = 0.0; c_open = crel;
     ++k;
-    if (ad.out_edges && p < a.P) ad.out_edges[(size_t)p * (N + 1) + k] = j;
+    if (ad.out_edges && pq < a.P) ad.out_edges[(size_t)pq * (N + 1) + k] = j;
     t_next = (k < k1) ? seg_target(C, k + 1, N) - cb0 : INFINITY;
   };
 
@@ -199,9 +221,19 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2_ad(DevCfg c, 
 
 __global__ void k_stitch_ad(const double* __restrict__ frag, int n_chunks, int P_pad, int P, double scale,
                             double* __restrict__ out, double* __restrict__ comp3, double x_scale, double h_scale,
-                            int* __restrict__ out_edges, int n_seg, int n_bins) {
+                            int* __restrict__ out_edges, int n_seg, int n_bins, const int* __restrict__ pmap = nullptr,
+                            const int* __restrict__ jlo = nullptr, const int* __restrict__ jhi = nullptr, int chunk_len = 1) {
   const int p = blockIdx.x * blockDim.x + threadIdx.x;
-  if (p >= P) return;
+  if (p >= (pmap ? P_pad : P)) return;
+  const int q = pmap ? pmap[p] : p;             // window sort: slot p holds particle q of the batch
+  if (q >= P) return;
+  // chunks wholly outside the particle's window hold the fragments of "nothing happened": only [c_lo, c_hi] is folded
+  int c_lo = 0, c_hi = n_chunks - 1;
+  if (jlo) {
+    const int lo = jlo[p], hi = jhi[p];
+    if (hi <= lo) { c_lo = 0; c_hi = -1; }
+    else { c_lo = max(lo / chunk_len, 0); c_hi = min((hi - 1) / chunk_len, n_chunks - 1); }
+  }
   double ups = 0.0, zr = 0.0, zi = 0.0, sg = 0.0, xs = 0.0, hs = 0.0;
   auto finish = [&]() {
     if (sg > 0.0) {
@@ -212,18 +244,18 @@ __global__ void k_stitch_ad(const double* __restrict__ frag, int n_chunks, int P
   };
   // serial fold in chunk order (bitwise reproducible), loads of kU chunks in flight (as in k_stitch)
   constexpr int kU = 8;
-  for (int c0 = 0; c0 < n_chunks; c0 += kU) {
+  for (int c0 = c_lo; c0 <= c_hi; c0 += kU) {
     double v[kU][8], w8[kU], w9[kU];
 #pragma unroll
     for (int u = 0; u < kU; ++u) {
-      const double* f = frag + (size_t)min(c0 + u, n_chunks - 1) * kFragAd * P_pad + p;
+      const double* f = frag + (size_t)min(c0 + u, c_hi) * kFragAd * P_pad + p;
 #pragma unroll
       for (int m = 0; m < 8; ++m) v[u][m] = f[(size_t)m * P_pad];
       w8[u] = comp3 ? f[(size_t)8 * P_pad] : 0.0; w9[u] = comp3 ? f[(size_t)9 * P_pad] : 0.0;
     }
 #pragma unroll
     for (int u = 0; u < kU; ++u) {
-      if (c0 + u >= n_chunks) break;
+      if (c0 + u > c_hi) break;
       zr += v[u][1]; zi += v[u][2]; sg += v[u][3];
       if (v[u][7] != 0.0) {
         finish();
@@ -234,9 +266,9 @@ __global__ void k_stitch_ad(const double* __restrict__ frag, int n_chunks, int P
     }
   }
   finish();                                     // the last segment closes at e_N = n_bins
-  if (out) out[p] = ups * scale;
-  if (comp3) { comp3[3 * (size_t)p] = ups * scale; comp3[3 * (size_t)p + 1] = xs * x_scale; comp3[3 * (size_t)p + 2] = hs * h_scale; }
-  if (out_edges) { out_edges[(size_t)p * (n_seg + 1)] = 0; out_edges[(size_t)p * (n_seg + 1) + n_seg] = n_bins; }
+  if (out) out[q] = ups * scale;
+  if (comp3) { comp3[3 * (size_t)q] = ups * scale; comp3[3 * (size_t)q + 1] = xs * x_scale; comp3[3 * (size_t)q + 2] = hs * h_scale; }
+  if (out_edges) { out_edges[(size_t)q * (n_seg + 1)] = 0; out_edges[(size_t)q * (n_seg + 1) + n_seg] = n_bins; }
 }
 
 }  // namespace

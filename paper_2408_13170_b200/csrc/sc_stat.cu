@@ -554,7 +554,7 @@ int run_adaptive(sc_handle* h, const double* params, int64_t P, int n_seg, doubl
     if ((rc = check_launch(h, "k_moments"))) return rc;
     h->ad_lg = dc.log2_stride;
   }
-  const size_t per_p = (size_t)kPcFields * 8 + 8 + (size_t)n_nodes * (4 + 8 + 4 * sizeof(float))
+  const size_t per_p = 2 * ((size_t)kPcFields * 8 + 8) + 16 + (size_t)n_nodes * (4 + 8 + 4 * sizeof(float))
                        + (size_t)(n_chunks + 1) * 8 + (size_t)n_chunks * kFragAd * 8;
   int64_t Pb_max = (int64_t)(h->scratch_cap / per_p) / kBlock * kBlock;
   if (Pb_max < kBlock) Pb_max = kBlock;
@@ -571,7 +571,23 @@ int run_adaptive(sc_handle* h, const double* params, int64_t P, int n_seg, doubl
   float* node_amp = (float*)take((size_t)n_nodes * 4 * sizeof(float) * P_pad);
   double* cbase = (double*)take((size_t)(n_chunks + 1) * 8 * P_pad);
   double* frag = (double*)take((size_t)n_chunks * kFragAd * 8 * P_pad);
+  // window sort, as in run_batches
+  const bool sorted = h->window_sort && P_pad > kBlock;
+  double* pc_u = (double*)take((size_t)kPcFields * 8 * P_pad);
+  int* jlo_u = (int*)take((size_t)4 * P_pad);
+  int* jhi_u = (int*)take((size_t)4 * P_pad);
+  int* key_s = (int*)take((size_t)4 * P_pad);
+  int* iota = (int*)take((size_t)4 * P_pad);
+  int* pmap = (int*)take((size_t)4 * P_pad);
   (void)base;
+  size_t sort_bytes = 0;
+  if (sorted) {
+    if (cub::DeviceRadixSort::SortPairs(nullptr, sort_bytes, jlo_u, key_s, iota, pmap, P_pad, 0, 32, st) != cudaSuccess)
+      return fail(h, SC_ERR_CUDA, "cub::DeviceRadixSort size query failed");
+    if ((rc = grow(h, &h->d_sort_tmp, &h->sort_cap, sort_bytes + 256))) return rc;
+    k_iota<<<(P_pad + 255) / 256, 256, 0, st>>>(iota, P_pad);
+    if ((rc = check_launch(h, "k_iota"))) return rc;
+  }
 
   const double four_df = 4.0 / h->cfg.T_obs_s;
   const int sincos = (h->sincos_mode == 0) ? (n_seg >= h->mufu_min_seg ? 2 : 0) : (h->sincos_mode == 2 ? 2 : 0);
@@ -583,12 +599,22 @@ int run_adaptive(sc_handle* h, const double* params, int64_t P, int n_seg, doubl
     const int Pn = (int)std::min<int64_t>(P_pad, P - pb);
     {
       Timed tm(h, st, SC_TIME_NODES);
-      k_particle_consts<<<(P_pad + 127) / 128, 128, 0, st>>>(dc, params + pb * 8, Pn, P_pad, pc, jlo, jhi, 0, dc.n_bins, h->d_counter);
+      k_particle_consts<<<(P_pad + 127) / 128, 128, 0, st>>>(dc, params + pb * 8, Pn, P_pad, sorted ? pc_u : pc, sorted ? jlo_u : jlo,
+                                                            sorted ? jhi_u : jhi, 0, dc.n_bins, h->d_counter);
     }
     if ((rc = check_launch(h, "k_particle_consts"))) return rc;
+    if (sorted) {
+      Timed tm(h, st, SC_TIME_NODES);
+      if (cub::DeviceRadixSort::SortPairs(h->d_sort_tmp, sort_bytes, jlo_u, key_s, iota, pmap, P_pad, 0, 32, st) != cudaSuccess)
+        return fail(h, SC_ERR_CUDA, "cub::DeviceRadixSort::SortPairs failed");
+      h->launches += 3;
+      k_gather_sorted<<<(P_pad + 127) / 128, 128, 0, st>>>(pmap, P_pad, pc_u, jlo_u, jhi_u, pc, jlo, jhi);
+      if ((rc = check_launch(h, "k_gather_sorted"))) return rc;
+    }
     {
       Timed tm(h, st, SC_TIME_NODES);
-      k_nodes<float><<<dim3((n_nodes + kNodesPerCta - 1) / kNodesPerCta, (P_pad + 127) / 128), 128, 0, st>>>(dc, pc, jlo, jhi, P_pad, node_n, node_frac, node_amp);
+      // (k_sigma_chunks and k_dense2_ad read a node only where a lane of the warp is inside its window: skip_unreached)
+      k_nodes<float><<<dim3((n_nodes + kNodesPerCta - 1) / kNodesPerCta, (P_pad + 127) / 128), 128, 0, st>>>(dc, pc, jlo, jhi, P_pad, node_n, node_frac, node_amp, nullptr, 0, 1);
     }
     if ((rc = check_launch(h, "k_nodes"))) return rc;
     DenseArgs a = {};
@@ -599,6 +625,7 @@ int run_adaptive(sc_handle* h, const double* params, int64_t P, int n_seg, doubl
     ad.gmom = reinterpret_cast<const ulonglong2*>(h->d_gmom); ad.smom = reinterpret_cast<const ulonglong2*>(h->d_smom);
     ad.lg_group = lg_group;
     ad.out_edges = out_edges ? out_edges + (size_t)pb * (n_seg + 1) : nullptr;
+    ad.pmap = sorted ? pmap : nullptr;
     const dim3 grid(n_chunks, P_pad / kBlock);
     {
       Timed tm(h, st, SC_TIME_OTHER);
@@ -616,9 +643,9 @@ int run_adaptive(sc_handle* h, const double* params, int64_t P, int n_seg, doubl
     if ((rc = check_launch(h, "k_dense2_ad"))) return rc;
     Timed tm2(h, st, SC_TIME_STITCH);
     const double g2 = (sincos == 2) ? h->mufu_gain2 : 1.0;
-    k_stitch_ad<<<(Pn + 127) / 128, 128, 0, st>>>(frag, n_chunks, P_pad, Pn, 1.0 / g2, out ? out + pb : nullptr,
+    k_stitch_ad<<<((sorted ? P_pad : Pn) + 127) / 128, 128, 0, st>>>(frag, n_chunks, P_pad, Pn, 1.0 / g2, out ? out + pb : nullptr,
                                                   out_comp ? out_comp + pb * 3 : nullptr, h->s0 * h0 / sqrt(g2),
-                                                  h->s0 * h->s0 * h0 * h0, ad.out_edges, n_seg, dc.n_bins);
+                                                  h->s0 * h->s0 * h0 * h0, ad.out_edges, n_seg, dc.n_bins, ad.pmap, jlo, jhi, CH);
     if ((rc = check_launch(h, "k_stitch_ad"))) return rc;
   }
   return SC_OK;

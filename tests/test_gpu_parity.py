@@ -580,3 +580,30 @@ def test_c3_adaptive_bench_configuration(oracle, torch_cuda, sc):
     assert np.all(np.isfinite(got)) and np.all(got >= 0)
     assert np.all(np.diff(ged, axis=1) >= 0) and np.all(ged[:, -1] == inp["cfg"]["n_bins"])
     H.close()
+
+
+def test_c5_adaptive_short_windows(oracle, torch_cuda, sc):
+    """Per-particle segments on c5's short, scattered time windows: the window sort, the empty-CTA exits, the skipped node
+    blocks and the windowed stitch of the adaptive path.  A sample against the oracle (edges within one bin, statistic on
+    the device's edges to 1e-6); sort on / off over the whole population: same edges up to one bin, and where every edge
+    agrees the same statistic to FP32 rounding."""
+    inp = sy.config_inputs(5, P=1280)
+    cfg, dA, dE = make_data(oracle, inp)
+    H = gpu_handle(inp, dA, dE)
+    H.set_option(sc.SC_OPT_TC_MAX_S, int(np.ceil(inp["hi"][2])))
+    par = _dev(torch_cuda, inp["particles"])
+    idx = _sample_idx(1280, 6, 77)
+    N = 50
+    res = {}
+    for srt in (1, 0):
+        H.set_option(sc.SC_OPT_WINDOW_SORT, srt)
+        g, e = H.eval_stat_adaptive(par, N, want_edges=True)
+        res[srt] = (g.cpu().numpy(), e.cpu().numpy())
+    H.close()
+    (a, ea), (b, eb) = res[1], res[0]
+    _check_adaptive(oracle, cfg, dA, dE, inp, inp["particles"][idx], N, a[idx], ea[idx])
+    assert np.abs(ea - eb).max() <= 1
+    same = np.all(ea == eb, axis=1) & (b > 0)
+    assert same.sum() > 900
+    assert rel_err(a[same], b[same]).max() <= 2e-7
+    assert np.all(np.diff(ea, axis=1) >= 0) and np.all(ea[:, -1] == inp["cfg"]["n_bins"]) and np.all(ea[:, 0] == 0)
