@@ -178,6 +178,23 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2_ad(DevCfg c, 
     sub_amps(c, a, p, ib, cf);
     u64 s2 = f2pack(0.0f, hS);
     const ulonglong2* rec = sD + ((ib - cs) >> 1) * kPairRec;
+    // First ask the question for the whole sub-interval (its moments are those k_sigma_chunks used): if no lane reaches its
+    // next target in it, all its groups take the unmasked path and the group moments are not needed at all.
+    if (all_in && ie - ib == Sf) {
+      const double sg_s = sigma_moments(cf, ad.smom + (size_t)(ib >> (c.log2_stride - 2)) * 4);
+      const bool cross_s = (k < k1) && (crel + sg_s * 1.0001 >= t_next);
+      if (!__any_sync(0xffffffffu, cross_s)) {
+        for (int gs = ib; gs < ie; gs += Gs) {
+          u64 zr2 = 0, zi2 = 0;
+          pairs_fast<SC>(ph, cf, s2, rec, Gs >> 1, h2, K2, zr2, zi2);
+          float zrl, zrh, zil, zih;
+          f2unpack(zr2, zrl, zrh); f2unpack(zi2, zil, zih);
+          Zr += (double)(zrl + zrh); Zi += (double)(zil + zih);
+        }
+        crel += sg_s;
+        continue;
+      }
+    }
     for (int gs = ib; gs < ie; gs += Gs) {
       const int ge = min(gs + Gs, ie);
       const double sg_m = sigma_moments(cf, ad.gmom + (size_t)(gs >> ad.lg_group) * 4);
