@@ -1,9 +1,10 @@
 """Pins for the oracle's phase and time-frequency map (sco_phase, sco_tf) -- SURVEY.md 8(c) O2/O3.
 
 The paper names TaylorF2Ecc [49] and prints no formula, so the pins are: the Newtonian closed
-forms, the textbook TaylorT2 time-to-coalescence through 2PN (an independently stated series), the t_c values
-the paper prints in Tables I and III, the SPA identity t(f) = Psi'(f)/2pi by finite differences, and the GW
-cycle count.  Parity with LALSimulation / TaylorF2Ecc beyond 2PN, and the eccentric coefficient, stay UNPINNED.
+forms, the textbook TaylorT2 time-to-coalescence through 3.5PN (an independently stated series with its own
+coefficients), the t_c values the paper prints in Tables I and III, the SPA identity t(f) = Psi'(f)/2pi by finite
+differences, and the GW cycle count.  The constant part of psi_5 (degenerate with phi_c, irrelevant to Upsilon), the
+eccentric coefficient and bit-level parity with LALSimulation / TaylorF2Ecc stay UNPINNED.
 """
 import json
 import os
@@ -49,6 +50,30 @@ def test_tf_taylorT2_series_through_2pn(oracle):
                           (3058673.0 / 508032.0 + 5429.0 * eta / 504.0 + 617.0 * eta ** 2 / 72.0) * v ** 4]
                 tau0 = 5.0 / 256.0 * (Mc * MS) ** (-5.0 / 3.0) * (np.pi * f) ** (-8.0 / 3.0)
                 assert -oracle.tf(cfg, th, f) == pytest.approx(tau0 * (1.0 + sum(series[:terms])), rel=1e-12)
+
+
+def test_tf_taylorT2_series_2p5_to_3p5pn(oracle):
+    """The same published TaylorT2 timing series continued to 3.5PN (its own rational coefficients, not those of the
+    TaylorF2 phase): -(7729/252 - 13 eta/3) pi v^5, the 3PN term with 128 pi^2/3, 6848 gamma_E/105 and
+    (3424/105) ln(16 v^2), and the 3.5PN term.  Pins psi_5's logarithm, psi_6 (every eta power, the Euler-gamma and log
+    terms) and psi_7 through t = Psi'/2pi -- a wrong digit in any of them moves t(f) by >> 1e-10 relative."""
+    gam = 0.5772156649015329
+    for pn, terms in ((5, 1), (6, 2), (7, 3)):
+        cfg = _cfg(oracle, pn=pn)
+        for Mc, eta in ((25.0, 0.21), (36.0, 0.25), (30.0, 0.2469)):
+            th = _theta(Mc, eta, tc=0.0)
+            for f in (0.012, 0.02, 0.035):
+                M = Mc * MS * eta ** -0.6
+                v = (np.pi * M * f) ** (1.0 / 3.0)
+                low = ((743.0 / 252.0 + 11.0 * eta / 3.0) * v ** 2 - (32.0 * np.pi / 5.0) * v ** 3
+                       + (3058673.0 / 508032.0 + 5429.0 * eta / 504.0 + 617.0 * eta ** 2 / 72.0) * v ** 4)
+                high = [-(7729.0 / 252.0 - 13.0 * eta / 3.0) * np.pi * v ** 5,
+                        (-10052469856691.0 / 23471078400.0 + 128.0 * np.pi ** 2 / 3.0 + 6848.0 * gam / 105.0
+                         + (3147553127.0 / 3048192.0 - 451.0 * np.pi ** 2 / 12.0) * eta - 15211.0 * eta ** 2 / 1728.0
+                         + 25565.0 * eta ** 3 / 1296.0 + 3424.0 / 105.0 * np.log(16.0 * v * v)) * v ** 6,
+                        (-15419335.0 / 127008.0 - 75703.0 * eta / 756.0 + 14809.0 * eta ** 2 / 378.0) * np.pi * v ** 7]
+                tau0 = 5.0 / 256.0 * (Mc * MS) ** (-5.0 / 3.0) * (np.pi * f) ** (-8.0 / 3.0)
+                assert -oracle.tf(cfg, th, f) == pytest.approx(tau0 * (1.0 + low + sum(high[:terms])), rel=1e-11)
 
 
 @pytest.mark.parametrize("table", ["table_I", "table_III"])
