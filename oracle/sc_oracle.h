@@ -16,9 +16,9 @@
  *                          Monte-Carlo moments of Eq. 11-12.
  *   sco_phase / sco_tf   : Newtonian closed form; Table I / III t_c values;
  *                          finite-difference identity t(f) = Psi'(f)/2pi in long double; cycle count; the published
- *                          TaylorT2 timing series through 3.5PN (pins psi_2 .. psi_7).
- *                          PARITY WITH LALSimulation / TaylorF2Ecc [49] ITSELF AND THE ECCENTRIC COEFFICIENT ARE UNPINNED
- *                          (not in the container).
+ *                          TaylorT2 timing series through 3.5PN (pins psi_2 .. psi_7); Peters' small-e equations
+ *                          (pin the leading eccentric coefficient).
+ *                          PARITY WITH THE LALSimulation / TaylorF2Ecc [49] CODE ITSELF IS UNPINNED (not in the container).
  *   sco_orbit/sco_template: arm lengths = L, centroid on the 1-AU circle; two-pulse single-link identity;
  *                          long-wavelength Michelson limit; T-combination -> 0; beta = +-pi/2 kills the Doppler term.
  *                          PARITY WITH BBHx [56] IS UNPINNED (not in the container).

@@ -3,8 +3,8 @@
 The paper names TaylorF2Ecc [49] and prints no formula, so the pins are: the Newtonian closed
 forms, the textbook TaylorT2 time-to-coalescence through 3.5PN (an independently stated series with its own
 coefficients), the t_c values the paper prints in Tables I and III, the SPA identity t(f) = Psi'(f)/2pi by finite
-differences, and the GW cycle count.  The constant part of psi_5 (degenerate with phi_c, irrelevant to Upsilon), the
-eccentric coefficient and bit-level parity with LALSimulation / TaylorF2Ecc stay UNPINNED.
+differences, and the GW cycle count.  The leading eccentric coefficient is pinned by Peters' small-e equations.  The constant part
+of psi_5 (degenerate with phi_c, irrelevant to Upsilon) and parity with the LALSimulation / TaylorF2Ecc code stay UNPINNED.
 """
 import json
 import os
@@ -142,6 +142,21 @@ def test_eccentric_term_scaling(oracle):
     assert d(0.1, 0.02) / d(0.05, 0.02) == pytest.approx(4.0, rel=1e-6)
     assert d(0.1, 0.02) / base(0.02) == pytest.approx(-(2355.0 / 1462.0) * 0.01, rel=1e-6)
     assert d(0.1, 0.03) / d(0.1, 0.02) == pytest.approx(1.5 ** (-34.0 / 9.0), rel=1e-6)
+
+
+def test_eccentric_coefficient_from_peters_equations(oracle):
+    """Pins 2355/1462 from quantities it is not written in: at small e Peters' equations give e = e_0 (f/f_ref)^(-19/18)
+    and df/dt = (96/5) pi^(8/3) M_c^(5/3) f^(11/3) (1 + 157 e^2/24); integrating dt = df/(df/dt) from f to infinity,
+    t_c - t(f) = tau_0(f) [1 - (157/43) e(f)^2]   (157/24 x (8/3)/(8/3 + 19/9) = 157/43).
+    The oracle gets t(f) from its phase term by t = Psi'/2pi; both must agree at Newtonian order."""
+    f_ref = 0.0175
+    cfg = _cfg(oracle, pn=0, ecc=1, f_ref=f_ref)
+    for Mc, eta, e0 in ((30.0, 0.2469, 0.1), (22.0, 0.23, 0.03)):
+        th = _theta(Mc, eta, tc=0.0, e0=e0)
+        for f in (0.012, 0.0175, 0.03):
+            tau0 = 5.0 / 256.0 * (Mc * MS) ** (-5.0 / 3.0) * (np.pi * f) ** (-8.0 / 3.0)
+            e2 = e0 ** 2 * (f / f_ref) ** (-19.0 / 9.0)
+            assert -oracle.tf(cfg, th, f) == pytest.approx(tau0 * (1.0 - 157.0 / 43.0 * e2), rel=1e-12)
 
 
 def test_invalid_theta_gives_zero_template(oracle):
