@@ -89,13 +89,67 @@ __device__ __forceinline__ double sigma_moments64(const double (&cf)[4][4], cons
   return sig;
 }
 
-// All-FP64 flavour (few segments, N_seg < 8 by default): one bin per step, quintic phase by 5 forward differences,
-// FP64 polynomial sin/cos, FP64 amplitudes and accumulation.
+// sin, cos of 2 pi x for any |x| < 2^49 turns: nearest quarter turn removed exactly, polynomials on |x| <= 1/8 turn.
+__device__ __forceinline__ void sincos_turns(double x, double& sr, double& cr) {
+  const double t = fma(x, 4.0, kMagic);
+  const int quad = __double2loint(t);
+  x = fma(t - kMagic, -0.25, x);
+  double sn, cn;
+  sincos_2pi_small(x, sn, cn);
+  const bool swp = quad & 1;
+  cr = swp ? sn : cn; sr = swp ? cn : sn;
+  cr = ((quad + 1) & 2) ? -cr : cr;
+  sr = (quad & 2) ? -sr : sr;
+}
+
+// Phase on fine sub-interval [ib, ib + Sf) as a cubic in unit bin steps from ib: quintic through 6 nodes -> Taylor shift to
+// the centre -> Chebyshev economisation to a cubic on [-H, H] (dropped: |b4| H^4 / 8 + |b5| H^5 / 16 turns, < 1e-11 rad
+// at the <= 2-day node spacing of this path) -> shift to the start.  Returns the phase at ib [turns] and its forward
+// differences d1 = Phi(1) - Phi(0), d2, d3 (constant).
+__device__ __forceinline__ void sub_phase_cubic(const DevCfg& c, const int* __restrict__ node_n,
+                                                const double* __restrict__ node_frac, int P_pad, int p, int ib,
+                                                double& p0, double& d1, double& d2, double& d3) {
+  const int ic = ib >> c.log2_stride;
+  const int i0 = ic + kNodeOff;
+  const int S = c.stride, Sf = S >> 2;
+  const size_t base = (size_t)i0 * P_pad + p;
+  const int n0 = node_n[base];
+  const double r0 = node_frac[base];
+  double Y[6];
+#pragma unroll
+  for (int m = -2; m <= 3; ++m) {
+    const size_t at = (size_t)(i0 + m) * P_pad + p;
+    Y[m + 2] = (double)(node_n[at] - n0) + (node_frac[at] - r0);
+  }
+  double b[6];
+  quintic_coeffs(Y, 1.0 / (double)S, b);
+  const double H = 0.5 * (double)Sf;
+  taylor_shift(b, (double)(ib - (ic << c.log2_stride)) + H);
+  const double H2 = H * H, H4 = H2 * H2;
+  b[0] = fma(-0.125 * H4, b[4], b[0]);
+  b[2] = fma(H2, b[4], b[2]);
+  b[1] = fma(-0.3125 * H4, b[5], b[1]);
+  b[3] = fma(1.25 * H2, b[5], b[3]);
+#pragma unroll
+  for (int i = 0; i < 3; ++i)
+#pragma unroll
+    for (int j = 2; j >= i; --j) b[j] = fma(-H, b[j + 1], b[j]);
+  p0 = r0 + b[0];
+  d1 = b[1] + b[2] + b[3];
+  d2 = 2.0 * b[2] + 6.0 * b[3];
+  d3 = 6.0 * b[3];
+}
+
+// All-FP64 flavour (few segments, N_seg < 8 by default): one bin per step, FP64 amplitudes and accumulation.  The phase
+// factor e^{2 pi i Phi_j} is carried by a rotation recurrence instead of being evaluated per bin: with the sub-interval's
+// cubic phase, E_j = e^{2 pi i Phi_j}, R_j = e^{2 pi i d1_j}, Q_j = e^{2 pi i d2_j} obey E_{j+1} = E_j R_j, R_{j+1} = R_j Q_j,
+// Q_{j+1} = Q_j (1 + 2 pi i d3) -- 10 FP64 operations per bin against 23 for five forward differences, the range reduction
+// and two polynomials.  E, R, Q are re-seeded with FP64 sin/cos at every fine sub-interval (<= 256 bins), over which the
+// recurrences' rounding grows to < 1e-10 rad (Q's error enters E as n^3/6 x 1.1e-16).
 template <bool SEG, bool ESC = false>
 __global__ void __launch_bounds__(kBlock) k_dense(DevCfg c, DenseArgs a, const double4* __restrict__ Wg,
                                                   const double2* __restrict__ Gg) {
   using R = double;
-  constexpr int SC = 0;
   using WT = typename DataT<R>::W;
   using GT = typename DataT<R>::G;
   constexpr int CH = DataT<R>::chunk;
@@ -157,9 +211,13 @@ __global__ void __launch_bounds__(kBlock) k_dense(DevCfg c, DenseArgs a, const d
     Zr = 0.0; Zi = 0.0; Sg = 0.0;
   };
 
-  int fd_pos = -1;                   // bin the forward-difference state is positioned at (-1: none)
-  double phi = 0.0, d1 = 0.0, d2 = 0.0, d3 = 0.0, d4 = 0.0, d5 = 0.0;
-  int quad = 0;
+  double Pr = 1.0, Pi = 0.0, Rr = 1.0, Ri = 0.0, Qr = 1.0, Qi = 0.0, eps = 0.0;   // rotation recurrence: P = E_j (see above)
+  auto rot_step = [&]() {
+    const double pr = fma(Pr, Rr, -(Pi * Ri)), pi = fma(Pr, Ri, Pi * Rr);
+    const double rr = fma(Rr, Qr, -(Ri * Qi)), ri = fma(Rr, Qi, Ri * Qr);
+    const double qr = fma(-eps, Qi, Qr), qi = fma(eps, Qr, Qi);
+    Pr = pr; Pi = pi; Rr = rr; Ri = ri; Qr = qr; Qi = qi;
+  };
   for (int ib = cs; ib < ce; ib += Sf) {
     const int ie = min(ib + Sf, ce);
     const bool lane_in = (ib >= jlo) && (ie <= jhi);
@@ -172,25 +230,17 @@ __global__ void __launch_bounds__(kBlock) k_dense(DevCfg c, DenseArgs a, const d
       const int ic = ib >> c.log2_stride;                      // coarse interval
       const int i0 = ic + kNodeOff;                            // table row of its left node
       const int q = (ib >> (c.log2_stride - 2)) & 3;           // fine sub-interval within the coarse one
-      if (fd_pos != ib || q == 0) {
-        // (re)build the phase forward differences at u0 = ib - ic*stride from the 6-node quintic
-        const size_t base = (size_t)i0 * a.P_pad + p;
-        const int n0 = a.node_n[base];
-        const double r0 = a.node_frac[base];
-        double Y[6];
-#pragma unroll
-        for (int m = -2; m <= 3; ++m) {
-          const size_t at = (size_t)(i0 + m) * a.P_pad + p;
-          Y[m + 2] = (double)(a.node_n[at] - n0) + (a.node_frac[at] - r0);
-        }
-        double b[6], d[6];
-        quintic_coeffs(Y, 1.0 / (double)S, b);
-        const int u0 = ib - (ic << c.log2_stride);
-        if (u0) taylor_shift(b, (double)u0);
-        forward_diffs(b, d);
-        phi = r0 + b[0]; d1 = d[1]; d2 = d[2]; d3 = d[3]; d4 = d[4]; d5 = d[5];
-        quad = 0;
-        fd_pos = ib;
+      if (lane_out) {
+        // a lane outside its window here may see stencil nodes beyond k_nodes' reach (written as zeros): its bins are
+        // masked, but the recurrence must stay finite (0 x Inf), so it idles on the unit circle
+        Pr = 1.0; Pi = 0.0; Rr = 1.0; Ri = 0.0; Qr = 1.0; Qi = 0.0; eps = 0.0;
+      } else {
+        double p0, d1, d2, d3;
+        sub_phase_cubic(c, a.node_n, a.node_frac, a.P_pad, p, ib, p0, d1, d2, d3);
+        sincos_turns(p0, Pi, Pr);
+        sincos_turns(d1, Ri, Rr);
+        sincos_turns(d2, Qi, Qr);
+        eps = 6.283185307179586477 * d3;
       }
 #pragma unroll
       for (int r = 0; r < 4; ++r) {
@@ -204,31 +254,10 @@ __global__ void __launch_bounds__(kBlock) k_dense(DevCfg c, DenseArgs a, const d
     }
     R s = R(0.0);
 
-    // one bin: phase step + reduction (FP64), sincos, amplitude cubic, multiply-accumulate
+    // one bin: phase factor from the recurrence, amplitude cubics, multiply-accumulate
     auto bin = [&](int j, bool masked, bool with_sg, R& zr, R& zi, R& sg) {
-      R cr, sr;
-      if (SC == 2 && sizeof(R) == 4) {
-        // The phase is never reduced in FP64: adding 1.5 * 2^20 leaves rint(phi * 2^32) mod 2^32 in the low word,
-        // i.e. the fraction of a turn in [-1/2, 1/2) as an int32; hardware sin/cos (MUFU) of that angle.
-        const int n = __double2loint(phi + 1572864.0);
-        const float xr = (float)n * 1.4629180792671596e-09f;          // 2 pi / 2^32
-        cr = (R)__cosf(xr); sr = (R)__sinf(xr);
-      } else {
-        // reduce phi to |x| <= 1/8 turn, carrying the quadrant
-        const double t = fma(phi, 4.0, kMagic);
-        quad += __double2loint(t);
-        const double kf = t - kMagic;
-        phi = fma(kf, -0.25, phi);
-        R sn, cn;
-        sincos_2pi_small((R)phi, sn, cn);
-        // rotate by quad * 90 degrees
-        const bool swp = quad & 1;
-        cr = swp ? sn : cn; sr = swp ? cn : sn;
-        cr = ((quad + 1) & 2) ? -cr : cr;
-        sr = (quad & 2) ? -sr : sr;
-      }
-      // advance the forward differences to the next bin
-      phi += d1; d1 += d2; d2 += d3; d3 += d4; d4 += d5;
+      const R cr = Pr, sr = Pi;
+      rot_step();
       // amplitudes
       const R Ar = fma(fma(fma(cf[0][3], s, cf[0][2]), s, cf[0][1]), s, cf[0][0]);
       const R Ai = fma(fma(fma(cf[1][3], s, cf[1][2]), s, cf[1][1]), s, cf[1][0]);
@@ -263,10 +292,9 @@ __global__ void __launch_bounds__(kBlock) k_dense(DevCfg c, DenseArgs a, const d
       const bool live = (k >= 0) && (k < a.n_seg);
       if (b > j) {
         if (all_out) {
-          // nothing to add; the forward-difference state is rebuilt at the next interval
+          // nothing to add; the recurrence is re-seeded at the next sub-interval
         } else if (!live) {
-          for (int jj = j; jj < b; ++jj) { phi += d1; d1 += d2; d2 += d3; d3 += d4; d4 += d5; s += hS; }
-          fd_pos = b;
+          for (int jj = j; jj < b; ++jj) { rot_step(); s += hS; }
         } else {
           for (int jj = j; jj < b;) {
             const int e2 = min(jj + kFlushBins, b);
@@ -277,7 +305,6 @@ __global__ void __launch_bounds__(kBlock) k_dense(DevCfg c, DenseArgs a, const d
             Zr += (double)zr; Zi += (double)zi; Sg += (double)sg;
           }
           if (use_mom) Sg += sigma_moments64(cf, a.moments64 + (size_t)piece * 7);
-          fd_pos = b;
         }
         ++piece;
         j = b;
