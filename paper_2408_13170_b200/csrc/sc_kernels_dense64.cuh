@@ -146,6 +146,7 @@ __device__ __forceinline__ void sub_phase_cubic(const DevCfg& c, const int* __re
 // Q_{j+1} = Q_j (1 + 2 pi i d3) -- 10 FP64 operations per bin against 23 for five forward differences, the range reduction
 // and two polynomials.  E, R, Q are re-seeded with FP64 sin/cos at every fine sub-interval (<= 256 bins), over which the
 // recurrences' rounding grows to < 1e-10 rad (Q's error enters E as n^3/6 x 1.1e-16).
+constexpr size_t kDense64Smem = (size_t)kChunkF64 * (sizeof(double4) + sizeof(double2) + sizeof(float4));
 template <bool SEG, bool ESC = false>
 __global__ void __launch_bounds__(kBlock) k_dense(DevCfg c, DenseArgs a, const double4* __restrict__ Wg,
                                                   const double2* __restrict__ Gg) {
@@ -153,8 +154,12 @@ __global__ void __launch_bounds__(kBlock) k_dense(DevCfg c, DenseArgs a, const d
   using WT = typename DataT<R>::W;
   using GT = typename DataT<R>::G;
   constexpr int CH = DataT<R>::chunk;
-  __shared__ WT sW[CH];
-  __shared__ GT sG[CH];
+  // dynamic shared memory (kDense64Smem = 64 KB per CTA, 3 CTAs per SM): the chunk's whitened data in FP64, the sigma
+  // weights, and an FP32 copy of the data for the correction term of the anchored path
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  WT* sW = reinterpret_cast<WT*>(smem_raw);
+  GT* sG = reinterpret_cast<GT*>(sW + CH);
+  float4* sW32 = reinterpret_cast<float4*>(sG + CH);
 
   const int chunk_l = blockIdx.x;                              // launched-chunk index
   const int cs = (a.chunk_first + chunk_l) * CH;
@@ -171,7 +176,11 @@ __global__ void __launch_bounds__(kBlock) k_dense(DevCfg c, DenseArgs a, const d
     }
   }
 
-  for (int t = threadIdx.x; t < ce - cs; t += kBlock) { sW[t] = Wg[cs + t]; sG[t] = Gg[cs + t]; }
+  for (int t = threadIdx.x; t < ce - cs; t += kBlock) {
+    const WT w = Wg[cs + t];
+    sW[t] = w; sG[t] = Gg[cs + t];
+    sW32[t] = make_float4((float)w.x, (float)w.y, (float)w.z, (float)w.w);
+  }
   __syncthreads();
 
   // one pass over the block's 128 particles; in the escalation pass the blocks stride over the selected particles
@@ -253,6 +262,19 @@ __global__ void __launch_bounds__(kBlock) k_dense(DevCfg c, DenseArgs a, const d
       }
     }
     R s = R(0.0);
+    // Anchored form of the amplitudes for the fast path below: c(s) = g0 + delta(d), d = s - 1/2, with the value at the
+    // centre of the sub-interval in FP64 and the cubic correction delta = d (g1 + d (g2 + d g3)) in FP32 (|delta| is a few
+    // 1e-2 of |c| over a <= 0.5-day sub-interval, so its FP32 rounding is ~1e-9 of the amplitude).
+    R g0[4];
+    float g1[4], g2[4], g3[4];
+    if (!all_out)
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+      g0[r] = fma(cf[r][3], 0.125, fma(cf[r][2], 0.25, fma(cf[r][1], 0.5, cf[r][0])));
+      g1[r] = (float)fma(cf[r][3], 0.75, cf[r][1] + cf[r][2]);
+      g2[r] = (float)fma(cf[r][3], 1.5, cf[r][2]);
+      g3[r] = (float)cf[r][3];
+    }
 
     // one bin: phase factor from the recurrence, amplitude cubics, multiply-accumulate
     auto bin = [&](int j, bool masked, bool with_sg, R& zr, R& zi, R& sg) {
@@ -295,16 +317,46 @@ __global__ void __launch_bounds__(kBlock) k_dense(DevCfg c, DenseArgs a, const d
           // nothing to add; the recurrence is re-seeded at the next sub-interval
         } else if (!live) {
           for (int jj = j; jj < b; ++jj) { rot_step(); s += hS; }
+        } else if (use_mom) {
+          // Fast path (every lane of the warp inside its window, sigma from the moments): with c = g0 + delta,
+          //   z_piece = conj(g0_A) T_A + conj(g0_E) T_E + sum_j [w_A conj(delta_A) + w_E conj(delta_E)] P_j,  T_a = sum_j w_a P_j.
+          // T_a is accumulated in FP64 (8 operations per bin, with the recurrence 18 in all against 37 for the direct
+          // form); the correction sum runs on the otherwise idle FP32 pipe and is folded into FP64 every kFlushBins bins.
+          double TAr = 0.0, TAi = 0.0, TEr = 0.0, TEi = 0.0;
+          float d = (float)(j - ib) * (float)hS - 0.5f;          // exact: multiples of 1/Sf
+          const float hSf = (float)hS;
+          for (int jj = j; jj < b;) {
+            const int e2 = min(jj + kFlushBins, b);
+            float zr = 0.f, zi = 0.f;
+            for (; jj < e2; ++jj) {
+              const WT w = sW[jj - cs];
+              const float4 v = sW32[jj - cs];
+              const float pr = (float)Pr, pi = (float)Pi;
+              TAr = fma(w.x, Pr, fma(-w.y, Pi, TAr)); TAi = fma(w.x, Pi, fma(w.y, Pr, TAi));
+              TEr = fma(w.z, Pr, fma(-w.w, Pi, TEr)); TEi = fma(w.z, Pi, fma(w.w, Pr, TEi));
+              rot_step();
+              const float dAr = d * fmaf(fmaf(g3[0], d, g2[0]), d, g1[0]), dAi = d * fmaf(fmaf(g3[1], d, g2[1]), d, g1[1]);
+              const float dEr = d * fmaf(fmaf(g3[2], d, g2[2]), d, g1[2]), dEi = d * fmaf(fmaf(g3[3], d, g2[3]), d, g1[3]);
+              d += hSf;
+              const float qr = fmaf(v.x, dAr, fmaf(v.y, dAi, fmaf(v.z, dEr, v.w * dEi)));
+              const float qi = fmaf(v.y, dAr, fmaf(-v.x, dAi, fmaf(v.w, dEr, -(v.z * dEi))));
+              zr = fmaf(qr, pr, fmaf(-qi, pi, zr));
+              zi = fmaf(qr, pi, fmaf(qi, pr, zi));
+            }
+            Zr += (double)zr; Zi += (double)zi;
+          }
+          Zr += fma(g0[0], TAr, fma(g0[1], TAi, fma(g0[2], TEr, g0[3] * TEi)));
+          Zi += fma(g0[0], TAi, fma(-g0[1], TAr, fma(g0[2], TEi, -(g0[3] * TEr))));
+          s = (R)(b - ib) * hS;
+          Sg += sigma_moments64(cf, a.moments64 + (size_t)piece * 7);
         } else {
           for (int jj = j; jj < b;) {
             const int e2 = min(jj + kFlushBins, b);
             R zr = R(0.0), zi = R(0.0), sg = R(0.0);
-            if (use_mom)     { for (; jj < e2; ++jj) bin(jj, false, false, zr, zi, sg); }
-            else if (all_in) { for (; jj < e2; ++jj) bin(jj, false, true, zr, zi, sg); }
+            if (all_in)      { for (; jj < e2; ++jj) bin(jj, false, true, zr, zi, sg); }
             else             { for (; jj < e2; ++jj) bin(jj, true, true, zr, zi, sg); }
             Zr += (double)zr; Zi += (double)zi; Sg += (double)sg;
           }
-          if (use_mom) Sg += sigma_moments64(cf, a.moments64 + (size_t)piece * 7);
         }
         ++piece;
         j = b;

@@ -320,9 +320,9 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
         else if (sincos == 2) k_dense2<false, 2><<<grid, kBlock, 0, st>>>(dc, a, Dp);
         else k_dense2<false, 0><<<grid, kBlock, 0, st>>>(dc, a, Dp);
       } else {
-        if (seg_mode) k_dense<true><<<grid, kBlock, 0, st>>>(dc, a, h->W64, h->G64);
-        else if (esc_count) k_dense<false, true><<<grid, kBlock, 0, st>>>(dc, a, h->W64, h->G64);
-        else k_dense<false><<<grid, kBlock, 0, st>>>(dc, a, h->W64, h->G64);
+        if (seg_mode) k_dense<true><<<grid, kBlock, kDense64Smem, st>>>(dc, a, h->W64, h->G64);
+        else if (esc_count) k_dense<false, true><<<grid, kBlock, kDense64Smem, st>>>(dc, a, h->W64, h->G64);
+        else k_dense<false><<<grid, kBlock, kDense64Smem, st>>>(dc, a, h->W64, h->G64);
       }
     }
     if ((rc = check_launch(h, "k_dense"))) return rc;
@@ -697,6 +697,10 @@ int init_common(sc_handle** out, const sc_config* cfg, const double* dA, const d
                                      "%s failed: %s", #call, cudaGetErrorString(e_));              \
                                 return bail(e_ == cudaErrorMemoryAllocation ? SC_ERR_OOM : SC_ERR_CUDA); } } while (0)
   SC_INIT(cudaGetDevice(&h->device));
+  // the all-FP64 kernel stages 64 KB per CTA in dynamic shared memory
+  SC_INIT(cudaFuncSetAttribute(k_dense<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kDense64Smem));
+  SC_INIT(cudaFuncSetAttribute(k_dense<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kDense64Smem));
+  SC_INIT(cudaFuncSetAttribute(k_dense<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kDense64Smem));
   const int n_pairs_pad = (n + kChunkF32 - 1) / kChunkF32 * (kChunkF32 / 2);
   SC_INIT(cudaMalloc(&h->D32, (size_t)n_pairs_pad * kPairRec * sizeof(float4)));
   SC_INIT(cudaMalloc(&h->W64, (size_t)n * sizeof(double4)));
