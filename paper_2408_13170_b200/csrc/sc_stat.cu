@@ -4,8 +4,10 @@
 // Pipeline of one sc_eval_stat call, per batch of particles:
 //   k_particle_consts  a1 + a3  per-particle constants, validity, time window [jlo, jhi) by bisection on t(f_j)
 //   k_nodes            a2       phase / amplitude at the coarse nodes (one node per `stride` bins)
-//   k_dense<R, SEG>    a4 + a5  THE HOT LOOP: lane = particle, warp walks the bins of its chunk in order;
-//                               whitened data broadcast from shared memory; FP64 phase by forward differences;
+//   k_dense2 / k_dense a4 + a5  THE HOT LOOP: lane = particle, warp walks the bins of its chunk in order;
+//                               whitened data broadcast from shared memory; k_dense2 (FP32 amplitudes, packed FFMA2):
+//                               FP64 phase by forward differences + FP32 sin/cos; k_dense (all-FP64): phase factor by
+//                               a rotation recurrence, amplitudes anchored in FP64 with an FP32 correction;
 //                               complete segments are finalised in registers, straddlers leave fragments
 //   k_stitch           a6       fixed-order stitch of the fragments -> Upsilon[p]
 // The kernels live in sc_kernels_*.cuh (included below in pipeline order, one translation unit); this file holds the
