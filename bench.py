@@ -481,9 +481,12 @@ def run_ours(args, rank, local_rank, world):
             dfma = None
         # roofline of the dominant kernel (k_dense), fixed FP64 op model of SURVEY.md 8(d): 24 FP64 instr = 48 flop per
         # EVALUATED (particle, bin); peak = measured DFMA rate x 2 flop
-        ach = 2.0 * C_DP * eval_bins / (dense_avg * 1e-3) / 1e12 if dense_avg > 0 else None
+        # populations beyond the scratch cap run in several batches: one evaluation = dense_per_eval launches of k_dense
+        dense_per_eval = max(1, int(round(dense_n / max(args.steps, 1))))
+        eval_bins_launch = eval_bins / dense_per_eval
+        ach = 2.0 * C_DP * eval_bins_launch / (dense_avg * 1e-3) / 1e12 if dense_avg > 0 else None
         peak = 2.0 * (dfma or NOMINAL_DFMA) / 1e12
-        pbs = eval_bins / (dense_avg * 1e-3) if dense_avg > 0 else None
+        pbs = eval_bins_launch / (dense_avg * 1e-3) if dense_avg > 0 else None
         roof = {"bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
                 "frac": (ach / peak) if ach else None, "traffic": dram_traffic_from_profile(),
                 "traffic_source": "profiles/r01d_k_dense2_full.md (ncu --set full, one launch, same command)",
@@ -496,7 +499,7 @@ def run_ours(args, rank, local_rank, world):
                 "peak_source": ("measured in this run by sc_measure_fp64_peak (DFMA/s x 2)" if dfma else
                                 "nominal 148 SM x 64 lanes x 1.965 GHz x 2"),
                 "peak_nominal_max_clock": 2.0 * NOMINAL_DFMA / 1e12,
-                "evaluated_particle_bins_per_launch": eval_bins,
+                "evaluated_particle_bins_per_launch": eval_bins_launch, "launches_per_evaluation": dense_per_eval,
                 "evaluated_pb_per_s": pbs,
                 "frac_vs_nominal_max_clock": (ach / (2.0 * NOMINAL_DFMA / 1e12)) if ach else None}
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
