@@ -77,7 +77,7 @@ enum {
                                 0 = off.  Not applied by sc_eval_segments / _components / _loglike / _adaptive.        */
   SC_OPT_ESC_TAU_POLY_X1000 = 10,  /* tau x 1000 for the polynomial sin/cos flavour (default 6000)                    */
   SC_OPT_ESC_TAU_MUFU_X1000 = 11,  /* tau x 1000 for the hardware sin/cos flavour (default 16000)                     */
-  SC_OPT_WINDOW_SORT = 12    /* 1 (default): each particle batch is processed in the order of the time-window starts (stable
+  SC_OPT_WINDOW_SORT = 12    /* 1 (default): each particle batch is processed in the order of the time-window centres (stable
                                 radix sort on the device), so that the 32 particles of a warp share their windows; results
                                 are bitwise reproducible for a given population and option set, but a particle's rounding
                                 (FP32 path: ~1e-8 relative) depends on which particles share its warp.  0 = input order.  */
@@ -229,7 +229,10 @@ typedef struct {
  * swarm of each particle, out = final.  lo, hi: DEVICE [8].  Outputs (HOST; all but best_* may be NULL):
  * best_pos [n_swarms][8], best_val [n_swarms] = swarm bests on the last rung; n_members [n_swarms]; passed [n_swarms] =
  * best_val >= threshold; iters_per_rung [n_rungs]; hist [n_rungs][n_swarms][max_iters_per_rung] = best after every
- * iteration (0 beyond the iterations run).  Synchronises the stream every iteration (S doubles read back). */
+ * iteration (0 beyond the iterations run).  Synchronises the stream every iteration (S doubles read back).
+ * Precision (automatic mode, two-channel handles): a shared-edge rung on which a particle's time window covers fewer than
+ * SC_OPT_F32_MIN_SEG segments on average (n_seg x the mean window fraction, measured once from the first shared-edge
+ * evaluation) runs on the all-FP64 path, like n_seg < SC_OPT_F32_MIN_SEG itself. */
 int sc_search_run(sc_handle* h, const sc_search_config* cfg, double* pos, double* vel, int32_t* label,
                   int64_t n_particles, int32_t n_swarms, const double* lo, const double* hi,
                   double* best_pos, double* best_val, int64_t* n_members, int32_t* passed, int32_t* iters_per_rung,

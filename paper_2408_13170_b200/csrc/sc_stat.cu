@@ -288,7 +288,10 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
     if ((rc = check_launch(h, "k_particle_consts"))) return rc;
     if (sorted && n_chunks > 0) {
       Timed tm(h, st, cls_nodes);
-      if (cub::DeviceRadixSort::SortPairs(h->d_sort_tmp, sort_bytes, jlo_u, key_s, iota, pmap, P_pad, 0, 32, st) != cudaSuccess)
+      // keys: window centres, staged in jlo (the sorted copy of the windows is written by k_gather_sorted afterwards)
+      k_sort_key<<<(P_pad + 255) / 256, 256, 0, st>>>(jlo_u, jhi_u, jlo, P_pad);
+      if ((rc = check_launch(h, "k_sort_key"))) return rc;
+      if (cub::DeviceRadixSort::SortPairs(h->d_sort_tmp, sort_bytes, jlo, key_s, iota, pmap, P_pad, 0, 32, st) != cudaSuccess)
         return fail(h, SC_ERR_CUDA, "cub::DeviceRadixSort::SortPairs failed");
       h->launches += 3;
       k_gather_sorted<<<(P_pad + 127) / 128, 128, 0, st>>>(pmap, P_pad, pc_u, jlo_u, jhi_u, pc, jlo, jhi);
@@ -607,7 +610,10 @@ int run_adaptive(sc_handle* h, const double* params, int64_t P, int n_seg, doubl
     if ((rc = check_launch(h, "k_particle_consts"))) return rc;
     if (sorted) {
       Timed tm(h, st, SC_TIME_NODES);
-      if (cub::DeviceRadixSort::SortPairs(h->d_sort_tmp, sort_bytes, jlo_u, key_s, iota, pmap, P_pad, 0, 32, st) != cudaSuccess)
+      // keys: window centres, staged in jlo (the sorted copy of the windows is written by k_gather_sorted afterwards)
+      k_sort_key<<<(P_pad + 255) / 256, 256, 0, st>>>(jlo_u, jhi_u, jlo, P_pad);
+      if ((rc = check_launch(h, "k_sort_key"))) return rc;
+      if (cub::DeviceRadixSort::SortPairs(h->d_sort_tmp, sort_bytes, jlo, key_s, iota, pmap, P_pad, 0, 32, st) != cudaSuccess)
         return fail(h, SC_ERR_CUDA, "cub::DeviceRadixSort::SortPairs failed");
       h->launches += 3;
       k_gather_sorted<<<(P_pad + 127) / 128, 128, 0, st>>>(pmap, P_pad, pc_u, jlo_u, jhi_u, pc, jlo, jhi);
@@ -911,6 +917,9 @@ int sc_search_run(sc_handle* h, const sc_search_config* sc, double* pos, double*
   // ranking precision (sc_search_config): force the FP32-amplitude path without escalation for the whole search
   const int saved_precision = h->precision, saved_escalate = h->escalate;
   if (sc->ranking_precision) { h->precision = 1; h->escalate = 0; }
+  const bool auto_precision = (h->precision == 0) && h->escalate && !h->sub;
+  double win_frac = -1.0;                          // mean window fraction, -1: not measured yet
+  unsigned long long ev_bins = 0;
   auto cleanup = [&](int code) { h->precision = saved_precision; h->escalate = saved_escalate; cudaFree(buf); return code; };
 #define SC_S(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cleanup(fail(h, SC_ERR_CUDA, "%s failed: %s", #call, cudaGetErrorString(e_))); } while (0)
   SC_S(cudaMemsetAsync(gbest_pos, 0, (size_t)S * 8 * 8, st));
@@ -927,16 +936,28 @@ int sc_search_run(sc_handle* h, const sc_search_config* sc, double* pos, double*
       for (int k = 0; k <= N; ++k) e[k] = (int32_t)(((long long)k * nb) / N);       // equal-width shared edges (Q2)
     }
     hst.assign((size_t)S * sc->max_iters_per_rung, 0.0);
+    const bool shared_rung = !(sc->adaptive_edges && N > 1);
+    // Shared edges and short time windows (c5: a window covers ~2.5 % of the band): a particle then sees only N x phi
+    // non-empty segments, and below f32_min_seg of them the FP32 pass would escalate nearly everybody.  phi = mean window
+    // fraction, measured once from the evaluated-bin count of the first shared-edge evaluation of the search (read in
+    // the synchronisation every iteration has anyway; a deterministic function of the first population).
+    if (shared_rung && auto_precision && win_frac >= 0.0) h->precision = ((double)N * win_frac < (double)h->f32_min_seg) ? 2 : 0;
     int it = 0;
     for (; it < sc->max_iters_per_rung; ++it) {
-      if (sc->adaptive_edges && N > 1) rc = sc_eval_stat_adaptive(h, pos, P, N, stat, nullptr, nullptr, stream);
+      if (!shared_rung) rc = sc_eval_stat_adaptive(h, pos, P, N, stat, nullptr, nullptr, stream);
       else rc = eval_any(h, pos, P, e.data(), N, stat, nullptr, stream, false);
       if (rc) return cleanup(rc);
+      const bool measure = shared_rung && auto_precision && win_frac < 0.0;
+      if (measure) SC_S(cudaMemcpyAsync(&ev_bins, h->d_counter, 8, cudaMemcpyDeviceToHost, st));
       rc = sc_pso_step_labeled(h, pos, vel, pbest_pos, pbest_val, stat, gbest_pos, gbest_val, label, lo, hi, eps_d,
                                sc->omega[r], sc->phi_p[r], sc->phi_g[r], sc->seed, iter_global++, P, S, stream);
       if (rc) return cleanup(rc);
       SC_S(cudaMemcpyAsync(gv.data(), gbest_val, (size_t)S * 8, cudaMemcpyDeviceToHost, st));
       SC_S(cudaStreamSynchronize(st));
+      if (measure) {
+        win_frac = (double)ev_bins / ((double)P * (double)nb);
+        h->precision = ((double)N * win_frac < (double)h->f32_min_seg) ? 2 : 0;
+      }
       bool all_conv = true;
       for (int s = 0; s < S; ++s) {
         hst[(size_t)s * sc->max_iters_per_rung + it] = gv[s];
@@ -948,6 +969,7 @@ int sc_search_run(sc_handle* h, const sc_search_config* sc, double* pos, double*
       }
       if (all_conv) { ++it; break; }
     }
+    if (auto_precision) h->precision = 0;
     if (iters_per_rung) iters_per_rung[r] = it;
     if (hist)
       for (int s = 0; s < S; ++s)
