@@ -166,6 +166,23 @@ __global__ void __launch_bounds__(kBlock) k_dense(DevCfg c, DenseArgs a, const d
   const int ce = min(cs + CH, c.n_bins);
   const int esc_lim = ESC ? min(*a.esc_count - a.esc_pb, a.P_pad) : 0;
   if (ESC && (int)(blockIdx.y * kBlock) >= esc_lim) return;
+  if (ESC) {
+    // escalation pass: the CTA strides over particle blocks; none of them may live in this chunk (short windows, batch
+    // sorted by window centre) -- then every block gets its empty fragments and the data is not staged
+    bool any = false;
+    for (int pblk = blockIdx.y; pblk * kBlock < esc_lim; pblk += gridDim.y) {
+      const int pp = pblk * kBlock + threadIdx.x;
+      any = any || ((a.jhi[pp] > cs) && (a.jlo[pp] < ce));
+    }
+    if (!__syncthreads_or(any)) {
+      for (int pblk = blockIdx.y; pblk * kBlock < esc_lim; pblk += gridDim.y) {
+        double* fz = a.frag + (size_t)chunk_l * kFragFields * a.P_pad + pblk * kBlock + threadIdx.x;
+#pragma unroll
+        for (int m = 0; m < kFragFields; ++m) fz[(size_t)m * a.P_pad] = 0.0;
+      }
+      return;
+    }
+  }
   if (!ESC) {                                                  // as in k_dense2: nothing of this block lives in this chunk
     const int p0 = blockIdx.y * kBlock + threadIdx.x;
     if (!__syncthreads_or((a.jhi[p0] > cs) && (a.jlo[p0] < ce))) {
@@ -189,6 +206,12 @@ __global__ void __launch_bounds__(kBlock) k_dense(DevCfg c, DenseArgs a, const d
   const int p = pblk * kBlock + threadIdx.x;                   // particle within the batch (P_pad is a multiple of kBlock)
 
   const int jlo = a.jlo[p], jhi = a.jhi[p];
+  if (ESC && !__any_sync(0xffffffffu, (jhi > cs) && (jlo < ce))) {   // no lane of this warp lives here (no barrier below)
+    double* fz = a.frag + (size_t)chunk_l * kFragFields * a.P_pad + p;
+#pragma unroll
+    for (int m = 0; m < kFragFields; ++m) fz[(size_t)m * a.P_pad] = 0.0;
+    continue;
+  }
   const int S = c.stride, Sf = S >> 2;
   const R hS = R(1.0) / R(Sf);
   const R* __restrict__ namp = reinterpret_cast<const R*>(a.node_amp);

@@ -21,16 +21,23 @@ __global__ void k_iota(int* __restrict__ v, int n) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n) v[i] = i;
 }
-__global__ void k_sort_key(const int* __restrict__ jlo_u, const int* __restrict__ jhi_u, int* __restrict__ key, int n) {
+// Escalation pass (esc_count != nullptr): only the first *esc_count - esc_pb slots of the unsorted arrays were written; the
+// others get the largest key (they sort to the end, stable) and an empty window.
+__global__ void k_sort_key(const int* __restrict__ jlo_u, const int* __restrict__ jhi_u, int* __restrict__ key, int n,
+                           const int* __restrict__ esc_count = nullptr, int esc_pb = 0) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < n) key[i] = (jlo_u[i] >> 1) + (jhi_u[i] >> 1);        // the centre (no overflow for n_bins < 2^31)
+  if (i >= n) return;
+  const bool live = !esc_count || i < *esc_count - esc_pb;
+  key[i] = live ? (jlo_u[i] >> 1) + (jhi_u[i] >> 1) : INT_MAX;  // the centre (no overflow for n_bins < 2^31)
 }
 __global__ void k_gather_sorted(const int* __restrict__ map, int P_pad, const double* __restrict__ pc_u,
                                 const int* __restrict__ jlo_u, const int* __restrict__ jhi_u, double* __restrict__ pc,
-                                int* __restrict__ jlo, int* __restrict__ jhi) {
+                                int* __restrict__ jlo, int* __restrict__ jhi, const int* __restrict__ esc_count = nullptr,
+                                int esc_pb = 0) {
   const int p = blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= P_pad) return;
   const int q = map[p];
+  if (esc_count && q >= *esc_count - esc_pb) { jlo[p] = 0; jhi[p] = 0; return; }
 #pragma unroll
   for (int f = 0; f < kPcFields; ++f) pc[(size_t)f * P_pad + p] = pc_u[(size_t)f * P_pad + q];
   jlo[p] = jlo_u[q]; jhi[p] = jhi_u[q];

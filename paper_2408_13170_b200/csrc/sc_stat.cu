@@ -249,9 +249,9 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
   double* node_frac = (double*)take((size_t)n_nodes * 8 * P_pad);
   R* node_amp = (R*)take((size_t)n_nodes * 4 * sizeof(R) * P_pad);
   double* frag = (double*)take((size_t)std::max(n_chunks, 1) * kFragFields * 8 * P_pad);
-  // window sort (see k_gather_sorted): not in the segment-table mode (rows are addressed by particle) nor in the
-  // escalation pass (few particles, count on the device)
-  const bool sorted = h->window_sort && !seg_mode && !esc_count && P_pad > kBlock;
+  // window sort (see k_gather_sorted): not in the segment-table mode (rows are addressed by particle).  In the escalation
+  // pass the count sits on the device: all P_pad slots are sorted, the unused ones to the end.
+  const bool sorted = h->window_sort && !seg_mode && P_pad > kBlock;
   double* pc_u = (double*)take((size_t)kPcFields * 8 * P_pad);
   int* jlo_u = (int*)take((size_t)4 * P_pad);
   int* jhi_u = (int*)take((size_t)4 * P_pad);
@@ -289,12 +289,12 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
     if (sorted && n_chunks > 0) {
       Timed tm(h, st, cls_nodes);
       // keys: window centres, staged in jlo (the sorted copy of the windows is written by k_gather_sorted afterwards)
-      k_sort_key<<<(P_pad + 255) / 256, 256, 0, st>>>(jlo_u, jhi_u, jlo, P_pad);
+      k_sort_key<<<(P_pad + 255) / 256, 256, 0, st>>>(jlo_u, jhi_u, jlo, P_pad, esc_count, (int)pb);
       if ((rc = check_launch(h, "k_sort_key"))) return rc;
       if (cub::DeviceRadixSort::SortPairs(h->d_sort_tmp, sort_bytes, jlo, key_s, iota, pmap, P_pad, 0, 32, st) != cudaSuccess)
         return fail(h, SC_ERR_CUDA, "cub::DeviceRadixSort::SortPairs failed");
       h->launches += 3;
-      k_gather_sorted<<<(P_pad + 127) / 128, 128, 0, st>>>(pmap, P_pad, pc_u, jlo_u, jhi_u, pc, jlo, jhi);
+      k_gather_sorted<<<(P_pad + 127) / 128, 128, 0, st>>>(pmap, P_pad, pc_u, jlo_u, jhi_u, pc, jlo, jhi, esc_count, (int)pb);
       if ((rc = check_launch(h, "k_gather_sorted"))) return rc;
     }
     if (n_chunks == 0) {
@@ -304,7 +304,7 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
     }
     {
       Timed tm(h, st, cls_nodes);
-      if (esc_count) k_nodes<R, true><<<dim3((n_nodes + kNodesPerCta - 1) / kNodesPerCta, pblocks), 128, 0, st>>>(dc, pc, jlo, jhi, P_pad, node_n, node_frac, node_amp, esc_count, (int)pb);
+      if (esc_count) k_nodes<R, true><<<dim3((n_nodes + kNodesPerCta - 1) / kNodesPerCta, pblocks), 128, 0, st>>>(dc, pc, jlo, jhi, P_pad, node_n, node_frac, node_amp, esc_count, (int)pb, 1);
       else k_nodes<R, false><<<dim3((n_nodes + kNodesPerCta - 1) / kNodesPerCta, pblocks), 128, 0, st>>>(dc, pc, jlo, jhi, P_pad, node_n, node_frac, node_amp, nullptr, 0, 1);
     }
     if ((rc = check_launch(h, "k_nodes"))) return rc;
