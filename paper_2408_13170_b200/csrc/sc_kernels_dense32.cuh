@@ -300,7 +300,7 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2(DevCfg c, Den
   const int ce2 = (ce + 1) & ~1;                               // pair-aligned end (data beyond n_bins is zero)
   const int p = blockIdx.y * kBlock + threadIdx.x;
 
-  // no particle of this block has its time window in this chunk (common once the batch is sorted by window start):
+  // no particle of this block has its time window in this chunk (common once the batch is sorted by window centre):
   // leave empty fragments and skip the staging of the data
   if (!__syncthreads_or((a.jhi[p] > cs) && (a.jlo[p] < ce))) {
     double* fz = a.frag + (size_t)chunk_l * kFragFields * a.P_pad + p;

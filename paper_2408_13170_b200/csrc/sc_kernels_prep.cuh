@@ -173,7 +173,7 @@ __global__ void k_nodes(DevCfg c, const double* __restrict__ pc, const int* __re
     const long long r_lo = (long long)lo - reach, r_hi = (long long)hi + reach;
     // skip_unreached (k_dense / k_dense2 as consumers): a warp reads a node only where one of its particles' windows is
     // within reach of it, and then for all its lanes -- so a block none of whose particles reaches the node need not write
-    // it at all (with the batch sorted by window start that is most of the table when the windows are short)
+    // it at all (with the batch sorted by window centre that is most of the table when the windows are short)
     const long long g_lo = ((long long)i_first - kNodeOff) << c.log2_stride, g_hi = ((long long)i_last - 1 - kNodeOff) << c.log2_stride;
     const bool group_reached = hi > lo && g_hi >= r_lo && g_lo <= r_hi;
     if (!(skip_unreached && !__syncthreads_or(group_reached))) {

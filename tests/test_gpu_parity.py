@@ -133,7 +133,7 @@ def test_escalation_of_ill_conditioned_particles(oracle, torch_cuda, sc, N):
 
 
 def test_window_sort_is_a_pure_reordering(oracle, torch_cuda, sc):
-    """SC_OPT_WINDOW_SORT: batches are processed in the order of the window starts.  Against the oracle nothing changes;
+    """SC_OPT_WINDOW_SORT: batches are processed in the order of the window centres.  Against the oracle nothing changes;
     against the input order only the rounding of the FP32 path does (the sigma of a sub-interval comes from the weight
     moments when all 32 particles of the warp are inside their windows, from the per-bin sum otherwise); the all-FP64
     path has one formula and agrees to its own rounding (a lane's phase differences are rebuilt or stepped on depending
