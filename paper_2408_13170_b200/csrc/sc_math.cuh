@@ -109,7 +109,13 @@ struct NodeOut {
   double Ar, Ai, Er, Ei;
 };
 
-__device__ __forceinline__ double sinc_d(double x) { return (x == 0.0) ? 1.0 : sin(x) / x; }
+
+// sin(x)/x given sin x from an angle-addition formula (absolute error ~1e-16): near x = 0 the quotient would lose
+// relative accuracy, so the series takes over below 1e-2 (next term x^6/5040 < 2e-16).
+__device__ __forceinline__ double sinc_from(double x, double sin_x) {
+  const double x2 = x * x;
+  return (x2 < 1.0e-4) ? fma(x2, fma(x2, 1.0 / 120.0, -1.0 / 6.0), 1.0) : sin_x / x;
+}
 
 __device__ NodeOut eval_node(const DevCfg& c, const Particle& q, long long jglob /* j0 + bin position */) {
   NodeOut o;
@@ -155,6 +161,10 @@ __device__ NodeOut eval_node(const DevCfg& c, const Particle& q, long long jglob
   const double ux = -q.sb * q.cl, uy = -q.sb * q.sl, uz = q.cb;
   const double vx = -q.sl, vy = q.cl;
   const double pfl = kPi * f * c.L;
+  // sin, cos of pi f L once per node: the six sinc arguments pfl (1 -+ k.n) and the delay D = e^{-2 i pfl} follow by the
+  // angle-addition formulas (one sincos of pfl k.n per arm instead of two sines, none for D)
+  double sp, cp;
+  sincos(pfl, &sp, &cp);
   // arms (s, r) = (1,2), (2,3), (3,1): y_sr and y_rs share zeta and the phase factor
   double ysr[3][2], yrs[3][2];
 #pragma unroll
@@ -171,12 +181,14 @@ __device__ NodeOut eval_node(const DevCfg& c, const Particle& q, long long jglob
     double es, ec;
     sincos(-kPi * f * (c.L + kd), &es, &ec);
     const double wr = ec * zr - es * zi, wi = ec * zi + es * zr;
-    const double a_sr = pfl * sinc_d(pfl * (1.0 - kn)), a_rs = pfl * sinc_d(pfl * (1.0 + kn));
+    double sb, cb;
+    sincos(pfl * kn, &sb, &cb);
+    const double a_sr = pfl * sinc_from(pfl * (1.0 - kn), fma(sp, cb, -(cp * sb)));
+    const double a_rs = pfl * sinc_from(pfl * (1.0 + kn), fma(sp, cb, cp * sb));
     ysr[a][0] = a_sr * wi; ysr[a][1] = -a_sr * wr;      // -i a (wr + i wi)
     yrs[a][0] = a_rs * wi; yrs[a][1] = -a_rs * wr;
   }
-  double Di, Dr;
-  sincos(-2.0 * kPi * f * c.L, &Di, &Dr);                // D = e^{-2 pi i f L}
+  const double Dr = fma(-2.0 * sp, sp, 1.0), Di = -2.0 * sp * cp;   // D = e^{-2 pi i f L} = cos 2 pfl - i sin 2 pfl
   const double gr = 1.0 - (Dr * Dr - Di * Di), gi = -2.0 * Dr * Di;
   // y12 = ysr[0], y21 = yrs[0], y23 = ysr[1], y32 = yrs[1], y31 = ysr[2], y13 = yrs[2]
   // X = (1-D^2)[(y31 + D y13) - (y21 + D y12)], Y, Z cyclic

@@ -250,8 +250,10 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
   R* node_amp = (R*)take((size_t)n_nodes * 4 * sizeof(R) * P_pad);
   double* frag = (double*)take((size_t)std::max(n_chunks, 1) * kFragFields * 8 * P_pad);
   // window sort (see k_gather_sorted): not in the segment-table mode (rows are addressed by particle).  In the escalation
-  // pass the count sits on the device: all P_pad slots are sorted, the unused ones to the end.
-  const bool sorted = h->window_sort && !seg_mode && P_pad > kBlock;
+  // pass the count sits on the device: all P_pad slots are sorted, the unused ones to the end -- only below 4096 segments
+  // (a rule of the call, not of the data: with that many segments hardly any particle is selected and the sort's seven
+  // small launches per batch would cost more than they save).
+  const bool sorted = h->window_sort && !seg_mode && P_pad > kBlock && (!esc_count || n_seg < 4096);
   double* pc_u = (double*)take((size_t)kPcFields * 8 * P_pad);
   int* jlo_u = (int*)take((size_t)4 * P_pad);
   int* jhi_u = (int*)take((size_t)4 * P_pad);
