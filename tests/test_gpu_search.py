@@ -175,3 +175,38 @@ def test_search_run_argument_errors(env):
         cfg = _search_cfg(sc, ladder, True, **bad)
         with pytest.raises(sc.SCError):
             H.search_run(cfg, pos, vel, lab, 1, lo, hi)
+
+
+def test_search_run_short_windows_take_the_fp64_path(oracle):
+    """c5-like tile (a window covers a few per cent of the band): on a shared-edge rung with N x (mean window fraction) < 8
+    the FP32 pass would escalate nearly every particle, so sc_search_run measures the fraction on its first evaluation and
+    runs the rest of the rung on the all-FP64 path (include/sc_stat.h).  Seen from outside: escalation kernels are
+    launched in the first iteration only, and the reported bests are the oracle's values."""
+    import torch
+    import paper_2408_13170_b200 as sc
+    from helpers import gpu_handle, make_data
+    P, S = 1536, 2
+    inp = sy.config_inputs(5, P=P)
+    cfg, dA, dE = make_data(oracle, inp)
+    H = gpu_handle(inp, dA, dE)
+    H.set_option(sc.SC_OPT_TC_MAX_S, int(np.ceil(inp["hi"][2])))
+    H.set_option(sc.SC_OPT_PROFILE, 1)
+    lo, hi = inp["lo"], inp["hi"]
+    rng = np.random.default_rng(5)
+    vel = (hi - lo) * rng.uniform(-0.1, 0.1, (P, 8))
+    label = np.repeat(np.arange(S, dtype=np.int32), P // S)
+    esc_launches = {}
+    for iters in (1, 4):
+        scfg = _search_cfg(sc, [50], False, max_iters_per_rung=iters, seed=7, threshold=100.0)
+        d_pos, d_vel, d_lab = _dev(torch, inp["particles"]), _dev(torch, vel), _dev(torch, label)
+        H.timing()
+        res = H.search_run(scfg, d_pos, d_vel, d_lab, S, _dev(torch, lo), _dev(torch, hi))
+        tm = H.timing()
+        assert list(res["iters_per_rung"]) == [iters]
+        esc_launches[iters] = tm["escalation"][1]
+        assert tm["dense"][1] >= iters
+    assert esc_launches[1] > 0 and esc_launches[4] == esc_launches[1]
+    b = int(np.argmax(res["best_val"]))
+    ref = oracle.eval_stat(cfg, dA, dE, inp["S_A"], inp["S_E"], res["best_pos"][b][None, :], sy.edges(inp["cfg"]["n_bins"], 50))
+    assert res["best_val"][b] == pytest.approx(ref[0], rel=1e-6)
+    H.close()
