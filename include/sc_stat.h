@@ -60,7 +60,7 @@ enum {
   SC_OPT_PRECISION = 1,      /* 0 = auto (FP32 amplitude path when n_seg >= SC_OPT_F32_MIN_SEG, else all-FP64),
                                 1 = force FP32 amplitude path, 2 = force all-FP64.  Phase is FP64 always.       */
   SC_OPT_F32_MIN_SEG = 2,    /* threshold of the auto rule (default 8)               */
-  SC_OPT_SCRATCH_BYTES = 3,  /* cap of the node-table scratch; larger populations are processed in batches      */
+  SC_OPT_SCRATCH_BYTES = 3,  /* cap of the node-table scratch (default 32 GiB); larger populations run in batches     */
   SC_OPT_TC_MAX_S = 4,       /* the caller's upper bound on t_c [s] over the particles (the search tile's t_c range,
                                 PAPER.md:253); sets the coarse node spacing to about one day of signal time at the
                                 low band edge.  Default 10 yr.                                  */

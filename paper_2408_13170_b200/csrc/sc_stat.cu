@@ -68,7 +68,7 @@ struct sc_handle : EdgeCache {
   double s0 = 1.0;                 // weight scale (power of two)
   float4* D32 = nullptr; double4* W64 = nullptr; double2* G64 = nullptr;   // D32: bin-pair layout of k_dense2
   // options
-  int precision = 0; int f32_min_seg = 8; size_t scratch_cap = (size_t)8 << 30;
+  int precision = 0; int f32_min_seg = 8; size_t scratch_cap = (size_t)32 << 30;   // of 180 GB per B200
   double tc_max_s = 10.0 * 31557600.0; int forced_stride_log2 = 0; int sincos_mode = 0; int mufu_min_seg = 32;
   int lg_f32 = 5, lg_f64 = 5;      // log2 of the coarse node spacing per precision mode (set_stride)
   double mufu_gain2 = 1.0;        // <cos^2 + sin^2> of the hardware sin/cos, measured at init
