@@ -176,6 +176,75 @@ __device__ __forceinline__ void sub_amps(const DevCfg& c, const DenseArgs& a, in
   }
 }
 
+// ---- merged coarse intervals (k_dense2<.., MERGE = true>, launched when the node stride is >= 512 bins) ----
+// The node stride is set by the slowest-chirping corner of the tile; towards higher frequencies a particle crosses a coarse
+// interval in less signal time than the day a FINE sub-interval is allowed to span.  Where that holds for every lane of the
+// warp (and every lane is inside its window over the whole coarse interval), one set-up serves the four fine
+// sub-intervals: the phase quintic is economised over the coarse interval and its forward differences run on through it;
+// the amplitudes are the plain cubic through nodes -1 .. 2 (the same <= 1-day spacing the fine cubics work with),
+// re-expanded per fine sub-interval (the pieces and their sigma moments stay as they are).
+// Signal time spanned by coarse interval ic, as a difference of phase slopes in turns per bin (t_f = T_obs dPhi/dj):
+// second difference of the node phases / stride.
+__device__ __forceinline__ double coarse_dslope(const DevCfg& c, const DenseArgs& a, int p, int ic) {
+  const size_t at0 = (size_t)(ic + kNodeOff) * a.P_pad + p, atm = at0 - a.P_pad, atp = at0 + a.P_pad;
+  const int n0 = a.node_n[at0];
+  const double r0 = a.node_frac[at0];
+  const double ym = (double)(a.node_n[atm] - n0) + (a.node_frac[atm] - r0);
+  const double yp = (double)(a.node_n[atp] - n0) + (a.node_frac[atp] - r0);
+  return fabs(ym + yp) / (double)c.stride;
+}
+// Phase over the whole coarse interval starting at bin ib (= ic * stride): as sub_phase with H = stride / 2.
+__device__ __forceinline__ void coarse_phase(const DevCfg& c, const DenseArgs& a, int p, int ib, PhaseFD& ph) {
+  const int i0 = (ib >> c.log2_stride) + kNodeOff;
+  const int S = c.stride;
+  const size_t base = (size_t)i0 * a.P_pad + p;
+  const int n0 = a.node_n[base];
+  const double r0 = a.node_frac[base];
+  double Y[6];
+#pragma unroll
+  for (int m = -2; m <= 3; ++m) {
+    const size_t at = (size_t)(i0 + m) * a.P_pad + p;
+    Y[m + 2] = (double)(a.node_n[at] - n0) + (a.node_frac[at] - r0);
+  }
+  double b[6];
+  quintic_coeffs(Y, 1.0 / (double)S, b);
+  const double H = 0.5 * (double)S;
+  taylor_shift(b, H);
+  const double H2 = H * H, H4 = H2 * H2;
+  b[0] = fma(-0.125 * H4, b[4], b[0]);
+  b[2] = fma(H2, b[4], b[2]);
+  b[1] = fma(-0.3125 * H4, b[5], b[1]);
+  b[3] = fma(1.25 * H2, b[5], b[3]);
+#pragma unroll
+  for (int i = 0; i < 3; ++i)
+#pragma unroll
+    for (int j = 2; j >= i; --j) b[j] = fma(-H, b[j + 1], b[j]);
+  phase_set(ph, r0 + b[0], b);
+}
+// Cubic through nodes -1 .. 2 of (Ar, Ai, Er, Ei) in t = (j - ib) / stride.
+__device__ __forceinline__ void coarse_amps(const DevCfg& c, const DenseArgs& a, int p, int ib, float (&cc)[4][4]) {
+  const int i0 = (ib >> c.log2_stride) + kNodeOff;
+  const float* __restrict__ namp = reinterpret_cast<const float*>(a.node_amp);
+#pragma unroll
+  for (int r = 0; r < 4; ++r) {
+    const float* col = namp + ((size_t)i0 * 4 + r) * a.P_pad + p;
+    const ptrdiff_t st = (ptrdiff_t)4 * a.P_pad;
+    cubic_coeffs<float>(col[-st], col[0], col[st], col[2 * st], cc[r][0], cc[r][1], cc[r][2], cc[r][3]);
+  }
+}
+// The same cubic in the variable of fine sub-interval q: t = (q + s) / 4.
+__device__ __forceinline__ void coarse_to_fine(const float (&cc)[4][4], int q, float (&cf)[4][4]) {
+  const float t0 = 0.25f * (float)q;
+#pragma unroll
+  for (int r = 0; r < 4; ++r) {
+    const float a0 = cc[r][0], a1 = cc[r][1], a2 = cc[r][2], a3 = cc[r][3];
+    cf[r][0] = fmaf(fmaf(fmaf(a3, t0, a2), t0, a1), t0, a0);
+    cf[r][1] = 0.25f * fmaf(fmaf(3.0f * a3, t0, 2.0f * a2), t0, a1);
+    cf[r][2] = 0.0625f * fmaf(3.0f * a3, t0, a2);
+    cf[r][3] = 0.015625f * a3;
+  }
+}
+
 // One bin pair (j, j+1): FP64 phase steps, sin/cos, amplitude cubics, multiply-accumulate into packed sums (low half =
 // even bin, high half = odd bin).  MASKED: apply the particle's time window per bin.  WITH_SG: accumulate |h|^2 per
 // bin (otherwise sigma comes from the moments).  s2 = (s_j, s_{j+1}), rec = the pair's data record; both advance.
@@ -289,7 +358,7 @@ __device__ __forceinline__ void pairs_fast(PhaseFD& ph, const float (&cf)[4][4],
   mac_pair(cf, s2, wA, wE, h2, cr, sr, zr2, zi2);
 }
 
-template <bool SEG, int SC>
+template <bool SEG, int SC, bool MERGE = false>
 __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2(DevCfg c, DenseArgs a, const ulonglong2* __restrict__ Dg) {
   constexpr int CH = kChunkF32;
   __shared__ ulonglong2 sD[CH / 2 * kPairRec];                 // 48 KB
@@ -354,6 +423,8 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2(DevCfg c, Den
   };
 
   PhaseFD fd = {};
+  float cc[MERGE ? 4 : 1][4];  // merged coarse interval: cubic of the amplitudes in t = (j - coarse start)/stride
+  int merged_left = 0;         // fine sub-intervals of the current merged coarse interval still to walk
   for (int ib = cs; ib < ce2; ib += Sf) {
     const int ie = min(ib + Sf, ce2);
     const bool lane_in = (ib >= jlo) && (ie <= jhi);
@@ -362,7 +433,19 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2(DevCfg c, Den
     const bool all_out = __all_sync(0xffffffffu, lane_out);
 
     float cf[4][4];    // cubic coefficients of (Ar, Ai, Er, Ei) in s = (j - ib)/Sf (FFMA2 broadcasts a scalar operand)
-    if (!all_out) {
+    if constexpr (MERGE) {
+      if (merged_left == 0 && (ib & (S - 1)) == 0 && ib + S <= ce2 &&
+          __all_sync(0xffffffffu, (ib >= jlo) && (ib + S <= jhi)) &&
+          __all_sync(0xffffffffu, coarse_dslope(c, a, p, ib >> c.log2_stride) <= a.merge_lim)) {
+        coarse_phase(c, a, p, ib, fd);
+        coarse_amps(c, a, p, ib, cc);
+        merged_left = 4;
+      }
+    }
+    if (MERGE && merged_left > 0) {
+      if constexpr (MERGE) coarse_to_fine(cc, 4 - merged_left, cf);   // the phase differences run on
+      --merged_left;
+    } else if (!all_out) {
       sub_phase(c, a, p, ib, fd);
       sub_amps(c, a, p, ib, cf);
     }

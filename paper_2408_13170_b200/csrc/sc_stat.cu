@@ -323,8 +323,14 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
       Timed tm(h, st, cls_dense);
       if (sizeof(R) == 4) {
         const ulonglong2* Dp = reinterpret_cast<const ulonglong2*>(h->D32);
+        // merged coarse intervals (see coarse_dslope): worth their test only where the coarse intervals are long; the
+        // fine sub-intervals may span kNodeDaysF32 / 4 days of signal time
+        const bool merge = dc.stride >= 512;
+        a.merge_lim = 86400.0 * (kNodeDaysF32 / 4.0) / h->cfg.T_obs_s;
         if (seg_mode) k_dense2<true, 0><<<grid, kBlock, 0, st>>>(dc, a, Dp);
+        else if (sincos == 2 && merge) k_dense2<false, 2, true><<<grid, kBlock, 0, st>>>(dc, a, Dp);
         else if (sincos == 2) k_dense2<false, 2><<<grid, kBlock, 0, st>>>(dc, a, Dp);
+        else if (merge) k_dense2<false, 0, true><<<grid, kBlock, 0, st>>>(dc, a, Dp);
         else k_dense2<false, 0><<<grid, kBlock, 0, st>>>(dc, a, Dp);
       } else {
         if (seg_mode) k_dense<true><<<grid, kBlock, kDense64Smem, st>>>(dc, a, h->W64, h->G64);
