@@ -490,7 +490,7 @@ def run_ours(args, rank, local_rank, world):
         roof = {"bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
                 "frac": (ach / peak) if ach else None, "traffic": dram_traffic_from_profile(),
                 "traffic_source": "profiles/r01g_k_dense2_full.md (ncu --set full, one launch, same command)",
-                "kernel": "k_dense2_ad<2>" if ad_N else "k_dense2<false,2>", "kernel_ms_per_launch": dense_avg,
+                "kernel": "k_dense2_ad<2,MERGE>" if ad_N else "k_dense2<false,2,MERGE>", "kernel_ms_per_launch": dense_avg,
                 "own_mix": {"what": "FP32 pipe of the kernel as built (packed FFMA2 loop): lane slots per evaluated "
                                     "particle-bin x evaluated particle-bins/s / (148 SM x 128 lanes x 1.965 GHz)",
                             "fp32_slots_per_bin": FP32_SLOTS_PER_BIN,

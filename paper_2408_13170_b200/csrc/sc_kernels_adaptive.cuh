@@ -104,7 +104,7 @@ __global__ void k_scan_chunks(double* __restrict__ cbase, int n_chunks, int P_pa
   }
 }
 
-template <int SC>
+template <int SC, bool MERGE = false>
 __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2_ad(DevCfg c, DenseArgs a, AdaptArgs ad,
                                                                       const ulonglong2* __restrict__ Dg) {
   constexpr int CH = kChunkF32;
@@ -166,6 +166,8 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2_ad(DevCfg c, 
   };
 
   PhaseFD ph = {};
+  float cc[MERGE ? 4 : 1][4];
+  int merged_left = 0;
   for (int ib = cs; ib < ce2; ib += Sf) {
     const int ie = min(ib + Sf, ce2);
     const bool lane_in = (ib >= jlo) && (ie <= jhi);
@@ -174,8 +176,23 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2_ad(DevCfg c, 
     const bool all_out = __all_sync(0xffffffffu, lane_out);
     if (all_out) continue;
     float cf[4][4];
-    sub_phase(c, a, p, ib, ph);
-    sub_amps(c, a, p, ib, cf);
+    // merged coarse intervals as in k_dense2 (the group and sub-interval moments stay those of the fine sub-intervals)
+    if constexpr (MERGE) {
+      if (merged_left == 0 && (ib & (c.stride - 1)) == 0 && ib + c.stride <= ce2 &&
+          __all_sync(0xffffffffu, (ib >= jlo) && (ib + c.stride <= jhi)) &&
+          __all_sync(0xffffffffu, coarse_dslope(c, a, p, ib >> c.log2_stride) <= a.merge_lim)) {
+        coarse_phase(c, a, p, ib, ph);
+        coarse_amps(c, a, p, ib, cc);
+        merged_left = 4;
+      }
+    }
+    if (MERGE && merged_left > 0) {
+      if constexpr (MERGE) coarse_to_fine(cc, 4 - merged_left, cf);
+      --merged_left;
+    } else {
+      sub_phase(c, a, p, ib, ph);
+      sub_amps(c, a, p, ib, cf);
+    }
     u64 s2 = f2pack(0.0f, hS);
     const ulonglong2* rec = sD + ((ib - cs) >> 1) * kPairRec;
     // First ask the question for the whole sub-interval (its moments are those k_sigma_chunks used): if no lane reaches its

@@ -653,7 +653,11 @@ int run_adaptive(sc_handle* h, const double* params, int64_t P, int n_seg, doubl
     {
       Timed tm(h, st, SC_TIME_DENSE);
       const ulonglong2* Dp = reinterpret_cast<const ulonglong2*>(h->D32);
-      if (sincos == 2) k_dense2_ad<2><<<grid, kBlock, 0, st>>>(dc, a, ad, Dp);
+      const bool merge = dc.stride >= 512;                     // as in run_batches
+      a.merge_lim = 86400.0 * (kNodeDaysF32 / 4.0) / h->cfg.T_obs_s;
+      if (sincos == 2 && merge) k_dense2_ad<2, true><<<grid, kBlock, 0, st>>>(dc, a, ad, Dp);
+      else if (sincos == 2) k_dense2_ad<2><<<grid, kBlock, 0, st>>>(dc, a, ad, Dp);
+      else if (merge) k_dense2_ad<0, true><<<grid, kBlock, 0, st>>>(dc, a, ad, Dp);
       else k_dense2_ad<0><<<grid, kBlock, 0, st>>>(dc, a, ad, Dp);
     }
     if ((rc = check_launch(h, "k_dense2_ad"))) return rc;
