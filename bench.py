@@ -37,7 +37,7 @@ NOMINAL_DFMA = 148 * 64 * 1.965e9   # 148 SMs x 64 FP64 lanes x max SM clock (B2
 # 26 packed FFMA2/FMUL2/FADD2 (2 slots each) + 3 scalar per bin PAIR; peak = 148 SMs x 128 FP32 lanes x max SM clock.
 FP32_SLOTS_PER_BIN = (26 * 2 + 3) / 2.0
 NOMINAL_FP32_SLOTS = 148 * 128 * 1.965e9
-DENSE_PROFILE = os.path.join(ROOT, "profiles", "r01g_k_dense2_full.md")
+DENSE_PROFILE = os.path.join(ROOT, "profiles", "r01h_k_dense2_full.md")
 
 
 def dram_traffic_from_profile():
@@ -489,7 +489,7 @@ def run_ours(args, rank, local_rank, world):
         pbs = eval_bins_launch / (dense_avg * 1e-3) if dense_avg > 0 else None
         roof = {"bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
                 "frac": (ach / peak) if ach else None, "traffic": dram_traffic_from_profile(),
-                "traffic_source": "profiles/r01g_k_dense2_full.md (ncu --set full, one launch, same command)",
+                "traffic_source": "profiles/r01h_k_dense2_full.md (ncu --set full, one launch, same command)",
                 "kernel": "k_dense2_ad<2,MERGE>" if ad_N else "k_dense2<false,2,MERGE>", "kernel_ms_per_launch": dense_avg,
                 "own_mix": {"what": "FP32 pipe of the kernel as built (packed FFMA2 loop): lane slots per evaluated "
                                     "particle-bin x evaluated particle-bins/s / (148 SM x 128 lanes x 1.965 GHz)",
