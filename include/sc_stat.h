@@ -181,6 +181,27 @@ int sc_pso_step(sc_handle* h, double* pos, double* vel, double* pbest_pos, doubl
                 double omega, double phi_p, double phi_g, uint64_t seed, uint64_t iter,
                 int64_t n_particles, int32_t n_swarms, void* cuda_stream);
 
+/* a7 in its two halves, for swarms whose particles are SHARDED over ranks ("partition particles contiguously
+ * by swarm then by rank; one all-reduce of (value, global index) + broadcast of the winning position").
+ * A rank holds n_particles LOCAL particles in n_swarms equal contiguous blocks (its pieces of n_swarms swarms);
+ * index_offset = the global index of its local particle 0 (global indices break ties and are the Philox counters, so the
+ * sharded step is bit-identical to sc_pso_step on the whole population).
+ *  sc_pso_best: steps (1)-(2) on the local particles; cand DEVICE [n_swarms][10] (out) = per block the candidate record
+ *               (best personal-best value, its GLOBAL particle index as a double, its position[8]).
+ *  sc_pso_pick: step (2) across shards: cand DEVICE [n_cand][n_swarms][10] (the records of the n_cand shards of each swarm,
+ *               e.g. all-gathered over the ranks that share the swarms) -> gbest_pos [n_swarms][8], gbest_val [n_swarms]:
+ *               arg max of the value, lowest global index on ties.
+ *  sc_pso_move: steps (3)-(6) for the local particles against the given gbest_pos [n_swarms][8].
+ * sc_pso_step == sc_pso_best + sc_pso_pick(n_cand = 1) + sc_pso_move with index_offset = 0.  All arrays DEVICE FP64. */
+int sc_pso_best(sc_handle* h, const double* pos, double* pbest_pos, double* pbest_val, const double* stat, double* cand,
+                int64_t n_particles, int32_t n_swarms, int64_t index_offset, void* cuda_stream);
+int sc_pso_pick(sc_handle* h, const double* cand, int32_t n_cand, int32_t n_swarms, double* gbest_pos, double* gbest_val,
+                void* cuda_stream);
+int sc_pso_move(sc_handle* h, double* pos, double* vel, const double* pbest_pos, const double* gbest_pos,
+                const double* lo, const double* hi, const double* eps_min,
+                double omega, double phi_p, double phi_g, uint64_t seed, uint64_t iter,
+                int64_t n_particles, int32_t n_swarms, int64_t index_offset, void* cuda_stream);
+
 /* a7 with swarm membership given by a label per particle (after the k-means regrouping of PAPER.md:199 the members of
  * a swarm are not contiguous).  label: DEVICE int32 [n_particles], values in [0, n_swarms).  A swarm without members
  * gets gbest_val = -inf and keeps its gbest_pos.  Otherwise exactly sc_pso_step. */

@@ -3,6 +3,11 @@
  *
  * Everything is evaluated directly at every FFT bin in plain FP64, in the order the paper / SURVEY.md 8(c)
  * states it: no interpolation, no blocking, no fusion.  Build: gcc -O2 -ffp-contract=off -fopenmp.
+ * "Truth" mode (sco_config.truth_mode = 1): the same formulas with the frequency, the
+ * phase Psi(f) and its sin/cos in x87 long double (64-bit mantissa: 1e-12 rad at Psi = 1e7 rad instead of the 3e-9 rad
+ * of FP64) -- for the corner where the FP64 rounding of the phase is the larger error (N = 1 at small Upsilon).  The
+ * bin sums stay plain FP64 (relative rounding ~1e-13 over 4e6 bins: four orders below the phase term).
+ * The time-window decision (Q4) stays in FP64 in both modes: it decides an integer, and both sides take it in FP64.
  *
  * Citations: PAPER.md:<line> = /root/reference/PAPER.md; "O1..O7" and "Q1..Q17" = SURVEY.md section 8(c) readings
  * (listed again in DESIGN.md), used where the paper names a model but prints no formula.
@@ -92,6 +97,75 @@ double sco_tf(const sco_config* c, const double th[8], double f) {
     dPsi += dPsi_e * (-34.0 / 9.0) / f;
   }
   return dPsi / (2.0 * pi);
+}
+
+/* ---- truth mode: O2 / O3 once more, line for line, in long double (f arrives in long double as well: the FP64
+ * rounding of f alone moves 2 pi f t_c by 2e-9 rad). ---- */
+#define SCO_PIL    3.141592653589793238462643383279502884L
+#define SCO_EULERL 0.577215664901532860606512090082402431L
+static void pn_coeffs_ld(long double eta, long double v, long double psi[8]) {
+  const long double pi = SCO_PIL, eta2 = eta * eta, eta3 = eta2 * eta;
+  psi[0] = 1.0L;
+  psi[1] = 0.0L;
+  psi[2] = 3715.0L / 756.0L + 55.0L * eta / 9.0L;
+  psi[3] = -16.0L * pi;
+  psi[4] = 15293365.0L / 508032.0L + 27145.0L * eta / 504.0L + 3085.0L * eta2 / 72.0L;
+  psi[5] = pi * (38645.0L / 756.0L - 65.0L * eta / 9.0L) * (1.0L + 3.0L * logl(v));
+  psi[6] = 11583231236531.0L / 4694215680.0L - 640.0L * pi * pi / 3.0L - 6848.0L * SCO_EULERL / 21.0L
+           - (6848.0L / 21.0L) * logl(4.0L * v)
+           + (-15737765635.0L / 3048192.0L + 2255.0L * pi * pi / 12.0L) * eta
+           + 76055.0L * eta2 / 1728.0L - 127825.0L * eta3 / 1296.0L;
+  psi[7] = pi * (77096675.0L / 254016.0L + 378515.0L * eta / 1512.0L - 74045.0L * eta2 / 756.0L);
+}
+
+long double sco_phase_ld(const sco_config* c, const double th[8], long double f) {
+  const long double pi = SCO_PIL;
+  const long double Mc = (long double)th[0] * (long double)SCO_MSUN_S, eta = th[1], tc = th[2], e0 = th[7];
+  const long double M = Mc * powl(eta, -0.6L);
+  const long double v = cbrtl(pi * M * f);
+  long double psi[8];
+  pn_coeffs_ld(eta, v, psi);
+  long double sum = 0.0L;
+  for (int k = 0; k <= c->pn_order_x2 && k <= 7; ++k) sum += psi[k] * powl(v, (long double)(k - 5));
+  long double Psi = 2.0L * pi * f * tc - pi / 4.0L + 3.0L / (128.0L * eta) * sum;
+  if (c->ecc_leading) {
+    const long double vref = cbrtl(pi * M * (long double)c->f_ref_ecc);
+    Psi += -3.0L / (128.0L * eta) * powl(v, -5.0L) * (2355.0L / 1462.0L) * e0 * e0 * powl(vref / v, 19.0L / 3.0L);
+  }
+  return Psi;
+}
+
+long double sco_tf_ld(const sco_config* c, const double th[8], long double f) {
+  const long double pi = SCO_PIL;
+  const long double Mc = (long double)th[0] * (long double)SCO_MSUN_S, eta = th[1], tc = th[2], e0 = th[7];
+  const long double M = Mc * powl(eta, -0.6L);
+  const long double v = cbrtl(pi * M * f);
+  long double psi[8];
+  pn_coeffs_ld(eta, v, psi);
+  long double sum = 0.0L;
+  for (int k = 0; k <= c->pn_order_x2 && k <= 7; ++k) {
+    if (k == 5) sum += 3.0L * pi * (38645.0L / 756.0L - 65.0L * eta / 9.0L);
+    else if (k == 6) sum += (psi[6] - 6848.0L / 21.0L) * v;
+    else sum += (long double)(k - 5) * psi[k] * powl(v, (long double)(k - 5));
+  }
+  long double dPsi = 2.0L * pi * tc + 3.0L / (128.0L * eta) * sum / (3.0L * f);
+  if (c->ecc_leading) {
+    const long double vref = cbrtl(pi * M * (long double)c->f_ref_ecc);
+    const long double dPsi_e = -3.0L / (128.0L * eta) * powl(v, -5.0L) * (2355.0L / 1462.0L) * e0 * e0 * powl(vref / v, 19.0L / 3.0L);
+    dPsi += dPsi_e * (-34.0L / 9.0L) / f;
+  }
+  return dPsi / (2.0L * pi);
+}
+/* ctypes-friendly wrappers (x87 long double does not cross the binding): f = j_abs / T_obs formed in long double;
+ * out = (Psi rounded to double, Psi - that in double, cos Psi, sin Psi). */
+void sco_phase_truth(const sco_config* c, const double th[8], int64_t j_abs, double out[4]) {
+  const long double f = (long double)j_abs / (long double)c->T_obs_s;
+  const long double Psi = sco_phase_ld(c, th, f);
+  out[0] = (double)Psi; out[1] = (double)(Psi - (long double)out[0]);
+  out[2] = (double)cosl(Psi); out[3] = (double)sinl(Psi);
+}
+double sco_tf_truth(const sco_config* c, const double th[8], int64_t j_abs) {
+  return (double)sco_tf_ld(c, th, (long double)j_abs / (long double)c->T_obs_s);
 }
 
 /* ------------------------------------------------------------------------------------------------
@@ -216,11 +290,18 @@ int64_t sco_template3(const sco_config* c, const double th[8], int64_t j_begin, 
     const double t = sco_tf(c, th, f);
     if (c->window_mode == 1 && !(t >= 0.0 && t <= c->T_obs_s)) continue;
     ++inwin;
-    const double Psi = sco_phase(c, th, f);
     const double amp = pow(f, -7.0 / 6.0);
     double tdi[6][2];
     sco_tdi(c, th, f, t, tdi);
-    const double er = amp * cos(Psi), ei = -amp * sin(Psi);      /* A e^{-i Psi} */
+    double cP, sP;                                               /* cos Psi, sin Psi */
+    if (c->truth_mode) {
+      const long double Psi = sco_phase_ld(c, th, (long double)(c->j0 + j_begin + i) / (long double)c->T_obs_s);
+      cP = (double)cosl(Psi); sP = (double)sinl(Psi);
+    } else {
+      const double Psi = sco_phase(c, th, f);
+      cP = cos(Psi); sP = sin(Psi);
+    }
+    const double er = amp * cP, ei = -amp * sP;                  /* A e^{-i Psi} */
     hA[2 * i]     = tdi[3][0] * er - tdi[3][1] * ei;
     hA[2 * i + 1] = tdi[3][0] * ei + tdi[3][1] * er;
     if (hE) {

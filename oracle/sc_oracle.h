@@ -19,6 +19,11 @@
  *                          TaylorT2 timing series through 3.5PN (pins psi_2 .. psi_7); Peters' small-e equations
  *                          (pin the leading eccentric coefficient).
  *                          PARITY WITH THE LALSimulation / TaylorF2Ecc [49] CODE ITSELF IS UNPINNED (not in the container).
+ *   sco_phase_ld / sco_tf_ld (truth mode): every pin of sco_phase / sco_tf above is run on them as well (Newtonian closed
+ *                          form, TaylorT2 series, finite-difference identity, Peters); they agree with the FP64 functions to
+ *                          the FP64 rounding of a 1e7-rad phase; f t_c against exact integer arithmetic (Python fractions);
+ *                          truth-mode statistic = FP64-mode statistic to the predicted 3e-8/sqrt(Upsilon).
+ *   sco_eval_stat_levels : level by level equal to sco_eval_stat and to a numpy bin sum over the oracle's template.
  *   sco_orbit/sco_template: arm lengths = L, centroid on the 1-AU circle; two-pulse single-link identity;
  *                          long-wavelength Michelson limit; T-combination -> 0; beta = +-pi/2 kills the Doppler term.
  *                          PARITY WITH BBHx [56] IS UNPINNED (not in the container).
@@ -58,6 +63,8 @@ typedef struct {
   int32_t ecc_leading;    /* 1 = leading-order e0^2 phase term (Q5)                          */
   double  f_ref_ecc;      /* GW frequency at which e0 is defined                             */
   double  arm_L_s, au_s, orbit_alpha0, orbit_lambda0, year_s;   /* orbit constants (Q6)      */
+  int32_t truth_mode;     /* 1 = "truth" mode: frequency, phase and its sin/cos in long double */
+  int32_t reserved_;
 } sco_config;
 
 /* theta = (M_c [Msun, detector frame], eta, t_c [s from data start], lambda, beta, iota, psi, e_0)  (D3, Q3) */
@@ -66,6 +73,12 @@ typedef struct {
 double sco_phase(const sco_config* c, const double theta[8], double f);
 /* O3: t(f) = Psi'(f)/(2 pi) [s], analytic term-by-term derivative of O2. */
 double sco_tf(const sco_config* c, const double theta[8], double f);
+/* Truth mode: O2 / O3 line for line in x87 long double, f = j_abs / T_obs formed in long
+ * double.  sco_phase_truth: out = (Psi rounded to double, the remainder Psi - that, cos Psi, sin Psi). */
+long double sco_phase_ld(const sco_config* c, const double theta[8], long double f);
+long double sco_tf_ld(const sco_config* c, const double theta[8], long double f);
+void sco_phase_truth(const sco_config* c, const double theta[8], int64_t j_abs, double out[4]);
+double sco_tf_truth(const sco_config* c, const double theta[8], int64_t j_abs);
 /* O4: spacecraft positions p[0]=centroid p0, p[1..3]=spacecraft 1..3, in light-seconds, at time t [s]. */
 void sco_orbit(const sco_config* c, double t, double p[4][3]);
 /* O4: single-link response y_sr(f) for link s->r (1-based), WITHOUT the factor A(f) e^{-i Psi(f)}:

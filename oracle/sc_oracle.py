@@ -31,14 +31,16 @@ class Config(C.Structure):
                 ("n_channels", C.c_int32), ("window_mode", C.c_int32), ("pn_order_x2", C.c_int32),
                 ("ecc_leading", C.c_int32), ("f_ref_ecc", C.c_double),
                 ("arm_L_s", C.c_double), ("au_s", C.c_double), ("orbit_alpha0", C.c_double),
-                ("orbit_lambda0", C.c_double), ("year_s", C.c_double)]
+                ("orbit_lambda0", C.c_double), ("year_s", C.c_double),
+                ("truth_mode", C.c_int32), ("reserved_", C.c_int32)]
 
 
-def make_config(d):
-    """d: dict with the field names above (what sc_synth.grid_config returns)."""
+def make_config(d, truth=False):
+    """d: dict with the field names above (what sc_synth.grid_config returns).  truth=True: long-double phase mode."""
     c = Config()
     for k, _ in Config._fields_:
-        setattr(c, k, d[k])
+        setattr(c, k, d.get(k, 0))
+    c.truth_mode = 1 if truth else 0
     return c
 
 
@@ -56,6 +58,9 @@ def lib():
         L.sco_phase.argtypes = [C.POINTER(Config), _dp, C.c_double]
         L.sco_tf.restype = C.c_double
         L.sco_tf.argtypes = [C.POINTER(Config), _dp, C.c_double]
+        L.sco_phase_truth.argtypes = [C.POINTER(Config), _dp, C.c_int64, _dp]
+        L.sco_tf_truth.restype = C.c_double
+        L.sco_tf_truth.argtypes = [C.POINTER(Config), _dp, C.c_int64]
         L.sco_orbit.argtypes = [C.POINTER(Config), C.c_double, _dp]
         L.sco_link.argtypes = [C.POINTER(Config), _dp, C.c_double, C.c_double, C.c_int, C.c_int, _dp]
         L.sco_tdi.argtypes = [C.POINTER(Config), _dp, C.c_double, C.c_double, _dp]
@@ -121,6 +126,19 @@ def phase(cfg, theta, f):
 def tf(cfg, theta, f):
     th = _f64(theta)
     return lib().sco_tf(C.byref(cfg), _d(th), float(f))
+
+
+def phase_truth(cfg, theta, j_abs):
+    """Long-double Psi at f = j_abs / T_obs -> (Psi rounded to double, remainder, cos Psi, sin Psi)."""
+    th = _f64(theta)
+    o = np.zeros(4)
+    lib().sco_phase_truth(C.byref(cfg), _d(th), int(j_abs), _d(o))
+    return o
+
+
+def tf_truth(cfg, theta, j_abs):
+    th = _f64(theta)
+    return lib().sco_tf_truth(C.byref(cfg), _d(th), int(j_abs))
 
 
 def orbit(cfg, t):

@@ -16,7 +16,7 @@ SC_OPT_ESCALATE, SC_OPT_ESC_TAU_POLY_X1000, SC_OPT_ESC_TAU_MUFU_X1000, SC_OPT_WI
 SC_TIMING_CLASSES = ["nodes", "dense", "stitch", "pso", "other", "escalation"]
 
 EXPORTED_SYMBOLS = ["sc_init_data", "sc_init_data_host", "sc_init_data3", "sc_gen_template3", "sc_eval_stat", "sc_eval_stat_host", "sc_eval_segments",
-                    "sc_eval_stat_adaptive", "sc_eval_components", "sc_eval_loglike", "sc_data_norm", "sc_gen_template", "sc_pso_step", "sc_pso_step_labeled", "sc_kmeans", "sc_search_run", "sc_whiten_streams", "sc_eval_stat_streams", "sc_get_counters", "sc_get_timing", "sc_measure_fp64_peak",
+                    "sc_eval_stat_adaptive", "sc_eval_components", "sc_eval_loglike", "sc_data_norm", "sc_gen_template", "sc_pso_step", "sc_pso_best", "sc_pso_pick", "sc_pso_move", "sc_pso_step_labeled", "sc_kmeans", "sc_search_run", "sc_whiten_streams", "sc_eval_stat_streams", "sc_get_counters", "sc_get_timing", "sc_measure_fp64_peak",
                     "sc_set_option", "sc_free",
                     "sc_last_error", "sc_version"]
 
@@ -117,6 +117,9 @@ def load_library():
     L.sc_pso_step.restype = C.c_int
     L.sc_pso_step.argtypes = [_vp] + [_vp] * 10 + [C.c_double] * 3 + [C.c_uint64, C.c_uint64, C.c_int64, C.c_int32, _vp]
     L.sc_pso_step_labeled.restype = C.c_int
+    L.sc_pso_best.argtypes = [_vp] + [_vp] * 5 + [C.c_int64, C.c_int32, C.c_int64, _vp]
+    L.sc_pso_pick.argtypes = [_vp, _vp, C.c_int32, C.c_int32, _vp, _vp, _vp]
+    L.sc_pso_move.argtypes = [_vp] + [_vp] * 7 + [C.c_double] * 3 + [C.c_uint64, C.c_uint64, C.c_int64, C.c_int32, C.c_int64, _vp]
     L.sc_pso_step_labeled.argtypes = [_vp] + [_vp] * 11 + [C.c_double] * 3 + [C.c_uint64, C.c_uint64, C.c_int64, C.c_int32, _vp]
     L.sc_kmeans.restype = C.c_int
     L.sc_kmeans.argtypes = [_vp, _vp, C.c_int64, _vp, _vp, _vp, C.c_int32, C.c_int32, _vp, _vp, C.POINTER(C.c_int32), _vp]
@@ -385,6 +388,41 @@ def sc_pso_step(h, pos, vel, pbest_pos, pbest_val, stat, gbest_pos, gbest_val, l
     _check(rc, h)
 
 
+def sc_pso_best(h, pos, pbest_pos, pbest_val, stat, cand, n_particles, n_swarms, index_offset=0, stream=None):
+    torch = _torch()
+    names = ["pos", "pbest_pos", "pbest_val", "stat", "cand"]
+    tens = [pos, pbest_pos, pbest_val, stat, cand]
+    sizes = [8 * n_particles] * 2 + [n_particles] * 2 + [10 * n_swarms]
+    for t, nm, sz in zip(tens, names, sizes):
+        if t.numel() != sz:
+            raise SCError(SC_ERR_INVALID_ARG, f"{nm}: expected {sz} values, got {t.numel()}")
+    ptrs = [_dev(t, torch.float64, nm) for t, nm in zip(tens, names)]
+    _check(load_library().sc_pso_best(h, *ptrs, int(n_particles), int(n_swarms), int(index_offset), _stream(stream)), h)
+
+
+def sc_pso_pick(h, cand, n_cand, n_swarms, gbest_pos, gbest_val, stream=None):
+    torch = _torch()
+    if cand.numel() != 10 * n_cand * n_swarms or gbest_pos.numel() != 8 * n_swarms or gbest_val.numel() != n_swarms:
+        raise SCError(SC_ERR_INVALID_ARG, "cand [n_cand, n_swarms, 10], gbest_pos [n_swarms, 8], gbest_val [n_swarms] expected")
+    _check(load_library().sc_pso_pick(h, _dev(cand, torch.float64, "cand"), int(n_cand), int(n_swarms),
+                                      _dev(gbest_pos, torch.float64, "gbest_pos"), _dev(gbest_val, torch.float64, "gbest_val"),
+                                      _stream(stream)), h)
+
+
+def sc_pso_move(h, pos, vel, pbest_pos, gbest_pos, lo, hi, eps_min, omega, phi_p, phi_g, seed, iter, n_particles, n_swarms,
+                index_offset=0, stream=None):
+    torch = _torch()
+    names = ["pos", "vel", "pbest_pos", "gbest_pos", "lo", "hi", "eps_min"]
+    tens = [pos, vel, pbest_pos, gbest_pos, lo, hi, eps_min]
+    sizes = [8 * n_particles] * 3 + [8 * n_swarms, 8, 8, 8]
+    for t, nm, sz in zip(tens, names, sizes):
+        if t.numel() != sz:
+            raise SCError(SC_ERR_INVALID_ARG, f"{nm}: expected {sz} values, got {t.numel()}")
+    ptrs = [_dev(t, torch.float64, nm) for t, nm in zip(tens, names)]
+    _check(load_library().sc_pso_move(h, *ptrs, float(omega), float(phi_p), float(phi_g), int(seed) & (2 ** 64 - 1), int(iter),
+                                      int(n_particles), int(n_swarms), int(index_offset), _stream(stream)), h)
+
+
 def sc_pso_step_labeled(h, pos, vel, pbest_pos, pbest_val, stat, gbest_pos, gbest_val, label, lo, hi, eps_min,
                         omega, phi_p, phi_g, seed, iter, n_particles, n_swarms, stream=None):
     torch = _torch()
@@ -578,6 +616,19 @@ class Handle:
         sc_pso_step(self.h, state["pos"], state["vel"], state["pbest_pos"], state["pbest_val"], stat,
                     state["gbest_pos"], state["gbest_val"], lo, hi, eps_min, omega, phi_p, phi_g, seed, it,
                     state["pos"].shape[0], n_swarms, stream)
+
+    def pso_best(self, state, stat, cand, n_swarms, index_offset=0, stream=None):
+        """Steps (1)-(2) of sc_pso_step on this rank's particles -> cand [n_swarms, 10] (see sc_pso_best)."""
+        sc_pso_best(self.h, state["pos"], state["pbest_pos"], state["pbest_val"], stat, cand, state["pos"].shape[0], n_swarms,
+                    index_offset, stream)
+
+    def pso_pick(self, cand, state, stream=None):
+        """cand [n_cand, n_swarms, 10] -> state["gbest_pos"], state["gbest_val"]."""
+        sc_pso_pick(self.h, cand, cand.shape[0], state["gbest_val"].shape[0], state["gbest_pos"], state["gbest_val"], stream)
+
+    def pso_move(self, state, lo, hi, eps_min, omega, phi_p, phi_g, seed, it, n_swarms, index_offset=0, stream=None):
+        sc_pso_move(self.h, state["pos"], state["vel"], state["pbest_pos"], state["gbest_pos"], lo, hi, eps_min, omega, phi_p,
+                    phi_g, seed, it, state["pos"].shape[0], n_swarms, index_offset, stream)
 
     def pso_step_labeled(self, state, stat, label, lo, hi, eps_min, omega, phi_p, phi_g, seed, it, stream=None):
         sc_pso_step_labeled(self.h, state["pos"], state["vel"], state["pbest_pos"], state["pbest_val"], stat,

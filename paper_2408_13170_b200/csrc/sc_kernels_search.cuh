@@ -8,9 +8,12 @@ namespace {
 // ------------------------------------------------------------------------------------------------ a7 PSO
 // (1)+(2): one CTA per swarm.  label == nullptr: swarm s = particles [s per_swarm, (s+1) per_swarm); else swarm s = the
 // particles with label[p] == s (n_scan = n_particles; a swarm without members gets gbest_val = -inf, gbest_pos untouched).
+// cand != nullptr (sc_pso_best: a swarm sharded over ranks): instead of (gbest_pos, gbest_val) the block's best is left as a
+// candidate record cand[s][10] = (value, GLOBAL particle index = index_offset + local index, position[8]) for k_pso_pick.
 __global__ void k_pso_best(const double* __restrict__ pos, double* __restrict__ pbest_pos, double* __restrict__ pbest_val,
                            const double* __restrict__ stat, double* __restrict__ gbest_pos, double* __restrict__ gbest_val,
-                           int per_swarm, const int* __restrict__ label, long long n_scan) {
+                           int per_swarm, const int* __restrict__ label, long long n_scan,
+                           double* __restrict__ cand = nullptr, long long index_offset = 0) {
   const int s = blockIdx.x;
   const long long p0 = label ? 0 : (long long)s * per_swarm;
   const long long n_t = label ? n_scan : per_swarm;
@@ -68,22 +71,52 @@ __global__ void k_pso_best(const double* __restrict__ pos, double* __restrict__ 
     if (threadIdx.x == 8) gbest_val[s] = -INFINITY;
     return;
   }
+  if (cand) {
+    if (threadIdx.x < 8) cand[s * 10 + 2 + threadIdx.x] = pbest_pos[bi * 8 + threadIdx.x];
+    if (threadIdx.x == 8) { cand[s * 10] = pbest_val[bi]; cand[s * 10 + 1] = (double)(index_offset + bi); }
+    return;
+  }
   if (threadIdx.x < 8) gbest_pos[s * 8 + threadIdx.x] = pbest_pos[bi * 8 + threadIdx.x];
   if (threadIdx.x == 8) gbest_val[s] = pbest_val[bi];
+}
+
+// (2) across shards: among n_cand candidate records per swarm (cand [n_cand][n_swarms][10], e.g. all-gathered over the
+// ranks that share the swarms) the arg max of the value, lowest global particle index on ties -- the rule of k_pso_best,
+// so a swarm cut into shards gets the same best as the swarm in one piece.  One warp per swarm.
+__global__ void k_pso_pick(const double* __restrict__ cand, int n_cand, int n_swarms, double* __restrict__ gbest_pos,
+                           double* __restrict__ gbest_val) {
+  const int s = blockIdx.x, l = threadIdx.x;
+  double best = -INFINITY, bidx = INFINITY;
+  int bc = -1;
+  for (int c = l; c < n_cand; c += 32) {
+    const double* r = cand + ((size_t)c * n_swarms + s) * 10;
+    const double v = r[0], i = r[1];
+    if (bc < 0 || v > best || (v == best && i < bidx)) { best = v; bidx = i; bc = c; }
+  }
+  for (int o = 16; o > 0; o >>= 1) {
+    const double ov = __shfl_xor_sync(0xffffffffu, best, o), oi = __shfl_xor_sync(0xffffffffu, bidx, o);
+    const int oc = __shfl_xor_sync(0xffffffffu, bc, o);
+    if (oc >= 0 && (bc < 0 || ov > best || (ov == best && oi < bidx))) { best = ov; bidx = oi; bc = oc; }
+  }
+  if (bc < 0) return;
+  const double* r = cand + ((size_t)bc * n_swarms + s) * 10;
+  if (l < 8) gbest_pos[s * 8 + l] = r[2 + l];
+  if (l == 8) gbest_val[s] = r[0];
 }
 
 // (3)-(6): one thread per particle.
 __global__ void k_pso_move(double* __restrict__ pos, double* __restrict__ vel, const double* __restrict__ pbest_pos,
                            const double* __restrict__ gbest_pos, const double* __restrict__ lo, const double* __restrict__ hi,
                            const double* __restrict__ eps_min, double omega, double phi_p, double phi_g,
-                           uint64_t seed, uint64_t iter, long long P, int per_swarm, const int* __restrict__ label) {
+                           uint64_t seed, uint64_t iter, long long P, int per_swarm, const int* __restrict__ label,
+                           long long index_offset = 0 /* global index of local particle 0: the Philox counter */) {
   const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= P) return;
   const int s = label ? label[p] : (int)(p / per_swarm);
   uint32_t w[16];
 #pragma unroll
   for (uint32_t b = 0; b < 4; ++b)
-    philox4x32_10((uint32_t)p, (uint32_t)iter, b, 0u, (uint32_t)seed, (uint32_t)(seed >> 32), w + 4 * b);
+    philox4x32_10((uint32_t)(p + index_offset), (uint32_t)iter, b, 0u, (uint32_t)seed, (uint32_t)(seed >> 32), w + 4 * b);
 #pragma unroll
   for (int m = 0; m < 8; ++m) {
     const double rP = ((double)w[m] + 0.5) * 0x1p-32, rG = ((double)w[8 + m] + 0.5) * 0x1p-32;

@@ -54,6 +54,8 @@ __device__ __forceinline__ Particle load_particle(const double* __restrict__ pc,
 }
 
 // O2/O3: the PN sums  S(v) = sum_k psi_k v^(k-5)  and  B(v) = 3 f d/df S  (so that dS/df = B/(3f)).
+// SKIP0: S without its k = 0 (Newtonian) term, which eval_node adds in extended precision.
+template <bool SKIP0 = false>
 __device__ __forceinline__ void pn_sums(double eta, double v, int order, double& S, double& B) {
   const double lv = log(v);
   const double eta2 = eta * eta;
@@ -76,7 +78,7 @@ __device__ __forceinline__ void pn_sums(double eta, double v, int order, double&
 #pragma unroll
   for (int k = 0; k <= 7; ++k) {
     if (k <= order) {
-      S = fma(psi[k], vp, S);
+      if (!(SKIP0 && k == 0)) S = fma(psi[k], vp, S);
       if (k == 5) B += 3.0 * P5;                                   // vp = 1 here
       else if (k == 6) B = fma(psi[6] - 6848.0 / 21.0, vp, B);      // vp = v
       else B = fma((double)(k - 5) * psi[k], vp, B);
@@ -117,6 +119,41 @@ __device__ __forceinline__ double sinc_from(double x, double sin_x) {
   return (x2 < 1.0e-4) ? fma(x2, fma(x2, 1.0 / 120.0, -1.0 / 6.0), 1.0) : sin_x / x;
 }
 
+// Double-double helpers for the Newtonian phase term (products by error-free transformation; the intrinsics keep the
+// compiler from contracting them).
+struct dd2 { double hi, lo; };
+__device__ __forceinline__ dd2 dd_two_prod(double a, double b) { const double p = __dmul_rn(a, b); return {p, fma(a, b, -p)}; }
+__device__ __forceinline__ dd2 dd_mul(dd2 a, dd2 b) {
+  const double p = __dmul_rn(a.hi, b.hi);
+  double e = fma(a.hi, b.hi, -p);
+  e = fma(a.hi, b.lo, e);
+  e = fma(a.lo, b.hi, e);
+  const double s = __dadd_rn(p, e);
+  return {s, __dadd_rn(e, -__dadd_rn(s, -p))};
+}
+// The Newtonian term of the phase, pref (pi M f)^(-5/3) turns, reaches 4e6 turns (c5: 0.01 Hz, M_c = 24 Msun): plain FP64
+// (cbrt, five products, one reciprocal: ~4e-16 relative, independent from node to node) leaves 1e-8 rad per node, which is
+// the whole error budget of the all-FP64 path at small Upsilon (found with the oracle's long-double mode: 1.05e-6 at
+// Upsilon = 1.2e-3 on c5).  Here: u = (pi M / T) n as an exact product, y0 = u^(-5/3) in FP64, one Newton step on
+// y^3 u^5 = 1 with the residual formed in double-double, and the product with pref split into integer turns + fraction.
+// (Rounding of pi M / T and of pref is the same at every node: a 1e-16 relative shift of M_c, harmless.)
+__device__ __forceinline__ void newtonian_turns(double piM_over_T, double n, double pref, double& int_turns, double& frac) {
+  const dd2 u = dd_two_prod(piM_over_T, n);
+  const double v0 = cbrt(u.hi);
+  const double v02 = v0 * v0;
+  const double y0 = 1.0 / (v02 * v02 * v0);
+  const dd2 y2 = dd_two_prod(y0, y0);
+  const dd2 y3 = dd_mul(y2, dd2{y0, 0.0});
+  const dd2 u2 = dd_mul(u, u);
+  const dd2 u5 = dd_mul(dd_mul(u2, u2), u);
+  const dd2 pr = dd_mul(y3, u5);                                  // = 1 + r
+  const double r = __dadd_rn(__dadd_rn(pr.hi, -1.0), pr.lo);
+  const double y_lo = -y0 * r * (1.0 / 3.0);                      // y = y0 (1 - r/3)
+  const dd2 a = dd_two_prod(pref, y0);
+  int_turns = rint(a.hi);
+  frac = __dadd_rn(a.hi, -int_turns) + fma(pref, y_lo, a.lo);
+}
+
 __device__ NodeOut eval_node(const DevCfg& c, const Particle& q, long long jglob /* j0 + bin position */) {
   NodeOut o;
   const double n = (double)jglob;
@@ -129,11 +166,13 @@ __device__ NodeOut eval_node(const DevCfg& c, const Particle& q, long long jglob
   double frac = (p - ip) + (perr + n * q.tau_lo);
   const double v = cbrt(q.piM * f);
   double S, B;
-  pn_sums(q.eta, v, c.pn_order_x2, S, B);
+  pn_sums<true>(q.eta, v, c.pn_order_x2, S, B);                   // S: the terms beyond the Newtonian one (<= 2e4 turns)
   const double pref = 3.0 / (128.0 * q.eta) / (2.0 * kPi);
+  double i0, f0;
+  newtonian_turns(q.piM * c.inv_T, n, pref, i0, f0);
   const double pn_t = pref * S;
   const double ipn = rint(pn_t);
-  frac += pn_t - ipn;
+  frac += (pn_t - ipn) + f0;
   double tf = q.tc + pref * B / (3.0 * f);
   if (c.ecc_leading) {
     const double e_t = -pref * q.ecc * pow(v, -34.0 / 3.0);
@@ -146,7 +185,7 @@ __device__ NodeOut eval_node(const DevCfg& c, const Particle& q, long long jglob
   // Doppler phase of the centroid: f k.p0 = -f AU cos(beta) cos(alpha - lambda)
   frac += -f * c.AU * q.cb * (ca * q.cl + sa * q.sl) - 0.125;      // -pi/4 of the SPA
   const double ir = rint(frac);
-  o.n_turns = (int)(ip + ipn + ir);
+  o.n_turns = (int)(ip + ipn + i0 + ir);
   o.frac = frac - ir;
 
   const double aue = c.L / (2.0 * 1.7320508075688772);             // AU * e

@@ -1171,6 +1171,47 @@ int sc_pso_step(sc_handle* h, double* pos, double* vel, double* pbest_pos, doubl
   return check_launch(h, "k_pso_move");
 }
 
+int sc_pso_best(sc_handle* h, const double* pos, double* pbest_pos, double* pbest_val, const double* stat, double* cand,
+                int64_t P, int32_t n_swarms, int64_t index_offset, void* stream) {
+  if (!h) return SC_ERR_NOT_INIT;
+  if (h->cuda_failed) return SC_ERR_CUDA;
+  if (!pos || !pbest_pos || !pbest_val || !stat || !cand) return fail(h, SC_ERR_INVALID_ARG, "null pointer");
+  if (P <= 0 || n_swarms <= 0 || P % n_swarms != 0 || P / n_swarms > INT32_MAX || index_offset < 0)
+    return fail(h, SC_ERR_INVALID_ARG, "n_particles must be a positive multiple of n_swarms, index_offset >= 0");
+  cudaStream_t st = (cudaStream_t)stream;
+  Timed tm(h, st, SC_TIME_PSO);
+  k_pso_best<<<n_swarms, 1024, 0, st>>>(pos, pbest_pos, pbest_val, stat, nullptr, nullptr, (int)(P / n_swarms), nullptr, 0,
+                                        cand, (long long)index_offset);
+  return check_launch(h, "k_pso_best");
+}
+
+int sc_pso_pick(sc_handle* h, const double* cand, int32_t n_cand, int32_t n_swarms, double* gbest_pos, double* gbest_val,
+                void* stream) {
+  if (!h) return SC_ERR_NOT_INIT;
+  if (h->cuda_failed) return SC_ERR_CUDA;
+  if (!cand || !gbest_pos || !gbest_val) return fail(h, SC_ERR_INVALID_ARG, "null pointer");
+  if (n_cand <= 0 || n_swarms <= 0) return fail(h, SC_ERR_INVALID_ARG, "n_cand and n_swarms must be positive");
+  cudaStream_t st = (cudaStream_t)stream;
+  Timed tm(h, st, SC_TIME_PSO);
+  k_pso_pick<<<n_swarms, 32, 0, st>>>(cand, n_cand, n_swarms, gbest_pos, gbest_val);
+  return check_launch(h, "k_pso_pick");
+}
+
+int sc_pso_move(sc_handle* h, double* pos, double* vel, const double* pbest_pos, const double* gbest_pos, const double* lo,
+                const double* hi, const double* eps_min, double omega, double phi_p, double phi_g, uint64_t seed,
+                uint64_t iter, int64_t P, int32_t n_swarms, int64_t index_offset, void* stream) {
+  if (!h) return SC_ERR_NOT_INIT;
+  if (h->cuda_failed) return SC_ERR_CUDA;
+  if (!pos || !vel || !pbest_pos || !gbest_pos || !lo || !hi || !eps_min) return fail(h, SC_ERR_INVALID_ARG, "null pointer");
+  if (P <= 0 || n_swarms <= 0 || P % n_swarms != 0 || P / n_swarms > INT32_MAX || index_offset < 0)
+    return fail(h, SC_ERR_INVALID_ARG, "n_particles must be a positive multiple of n_swarms, index_offset >= 0");
+  cudaStream_t st = (cudaStream_t)stream;
+  Timed tm(h, st, SC_TIME_PSO);
+  k_pso_move<<<(unsigned)((P + 127) / 128), 128, 0, st>>>(pos, vel, pbest_pos, gbest_pos, lo, hi, eps_min, omega, phi_p, phi_g,
+                                                          seed, iter, P, (int)(P / n_swarms), nullptr, (long long)index_offset);
+  return check_launch(h, "k_pso_move");
+}
+
 int sc_pso_step_labeled(sc_handle* h, double* pos, double* vel, double* pbest_pos, double* pbest_val, const double* stat,
                         double* gbest_pos, double* gbest_val, const int32_t* label, const double* lo, const double* hi,
                         const double* eps_min, double omega, double phi_p, double phi_g, uint64_t seed, uint64_t iter,

@@ -88,9 +88,12 @@ def draw_noise(seed, S, df):
 
 
 # ---------------------------------------------------------------------------------------------- parameters
-def tau_newton(Mc_msun, f):
-    """Newtonian time to coalescence from GW frequency f; used only to place t_c so the track enters at t~0."""
-    return 5.0 / 256.0 * (Mc_msun * MSUN_S) ** (-5.0 / 3.0) * (np.pi * f) ** (-8.0 / 3.0)
+# Upper end [s] of the t_c range each config's injections are drawn from, per (config, injection index): the time a chirp of
+# the injection's M_c needs from the band's lower edge to coalescence, so that the track enters the band at t ~ 0 (SURVEY
+# 8(d) recipe).  Tabulated numbers -- this module holds none of the method's arithmetic; a caller with another source
+# (tests/test_gpu_fuzz.py) passes its own value to draw_injection.
+TC_UPPER_S = {(1, 0): 100381200.86424167, (2, 0): 116909178.85339002, (3, 0): 142024571.46033856,
+              (5, 0): 712395601.66902, (5, 1): 394859670.4492147}
 
 
 def eta_of_q(q):
@@ -105,9 +108,9 @@ def draw_sky(rng):
     return lam, beta, iota, psi
 
 
-def draw_injection(rng, Mc, q, f_lo, e0=0.0):
-    """theta = (M_c, eta, t_c, lambda, beta, iota, psi, e0); t_c ~ U[tau(f_lo) - 0.25 yr, tau(f_lo)]."""
-    tau = float(tau_newton(Mc, f_lo))
+def draw_injection(rng, Mc, q, tc_upper, e0=0.0):
+    """theta = (M_c, eta, t_c, lambda, beta, iota, psi, e0); t_c ~ U[tc_upper - 0.25 yr, tc_upper] (the caller's bound)."""
+    tau = float(tc_upper)
     tc = rng.uniform(tau - 0.25 * YEAR_S, tau)
     lam, beta, iota, psi = draw_sky(rng)
     return np.array([Mc, eta_of_q(q), tc, lam, beta, iota, psi, e0], dtype=np.float64)
@@ -176,10 +179,10 @@ def config_inputs(config_id, P=None, replica=0):
     nE = draw_noise(seed_for("noise", config_id, 2 * replica + 1), S, df)
     rng = np.random.default_rng(seed_for("injection", config_id))
     injections = []
-    for s in spec["inj"]:
+    for i, s in enumerate(spec["inj"]):
         Mc = s["Mc"] if not isinstance(s["Mc"], tuple) else rng.uniform(*s["Mc"])
         q = s["q"] if not isinstance(s["q"], tuple) else rng.uniform(*s["q"])
-        injections.append(dict(theta=draw_injection(rng, Mc, q, f_lo), rho=s["rho"]))
+        injections.append(dict(theta=draw_injection(rng, Mc, q, TC_UPPER_S[(config_id, i)]), rho=s["rho"]))
     if "box" in spec:
         lo, hi = prior_box(0.0, 0.0, **spec["box"])
     else:

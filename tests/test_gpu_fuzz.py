@@ -1,7 +1,8 @@
 """Randomised GPU-vs-oracle parity (all `-m gpu`): grids, tiles, populations and edge lists the named configs do not
 visit -- odd bin counts, bands and observation times that give other node spacings, particles whose time windows
 (Q4) lie partly or wholly outside the band, irregular / partial / repeated segment edges, populations that are not
-a multiple of the 128-particle block.  Every particle is compared (<= 1e-6 relative, north_star; see the conditioning note in the test); inputs are seeded."""
+a multiple of the 128-particle block.  Every particle is compared (<= 1e-6 relative, north_star, flat: the reference is the oracle's long-double truth mode);
+inputs are seeded."""
 import numpy as np
 import pytest
 
@@ -23,7 +24,10 @@ def _case(seed):
     S = sy.psd_AE(f)
     df = 1.0 / cfg["T_obs_s"]
     Mc, q = float(rng.uniform(18.0, 45.0)), float(rng.uniform(0.5, 1.0))
-    th = sy.draw_injection(rng, Mc, q, f_lo)
+    # t_c such that the track enters the band near t = 0: Newtonian time to coalescence from f_lo (closed form of
+    # test_oracle_waveform.test_tf_newtonian_closed_form)
+    tau = 5.0 / 256.0 * (Mc * sy.MSUN_S) ** (-5.0 / 3.0) * (np.pi * f_lo) ** (-8.0 / 3.0)
+    th = sy.draw_injection(rng, Mc, q, tau)
     # a tile around the source, wide enough in t_c that many windows start or end inside the band or miss it
     lo, hi = sy.prior_box(th[0], th[2], eta_lo=0.16, dMc=float(rng.uniform(0.2, 2.0)),
                           dtc=float(rng.uniform(0.2, 1.5)) * T_yr * sy.YEAR_S)
@@ -55,7 +59,10 @@ def test_random_grids_tiles_and_edges(oracle, seed):
     if seed % 2:
         H.set_option(sc.SC_OPT_TC_MAX_S, int(np.ceil(max(inp["hi"][2], 1.0))))
     par = torch.from_numpy(inp["particles"]).to("cuda:0")
-    ref = oracle.eval_stat_levels(cfg, dA, dE, inp["S_A"], inp["S_E"], inp["particles"], lists)
+    # reference in the oracle's truth mode (long-double phase): Psi ~ 2 pi f t_c reaches 5e7 rad on these tiles, where the
+    # FP64 oracle's own per-bin rounding (1.3e-8 rad rms) would exceed the bar for Upsilon << 1; with it the bar is flat
+    cfg_truth = oracle.make_config(inp["cfg"], truth=True)
+    ref = oracle.eval_stat_levels(cfg_truth, dA, dE, inp["S_A"], inp["S_E"], inp["particles"], lists)
     n_live = 0
     for e, r in zip(lists, ref):
         got = H.eval_stat(par, e.astype(np.int32)).cpu().numpy()
@@ -65,13 +72,6 @@ def test_random_grids_tiles_and_edges(oracle, seed):
         n_live += int(ok.sum())
         if ok.any():
             err = rel_err(got[ok], r[ok])
-            # the oracle evaluates Psi(f) ~ 2 pi f t_c (up to 5e7 rad on these
-            # tiles) in plain FP64, i.e. with independent per-bin rounding noise of a few units of 2^-53 Psi (measured:
-            # white, rms 1.3e-8 rad at Psi = 4.5e7 rad, while the library reduces f t_c exactly); that noise moves
-            # Upsilon by ~2.8 eps / sqrt(Upsilon) relative, which exceeds 1e-6 only for Upsilon << 1
-            psi_max = 2.0 * np.pi * float(inp["cfg"]["j0"] + inp["cfg"]["n_bins"]) / inp["cfg"]["T_obs_s"] * float(inp["hi"][2])
-            bar = np.maximum(TOL, 30.0 * 2.0 ** -53 * psi_max / np.sqrt(r[ok]))
-            assert np.all(err <= bar), (seed, len(e), float(err.max()), float(r[ok][np.argmax(err)]))
-            assert np.all(err[r[ok] >= 0.05] <= TOL)
+            assert np.all(err <= TOL), (seed, len(e), float(err.max()), float(r[ok][np.argmax(err)]))
     assert n_live > 0
     H.close()
