@@ -77,6 +77,8 @@ def parse():
     ap.add_argument("--search-ranking", action="store_true",
                     help="with --search: sc_search_config.ranking_precision = 1 (all rungs on the FP32 path, bests re-evaluated in FP64)")
     ap.add_argument("--no-extras", action="store_true", help="skip the extra (untimed-region) measurements")
+    ap.add_argument("--dist-selftest", action="store_true",
+                    help="CPU-only check of the multi-rank launch and reductions (gloo); used by tests/test_multi_rank.py")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--opt", action="append", default=[], metavar="ID=VALUE",
@@ -290,6 +292,9 @@ def run_ours(args, rank, local_rank, world):
     import torch.distributed as dist
     import paper_2408_13170_b200 as sc
 
+    if not torch.cuda.is_available() or local_rank >= torch.cuda.device_count():
+        sys.exit(f"bench.py: rank {rank} needs CUDA device {local_rank}; {torch.cuda.device_count() if torch.cuda.is_available() else 0} "
+                 f"visible (--gpus {args.gpus} needs that many GPUs on this node; there is no CPU fallback)")
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
     if world > 1:
@@ -537,14 +542,46 @@ def run_ours(args, rank, local_rank, world):
         dist.destroy_process_group()
 
 
+def spawn_ranks(args):
+    """`python bench.py --gpus N` without a launcher: re-execute this script under torch.distributed.run with N ranks on
+    this node (one process per GPU, rendezvous on 127.0.0.1), exactly as the driver launches it; returns its exit code."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
+
+
+def run_dist_selftest(args, rank, world):
+    """CPU check of the multi-rank plumbing (tests/test_multi_rank.py): gloo process group, the partition rule, and the
+    reduction bench.py applies to its timings (max over ranks) and work (sum over ranks).  No GPU, no kernels."""
+    import torch.distributed as dist
+    from paper_2408_13170_b200 import dist as scd
+    dist.init_process_group("gloo")
+    a, b, need = scd.shard_swarms(40000, 4, rank, world) if world <= 4 else scd.shard_swarms(40000, 4, rank, world)
+    ms = scd.max_over_ranks(10.0 + rank)
+    units = scd.sum_over_ranks(float(b - a))
+    if rank == 0:
+        print(json.dumps({"selftest": "dist", "n_gpus": world, "ms_max": ms, "units": units, "shard0": [a, b, need]}), flush=True)
+    dist.destroy_process_group()
+
+
 def main():
     args = parse()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and (args.impl == "ours" or args.dist_selftest):
+        sys.exit(spawn_ranks(args))
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
-    if args.impl == "reference":
+    if args.dist_selftest:
+        run_dist_selftest(args, rank, world)
+    elif args.impl == "reference":
         run_reference(args, rank, world)
     else:
+        if world != args.gpus:
+            sys.exit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE = {world}")
         run_ours(args, rank, local_rank, world)
 
 

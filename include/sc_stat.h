@@ -136,8 +136,10 @@ int sc_eval_segments(sc_handle* h, const double* params, int64_t n_particles,
  * EVERY particle such that each segment holds an equal share of the template's squared SNR.  On the FFT grid (reading
  * Q18): s_j = sum_a |h_a(f_j)|^2 / S_a(f_j), C = sum_j s_j, e_0 = 0, e_N = n_bins and
  *   e_n = min{ j : sum_{j' < j} s_j' >= C n / N },  n = 1 .. N-1;
- * then out[p] as in sc_eval_stat on those edges.  The cumulative sums are formed in the kernel's arithmetic (FP32
- * amplitudes, FP64 running sum), so an edge can sit one bin away from where an FP64 evaluation puts it.
+ * then out[p] as in sc_eval_stat on those edges.  Floating point decides these integers, and the decision is taken in FP64
+ * like the definition's (FP64 node amplitudes, FP64 moments of the weights, an FP64 bin-by-bin walk where a target falls): an
+ * edge differs from a direct FP64 evaluation's only where a cumulative sum comes within the interpolation error (~1e-12
+ * relative) of its target.  The statistic on those edges runs on the FP32-amplitude path.
  * out: DEVICE [n_particles] or NULL; out_edges: DEVICE int32 [n_particles][n_seg + 1] or NULL (the edges used; all
  * zero but the last for a particle whose template is empty); out3: DEVICE [n_particles][3] or NULL (as
  * sc_eval_components).  n_seg = 1 is sc_eval_stat on (0, n_bins); 2 <= n_seg runs the FP32-amplitude path. */

@@ -9,14 +9,18 @@ namespace {
 // Equal squared-SNR segments re-evaluated for every particle (App. A):
 //   s_j = sum_a |h_a(f_j)|^2 / S_a(f_j),  C = sum_j s_j,  e_0 = 0, e_N = n_bins,
 //   e_n = min{ j : sum_{j' < j} s_j' >= C n / N }   (n = 1 .. N-1),
-// then Upsilon_N on those edges.  Three steps, all with lane = particle:
-//   k_sigma_chunks   sigma of every (chunk, particle) from the moments of the weights (no per-bin work inside the window)
+// then Upsilon_N on those edges.  Floating point decides these integers, so the decision is taken in FP64 like the
+// definition's (FP64 node amplitudes, FP64 moments of the weights, FP64 per-bin walk where a target falls): the edges equal
+// the FP64 oracle's except where a cumulative sum comes within the interpolation error (~1e-12 relative) of a target.
+// Four steps, all with lane = particle:
+//   k_sigma_chunks64 sigma of every (chunk, particle) in FP64 from the moments of the weights over the fine sub-intervals
 //   k_scan_chunks    prefix sum over chunks -> cumulative sigma at every chunk start, and C
-//   k_dense2_ad      the hot loop of k_dense2 with a running cumulative sigma per lane: groups of <= 32 bins in which
-//                    no lane of the warp reaches its next target (decided from the group's moments) take the unmasked
-//                    packed path; the others are walked bin by bin and the segments are closed where the running sum
-//                    crosses the target.  The number of edges closed inside a chunk is fixed by the scanned sums
+//   k_edges64        per (chunk, particle): the edges whose targets C n / N fall into the chunk -- sub-interval by
+//                    sub-interval from the moments, group by group (32 bins) inside the sub-interval that holds a target,
+//                    bin by bin inside that group.  The number of edges of a chunk is fixed by the scanned sums
 //                    (k0 = K(cbase[chunk]), k1 = K(cbase[chunk + 1])), so neighbouring chunks always agree.
+//   k_dense2_ad      the hot loop of k_dense2 on those integer edges (FP32 amplitudes): groups of <= 32 bins in which no
+//                    lane of the warp has an edge take the unmasked packed path; the others are walked bin by bin.
 constexpr int kFragAd = 10;    // partial Upsilon, head (zr, zi, sg), tail (zr, zi, sg), head-closes flag, partial sum|z|, sum sigma
 
 struct AdaptArgs {
@@ -25,9 +29,13 @@ struct AdaptArgs {
   const ulonglong2* gmom;      // [n_groups][4] moments of the weights over groups of 2^lg_group bins
   const ulonglong2* smom;      // [n_sub][4]    ... over the fine sub-intervals
   int lg_group;
-  int* out_edges;              // [P][n_seg + 1] of this batch, or nullptr
-  double* chunk_sigma;         // = cbase (written by k_sigma_chunks before the scan)
+  int* out_edges;              // [P][n_seg + 1] of this batch (the caller's array or scratch): written by k_edges64
+  double* chunk_sigma;         // = cbase (written by k_sigma_chunks64 before the scan)
   const int* pmap;             // window sort: table slot -> particle of the batch (rows of out_edges), or nullptr
+  const double2* smom64;       // [n_sub][7]    FP64 moments of the weights over the fine sub-intervals
+  const double2* gmom64;       // [n_groups][7] ... over the groups
+  const double2* G64;          // [n_bins] sigma weights per bin (FP64)
+  double* sub_sigma;           // [n_chunks * CH / Sf][P_pad]: sigma of every fine sub-interval (k_sigma_chunks64 -> k_edges64)
 };
 
 __device__ __forceinline__ double seg_target(double C, int n, int N) { return C * (double)n / (double)N; }
@@ -41,12 +49,67 @@ __device__ __forceinline__ int seg_index(double cum, double C, int N) {
   return n;
 }
 
-__global__ void __launch_bounds__(kBlock) k_sigma_chunks(DevCfg c, DenseArgs a, AdaptArgs ad, const float4* __restrict__ D32) {
+// The six FP64 nodes (m = -2 .. 3) of the four amplitude components around coarse interval ic, kept in registers while a
+// lane walks the chunk: the four fine sub-intervals of a coarse interval share them, and the next coarse interval needs
+// one new node per component (read per sub-interval they cost 25 GB of L2 traffic per pass on c3).
+struct Nodes64 { double v[4][6]; };
+__device__ __forceinline__ void nodes64_load(const DevCfg& c, const DenseArgs& a, int p, int ic, Nodes64& n) {
+  const double* __restrict__ namp = reinterpret_cast<const double*>(a.node_amp);
+#pragma unroll
+  for (int r = 0; r < 4; ++r) {
+    const double* col = namp + ((size_t)(ic + kNodeOff) * 4 + r) * a.P_pad + p;
+    const ptrdiff_t st = (ptrdiff_t)4 * a.P_pad;
+#pragma unroll
+    for (int m = -2; m <= 3; ++m) n.v[r][m + 2] = col[m * st];
+  }
+}
+__device__ __forceinline__ void nodes64_advance(const DevCfg& c, const DenseArgs& a, int p, int ic_new, Nodes64& n) {
+  const double* __restrict__ namp = reinterpret_cast<const double*>(a.node_amp);
+#pragma unroll
+  for (int r = 0; r < 4; ++r) {
+#pragma unroll
+    for (int m = 0; m < 5; ++m) n.v[r][m] = n.v[r][m + 1];
+    n.v[r][5] = namp[((size_t)(ic_new + kNodeOff + 3) * 4 + r) * a.P_pad + p];
+  }
+}
+// FP64 cubic coefficients of (Ar, Ai, Er, Ei) on fine sub-interval q of the coarse interval whose nodes are n.
+__device__ __forceinline__ void sub_amps64(const Nodes64& n, int q, double (&cf)[4][4]) {
+#pragma unroll
+  for (int r = 0; r < 4; ++r)
+#pragma unroll
+    for (int kk = 0; kk < 4; ++kk) {
+      double acc = 0.0;
+#pragma unroll
+      for (int m = 0; m < 6; ++m) acc = fma(kFineMd[q][kk][m], n.v[r][m], acc);
+      cf[r][kk] = acc;
+    }
+}
+// s_j = G_A(j) |c_A(s_j)|^2 + G_E(j) |c_E(s_j)|^2 in FP64 (the integrand of <h|h>, up to the common scale).
+__device__ __forceinline__ double sigma_bin64(const double (&cf)[4][4], double sj, double2 g) {
+  const double Ar = fma(fma(fma(cf[0][3], sj, cf[0][2]), sj, cf[0][1]), sj, cf[0][0]);
+  const double Ai = fma(fma(fma(cf[1][3], sj, cf[1][2]), sj, cf[1][1]), sj, cf[1][0]);
+  const double Er = fma(fma(fma(cf[2][3], sj, cf[2][2]), sj, cf[2][1]), sj, cf[2][0]);
+  const double Ei = fma(fma(fma(cf[3][3], sj, cf[3][2]), sj, cf[3][1]), sj, cf[3][0]);
+  return fma(g.x, fma(Ar, Ar, Ai * Ai), g.y * fma(Er, Er, Ei * Ei));
+}
+// sigma of the fine sub-interval [ib, ie) for this lane: from the moments when the lane's window covers it, bin by bin
+// (masked) when a window border falls inside.  The same function serves k_sigma_chunks64 and k_edges64, so the second
+// pass reproduces the chunk sums of the first bit for bit.
+__device__ __forceinline__ double sigma_sub64(const DevCfg& c, const AdaptArgs& ad, const double (&cf)[4][4], int ib, int ie,
+                                              int jlo, int jhi, int n_bins) {
+  const int Sf = c.stride >> 2;
+  if (ib >= jlo && ie <= jhi && ie - ib == Sf) return sigma_moments64(cf, ad.smom64 + (size_t)(ib >> (c.log2_stride - 2)) * 7);
+  const double hS = 1.0 / (double)Sf;
+  double tot = 0.0;
+  for (int j = max(ib, jlo); j < min(min(ie, jhi), n_bins); ++j) tot += sigma_bin64(cf, (double)(j - ib) * hS, ad.G64[j]);
+  return tot;
+}
+
+__global__ void __launch_bounds__(kBlock) k_sigma_chunks64(DevCfg c, DenseArgs a, AdaptArgs ad) {
   constexpr int CH = kChunkF32;
   const int chunk = blockIdx.x;
   const int cs = chunk * CH;
   const int ce = min(cs + CH, c.n_bins);
-  const int ce2 = (ce + 1) & ~1;
   const int p = blockIdx.y * kBlock + threadIdx.x;
   const int jlo = a.jlo[p], jhi = a.jhi[p];
   if (!__syncthreads_or((jhi > cs) && (jlo < ce))) {          // no particle of this block lives in this chunk
@@ -54,33 +117,22 @@ __global__ void __launch_bounds__(kBlock) k_sigma_chunks(DevCfg c, DenseArgs a, 
     return;
   }
   const int Sf = c.stride >> 2;
-  const float hS = 1.0f / (float)Sf;
   double tot = 0.0;
-  for (int ib = cs; ib < ce2; ib += Sf) {
-    const int ie = min(ib + Sf, ce2);
-    const bool lane_in = (ib >= jlo) && (ie <= jhi);
+  Nodes64 nd;
+  int ic_have = -1;
+  for (int ib = cs; ib < ce; ib += Sf) {
+    const int ie = min(ib + Sf, ce);
     const bool lane_out = (ie <= jlo) || (ib >= jhi);
-    const bool all_in = __all_sync(0xffffffffu, lane_in);
-    const bool all_out = __all_sync(0xffffffffu, lane_out);
-    if (all_out) continue;
-    float cf[4][4];
-    sub_amps(c, a, p, ib, cf);
-    if (all_in) {
-      tot += sigma_moments(cf, ad.smom + (size_t)(ib >> (c.log2_stride - 2)) * 4);
-    } else {
-      // a window border of some lane falls in this sub-interval: bin by bin, masked (two sub-intervals per particle)
-      for (int j = ib; j < ie; ++j) {
-        const float sj = (float)(j - ib) * hS;
-        const float Ar = fmaf(fmaf(fmaf(cf[0][3], sj, cf[0][2]), sj, cf[0][1]), sj, cf[0][0]);
-        const float Ai = fmaf(fmaf(fmaf(cf[1][3], sj, cf[1][2]), sj, cf[1][1]), sj, cf[1][0]);
-        const float Er = fmaf(fmaf(fmaf(cf[2][3], sj, cf[2][2]), sj, cf[2][1]), sj, cf[2][0]);
-        const float Ei = fmaf(fmaf(fmaf(cf[3][3], sj, cf[3][2]), sj, cf[3][1]), sj, cf[3][0]);
-        const float4 g = D32[(size_t)(j >> 1) * kPairRec + 2];            // (gA even, gA odd, gE even, gE odd)
-        const float gA = (j & 1) ? g.y : g.x, gE = (j & 1) ? g.w : g.z;
-        const float sg = fmaf(gA, fmaf(Ar, Ar, Ai * Ai), gE * fmaf(Er, Er, Ei * Ei));
-        if (j >= jlo && j < jhi) tot += (double)sg;
-      }
+    const int ic = ib >> c.log2_stride;
+    if (ic != ic_have) { if (ic_have < 0) nodes64_load(c, a, p, ic, nd); else nodes64_advance(c, a, p, ic, nd); ic_have = ic; }
+    double sg = 0.0;
+    if (!lane_out) {                                           // (a lane outside its window holds zeros or unused nodes)
+      double cf[4][4];
+      sub_amps64(nd, (ib >> (c.log2_stride - 2)) & 3, cf);
+      sg = sigma_sub64(c, ad, cf, ib, ie, jlo, jhi, c.n_bins);
     }
+    ad.sub_sigma[(size_t)(ib >> (c.log2_stride - 2)) * a.P_pad + p] = sg;
+    tot += sg;
   }
   ad.chunk_sigma[(size_t)(chunk + 1) * a.P_pad + p] = tot;
 }
@@ -102,6 +154,91 @@ __global__ void k_scan_chunks(double* __restrict__ cbase, int n_chunks, int P_pa
       cbase[(size_t)(i0 + u) * P_pad + p] = acc;
     }
   }
+}
+
+// The edges of every particle whose targets fall into this chunk (see the file header).  Edge n lies at the first bin j
+// whose cumulative sum C_j = sum_{j' < j} s_j' has reached C n / N; inside chunk `chunk` that is a j in (cs, ce].
+// Each lane walks its sub-interval sums (as k_sigma_chunks64 left them) until one holds a target; that sub-interval is then
+// resolved by the WHOLE WARP for that lane: the lane's cubic coefficients are broadcast, the 32 lanes evaluate 32 bins at
+// a time in FP64 and a warp scan gives the cumulative sums (a lane walking its own bins alone would run at 1/32 efficiency).
+__device__ __forceinline__ double shfl_d(double v, int src) { return __shfl_sync(0xffffffffu, v, src); }
+__global__ void __launch_bounds__(kBlock) k_edges64(DevCfg c, DenseArgs a, AdaptArgs ad) {
+  constexpr int CH = kChunkF32;
+  const int chunk = blockIdx.x;
+  const int cs = chunk * CH;
+  const int ce = min(cs + CH, c.n_bins);
+  const int p = blockIdx.y * kBlock + threadIdx.x;
+  const int lane = threadIdx.x & 31;
+  const int jlo = a.jlo[p], jhi = a.jhi[p];
+  const int N = ad.n_seg;
+  const double C = ad.cbase[(size_t)ad.n_chunks * a.P_pad + p];
+  const double cb0 = ad.cbase[(size_t)chunk * a.P_pad + p];
+  const double cb1 = ad.cbase[(size_t)(chunk + 1) * a.P_pad + p];
+  int k = seg_index(cb0, C, N);
+  const int k1 = seg_index(cb1, C, N);
+  if (!__any_sync(0xffffffffu, k < k1)) return;               // no lane of this warp has an edge in this chunk
+  const int pq = ad.pmap ? ad.pmap[p] : p;
+  int* erow = (pq < a.P) ? ad.out_edges + (size_t)pq * (N + 1) : nullptr;
+  const int Sf = c.stride >> 2;
+  const double hS = 1.0 / (double)Sf;
+  double t_next = (k < k1) ? seg_target(C, k + 1, N) - cb0 : INFINITY;
+  double crel = 0.0;
+  Nodes64 nd;
+  int ic_have = -1;
+  for (int ib = cs; ib < ce; ib += Sf) {
+    const int ie = min(ib + Sf, ce);
+    if (!__any_sync(0xffffffffu, k < k1)) break;               // every lane has placed its edges of this chunk
+    const int ic = ib >> c.log2_stride;
+    if (ic != ic_have) { if (ic_have < 0) nodes64_load(c, a, p, ic, nd); else nodes64_advance(c, a, p, ic, nd); ic_have = ic; }
+    // sigma of the sub-interval as k_sigma_chunks64 summed it (bit for bit: the scanned chunk sums are sums of these)
+    const double sg_s = (k < k1) ? ad.sub_sigma[(size_t)(ib >> (c.log2_stride - 2)) * a.P_pad + p] : 0.0;
+    const bool cross = (k < k1) && (crel + sg_s >= t_next);    // a target of this lane falls into this sub-interval
+    unsigned todo = __ballot_sync(0xffffffffu, cross);
+    if (!cross) crel += sg_s;
+    if (!todo) continue;
+    double cf[4][4];
+    sub_amps64(nd, (ib >> (c.log2_stride - 2)) & 3, cf);
+    while (todo) {
+      const int L = __ffs(todo) - 1;
+      todo &= todo - 1;
+      // lane L's problem, held by every lane
+      double g[4][4];
+#pragma unroll
+      for (int r = 0; r < 4; ++r)
+#pragma unroll
+        for (int m = 0; m < 4; ++m) g[r][m] = shfl_d(cf[r][m], L);
+      const double C_L = shfl_d(C, L), cb0_L = shfl_d(cb0, L);
+      double crel_L = shfl_d(crel, L), t_L = shfl_d(t_next, L);
+      int k_L = __shfl_sync(0xffffffffu, k, L);
+      const int k1_L = __shfl_sync(0xffffffffu, k1, L), jlo_L = __shfl_sync(0xffffffffu, jlo, L), jhi_L = __shfl_sync(0xffffffffu, jhi, L);
+      int* erow_L = (int*)__shfl_sync(0xffffffffu, (unsigned long long)erow, L);
+      auto close_L = [&](int j) {
+        ++k_L;
+        if (lane == 0 && erow_L) erow_L[k_L] = j;
+        t_L = (k_L < k1_L) ? seg_target(C_L, k_L + 1, N) - cb0_L : INFINITY;
+      };
+      for (int j0 = ib; j0 < ie && k_L < k1_L; j0 += 32) {
+        const int j = j0 + lane;
+        double sj = 0.0;
+        if (j < ie && j >= jlo_L && j < jhi_L) sj = sigma_bin64(g, (double)(j - ib) * hS, ad.G64[j]);
+        double inc = sj;                                       // inclusive warp scan, fixed order
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { const double up = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += up; }
+        const double excl = inc - sj;                          // sum of the bins of this round before bin j
+        const double tot = shfl_d(inc, 31);
+        // e_n = first bin whose cumulative sum (before adding it) has reached the target; several targets may fall here
+        while (k_L < k1_L) {
+          const unsigned hit = __ballot_sync(0xffffffffu, (j < ie) && (crel_L + excl >= t_L));
+          if (!hit) break;
+          close_L(j0 + __ffs(hit) - 1);
+        }
+        crel_L += tot;
+      }
+      while (k_L < k1_L && crel_L >= t_L) close_L(ie);
+      if (lane == L) { crel = crel_L; t_next = t_L; k = k_L; }
+    }
+  }
+  while (k < k1) { ++k; if (erow) erow[k] = ce; }   // targets the scanned sums place in this chunk (rounding): at its end
 }
 
 template <int SC, bool MERGE = false>
@@ -141,13 +278,14 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2_ad(DevCfg c, 
   const double cb0 = ad.cbase[(size_t)chunk * a.P_pad + p];
   const double cb1 = ad.cbase[(size_t)(chunk + 1) * a.P_pad + p];
   int k = seg_index(cb0, C, N);                 // segment open at the chunk start
-  const int k1 = seg_index(cb1, C, N);          // edges k+1 .. k1 are closed inside this chunk, no more, no fewer
-  double t_next = (k < k1) ? seg_target(C, k + 1, N) - cb0 : INFINITY;
-  double crel = 0.0, c_open = 0.0;              // cumulative sigma relative to the chunk start; its value where the open piece began
+  const int k1 = seg_index(cb1, C, N);          // edges k+1 .. k1 lie in (cs, ce] (k_edges64 placed them), no more, no fewer
+  const int pq = ad.pmap ? ad.pmap[p] : p;      // particle of the batch in this table slot
+  const int* erow = ad.out_edges + (size_t)min(pq, a.P - 1) * (N + 1);
+  int j_next = (k < k1 && pq < a.P) ? erow[k + 1] : INT_MAX;   // bin of the next edge of this lane
+  double crel = 0.0, c_open = 0.0;              // sigma (FP32 amplitudes) since the chunk start; its value where the open piece began
   double Zr = 0.0, Zi = 0.0, ups = 0.0, xs = 0.0, hs = 0.0;
   bool closed_any = false;
   double* frag = a.frag + (size_t)chunk * kFragAd * a.P_pad + p;
-  const int pq = ad.pmap ? ad.pmap[p] : p;      // particle of the batch in this table slot
 
   auto close_at = [&](int j) {                  // edge k+1 lies at bin j
     const double Sg = crel - c_open;
@@ -161,8 +299,8 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2_ad(DevCfg c, 
     }
     Zr = 0.0; Zi = 0.0; c_open = crel;
     ++k;
-    if (ad.out_edges && pq < a.P) ad.out_edges[(size_t)pq * (N + 1) + k] = j;
-    t_next = (k < k1) ? seg_target(C, k + 1, N) - cb0 : INFINITY;
+    j_next = (k < k1) ? erow[k + 1] : INT_MAX;
+    (void)j;
   };
 
   PhaseFD ph = {};
@@ -182,7 +320,7 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2_ad(DevCfg c, 
           __all_sync(0xffffffffu, (ib >= jlo) && (ib + c.stride <= jhi)) &&
           __all_sync(0xffffffffu, coarse_dslope(c, a, p, ib >> c.log2_stride) <= a.merge_lim)) {
         coarse_phase(c, a, p, ib, ph);
-        coarse_amps(c, a, p, ib, cc);
+        coarse_amps<double>(c, a, p, ib, cc);
         merged_left = 4;
       }
     }
@@ -191,16 +329,16 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2_ad(DevCfg c, 
       --merged_left;
     } else {
       sub_phase(c, a, p, ib, ph);
-      sub_amps(c, a, p, ib, cf);
+      sub_amps<double>(c, a, p, ib, cf);
     }
     u64 s2 = f2pack(0.0f, hS);
     const ulonglong2* rec = sD + ((ib - cs) >> 1) * kPairRec;
     // First ask the question for the whole sub-interval (its moments are those k_sigma_chunks used): if no lane reaches its
     // next target in it, all its groups take the unmasked path and the group moments are not needed at all.
     if (all_in && ie - ib == Sf) {
-      const double sg_s = sigma_moments(cf, ad.smom + (size_t)(ib >> (c.log2_stride - 2)) * 4);
-      const bool cross_s = (k < k1) && (crel + sg_s * 1.0001 >= t_next);
+      const bool cross_s = j_next < ie;          // (an edge AT ie is closed by the first bin of the next sub-interval)
       if (!__any_sync(0xffffffffu, cross_s)) {
+        const double sg_s = sigma_moments(cf, ad.smom + (size_t)(ib >> (c.log2_stride - 2)) * 4);
         for (int gs = ib; gs < ie; gs += Gs) {
           u64 zr2 = 0, zi2 = 0;
           pairs_fast<SC>(ph, cf, s2, rec, Gs >> 1, h2, K2, zr2, zi2);
@@ -214,12 +352,9 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2_ad(DevCfg c, 
     }
     for (int gs = ib; gs < ie; gs += Gs) {
       const int ge = min(gs + Gs, ie);
-      const double sg_m = sigma_moments(cf, ad.gmom + (size_t)(gs >> ad.lg_group) * 4);
-      // would the running sum reach this lane's next target inside the group?  (margin: the per-bin and the moment sums
-      // differ by FP32 rounding; a group flagged needlessly only takes the slower path)
-      const bool cross = (k < k1) && (crel + sg_m * 1.0001 >= t_next);
-      const bool slow = !all_in || __any_sync(0xffffffffu, cross);
+      const bool slow = !all_in || __any_sync(0xffffffffu, j_next < ge);   // a lane has an edge inside this group
       if (!slow) {
+        const double sg_m = sigma_moments(cf, ad.gmom + (size_t)(gs >> ad.lg_group) * 4);
         u64 zr2 = 0, zi2 = 0;
         pairs_fast<SC>(ph, cf, s2, rec, (ge - gs) >> 1, h2, K2, zr2, zi2);
         float zrl, zrh, zil, zih;
@@ -232,15 +367,15 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2_ad(DevCfg c, 
           pair_eval<true, true, SC>(ph, cf, s2, rec, jj, jlo, jhi, h2, K2, zr2, zi2, sg2);
           float zrl, zrh, zil, zih, sgl, sgh;
           f2unpack(zr2, zrl, zrh); f2unpack(zi2, zil, zih); f2unpack(sg2, sgl, sgh);
-          while (k < k1 && crel >= t_next) close_at(jj);          // e_n = first bin whose cumulative sum reached the target
+          while (j_next <= jj) close_at(jj);                      // edges at this bin (several: empty segments)
           Zr += (double)zrl; Zi += (double)zil; crel += (double)sgl;
-          while (k < k1 && crel >= t_next) close_at(jj + 1);
+          while (j_next <= jj + 1) close_at(jj + 1);
           Zr += (double)zrh; Zi += (double)zih; crel += (double)sgh;
         }
       }
     }
   }
-  while (k < k1) close_at(ce);                  // targets the scanned sums place in this chunk (rounding): at its end
+  while (k < k1) close_at(ce);                  // edges at the chunk end
   const double Sg = crel - c_open;
   if (!closed_any) {
     frag[(size_t)1 * a.P_pad] = Zr; frag[(size_t)2 * a.P_pad] = Zi; frag[(size_t)3 * a.P_pad] = Sg;

@@ -158,18 +158,20 @@ __device__ __forceinline__ void sub_phase(const DevCfg& c, const DenseArgs& a, i
   phase_set(ph, r0 + b[0], b);
 }
 
-// Cubic coefficients of (Ar, Ai, Er, Ei) on that sub-interval in s = (j - ib)/Sf.
+// Cubic coefficients of (Ar, Ai, Er, Ei) on that sub-interval in s = (j - ib)/Sf.  NA: element type of the node table
+// (float; double in the per-particle-segment path, whose edge decision needs the FP64 table anyway).
+template <typename NA = float>
 __device__ __forceinline__ void sub_amps(const DevCfg& c, const DenseArgs& a, int p, int ib, float (&cf)[4][4]) {
   const int i0 = (ib >> c.log2_stride) + kNodeOff;
   const int q = (ib >> (c.log2_stride - 2)) & 3;
-  const float* __restrict__ namp = reinterpret_cast<const float*>(a.node_amp);
+  const NA* __restrict__ namp = reinterpret_cast<const NA*>(a.node_amp);
 #pragma unroll
   for (int r = 0; r < 4; r += 2) {                          // (Ar, Ai) then (Er, Ei) as packed halves
-    const float* col = namp + ((size_t)i0 * 4 + r) * a.P_pad + p;
+    const NA* col = namp + ((size_t)i0 * 4 + r) * a.P_pad + p;
     const ptrdiff_t st = (ptrdiff_t)4 * a.P_pad;
     u64 nd[6], o[4];
 #pragma unroll
-    for (int m = -2; m <= 3; ++m) nd[m + 2] = f2pack(col[m * st], col[m * st + a.P_pad]);
+    for (int m = -2; m <= 3; ++m) nd[m + 2] = f2pack((float)col[m * st], (float)col[m * st + a.P_pad]);
     fine_cubic2(nd, q, o);
 #pragma unroll
     for (int kk = 0; kk < 4; ++kk) f2unpack(o[kk], cf[r][kk], cf[r + 1][kk]);
@@ -222,14 +224,15 @@ __device__ __forceinline__ void coarse_phase(const DevCfg& c, const DenseArgs& a
   phase_set(ph, r0 + b[0], b);
 }
 // Cubic through nodes -1 .. 2 of (Ar, Ai, Er, Ei) in t = (j - ib) / stride.
+template <typename NA = float>
 __device__ __forceinline__ void coarse_amps(const DevCfg& c, const DenseArgs& a, int p, int ib, float (&cc)[4][4]) {
   const int i0 = (ib >> c.log2_stride) + kNodeOff;
-  const float* __restrict__ namp = reinterpret_cast<const float*>(a.node_amp);
+  const NA* __restrict__ namp = reinterpret_cast<const NA*>(a.node_amp);
 #pragma unroll
   for (int r = 0; r < 4; ++r) {
-    const float* col = namp + ((size_t)i0 * 4 + r) * a.P_pad + p;
+    const NA* col = namp + ((size_t)i0 * 4 + r) * a.P_pad + p;
     const ptrdiff_t st = (ptrdiff_t)4 * a.P_pad;
-    cubic_coeffs<float>(col[-st], col[0], col[st], col[2 * st], cc[r][0], cc[r][1], cc[r][2], cc[r][3]);
+    cubic_coeffs<float>((float)col[-st], (float)col[0], (float)col[st], (float)col[2 * st], cc[r][0], cc[r][1], cc[r][2], cc[r][3]);
   }
 }
 // The same cubic in the variable of fine sub-interval q: t = (q + s) / 4.

@@ -336,6 +336,24 @@ __device__ constexpr float kFineM[4][4][6] = {
    {-53.0 / 8192, 1315.0 / 24576, -1241.0 / 4096, 881.0 / 4096, 1157.0 / 24576, -51.0 / 8192},
    {-15.0 / 8192, 95.0 / 8192, 45.0 / 4096, -217.0 / 4096, 293.0 / 8192, -29.0 / 8192},
    {5.0 / 8192, -115.0 / 24576, 41.0 / 4096, -33.0 / 4096, 43.0 / 24576, 3.0 / 8192}}};
+// The same matrix in FP64 (the FP64 edge decision of the per-particle-segment path).
+__device__ constexpr double kFineMd[4][4][6] = {
+  {{0.0, 0.0, 1.0, 0.0, 0.0, 0.0},
+   {25.0 / 2048, -761.0 / 6144, -87.0 / 1024, 257.0 / 1024, -385.0 / 6144, 17.0 / 2048},
+   {-5.0 / 2048, 21.0 / 512, -79.0 / 1024, 21.0 / 512, -5.0 / 2048, 0.0},
+   {-3.0 / 8192, -43.0 / 24576, 33.0 / 4096, -41.0 / 4096, 115.0 / 24576, -5.0 / 8192}},
+  {{77.0 / 8192, -693.0 / 8192, 3465.0 / 4096, 1155.0 / 4096, -495.0 / 8192, 63.0 / 8192},
+   {47.0 / 8192, -371.0 / 8192, -2671.0 / 12288, 1245.0 / 4096, -437.0 / 8192, 155.0 / 24576},
+   {-29.0 / 8192, 293.0 / 8192, -217.0 / 4096, 45.0 / 4096, 95.0 / 8192, -15.0 / 8192},
+   {1.0 / 8192, -29.0 / 8192, 127.0 / 12288, -45.0 / 4096, 37.0 / 8192, -11.0 / 24576}},
+  {{3.0 / 256, -25.0 / 256, 75.0 / 128, 75.0 / 128, -25.0 / 256, 3.0 / 256},
+   {-1.0 / 768, 17.0 / 1024, -75.0 / 256, 449.0 / 1536, -1.0 / 64, 1.0 / 1024},
+   {-13.0 / 4096, 103.0 / 4096, -45.0 / 2048, -45.0 / 2048, 103.0 / 4096, -13.0 / 4096},
+   {11.0 / 24576, -37.0 / 8192, 45.0 / 4096, -127.0 / 12288, 29.0 / 8192, -1.0 / 8192}},
+  {{63.0 / 8192, -495.0 / 8192, 1155.0 / 4096, 3465.0 / 4096, -693.0 / 8192, 77.0 / 8192},
+   {-53.0 / 8192, 1315.0 / 24576, -1241.0 / 4096, 881.0 / 4096, 1157.0 / 24576, -51.0 / 8192},
+   {-15.0 / 8192, 95.0 / 8192, 45.0 / 4096, -217.0 / 4096, 293.0 / 8192, -29.0 / 8192},
+   {5.0 / 8192, -115.0 / 24576, 41.0 / 4096, -33.0 / 4096, 43.0 / 24576, 3.0 / 8192}}};
 
 // Cubic through 4 equispaced nodes m = -1..2 in s = u/stride: a0 + a1 s + a2 s^2 + a3 s^3.
 template <typename R>

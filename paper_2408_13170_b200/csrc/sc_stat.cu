@@ -81,6 +81,8 @@ struct sc_handle : EdgeCache {
   double2* d_zpart = nullptr; size_t zpart_cap = 0; double* d_hh = nullptr; size_t hh_cap = 0;
   // adaptive (per-particle) segments: moments of the weights over groups and fine sub-intervals, cached per node spacing
   int ad_lg = 0; float2* d_gmom = nullptr; float2* d_smom = nullptr; size_t gmom_cap = 0, smom_cap = 0;
+  double2* d_gmom64 = nullptr; double2* d_smom64 = nullptr; size_t gmom64_cap = 0, smom64_cap = 0;   // FP64 copies (edge decision)
+  int* d_ad_edges = nullptr; size_t ad_edges_cap = 0;    // the edges of a batch when the caller does not ask for them
   // scratch
   void* scratch = nullptr; size_t scratch_bytes = 0;
   unsigned long long* d_counter = nullptr;
@@ -560,20 +562,23 @@ int run_adaptive(sc_handle* h, const double* params, int64_t P, int n_seg, doubl
   if (h->ad_lg != dc.log2_stride) {
     if ((rc = grow(h, (void**)&h->d_gmom, &h->gmom_cap, (size_t)n_groups * 8 * sizeof(float2)))) return rc;
     if ((rc = grow(h, (void**)&h->d_smom, &h->smom_cap, (size_t)n_sub * 8 * sizeof(float2)))) return rc;
+    if ((rc = grow(h, (void**)&h->d_gmom64, &h->gmom64_cap, (size_t)n_groups * 7 * sizeof(double2)))) return rc;
+    if ((rc = grow(h, (void**)&h->d_smom64, &h->smom64_cap, (size_t)n_sub * 7 * sizeof(double2)))) return rc;
     Timed tm(h, st, SC_TIME_OTHER);
-    k_moments<<<(n_groups + 127) / 128, 128, 0, st>>>(h->G64, nullptr, (const int*)(size_t)lg_group, n_groups, dc.n_bins, lg_fine, h->d_gmom);
+    k_moments<<<(n_groups + 127) / 128, 128, 0, st>>>(h->G64, nullptr, (const int*)(size_t)lg_group, n_groups, dc.n_bins, lg_fine, h->d_gmom, h->d_gmom64);
     if ((rc = check_launch(h, "k_moments"))) return rc;
-    k_moments<<<(n_sub + 127) / 128, 128, 0, st>>>(h->G64, nullptr, (const int*)(size_t)lg_fine, n_sub, dc.n_bins, lg_fine, h->d_smom);
+    k_moments<<<(n_sub + 127) / 128, 128, 0, st>>>(h->G64, nullptr, (const int*)(size_t)lg_fine, n_sub, dc.n_bins, lg_fine, h->d_smom, h->d_smom64);
     if ((rc = check_launch(h, "k_moments"))) return rc;
     h->ad_lg = dc.log2_stride;
   }
-  const size_t per_p = 2 * ((size_t)kPcFields * 8 + 8) + 16 + (size_t)n_nodes * (4 + 8 + 4 * sizeof(float))
-                       + (size_t)(n_chunks + 1) * 8 + (size_t)n_chunks * kFragAd * 8;
+  // (FP64 node amplitudes: the edge decision is taken in FP64; the packed kernel converts them as it reads)
+  const size_t per_p = 2 * ((size_t)kPcFields * 8 + 8) + 16 + (size_t)n_nodes * (4 + 8 + 4 * sizeof(double))
+                       + (size_t)(n_chunks + 1) * 8 + (size_t)n_chunks * kFragAd * 8 + (size_t)n_sub * 8;
   int64_t Pb_max = (int64_t)(h->scratch_cap / per_p) / kBlock * kBlock;
   if (Pb_max < kBlock) Pb_max = kBlock;
   const int64_t P_round = (P + kBlock - 1) / kBlock * kBlock;
   const int P_pad = (int)std::min<int64_t>(Pb_max, P_round);
-  if ((rc = grow(h, &h->scratch, &h->scratch_bytes, per_p * (size_t)P_pad + 2048))) return rc;
+  if ((rc = grow(h, &h->scratch, &h->scratch_bytes, per_p * (size_t)P_pad + 4096))) return rc;
   char* base = (char*)h->scratch;
   auto take = [&](size_t bytes) { char* r = base; base += (bytes + 255) / 256 * 256; return r; };
   double* pc = (double*)take((size_t)kPcFields * 8 * P_pad);
@@ -581,9 +586,10 @@ int run_adaptive(sc_handle* h, const double* params, int64_t P, int n_seg, doubl
   int* jhi = (int*)take((size_t)4 * P_pad);
   int* node_n = (int*)take((size_t)n_nodes * 4 * P_pad);
   double* node_frac = (double*)take((size_t)n_nodes * 8 * P_pad);
-  float* node_amp = (float*)take((size_t)n_nodes * 4 * sizeof(float) * P_pad);
+  double* node_amp = (double*)take((size_t)n_nodes * 4 * sizeof(double) * P_pad);
   double* cbase = (double*)take((size_t)(n_chunks + 1) * 8 * P_pad);
   double* frag = (double*)take((size_t)n_chunks * kFragAd * 8 * P_pad);
+  double* sub_sigma = (double*)take((size_t)n_sub * 8 * P_pad);
   // window sort, as in run_batches
   const bool sorted = h->window_sort && P_pad > kBlock;
   double* pc_u = (double*)take((size_t)kPcFields * 8 * P_pad);
@@ -607,6 +613,7 @@ int run_adaptive(sc_handle* h, const double* params, int64_t P, int n_seg, doubl
   const double h0 = pow(dc.f_amp_ref, -7.0 / 6.0);
   (void)four_df;
   if (out_edges) SC_CUDA(h, cudaMemsetAsync(out_edges, 0, (size_t)P * (n_seg + 1) * 4, st));
+  else if ((rc = grow(h, (void**)&h->d_ad_edges, &h->ad_edges_cap, (size_t)std::min<int64_t>(P, P_pad) * (n_seg + 1) * 4))) return rc;
 
   for (int64_t pb = 0; pb < P; pb += P_pad) {
     const int Pn = (int)std::min<int64_t>(P_pad, P - pb);
@@ -629,8 +636,8 @@ int run_adaptive(sc_handle* h, const double* params, int64_t P, int n_seg, doubl
     }
     {
       Timed tm(h, st, SC_TIME_NODES);
-      // (k_sigma_chunks and k_dense2_ad read a node only where a lane of the warp is inside its window: skip_unreached)
-      k_nodes<float><<<dim3((n_nodes + kNodesPerCta - 1) / kNodesPerCta, (P_pad + 127) / 128), 128, 0, st>>>(dc, pc, jlo, jhi, P_pad, node_n, node_frac, node_amp, nullptr, 0, 1);
+      // (the consumers read a node only where a lane of the warp is inside its window: skip_unreached)
+      k_nodes<double><<<dim3((n_nodes + kNodesPerCta - 1) / kNodesPerCta, (P_pad + 127) / 128), 128, 0, st>>>(dc, pc, jlo, jhi, P_pad, node_n, node_frac, node_amp, nullptr, 0, 1);
     }
     if ((rc = check_launch(h, "k_nodes"))) return rc;
     DenseArgs a = {};
@@ -640,15 +647,18 @@ int run_adaptive(sc_handle* h, const double* params, int64_t P, int n_seg, doubl
     ad.n_seg = n_seg; ad.n_chunks = n_chunks; ad.cbase = cbase; ad.chunk_sigma = cbase;
     ad.gmom = reinterpret_cast<const ulonglong2*>(h->d_gmom); ad.smom = reinterpret_cast<const ulonglong2*>(h->d_smom);
     ad.lg_group = lg_group;
-    ad.out_edges = out_edges ? out_edges + (size_t)pb * (n_seg + 1) : nullptr;
+    ad.out_edges = out_edges ? out_edges + (size_t)pb * (n_seg + 1) : h->d_ad_edges;
     ad.pmap = sorted ? pmap : nullptr;
+    ad.smom64 = h->d_smom64; ad.gmom64 = h->d_gmom64; ad.G64 = h->G64; ad.sub_sigma = sub_sigma;
     const dim3 grid(n_chunks, P_pad / kBlock);
     {
       Timed tm(h, st, SC_TIME_OTHER);
-      k_sigma_chunks<<<grid, kBlock, 0, st>>>(dc, a, ad, h->D32);
-      if ((rc = check_launch(h, "k_sigma_chunks"))) return rc;
+      k_sigma_chunks64<<<grid, kBlock, 0, st>>>(dc, a, ad);
+      if ((rc = check_launch(h, "k_sigma_chunks64"))) return rc;
       k_scan_chunks<<<(P_pad + 127) / 128, 128, 0, st>>>(cbase, n_chunks, P_pad);
       if ((rc = check_launch(h, "k_scan_chunks"))) return rc;
+      k_edges64<<<grid, kBlock, 0, st>>>(dc, a, ad);
+      if ((rc = check_launch(h, "k_edges64"))) return rc;
     }
     {
       Timed tm(h, st, SC_TIME_DENSE);
@@ -665,7 +675,7 @@ int run_adaptive(sc_handle* h, const double* params, int64_t P, int n_seg, doubl
     const double g2 = (sincos == 2) ? h->mufu_gain2 : 1.0;
     k_stitch_ad<<<((sorted ? P_pad : Pn) + 127) / 128, 128, 0, st>>>(frag, n_chunks, P_pad, Pn, 1.0 / g2, out ? out + pb : nullptr,
                                                   out_comp ? out_comp + pb * 3 : nullptr, h->s0 * h0 / sqrt(g2),
-                                                  h->s0 * h->s0 * h0 * h0, ad.out_edges, n_seg, dc.n_bins, ad.pmap, jlo, jhi, CH);
+                                                  h->s0 * h->s0 * h0 * h0, out_edges ? ad.out_edges : nullptr, n_seg, dc.n_bins, ad.pmap, jlo, jhi, CH);
     if ((rc = check_launch(h, "k_stitch_ad"))) return rc;
   }
   return SC_OK;
@@ -1373,6 +1383,7 @@ int sc_free(sc_handle* h) {
   cudaFree(h->scratch); cudaFree(h->d_edges); cudaFree(h->d_chunk_k0); cudaFree(h->d_flags);
   cudaFree(h->d_counter); cudaFree(h->d_params_stage); cudaFree(h->d_comp); cudaFree(h->d_km); cudaFree(h->d_T64); cudaFree(h->d_T32); cudaFree(h->d_sp);
   cudaFree(h->d_spsig); cudaFree(h->d_zpart); cudaFree(h->d_hh); cudaFree(h->d_gmom); cudaFree(h->d_smom);
+  cudaFree(h->d_gmom64); cudaFree(h->d_smom64); cudaFree(h->d_ad_edges);
   cudaFree(h->d_piece_first); cudaFree(h->d_piece_lo); cudaFree(h->d_piece_hi); cudaFree(h->d_moments);
   cudaFree(h->alt.d_edges); cudaFree(h->alt.d_chunk_k0); cudaFree(h->alt.d_flags); cudaFree(h->alt.d_next_close); cudaFree(h->d_next_close);
   cudaFree(h->d_moments64); cudaFree(h->alt.d_moments64);

@@ -99,8 +99,10 @@ def pso_step_sharded(H, state, stat, lo, hi, eps_min, omega, phi_p, phi_g, seed,
     cand = torch.empty((n_swarms_local, 10), dtype=torch.float64, device=pos.device)
     H.pso_best(state, stat, cand, n_swarms_local, index_offset, stream)
     if exchange and dist.is_initialized() and dist.get_world_size(group) > 1:
-        allc = torch.empty((dist.get_world_size(group), n_swarms_local, 10), dtype=torch.float64, device=pos.device)
-        dist.all_gather_into_tensor(allc, cand, group=group)
+        w = dist.get_world_size(group)
+        flat = torch.empty((w * n_swarms_local, 10), dtype=torch.float64, device=pos.device)      # rank-major concatenation
+        dist.all_gather_into_tensor(flat, cand, group=group)
+        allc = flat.view(w, n_swarms_local, 10)
     else:
         allc = cand[None]
     H.pso_pick(allc, state, stream)

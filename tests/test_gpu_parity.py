@@ -483,6 +483,58 @@ def test_pso_step_parity(c1, oracle, torch_cuda, P, S):
         assert (np.abs(st["vel"].cpu().numpy() - o["vel"]) / span).max() <= 1e-13
 
 
+@pytest.mark.parametrize("P,S,shards", [(10000, 1, 2), (40000, 4, 2), (4096, 1, 8), (600, 2, 3)])
+def test_pso_step_sharded_is_bit_identical(c1, torch_cuda, P, S, shards):
+    """every swarm cut into `shards` contiguous pieces (one per rank), evaluated piece by piece with
+    sc_pso_best -> (all-gather, here a concatenation on one GPU) -> sc_pso_pick -> sc_pso_move: personal bests, swarm
+    bests, positions and velocities are BIT-identical to one sc_pso_step on the whole population (global indices break
+    ties and are the Philox counters).  Three iterations with many exact ties in the statistic."""
+    from paper_2408_13170_b200 import dist as scd
+    H = c1["H"]
+    rng = np.random.default_rng(100 + P)
+    lo, hi = c1["inp"]["lo"], c1["inp"]["hi"].copy()
+    hi[7] = 0.1
+    pos = lo + (hi - lo) * rng.random((P, 8))
+    vel = (hi - lo) * rng.uniform(-0.4, 0.4, (P, 8))
+    eps = np.array([0.1, 0.05, 0.0, 0.1, 0.1, 0.2, 0.1, 0.1]) * 0.1
+    d = lambda a: _dev(torch_cuda, a)
+    whole = _pso_state(torch_cuda, pos, vel, S)
+    per, piece = P // S, P // S // shards
+    # "rank" r = (swarm s, piece k) owns particles [s per + k piece, s per + (k+1) piece)
+    ranks = []
+    for s_ in range(S):
+        for k in range(shards):
+            a = s_ * per + k * piece
+            ranks.append(dict(a=a, swarm=s_, st=_pso_state(torch_cuda, pos[a:a + piece], vel[a:a + piece], 1)))
+    args = (d(lo), d(hi), d(eps), 0.5, 0.2, 0.3, 12345678901234567)
+    for it in range(3):
+        stat = np.round(rng.normal(100, 3, P), 0)                 # rounded: many exact ties, also across shards
+        H.pso_step(whole, d(stat), *args, it, S)
+        cands = []
+        for r in ranks:
+            c = torch_cuda.empty((1, 10), dtype=torch_cuda.float64, device="cuda:0")
+            H.pso_best(r["st"], d(stat[r["a"]:r["a"] + piece]), c, 1, r["a"])
+            cands.append(c)
+        for r in ranks:
+            allc = torch_cuda.stack([c for c, q in zip(cands, ranks) if q["swarm"] == r["swarm"]])     # the all-gather
+            H.pso_pick(allc, r["st"])
+            H.pso_move(r["st"], *args, it, 1, r["a"])
+        for key in ("pos", "vel", "pbest_pos", "pbest_val"):
+            got = torch_cuda.cat([r["st"][key] for r in ranks]).cpu().numpy()
+            assert np.array_equal(got, whole[key].cpu().numpy()), (key, it)
+        for r in ranks:
+            assert np.array_equal(r["st"]["gbest_val"].cpu().numpy(), whole["gbest_val"][r["swarm"]:r["swarm"] + 1].cpu().numpy())
+            assert np.array_equal(r["st"]["gbest_pos"].cpu().numpy(), whole["gbest_pos"][r["swarm"]:r["swarm"] + 1].cpu().numpy())
+    # the same through dist.pso_step_sharded without a process group (one shard = the whole population)
+    one = _pso_state(torch_cuda, pos, vel, S)
+    ref = _pso_state(torch_cuda, pos, vel, S)
+    stat = d(np.round(rng.normal(100, 3, P), 0))
+    scd.pso_step_sharded(H, one, stat, *args, 9, S, 0)
+    H.pso_step(ref, stat, *args, 9, S)
+    for key in ("pos", "vel", "pbest_pos", "pbest_val", "gbest_pos", "gbest_val"):
+        assert np.array_equal(one[key].cpu().numpy(), ref[key].cpu().numpy()), key
+
+
 def test_pso_uniforms_bit_equal(c1, oracle, torch_cuda):
     """omega = phi_p = 0, phi_g = 1, pos = 0, gbest = 1 in every dimension: the new position IS r_G (Q10)."""
     H = c1["H"]
@@ -519,16 +571,20 @@ def test_device_resident_search_improves_best(c1, torch_cuda, sc):
 
 
 # ---------------------------------------------------------------------------------------------- per-particle segments
-def _check_adaptive(oracle, cfg, dA, dE, inp, parts, N, got, ged, comp=None):
-    """PAPER.md:120 segments.  Floating point decides the integer edges, so (i) the edges are checked for validity
-    against the oracle's own choice (|difference| <= 1 bin, almost all equal) and (ii) the statistic is compared with
-    the oracle evaluated ON THE DEVICE'S EDGES (sco_eval_stat_adaptive in_edges): the decision is taken once."""
+def _check_adaptive(oracle, cfg, dA, dE, inp, parts, N, got, ged, comp=None, exact=True):
+    """PAPER.md:120 segments.  Floating point decides the integer edges, and both sides take the decision in FP64: the
+    device's edges must EQUAL the oracle's (sco_equal_snr_edges) -- everywhere when `exact`, else in >= 99.9 % of the edges
+    and never more than one bin away (a cumulative sum within the interpolation error, ~1e-12 relative, of its target may
+    fall on the other side: probability ~1e-12 x n_bins per edge).  The statistic is then compared with the oracle evaluated
+    on the device's edges (sco_eval_stat_adaptive in_edges), which are the oracle's own wherever they agree."""
     nb = inp["cfg"]["n_bins"]
     ref_own, oed = oracle.eval_stat_adaptive(cfg, dA, dE, inp["S_A"], inp["S_E"], parts, N, want_edges=True)
     assert np.all(ged[:, 0] == 0) and np.all(ged[:, -1] == nb) and np.all(np.diff(ged, axis=1) >= 0)
     d = np.abs(ged.astype(np.int64) - oed)
-    assert d.max() <= 1, d.max()
-    assert (d == 0).mean() >= 0.85
+    if exact:
+        assert np.array_equal(ged.astype(np.int64), oed), (int(d.max()), float((d != 0).mean()))
+    else:
+        assert d.max() <= 1 and (d == 0).mean() >= 0.999, (int(d.max()), float((d != 0).mean()))
     ref, rc = oracle.eval_stat_adaptive(cfg, dA, dE, inp["S_A"], inp["S_E"], parts, N, in_edges=ged, want_comp=True)
     assert rel_err(got, ref).max() <= TOL, (N, rel_err(got, ref).max())
     # moving an edge by one bin changes Upsilon by O(1/bins-per-segment): the two choices give nearby statistics
@@ -595,11 +651,11 @@ def test_c3_adaptive_bench_configuration(oracle, torch_cuda, sc):
     H = gpu_handle(inp, dA, dE)
     H.set_option(sc.SC_OPT_TC_MAX_S, int(np.ceil(inp["hi"][2])))
     P = inp["particles"].shape[0]
-    idx = _sample_idx(P, 12, 33)
+    idx = _sample_idx(P, 32, 33)
     N = 100
     got, ged = H.eval_stat_adaptive(_dev(torch_cuda, inp["particles"]), N, want_edges=True)
     got, ged = got.cpu().numpy(), ged.cpu().numpy()
-    _check_adaptive(oracle, cfg, dA, dE, inp, inp["particles"][idx], N, got[idx], ged[idx])
+    _check_adaptive(oracle, cfg, dA, dE, inp, inp["particles"][idx], N, got[idx], ged[idx], exact=False)
     assert np.all(np.isfinite(got)) and np.all(got >= 0)
     assert np.all(np.diff(ged, axis=1) >= 0) and np.all(ged[:, -1] == inp["cfg"]["n_bins"])
     H.close()
@@ -607,15 +663,14 @@ def test_c3_adaptive_bench_configuration(oracle, torch_cuda, sc):
 
 def test_c5_adaptive_short_windows(oracle, torch_cuda, sc):
     """Per-particle segments on c5's short, scattered time windows: the window sort, the empty-CTA exits, the skipped node
-    blocks and the windowed stitch of the adaptive path.  A sample against the oracle (edges within one bin, statistic on
-    the device's edges to 1e-6); sort on / off over the whole population: same edges up to one bin, and where every edge
-    agrees the same statistic to FP32 rounding."""
+    blocks and the windowed stitch of the adaptive path.  A sample against the oracle (edges equal, statistic to 1e-6);
+    sort on / off over the whole population: same edges, and where every edge agrees the same statistic to FP32 rounding."""
     inp = sy.config_inputs(5, P=1280)
     cfg, dA, dE = make_data(oracle, inp)
     H = gpu_handle(inp, dA, dE)
     H.set_option(sc.SC_OPT_TC_MAX_S, int(np.ceil(inp["hi"][2])))
     par = _dev(torch_cuda, inp["particles"])
-    idx = _sample_idx(1280, 6, 77)
+    idx = _sample_idx(1280, 24, 77)
     N = 50
     res = {}
     for srt in (1, 0):
@@ -624,9 +679,9 @@ def test_c5_adaptive_short_windows(oracle, torch_cuda, sc):
         res[srt] = (g.cpu().numpy(), e.cpu().numpy())
     H.close()
     (a, ea), (b, eb) = res[1], res[0]
-    _check_adaptive(oracle, cfg, dA, dE, inp, inp["particles"][idx], N, a[idx], ea[idx])
-    assert np.abs(ea - eb).max() <= 1
+    _check_adaptive(oracle, cfg, dA, dE, inp, inp["particles"][idx], N, a[idx], ea[idx], exact=False)
+    assert np.abs(ea - eb).max() <= 1 and (ea == eb).mean() >= 0.9999          # the FP64 decision does not depend on the order
     same = np.all(ea == eb, axis=1) & (b > 0)
-    assert same.sum() > 900
+    assert same.sum() > 1200
     assert rel_err(a[same], b[same]).max() <= 2e-7
     assert np.all(np.diff(ea, axis=1) >= 0) and np.all(ea[:, -1] == inp["cfg"]["n_bins"]) and np.all(ea[:, 0] == 0)
