@@ -32,6 +32,7 @@ using namespace sc;
 #include "sc_kernels_prep.cuh"
 #include "sc_kernels_dense64.cuh"
 #include "sc_kernels_dense32.cuh"
+#include "sc_kernels_dense32tc.cuh"
 #include "sc_kernels_adaptive.cuh"
 #include "sc_kernels_stitch.cuh"
 #include "sc_kernels_search.cuh"
@@ -94,6 +95,8 @@ struct sc_handle : EdgeCache {
   int escalate = 1; double esc_tau_poly = 6.0, esc_tau_mufu = 16.0;
   int* d_esc_idx = nullptr; int* d_esc_count = nullptr; double* d_esc_params = nullptr; double* d_esc_out = nullptr;
   size_t esc_idx_cap = 0, esc_cnt_cap = 0, esc_par_cap = 0, esc_out_cap = 0; int* h_esc_hint = nullptr;
+  // tensor-core path of the FP32-amplitude kernel (k_dense2_tc): per-tile operand image, built for one node spacing
+  int use_tc = 1; uint4* d_tc_img = nullptr; size_t tc_img_cap = 0; int tc_img_lg = 0;
   int window_sort = 1; void* d_sort_tmp = nullptr; size_t sort_cap = 0;   // cub radix-sort workspace of the window sort
   // three-channel handles (A, E, T): the T channel lives in a second handle whose first slot carries T (chan_set = 1)
   // and whose second slot is empty; the per-segment sums of both are added before |z|^2/sigma is formed
@@ -281,6 +284,16 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
 
   // particle blocks launched per kernel: all of them, or (escalation pass) the caller's estimate -- the kernels stride
   const int pblocks = esc_count ? std::max(1, std::min(esc_blocks, P_pad / kBlock)) : P_pad / kBlock;
+  // tensor-core flavour of the FP32-amplitude kernel: fine sub-intervals of at least one 32-bin tile
+  const bool use_tc = sizeof(R) == 4 && h->use_tc && dc.log2_stride >= 7 && n_chunks > 0;
+  if (use_tc && h->tc_img_lg != dc.log2_stride) {
+    const long long n_tiles = (long long)((dc.n_bins + kChunkF32 - 1) / kChunkF32) * (kChunkF32 / tc::kTileBins);
+    if ((rc = grow(h, (void**)&h->d_tc_img, &h->tc_img_cap, (size_t)n_tiles * tc::kTileBytes))) return rc;
+    Timed tm(h, st, SC_TIME_OTHER);
+    k_tc_image<<<(unsigned)n_tiles, 32, 0, st>>>(h->D32, dc.log2_stride - 2, n_tiles, h->d_tc_img);
+    if ((rc = check_launch(h, "k_tc_image"))) return rc;
+    h->tc_img_lg = dc.log2_stride;
+  }
   for (int64_t pb = 0; pb < P; pb += P_pad) {
     const int Pn = (int)std::min<int64_t>(P_pad, P - pb);
     {
@@ -329,7 +342,16 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
         // fine sub-intervals may span kNodeDaysF32 / 4 days of signal time
         const bool merge = dc.stride >= 512;
         a.merge_lim = 86400.0 * (kNodeDaysF32 / 4.0) / h->cfg.T_obs_s;
-        if (seg_mode) k_dense2<true, 0><<<grid, kBlock, 0, st>>>(dc, a, Dp);
+        const dim3 grid_tc(pblocks, n_chunks);
+        if (use_tc) {
+          const uint4* Tg = h->d_tc_img;
+          if (seg_mode) k_dense2_tc<true, 0><<<grid_tc, kBlock, tc::kSmemBytes, st>>>(dc, a, Dp, Tg);
+          else if (sincos == 2 && merge) k_dense2_tc<false, 2, true><<<grid_tc, kBlock, tc::kSmemBytes, st>>>(dc, a, Dp, Tg);
+          else if (sincos == 2) k_dense2_tc<false, 2><<<grid_tc, kBlock, tc::kSmemBytes, st>>>(dc, a, Dp, Tg);
+          else if (merge) k_dense2_tc<false, 0, true><<<grid_tc, kBlock, tc::kSmemBytes, st>>>(dc, a, Dp, Tg);
+          else k_dense2_tc<false, 0><<<grid_tc, kBlock, tc::kSmemBytes, st>>>(dc, a, Dp, Tg);
+        }
+        else if (seg_mode) k_dense2<true, 0><<<grid, kBlock, 0, st>>>(dc, a, Dp);
         else if (sincos == 2 && merge) k_dense2<false, 2, true><<<grid, kBlock, 0, st>>>(dc, a, Dp);
         else if (sincos == 2) k_dense2<false, 2><<<grid, kBlock, 0, st>>>(dc, a, Dp);
         else if (merge) k_dense2<false, 0, true><<<grid, kBlock, 0, st>>>(dc, a, Dp);
@@ -731,6 +753,11 @@ int init_common(sc_handle** out, const sc_config* cfg, const double* dA, const d
   SC_INIT(cudaFuncSetAttribute(k_dense<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kDense64Smem));
   SC_INIT(cudaFuncSetAttribute(k_dense<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kDense64Smem));
   SC_INIT(cudaFuncSetAttribute(k_dense<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kDense64Smem));
+  SC_INIT(cudaFuncSetAttribute(k_dense2_tc<true, 0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::kSmemBytes));
+  SC_INIT(cudaFuncSetAttribute(k_dense2_tc<false, 2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::kSmemBytes));
+  SC_INIT(cudaFuncSetAttribute(k_dense2_tc<false, 2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::kSmemBytes));
+  SC_INIT(cudaFuncSetAttribute(k_dense2_tc<false, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::kSmemBytes));
+  SC_INIT(cudaFuncSetAttribute(k_dense2_tc<false, 0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::kSmemBytes));
   const int n_pairs_pad = (n + kChunkF32 - 1) / kChunkF32 * (kChunkF32 / 2);
   SC_INIT(cudaMalloc(&h->D32, (size_t)n_pairs_pad * kPairRec * sizeof(float4)));
   SC_INIT(cudaMalloc(&h->W64, (size_t)n * sizeof(double4)));
@@ -1354,6 +1381,9 @@ int sc_set_option(sc_handle* h, int32_t option, int64_t value) {
     case SC_OPT_WINDOW_SORT:
       if (value < 0 || value > 1) return fail(h, SC_ERR_INVALID_ARG, "window_sort must be 0 or 1");
       h->window_sort = (int)value; return SC_OK;
+    case SC_OPT_TENSOR_CORES:
+      if (value < 0 || value > 1) return fail(h, SC_ERR_INVALID_ARG, "tensor_cores must be 0 or 1");
+      h->use_tc = (int)value; return SC_OK;
     case SC_OPT_ESCALATE:
       if (value < 0 || value > 1) return fail(h, SC_ERR_INVALID_ARG, "escalate must be 0 or 1");
       h->escalate = (int)value; return SC_OK;
@@ -1379,7 +1409,7 @@ int sc_free(sc_handle* h) {
   if (!h) return SC_ERR_NOT_INIT;
   if (h->sub) sc_free(h->sub);
   cudaFree(h->d_seg3);
-  cudaFree(h->D32); cudaFree(h->W64); cudaFree(h->G64);
+  cudaFree(h->D32); cudaFree(h->W64); cudaFree(h->G64); cudaFree(h->d_tc_img);
   cudaFree(h->scratch); cudaFree(h->d_edges); cudaFree(h->d_chunk_k0); cudaFree(h->d_flags);
   cudaFree(h->d_counter); cudaFree(h->d_params_stage); cudaFree(h->d_comp); cudaFree(h->d_km); cudaFree(h->d_T64); cudaFree(h->d_T32); cudaFree(h->d_sp);
   cudaFree(h->d_spsig); cudaFree(h->d_zpart); cudaFree(h->d_hh); cudaFree(h->d_gmom); cudaFree(h->d_smom);
