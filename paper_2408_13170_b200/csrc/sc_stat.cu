@@ -345,11 +345,11 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
         const dim3 grid_tc(pblocks, n_chunks);
         if (use_tc) {
           const uint4* Tg = h->d_tc_img;
-          if (seg_mode) k_dense2_tc<true, 0><<<grid_tc, kBlock, tc::kSmemBytes, st>>>(dc, a, Dp, Tg);
-          else if (sincos == 2 && merge) k_dense2_tc<false, 2, true><<<grid_tc, kBlock, tc::kSmemBytes, st>>>(dc, a, Dp, Tg);
-          else if (sincos == 2) k_dense2_tc<false, 2><<<grid_tc, kBlock, tc::kSmemBytes, st>>>(dc, a, Dp, Tg);
-          else if (merge) k_dense2_tc<false, 0, true><<<grid_tc, kBlock, tc::kSmemBytes, st>>>(dc, a, Dp, Tg);
-          else k_dense2_tc<false, 0><<<grid_tc, kBlock, tc::kSmemBytes, st>>>(dc, a, Dp, Tg);
+          if (seg_mode) k_dense2_tc<true, 0><<<grid_tc, tc::kThreads, tc::kSmemBytes, st>>>(dc, a, Dp, Tg);
+          else if (sincos == 2 && merge) k_dense2_tc<false, 2, true><<<grid_tc, tc::kThreads, tc::kSmemBytes, st>>>(dc, a, Dp, Tg);
+          else if (sincos == 2) k_dense2_tc<false, 2><<<grid_tc, tc::kThreads, tc::kSmemBytes, st>>>(dc, a, Dp, Tg);
+          else if (merge) k_dense2_tc<false, 0, true><<<grid_tc, tc::kThreads, tc::kSmemBytes, st>>>(dc, a, Dp, Tg);
+          else k_dense2_tc<false, 0><<<grid_tc, tc::kThreads, tc::kSmemBytes, st>>>(dc, a, Dp, Tg);
         }
         else if (seg_mode) k_dense2<true, 0><<<grid, kBlock, 0, st>>>(dc, a, Dp);
         else if (sincos == 2 && merge) k_dense2<false, 2, true><<<grid, kBlock, 0, st>>>(dc, a, Dp);
