@@ -77,10 +77,11 @@ enum {
                                 0 = off.  Not applied by sc_eval_segments / _components / _loglike / _adaptive.        */
   SC_OPT_ESC_TAU_POLY_X1000 = 10,  /* tau x 1000 for the polynomial sin/cos flavour (default 6000)                    */
   SC_OPT_ESC_TAU_MUFU_X1000 = 11,  /* tau x 1000 for the hardware sin/cos flavour (default 16000)                     */
-  SC_OPT_TENSOR_CORES = 13,  /* 1 (default): the FP32-amplitude path evaluates the amplitude correction about the centre of every
-                                fine sub-interval as a TF32x3 contraction on the tensor cores (tcgen05, k_dense2_tc; node
-                                spacings >= 128 bins).  0 = the CUDA-core kernel k_dense2 (Horner cubics per bin).  Same
-                                definition, same tolerance; the two differ at the FP32 rounding level.                 */
+  SC_OPT_TENSOR_CORES = 13,  /* 0 (default): the CUDA-core kernel k_dense2 (Horner cubics per bin).  1: the FP32-amplitude path
+                                forms the amplitude x data factor of every bin as a split-TF32 contraction on the tensor cores
+                                (tcgen05, k_dense2_tc; node spacings >= 128 bins; chunks of 8192 bins).  Same definition, same
+                                tolerance, the two differ at the FP32 rounding level.  Measured on c3: 1.2 - 1.4 x SLOWER than
+                                k_dense2 (DESIGN.md section 6 says why) -- kept as a tested alternative, not the product path. */
   SC_OPT_WINDOW_SORT = 12    /* 1 (default): each particle batch is processed in the order of the time-window centres (stable
                                 radix sort on the device), so that the 32 particles of a warp share their windows; results
                                 are bitwise reproducible for a given population and option set, but a particle's rounding

@@ -48,12 +48,9 @@ constexpr int kOffA = 0;
 constexpr int kOffT = kABytes;                            // ring
 constexpr int kOffBar = kOffT + kStages * kTileBytes;     // b_full[4], s_free[4], d_full[4], buf_free[4], a_ready
 constexpr int kBarFull = 0, kBarSFree = 4, kBarDFull = 8, kBarBufFree = 12, kBarAReady = 16, kNumBars = 17;
-constexpr int kOffU = kOffBar + kNumBars * 8;             // tmem base, fast mask[2], merge mask, n_list
-constexpr int kOffList = kOffU + 24;                      // tile list (uint8 x 128), trigger list (uint8 x 128)
-constexpr int kSmemBytes = kOffList + 256;
-constexpr int kMaxTiles = kChunkF32 / kTileBins;          // 128
-constexpr uint32_t kTrigRows = 0xffu;                     // first tile after a gap: waits for the four warps' coefficient rows
-constexpr uint32_t kTrigNone = 0xfeu;                     // its next three tiles: nothing more to wait for
+constexpr int kOffU = kOffBar + kNumBars * 8;             // tmem base, i_lo (max), i_hi (min), merge mask
+constexpr int kSmemBytes = kOffU + 24;
+constexpr int kChunk = 8192;                              // bins per CTA (nothing but the tiles in flight is staged)
 constexpr int kThreads = kBlock + 32;                     // four consumer warps (lane = particle) and the producer warp
 // instruction descriptor: D = F32, A = B = TF32, both K-major, N = 32, M = 128
 constexpr uint32_t kIdesc = (1u << 4) | (2u << 7) | (2u << 10) | ((32u >> 3) << 17) | ((128u >> 4) << 24);
@@ -126,22 +123,29 @@ __device__ __forceinline__ void pin16(uint32_t* d) {    // (no instruction: orde
                     "+r"(d[8]), "+r"(d[9]), "+r"(d[10]), "+r"(d[11]), "+r"(d[12]), "+r"(d[13]), "+r"(d[14]), "+r"(d[15]) :: "memory");
 }
 
-// The producer (one thread of the fifth warp): for every listed tile g, in order, wait for its trigger (the four consumer
-// warps have released the TMEM buffer it reuses / have written the coefficient rows it needs) and for its operand image,
-// issue the 6 MMAs (M128 N32 K8) into TMEM buffer g & 3, commit to d_full (consumers) and s_free (the ring stage), then start
-// the load of tile g + 2 into the stage tile g - 2 has vacated.
-__device__ __noinline__ void producer(uint32_t sb, uint32_t tmem, const uint4* __restrict__ Tc, int n_list) {
+// The producer (one thread of the fifth warp): for every tile of the tensor-core range [i_lo, i_hi) of sub-intervals, in
+// walking order (g = 0, 1, ...), wait for its trigger (the four consumer warps have released the TMEM buffer it reuses /
+// have written the coefficient rows it needs) and for its operand image, issue the 6 MMAs (M128 N32 K8) into TMEM buffer
+// g & 3, commit to d_full (consumers) and s_free (the ring stage), then start the load of tile g + 2 into the stage tile
+// g - 2 has vacated.  Triggers: tile t >= 4 of a sub-interval -- tile g - 4 (its buffer); t < 4 of a sub-interval that
+// follows another -- the last tile of that one (the rows are rewritten when it is entered); the very first tile -- the rows.
+__device__ __noinline__ void producer(uint32_t sb, uint32_t tmem, const uint4* __restrict__ Tc, int i_lo, int i_hi, int lg_tps,
+                                      int n_last /* tiles of sub-interval i_hi - 1 */) {
   const uint32_t bar = sb + kOffBar;
-  uint32_t n_rows = 0;        // rendezvous passed so far
+  const int tps = 1 << lg_tps;                                // tiles per (full) sub-interval
+  const int n_list = ((i_hi - i_lo - 1) << lg_tps) + n_last;
+  const int tile0 = i_lo << lg_tps;                           // listed tile g is tile tile0 + g of the chunk
   for (int g = 0; g < min(n_list, 2); ++g) {
     mbar_expect_tx(bar + (kBarFull + g) * 8, kTileBytes);
-    bulk_g2s(sb + kOffT + g * kTileBytes, Tc + (size_t)lds_u8(sb + kOffList + g) * (kTileBytes / 16), kTileBytes, bar + (kBarFull + g) * 8);
+    bulk_g2s(sb + kOffT + g * kTileBytes, Tc + (size_t)(tile0 + g) * (kTileBytes / 16), kTileBytes, bar + (kBarFull + g) * 8);
   }
   for (int g = 0; g < n_list; ++g) {
-    const int stg = g & 3;
-    const uint32_t tr = lds_u8(sb + kOffList + kMaxTiles + g);
-    if (tr == kTrigRows) { mbar_wait(bar + kBarAReady * 8, n_rows & 1u); ++n_rows; }
-    else if (tr != kTrigNone) mbar_wait(bar + (kBarBufFree + (tr & 3u)) * 8, (tr >> 2) & 1u);
+    const int stg = g & 3, t = g & (tps - 1);
+    if (g == 0) mbar_wait(bar + kBarAReady * 8, 0u);
+    else if (g >= tps || g >= 4) {
+      const int tr = (g < tps || t >= 4) ? g - 4 : g - t - 1;
+      mbar_wait(bar + (kBarBufFree + (tr & 3)) * 8, (uint32_t)((tr >> 2) & 1));
+    }
     mbar_wait(bar + (kBarFull + stg) * 8, (uint32_t)((g >> 2) & 1));
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     const uint32_t aA = sb + kOffA, bB = sb + kOffT + stg * kTileBytes;
@@ -156,7 +160,7 @@ __device__ __noinline__ void producer(uint32_t sb, uint32_t tmem, const uint4* _
       const int x = g + 2, s2 = x & 3;
       if (x >= 4) mbar_wait(bar + (kBarSFree + s2) * 8, (uint32_t)(((x >> 2) - 1) & 1));   // the MMAs of tile x - 4 have read the stage
       mbar_expect_tx(bar + (kBarFull + s2) * 8, kTileBytes);
-      bulk_g2s(sb + kOffT + s2 * kTileBytes, Tc + (size_t)lds_u8(sb + kOffList + x) * (kTileBytes / 16), kTileBytes, bar + (kBarFull + s2) * 8);
+      bulk_g2s(sb + kOffT + s2 * kTileBytes, Tc + (size_t)(tile0 + x) * (kTileBytes / 16), kTileBytes, bar + (kBarFull + s2) * 8);
     }
   }
 }
@@ -219,18 +223,17 @@ __device__ __forceinline__ void tc_pair(PhaseFD& ph, u64 K2, u64 qr2, u64 qi2, u
   zi2 = f2fma(qr2, sr2, f2fma(qi2, cr2, zi2));
 }
 
+
 #ifndef SC_DENSE2TC_MINB
 #define SC_DENSE2TC_MINB 4
 #endif
 template <bool SEG, int SC, bool MERGE = false>
 __global__ void __launch_bounds__(tc::kThreads, SC_DENSE2TC_MINB) k_dense2_tc(DevCfg c, DenseArgs a, const ulonglong2* __restrict__ Dg,
-                                                         const uint4* __restrict__ Tg) {
-  constexpr int CH = kChunkF32;
+                                                                             const uint4* __restrict__ Tg) {
+  constexpr int CH = tc::kChunk;
   extern __shared__ __align__(128) unsigned char smem[];
   uint4* sA = reinterpret_cast<uint4*>(smem + tc::kOffA);
   uint32_t* sU = reinterpret_cast<uint32_t*>(smem + tc::kOffU);
-  uint8_t* tlist = smem + tc::kOffList;
-  uint8_t* trig = tlist + tc::kMaxTiles;
   const uint32_t sb = tc::smem_u32(smem);
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -254,7 +257,7 @@ __global__ void __launch_bounds__(tc::kThreads, SC_DENSE2TC_MINB) k_dense2_tc(De
   if (tid == 0) {
 #pragma unroll
     for (int i = 0; i < tc::kNumBars; ++i) tc::mbar_init(sb + tc::kOffBar + i * 8, (i >= tc::kBarBufFree) ? 4 : 1);
-    sU[1] = 0xffffffffu; sU[2] = 0xffffffffu; sU[3] = 0xffffffffu; sU[4] = 0u;
+    sU[1] = 0u; sU[2] = 0x7fffffffu; sU[3] = 0xffffffffu;
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 0) {
@@ -269,60 +272,37 @@ __global__ void __launch_bounds__(tc::kThreads, SC_DENSE2TC_MINB) k_dense2_tc(De
   const uint32_t tm_lane = tmem + ((uint32_t)(warp * 32) << 16);
 
   const int S = c.stride, Sf = S >> 2, lgSf = c.log2_stride - 2;
-  const int n_sub = CH >> lgSf;                                // <= 64 (Sf >= 32)
+  const int n_sub = (ce2 - cs + Sf - 1) >> lgSf;              // sub-intervals of this chunk (the last one may be cut by the band end)
   const float hS = 1.0f / (float)Sf;
   const u64 h2 = f2bcast(2.0f * hS);
   const u64 K2 = f2bcast(1.4629180792671596e-09f);            // 2 pi / 2^32
 
-  // which fine sub-intervals have all 128 lanes inside their windows (the tensor-core path), which coarse intervals merge
-  {
-    uint32_t m0 = 0u, m1 = 0u;
-    for (int i = 0; i < n_sub; ++i) {
-      const int ib = cs + (i << lgSf);
-      if (ib >= ce2) break;
-      if (is_prod || (ib >= jlo && min(ib + Sf, ce2) <= jhi)) { if (i < 32) m0 |= 1u << i; else m1 |= 1u << (i - 32); }
-    }
-    uint32_t mm = is_prod ? 0xffffffffu : 0u;
-    if (MERGE && !is_prod) {
-      const int n_co = CH >> c.log2_stride;                    // <= 4 (stride >= 512)
+  // The sub-intervals all 128 lanes spend inside their time windows form one range [i_lo, i_hi) (every window is an
+  // interval): the tensor-core range.  Which coarse intervals merge (see k_dense2) is decided for the CTA as well.
+  if (!is_prod) {
+    const int lo_l = max(0, (jlo - cs + Sf - 1) >> lgSf);
+    const int hi_l = (ce2 <= jhi) ? n_sub : min(max(jhi - cs, 0) >> lgSf, n_sub - 1);
+    uint32_t mm = 0u;
+    if constexpr (MERGE) {
+      const int n_co = CH >> c.log2_stride;                    // <= 16 (stride >= 512)
       for (int ic = 0; ic < n_co; ++ic) {
         const int ib = cs + (ic << c.log2_stride);
         const bool win = (ib >= jlo) && (ib + S <= jhi) && (ib + S <= ce2);
         if (win && coarse_dslope(c, a, p, ib >> c.log2_stride) <= a.merge_lim) mm |= 1u << ic;
       }
     }
-    m0 = __reduce_and_sync(0xffffffffu, m0); m1 = __reduce_and_sync(0xffffffffu, m1); mm = __reduce_and_sync(0xffffffffu, mm);
-    if (lane == 0) { atomicAnd(&sU[1], m0); atomicAnd(&sU[2], m1); atomicAnd(&sU[3], mm); }
+    const int lo_w = __reduce_max_sync(0xffffffffu, lo_l), hi_w = __reduce_min_sync(0xffffffffu, hi_l);
+    mm = __reduce_and_sync(0xffffffffu, mm);
+    if (lane == 0) { atomicMax(&sU[1], (uint32_t)lo_w); atomicMin(&sU[2], (uint32_t)hi_w); atomicAnd(&sU[3], mm); }
   }
   __syncthreads();
-  const unsigned long long fastmask = (unsigned long long)sU[1] | ((unsigned long long)sU[2] << 32);
+  const int i_lo = (int)sU[1], i_hi = max((int)sU[2], i_lo);   // (empty range: i_hi = i_lo)
   const uint32_t mergemask = MERGE ? sU[3] : 0u;
   const uint4* Tc = Tg + (size_t)(cs >> 4) * (tc::kTileBytes / 16);   // this chunk's tiles
-  // The tile list: the 16-bin tiles of the tensor-core sub-intervals in walking order, each with its trigger -- the listed
-  // tile whose release by all four warps lets the producer issue it: g - 4 (the TMEM buffer it reuses) inside a
-  // sub-interval, the last tile of the preceding sub-interval for the first four tiles of a sub-interval that follows
-  // another directly (the coefficient rows are rewritten when that tile is entered); after a gap the first tile waits for
-  // the rows (every buffer has been released by then).
-  if (tid == 0) {
-    int n = 0;
-    for (int i = 0; i < n_sub; ++i) {
-      if (!((fastmask >> i) & 1ull)) continue;
-      const int ib = cs + (i << lgSf);
-      const int nt = (min(ib + Sf, ce2) - ib + 15) >> 4;
-      const bool cold = (i == 0) || !((fastmask >> (i - 1)) & 1ull);
-      const int first = n;
-      for (int t = 0; t < nt; ++t) {
-        tlist[n] = (uint8_t)(((i << lgSf) >> 4) + t);
-        trig[n] = (uint8_t)((t >= 4) ? n - 4 : (cold ? (t == 0 ? tc::kTrigRows : tc::kTrigNone) : first - 1));
-        ++n;
-      }
-    }
-    sU[4] = (uint32_t)n;
-  }
-  __syncthreads();
-  const int n_list = (int)sU[4];
+  const int lg_tps = lgSf - 4;                                 // tiles per sub-interval
+  auto tiles_of = [&](int i) { const int ib = cs + (i << lgSf); return (min(ib + Sf, ce2) - ib + 15) >> 4; };
   if (is_prod) {
-    if (lane == 0) tc::producer(sb, tmem, Tc, n_list);
+    if (lane == 0 && i_hi > i_lo) tc::producer(sb, tmem, Tc, i_lo, i_hi, lg_tps, tiles_of(i_hi - 1));
     __syncwarp();
   }
 
@@ -407,25 +387,25 @@ __global__ void __launch_bounds__(tc::kThreads, SC_DENSE2TC_MINB) k_dense2_tc(De
   PhaseFD fd = {}, fd_n = {};
   float cf[4][4], cf_n[4][4];
   bool fresh_n = false, prepared = false;   // the next sub-interval's set-up has been made (and its row written)
-  int g_base = 0;              // listed tiles that belong to earlier sub-intervals
-  int nl = 0;                  // listed tiles below nl have been released by this warp
+  const uint32_t bar_d = sb + tc::kOffBar + tc::kBarDFull * 8, bar_f = sb + tc::kOffBar + tc::kBarBufFree * 8;
 
-  // this warp is done with listed tile u (its accumulator rows are in registers or consumed)
-  auto leave = [&](int u) {
+  // this warp is done with listed tile g (its accumulator row is in registers or consumed): one arrival per warp
+  auto leave = [&](int g) {
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-    __syncwarp();
-    if (tc::elect_one()) tc::mbar_arrive(sb + tc::kOffBar + (tc::kBarBufFree + (u & 3)) * 8);
+    asm volatile("{\n.reg .pred P1;\nsetp.eq.u32 P1, %1, 0;\n@P1 mbarrier.arrive.shared::cta.b64 _, [%0];\n}"
+                 :: "r"(bar_f + (uint32_t)(g & 3) * 8), "r"(lane) : "memory");
   };
 
   for (int ib = cs; ib < ce2; ib += Sf) {
     const int ie = min(ib + Sf, ce2);
     const int i_sub = (ib - cs) >> lgSf;
-    const bool fast = (fastmask >> i_sub) & 1ull;              // CTA-uniform
+    const bool fast = (i_sub >= i_lo) && (i_sub < i_hi);       // CTA-uniform
 
     if (fast) {
-      // ---------------------------------------------------------------- tensor-core sub-interval
+      // ---------------------------------------------------------------- tensor-core sub-interval, tile by tile
       const int n_t = (ie - ib + 15) >> 4;
-      const bool chain_next = (i_sub + 1 < n_sub) && ((fastmask >> (i_sub + 1)) & 1ull);
+      const int g_base = (i_sub - i_lo) << lg_tps;             // listed tiles that belong to earlier sub-intervals
+      const bool chain_next = (i_sub + 1 < i_hi);
       if (prepared) {
         if (fresh_n) fd = fd_n;
 #pragma unroll
@@ -438,13 +418,22 @@ __global__ void __launch_bounds__(tc::kThreads, SC_DENSE2TC_MINB) k_dense2_tc(De
         setup(ib, fd, fresh, cf);
         write_row(cf);
         __syncwarp();
-        if (tc::elect_one()) tc::mbar_arrive(sb + tc::kOffBar + tc::kBarAReady * 8);   // rendezvous: the producer waits for the four rows
+        if (lane == 0) tc::mbar_arrive(sb + tc::kOffBar + tc::kBarAReady * 8);   // the producer waits for the four rows
       }
-      int cur_t = -1;          // tile of this sub-interval whose MMAs this warp has waited for
-      auto enter = [&](int t) {
-        const int g = g_base + t;
-        while (nl < g) { leave(nl); ++nl; }
-        tc::mbar_wait(sb + tc::kOffBar + (tc::kBarDFull + (g & 3)) * 8, (uint32_t)((g >> 2) & 1));
+      int piece = a.piece_first[(ib >> lgSf) - ((a.chunk_first * CH) >> lgSf)];
+      u64 zr2 = 0, zi2 = 0;    // FP32 partial sums (even bins, odd bins) of the open piece since the last fold
+      bool live = (k >= 0) && (k < a.n_seg);
+      bool carry = false;      // the odd bin of a pair that straddled an edge waits in car_* for the piece it belongs to
+      float car_zr = 0.f, car_zi = 0.f;
+      auto fold = [&]() {
+        float zrl, zrh, zil, zih;
+        f2unpack(zr2, zrl, zrh); f2unpack(zi2, zil, zih);
+        if (live) { Zr += (double)(zrl + zrh); Zi += (double)(zil + zih); }
+        zr2 = 0; zi2 = 0;
+      };
+      for (int t = 0; t < n_t; ++t) {
+        const int tb = ib + (t << 4), te = min(tb + 16, ie), g = g_base + t;
+        tc::mbar_wait(bar_d + (uint32_t)(g & 3) * 8, (uint32_t)((g >> 2) & 1));
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         if (t == n_t - 1 && chain_next) {
           // every MMA of this sub-interval has completed: the row of the next one may be written now
@@ -452,86 +441,83 @@ __global__ void __launch_bounds__(tc::kThreads, SC_DENSE2TC_MINB) k_dense2_tc(De
           write_row(cf_n);
           prepared = true;
         }
-        cur_t = t;
-      };
-
-      int piece = a.piece_first[(ib >> lgSf) - ((a.chunk_first * CH) >> lgSf)];
-      u64 zr2 = 0, zi2 = 0;    // FP32 partial sums (even bins, odd bins) of the open piece since the last fold
-      auto fold = [&](bool live) {
-        float zrl, zrh, zil, zih;
-        f2unpack(zr2, zrl, zrh); f2unpack(zi2, zil, zih);
-        if (live) { Zr += (double)(zrl + zrh); Zi += (double)(zil + zih); }
-        zr2 = 0; zi2 = 0;
-      };
-      float car_zr = 0.f, car_zi = 0.f;
-      bool carry = false;
-      int pl = ib;
-      while (pl < ie) {
-        const int ph = min(next_edge, ie);                     // next_edge > pl: edges <= pl are consumed
-        const bool live = (k >= 0) && (k < a.n_seg);
-        int jj = pl;
-        if (carry) {
-          if (live) { Zr += (double)car_zr; Zi += (double)car_zi; }
-          carry = false;
-          jj = pl + 1;
-        }
-        const int jfull = ph & ~1;                             // full pairs end here; a straddling pair follows if ph is odd
-        if (!live && jj < jfull) {
-          for (int t = jj; t < jfull; t += 2) phase_skip_pair(fd);
-          jj = jfull;
-        }
-        while (jj < ph) {
-          const bool split = (jj == jfull);                    // the pair (ph - 1, ph)
-          const int e2 = split ? jj + 2 : min(jfull, (jj & ~15) + 16);   // a group stays inside one tile
-          const int t = (jj - ib) >> 4, g = g_base + t;
-          if (t != cur_t) enter(t);
-          const uint32_t tbuf = tm_lane + (uint32_t)((g & 3) * 32);
-          if (e2 - jj == 16) {
-            // a whole tile: all 32 accumulator columns at once, the buffer is released before the arithmetic
-            uint32_t d[32];
-            tc::tld16(tbuf, d); tc::tld16(tbuf + 16, d + 16);
-            tc::tld_wait16(d); tc::pin16(d + 16);
-            leave(g); nl = g + 1;
+        const uint32_t tbuf = tm_lane + (uint32_t)((g & 3) * 32);
+        if (next_edge >= te && live && !carry && te - tb == 16) {
+          // a whole tile inside one live piece: all 32 accumulator columns at once, the buffer is released before the arithmetic
+          uint32_t d[32];
+          tc::tld16(tbuf, d); tc::tld16(tbuf + 16, d + 16);
+          tc::tld_wait16(d); tc::pin16(d + 16);
+          leave(g);
 #if defined(SC_TC_EXP) && SC_TC_EXP == 5   /* timing experiment: pipeline only, no per-bin arithmetic */
 #pragma unroll
-            for (int i = 0; i < 8; ++i) { zr2 ^= (u64)d[4 * i] | ((u64)d[4 * i + 1] << 32); zi2 ^= (u64)d[4 * i + 2] | ((u64)d[4 * i + 3] << 32); }
+          for (int i = 0; i < 8; ++i) { zr2 ^= (u64)d[4 * i] | ((u64)d[4 * i + 1] << 32); zi2 ^= (u64)d[4 * i + 2] | ((u64)d[4 * i + 3] << 32); }
 #else
 #pragma unroll
-            for (int i = 0; i < 8; ++i)
-              tc_pair<SC>(fd, K2, f2pack(__uint_as_float(d[4 * i]), __uint_as_float(d[4 * i + 1])),
-                          f2pack(__uint_as_float(d[4 * i + 2]), __uint_as_float(d[4 * i + 3])), zr2, zi2);
+          for (int i = 0; i < 8; ++i)
+            tc_pair<SC>(fd, K2, f2pack(__uint_as_float(d[4 * i]), __uint_as_float(d[4 * i + 1])),
+                        f2pack(__uint_as_float(d[4 * i + 2]), __uint_as_float(d[4 * i + 3])), zr2, zi2);
 #endif
-          } else {
-            for (int j = jj; j < e2; j += 2) {
+          if (t & 1) fold();                                   // every 32 bins
+        } else {
+          // a tile cut by segment edges, outside [e_0, e_N), or cut by the band end: piece by piece, pair by pair
+          int jj = tb;
+          while (jj < te) {
+            const int ph = min(next_edge, te);                 // next_edge > jj (edges <= jj are consumed)
+            if (carry) {                                       // jj is the odd bin of the straddling pair: already evaluated
+              if (live) { Zr += (double)car_zr; Zi += (double)car_zi; }
+              carry = false;
+              ++jj;
+            }
+            const int jfull = ph & ~1;                         // full pairs end here; a straddling pair follows if ph is odd
+            for (; jj < jfull; jj += 2) {
+              if (live) {
+                uint32_t d[4];
+                tc::tld4(tbuf + (uint32_t)((jj & 15) * 2), d);
+                tc::tld_wait4(d);
+                tc_pair<SC>(fd, K2, f2pack(__uint_as_float(d[0]), __uint_as_float(d[1])), f2pack(__uint_as_float(d[2]), __uint_as_float(d[3])), zr2, zi2);
+              } else {
+                phase_skip_pair(fd);
+              }
+            }
+            if (jj < ph) {
+              // the pair (ph - 1, ph): even bin -> the piece that ends at ph, odd bin -> the next one
+              fold();
               uint32_t d[4];
-              tc::tld4(tbuf + (uint32_t)((j & 15) * 2), d);
+              tc::tld4(tbuf + (uint32_t)((jj & 15) * 2), d);
               tc::tld_wait4(d);
               tc_pair<SC>(fd, K2, f2pack(__uint_as_float(d[0]), __uint_as_float(d[1])), f2pack(__uint_as_float(d[2]), __uint_as_float(d[3])), zr2, zi2);
+              float zrl, zil;
+              f2unpack(zr2, zrl, car_zr); f2unpack(zi2, zil, car_zi);
+              if (live) { Zr += (double)zrl; Zi += (double)zil; }
+              zr2 = 0; zi2 = 0;
+              carry = true;
+              jj = ph;                                         // (the odd bin ph is taken at the top of the next piece)
+            }
+            if (ph == next_edge) {
+              // the piece ends at an edge inside (or at the end of) the tile
+              fold();
+              if (ph < ie) {                                   // (an edge on the sub-interval end is handled below)
+                if (live) Sg += sigma_moments(cf, a.moments + (size_t)piece * 4);
+                ++piece;
+                while (next_edge == ph) {
+                  if (k >= 0 && k < a.n_seg) close_piece(true);
+                  next_segment();
+                }
+                live = (k >= 0) && (k < a.n_seg);
+              }
             }
           }
-          jj = e2;
-          if (split) {
-            // (the sums were folded before this pair: see below) even bin -> the piece that ends, odd bin -> the next one
-            float zrl, zrh, zil, zih;
-            f2unpack(zr2, zrl, zrh); f2unpack(zi2, zil, zih);
-            if (live) { Zr += (double)zrl; Zi += (double)zil; }
-            car_zr = zrh; car_zi = zih; carry = true;
-            zr2 = 0; zi2 = 0;
-          } else if (jj == ph || (jj & 31) == 0 || jj == jfull) {
-            fold(live);                                        // piece end, every 32 bins, and before a straddling pair
-          }
+          leave(g);
+          if (t & 1) fold();
         }
-        if (live) Sg += sigma_moments(cf, a.moments + (size_t)piece * 4);
-        ++piece;
-        while (next_edge == ph) {                              // segments that end here (incl. empty ones)
-          if (k >= 0 && k < a.n_seg) close_piece(true);
-          next_segment();
-        }
-        pl = ph;
       }
-      if (cur_t != n_t - 1) enter(n_t - 1);                    // (tiles skipped outside [e_0, e_N): keep the chain going)
-      g_base += n_t;
-      if (!chain_next) while (nl < g_base) { leave(nl); ++nl; }   // a rendezvous follows: every buffer is free by then
+      // the piece open at the end of the sub-interval
+      fold();
+      if (live) Sg += sigma_moments(cf, a.moments + (size_t)piece * 4);
+      while (next_edge == ie) {                                // segments that end here (incl. empty ones)
+        if (k >= 0 && k < a.n_seg) close_piece(true);
+        next_segment();
+      }
       continue;
     }
 

@@ -95,8 +95,9 @@ struct sc_handle : EdgeCache {
   int escalate = 1; double esc_tau_poly = 6.0, esc_tau_mufu = 16.0;
   int* d_esc_idx = nullptr; int* d_esc_count = nullptr; double* d_esc_params = nullptr; double* d_esc_out = nullptr;
   size_t esc_idx_cap = 0, esc_cnt_cap = 0, esc_par_cap = 0, esc_out_cap = 0; int* h_esc_hint = nullptr;
-  // tensor-core path of the FP32-amplitude kernel (k_dense2_tc): per-tile operand image, built for one node spacing
-  int use_tc = 1; uint4* d_tc_img = nullptr; size_t tc_img_cap = 0; int tc_img_lg = 0;
+  // tensor-core flavour of the FP32-amplitude kernel (k_dense2_tc, SC_OPT_TENSOR_CORES; off by default: measured slower than
+  // k_dense2): per-tile operand image, built for one node spacing
+  int use_tc = 0; uint4* d_tc_img = nullptr; size_t tc_img_cap = 0; int tc_img_lg = 0;
   int window_sort = 1; void* d_sort_tmp = nullptr; size_t sort_cap = 0;   // cub radix-sort workspace of the window sort
   // three-channel handles (A, E, T): the T channel lives in a second handle whose first slot carries T (chan_set = 1)
   // and whose second slot is empty; the per-segment sums of both are added before |z|^2/sigma is formed
@@ -285,9 +286,9 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
   // particle blocks launched per kernel: all of them, or (escalation pass) the caller's estimate -- the kernels stride
   const int pblocks = esc_count ? std::max(1, std::min(esc_blocks, P_pad / kBlock)) : P_pad / kBlock;
   // tensor-core flavour of the FP32-amplitude kernel: fine sub-intervals of at least one 32-bin tile
-  const bool use_tc = sizeof(R) == 4 && h->use_tc && dc.log2_stride >= 7 && n_chunks > 0;
+  const bool use_tc = sizeof(R) == 4 && h->cached_chunk == tc::kChunk && n_chunks > 0;
   if (use_tc && h->tc_img_lg != dc.log2_stride) {
-    const long long n_tiles = (long long)((dc.n_bins + kChunkF32 - 1) / kChunkF32) * (kChunkF32 / tc::kTileBins);
+    const long long n_tiles = (long long)((dc.n_bins + tc::kChunk - 1) / tc::kChunk) * (tc::kChunk / tc::kTileBins);
     if ((rc = grow(h, (void**)&h->d_tc_img, &h->tc_img_cap, (size_t)n_tiles * tc::kTileBytes))) return rc;
     Timed tm(h, st, SC_TIME_OTHER);
     k_tc_image<<<(unsigned)n_tiles, 32, 0, st>>>(h->D32, dc.log2_stride - 2, n_tiles, h->d_tc_img);
@@ -373,7 +374,7 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
       k_stitch<<<esc_count ? pblocks : ((sorted ? P_pad : Pn) + 127) / 128, 128, 0, st>>>(frag, h->d_flags, n_chunks, P_pad, Pn, 1.0 / g2, out ? out + pb : nullptr,
                                                  out_comp ? out_comp + pb * 3 : nullptr, h->s0 * h0 / sqrt(g2),
                                                  h->s0 * h->s0 * h0 * h0, esc_count, (int)pb, sorted ? pmap : nullptr,
-                                                 jlo, jhi, h->chunk_first, sizeof(R) == 4 ? kChunkF32 : kChunkF64, h->d_next_close);
+                                                 jlo, jhi, h->chunk_first, h->cached_chunk, h->d_next_close);
     }
     if ((rc = check_launch(h, "k_stitch"))) return rc;
   }
@@ -472,7 +473,9 @@ int eval_common(sc_handle* h, const double* params, int64_t P, const int32_t* se
   const bool f64 = (h->precision == 2) || (h->precision == 0 && n_seg < h->f32_min_seg);
   // all-FP64 path: sigma from FP64 piece moments when a fine sub-interval is long enough to pay for them (>= 32 bins)
   const int lg_fine64 = (h->lg_f64 - 2 >= 5) ? h->lg_f64 - 2 : 0;
-  int rc = prepare_edges(h, seg_edges, n_seg, f64 ? kChunkF64 : kChunkF32, f64 ? lg_fine64 : h->lg_f32 - 2, st);
+  // chunk length: 1024 bins (all-FP64), 2048 (k_dense2: the chunk's data is staged in shared memory), 8192 (k_dense2_tc)
+  const int ch32 = (h->use_tc && h->lg_f32 >= 7) ? tc::kChunk : kChunkF32;
+  int rc = prepare_edges(h, seg_edges, n_seg, f64 ? kChunkF64 : ch32, f64 ? lg_fine64 : h->lg_f32 - 2, st);
   if (rc) return rc;
   SC_CUDA(h, cudaMemsetAsync(h->d_counter, 0, 8, st));
   if (seg_mode) SC_CUDA(h, cudaMemsetAsync(out_seg, 0, (size_t)P * n_seg * 3 * 8, st));
@@ -758,7 +761,7 @@ int init_common(sc_handle** out, const sc_config* cfg, const double* dA, const d
   SC_INIT(cudaFuncSetAttribute(k_dense2_tc<false, 2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::kSmemBytes));
   SC_INIT(cudaFuncSetAttribute(k_dense2_tc<false, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::kSmemBytes));
   SC_INIT(cudaFuncSetAttribute(k_dense2_tc<false, 0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::kSmemBytes));
-  const int n_pairs_pad = (n + kChunkF32 - 1) / kChunkF32 * (kChunkF32 / 2);
+  const int n_pairs_pad = (n + tc::kChunk - 1) / tc::kChunk * (tc::kChunk / 2);   // whole chunks of either FP32-amplitude kernel
   SC_INIT(cudaMalloc(&h->D32, (size_t)n_pairs_pad * kPairRec * sizeof(float4)));
   SC_INIT(cudaMalloc(&h->W64, (size_t)n * sizeof(double4)));
   SC_INIT(cudaMalloc(&h->G64, (size_t)n * sizeof(double2)));

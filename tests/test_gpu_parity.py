@@ -326,7 +326,7 @@ def _hard_particles(got, N, n_each=8):
     return np.concatenate([small, near])
 
 
-def _full_launch_case(oracle, torch, sc, cid, n_sample, seed, tc_hint=True):
+def _full_launch_case(oracle, torch, sc, cid, n_sample, seed, tc_hint=True, opts=()):
     """GPU: the whole population in bench.py's launch configuration, every level.  Oracle (truth mode: long-double phase,
     so the 1e-6 bar holds flat down to the smallest Upsilon): a seeded random sample of n_sample particles plus, per level,
     the 8 smallest non-zero and the 8 nearest the escalation threshold."""
@@ -335,6 +335,8 @@ def _full_launch_case(oracle, torch, sc, cid, n_sample, seed, tc_hint=True):
     H = gpu_handle(inp, dA, dE)
     if tc_hint:
         H.set_option(sc.SC_OPT_TC_MAX_S, int(np.ceil(inp["hi"][2])))      # what bench.py sets: the tile's t_c bound
+    for o, v in opts:
+        H.set_option(o, v)
     P = inp["particles"].shape[0]
     levels = inp["spec"]["n_segs"]
     par = _dev(torch, inp["particles"])
@@ -390,6 +392,13 @@ def test_c5_full_hierarchy_with_coherent_level(oracle, torch_cuda, sc):
     inp, levels, idx, ref, got, dd = _full_launch_case(oracle, torch_cuda, sc, 5, 64, 5)
     assert levels[-1] == 1
     _check_case(inp, levels, idx, ref, got, dd)
+
+
+@pytest.mark.parametrize("cid", [3, 4])
+def test_tensor_core_flavour(oracle, torch_cuda, sc, cid):
+    """SC_OPT_TENSOR_CORES = 1 (k_dense2_tc: the amplitude x data factor as a split-TF32 contraction on tcgen05, accumulators in
+    TMEM, 8192-bin chunks): same definition, same bar against the oracle -- c3 (N = 5000) and c4 (N = 50000, 5000, 500)."""
+    _check_case(*_full_launch_case(oracle, torch_cuda, sc, cid, 24, 10 + cid, opts=((sc.SC_OPT_TENSOR_CORES, 1),)))
 
 
 def test_default_stride_without_tile_hint(oracle, torch_cuda, sc):
