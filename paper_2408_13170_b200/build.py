@@ -9,7 +9,10 @@ DEPS = ([SRC, os.path.join(HERE, "..", "include", "sc_stat.h")]
 LIB = os.path.join(HERE, "libscstat.so")
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-              "-Xcompiler", "-fPIC", "-shared"]
+              "-Xcompiler", "-fPIC", "-shared",
+              # the CUDA runtime is linked dynamically (libcudart.so.12: the toolkit's copy by rpath, or the one the
+              # process has loaded already), so the library carries no runtime code of its own
+              "-cudart", "shared", "-Xlinker", "-rpath=/usr/local/cuda/lib64"]
 
 
 def nvcc():

@@ -120,7 +120,8 @@ __global__ void k_particle_consts(DevCfg c, const double* __restrict__ params, i
       if (c.window_mode == 1) {
         // Q4: the template lives where 0 <= t(f_j) <= T_obs; t(f) is monotone, so bisect on the bin index
         // with t(f_j) evaluated directly at the bin frequencies (same expression the definition uses).
-        int lo = 0, hi = c.n_bins;       // first j with t(f_j) >= 0
+        const int j_first = (c.j0 == 0) ? 1 : 0;   // (f = 0 carries no template: t(f) diverges there)
+        int lo = j_first, hi = c.n_bins;  // first j with t(f_j) >= 0
         while (lo < hi) {
           const int mid = (lo + hi) >> 1;
           if (tf_direct(c, q, (double)(c.j0 + mid) / c.T_obs) >= 0.0) hi = mid; else lo = mid + 1;
@@ -132,8 +133,23 @@ __global__ void k_particle_consts(DevCfg c, const double* __restrict__ params, i
           if (tf_direct(c, q, (double)(c.j0 + mid) / c.T_obs) > c.T_obs) hi = mid; else lo = mid + 1;
         }
         jhi = lo;
+        // The bisection assumes t(f) increasing over the band (true for the PN terms; the leading eccentric term can
+        // break it for large e_0 or far below f_ref_ecc).  Probe the window: t must increase from its first to its last
+        // bin through seven interior bins, all inside [0, T_obs]; a particle that fails has no contiguous window and is
+        // treated as invalid input (Upsilon = 0, include/sc_stat.h).
+        if (jhi > jlo + 1) {
+          double t_prev = tf_direct(c, q, (double)(c.j0 + jlo) / c.T_obs);
+          bool mono = (t_prev >= 0.0);
+          for (int s = 1; s <= 8 && mono; ++s) {
+            const int j = jlo + (int)(((long long)(jhi - 1 - jlo) * s) / 8);
+            const double t = tf_direct(c, q, (double)(c.j0 + j) / c.T_obs);
+            mono = (t >= t_prev) && (t <= c.T_obs);
+            t_prev = t;
+          }
+          if (!mono) { jlo = 0; jhi = 0; }
+        }
       } else {
-        jlo = 0; jhi = c.n_bins;
+        jlo = (c.j0 == 0) ? 1 : 0; jhi = c.n_bins;
       }
     }
     const int a = max(jlo, e_first), b = min(jhi, e_last);

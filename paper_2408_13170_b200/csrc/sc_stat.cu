@@ -448,19 +448,25 @@ int prepare_edges(sc_handle* h, const int32_t* seg_edges, int32_t n_seg, int CH,
   h->edges.swap(e);
   analyse_edges(h, CH);
   h->cached_lg = lg_fine;
-  int rc;
-  if (lg_fine > 0 && (rc = build_pieces(h, CH, lg_fine, st))) { h->cached_chunk = 0; return rc; }
-  if ((rc = grow(h, (void**)&h->d_edges, &h->edge_cap, h->edges.size() * 4))) return rc;
-  if ((rc = grow(h, (void**)&h->d_chunk_k0, &h->k0_cap, (size_t)std::max(h->n_chunks, 1) * 4))) return rc;
-  if ((rc = grow(h, (void**)&h->d_flags, &h->flags_cap, (size_t)std::max(h->n_chunks, 1)))) return rc;
-  if ((rc = grow(h, (void**)&h->d_next_close, &h->nc_cap, (size_t)std::max(h->n_chunks, 1) * 4))) return rc;
-  SC_CUDA(h, cudaMemcpyAsync(h->d_edges, h->edges.data(), h->edges.size() * 4, cudaMemcpyHostToDevice, st));
-  if (h->n_chunks > 0) {
-    SC_CUDA(h, cudaMemcpyAsync(h->d_chunk_k0, h->chunk_k0.data(), (size_t)h->n_chunks * 4, cudaMemcpyHostToDevice, st));
-    SC_CUDA(h, cudaMemcpyAsync(h->d_flags, h->flags.data(), (size_t)h->n_chunks, cudaMemcpyHostToDevice, st));
-    SC_CUDA(h, cudaMemcpyAsync(h->d_next_close, h->next_close.data(), (size_t)h->n_chunks * 4, cudaMemcpyHostToDevice, st));
-  }
-  return SC_OK;
+  // (the cache key is valid only once every table below is on the device: any failure invalidates it)
+  auto upload = [&]() -> int {
+    int rc;
+    if (lg_fine > 0 && (rc = build_pieces(h, CH, lg_fine, st))) return rc;
+    if ((rc = grow(h, (void**)&h->d_edges, &h->edge_cap, h->edges.size() * 4))) return rc;
+    if ((rc = grow(h, (void**)&h->d_chunk_k0, &h->k0_cap, (size_t)std::max(h->n_chunks, 1) * 4))) return rc;
+    if ((rc = grow(h, (void**)&h->d_flags, &h->flags_cap, (size_t)std::max(h->n_chunks, 1)))) return rc;
+    if ((rc = grow(h, (void**)&h->d_next_close, &h->nc_cap, (size_t)std::max(h->n_chunks, 1) * 4))) return rc;
+    SC_CUDA(h, cudaMemcpyAsync(h->d_edges, h->edges.data(), h->edges.size() * 4, cudaMemcpyHostToDevice, st));
+    if (h->n_chunks > 0) {
+      SC_CUDA(h, cudaMemcpyAsync(h->d_chunk_k0, h->chunk_k0.data(), (size_t)h->n_chunks * 4, cudaMemcpyHostToDevice, st));
+      SC_CUDA(h, cudaMemcpyAsync(h->d_flags, h->flags.data(), (size_t)h->n_chunks, cudaMemcpyHostToDevice, st));
+      SC_CUDA(h, cudaMemcpyAsync(h->d_next_close, h->next_close.data(), (size_t)h->n_chunks * 4, cudaMemcpyHostToDevice, st));
+    }
+    return SC_OK;
+  };
+  const int rc = upload();
+  if (rc) { h->cached_chunk = 0; h->cached_lg = 0; h->edges.clear(); }
+  return rc;
 }
 
 int eval_common(sc_handle* h, const double* params, int64_t P, const int32_t* seg_edges, int32_t n_seg,
@@ -563,11 +569,45 @@ int eval_any(sc_handle* h, const double* params, int64_t P, const int32_t* seg_e
       fail(h, rc, "T pass: %s", h->sub->err.c_str());
       return rc;
     }
-    Timed tm(h, st, SC_TIME_STITCH);
-    k_combine3<<<(unsigned)((Pn + 127) / 128), 128, 0, st>>>(segA, segT, (int)Pn, n_seg, four_df, out ? out + pb : nullptr,
-                                                            seg_mode ? out_seg + (size_t)pb * n_seg * 3 : nullptr,
-                                                            out_comp ? out_comp + pb * 3 : nullptr);
-    if ((rc = check_launch(h, "k_combine3"))) return rc;
+    {
+      Timed tm(h, st, SC_TIME_STITCH);
+      k_combine3<<<(unsigned)((Pn + 127) / 128), 128, 0, st>>>(segA, segT, (int)Pn, n_seg, four_df, out ? out + pb : nullptr,
+                                                              seg_mode ? out_seg + (size_t)pb * n_seg * 3 : nullptr,
+                                                              out_comp ? out_comp + pb * 3 : nullptr);
+      if ((rc = check_launch(h, "k_combine3"))) return rc;
+    }
+    // Escalation on three channels (SC_OPT_ESCALATE): both passes ran the FP32-amplitude kernels in segment-table mode
+    // (polynomial sin/cos), so a particle whose COMBINED statistic is below tau carries an error ~ 1e-6 / sqrt(Upsilon):
+    // those are evaluated again by the all-FP64 kernels, both passes, and combined.  This path reads the selected count
+    // back (one 4-byte copy per batch): three-channel evaluation is two passes plus a table pass, not the device-resident loop.
+    const bool f32_path = (h->precision == 1) || (h->precision == 0 && n_seg >= h->f32_min_seg);
+    if (h->escalate && h->precision == 0 && f32_path && !seg_mode && out && !out_comp && Pn <= INT32_MAX / 16) {
+      const size_t P_round = (size_t)((Pn + kBlock - 1) / kBlock * kBlock);
+      if ((rc = grow(h, (void**)&h->d_esc_idx, &h->esc_idx_cap, (size_t)Pn * 4))) return rc;
+      if ((rc = grow(h, (void**)&h->d_esc_count, &h->esc_cnt_cap, 256))) return rc;
+      if ((rc = grow(h, (void**)&h->d_esc_params, &h->esc_par_cap, P_round * 64))) return rc;
+      if ((rc = grow(h, (void**)&h->d_esc_out, &h->esc_out_cap, P_round * 8))) return rc;
+      {
+        Timed tm(h, st, SC_TIME_ESC);
+        k_esc_select<<<1, 1024, 0, st>>>(out + pb, params + pb * 8, (int)Pn, h->esc_tau_poly, h->d_esc_idx, h->d_esc_count, h->d_esc_params);
+      }
+      if ((rc = check_launch(h, "k_esc_select"))) return rc;
+      int n_esc = 0;
+      SC_CUDA(h, cudaMemcpyAsync(&n_esc, h->d_esc_count, 4, cudaMemcpyDeviceToHost, st));
+      SC_CUDA(h, cudaStreamSynchronize(st));
+      if (n_esc > 0) {
+        h->precision = 2; h->sub->precision = 2;
+        rc = eval_common(h, h->d_esc_params, n_esc, seg_edges, n_seg, nullptr, segA, stream, true);
+        if (!rc) rc = eval_common(h->sub, h->d_esc_params, n_esc, seg_edges, n_seg, nullptr, segT, stream, true);
+        h->precision = 0; h->sub->precision = 0;
+        if (rc) return rc;
+        Timed tm(h, st, SC_TIME_ESC);
+        k_combine3<<<(unsigned)((n_esc + 127) / 128), 128, 0, st>>>(segA, segT, n_esc, n_seg, four_df, h->d_esc_out, nullptr, nullptr);
+        if ((rc = check_launch(h, "k_combine3"))) return rc;
+        k_esc_scatter<<<(unsigned)((Pn + 127) / 128), 128, 0, st>>>(h->d_esc_idx, h->d_esc_count, h->d_esc_out, out + pb);
+        if ((rc = check_launch(h, "k_esc_scatter"))) return rc;
+      }
+    }
   }
   return SC_OK;
 }
@@ -955,10 +995,11 @@ int sc_search_run(sc_handle* h, const sc_search_config* sc, double* pos, double*
   const int64_t nb = h->cfg.n_bins;
   // device state owned by this call
   double* buf = nullptr;
-  const size_t n_d = (size_t)P * 8 + (size_t)P * 2 + (size_t)S * 8 * 2 + (size_t)S + 8;
+  const size_t n_stat = (size_t)std::max<int64_t>(P, S);    // statistic per particle; per swarm in the final re-evaluation
+  const size_t n_d = (size_t)P * 8 + (size_t)P + n_stat + (size_t)S * 8 * 2 + (size_t)S + 8;
   SC_CUDA(h, cudaMalloc(&buf, n_d * 8 + (size_t)S * 8));
   double* pbest_pos = buf; double* pbest_val = pbest_pos + (size_t)P * 8; double* stat = pbest_val + P;
-  double* gbest_pos = stat + P; double* cent = gbest_pos + (size_t)S * 8; double* gbest_val = cent + (size_t)S * 8;
+  double* gbest_pos = stat + n_stat; double* cent = gbest_pos + (size_t)S * 8; double* gbest_val = cent + (size_t)S * 8;
   double* eps_d = gbest_val + S;
   long long* cnt_d = (long long*)(eps_d + 8);
   std::vector<double> gv((size_t)S), hst;
@@ -968,11 +1009,13 @@ int sc_search_run(sc_handle* h, const sc_search_config* sc, double* pos, double*
   uint64_t iter_global = 0;
   // ranking precision (sc_search_config): force the FP32-amplitude path without escalation for the whole search
   const int saved_precision = h->precision, saved_escalate = h->escalate;
-  if (sc->ranking_precision) { h->precision = 1; h->escalate = 0; }
+  // (precision mode and escalation of a three-channel handle apply to both of its passes)
+  auto set_mode = [&](int prec, int esc) { h->precision = prec; h->escalate = esc; if (h->sub) { h->sub->precision = prec; h->sub->escalate = esc; } };
+  if (sc->ranking_precision) set_mode(1, 0);
   const bool auto_precision = (h->precision == 0) && h->escalate && !h->sub;
   double win_frac = -1.0;                          // mean window fraction, -1: not measured yet
   unsigned long long ev_bins = 0;
-  auto cleanup = [&](int code) { h->precision = saved_precision; h->escalate = saved_escalate; cudaFree(buf); return code; };
+  auto cleanup = [&](int code) { set_mode(saved_precision, saved_escalate); cudaFree(buf); return code; };
 #define SC_S(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cleanup(fail(h, SC_ERR_CUDA, "%s failed: %s", #call, cudaGetErrorString(e_))); } while (0)
   SC_S(cudaMemsetAsync(gbest_pos, 0, (size_t)S * 8 * 8, st));
 
@@ -1037,9 +1080,18 @@ int sc_search_run(sc_handle* h, const sc_search_config* sc, double* pos, double*
   if (sc->ranking_precision) {
     // the reported bests are re-evaluated at full accuracy (all-FP64 path) at the swarm-best positions
     const int N = sc->n_seg[sc->n_rungs - 1];
-    h->precision = 2;
-    if (sc->adaptive_edges && N > 1) rc = sc_eval_stat_adaptive(h, gbest_pos, S, N, stat, nullptr, nullptr, stream);
-    else rc = eval_any(h, gbest_pos, S, e.data(), N, stat, nullptr, stream, false);
+    set_mode(2, saved_escalate);
+    if (sc->adaptive_edges && N > 1) {
+      // per-particle segments: the edges each best was ranked on (decided in FP64), then the statistic on exactly those
+      // edges by the all-FP64 kernels, swarm by swarm
+      int32_t* ed = nullptr;
+      SC_S(cudaMalloc(&ed, (size_t)S * (N + 1) * 4));
+      rc = sc_eval_stat_adaptive(h, gbest_pos, S, N, stat, ed, nullptr, stream);
+      for (int s = 0; s < S && !rc; ++s)
+        rc = eval_common(h, gbest_pos + (size_t)s * 8, 1, ed + (size_t)s * (N + 1), N, stat + s, nullptr, stream, false);
+      cudaStreamSynchronize(st);
+      cudaFree(ed);
+    } else rc = eval_any(h, gbest_pos, S, e.data(), N, stat, nullptr, stream, false);
     if (rc) return cleanup(rc);
     k_keep_empty<<<1, 128, 0, st>>>(gbest_val, stat, S);
     if ((rc = check_launch(h, "k_keep_empty"))) return cleanup(rc);

@@ -93,6 +93,28 @@ def test_c2_three_channels_sampled(oracle):
     H.close()
 
 
+@pytest.mark.parametrize("N", [8, 16])
+def test_three_channel_escalation_of_ill_conditioned_particles(oracle, N):
+    """SC_OPT_ESCALATE on a three-channel handle: both passes run the FP32-amplitude kernels (segment tables), so a particle
+    whose COMBINED statistic is below tau is re-evaluated by the all-FP64 kernels (both passes) -- c2's population at a
+    coarse rung has such particles; every particle must meet the bar, an escalated one carries the all-FP64 value."""
+    torch, sc, inp, cfgd, cfg, S3, d3, th, kappa, h3, H = _setup(oracle, 2, 256, 17.0, 905)
+    e = sy.edges(cfgd["n_bins"], N)
+    par = _dev(torch, inp["particles"])
+    ref = oracle.eval_stat3(cfg, d3, S3, inp["particles"], e)
+    auto = H.eval_stat(par, e).cpu().numpy()
+    H.set_option(sc.SC_OPT_ESCALATE, 0)
+    plain = H.eval_stat(par, e).cpu().numpy()
+    H.set_option(sc.SC_OPT_PRECISION, 2)
+    f64 = H.eval_stat(par, e).cpu().numpy()
+    H.close()
+    esc = (plain > 0) & (plain < 6.0)
+    assert esc.sum() > 0                                           # the case is exercised
+    assert rel_err(auto[esc], f64[esc]).max() <= 1e-11 and np.array_equal(auto[~esc], plain[~esc])
+    ok = ref > 0
+    assert rel_err(auto[ok], ref[ok]).max() <= TOL
+
+
 def test_three_channel_restrictions_and_search(oracle):
     torch, sc, inp, cfgd, cfg, S3, d3, th, kappa, h3, H = _setup(oracle, 1, None, 20.0, 904)
     par = _dev(torch, inp["particles"])
