@@ -37,7 +37,8 @@ NOMINAL_DFMA = 148 * 64 * 1.965e9   # 148 SMs x 64 FP64 lanes x max SM clock (B2
 # 26 packed FFMA2/FMUL2/FADD2 (2 slots each) + 3 scalar per bin PAIR; peak = 148 SMs x 128 FP32 lanes x max SM clock.
 FP32_SLOTS_PER_BIN = (26 * 2 + 3) / 2.0
 NOMINAL_FP32_SLOTS = 148 * 128 * 1.965e9
-DENSE_PROFILE = os.path.join(ROOT, "profiles", "r01h_k_dense2_full.md")
+NOMINAL_FP32_TFLOPS = 2.0 * NOMINAL_FP32_SLOTS / 1e12   # 74.5 TFLOP/s: unit counts x clock of B200_PROFILING.md (no measured FP32 peak)
+DENSE_PROFILE = os.path.join(ROOT, "profiles", "r02_k_dense2_full.md")   # ncu --set full of the c3 launch (static figure, see roofline.traffic_source)
 
 
 def dram_traffic_from_profile():
@@ -398,6 +399,55 @@ def run_ours(args, rank, local_rank, world):
             "ms_per_eval": a.elapsed_time(b) / 3, "particle_bin_per_s": float(P) * nb / (a.elapsed_time(b) / 3 * 1e-3),
             "kernel_ms_per_eval": {k: v[0] / 3 for k, v in tma.items() if v[1]}}
 
+    # ---- extras: the all-FP64 kernel (every rung with N < 8: the paper's final N = 1 rung), the
+    # tensor-core flavour of the FP32-amplitude kernel, and the three-channel statistic (A, E, T)
+    def timed_evals(fn, reps=3):
+        fn(); torch.cuda.synchronize(); H.timing()
+        a_, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a_.record()
+        for _ in range(reps):
+            fn()
+        b_.record(); torch.cuda.synchronize()
+        return a_.elapsed_time(b_) / reps, {k: v[0] / reps for k, v in H.timing().items() if v[1]}
+
+    if not args.no_extras and not ad_N and rank == 0:
+        e1 = np.array([0, nb], dtype=np.int32)
+        ms1, k1 = timed_evals(lambda: H.eval_stat(state["pos"], e1, out=stat))
+        ev1 = H.counters()[0]
+        extras["coherent_N1"] = {"what": "sc_eval_stat at N = 1 (all-FP64 path, k_dense<false>), same population",
+                                 "ms_per_eval": ms1, "kernel_ms_per_eval": k1, "evaluated_particle_bin_per_s": ev1 / (ms1 * 1e-3),
+                                 "fp64_model_frac": (2.0 * C_DP * ev1 / (k1.get("dense", ms1) * 1e-3) / (2.0 * NOMINAL_DFMA))}
+        try:
+            H.set_option(sc.SC_OPT_TENSOR_CORES, 1)
+            mst, kt = timed_evals(lambda: H.eval_stat(state["pos"], e, out=stat))
+            extras["tensor_core_flavour"] = {
+                "what": "SC_OPT_TENSOR_CORES = 1: k_dense2_tc (amplitude x data factor as a split-TF32 contraction on tcgen05, "
+                        "TMEM accumulators), same evaluation; not the default (slower than k_dense2, DESIGN.md 6)",
+                "ms_per_eval": mst, "kernel_ms_per_eval": kt}
+        except sc.SCError as ex:
+            extras["tensor_core_flavour"] = {"skipped": str(ex)[:200]}
+        H.set_option(sc.SC_OPT_TENSOR_CORES, 0)
+        try:
+            cfg3 = dict(cfg, n_channels=3)
+            S_T = t(sy.psd_T(sy.freqs(cfg3)))
+            nT = t(sy.draw_noise(sy.MASTER_SEED + 7 + 100 * cid if hasattr(sy, "MASTER_SEED") else 240813177 + 100 * cid,
+                                 sy.psd_T(sy.freqs(cfg3)), inp["df"]))
+            H3 = sc.Handle(cfg3, torch.view_as_real(dA).contiguous(), torch.view_as_real(dE).contiguous(), S_A, S_E,
+                           dT=torch.view_as_real(nT).contiguous(), S_T=S_T)
+            H3.set_option(sc.SC_OPT_TC_MAX_S, int(np.ceil(inp["hi"][2])))
+            H3.eval_stat(state["pos"], e, out=stat); torch.cuda.synchronize()
+            a_, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a_.record()
+            for _ in range(2):
+                H3.eval_stat(state["pos"], e, out=stat)
+            b_.record(); torch.cuda.synchronize()
+            extras["three_channels"] = {"what": "sc_eval_stat on an (A, E, T) handle (T noise only), same population and edges: "
+                                                "two passes + segment-table combine", "ms_per_eval": a_.elapsed_time(b_) / 2}
+            H3.close()
+            del H3, nT, S_T
+        except (RuntimeError, sc.SCError, KeyError, AttributeError) as ex:
+            extras["three_channels"] = {"skipped": str(ex)[:200]}
+
     # ---- extras: the second workload (Fig. 3): many data streams x one template, HBM-bound
     if not args.no_extras and not ad_N and rank == 0:
         D = 256
@@ -465,15 +515,17 @@ def run_ours(args, rank, local_rank, world):
         H.timing()
 
     # ---- reduce over ranks: max time, summed work
-    ms_max, units = ms_total, float(P) * nb * args.steps
+    # work = EVALUATED (particle, bin) pairs: bins inside the particle's time window and [e_0, e_N) (the count of the last
+    # evaluation; the swarm moves a little from step to step).  The nominal P x n_bins rate is reported beside it.
+    ms_max, units, units_nominal = ms_total, float(eval_bins) * args.steps, float(P) * nb * args.steps
     e2e_ms_max = e2e["ms"] if e2e else 0.0
     if world > 1:
         v = torch.tensor([ms_total, e2e_ms_max], dtype=torch.float64, device=dev)
         dist.all_reduce(v, op=dist.ReduceOp.MAX)
         ms_max, e2e_ms_max = v[0].item(), v[1].item()
-        u = torch.tensor([units], dtype=torch.float64, device=dev)
+        u = torch.tensor([units, units_nominal], dtype=torch.float64, device=dev)
         dist.all_reduce(u, op=dist.ReduceOp.SUM)
-        units = u.item()
+        units, units_nominal = u[0].item(), u[1].item()
 
     if rank == 0:
         value = units / (ms_max * 1e-3)
@@ -492,21 +544,34 @@ def run_ours(args, rank, local_rank, world):
         ach = 2.0 * C_DP * eval_bins_launch / (dense_avg * 1e-3) / 1e12 if dense_avg > 0 else None
         peak = 2.0 * (dfma or NOMINAL_DFMA) / 1e12
         pbs = eval_bins_launch / (dense_avg * 1e-3) if dense_avg > 0 else None
-        roof = {"bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
-                "frac": (ach / peak) if ach else None, "traffic": dram_traffic_from_profile(),
-                "traffic_source": "profiles/r01h_k_dense2_full.md (ncu --set full, one launch, same command)",
+        # Two fractions (both kept): (1) frac = frac_pipe_fma -- the pipe the kernel as built runs on: FP32 lane slots it
+        # executes per evaluated bin (SASS of the pair loop: 26 packed x 2 + 3 scalar per bin pair) x evaluated bins/s
+        # against 148 SM x 128 lanes x max clock; ncu's sm__pipe_fma_cycles_active of the same launch is in profiles/.
+        # (2) frac_model -- the contract's fixed op model (24 FP64 instructions per evaluated bin)
+        # against the FP64 rate measured in this run; the kernel does NOT execute that FP64 work (3 DADD per bin), so
+        # this one is a speed-up over the model, not a utilisation, and may exceed 1.
+        slots = (pbs * FP32_SLOTS_PER_BIN) if pbs else None
+        is_c3_shared = (cid == 3 and not ad_N and not args.particles)
+        roof = {"bound": "alu", "achieved": (2.0 * slots / 1e12) if slots else None, "peak": NOMINAL_FP32_TFLOPS, "unit": "TFLOP/s",
+                "frac": (slots / NOMINAL_FP32_SLOTS) if slots else None,
+                "frac_pipe_fma": (slots / NOMINAL_FP32_SLOTS) if slots else None,
+                "frac_model": (ach / peak) if ach else None,
+                "traffic": dram_traffic_from_profile() if is_c3_shared else None,
+                "traffic_source": ("static: profiles/r02_k_dense2_full.md (ncu --set full of one k_dense2 launch of this c3 command), "
+                                   "not measured in this run") if is_c3_shared else None,
                 "kernel": "k_dense2_ad<2,MERGE>" if ad_N else "k_dense2<false,2,MERGE>", "kernel_ms_per_launch": dense_avg,
-                "own_mix": {"what": "FP32 pipe of the kernel as built (packed FFMA2 loop): lane slots per evaluated "
-                                    "particle-bin x evaluated particle-bins/s / (148 SM x 128 lanes x 1.965 GHz)",
-                            "fp32_slots_per_bin": FP32_SLOTS_PER_BIN,
-                            "frac": (pbs * FP32_SLOTS_PER_BIN / NOMINAL_FP32_SLOTS) if pbs else None},
-                "model": f"{C_DP} FP64 instr (= {2 * C_DP} flop) per evaluated particle-bin, SURVEY.md 8(d)",
-                "peak_source": ("measured in this run by sc_measure_fp64_peak (DFMA/s x 2)" if dfma else
-                                "nominal 148 SM x 64 lanes x 1.965 GHz x 2"),
-                "peak_nominal_max_clock": 2.0 * NOMINAL_DFMA / 1e12,
+                "peak_source": "FP32 pipe: 148 SM x 128 lanes x 1.965 GHz x 2 flop (unit counts and clocks of B200_PROFILING.md; "
+                               "MEASURED_PEAKS.json has no FP32 figure)",
+                "pipe_fma": {"fp32_lane_slots_per_evaluated_bin": FP32_SLOTS_PER_BIN, "lane_slots_per_s": slots,
+                             "peak_lane_slots_per_s": NOMINAL_FP32_SLOTS},
+                "model": {"what": f"{C_DP} FP64 instr (= {2 * C_DP} flop) per evaluated particle-bin, SURVEY.md 8(d)",
+                          "achieved_tflops": ach, "peak_tflops": peak,
+                          "peak_source": ("measured in this run by sc_measure_fp64_peak (DFMA/s x 2)" if dfma else
+                                          "nominal 148 SM x 64 lanes x 1.965 GHz x 2"),
+                          "peak_nominal_max_clock": 2.0 * NOMINAL_DFMA / 1e12,
+                          "frac_vs_nominal_max_clock": (ach / (2.0 * NOMINAL_DFMA / 1e12)) if ach else None},
                 "evaluated_particle_bins_per_launch": eval_bins_launch, "launches_per_evaluation": dense_per_eval,
-                "evaluated_pb_per_s": pbs,
-                "frac_vs_nominal_max_clock": (ach / (2.0 * NOMINAL_DFMA / 1e12)) if ach else None}
+                "evaluated_pb_per_s_dense_kernel": pbs}
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f64 phase + f32 amplitude/accumulate-flush-to-f64", "data": "synthetic",
@@ -514,6 +579,9 @@ def run_ours(args, rank, local_rank, world):
                            "(256 MiB write); per-step node tables + fragments (~1 GB) exceed L2 anyway",
                            "pso": {k: hp[k] for k in ("omega", "phi_p", "phi_g")}, "n_swarms": n_swarms,
                            "parallelism": f"independent tiles x{world}" if world > 1 else "1 GPU"},
+                "value_counts": "evaluated (particle, bin) pairs (inside the time windows and [e_0, e_N))",
+                "nominal_particle_bin_per_s": units_nominal / (ms_max * 1e-3),
+                "evaluated_fraction": units / units_nominal if units_nominal else None,
                 "swarm_iters_per_s": world * 1e3 / ms_per_step,
                 "kernel_ms_per_step": {k: v[0] / args.steps for k, v in timing.items() if v[1]},
                 "wall_s_timed_region": t_wall,
@@ -525,7 +593,7 @@ def run_ours(args, rank, local_rank, world):
         if extras:
             line["extras"] = extras
         if e2e:
-            line["e2e"] = {"value": world * float(P) * nb / (e2e_ms_max * 1e-3), "unit": UNIT,
+            line["e2e"] = {"value": units / args.steps / (e2e_ms_max * 1e-3), "unit": UNIT,
                            "h2d_bytes_per_step": e2e["h2d"], "d2h_bytes_per_step": e2e["d2h"],
                            "ms_per_step": e2e_ms_max}
         if not args.no_cpu_baseline and world == 1:
@@ -533,6 +601,7 @@ def run_ours(args, rank, local_rank, world):
             cores = orc.num_threads()
             n_p, k_cpu = 4 * max(8, min(32, cores)), 3          # ~10-20 s of CPU work on the box's cores
             sec, cores = oracle_sample_run(sy.config_inputs(cid, P=n_p), N, n_p, k_cpu, 0)
+            # (the oracle evaluates every bin of the band and masks those outside the window: its rate counts all of them)
             line["cpu_baseline"] = {"value": n_p * nb / sec, "unit": UNIT, "cores": cores, "kind": "oracle",
                                     "sample": f"{n_p} particles x all {nb} bins per step, {k_cpu} steps (statistic + PSO), "
                                               f"{sec * k_cpu:.1f} s wall"}
