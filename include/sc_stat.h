@@ -22,7 +22,10 @@
  *
  * Particle parameter row (D3, Q3), FP64, row-major [n_particles][8]:
  *    theta = ( M_c [Msun, detector frame], eta, t_c [s from data start], lambda, beta, iota, psi, e_0 ).
- * Per-particle invalid input (non-finite, eta outside (0, 0.25], M_c <= 0) gives Upsilon = 0, never NaN.
+ * Per-particle invalid input (non-finite, eta outside (0, 0.25], M_c <= 0) gives Upsilon = 0, never NaN.  So does a
+ * particle whose t(f) is not increasing across its time window (window_mode = 1: the window is found by bisection and
+ * verified at nine probe bins; the leading eccentric term can break monotonicity for large e_0): it has no contiguous
+ * window.  The bin f = 0 (j0 = 0) carries no template.
  */
 #ifndef SC_STAT_H
 #define SC_STAT_H
@@ -74,6 +77,9 @@ enum {
                                 driver re-evaluate, by the all-FP64 path, every particle whose FP32-path statistic came
                                 out as 0 < Upsilon < tau (the FP32 path's relative error grows like 1/sqrt(Upsilon));
                                 selection, compaction and scatter happen on the device, no host synchronisation.
+                                Three-channel handles (sc_init_data3): the selection is made on the COMBINED statistic,
+                                both passes re-run all-FP64 for the compacted set (tau of the polynomial flavour); there
+                                the selected count is read back (one 4-byte synchronising copy per particle batch).
                                 0 = off.  Not applied by sc_eval_segments / _components / _loglike / _adaptive.        */
   SC_OPT_ESC_TAU_POLY_X1000 = 10,  /* tau x 1000 for the polynomial sin/cos flavour (default 6000)                    */
   SC_OPT_ESC_TAU_MUFU_X1000 = 11,  /* tau x 1000 for the hardware sin/cos flavour (default 16000)                     */
@@ -246,7 +252,8 @@ typedef struct {
                                            escalation).  1: the swarm only has to be RANKED -- all rungs run the FP32-amplitude
                                            path without escalation (relative error <= 1.6e-6/sqrt(Upsilon): < 2e-7 for anything
                                            near the Upsilon_1 >= 100 threshold), about 3x faster on the N < 8 rungs; the
-                                           reported best_val are re-evaluated by the all-FP64 path at the end.            */
+                                           reported best_val are re-evaluated by the all-FP64 path at the end (with per-particle
+                                           segments: on the very edges each best was ranked on).                          */
   int32_t reserved_;                    /* 0 */
 } sc_search_config;
 /* For every rung N: { Upsilon_N(pos) for all particles; sc_pso_step_labeled } until every non-empty swarm satisfies
