@@ -78,7 +78,7 @@ enum {
                                 out as 0 < Upsilon < tau (the FP32 path's relative error grows like 1/sqrt(Upsilon));
                                 selection, compaction and scatter happen on the device, no host synchronisation.
                                 Three-channel handles (sc_init_data3): the selection is made on the COMBINED statistic,
-                                both passes re-run all-FP64 for the compacted set (tau of the polynomial flavour); there
+                                both passes re-run all-FP64 for the compacted set; there
                                 the selected count is read back (one 4-byte synchronising copy per particle batch).
                                 0 = off.  Not applied by sc_eval_segments / _components / _loglike / _adaptive.        */
   SC_OPT_ESC_TAU_POLY_X1000 = 10,  /* tau x 1000 for the polynomial sin/cos flavour (default 6000)                    */

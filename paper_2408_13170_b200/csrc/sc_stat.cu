@@ -281,7 +281,9 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
   // sin/cos flavour of the FP32 path: hardware MUFU (gain-calibrated) from mufu_min_seg segments up, else polynomial
   const int sincos = (h->sincos_mode == 0) ? (n_seg >= h->mufu_min_seg ? 2 : 0) : (h->sincos_mode == 2 ? 2 : 0);
   const double h0 = pow(dc.f_amp_ref, -7.0 / 6.0);
-  const double sz = h->s0 * h0 / four_df, ss = h->s0 * h->s0 * h0 * h0 / four_df;
+  // segment tables are in definition units; the hardware sin/cos gain g (g^2 = mufu_gain2) multiplies every z_k of the FP32 path
+  const double sz = h->s0 * h0 / four_df / ((sizeof(R) == 4 && sincos == 2) ? sqrt(h->mufu_gain2) : 1.0),
+               ss = h->s0 * h->s0 * h0 * h0 / four_df;
 
   // particle blocks launched per kernel: all of them, or (escalation pass) the caller's estimate -- the kernels stride
   const int pblocks = esc_count ? std::max(1, std::min(esc_blocks, P_pad / kBlock)) : P_pad / kBlock;
@@ -352,6 +354,9 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
           else if (merge) k_dense2_tc<false, 0, true><<<grid_tc, tc::kThreads, tc::kSmemBytes, st>>>(dc, a, Dp, Tg);
           else k_dense2_tc<false, 0><<<grid_tc, tc::kThreads, tc::kSmemBytes, st>>>(dc, a, Dp, Tg);
         }
+        else if (seg_mode && sincos == 2 && merge) k_dense2<true, 2, true><<<grid, kBlock, 0, st>>>(dc, a, Dp);
+        else if (seg_mode && sincos == 2) k_dense2<true, 2><<<grid, kBlock, 0, st>>>(dc, a, Dp);
+        else if (seg_mode && merge) k_dense2<true, 0, true><<<grid, kBlock, 0, st>>>(dc, a, Dp);
         else if (seg_mode) k_dense2<true, 0><<<grid, kBlock, 0, st>>>(dc, a, Dp);
         else if (sincos == 2 && merge) k_dense2<false, 2, true><<<grid, kBlock, 0, st>>>(dc, a, Dp);
         else if (sincos == 2) k_dense2<false, 2><<<grid, kBlock, 0, st>>>(dc, a, Dp);
@@ -577,7 +582,7 @@ int eval_any(sc_handle* h, const double* params, int64_t P, const int32_t* seg_e
       if ((rc = check_launch(h, "k_combine3"))) return rc;
     }
     // Escalation on three channels (SC_OPT_ESCALATE): both passes ran the FP32-amplitude kernels in segment-table mode
-    // (polynomial sin/cos), so a particle whose COMBINED statistic is below tau carries an error ~ 1e-6 / sqrt(Upsilon):
+    // (same sin/cos flavour rule as sc_eval_stat), so a particle whose COMBINED statistic is below tau carries an error ~ 1e-6 / sqrt(Upsilon):
     // those are evaluated again by the all-FP64 kernels, both passes, and combined.  This path reads the selected count
     // back (one 4-byte copy per batch): three-channel evaluation is two passes plus a table pass, not the device-resident loop.
     const bool f32_path = (h->precision == 1) || (h->precision == 0 && n_seg >= h->f32_min_seg);
@@ -589,7 +594,8 @@ int eval_any(sc_handle* h, const double* params, int64_t P, const int32_t* seg_e
       if ((rc = grow(h, (void**)&h->d_esc_out, &h->esc_out_cap, P_round * 8))) return rc;
       {
         Timed tm(h, st, SC_TIME_ESC);
-        k_esc_select<<<1, 1024, 0, st>>>(out + pb, params + pb * 8, (int)Pn, h->esc_tau_poly, h->d_esc_idx, h->d_esc_count, h->d_esc_params);
+        const bool mufu3 = (h->sincos_mode == 0) ? (n_seg >= h->mufu_min_seg) : (h->sincos_mode == 2);
+        k_esc_select<<<1, 1024, 0, st>>>(out + pb, params + pb * 8, (int)Pn, mufu3 ? h->esc_tau_mufu : h->esc_tau_poly, h->d_esc_idx, h->d_esc_count, h->d_esc_params);
       }
       if ((rc = check_launch(h, "k_esc_select"))) return rc;
       int n_esc = 0;
