@@ -442,7 +442,11 @@ def run_ours(args, rank, local_rank, world):
                 H3.eval_stat(state["pos"], e, out=stat)
             b_.record(); torch.cuda.synchronize()
             extras["three_channels"] = {"what": "sc_eval_stat on an (A, E, T) handle (T noise only), same population and edges: "
-                                                "two passes + segment-table combine", "ms_per_eval": a_.elapsed_time(b_) / 2}
+                                                "one pass through the fused kernel k_dense3 (SC_OPT_FUSED_AET = 1)", "ms_per_eval": a_.elapsed_time(b_) / 2}
+            H3.set_option(sc.SC_OPT_FUSED_AET, 0)
+            H3.eval_stat(state["pos"], e, out=stat); torch.cuda.synchronize()
+            a_.record(); H3.eval_stat(state["pos"], e, out=stat); b_.record(); torch.cuda.synchronize()
+            extras["three_channels"]["ms_per_eval_two_passes"] = a_.elapsed_time(b_)
             H3.close()
             del H3, nT, S_T
         except (RuntimeError, sc.SCError, KeyError, AttributeError) as ex:

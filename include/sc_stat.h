@@ -83,6 +83,10 @@ enum {
                                 0 = off.  Not applied by sc_eval_segments / _components / _loglike / _adaptive.        */
   SC_OPT_ESC_TAU_POLY_X1000 = 10,  /* tau x 1000 for the polynomial sin/cos flavour (default 6000)                    */
   SC_OPT_ESC_TAU_MUFU_X1000 = 11,  /* tau x 1000 for the hardware sin/cos flavour (default 16000)                     */
+  SC_OPT_FUSED_AET = 14,     /* three-channel handles (sc_init_data3).  1 (default): the FP32-amplitude path evaluates A, E and T in
+                                ONE pass (k_dense3: three channels in the pair loop).  0: two passes through the two-channel
+                                kernels, (A, E) and (T, nothing), with per-segment tables combined afterwards.  The all-FP64
+                                modes (n_seg < SC_OPT_F32_MIN_SEG, SC_OPT_PRECISION = 2, the escalation pass) always take two. */
   SC_OPT_TENSOR_CORES = 13,  /* 0 (default): the CUDA-core kernel k_dense2 (Horner cubics per bin).  1: the FP32-amplitude path
                                 forms the amplitude x data factor of every bin as a split-TF32 contraction on the tensor cores
                                 (tcgen05, k_dense2_tc; node spacings >= 128 bins; chunks of 8192 bins).  Same definition, same

@@ -60,6 +60,7 @@ struct DenseArgs {
   // k_dense2 only: pieces = fine sub-intervals cut at the segment edges, with the moments of the sigma weights
   const int* piece_first;      // [n_sub_launched + 1] first piece of each launched fine sub-interval
   const ulonglong2* moments;   // [n_pieces][4] = 8 packed (A, E) pairs: sum_j g_a(j) s_j^m, m = 0..6, pad
+  const ulonglong2* momentsT;  // k_dense3 only: the same for (T, 0)
   double merge_lim;            // k_dense2<.., MERGE>: a coarse interval every lane crosses in less signal time than this
                                // (as a slope difference, turns per bin) is set up once for its four fine sub-intervals
   // k_dense only: FP64 moments of the sigma weights per piece, [n_pieces][7] (A, E) pairs, or nullptr (per-bin sigma)

@@ -171,10 +171,10 @@ __global__ void k_particle_consts(DevCfg c, const double* __restrict__ params, i
 // One thread per (node, particle), particle fastest -> coalesced [node][particle] tables; a CTA takes 128 particles and
 // a group of kNodesPerCta consecutive nodes (one CTA per node is launch-bound when most of the table is out of reach).
 constexpr int kNodesPerCta = 16;
-template <typename R, bool ESC = false>
+template <typename R, bool ESC = false, int NA = 4 /* amplitude fields per node: 4 = (A, E) or (T, 0); 6 = (A, E, T) */>
 __global__ void k_nodes(DevCfg c, const double* __restrict__ pc, const int* __restrict__ jlo, const int* __restrict__ jhi,
                         int P_pad, int* __restrict__ node_n, double* __restrict__ node_frac,
-                        R* __restrict__ node_amp /* [node][4][P_pad] */, const int* __restrict__ esc_count = nullptr,
+                        R* __restrict__ node_amp /* [node][NA][P_pad] */, const int* __restrict__ esc_count = nullptr,
                         int esc_pb = 0, int skip_unreached = 0) {
   const int i_first = blockIdx.x * kNodesPerCta;            // nodes i_first .. i_last-1  <->  node index i - kNodeOff
   const int i_last = min(i_first + kNodesPerCta, c.n_nodes);
@@ -204,8 +204,9 @@ __global__ void k_nodes(DevCfg c, const double* __restrict__ pc, const int* __re
         const size_t at = (size_t)i * P_pad + p;
         node_n[at] = o.n_turns;
         node_frac[at] = o.frac;
-        R* a = node_amp + (size_t)i * 4 * P_pad + p;
+        R* a = node_amp + (size_t)i * NA * P_pad + p;
         a[0] = (R)o.Ar; a[(size_t)P_pad] = (R)o.Ai; a[2 * (size_t)P_pad] = (R)o.Er; a[3 * (size_t)P_pad] = (R)o.Ei;
+        if (NA == 6) { a[4 * (size_t)P_pad] = (R)o.Tr; a[5 * (size_t)P_pad] = (R)o.Ti; }
       }
     }
     if (!ESC) return;

@@ -28,7 +28,8 @@ struct DevCfg {
   double f_amp_ref;             // amplitude normalisation: A(f) = (f / f_amp_ref)^(-7/6)
   int log2_stride, stride;      // coarse node spacing in bins (power of two, >= 4)
   int n_nodes;                  // nodes i = -kNodeOff .. n_intervals + 3
-  int chan_set;                 // 0: the node amplitudes are (A, E); 1: (T, 0) -- the T pass of a three-channel handle
+  int chan_set;                 // 0: the node amplitudes are (A, E); 1: (T, 0) -- the T pass of a three-channel handle;
+                                // 2: (A, E, T) -- the fused three-channel kernel (k_dense3)
 };
 // Each coarse interval is cut into 4 fine sub-intervals (stride/4 bins) on which the amplitudes are local cubics.
 constexpr int kNodeOff = 2;     // the quintic phase stencil reaches 2 nodes to the left, 3 to the right
@@ -109,6 +110,7 @@ struct NodeOut {
   int n_turns;        // integer part of Phi
   double frac;        // fractional part, |frac| <= 0.5
   double Ar, Ai, Er, Ei;
+  double Tr, Ti;      // T = (X + Y + Z)/sqrt(3) (chan_set = 2 only)
 };
 
 
@@ -156,6 +158,7 @@ __device__ __forceinline__ void newtonian_turns(double piM_over_T, double n, dou
 
 __device__ NodeOut eval_node(const DevCfg& c, const Particle& q, long long jglob /* j0 + bin position */) {
   NodeOut o;
+  o.Tr = 0.0; o.Ti = 0.0;
   const double n = (double)jglob;
   const double f = n * c.inv_T;
   // --- O2 phase in turns.  The 2 pi f t_c term reaches ~5e6 turns: take its fractional part exactly,
@@ -250,6 +253,11 @@ __device__ NodeOut eval_node(const DevCfg& c, const Particle& q, long long jglob
     o.Ai = (XYZ[0][1] + XYZ[1][1] + XYZ[2][1]) * s3;
     o.Er = 0.0; o.Ei = 0.0;
     return o;
+  }
+  if (c.chan_set == 2) {
+    const double s3 = 0.5773502691896258 * amp;
+    o.Tr = (XYZ[0][0] + XYZ[1][0] + XYZ[2][0]) * s3;
+    o.Ti = (XYZ[0][1] + XYZ[1][1] + XYZ[2][1]) * s3;
   }
   o.Ar = (XYZ[2][0] - XYZ[0][0]) * s2;
   o.Ai = (XYZ[2][1] - XYZ[0][1]) * s2;

@@ -33,6 +33,7 @@ using namespace sc;
 #include "sc_kernels_dense64.cuh"
 #include "sc_kernels_dense32.cuh"
 #include "sc_kernels_dense32tc.cuh"
+#include "sc_kernels_dense32x3.cuh"
 #include "sc_kernels_adaptive.cuh"
 #include "sc_kernels_stitch.cuh"
 #include "sc_kernels_search.cuh"
@@ -60,6 +61,7 @@ struct EdgeCache {
   int* d_piece_first = nullptr; int* d_piece_lo = nullptr; int* d_piece_hi = nullptr; float2* d_moments = nullptr;
   size_t pf_cap = 0, plo_cap = 0, phi_cap = 0, mom_cap = 0;
   double2* d_moments64 = nullptr; size_t mom64_cap = 0;   // FP64 moments per piece (all-FP64 chunking only)
+  float2* d_momentsT = nullptr; size_t momT_cap = 0;      // moments of the T weights per piece (fused three-channel kernel)
 };
 
 struct sc_handle : EdgeCache {
@@ -102,6 +104,9 @@ struct sc_handle : EdgeCache {
   // three-channel handles (A, E, T): the T channel lives in a second handle whose first slot carries T (chan_set = 1)
   // and whose second slot is empty; the per-segment sums of both are added before |z|^2/sigma is formed
   sc_handle* sub = nullptr; double* d_seg3 = nullptr; size_t seg3_cap = 0;
+  // fused tables of the one-pass three-channel kernel k_dense3 (built by sc_init_data3): data records (wA, wE, wT) per bin
+  // pair, sigma weights per bin pair, and the T weights in FP64 for the piece moments; SC_OPT_FUSED_AET
+  float4* D3 = nullptr; float4* Gp3 = nullptr; double2* GT64 = nullptr; int use_fused3 = 1;
   // optional per-kernel-class device timing (SC_OPT_PROFILE): event pairs recorded around each launch
   bool profile = false;
   struct Ev { cudaEvent_t a, b; int cls; };
@@ -226,7 +231,7 @@ void analyse_edges(sc_handle* h, int CH) {
 
 template <typename R>
 int run_batches(sc_handle* h, const double* params, int64_t P, double* out, double* out_seg, double* out_comp,
-                cudaStream_t st, bool seg_mode, const int* esc_count = nullptr, int esc_blocks = 0) {
+                cudaStream_t st, bool seg_mode, const int* esc_count = nullptr, int esc_blocks = 0, bool fused3 = false) {
   // esc_count != nullptr: the escalation pass -- P is an upper bound, the number of particles sits on the device;
   // its launches are timed as SC_TIME_ESC and do not count evaluated bins twice
   const int cls_nodes = esc_count ? SC_TIME_ESC : SC_TIME_NODES, cls_dense = esc_count ? SC_TIME_ESC : SC_TIME_DENSE,
@@ -234,11 +239,13 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
   const int n_seg = (int)h->edges.size() - 1;
   DevCfg dc = h->dc;
   apply_stride(dc, sizeof(R) == 4 ? h->lg_f32 : h->lg_f64);
+  if (fused3) dc.chan_set = 2;                    // node amplitudes (A, E, T)
+  const int NA = fused3 ? 6 : 4;                  // amplitude fields per node
   const int n_nodes = dc.n_nodes;
   const int n_chunks = h->n_chunks;
   // per-particle scratch bytes
   const size_t per_p = 2 * ((size_t)kPcFields * 8 + 8) /* constants, jlo, jhi: unsorted + sorted */ + 16 /* sort keys, map */
-                       + (size_t)n_nodes * (4 + 8 + 4 * sizeof(R)) + (size_t)std::max(n_chunks, 1) * kFragFields * 8;
+                       + (size_t)n_nodes * (4 + 8 + NA * sizeof(R)) + (size_t)std::max(n_chunks, 1) * kFragFields * 8;
   int64_t Pb_max = (int64_t)(h->scratch_cap / per_p) / kBlock * kBlock;
   if (Pb_max < kBlock) Pb_max = kBlock;
   const int64_t P_round = (P + kBlock - 1) / kBlock * kBlock;
@@ -253,7 +260,7 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
   int* jhi = (int*)take((size_t)4 * P_pad);
   int* node_n = (int*)take((size_t)n_nodes * 4 * P_pad);
   double* node_frac = (double*)take((size_t)n_nodes * 8 * P_pad);
-  R* node_amp = (R*)take((size_t)n_nodes * 4 * sizeof(R) * P_pad);
+  R* node_amp = (R*)take((size_t)n_nodes * NA * sizeof(R) * P_pad);
   double* frag = (double*)take((size_t)std::max(n_chunks, 1) * kFragFields * 8 * P_pad);
   // window sort (see k_gather_sorted): not in the segment-table mode (rows are addressed by particle).  In the escalation
   // pass the count sits on the device: all P_pad slots are sorted, the unused ones to the end -- only below 4096 segments
@@ -288,7 +295,7 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
   // particle blocks launched per kernel: all of them, or (escalation pass) the caller's estimate -- the kernels stride
   const int pblocks = esc_count ? std::max(1, std::min(esc_blocks, P_pad / kBlock)) : P_pad / kBlock;
   // tensor-core flavour of the FP32-amplitude kernel: fine sub-intervals of at least one 32-bin tile
-  const bool use_tc = sizeof(R) == 4 && h->cached_chunk == tc::kChunk && n_chunks > 0;
+  const bool use_tc = sizeof(R) == 4 && h->cached_chunk == tc::kChunk && n_chunks > 0 && !fused3;
   if (use_tc && h->tc_img_lg != dc.log2_stride) {
     const long long n_tiles = (long long)((dc.n_bins + tc::kChunk - 1) / tc::kChunk) * (tc::kChunk / tc::kTileBins);
     if ((rc = grow(h, (void**)&h->d_tc_img, &h->tc_img_cap, (size_t)n_tiles * tc::kTileBytes))) return rc;
@@ -324,7 +331,8 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
     }
     {
       Timed tm(h, st, cls_nodes);
-      if (esc_count) k_nodes<R, true><<<dim3((n_nodes + kNodesPerCta - 1) / kNodesPerCta, pblocks), 128, 0, st>>>(dc, pc, jlo, jhi, P_pad, node_n, node_frac, node_amp, esc_count, (int)pb, 1);
+      if (fused3) k_nodes<R, false, 6><<<dim3((n_nodes + kNodesPerCta - 1) / kNodesPerCta, pblocks), 128, 0, st>>>(dc, pc, jlo, jhi, P_pad, node_n, node_frac, node_amp, nullptr, 0, 1);
+      else if (esc_count) k_nodes<R, true><<<dim3((n_nodes + kNodesPerCta - 1) / kNodesPerCta, pblocks), 128, 0, st>>>(dc, pc, jlo, jhi, P_pad, node_n, node_frac, node_amp, esc_count, (int)pb, 1);
       else k_nodes<R, false><<<dim3((n_nodes + kNodesPerCta - 1) / kNodesPerCta, pblocks), 128, 0, st>>>(dc, pc, jlo, jhi, P_pad, node_n, node_frac, node_amp, nullptr, 0, 1);
     }
     if ((rc = check_launch(h, "k_nodes"))) return rc;
@@ -335,6 +343,7 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
     a.frag = frag; a.out_seg = seg_mode ? out_seg + (size_t)pb * n_seg * 3 : nullptr; a.P = Pn;
     a.seg_scale_z = sz; a.seg_scale_s = ss; a.comp = out_comp ? 1 : 0;
     a.piece_first = h->d_piece_first; a.moments = reinterpret_cast<const ulonglong2*>(h->d_moments);
+    a.momentsT = reinterpret_cast<const ulonglong2*>(h->d_momentsT);
     a.moments64 = (sizeof(R) == 8 && h->cached_lg > 0) ? h->d_moments64 : nullptr;
     const dim3 grid(n_chunks, pblocks);
     {
@@ -346,7 +355,15 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
         const bool merge = dc.stride >= 512;
         a.merge_lim = 86400.0 * (kNodeDaysF32 / 4.0) / h->cfg.T_obs_s;
         const dim3 grid_tc(pblocks, n_chunks);
-        if (use_tc) {
+        if (fused3) {
+          const ulonglong2* D3p = reinterpret_cast<const ulonglong2*>(h->D3);
+          const ulonglong2* Gp = reinterpret_cast<const ulonglong2*>(h->Gp3);
+          if (seg_mode && sincos == 2) k_dense3<true, 2><<<grid, kBlock, 0, st>>>(dc, a, D3p, Gp);
+          else if (seg_mode) k_dense3<true, 0><<<grid, kBlock, 0, st>>>(dc, a, D3p, Gp);
+          else if (sincos == 2) k_dense3<false, 2><<<grid, kBlock, 0, st>>>(dc, a, D3p, Gp);
+          else k_dense3<false, 0><<<grid, kBlock, 0, st>>>(dc, a, D3p, Gp);
+        }
+        else if (use_tc) {
           const uint4* Tg = h->d_tc_img;
           if (seg_mode) k_dense2_tc<true, 0><<<grid_tc, tc::kThreads, tc::kSmemBytes, st>>>(dc, a, Dp, Tg);
           else if (sincos == 2 && merge) k_dense2_tc<false, 2, true><<<grid_tc, tc::kThreads, tc::kSmemBytes, st>>>(dc, a, Dp, Tg);
@@ -427,6 +444,12 @@ int build_pieces(sc_handle* h, int CH, int lg_fine, cudaStream_t st) {
     k_moments<<<(h->n_pieces + 127) / 128, 128, 0, st>>>(h->G64, h->d_piece_lo, h->d_piece_hi, h->n_pieces, (int)h->cfg.n_bins,
                                                         lg_fine, h->d_moments, f64 ? h->d_moments64 : nullptr);
     if ((rc = check_launch(h, "k_moments"))) return rc;
+    if (h->GT64 && !f64) {                         // fused three-channel kernel: the same moments of the T weights
+      if ((rc = grow(h, (void**)&h->d_momentsT, &h->momT_cap, std::max<size_t>(lo.size(), 1) * 8 * sizeof(float2)))) return rc;
+      k_moments<<<(h->n_pieces + 127) / 128, 128, 0, st>>>(h->GT64, h->d_piece_lo, h->d_piece_hi, h->n_pieces, (int)h->cfg.n_bins,
+                                                          lg_fine, h->d_momentsT, nullptr);
+      if ((rc = check_launch(h, "k_moments"))) return rc;
+    }
   } else {
     SC_CUDA(h, cudaStreamSynchronize(st));
   }
@@ -475,22 +498,24 @@ int prepare_edges(sc_handle* h, const int32_t* seg_edges, int32_t n_seg, int CH,
 }
 
 int eval_common(sc_handle* h, const double* params, int64_t P, const int32_t* seg_edges, int32_t n_seg,
-                double* out, double* out_seg, void* stream, bool seg_mode, double* out_comp = nullptr) {
+                double* out, double* out_seg, void* stream, bool seg_mode, double* out_comp = nullptr, bool fused3 = false) {
+  // fused3: the one-pass three-channel kernel (FP32-amplitude path of a three-channel handle; the caller escalates)
   if (!h) return SC_ERR_NOT_INIT;
   if (h->cuda_failed) return SC_ERR_CUDA;
   if (!params || P <= 0 || (!seg_mode && !out && !out_comp) || (seg_mode && !out_seg))
     return fail(h, SC_ERR_INVALID_ARG, "null pointer or n_particles <= 0");
   cudaStream_t st = (cudaStream_t)stream;
-  const bool f64 = (h->precision == 2) || (h->precision == 0 && n_seg < h->f32_min_seg);
+  const bool f64 = !fused3 && ((h->precision == 2) || (h->precision == 0 && n_seg < h->f32_min_seg));
   // all-FP64 path: sigma from FP64 piece moments when a fine sub-interval is long enough to pay for them (>= 32 bins)
   const int lg_fine64 = (h->lg_f64 - 2 >= 5) ? h->lg_f64 - 2 : 0;
   // chunk length: 1024 bins (all-FP64), 2048 (k_dense2: the chunk's data is staged in shared memory), 8192 (k_dense2_tc)
-  const int ch32 = (h->use_tc && h->lg_f32 >= 7) ? tc::kChunk : kChunkF32;
+  const int ch32 = (h->use_tc && h->lg_f32 >= 7 && !fused3) ? tc::kChunk : kChunkF32;
   int rc = prepare_edges(h, seg_edges, n_seg, f64 ? kChunkF64 : ch32, f64 ? lg_fine64 : h->lg_f32 - 2, st);
   if (rc) return rc;
   SC_CUDA(h, cudaMemsetAsync(h->d_counter, 0, 8, st));
   if (seg_mode) SC_CUDA(h, cudaMemsetAsync(out_seg, 0, (size_t)P * n_seg * 3 * 8, st));
   if (f64) return run_batches<double>(h, params, P, out, out_seg, out_comp, st, seg_mode);
+  if (fused3) return run_batches<float>(h, params, P, out, out_seg, out_comp, st, seg_mode, nullptr, 0, true);
   if ((rc = run_batches<float>(h, params, P, out, out_seg, out_comp, st, seg_mode))) return rc;
   // Escalation: the FP32 path's error is ~ c / sqrt(Upsilon) relative (c <= 1.0e-6 polynomial,
   // 1.6e-6 hardware sin/cos, measured against the oracle), so a particle whose statistic comes out below tau is evaluated
@@ -559,16 +584,60 @@ int eval_any(sc_handle* h, const double* params, int64_t P, const int32_t* seg_e
   if (!params || P <= 0 || (!seg_mode && !out && !out_comp) || (seg_mode && !out_seg) || !seg_edges || n_seg <= 0)
     return fail(h, SC_ERR_INVALID_ARG, "null pointer, n_particles <= 0 or n_seg <= 0");
   cudaStream_t st = (cudaStream_t)stream;
+  const size_t per_p = (size_t)n_seg * 24;                     // one particle's row of a segment table
+  const double four_df = 4.0 / h->cfg.T_obs_s;
+  int rc;
+  const bool f32_path = (h->precision == 1) || (h->precision == 0 && n_seg >= h->f32_min_seg);
+  // Escalation on three channels (SC_OPT_ESCALATE): the FP32-amplitude kernels leave an error ~ 1e-6 / sqrt(Upsilon), so the
+  // particles whose COMBINED statistic is below tau are evaluated again by the all-FP64 kernels -- two passes in
+  // segment-table mode, combined, scattered back.  The selected count is read back (one 4-byte copy per call or batch).
+  auto escalate3 = [&](double* outp, const double* par, int64_t Pn) -> int {
+    if (!(h->escalate && h->precision == 0 && f32_path && !seg_mode && outp && !out_comp && Pn <= INT32_MAX / 16)) return SC_OK;
+    int rc2;
+    const size_t P_round = (size_t)((Pn + kBlock - 1) / kBlock * kBlock);
+    if ((rc2 = grow(h, (void**)&h->d_esc_idx, &h->esc_idx_cap, (size_t)Pn * 4))) return rc2;
+    if ((rc2 = grow(h, (void**)&h->d_esc_count, &h->esc_cnt_cap, 256))) return rc2;
+    if ((rc2 = grow(h, (void**)&h->d_esc_params, &h->esc_par_cap, P_round * 64))) return rc2;
+    if ((rc2 = grow(h, (void**)&h->d_esc_out, &h->esc_out_cap, P_round * 8))) return rc2;
+    {
+      Timed tm(h, st, SC_TIME_ESC);
+      const bool mufu3 = (h->sincos_mode == 0) ? (n_seg >= h->mufu_min_seg) : (h->sincos_mode == 2);
+      k_esc_select<<<1, 1024, 0, st>>>(outp, par, (int)Pn, mufu3 ? h->esc_tau_mufu : h->esc_tau_poly, h->d_esc_idx, h->d_esc_count, h->d_esc_params);
+    }
+    if ((rc2 = check_launch(h, "k_esc_select"))) return rc2;
+    int n_esc = 0;
+    SC_CUDA(h, cudaMemcpyAsync(&n_esc, h->d_esc_count, 4, cudaMemcpyDeviceToHost, st));
+    SC_CUDA(h, cudaStreamSynchronize(st));
+    if (n_esc <= 0) return SC_OK;
+    // (the tables of the main passes are not needed any more: a call with the fused kernel has none, the two-pass loop has combined its batch)
+    if (2 * per_p * (size_t)n_esc > h->seg3_cap && (rc2 = grow(h, (void**)&h->d_seg3, &h->seg3_cap, 2 * per_p * (size_t)n_esc))) return rc2;
+    double* eA = h->d_seg3; double* eT = eA + (size_t)n_esc * n_seg * 3;
+    h->precision = 2; h->sub->precision = 2;
+    rc2 = eval_common(h, h->d_esc_params, n_esc, seg_edges, n_seg, nullptr, eA, stream, true);
+    if (!rc2) rc2 = eval_common(h->sub, h->d_esc_params, n_esc, seg_edges, n_seg, nullptr, eT, stream, true);
+    h->precision = 0; h->sub->precision = 0;
+    if (rc2) return rc2;
+    Timed tm(h, st, SC_TIME_ESC);
+    k_combine3<<<(unsigned)((n_esc + 127) / 128), 128, 0, st>>>(eA, eT, n_esc, n_seg, four_df, h->d_esc_out, nullptr, nullptr);
+    if ((rc2 = check_launch(h, "k_combine3"))) return rc2;
+    k_esc_scatter<<<(unsigned)((Pn + 127) / 128), 128, 0, st>>>(h->d_esc_idx, h->d_esc_count, h->d_esc_out, outp);
+    return check_launch(h, "k_esc_scatter");
+  };
+
+  // One pass (k_dense3: A, E, T in the pair loop) on the FP32-amplitude path; the all-FP64 modes take the two passes below.
+  if (h->D3 && h->use_fused3 && f32_path) {
+    if ((rc = eval_common(h, params, P, seg_edges, n_seg, out, out_seg, stream, seg_mode, out_comp, true))) return rc;
+    return escalate3(out, params, P);
+  }
+
+  // Two passes, (A, E) and (T, nothing), through the two-channel kernels in segment-table mode, then the combination;
   // batches of particles such that the two segment tables fit in 2 GiB
-  const size_t per_p = (size_t)n_seg * 24;
   int64_t Pb = (int64_t)std::max<size_t>(1, ((size_t)1 << 30) / per_p);
   Pb = std::min<int64_t>(Pb, P);
-  int rc = grow(h, (void**)&h->d_seg3, &h->seg3_cap, 2 * per_p * (size_t)Pb);
-  if (rc) return rc;
-  double* segA = h->d_seg3; double* segT = segA + (size_t)Pb * n_seg * 3;
-  const double four_df = 4.0 / h->cfg.T_obs_s;
   for (int64_t pb = 0; pb < P; pb += Pb) {
     const int64_t Pn = std::min<int64_t>(Pb, P - pb);
+    if ((rc = grow(h, (void**)&h->d_seg3, &h->seg3_cap, 2 * per_p * (size_t)Pb))) return rc;
+    double* segA = h->d_seg3; double* segT = segA + (size_t)Pb * n_seg * 3;
     if ((rc = eval_common(h, params + pb * 8, Pn, seg_edges, n_seg, nullptr, segA, stream, true))) return rc;
     if ((rc = eval_common(h->sub, params + pb * 8, Pn, seg_edges, n_seg, nullptr, segT, stream, true))) {
       fail(h, rc, "T pass: %s", h->sub->err.c_str());
@@ -581,39 +650,7 @@ int eval_any(sc_handle* h, const double* params, int64_t P, const int32_t* seg_e
                                                               out_comp ? out_comp + pb * 3 : nullptr);
       if ((rc = check_launch(h, "k_combine3"))) return rc;
     }
-    // Escalation on three channels (SC_OPT_ESCALATE): both passes ran the FP32-amplitude kernels in segment-table mode
-    // (same sin/cos flavour rule as sc_eval_stat), so a particle whose COMBINED statistic is below tau carries an error ~ 1e-6 / sqrt(Upsilon):
-    // those are evaluated again by the all-FP64 kernels, both passes, and combined.  This path reads the selected count
-    // back (one 4-byte copy per batch): three-channel evaluation is two passes plus a table pass, not the device-resident loop.
-    const bool f32_path = (h->precision == 1) || (h->precision == 0 && n_seg >= h->f32_min_seg);
-    if (h->escalate && h->precision == 0 && f32_path && !seg_mode && out && !out_comp && Pn <= INT32_MAX / 16) {
-      const size_t P_round = (size_t)((Pn + kBlock - 1) / kBlock * kBlock);
-      if ((rc = grow(h, (void**)&h->d_esc_idx, &h->esc_idx_cap, (size_t)Pn * 4))) return rc;
-      if ((rc = grow(h, (void**)&h->d_esc_count, &h->esc_cnt_cap, 256))) return rc;
-      if ((rc = grow(h, (void**)&h->d_esc_params, &h->esc_par_cap, P_round * 64))) return rc;
-      if ((rc = grow(h, (void**)&h->d_esc_out, &h->esc_out_cap, P_round * 8))) return rc;
-      {
-        Timed tm(h, st, SC_TIME_ESC);
-        const bool mufu3 = (h->sincos_mode == 0) ? (n_seg >= h->mufu_min_seg) : (h->sincos_mode == 2);
-        k_esc_select<<<1, 1024, 0, st>>>(out + pb, params + pb * 8, (int)Pn, mufu3 ? h->esc_tau_mufu : h->esc_tau_poly, h->d_esc_idx, h->d_esc_count, h->d_esc_params);
-      }
-      if ((rc = check_launch(h, "k_esc_select"))) return rc;
-      int n_esc = 0;
-      SC_CUDA(h, cudaMemcpyAsync(&n_esc, h->d_esc_count, 4, cudaMemcpyDeviceToHost, st));
-      SC_CUDA(h, cudaStreamSynchronize(st));
-      if (n_esc > 0) {
-        h->precision = 2; h->sub->precision = 2;
-        rc = eval_common(h, h->d_esc_params, n_esc, seg_edges, n_seg, nullptr, segA, stream, true);
-        if (!rc) rc = eval_common(h->sub, h->d_esc_params, n_esc, seg_edges, n_seg, nullptr, segT, stream, true);
-        h->precision = 0; h->sub->precision = 0;
-        if (rc) return rc;
-        Timed tm(h, st, SC_TIME_ESC);
-        k_combine3<<<(unsigned)((n_esc + 127) / 128), 128, 0, st>>>(segA, segT, n_esc, n_seg, four_df, h->d_esc_out, nullptr, nullptr);
-        if ((rc = check_launch(h, "k_combine3"))) return rc;
-        k_esc_scatter<<<(unsigned)((Pn + 127) / 128), 128, 0, st>>>(h->d_esc_idx, h->d_esc_count, h->d_esc_out, out + pb);
-        if ((rc = check_launch(h, "k_esc_scatter"))) return rc;
-      }
-    }
+    if ((rc = escalate3(out ? out + pb : nullptr, params + pb * 8, Pn))) return rc;
   }
   return SC_OK;
 }
@@ -898,6 +935,21 @@ int sc_init_data3(sc_handle** out, const sc_config* cfg, const double* dA, const
   cudaFree(zeros);
   if (rc) { sc_free(h); return rc; }
   h->cfg.n_channels = 3;
+  // fused tables of the one-pass kernel k_dense3: T's whitened data and weights at the (A, E) handle's scale
+  {
+    const int n = (int)cfg->n_bins;
+    const int n_pairs_pad = (n + tc::kChunk - 1) / tc::kChunk * (tc::kChunk / 2);
+    cudaStream_t st = (cudaStream_t)stream;
+    if (cudaMalloc(&h->D3, (size_t)n_pairs_pad * 3 * sizeof(float4)) != cudaSuccess ||
+        cudaMalloc(&h->Gp3, (size_t)n_pairs_pad * 2 * sizeof(float4)) != cudaSuccess ||
+        cudaMalloc(&h->GT64, (size_t)n * sizeof(double2)) != cudaSuccess) {
+      cudaGetLastError(); sc_free(h); return fail(nullptr, SC_ERR_OOM, "cudaMalloc failed (fused three-channel tables)");
+    }
+    const float r = (float)(h->sub->s0 / h->s0);              // both powers of two
+    k_fuse3<<<(n_pairs_pad + 255) / 256, 256, 0, st>>>(h->D32, h->sub->D32, h->sub->G64, n_pairs_pad, n, r, h->D3, h->Gp3, h->GT64);
+    h->launches++;
+    if (cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) { sc_free(h); return fail(nullptr, SC_ERR_CUDA, "k_fuse3 failed"); }
+  }
   *out = h;
   return SC_OK;
 }
@@ -1442,6 +1494,9 @@ int sc_set_option(sc_handle* h, int32_t option, int64_t value) {
     case SC_OPT_WINDOW_SORT:
       if (value < 0 || value > 1) return fail(h, SC_ERR_INVALID_ARG, "window_sort must be 0 or 1");
       h->window_sort = (int)value; return SC_OK;
+    case SC_OPT_FUSED_AET:
+      if (value < 0 || value > 1) return fail(h, SC_ERR_INVALID_ARG, "fused_aet must be 0 or 1");
+      h->use_fused3 = (int)value; return SC_OK;
     case SC_OPT_TENSOR_CORES:
       if (value < 0 || value > 1) return fail(h, SC_ERR_INVALID_ARG, "tensor_cores must be 0 or 1");
       h->use_tc = (int)value; return SC_OK;
@@ -1470,7 +1525,8 @@ int sc_free(sc_handle* h) {
   if (!h) return SC_ERR_NOT_INIT;
   if (h->sub) sc_free(h->sub);
   cudaFree(h->d_seg3);
-  cudaFree(h->D32); cudaFree(h->W64); cudaFree(h->G64); cudaFree(h->d_tc_img);
+  cudaFree(h->D32); cudaFree(h->W64); cudaFree(h->G64); cudaFree(h->d_tc_img); cudaFree(h->D3); cudaFree(h->Gp3); cudaFree(h->GT64);
+  cudaFree(h->d_momentsT); cudaFree(h->alt.d_momentsT);
   cudaFree(h->scratch); cudaFree(h->d_edges); cudaFree(h->d_chunk_k0); cudaFree(h->d_flags);
   cudaFree(h->d_counter); cudaFree(h->d_params_stage); cudaFree(h->d_comp); cudaFree(h->d_km); cudaFree(h->d_T64); cudaFree(h->d_T32); cudaFree(h->d_sp);
   cudaFree(h->d_spsig); cudaFree(h->d_zpart); cudaFree(h->d_hh); cudaFree(h->d_gmom); cudaFree(h->d_smom);

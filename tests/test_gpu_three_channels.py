@@ -78,6 +78,29 @@ def test_three_channel_template_and_noise_free_match(oracle):
     H2.close()
 
 
+def test_fused_and_two_pass_agree(oracle):
+    """SC_OPT_FUSED_AET: the one-pass kernel (A, E, T in the pair loop) and the two passes with combined segment tables are
+    the same definition -- statistic, segments and components agree to FP32 rounding for the whole population, at levels
+    that take the polynomial (N = 10) and the hardware (N = 100, 1000) sin/cos flavour."""
+    torch, sc, inp, cfgd, cfg, S3, d3, th, kappa, h3, H = _setup(oracle, 2, 512, 17.0, 906)
+    H.set_option(sc.SC_OPT_TC_MAX_S, int(np.ceil(inp["hi"][2])))
+    H.set_option(sc.SC_OPT_ESCALATE, 0)
+    par = _dev(torch, inp["particles"])
+    for N in (10, 100, 1000):
+        e = sy.edges(cfgd["n_bins"], N)
+        res = {}
+        for fused in (1, 0):
+            H.set_option(sc.SC_OPT_FUSED_AET, fused)
+            res[fused] = (H.eval_stat(par, e).cpu().numpy(), H.eval_segments(par, e).cpu().numpy(), H.eval_components(par, e).cpu().numpy())
+        a, b = res[1], res[0]
+        ok = b[0] > 1.0
+        assert ok.sum() > 400 and rel_err(a[0][ok], b[0][ok]).max() <= 2e-6 / np.sqrt(b[0][ok]).min()
+        scale = np.abs(b[1]).max(axis=1, keepdims=True)
+        assert (np.abs(a[1] - b[1]) / scale).max() <= 2e-6
+        assert rel_err(a[2][ok], b[2][ok]).max() <= 2e-6
+    H.close()
+
+
 def test_c2_three_channels_sampled(oracle):
     torch, sc, inp, cfgd, cfg, S3, d3, th, kappa, h3, H = _setup(oracle, 2, None, 17.0, 903)
     H.set_option(sc.SC_OPT_TC_MAX_S, int(np.ceil(inp["hi"][2])))
