@@ -718,3 +718,55 @@ void sco_eval_stat3(const sco_config* c, const double* dA, const double* dE, con
     free(hA); free(hE); free(hT);
   }
 }
+
+/* Per-particle equal-SNR^2 segments over three channels (PAPER.md:120 with the channel sums of PAPER.md:36, 59):
+ *   s_j = sum_{a in A,E,T} |h_a(f_j)|^2 / S_a(f_j),  then exactly the rule of sco_equal_snr_edges.  hT == NULL: two channels. */
+void sco_equal_snr_edges3(const double* hA, const double* hE, const double* hT, const double* SA, const double* SE,
+                          const double* ST, int64_t n_bins, int64_t n_seg, int64_t* edges) {
+  double total = 0.0;
+  for (int64_t j = 0; j < n_bins; ++j) {
+    total += (hA[2 * j] * hA[2 * j] + hA[2 * j + 1] * hA[2 * j + 1]) / SA[j];
+    total += (hE[2 * j] * hE[2 * j] + hE[2 * j + 1] * hE[2 * j + 1]) / SE[j];
+    if (hT && ST) total += (hT[2 * j] * hT[2 * j] + hT[2 * j + 1] * hT[2 * j + 1]) / ST[j];
+  }
+  edges[0] = 0; edges[n_seg] = n_bins;
+  double cum = 0.0;            /* C_j */
+  int64_t j = 0;
+  for (int64_t n = 1; n < n_seg; ++n) {
+    const double target = total * (double)n / (double)n_seg;
+    while (j < n_bins && !(cum >= target)) {
+      cum += (hA[2 * j] * hA[2 * j] + hA[2 * j + 1] * hA[2 * j + 1]) / SA[j];
+      cum += (hE[2 * j] * hE[2 * j] + hE[2 * j + 1] * hE[2 * j + 1]) / SE[j];
+      if (hT && ST) cum += (hT[2 * j] * hT[2 * j] + hT[2 * j + 1] * hT[2 * j + 1]) / ST[j];
+      ++j;
+    }
+    edges[n] = (total > 0.0) ? j : 0;
+  }
+}
+
+/* Upsilon_N over three channels with per-particle equal-SNR^2 edges; in_edges / out_edges / out_comp3 as in
+ * sco_eval_stat_adaptive. */
+void sco_eval_stat_adaptive3(const sco_config* c, const double* dA, const double* dE, const double* dT, const double* SA,
+                             const double* SE, const double* ST, const double* params, int64_t P, int64_t n_seg,
+                             const int64_t* in_edges, double* out, int64_t* out_edges, double* out_comp3) {
+  const int64_t n = c->n_bins;
+  const double df = 1.0 / c->T_obs_s;
+#pragma omp parallel
+  {
+    double* hA = (double*)malloc((size_t)n * 2 * sizeof(double));
+    double* hE = (double*)malloc((size_t)n * 2 * sizeof(double));
+    double* hT = (double*)malloc((size_t)n * 2 * sizeof(double));
+    int64_t* e = (int64_t*)malloc((size_t)(n_seg + 1) * sizeof(int64_t));
+    double* seg = (double*)malloc((size_t)n_seg * 3 * sizeof(double));
+#pragma omp for schedule(dynamic, 1)
+    for (int64_t p = 0; p < P; ++p) {
+      sco_template3(c, params + 8 * p, 0, n, hA, hE, hT);
+      if (in_edges) memcpy(e, in_edges + p * (n_seg + 1), (size_t)(n_seg + 1) * sizeof(int64_t));
+      else sco_equal_snr_edges3(hA, hE, hT, SA, SE, ST, n, n_seg, e);
+      out[p] = sco_stat_from_arrays3(dA, dE, dT, hA, hE, hT, SA, SE, ST, df, e, n_seg, seg);
+      if (out_edges) memcpy(out_edges + p * (n_seg + 1), e, (size_t)(n_seg + 1) * sizeof(int64_t));
+      if (out_comp3) sco_components_from_seg(seg, n_seg, df, out_comp3 + 3 * p);
+    }
+    free(hA); free(hE); free(hT); free(e); free(seg);
+  }
+}

@@ -145,6 +145,14 @@ double sco_stat_from_arrays3(const double* dA_ri, const double* dE_ri, const dou
                              const double* S_T, double df, const int64_t* edges, int64_t n_seg, double* out_seg);
 double sco_inner3(const double* aA, const double* aE, const double* aT, const double* bA, const double* bE, const double* bT,
                   const double* S_A, const double* S_E, const double* S_T, double df, int64_t n);
+/* Three-channel versions of sco_equal_snr_edges / sco_eval_stat_adaptive (s_j summed over A, E, T).  Pins: hT == NULL gives
+ * sco_equal_snr_edges; every segment holds C/N to within one bin's s_j; d = h over three channels gives rho^2 on its own
+ * edges; in_edges = the shared equal-width list gives sco_eval_stat3 (tests/test_oracle_three_channels.py). */
+void sco_equal_snr_edges3(const double* hA_ri, const double* hE_ri, const double* hT_ri, const double* S_A, const double* S_E,
+                          const double* S_T, int64_t n_bins, int64_t n_seg, int64_t* edges);
+void sco_eval_stat_adaptive3(const sco_config* c, const double* dA_ri, const double* dE_ri, const double* dT_ri,
+                             const double* S_A, const double* S_E, const double* S_T, const double* params, int64_t P,
+                             int64_t n_seg, const int64_t* in_edges, double* out, int64_t* out_edges, double* out_comp3);
 void sco_eval_stat3(const sco_config* c, const double* dA_ri, const double* dE_ri, const double* dT_ri, const double* S_A,
                     const double* S_E, const double* S_T, const double* params, int64_t n_particles,
                     const int64_t* edges, int64_t n_seg, double* out, double* out_seg);

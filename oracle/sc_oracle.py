@@ -97,6 +97,8 @@ def lib():
         L.sco_inner3.restype = C.c_double
         L.sco_inner3.argtypes = [_dp] * 9 + [C.c_double, C.c_int64]
         L.sco_eval_stat3.argtypes = [C.POINTER(Config)] + [_dp] * 7 + [C.c_int64, _ip, C.c_int64, _dp, _dp]
+        L.sco_equal_snr_edges3.argtypes = [_dp] * 6 + [C.c_int64, C.c_int64, _ip]
+        L.sco_eval_stat_adaptive3.argtypes = [C.POINTER(Config)] + [_dp] * 7 + [C.c_int64, C.c_int64, _ip, _dp, _ip, _dp]
         L.sco_converged.restype = C.c_int32
         L.sco_converged.argtypes = [_dp, C.c_int64, C.c_int32, C.c_double]
     return _lib
@@ -357,3 +359,33 @@ def eval_stat3(cfg, d3, S3, params, edges, want_seg=False):
     a = [_ri(x) for x in d3] + [_f64(x) for x in S3]
     lib().sco_eval_stat3(C.byref(cfg), *[_d(x) for x in a], _d(params), P, edges.ctypes.data_as(_ip), n_seg, _d(out), _d(seg))
     return (out, seg) if want_seg else out
+
+
+def equal_snr_edges3(h3, S3, n_seg):
+    """PAPER.md:120 over three channels; h3 = (hA, hE, hT) with hT possibly None (two channels)."""
+    hA, hE, hT = h3
+    n = len(hA)
+    e = np.zeros(n_seg + 1, dtype=np.int64)
+    lib().sco_equal_snr_edges3(_d(_ri(hA)), _d(_ri(hE)), None if hT is None else _d(_ri(hT)), _d(_f64(S3[0])), _d(_f64(S3[1])),
+                               None if hT is None else _d(_f64(S3[2])), n, n_seg, e.ctypes.data_as(_ip))
+    return e
+
+
+def eval_stat_adaptive3(cfg, d3, S3, params, n_seg, in_edges=None, want_edges=False, want_comp=False):
+    """Upsilon_N over A, E, T with per-particle equal-SNR^2 edges; in_edges [P][n_seg+1] overrides the choice."""
+    params = _f64(params).reshape(-1, 8)
+    P = params.shape[0]
+    out = np.zeros(P)
+    ie = None if in_edges is None else np.ascontiguousarray(in_edges, dtype=np.int64).reshape(P, n_seg + 1)
+    oe = np.zeros((P, n_seg + 1), dtype=np.int64) if want_edges else None
+    oc = np.zeros((P, 3)) if want_comp else None
+    a = [_ri(x) for x in d3] + [_f64(x) for x in S3]
+    lib().sco_eval_stat_adaptive3(C.byref(cfg), *[_d(x) for x in a], _d(params), P, n_seg,
+                                  None if ie is None else ie.ctypes.data_as(_ip), _d(out),
+                                  None if oe is None else oe.ctypes.data_as(_ip), _d(oc))
+    res = [out]
+    if want_edges:
+        res.append(oe)
+    if want_comp:
+        res.append(oc)
+    return res[0] if len(res) == 1 else tuple(res)

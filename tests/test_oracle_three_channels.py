@@ -115,3 +115,58 @@ def test_eval_stat3_matches_composition(oracle):
         h3 = oracle.template3(cfg, P[p])[:3]
         u, s = oracle.stat_from_arrays3(d3, h3, S3, df, e, want_seg=True)
         assert out[p] == u and np.array_equal(seg[p], s)
+
+
+def test_equal_snr_edges3_pins(oracle):
+    """PAPER.md:120 over three channels: (i) without T the rule is sco_equal_snr_edges; (ii) every segment holds C/N to within
+    one bin's s_j, with s_j written out here from the definition; (iii) flat s_j split over three channels gives
+    e_n = ceil(n n_bins / N); (iv) T matters: switching it on moves edges of a real template."""
+    cfgd, cfg, f, S3, th, rng = _tiny(oracle, 3)
+    n = len(f)
+    h3 = oracle.template3(oracle.make_config(dict(cfgd, window_mode=0)), th)[:3]
+    for N in (1, 2, 7, 40):
+        e2 = oracle.equal_snr_edges(h3[0], h3[1], S3[0], S3[1], N)
+        assert np.array_equal(oracle.equal_snr_edges3((h3[0], h3[1], None), S3, N), e2)
+        # make T count: scale it up so that it carries a third of the total
+        sA = np.abs(h3[0]) ** 2 / S3[0] + np.abs(h3[1]) ** 2 / S3[1]
+        sT = np.abs(h3[2]) ** 2 / S3[2]
+        g = np.sqrt(0.5 * sA.sum() / sT.sum())
+        hT = g * h3[2] * (1.0 + 0.5 * np.sin(np.arange(n) / 7.0))          # and give it a shape of its own
+        e3 = oracle.equal_snr_edges3((h3[0], h3[1], hT), S3, N)
+        s = sA + np.abs(hT) ** 2 / S3[2]
+        cum = np.concatenate([[0.0], np.cumsum(s)])
+        C = cum[-1]
+        assert e3[0] == 0 and e3[-1] == n and np.all(np.diff(e3) >= 0)
+        for k in range(1, N):
+            j = e3[k]
+            assert cum[j] >= C * k / N * (1 - 1e-12) and (j == 0 or cum[j - 1] < C * k / N * (1 + 1e-12))
+        if N == 40:
+            assert not np.array_equal(e3, e2)
+    ones = np.ones(n, dtype=complex)
+    for N in (3, 10):
+        e = oracle.equal_snr_edges3((ones, 2 * ones, 3 * ones), (np.ones(n), np.ones(n), np.ones(n)), N)
+        assert np.array_equal(e[1:-1], np.ceil(np.arange(1, N) * n / N).astype(np.int64))
+
+
+def test_eval_stat_adaptive3_composition_and_identities(oracle):
+    cfgd, cfg, f, S3, th, rng = _tiny(oracle, 4)
+    df = 1.0 / cfgd["T_obs_s"]
+    n = len(f)
+    h3 = oracle.template3(cfg, th)[:3]
+    d3 = [h + np.sqrt(S / (4 * df)) * (rng.standard_normal(n) + 1j * rng.standard_normal(n)) for h, S in zip(h3, S3)]
+    P = np.vstack([th, th * np.array([1.001, 1, 1, 1.1, 1, 1, 1, 1])])
+    for N in (1, 6):
+        out, ed, comp = oracle.eval_stat_adaptive3(cfg, d3, S3, P, N, want_edges=True, want_comp=True)
+        for p in range(2):
+            g3 = oracle.template3(cfg, P[p])[:3]
+            e = oracle.equal_snr_edges3(g3, S3, N)
+            assert np.array_equal(ed[p], e)
+            u, seg = oracle.stat_from_arrays3(d3, g3, S3, df, e, want_seg=True)
+            assert out[p] == u and np.array_equal(comp[p], oracle.components_from_seg(seg, df))
+        # given edges override the choice: the shared equal-width list reproduces sco_eval_stat3
+        sh = sy.edges(n, N)
+        assert np.array_equal(oracle.eval_stat_adaptive3(cfg, d3, S3, P, N, in_edges=np.tile(sh, (2, 1))), oracle.eval_stat3(cfg, d3, S3, P, sh))
+    # d = h over three channels: rho^2 on its own equal-SNR^2 edges, whatever N
+    rho2 = oracle.inner3(h3, h3, S3, df)
+    for N in (1, 5, 30):
+        assert oracle.eval_stat_adaptive3(cfg, h3, S3, th[None, :], N)[0] == pytest.approx(rho2, rel=1e-12)
