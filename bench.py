@@ -443,6 +443,9 @@ def run_ours(args, rank, local_rank, world):
             b_.record(); torch.cuda.synchronize()
             extras["three_channels"] = {"what": "sc_eval_stat on an (A, E, T) handle (T noise only), same population and edges: "
                                                 "one pass through the fused kernel k_dense3 (SC_OPT_FUSED_AET = 1)", "ms_per_eval": a_.elapsed_time(b_) / 2}
+            sc.sc_eval_stat_adaptive(H3.h, state["pos"], P, 100, stat); torch.cuda.synchronize()
+            a_.record(); sc.sc_eval_stat_adaptive(H3.h, state["pos"], P, 100, stat); b_.record(); torch.cuda.synchronize()
+            extras["three_channels"]["ms_per_eval_adaptive_N100"] = a_.elapsed_time(b_)   # the paper's own configuration
             H3.set_option(sc.SC_OPT_FUSED_AET, 0)
             H3.eval_stat(state["pos"], e, out=stat); torch.cuda.synchronize()
             a_.record(); H3.eval_stat(state["pos"], e, out=stat); b_.record(); torch.cuda.synchronize()

@@ -117,10 +117,11 @@ int sc_init_data_host(sc_handle** out, const sc_config* cfg,
 
 /* Three TDI channels A, E, T (Eq. 1 and Eq. 7 sum over alpha in {A, E, T}; T = (X + Y + Z)/sqrt(3),
  * reading Q16).  cfg->n_channels must be 3; all arrays DEVICE as in sc_init_data.  On such a handle sc_eval_stat[_host],
- * sc_eval_segments, sc_eval_components, sc_eval_loglike, sc_data_norm and sc_search_run (equal-width edges) include the
- * T channel: its per-segment sums come from a second pass through the same kernels and are added to those of A and E
- * before |z_k|^2 / sigma_k is formed (one common phase per segment, Q1).  sc_eval_stat_adaptive (n_seg > 1) and the
- * streams workload return SC_ERR_INVALID_ARG on three-channel handles. */
+ * sc_eval_segments, sc_eval_components, sc_eval_loglike, sc_data_norm, sc_eval_stat_adaptive and sc_search_run (shared or
+ * per-particle edges) include the T channel: z_k and sigma_k are summed over A, E and T before |z_k|^2 / sigma_k is formed
+ * (one common phase per segment, Q1), and the equal-SNR^2 edges are those of s_j summed over the three channels.  The
+ * FP32-amplitude path does this in one pass (SC_OPT_FUSED_AET), the all-FP64 modes in two passes whose per-segment sums are
+ * added.  The streams workload returns SC_ERR_INVALID_ARG on three-channel handles. */
 int sc_init_data3(sc_handle** out, const sc_config* cfg,
                   const double* dA_ri, const double* dE_ri, const double* dT_ri,
                   const double* S_A, const double* S_E, const double* S_T, void* cuda_stream);

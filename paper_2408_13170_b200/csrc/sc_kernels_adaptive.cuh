@@ -36,6 +36,8 @@ struct AdaptArgs {
   const double2* gmom64;       // [n_groups][7] ... over the groups
   const double2* G64;          // [n_bins] sigma weights per bin (FP64)
   double* sub_sigma;           // [n_chunks * CH / Sf][P_pad]: sigma of every fine sub-interval (k_sigma_chunks64 -> k_edges64)
+  // three-channel handles (NA = 6): the same tables for the T weights, as (T, 0) pairs
+  const ulonglong2* gmomT; const ulonglong2* smomT; const double2* smom64T; const double2* GT64;
 };
 
 __device__ __forceinline__ double seg_target(double C, int n, int N) { return C * (double)n / (double)N; }
@@ -52,30 +54,33 @@ __device__ __forceinline__ int seg_index(double cum, double C, int N) {
 // The six FP64 nodes (m = -2 .. 3) of the four amplitude components around coarse interval ic, kept in registers while a
 // lane walks the chunk: the four fine sub-intervals of a coarse interval share them, and the next coarse interval needs
 // one new node per component (read per sub-interval they cost 25 GB of L2 traffic per pass on c3).
-struct Nodes64 { double v[4][6]; };
-__device__ __forceinline__ void nodes64_load(const DevCfg& c, const DenseArgs& a, int p, int ic, Nodes64& n) {
+template <int NA> struct Nodes64 { double v[NA][6]; };      // NA = 4: (A, E); 6: (A, E, T)
+template <int NA>
+__device__ __forceinline__ void nodes64_load(const DevCfg& c, const DenseArgs& a, int p, int ic, Nodes64<NA>& n) {
   const double* __restrict__ namp = reinterpret_cast<const double*>(a.node_amp);
 #pragma unroll
-  for (int r = 0; r < 4; ++r) {
-    const double* col = namp + ((size_t)(ic + kNodeOff) * 4 + r) * a.P_pad + p;
-    const ptrdiff_t st = (ptrdiff_t)4 * a.P_pad;
+  for (int r = 0; r < NA; ++r) {
+    const double* col = namp + ((size_t)(ic + kNodeOff) * NA + r) * a.P_pad + p;
+    const ptrdiff_t st = (ptrdiff_t)NA * a.P_pad;
 #pragma unroll
     for (int m = -2; m <= 3; ++m) n.v[r][m + 2] = col[m * st];
   }
 }
-__device__ __forceinline__ void nodes64_advance(const DevCfg& c, const DenseArgs& a, int p, int ic_new, Nodes64& n) {
+template <int NA>
+__device__ __forceinline__ void nodes64_advance(const DevCfg& c, const DenseArgs& a, int p, int ic_new, Nodes64<NA>& n) {
   const double* __restrict__ namp = reinterpret_cast<const double*>(a.node_amp);
 #pragma unroll
-  for (int r = 0; r < 4; ++r) {
+  for (int r = 0; r < NA; ++r) {
 #pragma unroll
     for (int m = 0; m < 5; ++m) n.v[r][m] = n.v[r][m + 1];
-    n.v[r][5] = namp[((size_t)(ic_new + kNodeOff + 3) * 4 + r) * a.P_pad + p];
+    n.v[r][5] = namp[((size_t)(ic_new + kNodeOff + 3) * NA + r) * a.P_pad + p];
   }
 }
-// FP64 cubic coefficients of (Ar, Ai, Er, Ei) on fine sub-interval q of the coarse interval whose nodes are n.
-__device__ __forceinline__ void sub_amps64(const Nodes64& n, int q, double (&cf)[4][4]) {
+// FP64 cubic coefficients of (Ar, Ai, Er, Ei[, Tr, Ti]) on fine sub-interval q of the coarse interval whose nodes are n.
+template <int NA>
+__device__ __forceinline__ void sub_amps64(const Nodes64<NA>& n, int q, double (&cf)[NA][4]) {
 #pragma unroll
-  for (int r = 0; r < 4; ++r)
+  for (int r = 0; r < NA; ++r)
 #pragma unroll
     for (int kk = 0; kk < 4; ++kk) {
       double acc = 0.0;
@@ -84,27 +89,49 @@ __device__ __forceinline__ void sub_amps64(const Nodes64& n, int q, double (&cf)
       cf[r][kk] = acc;
     }
 }
-// s_j = G_A(j) |c_A(s_j)|^2 + G_E(j) |c_E(s_j)|^2 in FP64 (the integrand of <h|h>, up to the common scale).
-__device__ __forceinline__ double sigma_bin64(const double (&cf)[4][4], double sj, double2 g) {
+// s_j = sum_a G_a(j) |c_a(s_j)|^2 in FP64 (the integrand of <h|h>, up to the common scale).
+template <int NA>
+__device__ __forceinline__ double sigma_bin64(const double (&cf)[NA][4], double sj, double2 g, double gT) {
   const double Ar = fma(fma(fma(cf[0][3], sj, cf[0][2]), sj, cf[0][1]), sj, cf[0][0]);
   const double Ai = fma(fma(fma(cf[1][3], sj, cf[1][2]), sj, cf[1][1]), sj, cf[1][0]);
   const double Er = fma(fma(fma(cf[2][3], sj, cf[2][2]), sj, cf[2][1]), sj, cf[2][0]);
   const double Ei = fma(fma(fma(cf[3][3], sj, cf[3][2]), sj, cf[3][1]), sj, cf[3][0]);
-  return fma(g.x, fma(Ar, Ar, Ai * Ai), g.y * fma(Er, Er, Ei * Ei));
+  double s = fma(g.x, fma(Ar, Ar, Ai * Ai), g.y * fma(Er, Er, Ei * Ei));
+  if (NA == 6) {
+    const double Tr = fma(fma(fma(cf[NA - 2][3], sj, cf[NA - 2][2]), sj, cf[NA - 2][1]), sj, cf[NA - 2][0]);
+    const double Ti = fma(fma(fma(cf[NA - 1][3], sj, cf[NA - 1][2]), sj, cf[NA - 1][1]), sj, cf[NA - 1][0]);
+    s = fma(gT, fma(Tr, Tr, Ti * Ti), s);
+  }
+  return s;
+}
+// sigma over a run of bins from the FP64 moments of its weights, all channels
+template <int NA>
+__device__ __forceinline__ double sigma_mom64(const double (&cf)[NA][4], const double2* __restrict__ M, const double2* __restrict__ MT) {
+  double s = sigma_moments64(*reinterpret_cast<const double(*)[4][4]>(&cf[0]), M);
+  if (NA == 6) {
+    const double cT[4][4] = {{cf[NA - 2][0], cf[NA - 2][1], cf[NA - 2][2], cf[NA - 2][3]},
+                             {cf[NA - 1][0], cf[NA - 1][1], cf[NA - 1][2], cf[NA - 1][3]}, {0, 0, 0, 0}, {0, 0, 0, 0}};
+    s += sigma_moments64(cT, MT);
+  }
+  return s;
 }
 // sigma of the fine sub-interval [ib, ie) for this lane: from the moments when the lane's window covers it, bin by bin
 // (masked) when a window border falls inside.  The same function serves k_sigma_chunks64 and k_edges64, so the second
 // pass reproduces the chunk sums of the first bit for bit.
-__device__ __forceinline__ double sigma_sub64(const DevCfg& c, const AdaptArgs& ad, const double (&cf)[4][4], int ib, int ie,
+template <int NA>
+__device__ __forceinline__ double sigma_sub64(const DevCfg& c, const AdaptArgs& ad, const double (&cf)[NA][4], int ib, int ie,
                                               int jlo, int jhi, int n_bins) {
   const int Sf = c.stride >> 2;
-  if (ib >= jlo && ie <= jhi && ie - ib == Sf) return sigma_moments64(cf, ad.smom64 + (size_t)(ib >> (c.log2_stride - 2)) * 7);
+  const size_t isub = (size_t)(ib >> (c.log2_stride - 2));
+  if (ib >= jlo && ie <= jhi && ie - ib == Sf) return sigma_mom64<NA>(cf, ad.smom64 + isub * 7, NA == 6 ? ad.smom64T + isub * 7 : nullptr);
   const double hS = 1.0 / (double)Sf;
   double tot = 0.0;
-  for (int j = max(ib, jlo); j < min(min(ie, jhi), n_bins); ++j) tot += sigma_bin64(cf, (double)(j - ib) * hS, ad.G64[j]);
+  for (int j = max(ib, jlo); j < min(min(ie, jhi), n_bins); ++j)
+    tot += sigma_bin64<NA>(cf, (double)(j - ib) * hS, ad.G64[j], NA == 6 ? ad.GT64[j].x : 0.0);
   return tot;
 }
 
+template <int NA = 4>
 __global__ void __launch_bounds__(kBlock) k_sigma_chunks64(DevCfg c, DenseArgs a, AdaptArgs ad) {
   constexpr int CH = kChunkF32;
   const int chunk = blockIdx.x;
@@ -118,7 +145,7 @@ __global__ void __launch_bounds__(kBlock) k_sigma_chunks64(DevCfg c, DenseArgs a
   }
   const int Sf = c.stride >> 2;
   double tot = 0.0;
-  Nodes64 nd;
+  Nodes64<NA> nd;
   int ic_have = -1;
   for (int ib = cs; ib < ce; ib += Sf) {
     const int ie = min(ib + Sf, ce);
@@ -127,9 +154,9 @@ __global__ void __launch_bounds__(kBlock) k_sigma_chunks64(DevCfg c, DenseArgs a
     if (ic != ic_have) { if (ic_have < 0) nodes64_load(c, a, p, ic, nd); else nodes64_advance(c, a, p, ic, nd); ic_have = ic; }
     double sg = 0.0;
     if (!lane_out) {                                           // (a lane outside its window holds zeros or unused nodes)
-      double cf[4][4];
-      sub_amps64(nd, (ib >> (c.log2_stride - 2)) & 3, cf);
-      sg = sigma_sub64(c, ad, cf, ib, ie, jlo, jhi, c.n_bins);
+      double cf[NA][4];
+      sub_amps64<NA>(nd, (ib >> (c.log2_stride - 2)) & 3, cf);
+      sg = sigma_sub64<NA>(c, ad, cf, ib, ie, jlo, jhi, c.n_bins);
     }
     ad.sub_sigma[(size_t)(ib >> (c.log2_stride - 2)) * a.P_pad + p] = sg;
     tot += sg;
@@ -162,6 +189,7 @@ __global__ void k_scan_chunks(double* __restrict__ cbase, int n_chunks, int P_pa
 // resolved by the WHOLE WARP for that lane: the lane's cubic coefficients are broadcast, the 32 lanes evaluate 32 bins at
 // a time in FP64 and a warp scan gives the cumulative sums (a lane walking its own bins alone would run at 1/32 efficiency).
 __device__ __forceinline__ double shfl_d(double v, int src) { return __shfl_sync(0xffffffffu, v, src); }
+template <int NA = 4>
 __global__ void __launch_bounds__(kBlock) k_edges64(DevCfg c, DenseArgs a, AdaptArgs ad) {
   constexpr int CH = kChunkF32;
   const int chunk = blockIdx.x;
@@ -183,7 +211,7 @@ __global__ void __launch_bounds__(kBlock) k_edges64(DevCfg c, DenseArgs a, Adapt
   const double hS = 1.0 / (double)Sf;
   double t_next = (k < k1) ? seg_target(C, k + 1, N) - cb0 : INFINITY;
   double crel = 0.0;
-  Nodes64 nd;
+  Nodes64<NA> nd;
   int ic_have = -1;
   for (int ib = cs; ib < ce; ib += Sf) {
     const int ie = min(ib + Sf, ce);
@@ -196,15 +224,15 @@ __global__ void __launch_bounds__(kBlock) k_edges64(DevCfg c, DenseArgs a, Adapt
     unsigned todo = __ballot_sync(0xffffffffu, cross);
     if (!cross) crel += sg_s;
     if (!todo) continue;
-    double cf[4][4];
-    sub_amps64(nd, (ib >> (c.log2_stride - 2)) & 3, cf);
+    double cf[NA][4];
+    sub_amps64<NA>(nd, (ib >> (c.log2_stride - 2)) & 3, cf);
     while (todo) {
       const int L = __ffs(todo) - 1;
       todo &= todo - 1;
       // lane L's problem, held by every lane
-      double g[4][4];
+      double g[NA][4];
 #pragma unroll
-      for (int r = 0; r < 4; ++r)
+      for (int r = 0; r < NA; ++r)
 #pragma unroll
         for (int m = 0; m < 4; ++m) g[r][m] = shfl_d(cf[r][m], L);
       const double C_L = shfl_d(C, L), cb0_L = shfl_d(cb0, L);
@@ -220,7 +248,7 @@ __global__ void __launch_bounds__(kBlock) k_edges64(DevCfg c, DenseArgs a, Adapt
       for (int j0 = ib; j0 < ie && k_L < k1_L; j0 += 32) {
         const int j = j0 + lane;
         double sj = 0.0;
-        if (j < ie && j >= jlo_L && j < jhi_L) sj = sigma_bin64(g, (double)(j - ib) * hS, ad.G64[j]);
+        if (j < ie && j >= jlo_L && j < jhi_L) sj = sigma_bin64<NA>(g, (double)(j - ib) * hS, ad.G64[j], NA == 6 ? ad.GT64[j].x : 0.0);
         double inc = sj;                                       // inclusive warp scan, fixed order
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) { const double up = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += up; }
@@ -241,11 +269,15 @@ __global__ void __launch_bounds__(kBlock) k_edges64(DevCfg c, DenseArgs a, Adapt
   while (k < k1) { ++k; if (erow) erow[k] = ce; }   // targets the scanned sums place in this chunk (rounding): at its end
 }
 
-template <int SC, bool MERGE = false>
-__global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2_ad(DevCfg c, DenseArgs a, AdaptArgs ad,
-                                                                      const ulonglong2* __restrict__ Dg) {
+// NA = 6 (three-channel handles): the pair loop, the masked pairs and the moments of k_dense3; Dg = the fused records
+// (wA, wE, wT), Gp = the sigma weights per bin pair (masked pairs only); no merged coarse intervals.
+template <int SC, bool MERGE = false, int NA = 4>
+__global__ void __launch_bounds__(kBlock, NA == 6 ? SC_DENSE3_MINB : SC_DENSE2_MINB)
+k_dense2_ad(DevCfg c, DenseArgs a, AdaptArgs ad, const ulonglong2* __restrict__ Dg, const ulonglong2* __restrict__ Gp = nullptr) {
+  static_assert(!(MERGE && NA == 6), "merged coarse intervals are a two-channel variant");
   constexpr int CH = kChunkF32;
-  __shared__ ulonglong2 sD[CH / 2 * kPairRec];
+  constexpr int kRec = (NA == 6) ? kPairRec3 : kPairRec;
+  __shared__ ulonglong2 sD[CH / 2 * kRec];
   const int chunk = blockIdx.x;
   const int cs = chunk * CH;
   const int ce = min(cs + CH, c.n_bins);
@@ -261,9 +293,9 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2_ad(DevCfg c, 
     return;
   }
   {
-    const ulonglong2* src = Dg + (size_t)(cs >> 1) * kPairRec;
+    const ulonglong2* src = Dg + (size_t)(cs >> 1) * kRec;
 #pragma unroll 4
-    for (int t = threadIdx.x; t < CH / 2 * kPairRec; t += kBlock) sD[t] = src[t];
+    for (int t = threadIdx.x; t < CH / 2 * kRec; t += kBlock) sD[t] = src[t];
   }
   __syncthreads();
 
@@ -272,6 +304,15 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2_ad(DevCfg c, 
   const u64 h2 = f2bcast(2.0f * hS);
   const u64 K2 = f2bcast(1.4629180792671596e-09f);
   const int N = ad.n_seg;
+  // the channel-count-specific pieces of the walk
+  auto sig_mom = [&](const float (&cfx)[NA][4], const ulonglong2* m, const ulonglong2* mT, size_t idx) -> double {
+    if constexpr (NA == 6) return sigma_moments3(cfx, m + idx * 4, mT + idx * 4);
+    else return sigma_moments(cfx, m + idx * 4);
+  };
+  auto run_pairs = [&](PhaseFD& phx, const float (&cfx)[NA][4], u64& s2x, const ulonglong2*& recx, int n, u64& zr2, u64& zi2) {
+    if constexpr (NA == 6) pairs_fast3<SC>(phx, cfx, s2x, recx, n, h2, K2, zr2, zi2);
+    else pairs_fast<SC>(phx, cfx, s2x, recx, n, h2, K2, zr2, zi2);
+  };
   const int Gs = 1 << ad.lg_group;
 
   const double C = ad.cbase[(size_t)ad.n_chunks * a.P_pad + p];
@@ -313,7 +354,7 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2_ad(DevCfg c, 
     const bool all_in = __all_sync(0xffffffffu, lane_in);
     const bool all_out = __all_sync(0xffffffffu, lane_out);
     if (all_out) continue;
-    float cf[4][4];
+    float cf[NA][4];
     // merged coarse intervals as in k_dense2 (the group and sub-interval moments stay those of the fine sub-intervals)
     if constexpr (MERGE) {
       if (merged_left == 0 && (ib & (c.stride - 1)) == 0 && ib + c.stride <= ce2 &&
@@ -329,19 +370,20 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2_ad(DevCfg c, 
       --merged_left;
     } else {
       sub_phase(c, a, p, ib, ph);
-      sub_amps<double>(c, a, p, ib, cf);
+      if constexpr (NA == 6) sub_amps3<double>(c, a, p, ib, cf);
+      else sub_amps<double>(c, a, p, ib, cf);
     }
     u64 s2 = f2pack(0.0f, hS);
-    const ulonglong2* rec = sD + ((ib - cs) >> 1) * kPairRec;
+    const ulonglong2* rec = sD + ((ib - cs) >> 1) * kRec;
     // First ask the question for the whole sub-interval (its moments are those k_sigma_chunks used): if no lane reaches its
     // next target in it, all its groups take the unmasked path and the group moments are not needed at all.
     if (all_in && ie - ib == Sf) {
       const bool cross_s = j_next < ie;          // (an edge AT ie is closed by the first bin of the next sub-interval)
       if (!__any_sync(0xffffffffu, cross_s)) {
-        const double sg_s = sigma_moments(cf, ad.smom + (size_t)(ib >> (c.log2_stride - 2)) * 4);
+        const double sg_s = sig_mom(cf, ad.smom, ad.smomT, (size_t)(ib >> (c.log2_stride - 2)));
         for (int gs = ib; gs < ie; gs += Gs) {
           u64 zr2 = 0, zi2 = 0;
-          pairs_fast<SC>(ph, cf, s2, rec, Gs >> 1, h2, K2, zr2, zi2);
+          run_pairs(ph, cf, s2, rec, Gs >> 1, zr2, zi2);
           float zrl, zrh, zil, zih;
           f2unpack(zr2, zrl, zrh); f2unpack(zi2, zil, zih);
           Zr += (double)(zrl + zrh); Zi += (double)(zil + zih);
@@ -354,9 +396,9 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2_ad(DevCfg c, 
       const int ge = min(gs + Gs, ie);
       const bool slow = !all_in || __any_sync(0xffffffffu, j_next < ge);   // a lane has an edge inside this group
       if (!slow) {
-        const double sg_m = sigma_moments(cf, ad.gmom + (size_t)(gs >> ad.lg_group) * 4);
+        const double sg_m = sig_mom(cf, ad.gmom, ad.gmomT, (size_t)(gs >> ad.lg_group));
         u64 zr2 = 0, zi2 = 0;
-        pairs_fast<SC>(ph, cf, s2, rec, (ge - gs) >> 1, h2, K2, zr2, zi2);
+        run_pairs(ph, cf, s2, rec, (ge - gs) >> 1, zr2, zi2);
         float zrl, zrh, zil, zih;
         f2unpack(zr2, zrl, zrh); f2unpack(zi2, zil, zih);
         Zr += (double)(zrl + zrh); Zi += (double)(zil + zih);
@@ -364,7 +406,8 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2_ad(DevCfg c, 
       } else {
         for (int jj = gs; jj < ge; jj += 2) {
           u64 zr2 = 0, zi2 = 0, sg2 = 0;
-          pair_eval<true, true, SC>(ph, cf, s2, rec, jj, jlo, jhi, h2, K2, zr2, zi2, sg2);
+          if constexpr (NA == 6) pair_eval3<SC>(ph, cf, s2, rec, Gp + (size_t)(jj >> 1) * 2, jj, jlo, jhi, h2, K2, zr2, zi2, sg2);
+          else pair_eval<true, true, SC>(ph, cf, s2, rec, jj, jlo, jhi, h2, K2, zr2, zi2, sg2);
           float zrl, zrh, zil, zih, sgl, sgh;
           f2unpack(zr2, zrl, zrh); f2unpack(zi2, zil, zih); f2unpack(sg2, sgl, sgh);
           while (j_next <= jj) close_at(jj);                      // edges at this bin (several: empty segments)

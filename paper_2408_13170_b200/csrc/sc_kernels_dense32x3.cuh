@@ -35,17 +35,18 @@ __global__ void k_fuse3(const float4* __restrict__ D_ae, const float4* __restric
 }
 
 // Cubic coefficients of (Ar, Ai, Er, Ei, Tr, Ti) on the fine sub-interval starting at ib, in s = (j - ib)/Sf (see sub_amps).
+template <typename NT = float>   // element type of the node table (double in the per-particle-segment path)
 __device__ __forceinline__ void sub_amps3(const DevCfg& c, const DenseArgs& a, int p, int ib, float (&cf)[6][4]) {
   const int i0 = (ib >> c.log2_stride) + kNodeOff;
   const int q = (ib >> (c.log2_stride - 2)) & 3;
-  const float* __restrict__ namp = reinterpret_cast<const float*>(a.node_amp);
+  const NT* __restrict__ namp = reinterpret_cast<const NT*>(a.node_amp);
 #pragma unroll
   for (int r = 0; r < 6; r += 2) {
-    const float* col = namp + ((size_t)i0 * 6 + r) * a.P_pad + p;
+    const NT* col = namp + ((size_t)i0 * 6 + r) * a.P_pad + p;
     const ptrdiff_t st = (ptrdiff_t)6 * a.P_pad;
     u64 nd[6], o[4];
 #pragma unroll
-    for (int m = -2; m <= 3; ++m) nd[m + 2] = f2pack(col[m * st], col[m * st + a.P_pad]);
+    for (int m = -2; m <= 3; ++m) nd[m + 2] = f2pack((float)col[m * st], (float)col[m * st + a.P_pad]);
     fine_cubic2(nd, q, o);
 #pragma unroll
     for (int kk = 0; kk < 4; ++kk) f2unpack(o[kk], cf[r][kk], cf[r + 1][kk]);
@@ -88,6 +89,13 @@ __device__ __forceinline__ void pair_eval3(PhaseFD& ph, const float (&cf)[6][4],
   mac_pair3(cf, s2c, rec[0], rec[1], rec[2], h2, cr2, sr2, zr2, zi2);
   s2 = s2c;
   rec += kPairRec3;
+}
+
+// sigma of a run of bins from the moments of its weights, three channels: (A, E) packed as in sigma_moments, then (T, 0)
+__device__ __forceinline__ double sigma_moments3(const float (&cf)[6][4], const ulonglong2* __restrict__ mp, const ulonglong2* __restrict__ mpT) {
+  const float cT[4][4] = {{cf[4][0], cf[4][1], cf[4][2], cf[4][3]}, {cf[5][0], cf[5][1], cf[5][2], cf[5][3]},
+                          {0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
+  return sigma_moments(*reinterpret_cast<const float(*)[4][4]>(&cf[0]), mp) + sigma_moments(cT, mpT);
 }
 
 // n >= 1 consecutive unmasked pairs, software-pipelined like pairs_fast
@@ -190,12 +198,7 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE3_MINB) k_dense3(DevCfg c, Den
     }
     u64 s2 = 0;        // (s_j, s_{j+1}) of the next pair
     const ulonglong2* rec = sD;   // its data records
-    auto sigma_piece = [&](int piece) {
-      const float cT[4][4] = {{cf[4][0], cf[4][1], cf[4][2], cf[4][3]}, {cf[5][0], cf[5][1], cf[5][2], cf[5][3]},
-                              {0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
-      Sg += sigma_moments(*reinterpret_cast<const float(*)[4][4]>(&cf[0]), a.moments + (size_t)piece * 4)
-          + sigma_moments(cT, a.momentsT + (size_t)piece * 4);
-    };
+    auto sigma_piece = [&](int piece) { Sg += sigma_moments3(cf, a.moments + (size_t)piece * 4, a.momentsT + (size_t)piece * 4); };
     const bool use_mom = all_in;      // all lanes inside their windows: sigma from the piece moments, unmasked pairs
     int piece = use_mom ? a.piece_first[(ib >> (c.log2_stride - 2)) - ((a.chunk_first * CH) >> (c.log2_stride - 2))] : 0;
     float car_zr = 0.f, car_zi = 0.f, car_sg = 0.f;

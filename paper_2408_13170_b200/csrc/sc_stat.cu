@@ -85,6 +85,7 @@ struct sc_handle : EdgeCache {
   // adaptive (per-particle) segments: moments of the weights over groups and fine sub-intervals, cached per node spacing
   int ad_lg = 0; float2* d_gmom = nullptr; float2* d_smom = nullptr; size_t gmom_cap = 0, smom_cap = 0;
   double2* d_gmom64 = nullptr; double2* d_smom64 = nullptr; size_t gmom64_cap = 0, smom64_cap = 0;   // FP64 copies (edge decision)
+  float2* d_gmomT = nullptr; float2* d_smomT = nullptr; double2* d_smom64T = nullptr; size_t gmomT_cap = 0, smomT_cap = 0, smom64T_cap = 0;   // ... of the T weights (three-channel handles)
   int* d_ad_edges = nullptr; size_t ad_edges_cap = 0;    // the edges of a batch when the caller does not ask for them
   // scratch
   void* scratch = nullptr; size_t scratch_bytes = 0;
@@ -660,6 +661,9 @@ int run_adaptive(sc_handle* h, const double* params, int64_t P, int n_seg, doubl
                  cudaStream_t st) {
   DevCfg dc = h->dc;
   apply_stride(dc, h->lg_f32);
+  const bool three = (h->sub != nullptr);        // three-channel handle: (A, E, T) in every step (NA = 6 amplitude fields)
+  if (three) dc.chan_set = 2;
+  const int NA = three ? 6 : 4;
   const int CH = kChunkF32;
   const int n_nodes = dc.n_nodes;
   const int n_chunks = (dc.n_bins + CH - 1) / CH;
@@ -677,10 +681,19 @@ int run_adaptive(sc_handle* h, const double* params, int64_t P, int n_seg, doubl
     if ((rc = check_launch(h, "k_moments"))) return rc;
     k_moments<<<(n_sub + 127) / 128, 128, 0, st>>>(h->G64, nullptr, (const int*)(size_t)lg_fine, n_sub, dc.n_bins, lg_fine, h->d_smom, h->d_smom64);
     if ((rc = check_launch(h, "k_moments"))) return rc;
+    if (three) {
+      if ((rc = grow(h, (void**)&h->d_gmomT, &h->gmomT_cap, (size_t)n_groups * 8 * sizeof(float2)))) return rc;
+      if ((rc = grow(h, (void**)&h->d_smomT, &h->smomT_cap, (size_t)n_sub * 8 * sizeof(float2)))) return rc;
+      if ((rc = grow(h, (void**)&h->d_smom64T, &h->smom64T_cap, (size_t)n_sub * 7 * sizeof(double2)))) return rc;
+      k_moments<<<(n_groups + 127) / 128, 128, 0, st>>>(h->GT64, nullptr, (const int*)(size_t)lg_group, n_groups, dc.n_bins, lg_fine, h->d_gmomT, nullptr);
+      if ((rc = check_launch(h, "k_moments"))) return rc;
+      k_moments<<<(n_sub + 127) / 128, 128, 0, st>>>(h->GT64, nullptr, (const int*)(size_t)lg_fine, n_sub, dc.n_bins, lg_fine, h->d_smomT, h->d_smom64T);
+      if ((rc = check_launch(h, "k_moments"))) return rc;
+    }
     h->ad_lg = dc.log2_stride;
   }
   // (FP64 node amplitudes: the edge decision is taken in FP64; the packed kernel converts them as it reads)
-  const size_t per_p = 2 * ((size_t)kPcFields * 8 + 8) + 16 + (size_t)n_nodes * (4 + 8 + 4 * sizeof(double))
+  const size_t per_p = 2 * ((size_t)kPcFields * 8 + 8) + 16 + (size_t)n_nodes * (4 + 8 + NA * sizeof(double))
                        + (size_t)(n_chunks + 1) * 8 + (size_t)n_chunks * kFragAd * 8 + (size_t)n_sub * 8;
   int64_t Pb_max = (int64_t)(h->scratch_cap / per_p) / kBlock * kBlock;
   if (Pb_max < kBlock) Pb_max = kBlock;
@@ -694,7 +707,7 @@ int run_adaptive(sc_handle* h, const double* params, int64_t P, int n_seg, doubl
   int* jhi = (int*)take((size_t)4 * P_pad);
   int* node_n = (int*)take((size_t)n_nodes * 4 * P_pad);
   double* node_frac = (double*)take((size_t)n_nodes * 8 * P_pad);
-  double* node_amp = (double*)take((size_t)n_nodes * 4 * sizeof(double) * P_pad);
+  double* node_amp = (double*)take((size_t)n_nodes * NA * sizeof(double) * P_pad);
   double* cbase = (double*)take((size_t)(n_chunks + 1) * 8 * P_pad);
   double* frag = (double*)take((size_t)n_chunks * kFragAd * 8 * P_pad);
   double* sub_sigma = (double*)take((size_t)n_sub * 8 * P_pad);
@@ -745,7 +758,8 @@ int run_adaptive(sc_handle* h, const double* params, int64_t P, int n_seg, doubl
     {
       Timed tm(h, st, SC_TIME_NODES);
       // (the consumers read a node only where a lane of the warp is inside its window: skip_unreached)
-      k_nodes<double><<<dim3((n_nodes + kNodesPerCta - 1) / kNodesPerCta, (P_pad + 127) / 128), 128, 0, st>>>(dc, pc, jlo, jhi, P_pad, node_n, node_frac, node_amp, nullptr, 0, 1);
+      if (three) k_nodes<double, false, 6><<<dim3((n_nodes + kNodesPerCta - 1) / kNodesPerCta, (P_pad + 127) / 128), 128, 0, st>>>(dc, pc, jlo, jhi, P_pad, node_n, node_frac, node_amp, nullptr, 0, 1);
+      else k_nodes<double><<<dim3((n_nodes + kNodesPerCta - 1) / kNodesPerCta, (P_pad + 127) / 128), 128, 0, st>>>(dc, pc, jlo, jhi, P_pad, node_n, node_frac, node_amp, nullptr, 0, 1);
     }
     if ((rc = check_launch(h, "k_nodes"))) return rc;
     DenseArgs a = {};
@@ -758,14 +772,18 @@ int run_adaptive(sc_handle* h, const double* params, int64_t P, int n_seg, doubl
     ad.out_edges = out_edges ? out_edges + (size_t)pb * (n_seg + 1) : h->d_ad_edges;
     ad.pmap = sorted ? pmap : nullptr;
     ad.smom64 = h->d_smom64; ad.gmom64 = h->d_gmom64; ad.G64 = h->G64; ad.sub_sigma = sub_sigma;
+    ad.gmomT = reinterpret_cast<const ulonglong2*>(h->d_gmomT); ad.smomT = reinterpret_cast<const ulonglong2*>(h->d_smomT);
+    ad.smom64T = h->d_smom64T; ad.GT64 = h->GT64;
     const dim3 grid(n_chunks, P_pad / kBlock);
     {
       Timed tm(h, st, SC_TIME_OTHER);
-      k_sigma_chunks64<<<grid, kBlock, 0, st>>>(dc, a, ad);
+      if (three) k_sigma_chunks64<6><<<grid, kBlock, 0, st>>>(dc, a, ad);
+      else k_sigma_chunks64<4><<<grid, kBlock, 0, st>>>(dc, a, ad);
       if ((rc = check_launch(h, "k_sigma_chunks64"))) return rc;
       k_scan_chunks<<<(P_pad + 127) / 128, 128, 0, st>>>(cbase, n_chunks, P_pad);
       if ((rc = check_launch(h, "k_scan_chunks"))) return rc;
-      k_edges64<<<grid, kBlock, 0, st>>>(dc, a, ad);
+      if (three) k_edges64<6><<<grid, kBlock, 0, st>>>(dc, a, ad);
+      else k_edges64<4><<<grid, kBlock, 0, st>>>(dc, a, ad);
       if ((rc = check_launch(h, "k_edges64"))) return rc;
     }
     {
@@ -773,7 +791,13 @@ int run_adaptive(sc_handle* h, const double* params, int64_t P, int n_seg, doubl
       const ulonglong2* Dp = reinterpret_cast<const ulonglong2*>(h->D32);
       const bool merge = dc.stride >= 512;                     // as in run_batches
       a.merge_lim = 86400.0 * (kNodeDaysF32 / 4.0) / h->cfg.T_obs_s;
-      if (sincos == 2 && merge) k_dense2_ad<2, true><<<grid, kBlock, 0, st>>>(dc, a, ad, Dp);
+      if (three) {
+        const ulonglong2* D3p = reinterpret_cast<const ulonglong2*>(h->D3);
+        const ulonglong2* Gp = reinterpret_cast<const ulonglong2*>(h->Gp3);
+        if (sincos == 2) k_dense2_ad<2, false, 6><<<grid, kBlock, 0, st>>>(dc, a, ad, D3p, Gp);
+        else k_dense2_ad<0, false, 6><<<grid, kBlock, 0, st>>>(dc, a, ad, D3p, Gp);
+      }
+      else if (sincos == 2 && merge) k_dense2_ad<2, true><<<grid, kBlock, 0, st>>>(dc, a, ad, Dp);
       else if (sincos == 2) k_dense2_ad<2><<<grid, kBlock, 0, st>>>(dc, a, ad, Dp);
       else if (merge) k_dense2_ad<0, true><<<grid, kBlock, 0, st>>>(dc, a, ad, Dp);
       else k_dense2_ad<0><<<grid, kBlock, 0, st>>>(dc, a, ad, Dp);
@@ -1013,7 +1037,6 @@ int sc_eval_stat_adaptive(sc_handle* h, const double* params, int64_t P, int32_t
   if (!params || P <= 0 || n_seg <= 0 || (!out && !out3)) return fail(h, SC_ERR_INVALID_ARG, "null pointer, n_particles <= 0 or n_seg <= 0");
   if (n_seg > h->cfg.n_bins) return fail(h, SC_ERR_INVALID_ARG, "n_seg exceeds n_bins");
   cudaStream_t st = (cudaStream_t)stream;
-  if (h->sub && n_seg > 1) return fail(h, SC_ERR_INVALID_ARG, "per-particle segments are not available on three-channel handles");
   if (n_seg == 1) {                              // one segment: the edges are (0, n_bins) for every particle
     const int32_t e[2] = {0, (int32_t)h->cfg.n_bins};
     int rc = eval_any(h, params, P, e, 1, out, nullptr, stream, false, out3);
@@ -1047,7 +1070,6 @@ int sc_search_run(sc_handle* h, const sc_search_config* sc, double* pos, double*
     return fail(h, SC_ERR_INVALID_ARG, "conv_window, max_iters_per_rung must be >= 1 and kmeans_max_iters >= 0");
   for (int r = 0; r < sc->n_rungs; ++r)
     if (sc->n_seg[r] < 1 || sc->n_seg[r] > h->cfg.n_bins) return fail(h, SC_ERR_INVALID_ARG, "n_seg[%d] out of range", r);
-  if (h->sub && sc->adaptive_edges) return fail(h, SC_ERR_INVALID_ARG, "per-particle segments are not available on three-channel handles");
   cudaStream_t st = (cudaStream_t)stream;
   const int S = n_swarms;
   const int64_t nb = h->cfg.n_bins;
@@ -1146,7 +1168,7 @@ int sc_search_run(sc_handle* h, const sc_search_config* sc, double* pos, double*
       SC_S(cudaMalloc(&ed, (size_t)S * (N + 1) * 4));
       rc = sc_eval_stat_adaptive(h, gbest_pos, S, N, stat, ed, nullptr, stream);
       for (int s = 0; s < S && !rc; ++s)
-        rc = eval_common(h, gbest_pos + (size_t)s * 8, 1, ed + (size_t)s * (N + 1), N, stat + s, nullptr, stream, false);
+        rc = eval_any(h, gbest_pos + (size_t)s * 8, 1, ed + (size_t)s * (N + 1), N, stat + s, nullptr, stream, false);
       cudaStreamSynchronize(st);
       cudaFree(ed);
     } else rc = eval_any(h, gbest_pos, S, e.data(), N, stat, nullptr, stream, false);
@@ -1526,7 +1548,7 @@ int sc_free(sc_handle* h) {
   if (h->sub) sc_free(h->sub);
   cudaFree(h->d_seg3);
   cudaFree(h->D32); cudaFree(h->W64); cudaFree(h->G64); cudaFree(h->d_tc_img); cudaFree(h->D3); cudaFree(h->Gp3); cudaFree(h->GT64);
-  cudaFree(h->d_momentsT); cudaFree(h->alt.d_momentsT);
+  cudaFree(h->d_momentsT); cudaFree(h->alt.d_momentsT); cudaFree(h->d_gmomT); cudaFree(h->d_smomT); cudaFree(h->d_smom64T);
   cudaFree(h->scratch); cudaFree(h->d_edges); cudaFree(h->d_chunk_k0); cudaFree(h->d_flags);
   cudaFree(h->d_counter); cudaFree(h->d_params_stage); cudaFree(h->d_comp); cudaFree(h->d_km); cudaFree(h->d_T64); cudaFree(h->d_T32); cudaFree(h->d_sp);
   cudaFree(h->d_spsig); cudaFree(h->d_zpart); cudaFree(h->d_hh); cudaFree(h->d_gmom); cudaFree(h->d_smom);

@@ -138,18 +138,41 @@ def test_three_channel_escalation_of_ill_conditioned_particles(oracle, N):
     assert rel_err(auto[ok], ref[ok]).max() <= TOL
 
 
+@pytest.mark.parametrize("N", [2, 10, 50, 100, 1000])
+def test_c1_three_channels_adaptive_segments(oracle, N):
+    """Per-particle equal-SNR^2 segments over A, E, T (PAPER.md:120 with the channel sums of PAPER.md:36, 59 -- the paper's
+    own configuration): the device decides the integer edges in FP64 from all three channels; they must EQUAL
+    sco_equal_snr_edges3, and the statistic and the components must match the oracle on those edges."""
+    torch, sc, inp, cfgd, cfg, S3, d3, th, kappa, h3, H = _setup(oracle, 1, None, 20.0, 907)
+    nb = cfgd["n_bins"]
+    parts = np.vstack([inp["particles"], th[None, :]])
+    par = _dev(torch, parts)
+    got, ged, comp = H.eval_stat_adaptive(par, N, want_edges=True, want_comp=True)
+    got, ged, comp = got.cpu().numpy(), ged.cpu().numpy().astype(np.int64), comp.cpu().numpy()
+    H.close()
+    ref_own, oed = oracle.eval_stat_adaptive3(cfg, d3, S3, parts, N, want_edges=True)
+    assert np.all(ged[:, 0] == 0) and np.all(ged[:, -1] == nb) and np.all(np.diff(ged, axis=1) >= 0)
+    d = np.abs(ged - oed)
+    assert np.array_equal(ged, oed), (int(d.max()), float((d != 0).mean()))
+    ref, rc = oracle.eval_stat_adaptive3(cfg, d3, S3, parts, N, in_edges=ged, want_comp=True)
+    assert rel_err(got, ref).max() <= TOL, (N, rel_err(got, ref).max())
+    assert rel_err(comp, rc).max() <= TOL
+    # the T channel moves the edges: the two-channel rule on the same templates gives other edges somewhere
+    if N >= 50:
+        e2 = oracle.eval_stat_adaptive(oracle.make_config(inp["cfg"]), d3[0], d3[1], S3[0], S3[1], parts[-1:], N, want_edges=True)[1]
+        assert not np.array_equal(e2[0], oed[-1])
+
+
 def test_three_channel_restrictions_and_search(oracle):
     torch, sc, inp, cfgd, cfg, S3, d3, th, kappa, h3, H = _setup(oracle, 1, None, 20.0, 904)
     par = _dev(torch, inp["particles"])
-    with pytest.raises(sc.SCError):
-        H.eval_stat_adaptive(par, 10)
-    got = H.eval_stat_adaptive(par, 1).cpu().numpy()                # one segment needs no edges: allowed
+    got = H.eval_stat_adaptive(par, 1).cpu().numpy()                # one segment: the edges are (0, n_bins)
     assert np.array_equal(got, H.eval_stat(par, np.array([0, cfgd["n_bins"]])).cpu().numpy())
     with pytest.raises(sc.SCError):
         sc.Handle(dict(cfgd, n_channels=2), par, par, par, par, dT=par, S_T=par)
-    # a short equal-width-edges search runs through the three-channel statistic
+    # a short search on the paper's own configuration (A, E, T with per-particle equal-SNR^2 segments) runs through
     hyper = [sy.TABLE_IV[100], sy.TABLE_IV[1]]
-    scfg = sc.ScSearchConfig.make([100, 1], hyper, adaptive_edges=False, conv_window=3, max_iters_per_rung=5, seed=1)
+    scfg = sc.ScSearchConfig.make([100, 1], hyper, adaptive_edges=True, conv_window=3, max_iters_per_rung=5, seed=1)
     P = inp["particles"].shape[0]
     lab = torch.zeros(P, dtype=torch.int32, device="cuda:0")
     res = H.search_run(scfg, par.clone(), _dev(torch, inp["velocities"]), lab, 1, _dev(torch, inp["lo"]), _dev(torch, inp["hi"]))
