@@ -75,6 +75,9 @@ def parse():
     ap.add_argument("--fap", type=int, default=0, metavar="SEEDS",
                     help="extras: run the c4 workload (BASELINE configs[3]: noise only, 10^4 particles x 200 PSO iterations at "
                          "N = 50000/5000/500) over SEEDS noise realisations and report the maximum statistic per seed and level")
+    ap.add_argument("--search-channels", type=int, default=2, choices=[2, 3],
+                    help="with --search: 3 = the search runs on an (A, E, T) handle -- with the per-particle segments of the ladder "
+                         "this is the paper's own configuration (PAPER.md:36, 59, 120); the injection is made in all three channels")
     ap.add_argument("--search-ranking", action="store_true",
                     help="with --search: sc_search_config.ranking_precision = 1 (all rungs on the FP32 path, bests re-evaluated in FP64)")
     ap.add_argument("--no-extras", action="store_true", help="skip the extra (untimed-region) measurements")
@@ -193,7 +196,7 @@ class ClockSampler:
         return out
 
 
-def run_search(sc, torch, dev, inp, cid, rho, S_A, S_E, nA, nE, max_iters=1000, ranking=0):
+def run_search(sc, torch, dev, inp, cid, rho, S_A, S_E, nA, nE, max_iters=1000, ranking=0, channels=2):
     """One complete search of one tile (Fig. 2): init from the prior, the ladder with Table IV
     hyper-parameters, convergence rule of App. B, k-means regrouping between rungs, threshold Upsilon_1 >= 100.
     c5 (BASELINE configs[4]): its own 4 swarms x 10^4 particles, ladder 50000/5000/500/50/1 on shared equal-width edges, both
@@ -207,16 +210,31 @@ def run_search(sc, torch, dev, inp, cid, rho, S_A, S_E, nA, nE, max_iters=1000, 
     big = sy.config_inputs(cid, P=n_swarms * per_swarm)
     cfg, nb = inp["cfg"], inp["cfg"]["n_bins"]
     t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
-    H0 = sc.Handle(cfg, torch.view_as_real(nA).contiguous(), torch.view_as_real(nE).contiguous(), S_A, S_E)
+    ri = lambda z: torch.view_as_real(z).contiguous()
+    if channels == 3:
+        cfg = dict(cfg, n_channels=3)
+        S_T = t(sy.psd_T(sy.freqs(cfg)))
+        nT = t(sy.draw_noise(sy.MASTER_SEED + 7 + 100 * cid, sy.psd_T(sy.freqs(cfg)), inp["df"]))
+        H0 = sc.Handle(cfg, ri(nA), ri(nE), S_A, S_E, dT=ri(nT), S_T=S_T)
+    else:
+        H0 = sc.Handle(cfg, ri(nA), ri(nE), S_A, S_E)
     dA, dE, snrs = nA.clone(), nE.clone(), []
+    dT = nT.clone() if channels == 3 else None
     for inj in inp["injections"]:
-        hA, hE = H0.gen_template(t(inj["theta"][None, :]))
+        if channels == 3:
+            hA, hE, hT = H0.gen_template3(t(inj["theta"][None, :]))
+        else:
+            hA, hE = H0.gen_template(t(inj["theta"][None, :]))
         rho2 = 4.0 * inp["df"] * ((hA[0].abs() ** 2 / S_A).sum() + (hE[0].abs() ** 2 / S_E).sum())
+        if channels == 3:
+            rho2 = rho2 + 4.0 * inp["df"] * (hT[0].abs() ** 2 / S_T).sum()
         snrs.append(float(inj["rho"] if cid == 5 else rho))
         dA += snrs[-1] / torch.sqrt(rho2) * hA[0]
         dE += snrs[-1] / torch.sqrt(rho2) * hE[0]
+        if channels == 3:
+            dT += snrs[-1] / torch.sqrt(rho2) * hT[0]
     H0.close()
-    H = sc.Handle(cfg, torch.view_as_real(dA).contiguous(), torch.view_as_real(dE).contiguous(), S_A, S_E)
+    H = sc.Handle(cfg, ri(dA), ri(dE), S_A, S_E, dT=ri(dT), S_T=S_T) if channels == 3 else sc.Handle(cfg, ri(dA), ri(dE), S_A, S_E)
     H.set_option(sc.SC_OPT_TC_MAX_S, int(np.ceil(big["hi"][2])))
     hyper = [dict(sy.TABLE_IV[min(sy.TABLE_IV, key=lambda k: abs(np.log(k) - np.log(N)))]) for N in ladder]
     scfg = sc.ScSearchConfig.make(ladder, hyper, adaptive_edges=adaptive, max_iters_per_rung=max_iters, seed=2408, threshold=100.0,
@@ -234,7 +252,7 @@ def run_search(sc, torch, dev, inp, cid, rho, S_A, S_E, nA, nE, max_iters=1000, 
     b = int(np.argmax(res["best_val"]))
     near = int(np.argmin(np.abs(ths[:, 0] - res["best_pos"][b, 0])))          # the injection the best swarm sits on
     iters = [int(x) for x in res["iters_per_rung"]]
-    return {"what": f"sc_search_run on the c{cid} tile: {n_swarms} swarms x {per_swarm} particles, ladder {ladder}, "
+    return {"what": f"sc_search_run on the c{cid} tile ({'A, E, T' if channels == 3 else 'A, E'}): {n_swarms} swarms x {per_swarm} particles, ladder {ladder}, "
                     + ("per-particle equal-SNR^2 segments" if adaptive else "shared equal-width segments")
                     + f", Table IV hyper-parameters, injection SNRs {snrs}, ranking_precision = {ranking}",
             "wall_s": wall, "iters_per_rung": iters, "particle_bin_evals": float(sum(iters)) * n_swarms * per_swarm * nb,
@@ -493,7 +511,8 @@ def run_ours(args, rank, local_rank, world):
 
     # ---- extras (opt-in): one complete hierarchical search at the paper's scale (context for PAPER.md:365-367)
     if args.search > 0 and rank == 0 and inp["injections"]:
-        extras["hierarchical_search"] = run_search(sc, torch, dev, inp, cid, args.search, S_A, S_E, nA, nE, ranking=int(args.search_ranking))
+        extras["hierarchical_search"] = run_search(sc, torch, dev, inp, cid, args.search, S_A, S_E, nA, nE, ranking=int(args.search_ranking),
+                                                  channels=args.search_channels)
     if args.fap > 0 and rank == 0:
         extras["false_alarm_background"] = run_fap(sc, torch, dev, 4, args.fap)
 
