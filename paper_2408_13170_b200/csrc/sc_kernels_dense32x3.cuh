@@ -119,7 +119,7 @@ __device__ __forceinline__ void pairs_fast3(PhaseFD& ph, const float (&cf)[6][4]
 }
 
 #ifndef SC_DENSE3_MINB
-#define SC_DENSE3_MINB 3     /* CTAs per SM (168 registers/thread: six cubics live in the pair loop) */
+#define SC_DENSE3_MINB 4     /* CTAs per SM: 128 registers/thread with ~150 B of spills beats 168 registers at 3 CTAs (28.6 vs 32.0 ms on c3) */
 #endif
 template <bool SEG, int SC>
 __global__ void __launch_bounds__(kBlock, SC_DENSE3_MINB) k_dense3(DevCfg c, DenseArgs a, const ulonglong2* __restrict__ Dg,
