@@ -163,6 +163,32 @@ def test_c1_three_channels_adaptive_segments(oracle, N):
         assert not np.array_equal(e2[0], oed[-1])
 
 
+def test_c3_three_channels_bench_configuration(oracle):
+    """The bench's three-channel extra at full size: c3 (4 yr, 1.64 M bins, node stride 512), whole population through the
+    one-pass kernel at N = 5000 and through the per-particle-segment kernels at N = 100; the oracle (truth mode) on a sample."""
+    torch, sc, inp, cfgd, cfg, S3, d3, th, kappa, h3, H = _setup(oracle, 3, None, 17.0, 908)
+    H.set_option(sc.SC_OPT_TC_MAX_S, int(np.ceil(inp["hi"][2])))
+    P = inp["particles"].shape[0]
+    par = _dev(torch, inp["particles"])
+    cfg_t = oracle.make_config(cfgd, truth=True)
+    e = sy.edges(cfgd["n_bins"], 5000)
+    got = H.eval_stat(par, e).cpu().numpy()
+    idx = np.unique(np.concatenate([np.random.default_rng(12).choice(P, 12, replace=False), np.argsort(got)[:4]]))
+    ref = oracle.eval_stat3(cfg_t, d3, S3, inp["particles"][idx], e)
+    assert rel_err(got[idx], ref).max() <= TOL, rel_err(got[idx], ref).max()
+    assert np.all(np.isfinite(got)) and np.all(got >= 0)
+    # per-particle segments over the three channels
+    ga, ged = H.eval_stat_adaptive(par, 100, want_edges=True)
+    ga, ged = ga.cpu().numpy(), ged.cpu().numpy().astype(np.int64)
+    H.close()
+    sub = idx[:8]
+    ref_own, oed = oracle.eval_stat_adaptive3(cfg, d3, S3, inp["particles"][sub], 100, want_edges=True)
+    dlt = np.abs(ged[sub] - oed)
+    assert dlt.max() <= 1 and (dlt == 0).mean() >= 0.999, (int(dlt.max()), float((dlt != 0).mean()))
+    ref_a = oracle.eval_stat_adaptive3(cfg_t, d3, S3, inp["particles"][sub], 100, in_edges=ged[sub])
+    assert rel_err(ga[sub], ref_a).max() <= TOL, rel_err(ga[sub], ref_a).max()
+
+
 def test_three_channel_restrictions_and_search(oracle):
     torch, sc, inp, cfgd, cfg, S3, d3, th, kappa, h3, H = _setup(oracle, 1, None, 20.0, 904)
     par = _dev(torch, inp["particles"])
