@@ -613,8 +613,12 @@ int eval_any(sc_handle* h, const double* params, int64_t P, const int32_t* seg_e
     // (the tables of the main passes are not needed any more: a call with the fused kernel has none, the two-pass loop has combined its batch)
     if (2 * per_p * (size_t)n_esc > h->seg3_cap && (rc2 = grow(h, (void**)&h->d_seg3, &h->seg3_cap, 2 * per_p * (size_t)n_esc))) return rc2;
     double* eA = h->d_seg3; double* eT = eA + (size_t)n_esc * n_seg * 3;
+    // (the all-FP64 chunking of the same edges lives in the alternate cache, as in eval_common's own escalation pass: the
+    // FP32 kernels' analysis of the list stays valid for the next call)
     h->precision = 2; h->sub->precision = 2;
+    std::swap(static_cast<EdgeCache&>(*h), h->alt);
     rc2 = eval_common(h, h->d_esc_params, n_esc, seg_edges, n_seg, nullptr, eA, stream, true);
+    std::swap(static_cast<EdgeCache&>(*h), h->alt);
     if (!rc2) rc2 = eval_common(h->sub, h->d_esc_params, n_esc, seg_edges, n_seg, nullptr, eT, stream, true);
     h->precision = 0; h->sub->precision = 0;
     if (rc2) return rc2;
