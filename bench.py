@@ -85,6 +85,8 @@ def parse():
                     help="CPU-only check of the multi-rank launch and reductions (gloo); used by tests/test_multi_rank.py")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-window-hint", action="store_true",
+                    help="do not state the measured window fraction (SC_OPT_WINDOW_FRACTION_PPM): node spacing for N' = 8")
     ap.add_argument("--opt", action="append", default=[], metavar="ID=VALUE",
                     help="extra sc_set_option(ID, VALUE) calls on the handle (experiments)")
     return ap.parse_args()
@@ -375,6 +377,14 @@ def run_ours(args, rank, local_rank, world):
             H.eval_stat(state["pos"], e, out=stat)
         H.pso_step(state, stat, lo, hi, eps, hp["omega"], hp["phi_p"], hp["phi_g"], inp["pso_seed"], it, n_swarms)
 
+    # ... and how much of the band its particles' time windows cover, measured with one evaluation before anything is timed
+    # (what sc_search_run does for itself): the node spacing is then set for N' = n_seg x fraction segments per particle
+    win_frac = None
+    if not ad_N and not args.no_window_hint:
+        H.eval_stat(state["pos"], e, out=stat)
+        win_frac = H.counters()[0] / (float(P) * nb)
+        H.set_option(sc.SC_OPT_WINDOW_FRACTION_PPM, int(round(win_frac * 1e6)))
+
     for it in range(args.warmup):
         step(it)
     torch.cuda.synchronize()
@@ -453,6 +463,8 @@ def run_ours(args, rank, local_rank, world):
             H3 = sc.Handle(cfg3, torch.view_as_real(dA).contiguous(), torch.view_as_real(dE).contiguous(), S_A, S_E,
                            dT=torch.view_as_real(nT).contiguous(), S_T=S_T)
             H3.set_option(sc.SC_OPT_TC_MAX_S, int(np.ceil(inp["hi"][2])))
+            if win_frac is not None:
+                H3.set_option(sc.SC_OPT_WINDOW_FRACTION_PPM, int(round(win_frac * 1e6)))
             H3.eval_stat(state["pos"], e, out=stat); torch.cuda.synchronize()
             a_, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             a_.record()
@@ -604,6 +616,7 @@ def run_ours(args, rank, local_rank, world):
                 "config": {"workload": workload_name(cid, spec, cfg, P, N), "l2": "flushed between timed steps "
                            "(256 MiB write); per-step node tables + fragments (~1 GB) exceed L2 anyway",
                            "pso": {k: hp[k] for k in ("omega", "phi_p", "phi_g")}, "n_swarms": n_swarms,
+                           "window_fraction_stated": win_frac,
                            "parallelism": f"independent tiles x{world}" if world > 1 else "1 GPU"},
                 "value_counts": "evaluated (particle, bin) pairs (inside the time windows and [e_0, e_N))",
                 "nominal_particle_bin_per_s": units_nominal / (ms_max * 1e-3),

@@ -67,6 +67,18 @@ enum {
   SC_OPT_TC_MAX_S = 4,       /* the caller's upper bound on t_c [s] over the particles (the search tile's t_c range,
                                 PAPER.md:253); sets the coarse node spacing to about one day of signal time at the
                                 low band edge.  Default 10 yr.                                  */
+  SC_OPT_WINDOW_FRACTION_PPM = 15, /* the caller's statement of the mean share of the band that lies inside a particle's time
+                                window, in parts per million (0 = not stated, default; sc_get_counters after one evaluation gives
+                                evaluated_bins / (n_particles x n_bins)).  With shared edges a particle then has N' = n_seg x fraction
+                                non-empty segments, and the FP32-amplitude path spaces its nodes for that N': the interpolation
+                                errors of the segments are independent, so the error of Upsilon falls like 1/sqrt(N') and the node
+                                spacing may grow like N'^(1/12) at the same modelled error (half the
+                                stated fraction is used).  Not stated: N' = 8, the fewest segments that path is left with.
+                                Particles of such a population that end up with too few segments for the spacing chosen
+                                (Upsilon below twice 8 (days / 4)^12) go to the escalation pass like those below tau.
+                                sc_search_run measures the fraction itself when none is stated.  Per-segment output
+                                (sc_eval_segments) and per-particle segments (sc_eval_stat_adaptive: integer edges from the
+                                interpolated sigma) always keep the N' = 8 spacing. */
   SC_OPT_STRIDE_LOG2 = 5,    /* 0 = automatic (rule above), else log2 of the coarse node spacing in bins (3..12)   */
   SC_OPT_PROFILE = 6,        /* 1 = record a CUDA event pair around every kernel launch (read by sc_get_timing)     */
   SC_OPT_SINCOS = 7,         /* FP32 amplitude path: sin/cos of the phase.  0 = automatic: hardware MUFU sin/cos

@@ -15,6 +15,7 @@ SC_OPT_PRECISION, SC_OPT_F32_MIN_SEG, SC_OPT_SCRATCH_BYTES, SC_OPT_TC_MAX_S, SC_
 SC_OPT_ESCALATE, SC_OPT_ESC_TAU_POLY_X1000, SC_OPT_ESC_TAU_MUFU_X1000, SC_OPT_WINDOW_SORT = 9, 10, 11, 12
 SC_OPT_TENSOR_CORES = 13
 SC_OPT_FUSED_AET = 14
+SC_OPT_WINDOW_FRACTION_PPM = 15
 SC_TIMING_CLASSES = ["nodes", "dense", "stitch", "pso", "other", "escalation"]
 
 EXPORTED_SYMBOLS = ["sc_init_data", "sc_init_data_host", "sc_init_data3", "sc_gen_template3", "sc_eval_stat", "sc_eval_stat_host", "sc_eval_segments",

@@ -72,6 +72,7 @@ struct sc_handle : EdgeCache {
   float4* D32 = nullptr; double4* W64 = nullptr; double2* G64 = nullptr;   // D32: bin-pair layout of k_dense2
   // options
   int precision = 0; int f32_min_seg = 8; size_t scratch_cap = (size_t)32 << 30;   // of 180 GB per B200
+  double win_frac = 0.0;           // SC_OPT_WINDOW_FRACTION_PPM: mean share of the band inside a particle's time window (0: not stated)
   double tc_max_s = 10.0 * 31557600.0; int forced_stride_log2 = 0; int sincos_mode = 0; int mufu_min_seg = 32;
   int lg_f32 = 5, lg_f64 = 5;      // log2 of the coarse node spacing per precision mode (set_stride)
   double mufu_gain2 = 1.0;        // <cos^2 + sin^2> of the hardware sin/cos, measured at init
@@ -96,6 +97,7 @@ struct sc_handle : EdgeCache {
   // escalation: particles whose FP32-path Upsilon is below the mode's threshold are re-evaluated
   // by the all-FP64 path; compacted index list, count, gathered parameters and their results
   int escalate = 1; double esc_tau_poly = 6.0, esc_tau_mufu = 16.0;
+  double esc_tau_nodes = 0.0;      // threshold the node spacing of the current call adds (select_stride_f32)
   int* d_esc_idx = nullptr; int* d_esc_count = nullptr; double* d_esc_params = nullptr; double* d_esc_out = nullptr;
   size_t esc_idx_cap = 0, esc_cnt_cap = 0, esc_par_cap = 0, esc_out_cap = 0; int* h_esc_hint = nullptr;
   // tensor-core flavour of the FP32-amplitude kernel (k_dense2_tc, SC_OPT_TENSOR_CORES; off by default: measured slower than
@@ -121,6 +123,7 @@ namespace {
 
 int fail(sc_handle* h, int code, const char* fmt, ...);
 int pick_stride_log2(const sc_config& cfg, double tc_max_s, int forced, double max_days);
+double node_seconds_per_bin(const sc_config& cfg, double tc_max_s);
 
 // Node spacing per precision mode: the all-FP64 path (N_seg < 8, where 1e-8 rad matters)
 // keeps the nodes <= 2 days of signal time apart, the FP32-amplitude path (error floor ~1e-8 relative) <= 4 days.
@@ -137,6 +140,32 @@ void set_stride(sc_handle* h) {
   h->lg_f64 = pick_stride_log2(h->cfg, h->tc_max_s, h->forced_stride_log2, kNodeDaysF64);
   h->lg_f32 = pick_stride_log2(h->cfg, h->tc_max_s, h->forced_stride_log2, kNodeDaysF32);
   apply_stride(h->dc, h->lg_f64);
+}
+
+// Node spacing of the FP32-amplitude path for ONE call: the interpolation error of a
+// segment's z_k grows like (days per coarse interval)^6 and is independent from segment to segment, so the error of
+// Upsilon = sum over the N' segments inside a particle's window falls like 1 / sqrt(N'): measured on c1-c5,
+// max relative error <= 1.4e-10 days^6 / sqrt(N') for N' >= 8.  kNodeDaysF32 is the limit at N' = 8, the fewest
+// segments the FP32 path is left with (below that the escalation pass takes the particle); at larger N' the same
+// modelled error (2e-7) allows kNodeDaysF32 (N' / 8)^(1/12) days, capped at kNodeDaysMax.  N' = n_seg x window
+// fraction / 2 when the caller has stated the fraction (SC_OPT_WINDOW_FRACTION_PPM; the search measures it), else 8.
+// n_seg = 0 keeps the N' = 8 spacing: per-segment output (sc_eval_segments, the two-pass three-channel path), where
+// nothing averages, and per-particle segments (sc_eval_stat_adaptive), whose integer edges are decided on the
+// interpolated cumulative sigma -- wider nodes there move 0.3 % of the c3 edges by one bin instead of < 0.1 %.
+constexpr double kNodeDaysMax = 8.0;
+void select_stride_f32(sc_handle* h, int n_seg) {
+  double n_eff = 8.0;
+  if (n_seg > 0 && h->win_frac > 0.0) n_eff = 0.5 * (double)n_seg * h->win_frac;
+  const double days = std::min(kNodeDaysMax, kNodeDaysF32 * pow(std::max(n_eff, 8.0) / 8.0, 1.0 / 12.0));
+  h->lg_f32 = pick_stride_log2(h->cfg, h->tc_max_s, h->forced_stride_log2, days);
+  // A particle of the same population with far fewer segments than the mean (a window that leaves the band) does not
+  // average as much: with the spacing chosen, the model needs N' >= 8 (days / kNodeDaysF32)^12 segments, i.e.
+  // Upsilon ~ 2 N' above twice that -- below it the escalation pass (all-FP64 path, its own spacing) takes the particle.
+  h->esc_tau_nodes = 0.0;
+  if (n_seg > 0 && h->forced_stride_log2 == 0) {
+    const double d = (double)(1 << h->lg_f32) * node_seconds_per_bin(h->cfg, h->tc_max_s) / 86400.0;
+    if (d > kNodeDaysF32) h->esc_tau_nodes = 2.0 * 8.0 * pow(d / kNodeDaysF32, 12.0);
+  }
 }
 
 int fail(sc_handle* h, int code, const char* fmt, ...) {
@@ -179,10 +208,13 @@ int check_launch(sc_handle* h, const char* what) {
 // Coarse node spacing: the slowly varying amplitudes change on the orbital time scale,
 // so the spacing is set in TIME: at most max_days at the slowest-chirping corner of the problem.  Time per bin is
 // |dt/df| df = (8/3) tau / (f T_obs) with tau <= tc_max (Newtonian), largest at the low band edge.
+double node_seconds_per_bin(const sc_config& cfg, double tc_max_s) {
+  const double f_lo = (double)std::max<int64_t>(cfg.j0, 1) / cfg.T_obs_s;
+  return (8.0 / 3.0) * tc_max_s / (f_lo * cfg.T_obs_s);
+}
 int pick_stride_log2(const sc_config& cfg, double tc_max_s, int forced, double max_days) {
   if (forced > 0) return std::min(std::max(forced, 3), 12);
-  const double f_lo = (double)std::max<int64_t>(cfg.j0, 1) / cfg.T_obs_s;
-  const double s_per_bin = (8.0 / 3.0) * tc_max_s / (f_lo * cfg.T_obs_s);
+  const double s_per_bin = node_seconds_per_bin(cfg, tc_max_s);
   int lg = 5;
   while (lg < 11 && (double)(2 << lg) * s_per_bin <= max_days * 86400.0) ++lg;
   return lg;
@@ -507,6 +539,7 @@ int eval_common(sc_handle* h, const double* params, int64_t P, const int32_t* se
     return fail(h, SC_ERR_INVALID_ARG, "null pointer or n_particles <= 0");
   cudaStream_t st = (cudaStream_t)stream;
   const bool f64 = !fused3 && ((h->precision == 2) || (h->precision == 0 && n_seg < h->f32_min_seg));
+  select_stride_f32(h, seg_mode ? 0 : n_seg);
   // all-FP64 path: sigma from FP64 piece moments when a fine sub-interval is long enough to pay for them (>= 32 bins)
   const int lg_fine64 = (h->lg_f64 - 2 >= 5) ? h->lg_f64 - 2 : 0;
   // chunk length: 1024 bins (all-FP64), 2048 (k_dense2: the chunk's data is staged in shared memory), 8192 (k_dense2_tc)
@@ -532,7 +565,7 @@ int eval_common(sc_handle* h, const double* params, int64_t P, const int32_t* se
     if ((rc = grow(h, (void**)&h->d_esc_out, &h->esc_out_cap, P_round * 8))) return rc;
     {
       Timed tm(h, st, SC_TIME_ESC);
-      k_esc_select<<<1, 1024, 0, st>>>(out, params, (int)P, mufu ? h->esc_tau_mufu : h->esc_tau_poly, h->d_esc_idx,
+      k_esc_select<<<1, 1024, 0, st>>>(out, params, (int)P, std::max(mufu ? h->esc_tau_mufu : h->esc_tau_poly, h->esc_tau_nodes), h->d_esc_idx,
                                        h->d_esc_count, h->d_esc_params);
     }
     if ((rc = check_launch(h, "k_esc_select"))) return rc;
@@ -603,7 +636,7 @@ int eval_any(sc_handle* h, const double* params, int64_t P, const int32_t* seg_e
     {
       Timed tm(h, st, SC_TIME_ESC);
       const bool mufu3 = (h->sincos_mode == 0) ? (n_seg >= h->mufu_min_seg) : (h->sincos_mode == 2);
-      k_esc_select<<<1, 1024, 0, st>>>(outp, par, (int)Pn, mufu3 ? h->esc_tau_mufu : h->esc_tau_poly, h->d_esc_idx, h->d_esc_count, h->d_esc_params);
+      k_esc_select<<<1, 1024, 0, st>>>(outp, par, (int)Pn, std::max(mufu3 ? h->esc_tau_mufu : h->esc_tau_poly, h->esc_tau_nodes), h->d_esc_idx, h->d_esc_count, h->d_esc_params);
     }
     if ((rc2 = check_launch(h, "k_esc_select"))) return rc2;
     int n_esc = 0;
@@ -664,6 +697,7 @@ int eval_any(sc_handle* h, const double* params, int64_t P, const int32_t* seg_e
 int run_adaptive(sc_handle* h, const double* params, int64_t P, int n_seg, double* out, int32_t* out_edges, double* out_comp,
                  cudaStream_t st) {
   DevCfg dc = h->dc;
+  select_stride_f32(h, 0);
   apply_stride(dc, h->lg_f32);
   const bool three = (h->sub != nullptr);        // three-channel handle: (A, E, T) in every step (NA = 6 amplitude fields)
   if (three) dc.chan_set = 2;
@@ -1099,7 +1133,8 @@ int sc_search_run(sc_handle* h, const sc_search_config* sc, double* pos, double*
   const bool auto_precision = (h->precision == 0) && h->escalate && !h->sub;
   double win_frac = -1.0;                          // mean window fraction, -1: not measured yet
   unsigned long long ev_bins = 0;
-  auto cleanup = [&](int code) { set_mode(saved_precision, saved_escalate); cudaFree(buf); return code; };
+  const double saved_win_frac = h->win_frac;
+  auto cleanup = [&](int code) { set_mode(saved_precision, saved_escalate); h->win_frac = saved_win_frac; cudaFree(buf); return code; };
 #define SC_S(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cleanup(fail(h, SC_ERR_CUDA, "%s failed: %s", #call, cudaGetErrorString(e_))); } while (0)
   SC_S(cudaMemsetAsync(gbest_pos, 0, (size_t)S * 8 * 8, st));
 
@@ -1136,6 +1171,7 @@ int sc_search_run(sc_handle* h, const sc_search_config* sc, double* pos, double*
       if (measure) {
         win_frac = (double)ev_bins / ((double)P * (double)nb);
         h->precision = ((double)N * win_frac < (double)h->f32_min_seg) ? 2 : 0;
+        if (saved_win_frac == 0.0) h->win_frac = win_frac;     // node spacing of the later shared-edge evaluations (select_stride_f32)
       }
       bool all_conv = true;
       for (int s = 0; s < S; ++s) {
@@ -1539,6 +1575,9 @@ int sc_set_option(sc_handle* h, int32_t option, int64_t value) {
     case SC_OPT_TC_MAX_S:
       if (value < 1) return fail(h, SC_ERR_INVALID_ARG, "tc_max_s must be >= 1");
       h->tc_max_s = (double)value; set_stride(h); return SC_OK;
+    case SC_OPT_WINDOW_FRACTION_PPM:
+      if (value < 0 || value > 1000000) return fail(h, SC_ERR_INVALID_ARG, "window fraction must be 0 (not stated) .. 1000000 ppm");
+      h->win_frac = (double)value * 1e-6; return SC_OK;
     case SC_OPT_STRIDE_LOG2:
       if (value != 0 && (value < 3 || value > 12)) return fail(h, SC_ERR_INVALID_ARG, "stride_log2 must be 0 (auto) or 3..12");
       h->forced_stride_log2 = (int)value; set_stride(h); return SC_OK;

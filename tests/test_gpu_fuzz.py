@@ -64,14 +64,21 @@ def test_random_grids_tiles_and_edges(oracle, seed):
     cfg_truth = oracle.make_config(inp["cfg"], truth=True)
     ref = oracle.eval_stat_levels(cfg_truth, dA, dE, inp["S_A"], inp["S_E"], inp["particles"], lists)
     n_live = 0
-    for e, r in zip(lists, ref):
-        got = H.eval_stat(par, e.astype(np.int32)).cpu().numpy()
-        assert np.all(np.isfinite(got)) and np.all(got >= 0.0)
-        assert np.array_equal(got == 0.0, r == 0.0), (seed, len(e))          # same particles see an empty window
-        ok = r > 0
-        n_live += int(ok.sum())
-        if ok.any():
-            err = rel_err(got[ok], r[ok])
-            assert np.all(err <= TOL), (seed, len(e), float(err.max()), float(r[ok][np.argmax(err)]))
+    # second round: the caller states the measured window fraction (SC_OPT_WINDOW_FRACTION_PPM), which widens the node spacing of
+    # the FP32-amplitude path with the number of segments -- on tiles whose windows partly leave the band, the hard case of that rule
+    for hint in (False, True):
+        if hint:
+            H.eval_stat(par, lists[0].astype(np.int32))                      # whole band: evaluated bins = the windows
+            phi = H.counters()[0] / (len(inp["particles"]) * inp["cfg"]["n_bins"])
+            H.set_option(sc.SC_OPT_WINDOW_FRACTION_PPM, max(1, int(round(1e6 * phi))))
+        for e, r in zip(lists, ref):
+            got = H.eval_stat(par, e.astype(np.int32)).cpu().numpy()
+            assert np.all(np.isfinite(got)) and np.all(got >= 0.0)
+            assert np.array_equal(got == 0.0, r == 0.0), (seed, len(e))          # same particles see an empty window
+            ok = r > 0
+            n_live += int(ok.sum())
+            if ok.any():
+                err = rel_err(got[ok], r[ok])
+                assert np.all(err <= TOL), (seed, hint, len(e), float(err.max()), float(r[ok][np.argmax(err)]))
     assert n_live > 0
     H.close()

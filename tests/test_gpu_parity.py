@@ -326,7 +326,7 @@ def _hard_particles(got, N, n_each=8):
     return np.concatenate([small, near])
 
 
-def _full_launch_case(oracle, torch, sc, cid, n_sample, seed, tc_hint=True, opts=()):
+def _full_launch_case(oracle, torch, sc, cid, n_sample, seed, tc_hint=True, opts=(), win_hint=True):
     """GPU: the whole population in bench.py's launch configuration, every level.  Oracle (truth mode: long-double phase,
     so the 1e-6 bar holds flat down to the smallest Upsilon): a seeded random sample of n_sample particles plus, per level,
     the 8 smallest non-zero and the 8 nearest the escalation threshold."""
@@ -340,6 +340,9 @@ def _full_launch_case(oracle, torch, sc, cid, n_sample, seed, tc_hint=True, opts
     P = inp["particles"].shape[0]
     levels = inp["spec"]["n_segs"]
     par = _dev(torch, inp["particles"])
+    if win_hint:                       # ... and the measured share of the band inside the time windows (node spacing for N' segments)
+        H.eval_stat(par, inp["edges"][levels[0]])
+        H.set_option(sc.SC_OPT_WINDOW_FRACTION_PPM, int(round(1e6 * H.counters()[0] / (P * inp["cfg"]["n_bins"]))))
     got = {}
     for N in levels:
         got[N] = H.eval_stat(par, inp["edges"][N]).cpu().numpy()            # whole population, bench launch config
@@ -403,7 +406,7 @@ def test_tensor_core_flavour(oracle, torch_cuda, sc, cid):
 
 def test_default_stride_without_tile_hint(oracle, torch_cuda, sc):
     """Without SC_OPT_TC_MAX_S the conservative default (t_c <= 10 yr) must meet the same bar."""
-    inp, levels, idx, ref, got, dd = _full_launch_case(oracle, torch_cuda, sc, 2, 16, 7, tc_hint=False)
+    inp, levels, idx, ref, got, dd = _full_launch_case(oracle, torch_cuda, sc, 2, 16, 7, tc_hint=False, win_hint=False)
     _check_case(inp, levels, idx, ref, got, dd)
 
 
