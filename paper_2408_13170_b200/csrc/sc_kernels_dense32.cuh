@@ -361,7 +361,75 @@ __device__ __forceinline__ void pairs_fast(PhaseFD& ph, const float (&cf)[4][4],
   mac_pair(cf, s2, wA, wE, h2, cr, sr, zr2, zi2);
 }
 
-template <bool SEG, int SC, bool MERGE = false>
+// The same with the amplitudes QUADRATIC over runs of a quarter of the fine sub-interval (QUAD flavour, fine
+// sub-intervals of >= 256 bins): the sub-interval's cubic re-expanded about the run start in u = (j - run start)/run
+// length, its u^3 term economised (u^3 ~ 3/2 u^2 - 9/16 u + 1/32 on [0, 1], error <= |c_3| / (64 x 32) of the cubic's
+// own s^3 coefficient: <= 3e-8 of the amplitude at 4 days per coarse interval, oscillating inside the run) -- 8 packed
+// FMAs per bin pair instead of 12.  sigma keeps the cubic (sigma_moments).  off = first bin - sub-interval start,
+// lg_run = log2(run length in bins); s2 is not used by this flavour.
+struct QuadRun { float q[4][3]; };
+__device__ __forceinline__ void quad_run(const float (&cf)[4][4], int r, QuadRun& o) {
+  const float s0 = 0.25f * (float)r;
+#pragma unroll
+  for (int a = 0; a < 4; ++a) {
+    const float c0 = cf[a][0], c1 = cf[a][1], c2 = cf[a][2], c3 = cf[a][3];
+    const float a3 = c3 * (1.0f / 64.0f);
+    const float a2 = fmaf(3.0f * c3, s0, c2) * (1.0f / 16.0f);
+    const float a1 = fmaf(fmaf(3.0f * c3, s0, 2.0f * c2), s0, c1) * 0.25f;
+    const float a0 = fmaf(fmaf(fmaf(c3, s0, c2), s0, c1), s0, c0);
+    o.q[a][2] = fmaf(1.5f, a3, a2);
+    o.q[a][1] = fmaf(-0.5625f, a3, a1);
+    o.q[a][0] = fmaf(0.03125f, a3, a0);
+  }
+}
+__device__ __forceinline__ void mac_pair_q(const QuadRun& w, u64& u2, const ulonglong2 wA, const ulonglong2 wE, u64 hu2,
+                                           u64 cr2, u64 sr2, u64& zr2, u64& zi2) {
+  const u64 Ar = f2fma(f2fma(f2bcast(w.q[0][2]), u2, f2bcast(w.q[0][1])), u2, f2bcast(w.q[0][0]));
+  const u64 Ai = f2fma(f2fma(f2bcast(w.q[1][2]), u2, f2bcast(w.q[1][1])), u2, f2bcast(w.q[1][0]));
+  const u64 Er = f2fma(f2fma(f2bcast(w.q[2][2]), u2, f2bcast(w.q[2][1])), u2, f2bcast(w.q[2][0]));
+  const u64 Ei = f2fma(f2fma(f2bcast(w.q[3][2]), u2, f2bcast(w.q[3][1])), u2, f2bcast(w.q[3][0]));
+  u2 = f2add(u2, hu2);
+  const u64 qr = f2fma(wA.x, Ar, f2fma(wA.y, Ai, f2fma(wE.x, Er, f2mul(wE.y, Ei))));
+  const u64 qi = f2fma(wA.y, Ar, f2fma(f2neg(wA.x), Ai, f2fma(wE.y, Er, f2neg(f2mul(wE.x, Ei)))));
+  zr2 = f2fma(qr, cr2, f2fma(f2neg(qi), sr2, zr2));
+  zi2 = f2fma(qr, sr2, f2fma(qi, cr2, zi2));
+}
+// The run state lives across the flush groups of a piece: coefficients are rebuilt at run boundaries only.
+struct QuadState { QuadRun w; u64 u2; int left; int r; };
+__device__ __forceinline__ void quad_start(const float (&cf)[4][4], int off, int lg_run, QuadState& q) {
+  const int run_bins = 1 << lg_run;
+  const int o = off & (run_bins - 1);
+  const float hu = 1.0f / (float)run_bins;
+  q.r = off >> lg_run;
+  q.left = (run_bins - o) >> 1;                                 // pairs to the end of the run
+  q.u2 = f2pack((float)o * hu, (float)(o + 1) * hu);
+  quad_run(cf, q.r, q.w);
+}
+template <int SC>
+__device__ __forceinline__ void pairs_fast_q(PhaseFD& ph, const float (&cf)[4][4], QuadState& q, int lg_run, const ulonglong2*& rec,
+                                             int n, u64 K2, u64& zr2, u64& zi2) {
+  const int run_pairs = 1 << (lg_run - 1);
+  const float hu = 1.0f / (float)(2 * run_pairs);
+  const u64 hu2 = f2bcast(2.0f * hu);
+  u64 cr, sr;
+  sincos_pair<SC>(ph, K2, cr, sr);
+  ulonglong2 wA = rec[0], wE = rec[1];
+#pragma unroll 1
+  for (int i = 1; i < n; ++i) {
+    u64 crn, srn;
+    sincos_pair<SC>(ph, K2, crn, srn);
+    rec += kPairRec;
+    const ulonglong2 wAn = rec[0], wEn = rec[1];
+    mac_pair_q(q.w, q.u2, wA, wE, hu2, cr, sr, zr2, zi2);
+    if (--q.left == 0) { quad_run(cf, ++q.r, q.w); q.left = run_pairs; q.u2 = f2pack(0.0f, hu); }
+    cr = crn; sr = srn; wA = wAn; wE = wEn;
+  }
+  rec += kPairRec;
+  mac_pair_q(q.w, q.u2, wA, wE, hu2, cr, sr, zr2, zi2);
+  if (--q.left == 0) { quad_run(cf, ++q.r, q.w); q.left = run_pairs; q.u2 = f2pack(0.0f, hu); }
+}
+
+template <bool SEG, int SC, bool MERGE = false, bool QUAD = false>
 __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2(DevCfg c, DenseArgs a, const ulonglong2* __restrict__ Dg) {
   constexpr int CH = kChunkF32;
   __shared__ ulonglong2 sD[CH / 2 * kPairRec];                 // 48 KB
@@ -468,6 +536,7 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2(DevCfg c, Den
     int piece = use_mom ? a.piece_first[(ib >> (c.log2_stride - 2)) - ((a.chunk_first * CH) >> (c.log2_stride - 2))] : 0;
     float car_zr = 0.f, car_zi = 0.f, car_sg = 0.f;
     bool carry = false;
+    QuadState qs;
     int pl = ib;
     while (pl < ie) {
       const int ph = min(next_edge, ie);                       // next_edge > pl: edges <= pl are consumed
@@ -486,11 +555,16 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2(DevCfg c, Den
         }
         s2 = f2pack((float)(jj - ib) * hS, (float)(jj + 1 - ib) * hS);
         rec = sD + ((jj - cs) >> 1) * kPairRec;
+        if constexpr (QUAD) { if (use_mom && jj < ph) quad_start(cf, jj - ib, c.log2_stride - 4, qs); }
         while (jj < ph) {
           const bool split = (jj == jfull);                    // the pair (ph - 1, ph)
           const int e2 = split ? jj + 2 : min(jj + kFlushBins, jfull);
           u64 zr2 = 0, zi2 = 0, sg2 = 0;
-          if (use_mom) { pairs_fast<SC>(fd, cf, s2, rec, (e2 - jj) >> 1, h2, K2, zr2, zi2); jj = e2; }
+          if (use_mom) {
+            if constexpr (QUAD) pairs_fast_q<SC>(fd, cf, qs, c.log2_stride - 4, rec, (e2 - jj) >> 1, K2, zr2, zi2);
+            else pairs_fast<SC>(fd, cf, s2, rec, (e2 - jj) >> 1, h2, K2, zr2, zi2);
+            jj = e2;
+          }
           else         { for (; jj < e2; jj += 2) pair(jj, T_{}, T_{}, zr2, zi2, sg2); }
           float zrl, zrh, zil, zih, sgl, sgh;
           f2unpack(zr2, zrl, zrh); f2unpack(zi2, zil, zih); f2unpack(sg2, sgl, sgh);

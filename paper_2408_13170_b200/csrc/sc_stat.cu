@@ -97,6 +97,7 @@ struct sc_handle : EdgeCache {
   // escalation: particles whose FP32-path Upsilon is below the mode's threshold are re-evaluated
   // by the all-FP64 path; compacted index list, count, gathered parameters and their results
   int escalate = 1; double esc_tau_poly = 6.0, esc_tau_mufu = 16.0;
+  int quad_amp = 1;
   double esc_tau_nodes = 0.0;      // threshold the node spacing of the current call adds (select_stride_f32)
   int* d_esc_idx = nullptr; int* d_esc_count = nullptr; double* d_esc_params = nullptr; double* d_esc_out = nullptr;
   size_t esc_idx_cap = 0, esc_cnt_cap = 0, esc_par_cap = 0, esc_out_cap = 0; int* h_esc_hint = nullptr;
@@ -125,8 +126,13 @@ int fail(sc_handle* h, int code, const char* fmt, ...);
 int pick_stride_log2(const sc_config& cfg, double tc_max_s, int forced, double max_days);
 double node_seconds_per_bin(const sc_config& cfg, double tc_max_s);
 
-// Node spacing per precision mode: the all-FP64 path (N_seg < 8, where 1e-8 rad matters)
-// keeps the nodes <= 2 days of signal time apart, the FP32-amplitude path (error floor ~1e-8 relative) <= 4 days.
+// Node spacing per precision mode: measured against the oracle on c1-c5, the interpolation
+// error of Upsilon is <= K days^6 / sqrt(N') with days = signal time per coarse interval at the slowest-chirping corner,
+// N' = segments inside the particle's window, K = 7.5e-10 for N' = 1 (largest of 400 particles; the single coherent sum
+// has the heavier tail) and 1.4e-10 for N' >= 8.  The FP32-amplitude path (N' >= 8) keeps days <= 4: model 2e-7, a fifth
+// of the 1e-6 bar.  The all-FP64 path (any N', so N' = 1) keeps days <= 2: model 5e-8 -- it is also the path of the
+// ill-conditioned particles (Upsilon << 1, where the relative error is amplified): at 2.5 days c5's smallest Upsilon
+// reached 8.5e-7 and the escalation test failed, so the margin stays.
 constexpr double kNodeDaysF64 = 2.0, kNodeDaysF32 = 4.0;
 
 void apply_stride(DevCfg& d, int lg) {
@@ -386,6 +392,9 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
         // merged coarse intervals (see coarse_dslope): worth their test only where the coarse intervals are long; the
         // fine sub-intervals may span kNodeDaysF32 / 4 days of signal time
         const bool merge = dc.stride >= 512;
+        // quadratic amplitudes over runs of >= 64 bins (pairs_fast_q): where the pieces are long enough to pay for the run
+        // set-up at each piece start (c4 at N = 50 000, 33-bin segments: +1 %; c3/c4 at N = 5000, 328 bins: -4 %)
+        const bool quad = h->quad_amp && dc.stride >= 1024 && (long long)(e_last - e_first) >= 128LL * n_seg;
         a.merge_lim = 86400.0 * (kNodeDaysF32 / 4.0) / h->cfg.T_obs_s;
         const dim3 grid_tc(pblocks, n_chunks);
         if (fused3) {
@@ -408,6 +417,7 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
         else if (seg_mode && sincos == 2) k_dense2<true, 2><<<grid, kBlock, 0, st>>>(dc, a, Dp);
         else if (seg_mode && merge) k_dense2<true, 0, true><<<grid, kBlock, 0, st>>>(dc, a, Dp);
         else if (seg_mode) k_dense2<true, 0><<<grid, kBlock, 0, st>>>(dc, a, Dp);
+        else if (sincos == 2 && merge && quad) k_dense2<false, 2, true, true><<<grid, kBlock, 0, st>>>(dc, a, Dp);
         else if (sincos == 2 && merge) k_dense2<false, 2, true><<<grid, kBlock, 0, st>>>(dc, a, Dp);
         else if (sincos == 2) k_dense2<false, 2><<<grid, kBlock, 0, st>>>(dc, a, Dp);
         else if (merge) k_dense2<false, 0, true><<<grid, kBlock, 0, st>>>(dc, a, Dp);
