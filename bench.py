@@ -35,7 +35,9 @@ C_DP = 24          # FP64 instructions per (particle, bin) of the fixed op model
 NOMINAL_DFMA = 148 * 64 * 1.965e9   # 148 SMs x 64 FP64 lanes x max SM clock (B200_PROFILING.md unit counts / clocks)
 # The kernel's own mix: FP32-pipe lane slots per evaluated (particle, bin) in the k_dense2 loop,
 # 26 packed FFMA2/FMUL2/FADD2 (2 slots each) + 3 scalar per bin PAIR; peak = 148 SMs x 128 FP32 lanes x max SM clock.
+# The QUAD flavour (quadratic amplitudes over runs, sc_get_launch_info) executes 22 packed instead of 26.
 FP32_SLOTS_PER_BIN = (26 * 2 + 3) / 2.0
+FP32_SLOTS_PER_BIN_QUAD = (22 * 2 + 3) / 2.0
 NOMINAL_FP32_SLOTS = 148 * 128 * 1.965e9
 NOMINAL_FP32_TFLOPS = 2.0 * NOMINAL_FP32_SLOTS / 1e12   # 74.5 TFLOP/s: unit counts x clock of B200_PROFILING.md (no measured FP32 peak)
 DENSE_PROFILE = os.path.join(ROOT, "profiles", "r02_k_dense2_full.md")   # ncu --set full of the c3 launch (static figure, see roofline.traffic_source)
@@ -583,12 +585,16 @@ def run_ours(args, rank, local_rank, world):
         peak = 2.0 * (dfma or NOMINAL_DFMA) / 1e12
         pbs = eval_bins_launch / (dense_avg * 1e-3) if dense_avg > 0 else None
         # Two fractions (both kept): (1) frac = frac_pipe_fma -- the pipe the kernel as built runs on: FP32 lane slots it
-        # executes per evaluated bin (SASS of the pair loop: 26 packed x 2 + 3 scalar per bin pair) x evaluated bins/s
+        # executes per evaluated bin (SASS of the pair loop: 26 packed x 2 + 3 scalar per bin pair; 22 packed in the QUAD flavour,
+        # so a faster kernel can show a LOWER fraction: it does less work) x evaluated bins/s
         # against 148 SM x 128 lanes x max clock; ncu's sm__pipe_fma_cycles_active of the same launch is in profiles/.
         # (2) frac_model -- the contract's fixed op model (24 FP64 instructions per evaluated bin)
         # against the FP64 rate measured in this run; the kernel does NOT execute that FP64 work (3 DADD per bin), so
         # this one is a speed-up over the model, not a utilisation, and may exceed 1.
-        slots = (pbs * FP32_SLOTS_PER_BIN) if pbs else None
+        lg_nodes, flavour = H.launch_info()
+        quad = bool(flavour & sc.SC_FLAVOUR_QUAD) and not ad_N
+        slots_per_bin = FP32_SLOTS_PER_BIN_QUAD if quad else FP32_SLOTS_PER_BIN
+        slots = (pbs * slots_per_bin) if pbs else None
         is_c3_shared = (cid == 3 and not ad_N and not args.particles)
         roof = {"bound": "alu", "achieved": (2.0 * slots / 1e12) if slots else None, "peak": NOMINAL_FP32_TFLOPS, "unit": "TFLOP/s",
                 "frac": (slots / NOMINAL_FP32_SLOTS) if slots else None,
@@ -597,10 +603,12 @@ def run_ours(args, rank, local_rank, world):
                 "traffic": dram_traffic_from_profile() if is_c3_shared else None,
                 "traffic_source": ("static: profiles/r02_k_dense2_full.md (ncu --set full of one k_dense2 launch of this c3 command), "
                                    "not measured in this run") if is_c3_shared else None,
-                "kernel": "k_dense2_ad<2,MERGE>" if ad_N else "k_dense2<false,2,MERGE>", "kernel_ms_per_launch": dense_avg,
+                "kernel": "k_dense2_ad<2,MERGE>" if ad_N else ("k_dense2<false,2,MERGE,QUAD>" if quad else "k_dense2<false,2,MERGE>"),
+                "kernel_ms_per_launch": dense_avg, "node_stride_log2": lg_nodes, "flavour_bits": flavour,
                 "peak_source": "FP32 pipe: 148 SM x 128 lanes x 1.965 GHz x 2 flop (unit counts and clocks of B200_PROFILING.md; "
                                "MEASURED_PEAKS.json has no FP32 figure)",
-                "pipe_fma": {"fp32_lane_slots_per_evaluated_bin": FP32_SLOTS_PER_BIN, "lane_slots_per_s": slots,
+                "pipe_fma": {"fp32_lane_slots_per_evaluated_bin": slots_per_bin,
+                             "packed_fp32_instructions_per_bin_pair": 22 if quad else 26, "lane_slots_per_s": slots,
                              "peak_lane_slots_per_s": NOMINAL_FP32_SLOTS},
                 "model": {"what": f"{C_DP} FP64 instr (= {2 * C_DP} flop) per evaluated particle-bin, SURVEY.md 8(d)",
                           "achieved_tflops": ach, "peak_tflops": peak,

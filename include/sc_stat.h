@@ -309,6 +309,14 @@ int sc_eval_stat_streams(sc_handle* h, const double* theta, const void* W, int32
  *  kernel_launches = CUDA kernels launched by the library since the handle was created. */
 int sc_get_counters(sc_handle* h, int64_t* evaluated_bins, int64_t* kernel_launches, void* cuda_stream);
 
+/* What the last FP32-amplitude pass of sc_eval_stat / sc_eval_segments / sc_eval_stat_host launched (host values, no
+ * synchronisation; 0, 0 before the first such pass): log2 of the coarse node spacing in bins, and the kernel flavour as
+ * a bit set -- SC_FLAVOUR_MUFU (hardware sin/cos), SC_FLAVOUR_MERGE (one set-up per coarse interval where it holds),
+ * SC_FLAVOUR_QUAD (quadratic amplitudes over runs, 22 packed FP32 instructions per bin pair instead of 26),
+ * SC_FLAVOUR_TC (k_dense2_tc), SC_FLAVOUR_AET (k_dense3).  For reporting (bench.py's instruction count) and tests. */
+enum { SC_FLAVOUR_MUFU = 1, SC_FLAVOUR_MERGE = 2, SC_FLAVOUR_QUAD = 4, SC_FLAVOUR_TC = 8, SC_FLAVOUR_AET = 16 };
+int sc_get_launch_info(sc_handle* h, int32_t* stride_log2, int32_t* flavour);
+
 /* With SC_OPT_PROFILE = 1: device time [ms] and launch count per kernel class since the previous call, measured with
  * CUDA events on the launching stream (ms_per_class, launches_per_class: HOST arrays of SC_N_TIMING_CLASSES; either
  * may be NULL).  Synchronises the stream and resets the accumulators. */

@@ -19,7 +19,7 @@ SC_OPT_WINDOW_FRACTION_PPM = 15
 SC_TIMING_CLASSES = ["nodes", "dense", "stitch", "pso", "other", "escalation"]
 
 EXPORTED_SYMBOLS = ["sc_init_data", "sc_init_data_host", "sc_init_data3", "sc_gen_template3", "sc_eval_stat", "sc_eval_stat_host", "sc_eval_segments",
-                    "sc_eval_stat_adaptive", "sc_eval_components", "sc_eval_loglike", "sc_data_norm", "sc_gen_template", "sc_pso_step", "sc_pso_best", "sc_pso_pick", "sc_pso_move", "sc_pso_step_labeled", "sc_kmeans", "sc_search_run", "sc_whiten_streams", "sc_eval_stat_streams", "sc_get_counters", "sc_get_timing", "sc_measure_fp64_peak",
+                    "sc_eval_stat_adaptive", "sc_eval_components", "sc_eval_loglike", "sc_data_norm", "sc_gen_template", "sc_pso_step", "sc_pso_best", "sc_pso_pick", "sc_pso_move", "sc_pso_step_labeled", "sc_kmeans", "sc_search_run", "sc_whiten_streams", "sc_eval_stat_streams", "sc_get_counters", "sc_get_launch_info", "sc_get_timing", "sc_measure_fp64_peak",
                     "sc_set_option", "sc_free",
                     "sc_last_error", "sc_version"]
 
@@ -135,6 +135,8 @@ def load_library():
     L.sc_eval_stat_streams.argtypes = [_vp, _vp, _vp, C.c_int32, C.c_int64, _vp, C.c_int32, _vp, _vp]
     L.sc_get_counters.restype = C.c_int
     L.sc_get_counters.argtypes = [_vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64), _vp]
+    L.sc_get_launch_info.restype = C.c_int
+    L.sc_get_launch_info.argtypes = [_vp, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
     L.sc_get_timing.restype = C.c_int
     L.sc_get_timing.argtypes = [_vp, C.POINTER(C.c_double), C.POINTER(C.c_int64), _vp]
     L.sc_measure_fp64_peak.restype = C.c_int
@@ -512,6 +514,16 @@ def sc_get_counters(h, stream=None):
     return a.value, b.value
 
 
+SC_FLAVOUR_MUFU, SC_FLAVOUR_MERGE, SC_FLAVOUR_QUAD, SC_FLAVOUR_TC, SC_FLAVOUR_AET = 1, 2, 4, 8, 16
+
+
+def sc_get_launch_info(h):
+    """(log2 node spacing, flavour bits) of the last FP32-amplitude pass."""
+    a, b = C.c_int32(0), C.c_int32(0)
+    _check(load_library().sc_get_launch_info(h, C.byref(a), C.byref(b)), h)
+    return a.value, b.value
+
+
 def sc_get_timing(h, stream=None):
     """{class: (ms, launches)} since the previous call (needs SC_OPT_PROFILE = 1); synchronises the stream."""
     ms = (C.c_double * len(SC_TIMING_CLASSES))()
@@ -670,6 +682,9 @@ class Handle:
 
     def timing(self, stream=None):
         return sc_get_timing(self.h, stream)
+
+    def launch_info(self):
+        return sc_get_launch_info(self.h)
 
     def set_option(self, option, value):
         sc_set_option(self.h, option, value)

@@ -40,6 +40,10 @@ __device__ __forceinline__ void fine_cubic2(const u64 nd[6], int q, u64 out[4]) 
   }
 }
 
+#ifndef SC_QUAD_FLUSH
+#define SC_QUAD_FLUSH 64     /* bins per FP32 flush group of the QUAD flavour's unmasked runs (measured on c3, 264 particles:
+                                32 bins 18.47 ms, rms error 4.2e-9; 64 bins 18.04 ms; 128 bins 17.83 ms, rms 5.6e-9) */
+#endif
 #ifndef SC_DENSE2_MINB
 #define SC_DENSE2_MINB 4     /* CTAs per SM the register allocation aims at (128 registers/thread) */
 #endif
@@ -558,7 +562,7 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2(DevCfg c, Den
         if constexpr (QUAD) { if (use_mom && jj < ph) quad_start(cf, jj - ib, c.log2_stride - 4, qs); }
         while (jj < ph) {
           const bool split = (jj == jfull);                    // the pair (ph - 1, ph)
-          const int e2 = split ? jj + 2 : min(jj + kFlushBins, jfull);
+          const int e2 = split ? jj + 2 : min(jj + ((QUAD && use_mom) ? SC_QUAD_FLUSH : kFlushBins), jfull);
           u64 zr2 = 0, zi2 = 0, sg2 = 0;
           if (use_mom) {
             if constexpr (QUAD) pairs_fast_q<SC>(fd, cf, qs, c.log2_stride - 4, rec, (e2 - jj) >> 1, K2, zr2, zi2);

@@ -98,6 +98,7 @@ struct sc_handle : EdgeCache {
   // by the all-FP64 path; compacted index list, count, gathered parameters and their results
   int escalate = 1; double esc_tau_poly = 6.0, esc_tau_mufu = 16.0;
   int quad_amp = 1;
+  int last_lg = 0, last_flavour = 0;   // sc_get_launch_info
   double esc_tau_nodes = 0.0;      // threshold the node spacing of the current call adds (select_stride_f32)
   int* d_esc_idx = nullptr; int* d_esc_count = nullptr; double* d_esc_params = nullptr; double* d_esc_out = nullptr;
   size_t esc_idx_cap = 0, esc_cnt_cap = 0, esc_par_cap = 0, esc_out_cap = 0; int* h_esc_hint = nullptr;
@@ -397,6 +398,11 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
         const bool quad = h->quad_amp && dc.stride >= 1024 && (long long)(e_last - e_first) >= 128LL * n_seg;
         a.merge_lim = 86400.0 * (kNodeDaysF32 / 4.0) / h->cfg.T_obs_s;
         const dim3 grid_tc(pblocks, n_chunks);
+        if (!esc_count) {
+          h->last_lg = dc.log2_stride;
+          h->last_flavour = (sincos == 2 ? SC_FLAVOUR_MUFU : 0) | (fused3 ? SC_FLAVOUR_AET : use_tc ? SC_FLAVOUR_TC :
+                            ((merge ? SC_FLAVOUR_MERGE : 0) | ((quad && merge && sincos == 2 && !seg_mode) ? SC_FLAVOUR_QUAD : 0)));
+        }
         if (fused3) {
           const ulonglong2* D3p = reinterpret_cast<const ulonglong2*>(h->D3);
           const ulonglong2* Gp = reinterpret_cast<const ulonglong2*>(h->Gp3);
@@ -1494,6 +1500,13 @@ int sc_get_counters(sc_handle* h, int64_t* evaluated_bins, int64_t* kernel_launc
   SC_CUDA(h, cudaStreamSynchronize((cudaStream_t)stream));
   if (evaluated_bins) *evaluated_bins = (int64_t)v;
   if (kernel_launches) *kernel_launches = h->launches;
+  return SC_OK;
+}
+
+int sc_get_launch_info(sc_handle* h, int32_t* stride_log2, int32_t* flavour) {
+  if (!h) return SC_ERR_NOT_INIT;
+  if (stride_log2) *stride_log2 = h->last_lg;
+  if (flavour) *flavour = h->last_flavour;
   return SC_OK;
 }
 
