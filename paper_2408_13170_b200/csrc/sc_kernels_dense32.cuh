@@ -444,12 +444,15 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2(DevCfg c, Den
   const int ce2 = (ce + 1) & ~1;                               // pair-aligned end (data beyond n_bins is zero)
   const int p = blockIdx.y * kBlock + threadIdx.x;
 
-  // no particle of this block has its time window in this chunk (common once the batch is sorted by window centre):
-  // leave empty fragments and skip the staging of the data
+  // no particle of this block has its time window in this chunk (common once the batch is sorted by window centre): skip
+  // the staging of the data.  k_stitch reads a particle's fragments only in the chunks its window overlaps, i.e. never
+  // those of such a CTA; k_stitch_seg (SEG) reads every chunk and gets empty fragments.
   if (!__syncthreads_or((a.jhi[p] > cs) && (a.jlo[p] < ce))) {
-    double* fz = a.frag + (size_t)chunk_l * kFragFields * a.P_pad + p;
+    if constexpr (SEG) {
+      double* fz = a.frag + (size_t)chunk_l * kFragFields * a.P_pad + p;
 #pragma unroll
-    for (int m = 0; m < kFragFields; ++m) fz[(size_t)m * a.P_pad] = 0.0;
+      for (int m = 0; m < kFragFields; ++m) fz[(size_t)m * a.P_pad] = 0.0;
+    }
     return;
   }
 

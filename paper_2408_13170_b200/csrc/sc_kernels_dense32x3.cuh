@@ -133,10 +133,12 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE3_MINB) k_dense3(DevCfg c, Den
   const int ce2 = (ce + 1) & ~1;                               // pair-aligned end (data beyond n_bins is zero)
   const int p = blockIdx.y * kBlock + threadIdx.x;
 
-  if (!__syncthreads_or((a.jhi[p] > cs) && (a.jlo[p] < ce))) {
-    double* fz = a.frag + (size_t)chunk_l * kFragFields * a.P_pad + p;
+  if (!__syncthreads_or((a.jhi[p] > cs) && (a.jlo[p] < ce))) {     // (see k_dense2: only k_stitch_seg reads these fragments)
+    if constexpr (SEG) {
+      double* fz = a.frag + (size_t)chunk_l * kFragFields * a.P_pad + p;
 #pragma unroll
-    for (int m = 0; m < kFragFields; ++m) fz[(size_t)m * a.P_pad] = 0.0;
+      for (int m = 0; m < kFragFields; ++m) fz[(size_t)m * a.P_pad] = 0.0;
+    }
     return;
   }
   {

@@ -188,10 +188,12 @@ __global__ void __launch_bounds__(kBlock) k_dense(DevCfg c, DenseArgs a, const d
   }
   if (!ESC) {                                                  // as in k_dense2: nothing of this block lives in this chunk
     const int p0 = blockIdx.y * kBlock + threadIdx.x;
-    if (!__syncthreads_or((a.jhi[p0] > cs) && (a.jlo[p0] < ce))) {
-      double* fz = a.frag + (size_t)chunk_l * kFragFields * a.P_pad + p0;
+    if (!__syncthreads_or((a.jhi[p0] > cs) && (a.jlo[p0] < ce))) {   // (see k_dense2: only k_stitch_seg reads these fragments)
+      if constexpr (SEG) {
+        double* fz = a.frag + (size_t)chunk_l * kFragFields * a.P_pad + p0;
 #pragma unroll
-      for (int m = 0; m < kFragFields; ++m) fz[(size_t)m * a.P_pad] = 0.0;
+        for (int m = 0; m < kFragFields; ++m) fz[(size_t)m * a.P_pad] = 0.0;
+      }
       return;
     }
   }

@@ -400,8 +400,10 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
         const dim3 grid_tc(pblocks, n_chunks);
         if (!esc_count) {
           h->last_lg = dc.log2_stride;
-          h->last_flavour = (sincos == 2 ? SC_FLAVOUR_MUFU : 0) | (fused3 ? SC_FLAVOUR_AET : use_tc ? SC_FLAVOUR_TC :
-                            ((merge ? SC_FLAVOUR_MERGE : 0) | ((quad && merge && sincos == 2 && !seg_mode) ? SC_FLAVOUR_QUAD : 0)));
+          const bool quad_on = quad && sincos == 2 && !seg_mode;
+          h->last_flavour = (sincos == 2 ? SC_FLAVOUR_MUFU : 0) |
+                            (fused3 ? SC_FLAVOUR_AET : use_tc ? SC_FLAVOUR_TC :   // (k_dense3 with quadratic runs: 26.9 -> 30.3 ms on c3, spills; not built)
+                             ((merge ? SC_FLAVOUR_MERGE : 0) | ((quad_on && merge) ? SC_FLAVOUR_QUAD : 0)));
         }
         if (fused3) {
           const ulonglong2* D3p = reinterpret_cast<const ulonglong2*>(h->D3);

@@ -697,3 +697,36 @@ def test_c5_adaptive_short_windows(oracle, torch_cuda, sc):
     assert same.sum() > 1200
     assert rel_err(a[same], b[same]).max() <= 2e-7
     assert np.all(np.diff(ea, axis=1) >= 0) and np.all(ea[:, -1] == inp["cfg"]["n_bins"]) and np.all(ea[:, 0] == 0)
+
+
+def test_node_spacing_error_model(oracle, torch_cuda, sc):
+    """with the coarse node spacing forced (all-FP64 kernels, so nothing but the interpolation shows), the
+    error of Upsilon stays below K days^6 / sqrt(N') -- days = signal time per coarse interval at the slowest-chirping corner,
+    N' = segments inside the window, K = 7.5e-10 (N' = 1) and 1.4e-10 (N' >= 8) as measured -- which is what the spacing rules
+    (2 days all-FP64, 4 (N'/8)^(1/12) days FP32 amplitudes) are derived from.  c5: every window sits at that corner."""
+    inp = sy.config_inputs(5, P=160)
+    cfg, dA, dE = make_data(oracle, inp)
+    par = _dev(torch_cuda, inp["particles"])
+    nb, T = inp["cfg"]["n_bins"], inp["cfg"]["T_obs_s"]
+    tc_max = float(np.ceil(inp["hi"][2]))
+    s_per_bin = (8.0 / 3.0) * tc_max / ((inp["cfg"]["j0"] / T) * T)
+    levels = [1, 5000, 50000]
+    edges = [sy.edges(nb, N) for N in levels]
+    ref = oracle.eval_stat_levels(oracle.make_config(inp["cfg"], truth=True), dA, dE, inp["S_A"], inp["S_E"], inp["particles"], edges)
+    worst = {}
+    for lg in (7, 8, 9):
+        H = gpu_handle(inp, dA, dE)
+        H.set_option(sc.SC_OPT_TC_MAX_S, int(tc_max))
+        H.set_option(sc.SC_OPT_STRIDE_LOG2, lg)
+        H.set_option(sc.SC_OPT_PRECISION, 2)
+        days = (1 << lg) * s_per_bin / 86400.0
+        for N, e, r in zip(levels, edges, ref):
+            got = H.eval_stat(par, e).cpu().numpy()
+            phi = H.counters()[0] / (len(r) * nb)
+            live = r > 0
+            n_eff = max(1.0, N * phi)
+            K = 7.5e-10 if N == 1 else 1.4e-10
+            worst[(lg, N)] = rel_err(got[live], r[live]).max()
+            assert worst[(lg, N)] <= 2.0 * K * days ** 6 / np.sqrt(n_eff) + 2e-9, (lg, N, days, n_eff, worst[(lg, N)])
+        H.close()
+    assert worst[(9, 1)] > 50 * worst[(7, 1)]             # ~ days^6: the model is not vacuous
