@@ -190,7 +190,7 @@ __global__ void k_scan_chunks(double* __restrict__ cbase, int n_chunks, int P_pa
 // a time in FP64 and a warp scan gives the cumulative sums (a lane walking its own bins alone would run at 1/32 efficiency).
 __device__ __forceinline__ double shfl_d(double v, int src) { return __shfl_sync(0xffffffffu, v, src); }
 template <int NA = 4>
-__global__ void __launch_bounds__(kBlock) k_edges64(DevCfg c, DenseArgs a, AdaptArgs ad) {
+__global__ void __launch_bounds__(kBlock, NA == 6 ? 4 : 6) k_edges64(DevCfg c, DenseArgs a, AdaptArgs ad) {
   constexpr int CH = kChunkF32;
   const int chunk = blockIdx.x;
   const int cs = chunk * CH;
@@ -245,10 +245,25 @@ __global__ void __launch_bounds__(kBlock) k_edges64(DevCfg c, DenseArgs a, Adapt
         if (lane == 0 && erow_L) erow_L[k_L] = j;
         t_L = (k_L < k1_L) ? seg_target(C_L, k_L + 1, N) - cb0_L : INFINITY;
       };
-      for (int j0 = ib; j0 < ie && k_L < k1_L; j0 += 32) {
+      // (the sigma weights of kPre rounds are fetched together: the rounds are serial, their loads need not be)
+      constexpr int kPre = 4;
+      for (int jb = ib; jb < ie && k_L < k1_L; jb += 32 * kPre) {
+      double2 gw[kPre];
+      double gt[kPre];
+#pragma unroll
+      for (int u = 0; u < kPre; ++u) {
+        const int j = jb + 32 * u + lane;
+        const bool in = (j < ie) && (j >= jlo_L) && (j < jhi_L);
+        gw[u] = in ? ad.G64[j] : make_double2(0.0, 0.0);
+        gt[u] = (NA == 6 && in) ? ad.GT64[j].x : 0.0;
+      }
+#pragma unroll
+      for (int u = 0; u < kPre; ++u) {
+        const int j0 = jb + 32 * u;
+        if (j0 >= ie || k_L >= k1_L) break;
         const int j = j0 + lane;
         double sj = 0.0;
-        if (j < ie && j >= jlo_L && j < jhi_L) sj = sigma_bin64<NA>(g, (double)(j - ib) * hS, ad.G64[j], NA == 6 ? ad.GT64[j].x : 0.0);
+        if (j < ie && j >= jlo_L && j < jhi_L) sj = sigma_bin64<NA>(g, (double)(j - ib) * hS, gw[u], gt[u]);
         double inc = sj;                                       // inclusive warp scan, fixed order
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) { const double up = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += up; }
@@ -261,6 +276,7 @@ __global__ void __launch_bounds__(kBlock) k_edges64(DevCfg c, DenseArgs a, Adapt
           close_L(j0 + __ffs(hit) - 1);
         }
         crel_L += tot;
+      }
       }
       while (k_L < k1_L && crel_L >= t_L) close_L(ie);
       if (lane == L) { crel = crel_L; t_next = t_L; k = k_L; }
