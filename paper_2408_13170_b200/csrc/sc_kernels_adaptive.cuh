@@ -287,10 +287,13 @@ __global__ void __launch_bounds__(kBlock, NA == 6 ? 4 : 6) k_edges64(DevCfg c, D
 
 // NA = 6 (three-channel handles): the pair loop, the masked pairs and the moments of k_dense3; Dg = the fused records
 // (wA, wE, wT), Gp = the sigma weights per bin pair (masked pairs only); no merged coarse intervals.
-template <int SC, bool MERGE = false, int NA = 4>
+// QUAD (two channels, fine sub-intervals >= 256 bins): the unmasked runs evaluate the amplitudes as quadratics over runs of
+// a quarter sub-interval (pairs_fast_q of sc_kernels_dense32.cuh); the run state lives across the 32-bin groups.
+template <int SC, bool MERGE = false, int NA = 4, bool QUAD = false>
 __global__ void __launch_bounds__(kBlock, NA == 6 ? SC_DENSE3_MINB : SC_DENSE2_MINB)
 k_dense2_ad(DevCfg c, DenseArgs a, AdaptArgs ad, const ulonglong2* __restrict__ Dg, const ulonglong2* __restrict__ Gp = nullptr) {
   static_assert(!(MERGE && NA == 6), "merged coarse intervals are a two-channel variant");
+  static_assert(!(QUAD && NA == 6), "quadratic runs are a two-channel variant");
   constexpr int CH = kChunkF32;
   constexpr int kRec = (NA == 6) ? kPairRec3 : kPairRec;
   __shared__ ulonglong2 sD[CH / 2 * kRec];
@@ -325,8 +328,17 @@ k_dense2_ad(DevCfg c, DenseArgs a, AdaptArgs ad, const ulonglong2* __restrict__ 
     if constexpr (NA == 6) return sigma_moments3(cfx, m + idx * 4, mT + idx * 4);
     else return sigma_moments(cfx, m + idx * 4);
   };
-  auto run_pairs = [&](PhaseFD& phx, const float (&cfx)[NA][4], u64& s2x, const ulonglong2*& recx, int n, u64& zr2, u64& zi2) {
+  QuadState qs;
+  int q_off = -1;                               // bins from the sub-interval start where qs stands (-1: nowhere)
+  const int lg_run = c.log2_stride - 4;
+  // off = first bin of the run of pairs, counted from the sub-interval start
+  auto run_pairs = [&](PhaseFD& phx, const float (&cfx)[NA][4], u64& s2x, const ulonglong2*& recx, int n, u64& zr2, u64& zi2, int off) {
     if constexpr (NA == 6) pairs_fast3<SC>(phx, cfx, s2x, recx, n, h2, K2, zr2, zi2);
+    else if constexpr (QUAD) {
+      if (q_off != off) quad_start(cfx, off, lg_run, qs);
+      pairs_fast_q<SC>(phx, cfx, qs, lg_run, recx, n, K2, zr2, zi2);
+      q_off = off + 2 * n;
+    }
     else pairs_fast<SC>(phx, cfx, s2x, recx, n, h2, K2, zr2, zi2);
   };
   const int Gs = 1 << ad.lg_group;
@@ -390,6 +402,7 @@ k_dense2_ad(DevCfg c, DenseArgs a, AdaptArgs ad, const ulonglong2* __restrict__ 
       else sub_amps<double>(c, a, p, ib, cf);
     }
     u64 s2 = f2pack(0.0f, hS);
+    q_off = -1;                                 // new coefficients
     const ulonglong2* rec = sD + ((ib - cs) >> 1) * kRec;
     // First ask the question for the whole sub-interval (its moments are those k_sigma_chunks used): if no lane reaches its
     // next target in it, all its groups take the unmasked path and the group moments are not needed at all.
@@ -399,7 +412,7 @@ k_dense2_ad(DevCfg c, DenseArgs a, AdaptArgs ad, const ulonglong2* __restrict__ 
         const double sg_s = sig_mom(cf, ad.smom, ad.smomT, (size_t)(ib >> (c.log2_stride - 2)));
         for (int gs = ib; gs < ie; gs += Gs) {
           u64 zr2 = 0, zi2 = 0;
-          run_pairs(ph, cf, s2, rec, Gs >> 1, zr2, zi2);
+          run_pairs(ph, cf, s2, rec, Gs >> 1, zr2, zi2, gs - ib);
           float zrl, zrh, zil, zih;
           f2unpack(zr2, zrl, zrh); f2unpack(zi2, zil, zih);
           Zr += (double)(zrl + zrh); Zi += (double)(zil + zih);
@@ -414,12 +427,13 @@ k_dense2_ad(DevCfg c, DenseArgs a, AdaptArgs ad, const ulonglong2* __restrict__ 
       if (!slow) {
         const double sg_m = sig_mom(cf, ad.gmom, ad.gmomT, (size_t)(gs >> ad.lg_group));
         u64 zr2 = 0, zi2 = 0;
-        run_pairs(ph, cf, s2, rec, (ge - gs) >> 1, zr2, zi2);
+        run_pairs(ph, cf, s2, rec, (ge - gs) >> 1, zr2, zi2, gs - ib);
         float zrl, zrh, zil, zih;
         f2unpack(zr2, zrl, zrh); f2unpack(zi2, zil, zih);
         Zr += (double)(zrl + zrh); Zi += (double)(zil + zih);
         crel += sg_m;
       } else {
+        if constexpr (QUAD) s2 = f2pack((float)(gs - ib) * hS, (float)(gs + 1 - ib) * hS);   // (the quadratic runs do not advance it)
         for (int jj = gs; jj < ge; jj += 2) {
           u64 zr2 = 0, zi2 = 0, sg2 = 0;
           if constexpr (NA == 6) pair_eval3<SC>(ph, cf, s2, rec, Gp + (size_t)(jj >> 1) * 2, jj, jlo, jhi, h2, K2, zr2, zi2, sg2);

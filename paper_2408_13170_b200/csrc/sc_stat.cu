@@ -846,6 +846,7 @@ int run_adaptive(sc_handle* h, const double* params, int64_t P, int n_seg, doubl
       Timed tm(h, st, SC_TIME_DENSE);
       const ulonglong2* Dp = reinterpret_cast<const ulonglong2*>(h->D32);
       const bool merge = dc.stride >= 512;                     // as in run_batches
+      const bool quad = h->quad_amp && dc.stride >= 1024 && (long long)dc.n_bins >= 128LL * n_seg;
       a.merge_lim = 86400.0 * (kNodeDaysF32 / 4.0) / h->cfg.T_obs_s;
       if (three) {
         const ulonglong2* D3p = reinterpret_cast<const ulonglong2*>(h->D3);
@@ -853,6 +854,7 @@ int run_adaptive(sc_handle* h, const double* params, int64_t P, int n_seg, doubl
         if (sincos == 2) k_dense2_ad<2, false, 6><<<grid, kBlock, 0, st>>>(dc, a, ad, D3p, Gp);
         else k_dense2_ad<0, false, 6><<<grid, kBlock, 0, st>>>(dc, a, ad, D3p, Gp);
       }
+      else if (sincos == 2 && merge && quad) k_dense2_ad<2, true, 4, true><<<grid, kBlock, 0, st>>>(dc, a, ad, Dp);
       else if (sincos == 2 && merge) k_dense2_ad<2, true><<<grid, kBlock, 0, st>>>(dc, a, ad, Dp);
       else if (sincos == 2) k_dense2_ad<2><<<grid, kBlock, 0, st>>>(dc, a, ad, Dp);
       else if (merge) k_dense2_ad<0, true><<<grid, kBlock, 0, st>>>(dc, a, ad, Dp);
