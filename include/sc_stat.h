@@ -79,6 +79,11 @@ enum {
                                 sc_search_run measures the fraction itself when none is stated.  Per-segment output
                                 (sc_eval_segments) and per-particle segments (sc_eval_stat_adaptive: integer edges from the
                                 interpolated sigma) always keep the N' = 8 spacing. */
+  SC_OPT_QUAD_AMPLITUDES = 16, /* 1 (default): where the fine sub-intervals are >= 256 bins (node spacing >= 1024) and the segments
+                                >= 128 bins on average, the unmasked pair loop of k_dense2 / k_dense2_ad evaluates the amplitudes as
+                                quadratics over runs of a quarter sub-interval (22 packed FP32 instructions per bin pair instead of
+                                26; the dropped term is <= 3e-8 of the amplitude).  0: cubics
+                                everywhere. */
   SC_OPT_STRIDE_LOG2 = 5,    /* 0 = automatic (rule above), else log2 of the coarse node spacing in bins (3..12)   */
   SC_OPT_PROFILE = 6,        /* 1 = record a CUDA event pair around every kernel launch (read by sc_get_timing)     */
   SC_OPT_SINCOS = 7,         /* FP32 amplitude path: sin/cos of the phase.  0 = automatic: hardware MUFU sin/cos

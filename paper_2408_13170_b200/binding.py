@@ -16,6 +16,7 @@ SC_OPT_ESCALATE, SC_OPT_ESC_TAU_POLY_X1000, SC_OPT_ESC_TAU_MUFU_X1000, SC_OPT_WI
 SC_OPT_TENSOR_CORES = 13
 SC_OPT_FUSED_AET = 14
 SC_OPT_WINDOW_FRACTION_PPM = 15
+SC_OPT_QUAD_AMPLITUDES = 16
 SC_TIMING_CLASSES = ["nodes", "dense", "stitch", "pso", "other", "escalation"]
 
 EXPORTED_SYMBOLS = ["sc_init_data", "sc_init_data_host", "sc_init_data3", "sc_gen_template3", "sc_eval_stat", "sc_eval_stat_host", "sc_eval_segments",

@@ -1602,6 +1602,9 @@ int sc_set_option(sc_handle* h, int32_t option, int64_t value) {
     case SC_OPT_TC_MAX_S:
       if (value < 1) return fail(h, SC_ERR_INVALID_ARG, "tc_max_s must be >= 1");
       h->tc_max_s = (double)value; set_stride(h); return SC_OK;
+    case SC_OPT_QUAD_AMPLITUDES:
+      if (value < 0 || value > 1) return fail(h, SC_ERR_INVALID_ARG, "quad_amplitudes must be 0 or 1");
+      h->quad_amp = (int)value; return SC_OK;
     case SC_OPT_WINDOW_FRACTION_PPM:
       if (value < 0 || value > 1000000) return fail(h, SC_ERR_INVALID_ARG, "window fraction must be 0 (not stated) .. 1000000 ppm");
       h->win_frac = (double)value * 1e-6; return SC_OK;

@@ -78,3 +78,30 @@ def test_launch_info_and_window_fraction_hint(torch_cuda, sc):
     with pytest.raises(sc.SCError):
         H.set_option(sc.SC_OPT_WINDOW_FRACTION_PPM, 1000001)
     H.close()
+
+
+def test_quadratic_amplitude_runs_are_a_small_perturbation(torch_cuda, sc):
+    """SC_OPT_QUAD_AMPLITUDES: the QUAD flavour of the pair loop (shared edges and per-particle segments) against the cubic one on
+    the same handle -- the economised u^3 term is <= 3e-8 of the amplitude, so Upsilon moves by far less than the 1e-6 bar."""
+    import numpy as np
+    import sc_synth as sy
+    inp = sy.config_inputs(3, P=512)
+    t = lambda a: torch_cuda.from_numpy(np.ascontiguousarray(a)).to("cuda:0")
+    H = sc.Handle(inp["cfg"], torch_cuda.view_as_real(t(inp["noise_A"])).contiguous(), torch_cuda.view_as_real(t(inp["noise_E"])).contiguous(),
+                  t(inp["S_A"]), t(inp["S_E"]))
+    H.set_option(sc.SC_OPT_TC_MAX_S, int(np.ceil(inp["hi"][2])))
+    par, e = t(inp["particles"]), inp["edges"][5000]
+    st = torch_cuda.empty(512, dtype=torch_cuda.float64, device="cuda:0")
+    out = {}
+    for quad in (1, 0):
+        H.set_option(sc.SC_OPT_QUAD_AMPLITUDES, quad)
+        out[("shared", quad)] = H.eval_stat(par, e).cpu().numpy()
+        assert bool(H.launch_info()[1] & sc.SC_FLAVOUR_QUAD) == bool(quad)
+        sc.sc_eval_stat_adaptive(H.h, par, 512, 100, st)
+        out[("adaptive", quad)] = st.cpu().numpy().copy()
+    for kind in ("shared", "adaptive"):
+        a, b = out[(kind, 1)], out[(kind, 0)]
+        live = b > 0
+        d = np.abs(a[live] - b[live]) / b[live]
+        assert live.sum() > 400 and d.max() < 5e-8 and d.max() > 0, (kind, d.max())
+    H.close()
