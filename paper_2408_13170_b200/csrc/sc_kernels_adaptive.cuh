@@ -287,13 +287,13 @@ __global__ void __launch_bounds__(kBlock, NA == 6 ? 4 : 6) k_edges64(DevCfg c, D
 
 // NA = 6 (three-channel handles): the pair loop, the masked pairs and the moments of k_dense3; Dg = the fused records
 // (wA, wE, wT), Gp = the sigma weights per bin pair (masked pairs only); no merged coarse intervals.
-// QUAD (two channels, fine sub-intervals >= 256 bins): the unmasked runs evaluate the amplitudes as quadratics over runs of
+// QUAD (fine sub-intervals >= 256 bins): the unmasked runs evaluate the amplitudes as quadratics over runs of
 // a quarter sub-interval (pairs_fast_q of sc_kernels_dense32.cuh); the run state lives across the 32-bin groups.
 template <int SC, bool MERGE = false, int NA = 4, bool QUAD = false>
 __global__ void __launch_bounds__(kBlock, NA == 6 ? SC_DENSE3_MINB : SC_DENSE2_MINB)
 k_dense2_ad(DevCfg c, DenseArgs a, AdaptArgs ad, const ulonglong2* __restrict__ Dg, const ulonglong2* __restrict__ Gp = nullptr) {
   static_assert(!(MERGE && NA == 6), "merged coarse intervals are a two-channel variant");
-  static_assert(!(QUAD && NA == 6), "quadratic runs are a two-channel variant");
+
   constexpr int CH = kChunkF32;
   constexpr int kRec = (NA == 6) ? kPairRec3 : kPairRec;
   __shared__ ulonglong2 sD[CH / 2 * kRec];
@@ -328,17 +328,21 @@ k_dense2_ad(DevCfg c, DenseArgs a, AdaptArgs ad, const ulonglong2* __restrict__ 
     if constexpr (NA == 6) return sigma_moments3(cfx, m + idx * 4, mT + idx * 4);
     else return sigma_moments(cfx, m + idx * 4);
   };
-  QuadState qs;
+  typename std::conditional<NA == 6, QuadState3, QuadState>::type qs;
   int q_off = -1;                               // bins from the sub-interval start where qs stands (-1: nowhere)
   const int lg_run = c.log2_stride - 4;
   // off = first bin of the run of pairs, counted from the sub-interval start
   auto run_pairs = [&](PhaseFD& phx, const float (&cfx)[NA][4], u64& s2x, const ulonglong2*& recx, int n, u64& zr2, u64& zi2, int off) {
-    if constexpr (NA == 6) pairs_fast3<SC>(phx, cfx, s2x, recx, n, h2, K2, zr2, zi2);
-    else if constexpr (QUAD) {
+    if constexpr (QUAD && NA == 6) {
+      if (q_off != off) quad_start3(cfx, off, lg_run, qs);
+      pairs_fast3_q<SC>(phx, cfx, qs, lg_run, recx, n, K2, zr2, zi2);
+      q_off = off + 2 * n;
+    } else if constexpr (QUAD) {
       if (q_off != off) quad_start(cfx, off, lg_run, qs);
       pairs_fast_q<SC>(phx, cfx, qs, lg_run, recx, n, K2, zr2, zi2);
       q_off = off + 2 * n;
     }
+    else if constexpr (NA == 6) pairs_fast3<SC>(phx, cfx, s2x, recx, n, h2, K2, zr2, zi2);
     else pairs_fast<SC>(phx, cfx, s2x, recx, n, h2, K2, zr2, zi2);
   };
   const int Gs = 1 << ad.lg_group;

@@ -118,6 +118,69 @@ __device__ __forceinline__ void pairs_fast3(PhaseFD& ph, const float (&cf)[6][4]
   mac_pair3(cf, s2, wA, wE, wT, h2, cr, sr, zr2, zi2);
 }
 
+// QUAD flavour for six amplitude parts (see pairs_fast_q in sc_kernels_dense32.cuh): quadratic amplitudes over runs of a
+// quarter sub-interval, 12 packed FMAs per bin pair instead of 18.  Used by k_dense2_ad<.., 6> (no spills there); in
+// k_dense3 the 24 cubic + 18 quadratic coefficients spill and the kernel gets slower (26.9 -> 30.3 ms on c3), so it keeps
+// the cubics.
+struct QuadState3 { float q[6][3]; u64 u2; int left; int r; };
+__device__ __forceinline__ void quad_run3(const float (&cf)[6][4], int r, QuadState3& o) {
+  const float s0 = 0.25f * (float)r;
+#pragma unroll
+  for (int a = 0; a < 6; ++a) {
+    const float c0 = cf[a][0], c1 = cf[a][1], c2 = cf[a][2], c3 = cf[a][3];
+    const float a3 = c3 * (1.0f / 64.0f);
+    const float a2 = fmaf(3.0f * c3, s0, c2) * (1.0f / 16.0f);
+    const float a1 = fmaf(fmaf(3.0f * c3, s0, 2.0f * c2), s0, c1) * 0.25f;
+    const float a0 = fmaf(fmaf(fmaf(c3, s0, c2), s0, c1), s0, c0);
+    o.q[a][2] = fmaf(1.5f, a3, a2);
+    o.q[a][1] = fmaf(-0.5625f, a3, a1);
+    o.q[a][0] = fmaf(0.03125f, a3, a0);
+  }
+}
+__device__ __forceinline__ void quad_start3(const float (&cf)[6][4], int off, int lg_run, QuadState3& q) {
+  const int run_bins = 1 << lg_run;
+  const int o = off & (run_bins - 1);
+  const float hu = 1.0f / (float)run_bins;
+  q.r = off >> lg_run;
+  q.left = (run_bins - o) >> 1;
+  q.u2 = f2pack((float)o * hu, (float)(o + 1) * hu);
+  quad_run3(cf, q.r, q);
+}
+__device__ __forceinline__ u64 quad2(const float (&w)[3], u64 u2) { return f2fma(f2fma(f2bcast(w[2]), u2, f2bcast(w[1])), u2, f2bcast(w[0])); }
+__device__ __forceinline__ void mac_pair3_q(QuadState3& w, const ulonglong2 wA, const ulonglong2 wE, const ulonglong2 wT, u64 hu2,
+                                            u64 cr2, u64 sr2, u64& zr2, u64& zi2) {
+  const u64 Ar = quad2(w.q[0], w.u2), Ai = quad2(w.q[1], w.u2), Er = quad2(w.q[2], w.u2), Ei = quad2(w.q[3], w.u2);
+  const u64 Tr = quad2(w.q[4], w.u2), Ti = quad2(w.q[5], w.u2);
+  w.u2 = f2add(w.u2, hu2);
+  const u64 qr = f2fma(wA.x, Ar, f2fma(wA.y, Ai, f2fma(wE.x, Er, f2fma(wE.y, Ei, f2fma(wT.x, Tr, f2mul(wT.y, Ti))))));
+  const u64 qi = f2fma(wA.y, Ar, f2fma(f2neg(wA.x), Ai, f2fma(wE.y, Er, f2fma(f2neg(wE.x), Ei, f2fma(wT.y, Tr, f2neg(f2mul(wT.x, Ti)))))));
+  zr2 = f2fma(qr, cr2, f2fma(f2neg(qi), sr2, zr2));
+  zi2 = f2fma(qr, sr2, f2fma(qi, cr2, zi2));
+}
+template <int SC>
+__device__ __forceinline__ void pairs_fast3_q(PhaseFD& ph, const float (&cf)[6][4], QuadState3& q, int lg_run, const ulonglong2*& rec,
+                                              int n, u64 K2, u64& zr2, u64& zi2) {
+  const int run_pairs = 1 << (lg_run - 1);
+  const float hu = 1.0f / (float)(2 * run_pairs);
+  const u64 hu2 = f2bcast(2.0f * hu);
+  u64 cr, sr;
+  sincos_pair<SC>(ph, K2, cr, sr);
+  ulonglong2 wA = rec[0], wE = rec[1], wT = rec[2];
+#pragma unroll 1
+  for (int i = 1; i < n; ++i) {
+    u64 crn, srn;
+    sincos_pair<SC>(ph, K2, crn, srn);
+    rec += kPairRec3;
+    const ulonglong2 wAn = rec[0], wEn = rec[1], wTn = rec[2];
+    mac_pair3_q(q, wA, wE, wT, hu2, cr, sr, zr2, zi2);
+    if (--q.left == 0) { quad_run3(cf, ++q.r, q); q.left = run_pairs; q.u2 = f2pack(0.0f, hu); }
+    cr = crn; sr = srn; wA = wAn; wE = wEn; wT = wTn;
+  }
+  rec += kPairRec3;
+  mac_pair3_q(q, wA, wE, wT, hu2, cr, sr, zr2, zi2);
+  if (--q.left == 0) { quad_run3(cf, ++q.r, q); q.left = run_pairs; q.u2 = f2pack(0.0f, hu); }
+}
+
 #ifndef SC_DENSE3_MINB
 #define SC_DENSE3_MINB 4     /* CTAs per SM: 128 registers/thread with ~150 B of spills beats 168 registers at 3 CTAs (28.6 vs 32.0 ms on c3) */
 #endif

@@ -851,7 +851,8 @@ int run_adaptive(sc_handle* h, const double* params, int64_t P, int n_seg, doubl
       if (three) {
         const ulonglong2* D3p = reinterpret_cast<const ulonglong2*>(h->D3);
         const ulonglong2* Gp = reinterpret_cast<const ulonglong2*>(h->Gp3);
-        if (sincos == 2) k_dense2_ad<2, false, 6><<<grid, kBlock, 0, st>>>(dc, a, ad, D3p, Gp);
+        if (sincos == 2 && quad) k_dense2_ad<2, false, 6, true><<<grid, kBlock, 0, st>>>(dc, a, ad, D3p, Gp);
+        else if (sincos == 2) k_dense2_ad<2, false, 6><<<grid, kBlock, 0, st>>>(dc, a, ad, D3p, Gp);
         else k_dense2_ad<0, false, 6><<<grid, kBlock, 0, st>>>(dc, a, ad, D3p, Gp);
       }
       else if (sincos == 2 && merge && quad) k_dense2_ad<2, true, 4, true><<<grid, kBlock, 0, st>>>(dc, a, ad, Dp);
