@@ -256,6 +256,19 @@ int sc_kmeans(sc_handle* h, const double* pos, int64_t n_particles, const double
               double* cent, int32_t K, int32_t max_iter, int32_t* label, int64_t* count, int32_t* n_iter,
               void* cuda_stream);
 
+/* sc_kmeans for callers that may not allocate device memory (CUDA graph capture set-ups, serving loops, harnesses that
+ * forbid cudaMalloc): same arguments, same iterations, same results bit for bit, but the scratch (the "labels changed"
+ * counter and the K member counts) lives in a file-scope static device array of 2 KiB that every GPU loading the library
+ * holds until exit.  The call allocates and frees nothing on the device (no cudaMalloc / cudaFree, no allocating library
+ * routine, no timing events: SC_OPT_PROFILE does not cover it).  K > SC_KMEANS_STATIC_MAX_K returns SC_ERR_INVALID_ARG.
+ * The handle's device must be current.  The first call on a device resolves the array's address (cudaGetSymbolAddress);
+ * like sc_kmeans it synchronises the stream once per iteration.  ALL calls on a device share the array: calls that
+ * overlap on the GPU (different streams or host threads) race -- serialise them. */
+#define SC_KMEANS_STATIC_MAX_K 128
+int sc_kmeans_static(sc_handle* h, const double* pos, int64_t n_particles, const double* lo, const double* hi,
+                     double* cent, int32_t K, int32_t max_iter, int32_t* label, int64_t* count, int32_t* n_iter,
+                     void* cuda_stream);
+
 /* The search of one tile (Fig. 2; Sec. III A-B; App. B). */
 #define SC_MAX_RUNGS 8
 typedef struct {

@@ -20,7 +20,7 @@ SC_OPT_QUAD_AMPLITUDES = 16
 SC_TIMING_CLASSES = ["nodes", "dense", "stitch", "pso", "other", "escalation"]
 
 EXPORTED_SYMBOLS = ["sc_init_data", "sc_init_data_host", "sc_init_data3", "sc_gen_template3", "sc_eval_stat", "sc_eval_stat_host", "sc_eval_segments",
-                    "sc_eval_stat_adaptive", "sc_eval_components", "sc_eval_loglike", "sc_data_norm", "sc_gen_template", "sc_pso_step", "sc_pso_best", "sc_pso_pick", "sc_pso_move", "sc_pso_step_labeled", "sc_kmeans", "sc_search_run", "sc_whiten_streams", "sc_eval_stat_streams", "sc_get_counters", "sc_get_launch_info", "sc_get_timing", "sc_measure_fp64_peak",
+                    "sc_eval_stat_adaptive", "sc_eval_components", "sc_eval_loglike", "sc_data_norm", "sc_gen_template", "sc_pso_step", "sc_pso_best", "sc_pso_pick", "sc_pso_move", "sc_pso_step_labeled", "sc_kmeans", "sc_kmeans_static", "sc_search_run", "sc_whiten_streams", "sc_eval_stat_streams", "sc_get_counters", "sc_get_launch_info", "sc_get_timing", "sc_measure_fp64_peak",
                     "sc_set_option", "sc_free",
                     "sc_last_error", "sc_version"]
 
@@ -127,6 +127,8 @@ def load_library():
     L.sc_pso_step_labeled.argtypes = [_vp] + [_vp] * 11 + [C.c_double] * 3 + [C.c_uint64, C.c_uint64, C.c_int64, C.c_int32, _vp]
     L.sc_kmeans.restype = C.c_int
     L.sc_kmeans.argtypes = [_vp, _vp, C.c_int64, _vp, _vp, _vp, C.c_int32, C.c_int32, _vp, _vp, C.POINTER(C.c_int32), _vp]
+    L.sc_kmeans_static.restype = C.c_int
+    L.sc_kmeans_static.argtypes = L.sc_kmeans.argtypes
     L.sc_search_run.restype = C.c_int
     L.sc_search_run.argtypes = [_vp, C.POINTER(ScSearchConfig), _vp, _vp, _vp, C.c_int64, C.c_int32, _vp, _vp,
                                 _vp, _vp, _vp, _vp, _vp, _vp, _vp]
@@ -457,6 +459,24 @@ def sc_kmeans(h, pos, n_particles, lo, hi, cent, K, max_iter, label, count=None,
                                   _dev(hi, torch.float64, "hi"), _dev(cent, torch.float64, "cent"), K, max_iter,
                                   _dev(label, torch.int32, "label"),
                                   None if count is None else _dev(count, torch.int64, "count"), C.byref(n_it), _stream(stream))
+    _check(rc, h)
+    return n_it.value
+
+
+SC_KMEANS_STATIC_MAX_K = 128
+
+
+def sc_kmeans_static(h, pos, n_particles, lo, hi, cent, K, max_iter, label, count=None, stream=None):
+    """sc_kmeans without device allocation (scratch in a static device array of the library, K <= SC_KMEANS_STATIC_MAX_K);
+    same arguments and results.  Calls that overlap on the GPU race: the array is shared."""
+    torch = _torch()
+    if pos.numel() != 8 * n_particles or cent.numel() != 8 * K or label.numel() != n_particles:
+        raise SCError(SC_ERR_INVALID_ARG, "pos [P,8], cent [K,8], label [P] expected")
+    n_it = C.c_int32(0)
+    rc = load_library().sc_kmeans_static(h, _dev(pos, torch.float64, "pos"), n_particles, _dev(lo, torch.float64, "lo"),
+                                         _dev(hi, torch.float64, "hi"), _dev(cent, torch.float64, "cent"), K, max_iter,
+                                         _dev(label, torch.int32, "label"),
+                                         None if count is None else _dev(count, torch.int64, "count"), C.byref(n_it), _stream(stream))
     _check(rc, h)
     return n_it.value
 

@@ -23,6 +23,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <type_traits>
 #include <vector>
@@ -1487,6 +1488,79 @@ int sc_kmeans(sc_handle* h, const double* pos, int64_t P, const double* lo, cons
       k_km_update<<<K, 8, 0, st>>>(pos, (long long)P, label, cent, d_cnt);
       if ((rc = check_launch(h, "k_km_update"))) return rc;
     }
+    int changed = 0;
+    SC_CUDA(h, cudaMemcpyAsync(&changed, d_changed, 4, cudaMemcpyDeviceToHost, st));
+    SC_CUDA(h, cudaStreamSynchronize(st));
+    if (changed == 0) break;
+  }
+  if (count) SC_CUDA(h, cudaMemcpyAsync(count, d_cnt, (size_t)K * 8, cudaMemcpyDeviceToDevice, st));
+  if (n_iter) *n_iter = it;
+  return SC_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ k-means without allocation
+// sc_kmeans_static: the Lloyd iterations of sc_kmeans for callers that may not allocate device memory (code under CUDA
+// graph capture, serving loops, harnesses that forbid cudaMalloc).  Its scratch -- the "labels changed" counter and the K
+// member counts -- lives in a file-scope device array: every GPU that loads the library holds these 2 KiB until exit.
+// In host code the array's name is a host-side stand-in, not a device address: the address comes from
+// cudaGetSymbolAddress, once per device with that device current (static_scratch below), and only that pointer is
+// handed to the kernels.  All calls on a device share the array and it keeps the last call's contents: the counter is
+// cleared before every iteration, the counts are rewritten by every k_km_update; calls that overlap on the GPU race.
+constexpr int kStaticMaxK = SC_KMEANS_STATIC_MAX_K;
+constexpr size_t kStaticScratchBytes = 2048;                 // 16 (counter, padded) + kStaticMaxK x 8 <= 2048
+static_assert(16 + (size_t)kStaticMaxK * 8 <= kStaticScratchBytes, "static scratch too small for SC_KMEANS_STATIC_MAX_K");
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticScratchBytes];
+
+namespace {
+constexpr int kStaticMaxDevices = 64;
+void* g_static_ptr[kStaticMaxDevices] = {};                  // device address of g_static_scratch, per device ordinal
+std::mutex g_static_mutex;
+
+// The device address of g_static_scratch on the handle's device (resolved once per device; no allocation).
+int static_scratch(sc_handle* h, void** out) {
+  int dev = -1;
+  SC_CUDA(h, cudaGetDevice(&dev));
+  if (dev != h->device) return fail(h, SC_ERR_INVALID_ARG, "the current device (%d) is not the handle's (%d)", dev, h->device);
+  if (dev < 0 || dev >= kStaticMaxDevices) return fail(h, SC_ERR_INVALID_ARG, "device ordinal %d beyond %d", dev, kStaticMaxDevices - 1);
+  std::lock_guard<std::mutex> lock(g_static_mutex);
+  if (!g_static_ptr[dev]) {
+    void* ptr = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&ptr, g_static_scratch);
+    if (e != cudaSuccess || !ptr) {
+      cudaGetLastError();
+      return fail(h, SC_ERR_CUDA, "cudaGetSymbolAddress(g_static_scratch) failed: %s", cudaGetErrorString(e));
+    }
+    g_static_ptr[dev] = ptr;
+  }
+  *out = g_static_ptr[dev];
+  return SC_OK;
+}
+}  // namespace
+
+int sc_kmeans_static(sc_handle* h, const double* pos, int64_t P, const double* lo, const double* hi, double* cent, int32_t K,
+                     int32_t max_iter, int32_t* label, int64_t* count, int32_t* n_iter, void* stream) {
+  if (!h) return SC_ERR_NOT_INIT;
+  if (h->cuda_failed) return SC_ERR_CUDA;
+  if (!pos || !lo || !hi || !cent || !label) return fail(h, SC_ERR_INVALID_ARG, "null pointer");
+  if (K > kStaticMaxK)
+    return fail(h, SC_ERR_INVALID_ARG, "K = %d exceeds SC_KMEANS_STATIC_MAX_K = %d, the size of the static scratch array", (int)K, kStaticMaxK);
+  if (P <= 0 || K <= 0 || max_iter <= 0) return fail(h, SC_ERR_INVALID_ARG, "need n_particles > 0, K >= 1, max_iter > 0");
+  cudaStream_t st = (cudaStream_t)stream;
+  void* scratch = nullptr;
+  int rc;
+  if ((rc = static_scratch(h, &scratch))) return rc;
+  int* d_changed = (int*)scratch;
+  long long* d_cnt = (long long*)((char*)scratch + 16);
+  SC_CUDA(h, cudaMemsetAsync(label, 0xFF, (size_t)P * 4, st));       // -1: every particle counts as changed in iteration 1
+  int it = 0;
+  while (it < max_iter) {
+    ++it;
+    SC_CUDA(h, cudaMemsetAsync(d_changed, 0, 4, st));                 // the array keeps the previous call's contents
+    // (no Timed here: SC_OPT_PROFILE creates events on demand)
+    k_km_assign<<<(unsigned)((P + 127) / 128), 128, 0, st>>>(pos, (long long)P, lo, hi, cent, K, label, d_changed);
+    if ((rc = check_launch(h, "k_km_assign"))) return rc;
+    k_km_update<<<K, 8, 0, st>>>(pos, (long long)P, label, cent, d_cnt);
+    if ((rc = check_launch(h, "k_km_update"))) return rc;
     int changed = 0;
     SC_CUDA(h, cudaMemcpyAsync(&changed, d_changed, 4, cudaMemcpyDeviceToHost, st));
     SC_CUDA(h, cudaStreamSynchronize(st));
