@@ -41,8 +41,9 @@ __device__ __forceinline__ void fine_cubic2(const u64 nd[6], int q, u64 out[4]) 
 }
 
 #ifndef SC_QUAD_FLUSH
-#define SC_QUAD_FLUSH 64     /* bins per FP32 flush group of the QUAD flavour's unmasked runs (measured on c3, 264 particles:
-                                32 bins 18.47 ms, rms error 4.2e-9; 64 bins 18.04 ms; 128 bins 17.83 ms, rms 5.6e-9) */
+#define SC_QUAD_FLUSH 128     /* bins per FP32 flush group of the QUAD flavour's unmasked runs (measured on c3, 264 particles:
+                                32 bins 18.47 ms, rms error 4.2e-9; 64 bins 18.04 ms; 128 bins 17.85 ms, rms 5.6e-9, and error x sqrt(Upsilon) <= 1.73e-6
+                                over c2 / c3 / c4 samples, i.e. <= 4.3e-7 at the escalation threshold tau = 16) */
 #endif
 #ifndef SC_DENSE2_MINB
 #define SC_DENSE2_MINB 4     /* CTAs per SM the register allocation aims at (128 registers/thread) */
