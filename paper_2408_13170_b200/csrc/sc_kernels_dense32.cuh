@@ -434,10 +434,36 @@ __device__ __forceinline__ void pairs_fast_q(PhaseFD& ph, const float (&cf)[4][4
   if (--q.left == 0) { quad_run(cf, ++q.r, q.w); q.left = run_pairs; q.u2 = f2pack(0.0f, hu); }
 }
 
+// Staging of the chunk's data records: ONE bulk copy (cp.async.bulk, the TMA unit) of 48 KB issued by thread 0, completion on
+// an mbarrier; the threads load their per-particle state while it is in flight and wait on the barrier before the walk.
+namespace stg {
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t b, uint32_t cnt) { asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(b), "r"(cnt)); }
+__device__ __forceinline__ void mbar_expect_tx(uint32_t b, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(b), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t b, uint32_t parity) {
+  asm volatile("{\n.reg .pred P1;\nLAB_WAIT:\nmbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n@P1 bra DONE;\nbra LAB_WAIT;\nDONE:\n}"
+               :: "r"(b), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               :: "r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+}  // namespace stg
+constexpr int kDense2DataBytes = kChunkF32 / 2 * kPairRec * 16;              // 48 KB of data records per chunk
+constexpr int kDense2Smem = kDense2DataBytes + 16;                           // + the mbarrier (dynamic shared memory: > 48 KB)
+
 template <bool SEG, int SC, bool MERGE = false, bool QUAD = false>
 __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2(DevCfg c, DenseArgs a, const ulonglong2* __restrict__ Dg) {
   constexpr int CH = kChunkF32;
-  __shared__ ulonglong2 sD[CH / 2 * kPairRec];                 // 48 KB
+  extern __shared__ __align__(128) unsigned char smem_d2[];
+  ulonglong2* sD = reinterpret_cast<ulonglong2*>(smem_d2);     // 48 KB
+  const uint32_t bar = stg::smem_u32(smem_d2 + kDense2DataBytes);
+  if (threadIdx.x == 0) {
+    stg::mbar_init(bar, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
 
   const int chunk_l = blockIdx.x;
   const int cs = (a.chunk_first + chunk_l) * CH;
@@ -457,12 +483,11 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2(DevCfg c, Den
     return;
   }
 
-  {
-    const ulonglong2* src = Dg + (size_t)(cs >> 1) * kPairRec;
-#pragma unroll 4
-    for (int t = threadIdx.x; t < CH / 2 * kPairRec; t += kBlock) sD[t] = src[t];
+  // (the __syncthreads_or above orders the barrier's initialisation before every wait)
+  if (threadIdx.x == 0) {
+    stg::mbar_expect_tx(bar, kDense2DataBytes);
+    stg::bulk_g2s(stg::smem_u32(sD), Dg + (size_t)(cs >> 1) * kPairRec, kDense2DataBytes, bar);
   }
-  __syncthreads();
 
   const int jlo = a.jlo[p], jhi = a.jhi[p];
   const int S = c.stride, Sf = S >> 2;
@@ -504,6 +529,7 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2(DevCfg c, Den
   PhaseFD fd = {};
   float cc[MERGE ? 4 : 1][4];  // merged coarse interval: cubic of the amplitudes in t = (j - coarse start)/stride
   int merged_left = 0;         // fine sub-intervals of the current merged coarse interval still to walk
+  bool landed = false;         // the chunk's data records: waited for after the first sub-interval's set-up (node reads only)
   for (int ib = cs; ib < ce2; ib += Sf) {
     const int ie = min(ib + Sf, ce2);
     const bool lane_in = (ib >= jlo) && (ie <= jhi);
@@ -529,6 +555,7 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2(DevCfg c, Den
       sub_amps(c, a, p, ib, cf);
     }
 
+    if (!landed) { stg::mbar_wait(bar, 0); landed = true; }
     u64 s2 = 0;        // (s_j, s_{j+1}) of the next pair
     const ulonglong2* rec = sD;   // its data record
     auto pair = [&](int j, auto masked_c, auto with_sg_c, u64& zr2, u64& zi2, u64& sg2) {

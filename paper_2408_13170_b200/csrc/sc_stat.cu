@@ -422,15 +422,15 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
           else if (merge) k_dense2_tc<false, 0, true><<<grid_tc, tc::kThreads, tc::kSmemBytes, st>>>(dc, a, Dp, Tg);
           else k_dense2_tc<false, 0><<<grid_tc, tc::kThreads, tc::kSmemBytes, st>>>(dc, a, Dp, Tg);
         }
-        else if (seg_mode && sincos == 2 && merge) k_dense2<true, 2, true><<<grid, kBlock, 0, st>>>(dc, a, Dp);
-        else if (seg_mode && sincos == 2) k_dense2<true, 2><<<grid, kBlock, 0, st>>>(dc, a, Dp);
-        else if (seg_mode && merge) k_dense2<true, 0, true><<<grid, kBlock, 0, st>>>(dc, a, Dp);
-        else if (seg_mode) k_dense2<true, 0><<<grid, kBlock, 0, st>>>(dc, a, Dp);
-        else if (sincos == 2 && merge && quad) k_dense2<false, 2, true, true><<<grid, kBlock, 0, st>>>(dc, a, Dp);
-        else if (sincos == 2 && merge) k_dense2<false, 2, true><<<grid, kBlock, 0, st>>>(dc, a, Dp);
-        else if (sincos == 2) k_dense2<false, 2><<<grid, kBlock, 0, st>>>(dc, a, Dp);
-        else if (merge) k_dense2<false, 0, true><<<grid, kBlock, 0, st>>>(dc, a, Dp);
-        else k_dense2<false, 0><<<grid, kBlock, 0, st>>>(dc, a, Dp);
+        else if (seg_mode && sincos == 2 && merge) k_dense2<true, 2, true><<<grid, kBlock, kDense2Smem, st>>>(dc, a, Dp);
+        else if (seg_mode && sincos == 2) k_dense2<true, 2><<<grid, kBlock, kDense2Smem, st>>>(dc, a, Dp);
+        else if (seg_mode && merge) k_dense2<true, 0, true><<<grid, kBlock, kDense2Smem, st>>>(dc, a, Dp);
+        else if (seg_mode) k_dense2<true, 0><<<grid, kBlock, kDense2Smem, st>>>(dc, a, Dp);
+        else if (sincos == 2 && merge && quad) k_dense2<false, 2, true, true><<<grid, kBlock, kDense2Smem, st>>>(dc, a, Dp);
+        else if (sincos == 2 && merge) k_dense2<false, 2, true><<<grid, kBlock, kDense2Smem, st>>>(dc, a, Dp);
+        else if (sincos == 2) k_dense2<false, 2><<<grid, kBlock, kDense2Smem, st>>>(dc, a, Dp);
+        else if (merge) k_dense2<false, 0, true><<<grid, kBlock, kDense2Smem, st>>>(dc, a, Dp);
+        else k_dense2<false, 0><<<grid, kBlock, kDense2Smem, st>>>(dc, a, Dp);
       } else {
         if (seg_mode) k_dense<true><<<grid, kBlock, kDense64Smem, st>>>(dc, a, h->W64, h->G64);
         else if (esc_count) k_dense<false, true><<<grid, kBlock, kDense64Smem, st>>>(dc, a, h->W64, h->G64);
@@ -923,6 +923,15 @@ int init_common(sc_handle** out, const sc_config* cfg, const double* dA, const d
   SC_INIT(cudaFuncSetAttribute(k_dense<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kDense64Smem));
   SC_INIT(cudaFuncSetAttribute(k_dense<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kDense64Smem));
   SC_INIT(cudaFuncSetAttribute(k_dense<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kDense64Smem));
+  SC_INIT(cudaFuncSetAttribute(k_dense2<false, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kDense2Smem));
+  SC_INIT(cudaFuncSetAttribute(k_dense2<false, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, kDense2Smem));
+  SC_INIT(cudaFuncSetAttribute(k_dense2<false, 2, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kDense2Smem));
+  SC_INIT(cudaFuncSetAttribute(k_dense2<false, 2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kDense2Smem));
+  SC_INIT(cudaFuncSetAttribute(k_dense2<false, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kDense2Smem));
+  SC_INIT(cudaFuncSetAttribute(k_dense2<true, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kDense2Smem));
+  SC_INIT(cudaFuncSetAttribute(k_dense2<true, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, kDense2Smem));
+  SC_INIT(cudaFuncSetAttribute(k_dense2<true, 2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kDense2Smem));
+  SC_INIT(cudaFuncSetAttribute(k_dense2<true, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kDense2Smem));
   SC_INIT(cudaFuncSetAttribute(k_dense2_tc<true, 0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::kSmemBytes));
   SC_INIT(cudaFuncSetAttribute(k_dense2_tc<false, 2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::kSmemBytes));
   SC_INIT(cudaFuncSetAttribute(k_dense2_tc<false, 2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::kSmemBytes));
