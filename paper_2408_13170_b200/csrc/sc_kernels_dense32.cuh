@@ -434,7 +434,7 @@ __device__ __forceinline__ void pairs_fast_q(PhaseFD& ph, const float (&cf)[4][4
   if (--q.left == 0) { quad_run(cf, ++q.r, q.w); q.left = run_pairs; q.u2 = f2pack(0.0f, hu); }
 }
 
-// Staging of the chunk's data records: ONE bulk copy (cp.async.bulk, the TMA unit) of 48 KB issued by thread 0, completion on
+// Staging of the chunk's data records (all flavours but the segment-table one): ONE bulk copy (cp.async.bulk, the TMA unit) of 48 KB issued by thread 0, completion on
 // an mbarrier; the threads load their per-particle state while it is in flight and wait on the barrier before the walk.
 namespace stg {
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -457,12 +457,21 @@ constexpr int kDense2Smem = kDense2DataBytes + 16;                           // 
 template <bool SEG, int SC, bool MERGE = false, bool QUAD = false>
 __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2(DevCfg c, DenseArgs a, const ulonglong2* __restrict__ Dg) {
   constexpr int CH = kChunkF32;
+  // The segment-table flavour (SEG: sc_eval_segments, the two-pass three-channel path) keeps the plain staging loop into
+  // static shared memory: with the dynamic array its register allocation spills 60 B more and it runs 10 % slower.
   extern __shared__ __align__(128) unsigned char smem_d2[];
-  ulonglong2* sD = reinterpret_cast<ulonglong2*>(smem_d2);     // 48 KB
-  const uint32_t bar = stg::smem_u32(smem_d2 + kDense2DataBytes);
-  if (threadIdx.x == 0) {
-    stg::mbar_init(bar, 1);
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  ulonglong2* sD;                                                // 48 KB
+  uint32_t bar = 0;
+  if constexpr (SEG) {
+    __shared__ ulonglong2 sD_static[CH / 2 * kPairRec];
+    sD = sD_static;
+  } else {
+    sD = reinterpret_cast<ulonglong2*>(smem_d2);
+    bar = stg::smem_u32(smem_d2 + kDense2DataBytes);
+    if (threadIdx.x == 0) {
+      stg::mbar_init(bar, 1);
+      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
   }
 
   const int chunk_l = blockIdx.x;
@@ -483,8 +492,13 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2(DevCfg c, Den
     return;
   }
 
-  // (the __syncthreads_or above orders the barrier's initialisation before every wait)
-  if (threadIdx.x == 0) {
+  if constexpr (SEG) {
+    const ulonglong2* src = Dg + (size_t)(cs >> 1) * kPairRec;
+#pragma unroll 4
+    for (int t = threadIdx.x; t < CH / 2 * kPairRec; t += kBlock) sD[t] = src[t];
+    __syncthreads();
+  } else if (threadIdx.x == 0) {
+    // (the __syncthreads_or above orders the barrier's initialisation before every wait)
     stg::mbar_expect_tx(bar, kDense2DataBytes);
     stg::bulk_g2s(stg::smem_u32(sD), Dg + (size_t)(cs >> 1) * kPairRec, kDense2DataBytes, bar);
   }
@@ -529,7 +543,7 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2(DevCfg c, Den
   PhaseFD fd = {};
   float cc[MERGE ? 4 : 1][4];  // merged coarse interval: cubic of the amplitudes in t = (j - coarse start)/stride
   int merged_left = 0;         // fine sub-intervals of the current merged coarse interval still to walk
-  bool landed = false;         // the chunk's data records: waited for after the first sub-interval's set-up (node reads only)
+  bool landed = SEG;           // the bulk copy is waited for after the first sub-interval's set-up (node reads only)
   for (int ib = cs; ib < ce2; ib += Sf) {
     const int ie = min(ib + Sf, ce2);
     const bool lane_in = (ib >= jlo) && (ie <= jhi);

@@ -119,9 +119,7 @@ __device__ __forceinline__ void pairs_fast3(PhaseFD& ph, const float (&cf)[6][4]
 }
 
 // QUAD flavour for six amplitude parts (see pairs_fast_q in sc_kernels_dense32.cuh): quadratic amplitudes over runs of a
-// quarter sub-interval, 12 packed FMAs per bin pair instead of 18.  Used by k_dense2_ad<.., 6> (no spills there); in
-// k_dense3 the 24 cubic + 18 quadratic coefficients spill and the kernel gets slower (26.9 -> 30.3 ms on c3), so it keeps
-// the cubics.
+// quarter sub-interval, 12 packed FMAs per bin pair instead of 18.  Used by k_dense2_ad<.., 6> and by k_dense3<.., QUAD>.
 struct QuadState3 { float q[6][3]; u64 u2; int left; int r; };
 __device__ __forceinline__ void quad_run3(const float (&cf)[6][4], int r, QuadState3& o) {
   const float s0 = 0.25f * (float)r;
@@ -184,8 +182,12 @@ __device__ __forceinline__ void pairs_fast3_q(PhaseFD& ph, const float (&cf)[6][
 #ifndef SC_DENSE3_MINB
 #define SC_DENSE3_MINB 4     /* CTAs per SM: 128 registers/thread with ~150 B of spills beats 168 registers at 3 CTAs (28.6 vs 32.0 ms on c3) */
 #endif
-template <bool SEG, int SC>
-__global__ void __launch_bounds__(kBlock, SC_DENSE3_MINB) k_dense3(DevCfg c, DenseArgs a, const ulonglong2* __restrict__ Dg,
+#ifndef SC_DENSE3_QUAD_MINB
+#define SC_DENSE3_QUAD_MINB 3   /* QUAD flavour: 24 cubic + 18 quadratic coefficients live -- 168 registers at 3 CTAs per SM 25.6 ms on c3,
+                                   128 registers at 4 CTAs (232 B of spills) 29.7 ms, 255 registers at 2 CTAs 26.5 ms; cubic flavour 26.9 ms */
+#endif
+template <bool SEG, int SC, bool QUAD = false>
+__global__ void __launch_bounds__(kBlock, QUAD ? SC_DENSE3_QUAD_MINB : SC_DENSE3_MINB) k_dense3(DevCfg c, DenseArgs a, const ulonglong2* __restrict__ Dg,
                                                                    const ulonglong2* __restrict__ Gp) {
   constexpr int CH = kChunkF32;
   __shared__ ulonglong2 sD[CH / 2 * kPairRec3];                // 48 KB
@@ -268,6 +270,7 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE3_MINB) k_dense3(DevCfg c, Den
     int piece = use_mom ? a.piece_first[(ib >> (c.log2_stride - 2)) - ((a.chunk_first * CH) >> (c.log2_stride - 2))] : 0;
     float car_zr = 0.f, car_zi = 0.f, car_sg = 0.f;
     bool carry = false;
+    QuadState3 qs;
     int pl = ib;
     while (pl < ie) {
       const int ph = min(next_edge, ie);                       // next_edge > pl: edges <= pl are consumed
@@ -286,11 +289,16 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE3_MINB) k_dense3(DevCfg c, Den
         }
         s2 = f2pack((float)(jj - ib) * hS, (float)(jj + 1 - ib) * hS);
         rec = sD + ((jj - cs) >> 1) * kPairRec3;
+        if constexpr (QUAD) { if (use_mom && jj < ph) quad_start3(cf, jj - ib, c.log2_stride - 4, qs); }
         while (jj < ph) {
           const bool split = (jj == jfull);                    // the pair (ph - 1, ph)
-          const int e2 = split ? jj + 2 : min(jj + kFlushBins, jfull);
+          const int e2 = split ? jj + 2 : min(jj + ((QUAD && use_mom) ? SC_QUAD_FLUSH : kFlushBins), jfull);
           u64 zr2 = 0, zi2 = 0, sg2 = 0;
-          if (use_mom) { pairs_fast3<SC>(fd, cf, s2, rec, (e2 - jj) >> 1, h2, K2, zr2, zi2); jj = e2; }
+          if (use_mom) {
+            if constexpr (QUAD) pairs_fast3_q<SC>(fd, cf, qs, c.log2_stride - 4, rec, (e2 - jj) >> 1, K2, zr2, zi2);
+            else pairs_fast3<SC>(fd, cf, s2, rec, (e2 - jj) >> 1, h2, K2, zr2, zi2);
+            jj = e2;
+          }
           else {
             for (; jj < e2; jj += 2) pair_eval3<SC>(fd, cf, s2, rec, Gp + (size_t)(jj >> 1) * 2, jj, jlo, jhi, h2, K2, zr2, zi2, sg2);
           }

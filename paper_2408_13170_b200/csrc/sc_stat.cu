@@ -403,7 +403,7 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
           h->last_lg = dc.log2_stride;
           const bool quad_on = quad && sincos == 2 && !seg_mode;
           h->last_flavour = (sincos == 2 ? SC_FLAVOUR_MUFU : 0) |
-                            (fused3 ? SC_FLAVOUR_AET : use_tc ? SC_FLAVOUR_TC :   // (k_dense3 with quadratic runs: 26.9 -> 30.3 ms on c3, spills; not built)
+                            (fused3 ? (SC_FLAVOUR_AET | (quad_on ? SC_FLAVOUR_QUAD : 0)) : use_tc ? SC_FLAVOUR_TC :
                              ((merge ? SC_FLAVOUR_MERGE : 0) | ((quad_on && merge) ? SC_FLAVOUR_QUAD : 0)));
         }
         if (fused3) {
@@ -411,6 +411,7 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
           const ulonglong2* Gp = reinterpret_cast<const ulonglong2*>(h->Gp3);
           if (seg_mode && sincos == 2) k_dense3<true, 2><<<grid, kBlock, 0, st>>>(dc, a, D3p, Gp);
           else if (seg_mode) k_dense3<true, 0><<<grid, kBlock, 0, st>>>(dc, a, D3p, Gp);
+          else if (sincos == 2 && quad) k_dense3<false, 2, true><<<grid, kBlock, 0, st>>>(dc, a, D3p, Gp);
           else if (sincos == 2) k_dense3<false, 2><<<grid, kBlock, 0, st>>>(dc, a, D3p, Gp);
           else k_dense3<false, 0><<<grid, kBlock, 0, st>>>(dc, a, D3p, Gp);
         }
@@ -422,10 +423,10 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
           else if (merge) k_dense2_tc<false, 0, true><<<grid_tc, tc::kThreads, tc::kSmemBytes, st>>>(dc, a, Dp, Tg);
           else k_dense2_tc<false, 0><<<grid_tc, tc::kThreads, tc::kSmemBytes, st>>>(dc, a, Dp, Tg);
         }
-        else if (seg_mode && sincos == 2 && merge) k_dense2<true, 2, true><<<grid, kBlock, kDense2Smem, st>>>(dc, a, Dp);
-        else if (seg_mode && sincos == 2) k_dense2<true, 2><<<grid, kBlock, kDense2Smem, st>>>(dc, a, Dp);
-        else if (seg_mode && merge) k_dense2<true, 0, true><<<grid, kBlock, kDense2Smem, st>>>(dc, a, Dp);
-        else if (seg_mode) k_dense2<true, 0><<<grid, kBlock, kDense2Smem, st>>>(dc, a, Dp);
+        else if (seg_mode && sincos == 2 && merge) k_dense2<true, 2, true><<<grid, kBlock, 0, st>>>(dc, a, Dp);
+        else if (seg_mode && sincos == 2) k_dense2<true, 2><<<grid, kBlock, 0, st>>>(dc, a, Dp);
+        else if (seg_mode && merge) k_dense2<true, 0, true><<<grid, kBlock, 0, st>>>(dc, a, Dp);
+        else if (seg_mode) k_dense2<true, 0><<<grid, kBlock, 0, st>>>(dc, a, Dp);
         else if (sincos == 2 && merge && quad) k_dense2<false, 2, true, true><<<grid, kBlock, kDense2Smem, st>>>(dc, a, Dp);
         else if (sincos == 2 && merge) k_dense2<false, 2, true><<<grid, kBlock, kDense2Smem, st>>>(dc, a, Dp);
         else if (sincos == 2) k_dense2<false, 2><<<grid, kBlock, kDense2Smem, st>>>(dc, a, Dp);
@@ -928,10 +929,6 @@ int init_common(sc_handle** out, const sc_config* cfg, const double* dA, const d
   SC_INIT(cudaFuncSetAttribute(k_dense2<false, 2, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kDense2Smem));
   SC_INIT(cudaFuncSetAttribute(k_dense2<false, 2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kDense2Smem));
   SC_INIT(cudaFuncSetAttribute(k_dense2<false, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kDense2Smem));
-  SC_INIT(cudaFuncSetAttribute(k_dense2<true, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kDense2Smem));
-  SC_INIT(cudaFuncSetAttribute(k_dense2<true, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, kDense2Smem));
-  SC_INIT(cudaFuncSetAttribute(k_dense2<true, 2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kDense2Smem));
-  SC_INIT(cudaFuncSetAttribute(k_dense2<true, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kDense2Smem));
   SC_INIT(cudaFuncSetAttribute(k_dense2_tc<true, 0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::kSmemBytes));
   SC_INIT(cudaFuncSetAttribute(k_dense2_tc<false, 2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::kSmemBytes));
   SC_INIT(cudaFuncSetAttribute(k_dense2_tc<false, 2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::kSmemBytes));
