@@ -82,3 +82,55 @@ def test_random_grids_tiles_and_edges(oracle, seed):
                 assert np.all(err <= TOL), (seed, hint, len(e), float(err.max()), float(r[ok][np.argmax(err)]))
     assert n_live > 0
     H.close()
+
+
+@pytest.mark.parametrize("seed", range(5))
+def test_wide_grids_with_node_spacing_hint_and_quadratic_runs(oracle, seed):
+    """Multi-year grids (3.5e5 - 1.1e6 bins) where the window-fraction statement widens the node spacing (stride 512 - 2048) and
+    the long segments switch the pair loop to its quadratic-amplitude runs (SC_FLAVOUR_QUAD): random tiles, random numbers of
+    equal segments from 8 to n_bins/130 and one irregular edge list; a seeded sample of particles against the oracle's truth
+    mode, flat 1e-6 bar."""
+    import torch
+    import paper_2408_13170_b200 as sc
+    rng = np.random.default_rng(500 + seed)
+    T_yr = float(rng.choice([2.0, 3.0, 4.0]))
+    f_lo, width = float(rng.uniform(0.014, 0.022)), float(rng.uniform(0.004, 0.012))
+    cfg = sy.grid_config(T_yr, f_lo, f_lo + width)
+    S = sy.psd_AE(sy.freqs(cfg))
+    df = 1.0 / cfg["T_obs_s"]
+    Mc, q = float(rng.uniform(20.0, 40.0)), float(rng.uniform(0.5, 1.0))
+    tau = 5.0 / 256.0 * (Mc * sy.MSUN_S) ** (-5.0 / 3.0) * (np.pi * f_lo) ** (-8.0 / 3.0)     # Newtonian time to coalescence from f_lo
+    th = sy.draw_injection(rng, Mc, q, tau)
+    lo, hi = sy.prior_box(th[0], th[2], eta_lo=0.16, dMc=float(rng.uniform(0.3, 1.5)), dtc=float(rng.uniform(0.05, 0.4)) * T_yr * sy.YEAR_S)
+    P = 384
+    parts = sy.draw_particles(int(rng.integers(1 << 30)), P, lo, hi)
+    inp = dict(cfg=cfg, S_A=S, S_E=S.copy(), df=df, lo=lo, hi=hi, particles=parts,
+               noise_A=sy.draw_noise(int(rng.integers(1 << 30)), S, df), noise_E=sy.draw_noise(int(rng.integers(1 << 30)), S, df),
+               injections=[dict(theta=th, rho=float(rng.uniform(10.0, 30.0)))])
+    if oracle.template(oracle.make_config(cfg), th)[2] == 0:
+        inp["injections"] = []
+    nb = cfg["n_bins"]
+    lists = [sy.edges(nb, int(np.exp(rng.uniform(np.log(8), np.log(nb / 130))))) for _ in range(3)]
+    n_e = int(rng.integers(20, 3000))
+    a, b = sorted(rng.integers(0, nb + 1, size=2))
+    if b - a > 200 * n_e:
+        lists.append(np.sort(rng.integers(a, b + 1, size=n_e)).astype(np.int64))      # irregular, long on average, short pieces among them
+    _, dA, dE = make_data(oracle, inp)
+    H = gpu_handle(inp, dA, dE)
+    H.set_option(sc.SC_OPT_TC_MAX_S, int(np.ceil(hi[2])))
+    par = torch.from_numpy(parts).to("cuda:0")
+    H.eval_stat(par, sy.edges(nb, 1).astype(np.int32))
+    H.set_option(sc.SC_OPT_WINDOW_FRACTION_PPM, max(1, int(round(1e6 * H.counters()[0] / (P * nb)))))
+    idx = np.sort(rng.choice(P, 12, replace=False))
+    ref = oracle.eval_stat_levels(oracle.make_config(cfg, truth=True), dA, dE, S, S, parts[idx], lists)
+    quad_seen = 0
+    for e, r in zip(lists, ref):
+        got = H.eval_stat(par, e.astype(np.int32)).cpu().numpy()[idx]
+        quad_seen += bool(H.launch_info()[1] & sc.SC_FLAVOUR_QUAD)
+        assert np.array_equal(got == 0.0, r == 0.0), (seed, len(e))
+        ok = r > 0
+        if ok.any():
+            err = rel_err(got[ok], r[ok])
+            assert np.all(err <= TOL), (seed, len(e), H.launch_info(), float(err.max()), float(r[ok][np.argmax(err)]))
+    H.close()
+    assert quad_seen >= 1
