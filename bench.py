@@ -603,7 +603,8 @@ def run_ours(args, rank, local_rank, world):
                 "traffic": dram_traffic_from_profile() if is_c3_shared else None,
                 "traffic_source": ("static: profiles/r02_k_dense2_full.md (ncu --set full of one k_dense2 launch of this c3 command), "
                                    "not measured in this run") if is_c3_shared else None,
-                "kernel": "k_dense2_ad<2,MERGE>" if ad_N else ("k_dense2<false,2,MERGE,QUAD>" if quad else "k_dense2<false,2,MERGE>"),
+                "kernel": "k_dense2_ad<2,MERGE>" if ad_N else ("k_dense2<false," + ("2" if flavour & sc.SC_FLAVOUR_MUFU else "0")
+                                                                + (",MERGE" if flavour & sc.SC_FLAVOUR_MERGE else "") + (",QUAD" if quad else "") + ">"),
                 "kernel_ms_per_launch": dense_avg, "node_stride_log2": lg_nodes, "flavour_bits": flavour,
                 "peak_source": "FP32 pipe: 148 SM x 128 lanes x 1.965 GHz x 2 flop (unit counts and clocks of B200_PROFILING.md; "
                                "MEASURED_PEAKS.json has no FP32 figure)",
