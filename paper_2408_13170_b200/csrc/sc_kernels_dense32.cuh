@@ -586,6 +586,7 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2(DevCfg c, Den
     float car_zr = 0.f, car_zi = 0.f, car_sg = 0.f;
     bool carry = false;
     QuadState qs;
+    int q_pos = -1;            // the bin qs stands at (-1: nowhere; a new sub-interval has new coefficients)
     int pl = ib;
     while (pl < ie) {
       const int ph = min(next_edge, ie);                       // next_edge > pl: edges <= pl are consumed
@@ -604,13 +605,14 @@ __global__ void __launch_bounds__(kBlock, SC_DENSE2_MINB) k_dense2(DevCfg c, Den
         }
         s2 = f2pack((float)(jj - ib) * hS, (float)(jj + 1 - ib) * hS);
         rec = sD + ((jj - cs) >> 1) * kPairRec;
-        if constexpr (QUAD) { if (use_mom && jj < ph) quad_start(cf, jj - ib, c.log2_stride - 4, qs); }
+        // (a piece that begins where the previous one's pairs ended finds the run state in place)
+        if constexpr (QUAD) { if (use_mom && jj < ph && q_pos != jj) quad_start(cf, jj - ib, c.log2_stride - 4, qs); }
         while (jj < ph) {
           const bool split = (jj == jfull);                    // the pair (ph - 1, ph)
           const int e2 = split ? jj + 2 : min(jj + ((QUAD && use_mom) ? SC_QUAD_FLUSH : kFlushBins), jfull);
           u64 zr2 = 0, zi2 = 0, sg2 = 0;
           if (use_mom) {
-            if constexpr (QUAD) pairs_fast_q<SC>(fd, cf, qs, c.log2_stride - 4, rec, (e2 - jj) >> 1, K2, zr2, zi2);
+            if constexpr (QUAD) { pairs_fast_q<SC>(fd, cf, qs, c.log2_stride - 4, rec, (e2 - jj) >> 1, K2, zr2, zi2); q_pos = e2; }
             else pairs_fast<SC>(fd, cf, s2, rec, (e2 - jj) >> 1, h2, K2, zr2, zi2);
             jj = e2;
           }
