@@ -271,6 +271,7 @@ __global__ void __launch_bounds__(kBlock, QUAD ? SC_DENSE3_QUAD_MINB : SC_DENSE3
     float car_zr = 0.f, car_zi = 0.f, car_sg = 0.f;
     bool carry = false;
     QuadState3 qs;
+    int q_pos = -1;            // the bin qs stands at (see k_dense2)
     int pl = ib;
     while (pl < ie) {
       const int ph = min(next_edge, ie);                       // next_edge > pl: edges <= pl are consumed
@@ -289,13 +290,13 @@ __global__ void __launch_bounds__(kBlock, QUAD ? SC_DENSE3_QUAD_MINB : SC_DENSE3
         }
         s2 = f2pack((float)(jj - ib) * hS, (float)(jj + 1 - ib) * hS);
         rec = sD + ((jj - cs) >> 1) * kPairRec3;
-        if constexpr (QUAD) { if (use_mom && jj < ph) quad_start3(cf, jj - ib, c.log2_stride - 4, qs); }
+        if constexpr (QUAD) { if (use_mom && jj < ph && q_pos != jj) quad_start3(cf, jj - ib, c.log2_stride - 4, qs); }
         while (jj < ph) {
           const bool split = (jj == jfull);                    // the pair (ph - 1, ph)
           const int e2 = split ? jj + 2 : min(jj + ((QUAD && use_mom) ? SC_QUAD_FLUSH : kFlushBins), jfull);
           u64 zr2 = 0, zi2 = 0, sg2 = 0;
           if (use_mom) {
-            if constexpr (QUAD) pairs_fast3_q<SC>(fd, cf, qs, c.log2_stride - 4, rec, (e2 - jj) >> 1, K2, zr2, zi2);
+            if constexpr (QUAD) { pairs_fast3_q<SC>(fd, cf, qs, c.log2_stride - 4, rec, (e2 - jj) >> 1, K2, zr2, zi2); q_pos = e2; }
             else pairs_fast3<SC>(fd, cf, s2, rec, (e2 - jj) >> 1, h2, K2, zr2, zi2);
             jj = e2;
           }
