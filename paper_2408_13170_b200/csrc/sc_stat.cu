@@ -286,7 +286,8 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
   const int n_chunks = h->n_chunks;
   // per-particle scratch bytes
   const size_t per_p = 2 * ((size_t)kPcFields * 8 + 8) /* constants, jlo, jhi: unsorted + sorted */ + 16 /* sort keys, map */
-                       + (size_t)n_nodes * (4 + 8 + NA * sizeof(R)) + (size_t)std::max(n_chunks, 1) * kFragFields * 8;
+                       + (size_t)n_nodes * (4 + 8 + NA * sizeof(R)) + (size_t)std::max(n_chunks, 1) * kFragFields * 8
+                       + (size_t)kStitchParts * kStitchRec * 8;
   int64_t Pb_max = (int64_t)(h->scratch_cap / per_p) / kBlock * kBlock;
   if (Pb_max < kBlock) Pb_max = kBlock;
   const int64_t P_round = (P + kBlock - 1) / kBlock * kBlock;
@@ -303,6 +304,7 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
   double* node_frac = (double*)take((size_t)n_nodes * 8 * P_pad);
   R* node_amp = (R*)take((size_t)n_nodes * NA * sizeof(R) * P_pad);
   double* frag = (double*)take((size_t)std::max(n_chunks, 1) * kFragFields * 8 * P_pad);
+  double* stitch_rec = (double*)take((size_t)kStitchParts * kStitchRec * 8 * P_pad);
   // window sort (see k_gather_sorted): not in the segment-table mode (rows are addressed by particle).  In the escalation
   // pass the count sits on the device: all P_pad slots are sorted, the unused ones to the end -- only below 4096 segments
   // (a rule of the call, not of the data: with that many segments hardly any particle is selected and the sort's seven
@@ -446,6 +448,17 @@ int run_batches(sc_handle* h, const double* params, int64_t P, double* out, doub
       // the hardware sin/cos gain g (g^2 = mufu_gain2) multiplies every |z_k|: Upsilon by g^2, O_hat by g, <h|h> not at all.
       // Units (whitened -> definition): Upsilon is scale free, x_k = 4 df |z_k| = |Z_k| s0 h0, [h|h]_k = Sg_k s0^2 h0^2.
       const double g2 = (sizeof(R) == 4 && sincos == 2) ? h->mufu_gain2 : 1.0;
+      // many chunks: a particle's range folded in kStitchParts parts by as many threads, then joined (k_stitch_parts)
+      if (!esc_count && n_chunks >= 64) {
+        const int n_slots = sorted ? P_pad : Pn;
+        k_stitch_parts<<<dim3((n_slots + 127) / 128, kStitchParts), 128, 0, st>>>(frag, h->d_flags, n_chunks, P_pad, n_slots, out_comp ? 1 : 0,
+                                                                                 jlo, jhi, h->chunk_first, h->cached_chunk, stitch_rec);
+        if ((rc = check_launch(h, "k_stitch_parts"))) return rc;
+        k_stitch_join<<<(n_slots + 127) / 128, 128, 0, st>>>(stitch_rec, n_chunks, P_pad, Pn, 1.0 / g2, out ? out + pb : nullptr,
+                                                            out_comp ? out_comp + pb * 3 : nullptr, h->s0 * h0 / sqrt(g2),
+                                                            h->s0 * h->s0 * h0 * h0, sorted ? pmap : nullptr, jlo, jhi, h->chunk_first,
+                                                            h->cached_chunk, h->d_next_close);
+      } else
       k_stitch<<<esc_count ? pblocks : ((sorted ? P_pad : Pn) + 127) / 128, 128, 0, st>>>(frag, h->d_flags, n_chunks, P_pad, Pn, 1.0 / g2, out ? out + pb : nullptr,
                                                  out_comp ? out_comp + pb * 3 : nullptr, h->s0 * h0 / sqrt(g2),
                                                  h->s0 * h->s0 * h0 * h0, esc_count, (int)pb, sorted ? pmap : nullptr,
