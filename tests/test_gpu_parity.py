@@ -730,3 +730,26 @@ def test_node_spacing_error_model(oracle, torch_cuda, sc):
             assert worst[(lg, N)] <= 2.0 * K * days ** 6 / np.sqrt(n_eff) + 2e-9, (lg, N, days, n_eff, worst[(lg, N)])
         H.close()
     assert worst[(9, 1)] > 50 * worst[(7, 1)]             # ~ days^6: the model is not vacuous
+
+
+@pytest.mark.parametrize("N,prec", [(1, 0), (100, 0), (2000, 0), (2000, 2)])
+def test_c2_components_many_chunks(oracle, torch_cuda, sc, N, prec):
+    """Eq. 8 / Eq. 3 on c2 (123 chunks of 2048 bins, 247 of 1024: the chunk walk of a particle is folded in parts by k_stitch_parts /
+    k_stitch_join, with the partial sums of |z_k| and sigma_k) against the oracle's segments, 24 particles."""
+    inp = sy.config_inputs(2, P=24)
+    cfg, dA, dE = make_data(oracle, inp)
+    H = gpu_handle(inp, dA, dE)
+    H.set_option(sc.SC_OPT_TC_MAX_S, int(np.ceil(inp["hi"][2])))
+    H.set_option(sc.SC_OPT_PRECISION, prec)
+    e = sy.edges(inp["cfg"]["n_bins"], N)
+    ref, refseg = oracle.eval_stat(oracle.make_config(inp["cfg"], truth=True), dA, dE, inp["S_A"], inp["S_E"], inp["particles"], e, want_seg=True)
+    comp_ref = np.array([oracle.components_from_seg(s, inp["df"]) for s in refseg])
+    par = _dev(torch_cuda, inp["particles"])
+    comp = H.eval_components(par, e).cpu().numpy()
+    live = ref > 0
+    assert live.sum() >= 12 and np.array_equal(comp[:, 0] == 0, ~live)
+    assert rel_err(comp[live, 0], ref[live]).max() <= TOL
+    assert np.array_equal(comp[:, 0], H.eval_stat(par, e).cpu().numpy())      # same kernels, same order
+    assert rel_err(comp[live, 1], comp_ref[live, 1]).max() <= TOL
+    assert rel_err(comp[live, 2], comp_ref[live, 2]).max() <= TOL
+    H.close()
