@@ -132,7 +132,7 @@ __device__ __forceinline__ double sigma_sub64(const DevCfg& c, const AdaptArgs& 
 }
 
 template <int NA = 4>
-__global__ void __launch_bounds__(kBlock) k_sigma_chunks64(DevCfg c, DenseArgs a, AdaptArgs ad) {
+__global__ void __launch_bounds__(kBlock, NA == 6 ? 3 : 4) k_sigma_chunks64(DevCfg c, DenseArgs a, AdaptArgs ad) {
   constexpr int CH = kChunkF32;
   const int chunk = blockIdx.x;
   const int cs = chunk * CH;
