@@ -171,8 +171,12 @@ __global__ void k_particle_consts(DevCfg c, const double* __restrict__ params, i
 // One thread per (node, particle), particle fastest -> coalesced [node][particle] tables; a CTA takes 128 particles and
 // a group of kNodesPerCta consecutive nodes (one CTA per node is launch-bound when most of the table is out of reach).
 constexpr int kNodesPerCta = 16;
+#ifndef SC_NODES_MINB
+#define SC_NODES_MINB 4   /* CTAs per SM: 128 registers instead of 143 at 3 (same 40 B of spills) -- the kernel is FP64-latency bound;
+                             c3 0.63 -> 0.57 ms, c5 1.36 -> 1.18 ms; 5 CTAs / 96 registers the same */
+#endif
 template <typename R, bool ESC = false, int NA = 4 /* amplitude fields per node: 4 = (A, E) or (T, 0); 6 = (A, E, T) */>
-__global__ void k_nodes(DevCfg c, const double* __restrict__ pc, const int* __restrict__ jlo, const int* __restrict__ jhi,
+__global__ void __launch_bounds__(128, SC_NODES_MINB) k_nodes(DevCfg c, const double* __restrict__ pc, const int* __restrict__ jlo, const int* __restrict__ jhi,
                         int P_pad, int* __restrict__ node_n, double* __restrict__ node_frac,
                         R* __restrict__ node_amp /* [node][NA][P_pad] */, const int* __restrict__ esc_count = nullptr,
                         int esc_pb = 0, int skip_unreached = 0) {
